@@ -1,0 +1,295 @@
+/*
+ * brmppi_oracle.c -- CPU oracle (fp64, single pass, no blocking / fusion / reordering).
+ * TEST INFRASTRUCTURE ONLY; see brmppi_oracle.h for the passages followed and the pin status.
+ *
+ * Build:  gcc -O2 -std=c11 -fPIC -shared -o liboracle.so brmppi_oracle.c -lm -lpthread
+ *         (-ffp-contract=off so that the result does not depend on FMA availability)
+ */
+#include "brmppi_oracle.h"
+
+#include <math.h>
+#include <pthread.h>
+#include <stdlib.h>
+#include <string.h>
+
+#ifndef M_PI
+#define M_PI 3.14159265358979323846
+#endif
+
+/* ------------------------------------------------------------------------------------------
+ * Philox4x32-10.  J. K. Salmon, M. A. Moraes, R. O. Dror, D. E. Shaw, "Parallel random
+ * numbers: as easy as 1, 2, 3", SC'11.  One round:
+ *   (hi0, lo0) = M0 * c0;  (hi1, lo1) = M1 * c2;
+ *   (c0, c1, c2, c3) <- (hi1 ^ c1 ^ k0,  lo1,  hi0 ^ c3 ^ k1,  lo0)
+ * and the key is bumped by (W0, W1) between rounds (not after the last).
+ * ---------------------------------------------------------------------------------------- */
+void orc_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]) {
+  const uint32_t M0 = 0xD2511F53u, M1 = 0xCD9E8D57u;
+  const uint32_t W0 = 0x9E3779B9u, W1 = 0xBB67AE85u;
+  uint32_t c0 = ctr[0], c1 = ctr[1], c2 = ctr[2], c3 = ctr[3];
+  uint32_t k0 = key[0], k1 = key[1];
+  for (int round = 0; round < 10; ++round) {
+    uint64_t p0 = (uint64_t)M0 * (uint64_t)c0;
+    uint64_t p1 = (uint64_t)M1 * (uint64_t)c2;
+    uint32_t hi0 = (uint32_t)(p0 >> 32), lo0 = (uint32_t)p0;
+    uint32_t hi1 = (uint32_t)(p1 >> 32), lo1 = (uint32_t)p1;
+    uint32_t n0 = hi1 ^ c1 ^ k0;
+    uint32_t n1 = lo1;
+    uint32_t n2 = hi0 ^ c3 ^ k1;
+    uint32_t n3 = lo0;
+    c0 = n0; c1 = n1; c2 = n2; c3 = n3;
+    k0 += W0; k1 += W1;
+  }
+  out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+double orc_uniform(uint32_t w) { return (double)(w >> 9) * (1.0 / 8388608.0); }
+
+static void seed_key(uint64_t seed, uint32_t key[2]) {
+  key[0] = (uint32_t)(seed & 0xFFFFFFFFu);
+  key[1] = (uint32_t)(seed >> 32);
+}
+
+/* PAPER.md:89 "draws S independent noise rollouts w ~ N(0, Sigma_w)"; reading 5: Box-Muller on
+ * two 23-bit uniforms of the Philox block with counter (t, n, k, 0). */
+void orc_normals(uint64_t seed, uint32_t n, uint32_t k, uint32_t t, double z[2]) {
+  uint32_t key[2], ctr[4] = {t, n, k, 0u}, w[4];
+  seed_key(seed, key);
+  orc_philox4x32_10(ctr, key, w);
+  double u1 = 1.0 - orc_uniform(w[0]); /* in (0, 1] */
+  double u2 = orc_uniform(w[1]);       /* in [0, 1) */
+  double r = sqrt(-2.0 * log(u1));
+  z[0] = r * cos(2.0 * M_PI * u2);
+  z[1] = r * sin(2.0 * M_PI * u2);
+}
+
+/* Reading 8: one alpha per sample, U[alpha_lo, alpha_hi), Philox counter (0, n, k, 1). */
+double orc_alpha(const orc_params* p, uint32_t n, uint32_t k) {
+  uint32_t key[2], ctr[4] = {0u, n, k, 1u}, w[4];
+  seed_key(p->seed, key);
+  orc_philox4x32_10(ctr, key, w);
+  return p->alpha_lo + (p->alpha_hi - p->alpha_lo) * orc_uniform(w[0]);
+}
+
+double orc_wrap(double a) { return a - 2.0 * M_PI * rint(a / (2.0 * M_PI)); }
+
+static double clampd(double x, double lo, double hi) { return x < lo ? lo : (x > hi ? hi : x); }
+
+/* Reduced eq. (6): explicit Euler, every right-hand side at step k. */
+void orc_kinematic_step(const orc_params* p, const double x[4], double v, double delta,
+                        double xn[4]) {
+  double px = x[0], py = x[1], psi1 = x[2], psi2 = x[3];
+  double td = tan(delta);
+  double beta = psi1 - psi2;
+  xn[0] = px + p->dt * v * cos(psi1);
+  xn[1] = py + p->dt * v * sin(psi1);
+  xn[2] = psi1 + p->dt * (v / p->L1) * td;
+  xn[3] = psi2 + p->dt * (v / p->L2) * (sin(beta) - (p->Lh / p->L1) * cos(beta) * td);
+}
+
+/* Hitch point p_h = (x - Lh cos psi1, y - Lh sin psi1); disc centre = p_h + offset * body axis
+ * ("cover the vehicle body with discs of radius r"; reading 11). */
+void orc_disc_centre(const orc_params* p, const double x[4], int j, double c[2]) {
+  double hx = x[0] - p->Lh * cos(x[2]);
+  double hy = x[1] - p->Lh * sin(x[2]);
+  double psi = (p->disc_body[j] == 0) ? x[2] : x[3];
+  c[0] = hx + p->disc_offset[j] * cos(psi);
+  c[1] = hy + p->disc_offset[j] * sin(psi);
+}
+
+/* Eq. (16) with e = 2, m_x = m_y = R, inflated by the vehicle disc radius. */
+double orc_barrier(const orc_params* p, const double c[2], const double o[2], double R) {
+  double rho = R + p->disc_radius;
+  double dx = c[0] - o[0], dy = c[1] - o[1];
+  return (dx * dx + dy * dy) / (rho * rho) - 1.0;
+}
+
+double orc_goal_cost(const orc_params* p, const double x[4], const double g[4]) {
+  double ex = x[0] - g[0], ey = x[1] - g[1];
+  double e1 = orc_wrap(x[2] - g[2]), e2 = orc_wrap(x[3] - g[3]);
+  return p->w_pos * (ex * ex + ey * ey) + p->w_head * (e1 * e1 + e2 * e2);
+}
+
+/* Obstacle i at rollout step t: constant-velocity prediction (Assumption 2). */
+static void obstacle_at(const orc_params* p, const double* obstacles, int i, int t, double o[2]) {
+  const double* ob = obstacles + 5 * i;
+  o[0] = ob[0] + (double)t * p->dt * ob[3];
+  o[1] = ob[1] + (double)t * p->dt * ob[4];
+}
+
+double orc_rollout(const orc_params* p, const double x0[4], const double goal[4], int n_obs,
+                   const double* obstacles, const double* u, double alpha, double xT[4],
+                   double* traj, double* pen_out) {
+  const int T = p->T, D = p->n_discs;
+  double X[4] = {x0[0], x0[1], x0[2], x0[3]};
+  double S = 0.0, pen_total = 0.0;
+  double* hprev = (double*)malloc(sizeof(double) * (size_t)(n_obs > 0 ? n_obs : 1) * ORC_MAX_DISCS);
+
+  /* h at (x_0, o(0)) */
+  for (int i = 0; i < n_obs; ++i) {
+    double o[2];
+    obstacle_at(p, obstacles, i, 0, o);
+    for (int j = 0; j < D; ++j) {
+      double c[2];
+      orc_disc_centre(p, X, j, c);
+      hprev[i * ORC_MAX_DISCS + j] = orc_barrier(p, c, o, obstacles[5 * i + 2]);
+    }
+  }
+  if (traj) memcpy(traj, X, sizeof(X));
+
+  for (int t = 0; t < T; ++t) {
+    double v = u[2 * t + 0], d = u[2 * t + 1];
+    double Xn[4];
+    orc_kinematic_step(p, X, v, d, Xn);
+
+    /* barrier-rate condition h_{t+1} - h_t >= -alpha h_t (reading 1) as a
+     * linear hinge penalty summed over obstacles and discs (reading 14);
+     * h_{t+1} pairs x_{t+1} with o(t+1) (reading 13). */
+    double pen = 0.0;
+    for (int i = 0; i < n_obs; ++i) {
+      double o[2];
+      obstacle_at(p, obstacles, i, t + 1, o);
+      for (int j = 0; j < D; ++j) {
+        double c[2];
+        orc_disc_centre(p, Xn, j, c);
+        double hn = orc_barrier(p, c, o, obstacles[5 * i + 2]);
+        double viol = (1.0 - alpha) * hprev[i * ORC_MAX_DISCS + j] - hn;
+        if (viol > 0.0) pen += viol;
+        hprev[i * ORC_MAX_DISCS + j] = hn;
+      }
+    }
+    pen_total += pen;
+
+    /* stage cost on (x_{t+1}, u_t) (reading 3); hitch: squared hinge at hitch_max (reading 15) */
+    double hitch = fabs(orc_wrap(Xn[2] - Xn[3])) - p->hitch_max;
+    if (hitch < 0.0) hitch = 0.0;
+    S += orc_goal_cost(p, Xn, goal) + p->w_v * v * v + p->w_delta * d * d +
+         p->w_hitch * hitch * hitch + p->w_bar * pen;
+
+    memcpy(X, Xn, sizeof(X));
+    if (traj) memcpy(traj + 4 * (t + 1), X, sizeof(X));
+  }
+  S += p->w_term * orc_goal_cost(p, X, goal); /* terminal cost r_N(x_N), eq. (7) */
+  memcpy(xT, X, sizeof(X));
+  if (pen_out) *pen_out = pen_total;
+  free(hprev);
+  return S;
+}
+
+int orc_weights_update(int K, int T, double lambda, const double* S, const double* u,
+                       double* U_out, double* w, int* argmin, double* gap, double* eta) {
+  int kstar = -1, nonfinite = 0;
+  double s1 = INFINITY, s2 = INFINITY;
+  for (int k = 0; k < K; ++k) {
+    if (!isfinite(S[k])) { ++nonfinite; continue; }
+    if (S[k] < s1) { s2 = s1; s1 = S[k]; kstar = k; }   /* strict: lowest index wins ties */
+    else if (S[k] < s2) { s2 = S[k]; }
+  }
+  if (argmin) *argmin = kstar;
+  if (gap) *gap = s2 - s1;
+  if (kstar < 0) { if (eta) *eta = 0.0; return nonfinite; }
+
+  /* gamma_s = exp(-(J_s - min_j J_j)/lambda) */
+  double sum_w = 0.0;
+  double* wk = (double*)malloc(sizeof(double) * (size_t)K);
+  for (int k = 0; k < K; ++k) {
+    wk[k] = isfinite(S[k]) ? exp(-(S[k] - s1) / lambda) : 0.0;
+    sum_w += wk[k];
+  }
+  /* u_nom <- sum_s gamma_bar_s u~_s, eq. (5) */
+  for (int t = 0; t < 2 * T; ++t) {
+    double acc = 0.0;
+    for (int k = 0; k < K; ++k) acc += wk[k] * u[(size_t)k * 2 * T + t];
+    U_out[t] = acc / sum_w;
+  }
+  if (w) memcpy(w, wk, sizeof(double) * (size_t)K);
+  if (eta) *eta = sum_w;
+  free(wk);
+  return nonfinite;
+}
+
+typedef struct {
+  const orc_params* p;
+  uint32_t n;
+  const double *x0, *goal, *obstacles, *U_in;
+  int n_obs, k_begin, k_end;
+  double *S, *XT, *u_all;
+} sample_job;
+
+static void* sample_worker(void* arg) {
+  sample_job* job = (sample_job*)arg;
+  const orc_params* p = job->p;
+  const int T = p->T;
+  for (int k = job->k_begin; k < job->k_end; ++k) {
+    double* u = job->u_all + (size_t)k * 2 * T;
+    double alpha = orc_alpha(p, job->n, (uint32_t)k);
+    for (int t = 0; t < T; ++t) {
+      double z[2];
+      orc_normals(p->seed, job->n, (uint32_t)k, (uint32_t)t, z);
+      /* u~ = u_nom + w~, hard clamp to the control bounds (reading 9) */
+      u[2 * t + 0] = clampd(job->U_in[2 * t + 0] + p->sigma_v * z[0], p->v_min, p->v_max);
+      u[2 * t + 1] = clampd(job->U_in[2 * t + 1] + p->sigma_delta * z[1], p->delta_min, p->delta_max);
+    }
+    job->S[k] = orc_rollout(p, job->x0, job->goal, job->n_obs, job->obstacles, u, alpha,
+                            job->XT + 4 * (size_t)k, NULL, NULL);
+  }
+  return NULL;
+}
+
+int orc_iteration(const orc_params* p, uint32_t n, const double x0[4], const double goal[4],
+                  int n_obs, const double* obstacles, const double* U_in, double* U_out,
+                  double* S, double* XT, double* u_all, double* w, int* argmin, double* gap,
+                  double* eta, int n_threads) {
+  const int K = p->K, T = p->T;
+  double* S_buf = S ? S : (double*)malloc(sizeof(double) * (size_t)K);
+  double* XT_buf = XT ? XT : (double*)malloc(sizeof(double) * 4 * (size_t)K);
+  double* u_buf = u_all ? u_all : (double*)malloc(sizeof(double) * 2 * (size_t)T * (size_t)K);
+  double* U_nom = (double*)malloc(sizeof(double) * 2 * (size_t)T);
+  memcpy(U_nom, U_in, sizeof(double) * 2 * (size_t)T);
+
+  if (n_threads < 1) n_threads = 1;
+  if (n_threads > K) n_threads = K;
+  sample_job* jobs = (sample_job*)malloc(sizeof(sample_job) * (size_t)n_threads);
+  pthread_t* tids = (pthread_t*)malloc(sizeof(pthread_t) * (size_t)n_threads);
+  for (int i = 0; i < n_threads; ++i) {
+    jobs[i] = (sample_job){p, n, x0, goal, obstacles, U_nom, n_obs,
+                           (int)((long long)K * i / n_threads),
+                           (int)((long long)K * (i + 1) / n_threads), S_buf, XT_buf, u_buf};
+  }
+  if (n_threads == 1) {
+    sample_worker(&jobs[0]);
+  } else {
+    for (int i = 0; i < n_threads; ++i) pthread_create(&tids[i], NULL, sample_worker, &jobs[i]);
+    for (int i = 0; i < n_threads; ++i) pthread_join(tids[i], NULL);
+  }
+
+  /* U_out keeps U_in if every cost is non-finite */
+  if (U_out != U_in) memcpy(U_out, U_nom, sizeof(double) * 2 * (size_t)T);
+  int nonfinite = orc_weights_update(K, T, p->lambda, S_buf, u_buf, U_out, w, argmin, gap, eta);
+
+  free(jobs); free(tids); free(U_nom);
+  if (!S) free(S_buf);
+  if (!XT) free(XT_buf);
+  if (!u_all) free(u_buf);
+  return nonfinite;
+}
+
+void orc_shift(int T, double* U) {
+  for (int t = 0; t + 1 < T; ++t) {
+    U[2 * t + 0] = U[2 * (t + 1) + 0];
+    U[2 * t + 1] = U[2 * (t + 1) + 1];
+  }
+}
+
+void orc_plant_step(const orc_params* p, double x0[4], const double u0[2], int n_obs,
+                    double* obstacles) {
+  double xn[4];
+  orc_kinematic_step(p, x0, u0[0], u0[1], xn);
+  xn[2] = orc_wrap(xn[2]);
+  xn[3] = orc_wrap(xn[3]);
+  memcpy(x0, xn, sizeof(xn));
+  for (int i = 0; i < n_obs; ++i) {
+    obstacles[5 * i + 0] += p->dt * obstacles[5 * i + 3];
+    obstacles[5 * i + 1] += p->dt * obstacles[5 * i + 4];
+  }
+}

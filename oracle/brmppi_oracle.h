@@ -1,0 +1,134 @@
+/*
+ * brmppi_oracle.h -- CPU oracle for one BR-MPPI solve of a kinematic tractor-trailer.
+ *
+ * TEST INFRASTRUCTURE ONLY.  This is the plain, slow, obviously-correct restatement of the
+ * method in fp64 that the CUDA path is checked against.  Only tests/, __graft_entry__.smoke()
+ * and bench.py's cpu_baseline / --impl reference legs may call it.  It shares no code, header,
+ * table or constant generator with paper_2508_05773_b200/csrc/ and includes nothing from there.
+ *
+ * Passages followed (PAPER.md = text of arxiv 2508.05773; SURVEY.md §8(c) = the readings taken
+ * where the paper is silent, all listed again in DESIGN.md):
+ *   MPPI loop, weights, update (5), shift ........ PAPER.md:89-98
+ *   tractor-trailer kinematics, eq. (6) ........... PAPER.md:121-127 (reduced to [x,y,psi1,psi2])
+ *   discrete barrier-rate condition, eq. (2) ...... PAPER.md:64-74
+ *   disc barrier = eq. (16) with e = 2 ............ PAPER.md:216-225
+ *   stage + terminal cost structure, eq. (7) ...... PAPER.md:135
+ *   quadratic tracking / heading / effort terms ... PAPER.md:202
+ *   hitch-angle limit ............................. PAPER.md:231-235
+ *
+ * Pin status (tests/test_oracle_*.py, all `-m "not gpu"`):
+ *   philox4x32_10 ............ pinned: published known-answer vectors + cuRAND header constants
+ *   uniforms / Box-Muller .... pinned: exact representability, range, moments
+ *   kinematic step ........... pinned: straight line, Euler-circle radius, hitch relaxation
+ *                              closed form, steady-turn fixed point
+ *   barrier / hinge .......... pinned: h=0 on the inflated circle, h=3 at 2 rho, hand-computed
+ *                              step, receding sample => 0, stationary inside => T*alpha*|h|
+ *   weights / update / shift . pinned: positivity, sum to 1, shift invariance, permutation
+ *                              invariance, lambda->0 argmin, lambda->inf mean, sigma=0 fixed point
+ *   whole solve .............. pinned: brute force (independent mpmath transcription) K<=8, T<=5
+ *   cost weights, disc placement, hinge shapes (linear barrier hinge, squared hitch hinge),
+ *   scene generators ......... PARITY UNPINNED by the paper (never printed there); fixed by the
+ *                              readings in DESIGN.md only.
+ */
+#ifndef BRMPPI_ORACLE_H
+#define BRMPPI_ORACLE_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define ORC_MAX_DISCS 4
+
+/* All lengths in metres, angles in radians, times in seconds. */
+typedef struct {
+  int K;                  /* samples (rollouts) per iteration                         */
+  int T;                  /* horizon: controls u_0..u_{T-1}, states x_0..x_T          */
+  int n_discs;            /* vehicle discs, <= ORC_MAX_DISCS                           */
+  int disc_body[ORC_MAX_DISCS];     /* 0 = tractor (psi1), 1 = trailer (psi2)          */
+  double disc_offset[ORC_MAX_DISCS];/* metres from the hitch point along the body axis */
+  double disc_radius;     /* r_v                                                       */
+  double dt, L1, L2, Lh;
+  double v_min, v_max, delta_min, delta_max;
+  double sigma_v, sigma_delta;
+  double alpha_lo, alpha_hi;
+  double w_pos, w_head, w_v, w_delta, w_hitch, hitch_max, w_bar, w_term, lambda;
+  uint64_t seed;          /* Philox key = (lo32(seed), hi32(seed))                     */
+} orc_params;
+
+/* Philox4x32-10 block function (Salmon et al., SC'11). out = P(ctr; key). */
+void orc_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]);
+
+/* f(w) = (w >> 9) * 2^-23, in [0,1), exact in fp32 and fp64.  SURVEY §8(c) reading 5. */
+double orc_uniform(uint32_t w);
+
+/* The two standard normals of (seed, n, k, t): Philox ctr = (t, n, k, 0), words 0,1,
+ * Box-Muller with u1 = 1 - f(w0), u2 = f(w1).  z[0] -> speed channel, z[1] -> steering. */
+void orc_normals(uint64_t seed, uint32_t n, uint32_t k, uint32_t t, double z[2]);
+
+/* alpha_k of (seed, n, k): Philox ctr = (0, n, k, 1), word 0. */
+double orc_alpha(const orc_params* p, uint32_t n, uint32_t k);
+
+/* wrap(a) = a - 2 pi rint(a / 2 pi). */
+double orc_wrap(double a);
+
+/* One explicit-Euler step of the reduced eq. (6); every right-hand side at x. */
+void orc_kinematic_step(const orc_params* p, const double x[4], double v, double delta,
+                        double x_next[4]);
+
+/* Centre of vehicle disc j at state x. */
+void orc_disc_centre(const orc_params* p, const double x[4], int j, double c[2]);
+
+/* h = ||c - o||^2 / (R + r_v)^2 - 1 for disc centre c and obstacle centre o, radius R. */
+double orc_barrier(const orc_params* p, const double c[2], const double o[2], double R);
+
+/* G(x) = w_pos ||p - g_p||^2 + w_head (wrap(psi1-g_psi1)^2 + wrap(psi2-g_psi2)^2). */
+double orc_goal_cost(const orc_params* p, const double x[4], const double goal[4]);
+
+/*
+ * Roll out ONE sample under the given control sequence u[T][2] (already perturbed and
+ * clamped) and barrier-rate alpha.  obstacles = n_obs x (cx, cy, R, vx, vy) at rollout time 0.
+ * Returns S (total cost); x_T -> xT[4]; if traj != NULL it receives (T+1) x 4 states; if
+ * pen_out != NULL it receives the un-weighted barrier-rate penalty sum.
+ */
+double orc_rollout(const orc_params* p, const double x0[4], const double goal[4], int n_obs,
+                   const double* obstacles, const double* u, double alpha, double xT[4],
+                   double* traj, double* pen_out);
+
+/*
+ * Weights and update from costs S[K] and sampled controls u[K][T][2]:
+ *   k* = lowest k attaining the minimum finite S;  w_k = exp(-(S_k - S_k*)/lambda) (0 if S_k is
+ *   not finite);  eta = sum w;  U[t] = sum_k w_k u[k][t] / eta.
+ * Writes w[K] (un-normalised) if w != NULL.  Returns number of non-finite costs; if all K are
+ * non-finite U_out is left untouched, *argmin = -1.
+ * *gap = (second smallest S) - (smallest S)   (+inf if K == 1).
+ */
+int orc_weights_update(int K, int T, double lambda, const double* S, const double* u,
+                       double* U_out, double* w, int* argmin, double* gap, double* eta);
+
+/*
+ * One full MPPI iteration with global iteration counter n:
+ * sample, perturb + clamp, roll out, weight, update.  U_in[T][2] -> U_out[T][2] (may alias).
+ * Optional outputs (NULL to skip): S[K], XT[K][4], u_all[K][T][2], w[K].
+ * n_threads > 1 partitions the sample loop over pthreads; results are bit-identical to
+ * n_threads == 1 because every sample is independent and the reduction is done afterwards,
+ * single-threaded, in index order.
+ * Returns the number of non-finite costs.
+ */
+int orc_iteration(const orc_params* p, uint32_t n, const double x0[4], const double goal[4],
+                  int n_obs, const double* obstacles, const double* U_in, double* U_out,
+                  double* S, double* XT, double* u_all, double* w, int* argmin, double* gap,
+                  double* eta, int n_threads);
+
+/* Warm-start shift: U[t] = U[t+1] for t < T-1; U[T-1] unchanged (reading 4). */
+void orc_shift(int T, double* U);
+
+/* Plant step: x0 <- Euler(x0, u0), psi wrapped to [-pi, pi); obstacles advanced by dt * vel. */
+void orc_plant_step(const orc_params* p, double x0[4], const double u0[2], int n_obs,
+                    double* obstacles);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

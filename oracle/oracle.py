@@ -1,0 +1,251 @@
+"""ctypes front-end of the CPU oracle (oracle/brmppi_oracle.c).  TEST INFRASTRUCTURE ONLY:
+imported by tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs,
+never by paper_2508_05773_b200/.  Argument marshalling only -- all arithmetic is in the C file."""
+import ctypes as C
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "brmppi_oracle.c")
+_LIB = os.path.join(_HERE, "liboracle.so")
+ORC_MAX_DISCS = 4
+
+
+def build(force: bool = False) -> str:
+    """gcc -O2 build of liboracle.so next to its source (rebuilt when the source is newer)."""
+    hdr = os.path.join(_HERE, "brmppi_oracle.h")
+    stale = (not os.path.exists(_LIB)) or any(
+        os.path.getmtime(f) > os.path.getmtime(_LIB) for f in (_SRC, hdr))
+    if force or stale:
+        cmd = ["gcc", "-O2", "-std=c11", "-ffp-contract=off", "-fPIC", "-shared", "-o", _LIB, _SRC,
+               "-lm", "-lpthread"]
+        subprocess.check_call(cmd)
+    return _LIB
+
+
+class _Params(C.Structure):
+    _fields_ = [("K", C.c_int), ("T", C.c_int), ("n_discs", C.c_int),
+                ("disc_body", C.c_int * ORC_MAX_DISCS), ("disc_offset", C.c_double * ORC_MAX_DISCS),
+                ("disc_radius", C.c_double),
+                ("dt", C.c_double), ("L1", C.c_double), ("L2", C.c_double), ("Lh", C.c_double),
+                ("v_min", C.c_double), ("v_max", C.c_double),
+                ("delta_min", C.c_double), ("delta_max", C.c_double),
+                ("sigma_v", C.c_double), ("sigma_delta", C.c_double),
+                ("alpha_lo", C.c_double), ("alpha_hi", C.c_double),
+                ("w_pos", C.c_double), ("w_head", C.c_double), ("w_v", C.c_double),
+                ("w_delta", C.c_double), ("w_hitch", C.c_double), ("hitch_max", C.c_double),
+                ("w_bar", C.c_double), ("w_term", C.c_double), ("lam", C.c_double),
+                ("seed", C.c_uint64)]
+
+
+_lib = None
+_dp = C.POINTER(C.c_double)
+_u32p = C.POINTER(C.c_uint32)
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        L = C.CDLL(build())
+        L.orc_philox4x32_10.argtypes = [_u32p, _u32p, _u32p]
+        L.orc_philox4x32_10.restype = None
+        L.orc_uniform.argtypes = [C.c_uint32]
+        L.orc_uniform.restype = C.c_double
+        L.orc_normals.argtypes = [C.c_uint64, C.c_uint32, C.c_uint32, C.c_uint32, _dp]
+        L.orc_normals.restype = None
+        L.orc_alpha.argtypes = [C.POINTER(_Params), C.c_uint32, C.c_uint32]
+        L.orc_alpha.restype = C.c_double
+        L.orc_wrap.argtypes = [C.c_double]
+        L.orc_wrap.restype = C.c_double
+        L.orc_kinematic_step.argtypes = [C.POINTER(_Params), _dp, C.c_double, C.c_double, _dp]
+        L.orc_kinematic_step.restype = None
+        L.orc_disc_centre.argtypes = [C.POINTER(_Params), _dp, C.c_int, _dp]
+        L.orc_disc_centre.restype = None
+        L.orc_barrier.argtypes = [C.POINTER(_Params), _dp, _dp, C.c_double]
+        L.orc_barrier.restype = C.c_double
+        L.orc_goal_cost.argtypes = [C.POINTER(_Params), _dp, _dp]
+        L.orc_goal_cost.restype = C.c_double
+        L.orc_rollout.argtypes = [C.POINTER(_Params), _dp, _dp, C.c_int, _dp, _dp, C.c_double,
+                                  _dp, _dp, _dp]
+        L.orc_rollout.restype = C.c_double
+        L.orc_weights_update.argtypes = [C.c_int, C.c_int, C.c_double, _dp, _dp, _dp, _dp,
+                                         C.POINTER(C.c_int), _dp, _dp]
+        L.orc_weights_update.restype = C.c_int
+        L.orc_iteration.argtypes = [C.POINTER(_Params), C.c_uint32, _dp, _dp, C.c_int, _dp, _dp,
+                                    _dp, _dp, _dp, _dp, _dp, C.POINTER(C.c_int), _dp, _dp, C.c_int]
+        L.orc_iteration.restype = C.c_int
+        L.orc_shift.argtypes = [C.c_int, _dp]
+        L.orc_shift.restype = None
+        L.orc_plant_step.argtypes = [C.POINTER(_Params), _dp, _dp, C.c_int, _dp]
+        L.orc_plant_step.restype = None
+        _lib = L
+    return _lib
+
+
+def _cparams(p) -> _Params:
+    """scenes.Params (plain data) -> C struct."""
+    s = _Params()
+    s.K, s.T, s.n_discs = int(p.K), int(p.T), len(p.discs)
+    for j, (body, off) in enumerate(p.discs):
+        s.disc_body[j] = int(body)
+        s.disc_offset[j] = float(off)
+    for name in ("disc_radius", "dt", "L1", "L2", "Lh", "v_min", "v_max", "delta_min",
+                 "delta_max", "sigma_v", "sigma_delta", "alpha_lo", "alpha_hi", "w_pos", "w_head",
+                 "w_v", "w_delta", "w_hitch", "hitch_max", "w_bar", "w_term", "lam"):
+        setattr(s, name, float(getattr(p, name)))
+    s.seed = int(p.seed) & 0xFFFFFFFFFFFFFFFF
+    return s
+
+
+def _d(a, shape=None):
+    a = np.ascontiguousarray(a, dtype=np.float64)
+    if shape is not None:
+        a = a.reshape(shape)
+    return a
+
+
+def _ptr(a):
+    return a.ctypes.data_as(_dp)
+
+
+def philox(ctr, key):
+    c = (C.c_uint32 * 4)(*[int(x) & 0xFFFFFFFF for x in ctr])
+    k = (C.c_uint32 * 2)(*[int(x) & 0xFFFFFFFF for x in key])
+    o = (C.c_uint32 * 4)()
+    lib().orc_philox4x32_10(c, k, o)
+    return tuple(int(x) for x in o)
+
+
+def uniform(w):
+    return lib().orc_uniform(int(w) & 0xFFFFFFFF)
+
+
+def normals(seed, n, k, t):
+    z = np.zeros(2)
+    lib().orc_normals(int(seed), int(n), int(k), int(t), _ptr(z))
+    return z
+
+
+def alpha(p, n, k):
+    cp = _cparams(p)
+    return lib().orc_alpha(C.byref(cp), int(n), int(k))
+
+
+def wrap(a):
+    return lib().orc_wrap(float(a))
+
+
+def kinematic_step(p, x, v, delta):
+    cp = _cparams(p)
+    x = _d(x, (4,))
+    xn = np.zeros(4)
+    lib().orc_kinematic_step(C.byref(cp), _ptr(x), float(v), float(delta), _ptr(xn))
+    return xn
+
+
+def disc_centre(p, x, j):
+    cp = _cparams(p)
+    x = _d(x, (4,))
+    c = np.zeros(2)
+    lib().orc_disc_centre(C.byref(cp), _ptr(x), int(j), _ptr(c))
+    return c
+
+
+def barrier(p, c, o, R):
+    cp = _cparams(p)
+    c, o = _d(c, (2,)), _d(o, (2,))
+    return lib().orc_barrier(C.byref(cp), _ptr(c), _ptr(o), float(R))
+
+
+def goal_cost(p, x, goal):
+    cp = _cparams(p)
+    x, goal = _d(x, (4,)), _d(goal, (4,))
+    return lib().orc_goal_cost(C.byref(cp), _ptr(x), _ptr(goal))
+
+
+def rollout(p, x0, goal, obstacles, u, alpha_k, want_traj=False):
+    """One sample.  Returns dict(S, xT, pen, traj)."""
+    cp = _cparams(p)
+    x0, goal = _d(x0, (4,)), _d(goal, (4,))
+    obstacles = _d(obstacles).reshape(-1, 5)
+    u = _d(u, (p.T, 2))
+    xT = np.zeros(4)
+    traj = np.zeros((p.T + 1, 4)) if want_traj else None
+    pen = C.c_double(0.0)
+    S = lib().orc_rollout(C.byref(cp), _ptr(x0), _ptr(goal), obstacles.shape[0], _ptr(obstacles),
+                          _ptr(u), float(alpha_k), _ptr(xT), _ptr(traj) if want_traj else None,
+                          C.cast(C.byref(pen), _dp))
+    return dict(S=S, xT=xT, pen=pen.value, traj=traj)
+
+
+def weights_update(S, u, lam):
+    """S[K], u[K][T][2] -> dict(U, w, argmin, gap, eta, nonfinite)."""
+    S = _d(S)
+    K = S.shape[0]
+    u = _d(u).reshape(K, -1, 2)
+    T = u.shape[1]
+    U = np.zeros((T, 2))
+    w = np.zeros(K)
+    am = C.c_int(0)
+    gap = C.c_double(0.0)
+    eta = C.c_double(0.0)
+    nf = lib().orc_weights_update(K, T, float(lam), _ptr(S), _ptr(u), _ptr(U), _ptr(w),
+                                  C.byref(am), C.cast(C.byref(gap), _dp),
+                                  C.cast(C.byref(eta), _dp))
+    return dict(U=U, w=w, argmin=am.value, gap=gap.value, eta=eta.value, nonfinite=nf)
+
+
+def iteration(p, n, x0, goal, obstacles, U_in, n_threads=1, want_samples=False):
+    """One MPPI iteration with global counter n.  Returns dict(U, S, XT, argmin, gap, eta,
+    nonfinite[, u, w])."""
+    cp = _cparams(p)
+    K, T = p.K, p.T
+    x0, goal = _d(x0, (4,)), _d(goal, (4,))
+    obstacles = _d(obstacles).reshape(-1, 5)
+    U_in = _d(U_in, (T, 2))
+    U = np.zeros((T, 2))
+    S = np.zeros(K)
+    XT = np.zeros((K, 4))
+    u = np.zeros((K, T, 2)) if want_samples else None
+    w = np.zeros(K) if want_samples else None
+    am = C.c_int(0)
+    gap = C.c_double(0.0)
+    eta = C.c_double(0.0)
+    nf = lib().orc_iteration(C.byref(cp), int(n), _ptr(x0), _ptr(goal), obstacles.shape[0],
+                             _ptr(obstacles), _ptr(U_in), _ptr(U), _ptr(S), _ptr(XT),
+                             _ptr(u) if want_samples else None, _ptr(w) if want_samples else None,
+                             C.byref(am), C.cast(C.byref(gap), _dp), C.cast(C.byref(eta), _dp),
+                             int(n_threads))
+    out = dict(U=U, S=S, XT=XT, argmin=am.value, gap=gap.value, eta=eta.value, nonfinite=nf)
+    if want_samples:
+        out["u"], out["w"] = u, w
+    return out
+
+
+def solve(p, n0, x0, goal, obstacles, U_in, n_threads=1):
+    """p.n_iter iterations starting at counter n0, no shift in between (CFG2).  Returns the list
+    of per-iteration results; the last one's U is the solve's output."""
+    U = _d(U_in, (p.T, 2)).copy()
+    outs = []
+    for it in range(p.n_iter):
+        r = iteration(p, n0 + it, x0, goal, obstacles, U, n_threads=n_threads)
+        U = r["U"]
+        outs.append(r)
+    return outs
+
+
+def shift(U):
+    U = _d(U).copy()
+    lib().orc_shift(U.shape[0], _ptr(U))
+    return U
+
+
+def plant_step(p, x0, u0, obstacles):
+    cp = _cparams(p)
+    x = _d(x0, (4,)).copy()
+    u0 = _d(u0, (2,))
+    obs = _d(obstacles).reshape(-1, 5).copy()
+    lib().orc_plant_step(C.byref(cp), _ptr(x), _ptr(u0), obs.shape[0], _ptr(obs))
+    return x, obs
