@@ -1,0 +1,182 @@
+/*
+ * brmppi.h -- C ABI of the B200 (sm_100a) Barrier-Rate guided MPPI solver for a kinematic
+ * tractor-trailer (arxiv 2508.05773).  Plain C: no C++ types, no exceptions, no torch types.
+ *
+ * What the calls are, and where the paper defines them:
+ *   "At each control step, BR-MPPI receives the current state of the TT system and its
+ *    environment, including static obstacles and predicted pedestrian motion, and generates
+ *    control inputs"
+ *   one MPPI solve = sample, roll out, weight, update                  (eq. 5)
+ *   "u_k = u_nom,k is applied ... the last input is shifted, and the process repeats"
+ *
+ *   nominal control sequence initialised with zero
+ *   model: eq. (6) reduced to [x, y, psi1, psi2] with controls (v, delta)
+ *   barrier: eq. (16), e = 2 (discs); barrier-rate condition eq. (2)
+ * The instance (4-state model, disc obstacles, per-sample alpha, hinge penalty) is the one
+ * BASELINE.json's north_star names; every reading of the paper is listed in DESIGN.md.
+ *
+ * Pointer kinds.  Unless a parameter says DEVICE, every pointer is a HOST pointer owned by the
+ * caller; the library copies in/out and keeps no reference after the call returns.
+ * Ownership.  The caller owns the device workspace and the CUDA stream (with PyTorch:
+ * torch.empty(bytes, dtype=torch.uint8, device="cuda").data_ptr() and
+ * torch.cuda.Stream().cuda_stream); both must outlive the context.  The library never calls
+ * cudaMalloc for solver data; it owns only the small host-side context object (and the CUDA
+ * graph it captures for brmppi_step).
+ * Errors.  Every call returns 0 (BRMPPI_OK) or a negative brmppi_status; nothing aborts, throws
+ * or prints.  brmppi_strerror() maps a status to text; for BRMPPI_ERR_CUDA the text of the last
+ * CUDA error seen by that call is appended.
+ * Threads.  A context is not thread-safe; distinct contexts are independent.
+ * Stream order.  solve / shift / set_* are enqueued on the context's stream and return without
+ * waiting; get_* and brmppi_step synchronise that stream before returning.
+ * No CPU fallback exists: without a CUDA device brmppi_create returns BRMPPI_ERR_CUDA.
+ */
+#ifndef BRMPPI_H
+#define BRMPPI_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define BRMPPI_MAX_DISCS 4
+
+typedef enum {
+  BRMPPI_OK = 0,
+  BRMPPI_ERR_NULL = -1,                /* a required pointer was NULL                         */
+  BRMPPI_ERR_INVALID_ARG = -2,         /* K<1, T<1, dt<=0, lambda<=0, sigma<0, bounds inverted,
+                                          L<=0, scene out of range, unknown flag ...           */
+  BRMPPI_ERR_WORKSPACE_TOO_SMALL = -3,
+  BRMPPI_ERR_TOO_MANY_OBSTACLES = -4,
+  BRMPPI_ERR_NONFINITE_INPUT = -5,     /* NaN/Inf in a state, goal, obstacle or control input  */
+  BRMPPI_ERR_NOT_READY = -6,           /* solve/step before state and goal of every scene set;
+                                          get_costs/get_final_states without FLAG_WRITE_SAMPLES */
+  BRMPPI_ERR_CUDA = -7,
+  BRMPPI_ERR_UNALIGNED = -8            /* workspace not 256-byte aligned                       */
+} brmppi_status;
+
+/* Disc obstacle with constant-velocity prediction (Assumption 2):
+ * centre at rollout step t is (cx + t dt vx, cy + t dt vy).  radius > 0. */
+typedef struct { float cx, cy, radius, vx, vy; } brmppi_obstacle;
+
+/* Vehicle disc: body 0 = tractor axis (psi1), 1 = trailer axis (psi2); offset in metres from the
+ * hitch point p_h = (x - Lh cos psi1, y - Lh sin psi1) along that axis. */
+typedef struct { int body; float offset; } brmppi_disc;
+
+/* flags */
+#define BRMPPI_FLAG_WRITE_SAMPLES 1u   /* write S_k and x_T of every sample to HBM (parity /
+                                          diagnostics; 20 B per sample)                        */
+#define BRMPPI_FLAG_PRECISE_MATH  2u   /* sinf/cosf/tanf/logf instead of MUFU intrinsics      */
+#define BRMPPI_FLAG_KERNEL_THREAD_PER_SAMPLE 4u  /* baseline kernel: one thread per sample, all
+                                          steps fused (north_star item 2).  Default is the
+                                          phase-split tile kernel.               */
+
+typedef struct {
+  int K;              /* samples per iteration, >= 1                                            */
+  int T;              /* horizon steps, 1..BRMPPI_MAX_T                                         */
+  int n_iter;         /* MPPI iterations per solve (no shift in between), >= 1                  */
+  int n_scenes;       /* independent scenes solved per launch, >= 1; scene s uses seed + s      */
+  int max_obstacles;  /* capacity per scene, 0..BRMPPI_MAX_OBSTACLES                            */
+  int n_discs;        /* 1..BRMPPI_MAX_DISCS                                                    */
+  brmppi_disc discs[BRMPPI_MAX_DISCS];
+  float disc_radius;  /* r_v: obstacles are inflated to R + r_v                                 */
+  float dt, L1, L2, Lh;
+  float v_min, v_max, delta_min, delta_max;   /* hard clamp after perturbation (reading 9)      */
+  float sigma_v, sigma_delta;                 /* Sigma_w = diag(sigma_v^2, sigma_delta^2)        */
+  float alpha_lo, alpha_hi;                   /* alpha_k ~ U[alpha_lo, alpha_hi)                 */
+  float w_pos, w_head, w_v, w_delta, w_hitch, hitch_max, w_bar, w_term, lambda;
+  unsigned long long seed;
+  unsigned int flags;
+} brmppi_params;
+
+#define BRMPPI_MAX_T 512
+#define BRMPPI_MAX_OBSTACLES 64
+
+typedef struct brmppi_ctx brmppi_ctx;   /* opaque, library-owned host object */
+
+typedef struct {
+  float S_min;              /* smallest finite cost of the last iteration                       */
+  int argmin;               /* its sample index (lowest index on ties), -1 if none finite       */
+  float eta;                /* sum_k exp(-(S_k - S_min)/lambda)                                 */
+  float ess;                /* effective sample size eta^2 / sum w^2                            */
+  unsigned long long n;     /* global iteration counter after the last iteration                */
+  int nonfinite;            /* samples whose cost was NaN/Inf (weight 0, skipped by argmin)     */
+} brmppi_diag;
+
+/* Bytes of device workspace brmppi_create needs for these parameters; 0 if they are invalid. */
+size_t brmppi_workspace_bytes(const brmppi_params* p);
+
+/* Create a context on the CURRENT CUDA device.  dev_workspace: DEVICE pointer, 256-byte aligned,
+ * >= brmppi_workspace_bytes(p) bytes; cuda_stream: a cudaStream_t (NULL = legacy default
+ * stream).  Nominal controls start at zero, iteration counter n = 0. */
+int brmppi_create(const brmppi_params* p, void* dev_workspace, size_t workspace_bytes,
+                  void* cuda_stream, brmppi_ctx** out);
+
+/* Destroys the host object (and any captured graph).  Never frees the workspace. */
+int brmppi_destroy(brmppi_ctx* ctx);
+
+/* Vehicle state (x, y, psi1, psi2) of one scene.  psi1, psi2 are wrapped to [-pi, pi]. */
+int brmppi_set_state(brmppi_ctx* ctx, int scene, const float x[4]);
+/* Goal pose (g_x, g_y, g_psi1, g_psi2). */
+int brmppi_set_goal(brmppi_ctx* ctx, int scene, const float g[4]);
+/* Obstacles of one scene at rollout time 0; 0 <= n <= max_obstacles (NULL allowed when n = 0). */
+int brmppi_set_obstacles(brmppi_ctx* ctx, int scene, int n, const brmppi_obstacle* obstacles);
+/* Nominal control sequence U[T][2] = (v, delta) per step; NULL = zeros.  Values must lie in
+ * the control box (else BRMPPI_ERR_INVALID_ARG). */
+int brmppi_set_nominal(brmppi_ctx* ctx, int scene, const float* U);
+/* Set the global iteration counter n (the Philox counter word; reading 7).  All scenes. */
+int brmppi_set_counter(brmppi_ctx* ctx, unsigned int n);
+/* U = 0 and n = 0 for all scenes (state, goal and obstacles are kept). */
+int brmppi_reset(brmppi_ctx* ctx);
+
+/* One solve of every scene: n_iter x { sample, roll out, weight, update (5) }, n += n_iter.
+ * Asynchronous on the stream.  A sample with non-finite cost gets weight 0; if all K are
+ * non-finite U is left unchanged (diag.nonfinite == K). */
+int brmppi_solve(brmppi_ctx* ctx);
+/* Warm-start shift U[t] <- U[t+1], last element kept (reading 4).  Asynchronous. */
+int brmppi_shift(brmppi_ctx* ctx);
+/* One closed-loop control step as a single CUDA-graph replay: solve; apply U[0] to the
+ * kinematic model (one Euler step of eq. (6), psi wrapped); advance obstacles by dt * velocity;
+ * shift.  Synchronises; u0_out[n_scenes][2] receives the applied control of each scene. */
+int brmppi_step(brmppi_ctx* ctx, float* u0_out);
+
+/* Results.  All synchronise the stream. */
+int brmppi_get_controls(brmppi_ctx* ctx, int scene, float* U_out /* T*2 */);
+int brmppi_get_state(brmppi_ctx* ctx, int scene, float x_out[4]);
+int brmppi_get_obstacles(brmppi_ctx* ctx, int scene, int* n_out, brmppi_obstacle* out /* max_obstacles */);
+int brmppi_get_costs(brmppi_ctx* ctx, int scene, float* S_out /* K */);             /* FLAG_WRITE_SAMPLES */
+int brmppi_get_final_states(brmppi_ctx* ctx, int scene, float* X_out /* K*4 */);    /* FLAG_WRITE_SAMPLES */
+int brmppi_get_diag(brmppi_ctx* ctx, int scene, brmppi_diag* out);
+
+/* Number of kernel launches this context has enqueued so far (graph replays count the kernels
+ * inside the graph). */
+unsigned long long brmppi_launch_count(const brmppi_ctx* ctx);
+
+const char* brmppi_strerror(int status);
+
+/* ---- test / measurement entry points --------------------------------------------------- */
+
+/* Raw words of the in-kernel Philox4x32-10 generator: for k < K, t < T writes the four words
+ * of the block with counter (t, n, k, tag) and key (lo32(seed), hi32(seed)) to
+ * dev_out[(k*T + t)*4 + 0..3] (DEVICE pointer, K*T*4 uint32).  Uses the same device function as
+ * the rollout kernels.  Synchronises. */
+int brmppi_debug_philox(void* cuda_stream, unsigned long long seed, unsigned int n, int K, int T,
+                        unsigned int tag, unsigned int* dev_out);
+
+/* The perturbed, clamped controls and alpha the kernels draw for (params, n, nominal U): writes
+ * u[K][T][2] and alpha[K] (DEVICE pointers; either may be NULL).  U_nominal: HOST T*2 or NULL.
+ * Same device functions as the rollout kernels.  Synchronises. */
+int brmppi_debug_sample_controls(void* cuda_stream, const brmppi_params* p, unsigned int n,
+                                 const float* U_nominal, float* dev_u, float* dev_alpha);
+
+/* Issue-rate micro-benchmarks for the roofline denominator: thread-instructions
+ * per clock per SM achieved by dependent-chain-free streams of FFMA, LOP3/IADD3 (ALU pipe),
+ * MUFU (XU pipe) and the FFMA+ALU mix, plus the SM count and the clock measured in-kernel.
+ * out[0..7] = {ffma, alu, mufu, mix, imad_wide, n_sms, sm_mhz_measured, ffma rate cross-checked
+ * on the globaltimer}. */
+int brmppi_measure_peaks(void* cuda_stream, float out[8]);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

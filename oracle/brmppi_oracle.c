@@ -216,23 +216,29 @@ typedef struct {
   double *S, *XT, *u_all;
 } sample_job;
 
+/* Sample k of iteration n: draw alpha_k and the perturbed, clamped controls, roll out. */
+double orc_sample(const orc_params* p, uint32_t n, uint32_t k, const double x0[4],
+                  const double goal[4], int n_obs, const double* obstacles, const double* U_in,
+                  double* u /* T*2 */, double xT[4]) {
+  const int T = p->T;
+  double alpha = orc_alpha(p, n, k);
+  for (int t = 0; t < T; ++t) {
+    double z[2];
+    orc_normals(p->seed, n, k, (uint32_t)t, z);
+    /* u~ = u_nom + w~, hard clamp to the control bounds (reading 9) */
+    u[2 * t + 0] = clampd(U_in[2 * t + 0] + p->sigma_v * z[0], p->v_min, p->v_max);
+    u[2 * t + 1] = clampd(U_in[2 * t + 1] + p->sigma_delta * z[1], p->delta_min, p->delta_max);
+  }
+  return orc_rollout(p, x0, goal, n_obs, obstacles, u, alpha, xT, NULL, NULL);
+}
+
 static void* sample_worker(void* arg) {
   sample_job* job = (sample_job*)arg;
-  const orc_params* p = job->p;
-  const int T = p->T;
-  for (int k = job->k_begin; k < job->k_end; ++k) {
-    double* u = job->u_all + (size_t)k * 2 * T;
-    double alpha = orc_alpha(p, job->n, (uint32_t)k);
-    for (int t = 0; t < T; ++t) {
-      double z[2];
-      orc_normals(p->seed, job->n, (uint32_t)k, (uint32_t)t, z);
-      /* u~ = u_nom + w~, hard clamp to the control bounds (reading 9) */
-      u[2 * t + 0] = clampd(job->U_in[2 * t + 0] + p->sigma_v * z[0], p->v_min, p->v_max);
-      u[2 * t + 1] = clampd(job->U_in[2 * t + 1] + p->sigma_delta * z[1], p->delta_min, p->delta_max);
-    }
-    job->S[k] = orc_rollout(p, job->x0, job->goal, job->n_obs, job->obstacles, u, alpha,
-                            job->XT + 4 * (size_t)k, NULL, NULL);
-  }
+  const int T = job->p->T;
+  for (int k = job->k_begin; k < job->k_end; ++k)
+    job->S[k] = orc_sample(job->p, job->n, (uint32_t)k, job->x0, job->goal, job->n_obs,
+                           job->obstacles, job->U_in, job->u_all + (size_t)k * 2 * T,
+                           job->XT + 4 * (size_t)k);
   return NULL;
 }
 

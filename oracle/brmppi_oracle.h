@@ -96,6 +96,12 @@ double orc_rollout(const orc_params* p, const double x0[4], const double goal[4]
                    const double* obstacles, const double* u, double alpha, double xT[4],
                    double* traj, double* pen_out);
 
+/* Sample k of iteration n with nominal U_in[T][2]: draws alpha_k and u~_k (written to u[T][2]),
+ * rolls out, returns S_k; x_T -> xT. */
+double orc_sample(const orc_params* p, uint32_t n, uint32_t k, const double x0[4],
+                  const double goal[4], int n_obs, const double* obstacles, const double* U_in,
+                  double* u, double xT[4]);
+
 /*
  * Weights and update from costs S[K] and sampled controls u[K][T][2]:
  *   k* = lowest k attaining the minimum finite S;  w_k = exp(-(S_k - S_k*)/lambda) (0 if S_k is

@@ -70,6 +70,9 @@ def lib():
         L.orc_rollout.argtypes = [C.POINTER(_Params), _dp, _dp, C.c_int, _dp, _dp, C.c_double,
                                   _dp, _dp, _dp]
         L.orc_rollout.restype = C.c_double
+        L.orc_sample.argtypes = [C.POINTER(_Params), C.c_uint32, C.c_uint32, _dp, _dp, C.c_int, _dp,
+                                 _dp, _dp, _dp]
+        L.orc_sample.restype = C.c_double
         L.orc_weights_update.argtypes = [C.c_int, C.c_int, C.c_double, _dp, _dp, _dp, _dp,
                                          C.POINTER(C.c_int), _dp, _dp]
         L.orc_weights_update.restype = C.c_int
@@ -178,6 +181,19 @@ def rollout(p, x0, goal, obstacles, u, alpha_k, want_traj=False):
                           _ptr(u), float(alpha_k), _ptr(xT), _ptr(traj) if want_traj else None,
                           C.cast(C.byref(pen), _dp))
     return dict(S=S, xT=xT, pen=pen.value, traj=traj)
+
+
+def sample(p, n, k, x0, goal, obstacles, U_in):
+    """Sample k of iteration n alone: dict(S, xT, u)."""
+    cp = _cparams(p)
+    x0, goal = _d(x0, (4,)), _d(goal, (4,))
+    obstacles = _d(obstacles).reshape(-1, 5)
+    U_in = _d(U_in, (p.T, 2))
+    u = np.zeros((p.T, 2))
+    xT = np.zeros(4)
+    S = lib().orc_sample(C.byref(cp), int(n), int(k), _ptr(x0), _ptr(goal), obstacles.shape[0],
+                         _ptr(obstacles), _ptr(U_in), _ptr(u), _ptr(xT))
+    return dict(S=S, xT=xT, u=u)
 
 
 def weights_update(S, u, lam):

@@ -1,0 +1,288 @@
+"""Thin Python binding of the C ABI in include/brmppi.h -- same names, argument marshalling only.
+
+PyTorch provides device memory (the workspace tensor) and the CUDA stream; every step of the hot
+path runs in libbrmppi.so's kernels.  There is no CPU fallback: if the CUDA library is missing or
+no device is present, construction raises."""
+import ctypes as C
+import os
+
+import numpy as np
+
+from . import build as _build
+
+MAX_DISCS = 4
+FLAG_WRITE_SAMPLES = 1
+FLAG_PRECISE_MATH = 2
+FLAG_KERNEL_THREAD_PER_SAMPLE = 4
+
+OK = 0
+ERR_NULL, ERR_INVALID_ARG, ERR_WORKSPACE_TOO_SMALL, ERR_TOO_MANY_OBSTACLES = -1, -2, -3, -4
+ERR_NONFINITE_INPUT, ERR_NOT_READY, ERR_CUDA, ERR_UNALIGNED = -5, -6, -7, -8
+
+EXPORTS = [
+    "brmppi_workspace_bytes", "brmppi_create", "brmppi_destroy", "brmppi_set_state",
+    "brmppi_set_goal", "brmppi_set_obstacles", "brmppi_set_nominal", "brmppi_set_counter",
+    "brmppi_reset", "brmppi_solve", "brmppi_shift", "brmppi_step", "brmppi_get_controls",
+    "brmppi_get_state", "brmppi_get_obstacles", "brmppi_get_costs", "brmppi_get_final_states",
+    "brmppi_get_diag", "brmppi_launch_count", "brmppi_strerror", "brmppi_debug_philox",
+    "brmppi_debug_sample_controls", "brmppi_measure_peaks",
+]
+
+
+class Obstacle(C.Structure):
+    _fields_ = [("cx", C.c_float), ("cy", C.c_float), ("radius", C.c_float),
+                ("vx", C.c_float), ("vy", C.c_float)]
+
+
+class Disc(C.Structure):
+    _fields_ = [("body", C.c_int), ("offset", C.c_float)]
+
+
+class CParams(C.Structure):
+    _fields_ = [("K", C.c_int), ("T", C.c_int), ("n_iter", C.c_int), ("n_scenes", C.c_int),
+                ("max_obstacles", C.c_int), ("n_discs", C.c_int), ("discs", Disc * MAX_DISCS),
+                ("disc_radius", C.c_float),
+                ("dt", C.c_float), ("L1", C.c_float), ("L2", C.c_float), ("Lh", C.c_float),
+                ("v_min", C.c_float), ("v_max", C.c_float),
+                ("delta_min", C.c_float), ("delta_max", C.c_float),
+                ("sigma_v", C.c_float), ("sigma_delta", C.c_float),
+                ("alpha_lo", C.c_float), ("alpha_hi", C.c_float),
+                ("w_pos", C.c_float), ("w_head", C.c_float), ("w_v", C.c_float),
+                ("w_delta", C.c_float), ("w_hitch", C.c_float), ("hitch_max", C.c_float),
+                ("w_bar", C.c_float), ("w_term", C.c_float), ("lam", C.c_float),
+                ("seed", C.c_ulonglong), ("flags", C.c_uint)]
+
+
+class Diag(C.Structure):
+    _fields_ = [("S_min", C.c_float), ("argmin", C.c_int), ("eta", C.c_float), ("ess", C.c_float),
+                ("n", C.c_ulonglong), ("nonfinite", C.c_int)]
+
+
+class BrmppiError(RuntimeError):
+    def __init__(self, status, text):
+        super().__init__(f"brmppi status {status}: {text}")
+        self.status = status
+
+
+_lib = None
+_fp = C.POINTER(C.c_float)
+
+
+def lib():
+    """Load libbrmppi.so (building it in-tree first if its sources are newer)."""
+    global _lib
+    if _lib is None:
+        # BRMPPI_LIB: load a pre-built variant of the library (kernel-tuning experiments)
+        path = os.environ.get("BRMPPI_LIB") or _build.build()
+        L = C.CDLL(path)
+        vp = C.c_void_p
+        L.brmppi_workspace_bytes.argtypes = [C.POINTER(CParams)]
+        L.brmppi_workspace_bytes.restype = C.c_size_t
+        L.brmppi_create.argtypes = [C.POINTER(CParams), vp, C.c_size_t, vp, C.POINTER(vp)]
+        L.brmppi_destroy.argtypes = [vp]
+        L.brmppi_set_state.argtypes = [vp, C.c_int, _fp]
+        L.brmppi_set_goal.argtypes = [vp, C.c_int, _fp]
+        L.brmppi_set_obstacles.argtypes = [vp, C.c_int, C.c_int, C.POINTER(Obstacle)]
+        L.brmppi_set_nominal.argtypes = [vp, C.c_int, _fp]
+        L.brmppi_set_counter.argtypes = [vp, C.c_uint]
+        L.brmppi_reset.argtypes = [vp]
+        L.brmppi_solve.argtypes = [vp]
+        L.brmppi_shift.argtypes = [vp]
+        L.brmppi_step.argtypes = [vp, _fp]
+        L.brmppi_get_controls.argtypes = [vp, C.c_int, _fp]
+        L.brmppi_get_state.argtypes = [vp, C.c_int, _fp]
+        L.brmppi_get_obstacles.argtypes = [vp, C.c_int, C.POINTER(C.c_int), C.POINTER(Obstacle)]
+        L.brmppi_get_costs.argtypes = [vp, C.c_int, _fp]
+        L.brmppi_get_final_states.argtypes = [vp, C.c_int, _fp]
+        L.brmppi_get_diag.argtypes = [vp, C.c_int, C.POINTER(Diag)]
+        L.brmppi_launch_count.argtypes = [vp]
+        L.brmppi_launch_count.restype = C.c_ulonglong
+        L.brmppi_strerror.argtypes = [C.c_int]
+        L.brmppi_strerror.restype = C.c_char_p
+        L.brmppi_debug_philox.argtypes = [vp, C.c_ulonglong, C.c_uint, C.c_int, C.c_int, C.c_uint, vp]
+        L.brmppi_debug_sample_controls.argtypes = [vp, C.POINTER(CParams), C.c_uint, _fp, vp, vp]
+        L.brmppi_measure_peaks.argtypes = [vp, _fp]
+        _lib = L
+    return _lib
+
+
+def strerror(status):
+    return lib().brmppi_strerror(int(status)).decode()
+
+
+def _check(status):
+    if status != OK:
+        raise BrmppiError(status, strerror(status))
+
+
+def make_cparams(p, n_scenes=1, max_obstacles=8, flags=0) -> CParams:
+    """scenes.Params (plain data) -> brmppi_params."""
+    c = CParams()
+    c.K, c.T, c.n_iter, c.n_scenes = int(p.K), int(p.T), int(p.n_iter), int(n_scenes)
+    c.max_obstacles, c.n_discs = int(max_obstacles), len(p.discs)
+    for j, (body, off) in enumerate(p.discs):
+        c.discs[j].body, c.discs[j].offset = int(body), float(off)
+    for name in ("disc_radius", "dt", "L1", "L2", "Lh", "v_min", "v_max", "delta_min", "delta_max",
+                 "sigma_v", "sigma_delta", "alpha_lo", "alpha_hi", "w_pos", "w_head", "w_v",
+                 "w_delta", "w_hitch", "hitch_max", "w_bar", "w_term", "lam"):
+        setattr(c, name, float(getattr(p, name)))
+    c.seed, c.flags = int(p.seed) & 0xFFFFFFFFFFFFFFFF, int(flags)
+    return c
+
+
+def _f32(a, shape=None):
+    a = np.ascontiguousarray(a, dtype=np.float32)
+    return a.reshape(shape) if shape is not None else a
+
+
+def _p(a):
+    return a.ctypes.data_as(_fp)
+
+
+class Solver:
+    """One brmppi_ctx plus the torch-owned workspace and stream it lives on."""
+
+    def __init__(self, params, n_scenes=1, max_obstacles=8, flags=0, stream=None, device="cuda:0"):
+        import torch
+        if not torch.cuda.is_available():
+            raise RuntimeError("brmppi needs a CUDA device (there is no CPU fallback)")
+        self._torch = torch
+        self.device = torch.device(device)
+        torch.cuda.set_device(self.device)
+        self.params = params
+        self.cparams = make_cparams(params, n_scenes, max_obstacles, flags)
+        self.n_scenes, self.K, self.T = int(n_scenes), int(params.K), int(params.T)
+        self.max_obstacles = int(max_obstacles)
+        L = lib()
+        nbytes = L.brmppi_workspace_bytes(C.byref(self.cparams))
+        if nbytes == 0:
+            raise BrmppiError(ERR_INVALID_ARG, strerror(ERR_INVALID_ARG))
+        self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+        ptr = (self.workspace.data_ptr() + 255) // 256 * 256
+        self.stream = stream if stream is not None else torch.cuda.Stream(device=self.device)
+        self._ctx = C.c_void_p()
+        torch.cuda.synchronize(self.device)
+        _check(L.brmppi_create(C.byref(self.cparams), C.c_void_p(ptr), C.c_size_t(nbytes),
+                               C.c_void_p(self.stream.cuda_stream), C.byref(self._ctx)))
+
+    def close(self):
+        if getattr(self, "_ctx", None) is not None and self._ctx.value:
+            self.stream.synchronize()
+            lib().brmppi_destroy(self._ctx)
+            self._ctx = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # ---- inputs -------------------------------------------------------------------------
+    def set_state(self, x, scene=0):
+        _check(lib().brmppi_set_state(self._ctx, scene, _p(_f32(x, (4,)))))
+
+    def set_goal(self, g, scene=0):
+        _check(lib().brmppi_set_goal(self._ctx, scene, _p(_f32(g, (4,)))))
+
+    def set_obstacles(self, obstacles, scene=0):
+        obs = _f32(obstacles).reshape(-1, 5)
+        n = obs.shape[0]
+        ptr = obs.ctypes.data_as(C.POINTER(Obstacle)) if n else None
+        _check(lib().brmppi_set_obstacles(self._ctx, scene, n, ptr))
+
+    def set_nominal(self, U=None, scene=0):
+        _check(lib().brmppi_set_nominal(self._ctx, scene, None if U is None else _p(_f32(U, (self.T, 2)))))
+
+    def set_counter(self, n):
+        _check(lib().brmppi_set_counter(self._ctx, int(n)))
+
+    def reset(self):
+        _check(lib().brmppi_reset(self._ctx))
+
+    def set_scene(self, scene_obj, scene=0):
+        self.set_state(scene_obj.x0, scene)
+        self.set_goal(scene_obj.goal, scene)
+        self.set_obstacles(scene_obj.obstacles, scene)
+
+    # ---- work ---------------------------------------------------------------------------
+    def solve(self):
+        _check(lib().brmppi_solve(self._ctx))
+
+    def shift(self):
+        _check(lib().brmppi_shift(self._ctx))
+
+    def step(self):
+        u0 = np.zeros((self.n_scenes, 2), dtype=np.float32)
+        _check(lib().brmppi_step(self._ctx, _p(u0)))
+        return u0
+
+    def synchronize(self):
+        self.stream.synchronize()
+
+    # ---- outputs ------------------------------------------------------------------------
+    def get_controls(self, scene=0):
+        U = np.zeros((self.T, 2), dtype=np.float32)
+        _check(lib().brmppi_get_controls(self._ctx, scene, _p(U)))
+        return U
+
+    def get_state(self, scene=0):
+        x = np.zeros(4, dtype=np.float32)
+        _check(lib().brmppi_get_state(self._ctx, scene, _p(x)))
+        return x
+
+    def get_obstacles(self, scene=0):
+        n = C.c_int(0)
+        buf = np.zeros((max(self.max_obstacles, 1), 5), dtype=np.float32)
+        _check(lib().brmppi_get_obstacles(self._ctx, scene, C.byref(n), buf.ctypes.data_as(C.POINTER(Obstacle))))
+        return buf[:n.value].copy()
+
+    def get_costs(self, scene=0):
+        S = np.zeros(self.K, dtype=np.float32)
+        _check(lib().brmppi_get_costs(self._ctx, scene, _p(S)))
+        return S
+
+    def get_final_states(self, scene=0):
+        X = np.zeros((self.K, 4), dtype=np.float32)
+        _check(lib().brmppi_get_final_states(self._ctx, scene, _p(X)))
+        return X
+
+    def get_diag(self, scene=0):
+        d = Diag()
+        _check(lib().brmppi_get_diag(self._ctx, scene, C.byref(d)))
+        return dict(S_min=d.S_min, argmin=d.argmin, eta=d.eta, ess=d.ess, n=d.n, nonfinite=d.nonfinite)
+
+    def launch_count(self):
+        return int(lib().brmppi_launch_count(self._ctx))
+
+
+def debug_philox(seed, n, K, T, tag=0):
+    """Raw Philox words of the in-kernel generator: uint32 array [K][T][4]."""
+    import torch
+    out = torch.empty(K * T * 4, dtype=torch.int32, device="cuda")
+    st = torch.cuda.current_stream()
+    _check(lib().brmppi_debug_philox(C.c_void_p(st.cuda_stream), int(seed) & 0xFFFFFFFFFFFFFFFF, int(n),
+                                     int(K), int(T), int(tag), C.c_void_p(out.data_ptr())))
+    return out.cpu().numpy().view(np.uint32).reshape(K, T, 4)
+
+
+def debug_sample_controls(params, n, U_nominal=None, flags=0):
+    """Perturbed, clamped controls u[K][T][2] and alpha[K] exactly as the kernels draw them."""
+    import torch
+    cp = make_cparams(params, 1, 0, flags)
+    u = torch.empty(params.K * params.T * 2, dtype=torch.float32, device="cuda")
+    a = torch.empty(params.K, dtype=torch.float32, device="cuda")
+    st = torch.cuda.current_stream()
+    Un = None if U_nominal is None else _p(_f32(U_nominal, (params.T, 2)))
+    _check(lib().brmppi_debug_sample_controls(C.c_void_p(st.cuda_stream), C.byref(cp), int(n), Un,
+                                              C.c_void_p(u.data_ptr()), C.c_void_p(a.data_ptr())))
+    return u.cpu().numpy().reshape(params.K, params.T, 2), a.cpu().numpy()
+
+
+def measure_peaks():
+    import torch
+    out = np.zeros(8, dtype=np.float32)
+    st = torch.cuda.current_stream()
+    _check(lib().brmppi_measure_peaks(C.c_void_p(st.cuda_stream), _p(out)))
+    return dict(ffma=float(out[0]), alu=float(out[1]), mufu=float(out[2]), mix=float(out[3]),
+                imad_wide=float(out[4]), n_sms=int(out[5]), sm_mhz=float(out[6]),
+                ffma_globaltimer=float(out[7]))

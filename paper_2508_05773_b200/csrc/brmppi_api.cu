@@ -1,0 +1,615 @@
+// brmppi_api.cu -- host side of the C ABI declared in include/brmppi.h: validation, workspace
+// layout, launches, CUDA-graph capture.  Every step of the hot path runs in the kernels included
+// below; this file only marshals arguments and enqueues work.  There is no CPU fallback.
+#include <cuda_runtime.h>
+#include <math_constants.h>
+
+#include <cmath>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+
+#include "../../include/brmppi.h"
+#include "brmppi_device.cuh"
+#include "peaks.cuh"
+#include "rollout_thread.cuh"
+#include "rollout_tile.cuh"
+#include "rollout_tile_kernel.cuh"
+#include "update.cuh"
+
+using namespace brmppi;
+
+namespace {
+
+thread_local char g_errbuf[256];
+thread_local cudaError_t g_last_cuda = cudaSuccess;
+
+inline int cuda_fail(cudaError_t e) {
+  g_last_cuda = e;
+  return BRMPPI_ERR_CUDA;
+}
+#define CU(expr)                                         \
+  do {                                                   \
+    cudaError_t e__ = (expr);                            \
+    if (e__ != cudaSuccess) return cuda_fail(e__);       \
+  } while (0)
+
+inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+bool finite_all(const float* v, int n) {
+  for (int i = 0; i < n; ++i)
+    if (!std::isfinite(v[i])) return false;
+  return true;
+}
+
+bool params_valid(const brmppi_params* p) {
+  if (!p) return false;
+  if (p->K < 1 || p->K > (1 << 27)) return false;
+  if (p->T < 1 || p->T > BRMPPI_MAX_T) return false;
+  if (p->n_iter < 1 || p->n_scenes < 1 || p->n_scenes > 65535) return false;
+  if ((long long)p->K * p->n_scenes > 0x7fffffffLL) return false;
+  if (p->max_obstacles < 0 || p->max_obstacles > BRMPPI_MAX_OBSTACLES) return false;
+  if (p->n_discs < 1 || p->n_discs > BRMPPI_MAX_DISCS) return false;
+  for (int j = 0; j < p->n_discs; ++j) {
+    if (p->discs[j].body != 0 && p->discs[j].body != 1) return false;
+    if (!std::isfinite(p->discs[j].offset)) return false;
+  }
+  const float f[] = {p->disc_radius, p->dt, p->L1, p->L2, p->Lh, p->v_min, p->v_max, p->delta_min,
+                     p->delta_max, p->sigma_v, p->sigma_delta, p->alpha_lo, p->alpha_hi, p->w_pos,
+                     p->w_head, p->w_v, p->w_delta, p->w_hitch, p->hitch_max, p->w_bar, p->w_term,
+                     p->lambda};
+  if (!finite_all(f, (int)(sizeof(f) / sizeof(f[0])))) return false;
+  if (!(p->dt > 0.f) || !(p->L1 > 0.f) || !(p->L2 > 0.f) || !(p->lambda > 0.f)) return false;
+  if (p->disc_radius < 0.f || p->sigma_v < 0.f || p->sigma_delta < 0.f) return false;
+  if (p->v_min > p->v_max || p->delta_min > p->delta_max) return false;
+  if (p->delta_min <= -1.5f || p->delta_max >= 1.5f) return false;   // tan(delta) must stay finite
+  if (p->alpha_lo > p->alpha_hi) return false;
+  const unsigned known = BRMPPI_FLAG_WRITE_SAMPLES | BRMPPI_FLAG_PRECISE_MATH |
+                         BRMPPI_FLAG_KERNEL_THREAD_PER_SAMPLE;
+  if (p->flags & ~known) return false;
+  return true;
+}
+
+struct Layout {
+  size_t state, goal, n_obs, obstacles, U, counter, u0, part_m, part_argmin, part_eta, part_w2,
+      part_nf, part_A, diag, S, XT, total;
+};
+
+// Launch plan: which rollout kernel, how the sample axis is tiled, how many partials.
+struct Plan {
+  bool tile_kernel;
+  int n_partials;
+  TilePlan tile;
+};
+
+Plan make_plan(const brmppi_params& p) {
+  Plan pl{};
+  pl.tile_kernel = !(p.flags & BRMPPI_FLAG_KERNEL_THREAD_PER_SAMPLE);
+  if (pl.tile_kernel) {
+    pl.tile = make_tile_plan(p.K, p.T, p.n_scenes, p.max_obstacles);
+    pl.n_partials = pl.tile.blocks_per_scene;
+  } else {
+    pl.n_partials = (p.K + kThreadBlock - 1) / kThreadBlock;
+  }
+  return pl;
+}
+
+Layout make_layout(const brmppi_params& p, const Plan& pl) {
+  Layout L{};
+  size_t off = 0;
+  const size_t ns = (size_t)p.n_scenes, P = (size_t)pl.n_partials, T = (size_t)p.T;
+  auto take = [&](size_t bytes) { size_t o = off; off = align_up(off + bytes, 256); return o; };
+  L.state = take(ns * 16);
+  L.goal = take(ns * 16);
+  L.n_obs = take(ns * 4);
+  L.obstacles = take(ns * (size_t)(p.max_obstacles > 0 ? p.max_obstacles : 1) * 20);
+  L.U = take(ns * T * 8);
+  L.counter = take(4);
+  L.u0 = take(ns * 8);
+  L.part_m = take(ns * P * 8);
+  L.part_argmin = take(ns * P * 4);
+  L.part_eta = take(ns * P * 4);
+  L.part_w2 = take(ns * P * 4);
+  L.part_nf = take(ns * P * 4);
+  L.part_A = take(ns * 2 * T * P * 4);
+  L.diag = take(ns * sizeof(brmppi_diag));
+  if (p.flags & BRMPPI_FLAG_WRITE_SAMPLES) {
+    L.S = take(ns * (size_t)p.K * 4);
+    L.XT = take(ns * (size_t)p.K * 16);
+  }
+  L.total = off;
+  return L;
+}
+
+}  // namespace
+
+struct brmppi_ctx {
+  brmppi_params p;
+  DeviceParams d;
+  Plan plan;
+  Layout layout;
+  cudaStream_t stream;
+  unsigned char* state_set;
+  unsigned char* goal_set;
+  unsigned long long launches;
+  unsigned int n_host;          // host mirror of the device iteration counter
+  cudaGraphExec_t solve_graph, step_graph;
+  float* pinned_u0;             // [n_scenes][2] staging for brmppi_step
+  size_t smem_rollout, smem_update;
+};
+
+namespace {
+
+int enqueue_iteration(brmppi_ctx* c) {
+  const DeviceParams& d = c->d;
+  const bool precise = (c->p.flags & BRMPPI_FLAG_PRECISE_MATH) != 0;
+  if (c->plan.tile_kernel) {
+    CU(launch_rollout_tile(d, c->plan.tile, precise, c->smem_rollout, c->stream));
+  } else {
+    dim3 grid((unsigned)c->plan.n_partials, (unsigned)d.n_scenes);
+    if (precise)
+      rollout_thread_per_sample<true><<<grid, kThreadBlock, c->smem_rollout, c->stream>>>(d);
+    else
+      rollout_thread_per_sample<false><<<grid, kThreadBlock, c->smem_rollout, c->stream>>>(d);
+    CU(cudaGetLastError());
+  }
+  dim3 ugrid((unsigned)((2 * d.T + kUpdateOutputsPerBlock - 1) / kUpdateOutputsPerBlock),
+             (unsigned)d.n_scenes);
+  merge_update<<<ugrid, kUpdateBlock, c->smem_update, c->stream>>>(d);
+  CU(cudaGetLastError());
+  return BRMPPI_OK;
+}
+
+int enqueue_solve(brmppi_ctx* c) {
+  for (int it = 0; it < c->p.n_iter; ++it) {
+    int r = enqueue_iteration(c);
+    if (r) return r;
+  }
+  return BRMPPI_OK;
+}
+
+int ready(const brmppi_ctx* c) {
+  for (int s = 0; s < c->p.n_scenes; ++s)
+    if (!c->state_set[s] || !c->goal_set[s]) return BRMPPI_ERR_NOT_READY;
+  return BRMPPI_OK;
+}
+
+template <class F>
+int capture(brmppi_ctx* c, cudaGraphExec_t* exec, F&& body) {
+  cudaGraph_t graph = nullptr;
+  CU(cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeThreadLocal));
+  int r = body();
+  cudaError_t e = cudaStreamEndCapture(c->stream, &graph);
+  if (r) { if (graph) cudaGraphDestroy(graph); return r; }
+  if (e != cudaSuccess) return cuda_fail(e);
+  e = cudaGraphInstantiate(exec, graph, 0);
+  cudaGraphDestroy(graph);
+  if (e != cudaSuccess) return cuda_fail(e);
+  return BRMPPI_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+size_t brmppi_workspace_bytes(const brmppi_params* p) {
+  if (!params_valid(p)) return 0;
+  return make_layout(*p, make_plan(*p)).total;
+}
+
+int brmppi_create(const brmppi_params* p, void* dev_workspace, size_t workspace_bytes,
+                  void* cuda_stream, brmppi_ctx** out) {
+  if (!p || !dev_workspace || !out) return BRMPPI_ERR_NULL;
+  *out = nullptr;
+  if (!params_valid(p)) return BRMPPI_ERR_INVALID_ARG;
+  if ((uintptr_t)dev_workspace % 256 != 0) return BRMPPI_ERR_UNALIGNED;
+  int dev = 0;
+  CU(cudaGetDevice(&dev));
+  cudaDeviceProp prop;
+  CU(cudaGetDeviceProperties(&prop, dev));
+
+  brmppi_ctx* c = new (std::nothrow) brmppi_ctx();
+  if (!c) return BRMPPI_ERR_NULL;
+  c->p = *p;
+  c->plan = make_plan(*p);
+  c->layout = make_layout(*p, c->plan);
+  if (workspace_bytes < c->layout.total) { delete c; return BRMPPI_ERR_WORKSPACE_TOO_SMALL; }
+  c->stream = (cudaStream_t)cuda_stream;
+  c->state_set = (unsigned char*)calloc((size_t)p->n_scenes, 1);
+  c->goal_set = (unsigned char*)calloc((size_t)p->n_scenes, 1);
+  c->launches = 0;
+  c->n_host = 0;
+  c->solve_graph = nullptr;
+  c->step_graph = nullptr;
+  c->pinned_u0 = nullptr;
+
+  DeviceParams& d = c->d;
+  memset(&d, 0, sizeof(d));
+  d.K = p->K; d.T = p->T; d.n_scenes = p->n_scenes; d.max_obstacles = p->max_obstacles;
+  d.n_discs = p->n_discs;
+  for (int j = 0; j < p->n_discs; ++j) { d.disc_body[j] = p->discs[j].body; d.disc_offset[j] = p->discs[j].offset; }
+  d.disc_radius = p->disc_radius;
+  d.dt = p->dt; d.inv_L1 = 1.0f / p->L1; d.inv_L2 = 1.0f / p->L2; d.Lh = p->Lh;
+  d.Lh_over_L1 = p->Lh / p->L1; d.Lh_over_L2 = p->Lh / p->L2;
+  d.v_min = p->v_min; d.v_max = p->v_max; d.delta_min = p->delta_min; d.delta_max = p->delta_max;
+  d.sigma_v = p->sigma_v; d.sigma_delta = p->sigma_delta;
+  d.alpha_lo = p->alpha_lo; d.alpha_span = p->alpha_hi - p->alpha_lo;
+  d.w_pos = p->w_pos; d.w_head = p->w_head; d.w_v = p->w_v; d.w_delta = p->w_delta;
+  d.w_hitch = p->w_hitch; d.hitch_max = p->hitch_max; d.w_bar = p->w_bar; d.w_term = p->w_term;
+  d.inv_lambda = 1.0f / p->lambda;
+  d.key0 = (uint32_t)(p->seed & 0xFFFFFFFFull); d.key1 = (uint32_t)(p->seed >> 32);
+  d.flags = p->flags;
+  d.n_partials = c->plan.n_partials;
+  if (c->plan.tile_kernel) {
+    d.tiles_per_scene = c->plan.tile.tiles_per_scene;
+    d.chunks = c->plan.tile.chunks;
+    d.chunk_len = c->plan.tile.chunk_len;
+    d.t_stride = c->plan.tile.t_stride;
+    d.obs_padded = c->plan.tile.obs_padded;
+    const TileSmem ts = tile_smem_layout(d.T, d.obs_padded, d.chunks, d.t_stride);
+    d.off_obs = (int)ts.obs; d.off_vel = (int)ts.vel; d.off_xy = (int)ts.xy; d.off_unom = (int)ts.unom;
+    d.off_planes = (int)ts.planes; d.off_cost = (int)ts.cost; d.off_A = (int)ts.A; d.off_misc = (int)ts.misc;
+  }
+  unsigned char* base = (unsigned char*)dev_workspace;
+  const Layout& L = c->layout;
+  d.state = (float*)(base + L.state); d.goal = (float*)(base + L.goal);
+  d.n_obs = (int*)(base + L.n_obs); d.obstacles = (float*)(base + L.obstacles);
+  d.U = (float*)(base + L.U); d.counter = (uint32_t*)(base + L.counter);
+  d.u0_applied = (float*)(base + L.u0);
+  d.part_m = (double*)(base + L.part_m); d.part_argmin = (int*)(base + L.part_argmin);
+  d.part_eta = (float*)(base + L.part_eta); d.part_w2 = (float*)(base + L.part_w2);
+  d.part_nonfinite = (int*)(base + L.part_nf); d.part_A = (float*)(base + L.part_A);
+  d.diag = (brmppi_diag*)(base + L.diag);
+  if (p->flags & BRMPPI_FLAG_WRITE_SAMPLES) { d.S = (float*)(base + L.S); d.XT = (float*)(base + L.XT); }
+
+  c->smem_update = sizeof(float) * (size_t)c->plan.n_partials;
+  cudaError_t e = cudaSuccess;
+  if (c->plan.tile_kernel) {
+    c->smem_rollout = rollout_tile_smem_bytes(d, c->plan.tile);
+    e = configure_rollout_tile((p->flags & BRMPPI_FLAG_PRECISE_MATH) != 0, p->n_discs, c->smem_rollout);
+  } else {
+    c->smem_rollout = rollout_thread_smem_bytes(d);
+    if (c->smem_rollout > 48 * 1024) {
+      e = cudaFuncSetAttribute(rollout_thread_per_sample<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_rollout);
+      if (e == cudaSuccess)
+        e = cudaFuncSetAttribute(rollout_thread_per_sample<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_rollout);
+    }
+  }
+  if (e == cudaSuccess && c->smem_update > 48 * 1024)
+    e = cudaFuncSetAttribute(merge_update, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_update);
+  if (e == cudaSuccess && (c->smem_rollout > prop.sharedMemPerBlockOptin || c->smem_update > prop.sharedMemPerBlockOptin))
+    e = cudaErrorInvalidValue;
+  // zero: n_obs, U, counter, diag, u0 (state/goal stay unset until the caller provides them)
+  if (e == cudaSuccess) e = cudaMemsetAsync(base, 0, L.part_m, c->stream);
+  if (e == cudaSuccess) e = cudaMemsetAsync(base + L.diag, 0, (size_t)p->n_scenes * sizeof(brmppi_diag), c->stream);
+  if (e == cudaSuccess) e = cudaMallocHost((void**)&c->pinned_u0, sizeof(float) * 2 * (size_t)p->n_scenes);
+  if (e != cudaSuccess) {
+    free(c->state_set); free(c->goal_set);
+    delete c;
+    return cuda_fail(e);
+  }
+  *out = c;
+  return BRMPPI_OK;
+}
+
+int brmppi_destroy(brmppi_ctx* c) {
+  if (!c) return BRMPPI_ERR_NULL;
+  if (c->solve_graph) cudaGraphExecDestroy(c->solve_graph);
+  if (c->step_graph) cudaGraphExecDestroy(c->step_graph);
+  if (c->pinned_u0) cudaFreeHost(c->pinned_u0);
+  free(c->state_set);
+  free(c->goal_set);
+  delete c;
+  return BRMPPI_OK;
+}
+
+static int check_scene(const brmppi_ctx* c, int scene) {
+  if (!c) return BRMPPI_ERR_NULL;
+  if (scene < 0 || scene >= c->p.n_scenes) return BRMPPI_ERR_INVALID_ARG;
+  return BRMPPI_OK;
+}
+
+static float wrap_pi(float a) {
+  const double two_pi = 6.283185307179586476925286766559;
+  return (float)((double)a - two_pi * std::nearbyint((double)a / two_pi));
+}
+
+int brmppi_set_state(brmppi_ctx* c, int scene, const float x[4]) {
+  int r = check_scene(c, scene);
+  if (r) return r;
+  if (!x) return BRMPPI_ERR_NULL;
+  if (!finite_all(x, 4)) return BRMPPI_ERR_NONFINITE_INPUT;
+  const float v[4] = {x[0], x[1], wrap_pi(x[2]), wrap_pi(x[3])};
+  CU(cudaMemcpyAsync(c->d.state + 4 * scene, v, sizeof(v), cudaMemcpyHostToDevice, c->stream));
+  c->state_set[scene] = 1;
+  return BRMPPI_OK;
+}
+
+int brmppi_set_goal(brmppi_ctx* c, int scene, const float g[4]) {
+  int r = check_scene(c, scene);
+  if (r) return r;
+  if (!g) return BRMPPI_ERR_NULL;
+  if (!finite_all(g, 4)) return BRMPPI_ERR_NONFINITE_INPUT;
+  CU(cudaMemcpyAsync(c->d.goal + 4 * scene, g, 16, cudaMemcpyHostToDevice, c->stream));
+  c->goal_set[scene] = 1;
+  return BRMPPI_OK;
+}
+
+int brmppi_set_obstacles(brmppi_ctx* c, int scene, int n, const brmppi_obstacle* obs) {
+  int r = check_scene(c, scene);
+  if (r) return r;
+  if (n < 0) return BRMPPI_ERR_INVALID_ARG;
+  if (n > c->p.max_obstacles) return BRMPPI_ERR_TOO_MANY_OBSTACLES;
+  if (n > 0 && !obs) return BRMPPI_ERR_NULL;
+  for (int i = 0; i < n; ++i) {
+    if (!finite_all(&obs[i].cx, 5)) return BRMPPI_ERR_NONFINITE_INPUT;
+    if (!(obs[i].radius > 0.f)) return BRMPPI_ERR_INVALID_ARG;
+  }
+  if (n > 0)
+    CU(cudaMemcpyAsync(c->d.obstacles + (size_t)scene * c->p.max_obstacles * 5, obs,
+                       sizeof(brmppi_obstacle) * (size_t)n, cudaMemcpyHostToDevice, c->stream));
+  CU(cudaMemcpyAsync(c->d.n_obs + scene, &n, sizeof(int), cudaMemcpyHostToDevice, c->stream));
+  return BRMPPI_OK;
+}
+
+int brmppi_set_nominal(brmppi_ctx* c, int scene, const float* U) {
+  int r = check_scene(c, scene);
+  if (r) return r;
+  float* dst = c->d.U + (size_t)scene * c->p.T * 2;
+  const size_t bytes = sizeof(float) * 2 * (size_t)c->p.T;
+  if (!U) { CU(cudaMemsetAsync(dst, 0, bytes, c->stream)); return BRMPPI_OK; }
+  if (!finite_all(U, 2 * c->p.T)) return BRMPPI_ERR_NONFINITE_INPUT;
+  for (int t = 0; t < c->p.T; ++t) {
+    if (U[2 * t] < c->p.v_min || U[2 * t] > c->p.v_max) return BRMPPI_ERR_INVALID_ARG;
+    if (U[2 * t + 1] < c->p.delta_min || U[2 * t + 1] > c->p.delta_max) return BRMPPI_ERR_INVALID_ARG;
+  }
+  CU(cudaMemcpyAsync(dst, U, bytes, cudaMemcpyHostToDevice, c->stream));
+  return BRMPPI_OK;
+}
+
+int brmppi_set_counter(brmppi_ctx* c, unsigned int n) {
+  if (!c) return BRMPPI_ERR_NULL;
+  CU(cudaMemcpyAsync(c->d.counter, &n, sizeof(n), cudaMemcpyHostToDevice, c->stream));
+  c->n_host = n;
+  return BRMPPI_OK;
+}
+
+int brmppi_reset(brmppi_ctx* c) {
+  if (!c) return BRMPPI_ERR_NULL;
+  CU(cudaMemsetAsync(c->d.U, 0, sizeof(float) * 2 * (size_t)c->p.T * (size_t)c->p.n_scenes, c->stream));
+  return brmppi_set_counter(c, 0u);
+}
+
+int brmppi_solve(brmppi_ctx* c) {
+  if (!c) return BRMPPI_ERR_NULL;
+  int r = ready(c);
+  if (r) return r;
+  if (c->stream == nullptr) {           // the legacy default stream cannot be captured
+    r = enqueue_solve(c);
+    if (r) return r;
+  } else {
+    if (!c->solve_graph) {
+      r = capture(c, &c->solve_graph, [&] { return enqueue_solve(c); });
+      if (r) return r;
+    }
+    CU(cudaGraphLaunch(c->solve_graph, c->stream));
+  }
+  c->launches += 2ull * (unsigned)c->p.n_iter;
+  c->n_host += (unsigned)c->p.n_iter;
+  return BRMPPI_OK;
+}
+
+int brmppi_shift(brmppi_ctx* c) {
+  if (!c) return BRMPPI_ERR_NULL;
+  shift_plant<false><<<(unsigned)c->p.n_scenes, kShiftBlock, 0, c->stream>>>(c->d);
+  CU(cudaGetLastError());
+  c->launches += 1;
+  return BRMPPI_OK;
+}
+
+int brmppi_step(brmppi_ctx* c, float* u0_out) {
+  if (!c) return BRMPPI_ERR_NULL;
+  int r = ready(c);
+  if (r) return r;
+  if (c->stream == nullptr) return BRMPPI_ERR_INVALID_ARG;   // graph replay needs a real stream
+  if (!c->step_graph) {
+    r = capture(c, &c->step_graph, [&] {
+      int rr = enqueue_solve(c);
+      if (rr) return rr;
+      shift_plant<true><<<(unsigned)c->p.n_scenes, kShiftBlock, 0, c->stream>>>(c->d);
+      CU(cudaGetLastError());
+      CU(cudaMemcpyAsync(c->pinned_u0, c->d.u0_applied, sizeof(float) * 2 * (size_t)c->p.n_scenes,
+                         cudaMemcpyDeviceToHost, c->stream));
+      return (int)BRMPPI_OK;
+    });
+    if (r) return r;
+  }
+  CU(cudaGraphLaunch(c->step_graph, c->stream));
+  c->launches += 2ull * (unsigned)c->p.n_iter + 1ull;
+  c->n_host += (unsigned)c->p.n_iter;
+  CU(cudaStreamSynchronize(c->stream));
+  if (u0_out) memcpy(u0_out, c->pinned_u0, sizeof(float) * 2 * (size_t)c->p.n_scenes);
+  return BRMPPI_OK;
+}
+
+static int d2h(brmppi_ctx* c, void* dst, const void* src, size_t bytes) {
+  CU(cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDeviceToHost, c->stream));
+  CU(cudaStreamSynchronize(c->stream));
+  return BRMPPI_OK;
+}
+
+int brmppi_get_controls(brmppi_ctx* c, int scene, float* U_out) {
+  int r = check_scene(c, scene);
+  if (r) return r;
+  if (!U_out) return BRMPPI_ERR_NULL;
+  return d2h(c, U_out, c->d.U + (size_t)scene * c->p.T * 2, sizeof(float) * 2 * (size_t)c->p.T);
+}
+
+int brmppi_get_state(brmppi_ctx* c, int scene, float x_out[4]) {
+  int r = check_scene(c, scene);
+  if (r) return r;
+  if (!x_out) return BRMPPI_ERR_NULL;
+  return d2h(c, x_out, c->d.state + 4 * scene, 16);
+}
+
+int brmppi_get_obstacles(brmppi_ctx* c, int scene, int* n_out, brmppi_obstacle* out) {
+  int r = check_scene(c, scene);
+  if (r) return r;
+  if (!n_out) return BRMPPI_ERR_NULL;
+  r = d2h(c, n_out, c->d.n_obs + scene, sizeof(int));
+  if (r) return r;
+  if (out && *n_out > 0)
+    return d2h(c, out, c->d.obstacles + (size_t)scene * c->p.max_obstacles * 5,
+               sizeof(brmppi_obstacle) * (size_t)*n_out);
+  return BRMPPI_OK;
+}
+
+int brmppi_get_costs(brmppi_ctx* c, int scene, float* S_out) {
+  int r = check_scene(c, scene);
+  if (r) return r;
+  if (!S_out) return BRMPPI_ERR_NULL;
+  if (!(c->p.flags & BRMPPI_FLAG_WRITE_SAMPLES)) return BRMPPI_ERR_NOT_READY;
+  return d2h(c, S_out, c->d.S + (size_t)scene * c->p.K, sizeof(float) * (size_t)c->p.K);
+}
+
+int brmppi_get_final_states(brmppi_ctx* c, int scene, float* X_out) {
+  int r = check_scene(c, scene);
+  if (r) return r;
+  if (!X_out) return BRMPPI_ERR_NULL;
+  if (!(c->p.flags & BRMPPI_FLAG_WRITE_SAMPLES)) return BRMPPI_ERR_NOT_READY;
+  return d2h(c, X_out, c->d.XT + (size_t)scene * c->p.K * 4, sizeof(float) * 4 * (size_t)c->p.K);
+}
+
+int brmppi_get_diag(brmppi_ctx* c, int scene, brmppi_diag* out) {
+  int r = check_scene(c, scene);
+  if (r) return r;
+  if (!out) return BRMPPI_ERR_NULL;
+  r = d2h(c, out, c->d.diag + scene, sizeof(brmppi_diag));
+  out->n = c->n_host;
+  return r;
+}
+
+unsigned long long brmppi_launch_count(const brmppi_ctx* c) { return c ? c->launches : 0ull; }
+
+const char* brmppi_strerror(int status) {
+  switch (status) {
+    case BRMPPI_OK: return "ok";
+    case BRMPPI_ERR_NULL: return "null pointer";
+    case BRMPPI_ERR_INVALID_ARG: return "invalid argument";
+    case BRMPPI_ERR_WORKSPACE_TOO_SMALL: return "workspace too small";
+    case BRMPPI_ERR_TOO_MANY_OBSTACLES: return "too many obstacles";
+    case BRMPPI_ERR_NONFINITE_INPUT: return "non-finite input";
+    case BRMPPI_ERR_NOT_READY: return "not ready (state/goal unset, or sample outputs not enabled)";
+    case BRMPPI_ERR_UNALIGNED: return "workspace not 256-byte aligned";
+    case BRMPPI_ERR_CUDA:
+      snprintf(g_errbuf, sizeof(g_errbuf), "CUDA error: %s", cudaGetErrorString(g_last_cuda));
+      return g_errbuf;
+    default: return "unknown status";
+  }
+}
+
+int brmppi_debug_philox(void* cuda_stream, unsigned long long seed, unsigned int n, int K, int T,
+                        unsigned int tag, unsigned int* dev_out) {
+  if (!dev_out) return BRMPPI_ERR_NULL;
+  if (K < 1 || T < 1) return BRMPPI_ERR_INVALID_ARG;
+  cudaStream_t s = (cudaStream_t)cuda_stream;
+  const size_t total = (size_t)K * T;
+  debug_philox<<<(unsigned)((total + 255) / 256), 256, 0, s>>>(
+      (uint32_t)(seed & 0xFFFFFFFFull), (uint32_t)(seed >> 32), n, K, T, tag, (uint4*)dev_out);
+  CU(cudaGetLastError());
+  CU(cudaStreamSynchronize(s));
+  return BRMPPI_OK;
+}
+
+int brmppi_debug_sample_controls(void* cuda_stream, const brmppi_params* p, unsigned int n,
+                                 const float* U_nominal, float* dev_u, float* dev_alpha) {
+  if (!p) return BRMPPI_ERR_NULL;
+  if (!params_valid(p)) return BRMPPI_ERR_INVALID_ARG;
+  cudaStream_t s = (cudaStream_t)cuda_stream;
+  DeviceParams d;
+  memset(&d, 0, sizeof(d));
+  d.K = p->K; d.T = p->T;
+  d.v_min = p->v_min; d.v_max = p->v_max; d.delta_min = p->delta_min; d.delta_max = p->delta_max;
+  d.sigma_v = p->sigma_v; d.sigma_delta = p->sigma_delta;
+  d.alpha_lo = p->alpha_lo; d.alpha_span = p->alpha_hi - p->alpha_lo;
+  d.key0 = (uint32_t)(p->seed & 0xFFFFFFFFull); d.key1 = (uint32_t)(p->seed >> 32);
+  float2* dU = nullptr;
+  CU(cudaMalloc((void**)&dU, sizeof(float2) * (size_t)p->T));   // debug-only scratch
+  cudaError_t e = U_nominal ? cudaMemcpyAsync(dU, U_nominal, sizeof(float2) * (size_t)p->T, cudaMemcpyHostToDevice, s)
+                            : cudaMemsetAsync(dU, 0, sizeof(float2) * (size_t)p->T, s);
+  if (e == cudaSuccess) {
+    const size_t total = (size_t)p->K * p->T;
+    const unsigned grid = (unsigned)((total + 255) / 256);
+    if (p->flags & BRMPPI_FLAG_PRECISE_MATH)
+      debug_sample_controls<true><<<grid, 256, 0, s>>>(d, n, dU, (float2*)dev_u, dev_alpha);
+    else
+      debug_sample_controls<false><<<grid, 256, 0, s>>>(d, n, dU, (float2*)dev_u, dev_alpha);
+    e = cudaGetLastError();
+  }
+  if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+  cudaFree(dU);
+  if (e != cudaSuccess) return cuda_fail(e);
+  return BRMPPI_OK;
+}
+
+int brmppi_measure_peaks(void* cuda_stream, float out[8]) {
+  if (!out) return BRMPPI_ERR_NULL;
+  cudaStream_t s = (cudaStream_t)cuda_stream;
+  int dev = 0;
+  CU(cudaGetDevice(&dev));
+  cudaDeviceProp prop;
+  CU(cudaGetDeviceProperties(&prop, dev));
+  const int blocks = prop.multiProcessorCount * 4;   // 4 x 256 threads resident per SM, one wave
+  long long* spans = nullptr;
+  float* sink = nullptr;
+  CU(cudaMalloc((void**)&spans, sizeof(long long) * 3 * (size_t)blocks));
+  CU(cudaMalloc((void**)&sink, sizeof(float) * 4));
+  long long* h = (long long*)malloc(sizeof(long long) * 3 * (size_t)blocks);
+  double wall_ns[5] = {0, 0, 0, 0, 0};
+  cudaError_t e = cudaSuccess;
+  for (int kind = 0; kind < 5 && e == cudaSuccess; ++kind) {
+    for (int rep = 0; rep < 3 && e == cudaSuccess; ++rep) {   // last repetition is the one kept
+      switch (kind) {
+        case PEAK_FFMA: peak_kernel<PEAK_FFMA><<<blocks, 256, 0, s>>>(1.0f, spans, sink); break;
+        case PEAK_ALU: peak_kernel<PEAK_ALU><<<blocks, 256, 0, s>>>(1.0f, spans, sink); break;
+        case PEAK_MUFU: peak_kernel<PEAK_MUFU><<<blocks, 256, 0, s>>>(1.0f, spans, sink); break;
+        case PEAK_MIX: peak_kernel<PEAK_MIX><<<blocks, 256, 0, s>>>(1.0f, spans, sink); break;
+        default: peak_kernel<PEAK_IMAD_WIDE><<<blocks, 256, 0, s>>>(1.0f, spans, sink); break;
+      }
+      e = cudaGetLastError();
+    }
+    if (e == cudaSuccess) e = cudaMemcpyAsync(h, spans, sizeof(long long) * 3 * (size_t)blocks, cudaMemcpyDeviceToHost, s);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+    if (e != cudaSuccess) break;
+    long long mx = 0, gmin = h[1], gmax = h[2];
+    for (int b = 0; b < blocks; ++b) {
+      mx = h[3 * b] > mx ? h[3 * b] : mx;
+      gmin = h[3 * b + 1] < gmin ? h[3 * b + 1] : gmin;
+      gmax = h[3 * b + 2] > gmax ? h[3 * b + 2] : gmax;
+    }
+    wall_ns[kind] = (double)(gmax - gmin);
+    const double per_thread = (double)kPeakIters * kPeakReps * kPeakChains * (kind == PEAK_MIX ? 2.0 : 1.0);
+    out[kind] = (float)(per_thread * 1024.0 / (double)mx);   // thread-instr / clk / SM
+  }
+  if (e == cudaSuccess) {
+    clock_rate_kernel<<<1, 1, 0, s>>>(sink);
+    e = cudaGetLastError();
+    float mhz[2] = {0, 0};
+    if (e == cudaSuccess) e = cudaMemcpyAsync(mhz, sink, sizeof(float) * 2, cudaMemcpyDeviceToHost, s);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+    out[5] = (float)prop.multiProcessorCount;
+    out[6] = mhz[0];
+    // cross-check of the FFMA rate on the nanosecond globaltimer (first block start to last
+    // block end), converted with the measured clock
+    out[7] = (float)((double)kPeakIters * kPeakReps * kPeakChains * 1024.0 /
+                     (wall_ns[PEAK_FFMA] * 1e-3 * (double)mhz[0]));
+  }
+  free(h);
+  cudaFree(spans);
+  cudaFree(sink);
+  if (e != cudaSuccess) return cuda_fail(e);
+  return BRMPPI_OK;
+}
+
+}  // extern "C"

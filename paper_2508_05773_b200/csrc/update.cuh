@@ -1,0 +1,157 @@
+// update.cuh -- grid-level merge of the per-block online-softmax partials and the nominal update
+// (DESIGN.md §2 rows a7/a8), warm-start shift and plant step (a9), and the debug kernels behind
+// brmppi_debug_*.
+//
+// Merge of partials (m_p, eta_p, A_p[2T]) in partial-index order (deterministic, SURVEY §7 hard
+// part 6):   m = min_p m_p;  c_p = exp(-(m_p - m)/lambda);  eta = sum_p c_p eta_p;
+//            U[o] = sum_p c_p A_p[o] / eta                          (eq. 5)
+#pragma once
+
+#include "brmppi_device.cuh"
+
+namespace brmppi {
+
+constexpr int kUpdateBlock = 256;
+constexpr int kUpdateOutputsPerBlock = kUpdateBlock / 32;   // one warp per output channel
+
+__global__ void __launch_bounds__(kUpdateBlock)
+merge_update(const __grid_constant__ DeviceParams P) {
+  extern __shared__ float sScale[];                 // [n_partials]
+  __shared__ double sM[kUpdateBlock / 32];
+  __shared__ int sI[kUpdateBlock / 32];
+  const int scene = blockIdx.y;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int Pn = P.n_partials;
+  const double* pm = P.part_m + (size_t)scene * Pn;
+  const int* pi = P.part_argmin + (size_t)scene * Pn;
+
+  // global minimum and its sample index (lowest index on ties)
+  double m = CUDART_INF;
+  int idx = 0x7fffffff;
+  for (int p = tid; p < Pn; p += kUpdateBlock) {
+    const double om = pm[p];
+    const int oi = pi[p];
+    if (om < m || (om == m && oi < idx)) { m = om; idx = oi; }
+  }
+  warp_argmin(m, idx);
+  if (lane == 0) { sM[warp] = m; sI[warp] = idx; }
+  __syncthreads();
+  m = sM[0]; idx = sI[0];
+#pragma unroll
+  for (int w = 1; w < kUpdateBlock / 32; ++w)
+    if (sM[w] < m || (sM[w] == m && sI[w] < idx)) { m = sM[w]; idx = sI[w]; }
+  const bool any_finite = m < CUDART_INF;
+
+  for (int p = tid; p < Pn; p += kUpdateBlock) {
+    const double mp = pm[p];
+    sScale[p] = (any_finite && mp < CUDART_INF) ? expf((float)(-(mp - m) * (double)P.inv_lambda)) : 0.0f;
+  }
+  __syncthreads();
+
+  // one warp per output channel o = 2 t + c; lanes stride over partials (coalesced rows)
+  const int o = blockIdx.x * kUpdateOutputsPerBlock + warp;
+  const float* peta = P.part_eta + (size_t)scene * Pn;
+  float eta = 0.0f, acc = 0.0f;
+  if (o < 2 * P.T) {
+    const float* pa = P.part_A + ((size_t)scene * 2 * P.T + o) * Pn;
+    for (int p = lane; p < Pn; p += 32) {
+      const float c = sScale[p];
+      eta = fmaf(c, peta[p], eta);
+      acc = fmaf(c, pa[p], acc);
+    }
+  } else {
+    for (int p = lane; p < Pn; p += 32) eta = fmaf(sScale[p], peta[p], eta);
+  }
+  eta = warp_sum(eta);
+  acc = warp_sum(acc);
+  if (o < 2 * P.T && lane == 0 && any_finite && eta > 0.0f) P.U[(size_t)scene * 2 * P.T + o] = acc / eta;
+
+  if (blockIdx.x == 0 && warp == 0) {
+    float w2 = 0.0f, nf = 0.0f;
+    const float* pw2 = P.part_w2 + (size_t)scene * Pn;
+    const int* pnf = P.part_nonfinite + (size_t)scene * Pn;
+    for (int p = lane; p < Pn; p += 32) {
+      const float c = sScale[p];
+      w2 = fmaf(c * c, pw2[p], w2);
+      nf += (float)pnf[p];
+    }
+    w2 = warp_sum(w2);
+    nf = warp_sum(nf);
+    if (lane == 0) {
+      brmppi_diag d;
+      d.S_min = any_finite ? (float)m : CUDART_INF_F;
+      d.argmin = any_finite ? idx : -1;
+      d.eta = eta;
+      d.ess = w2 > 0.0f ? eta * eta / w2 : 0.0f;
+      d.n = 0ull;                       // filled in by the host, which tracks the counter
+      d.nonfinite = (int)nf;
+      P.diag[scene] = d;
+      // the rollout kernels of this iteration have all finished (kernel boundary); the next
+      // iteration draws fresh noise (reading 7).  Only this one thread touches the counter.
+      if (scene == 0) *P.counter = *P.counter + 1u;
+    }
+  }
+}
+
+// Warm-start shift (reading 4) and, when PLANT, the kinematic plant step with the
+// first control and constant-velocity obstacle advance (DESIGN.md §2 row a9).  One block per
+// scene.  The plant step always uses libdevice sincosf/tanf: it runs once per control step.
+constexpr int kShiftBlock = 128;
+constexpr int kShiftMaxPerThread = (BRMPPI_MAX_T + kShiftBlock - 1) / kShiftBlock;
+
+template <bool PLANT>
+__global__ void __launch_bounds__(kShiftBlock) shift_plant(const __grid_constant__ DeviceParams P) {
+  const int scene = blockIdx.x, tid = threadIdx.x, T = P.T;
+  float2* U = reinterpret_cast<float2*>(P.U) + (size_t)scene * T;
+  if (PLANT) {
+    if (tid == 0) {
+      const float2 u0 = U[0];
+      float4 x = reinterpret_cast<float4*>(P.state)[scene];
+      float s1, c1, s2, c2;
+      sincosf(x.z, &s1, &c1);
+      sincosf(x.w, &s2, &c2);
+      const State N = kinematic_step(P, State{x.x, x.y, x.z, x.w}, s1, c1, s2, c2, u0.x, tanf(u0.y));
+      reinterpret_cast<float4*>(P.state)[scene] = make_float4(N.x, N.y, wrap_angle(N.psi1), wrap_angle(N.psi2));
+      reinterpret_cast<float2*>(P.u0_applied)[scene] = u0;
+    }
+    const int n_obs = P.n_obs[scene];
+    for (int i = tid; i < n_obs; i += kShiftBlock) {
+      float* ob = P.obstacles + ((size_t)scene * P.max_obstacles + i) * 5;
+      ob[0] = fmaf(P.dt, ob[3], ob[0]);
+      ob[1] = fmaf(P.dt, ob[4], ob[1]);
+    }
+  }
+  float2 next[kShiftMaxPerThread];
+#pragma unroll
+  for (int r = 0; r < kShiftMaxPerThread; ++r) {
+    const int t = tid + r * kShiftBlock;
+    if (t + 1 < T) next[r] = U[t + 1];
+  }
+  __syncthreads();
+#pragma unroll
+  for (int r = 0; r < kShiftMaxPerThread; ++r) {
+    const int t = tid + r * kShiftBlock;
+    if (t + 1 < T) U[t] = next[r];
+  }
+}
+
+// ---- debug kernels (brmppi_debug_*) ----------------------------------------------------------
+__global__ void debug_philox(uint32_t key0, uint32_t key1, uint32_t n, int K, int T, uint32_t tag,
+                             uint4* out) {
+  const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= (size_t)K * T) return;
+  const uint32_t k = (uint32_t)(i / T), t = (uint32_t)(i % T);
+  out[i] = philox4x32_10(t, n, k, tag, key0, key1);
+}
+
+template <bool PRECISE>
+__global__ void debug_sample_controls(const __grid_constant__ DeviceParams P, uint32_t n,
+                                      const float2* U_nom, float2* u_out, float* alpha_out) {
+  const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= (size_t)P.K * P.T) return;
+  const uint32_t k = (uint32_t)(i / P.T), t = (uint32_t)(i % P.T);
+  if (u_out) u_out[i] = sample_control<PRECISE>(P, U_nom[t], t, n, k, P.key0, P.key1);
+  if (alpha_out && t == 0) alpha_out[k] = sample_alpha(P, n, k, P.key0, P.key1);
+}
+
+}  // namespace brmppi

@@ -1,0 +1,373 @@
+"""Parity of the CUDA path (through the C ABI) against the CPU oracle on the same seeded inputs.
+
+Tolerances (north_star; reading 22): Philox integers and the argmin index bit-exact;
+final states, costs and controls within 1e-4 relative, i.e. |a-b| <= 1e-4 max(|b|, floor) with
+floor = 1 (m, rad) for x_T and S_k, and v_max / delta_max for the two control channels.  The
+argmin index is required to match only when the oracle's gap S_(2) - S_(1) exceeds
+1e-3 max(1, |S_(1)|) (reading 21)."""
+import numpy as np
+import pytest
+
+import scenes
+
+pytestmark = pytest.mark.gpu
+
+RTOL = 1e-4
+
+
+@pytest.fixture(scope="module")
+def B():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("GPU tests need a CUDA device; there is no CPU fallback")
+    from paper_2508_05773_b200 import brmppi
+    brmppi.lib()
+    return brmppi
+
+
+def close(a, b, floor):
+    a, b = np.asarray(a, dtype=np.float64), np.asarray(b, dtype=np.float64)
+    return np.abs(a - b) <= RTOL * np.maximum(np.abs(b), floor)
+
+
+def gpu_solve(B, sc, p, flags=0, n0=0, U0=None, max_obstacles=None):
+    n_obs = len(sc.obstacles)
+    mo = max_obstacles if max_obstacles is not None else max(n_obs, 1)
+    s = B.Solver(p, 1, mo, flags | B.FLAG_WRITE_SAMPLES)
+    s.set_scene(sc)
+    s.set_nominal(U0)
+    s.set_counter(n0)
+    s.solve()
+    out = dict(U=s.get_controls(), S=s.get_costs(), XT=s.get_final_states(), diag=s.get_diag())
+    s.close()
+    return out
+
+
+def check_against_oracle(O, got, sc, p, n0=0, U0=None, n_threads=8):
+    U = np.zeros((p.T, 2)) if U0 is None else np.asarray(U0, dtype=np.float64)
+    ref = O.solve(p, n0, sc.x0, sc.goal, sc.obstacles, U, n_threads=n_threads)[-1]
+    okS = close(got["S"], ref["S"], 1.0)
+    assert okS.all(), f"S_k: {np.count_nonzero(~okS)} of {p.K} off, worst {np.abs(got['S'] - ref['S']).max()}"
+    okX = close(got["XT"], ref["XT"], 1.0)
+    assert okX.all(), f"x_T worst {np.abs(got['XT'] - ref['XT']).max()}"
+    floors = np.array([p.v_max, p.delta_max])
+    okU = close(got["U"], ref["U"], floors[None, :])
+    err = np.abs(got["U"] - ref["U"]) / (RTOL * np.maximum(np.abs(ref["U"]), floors[None, :]))
+    assert okU.all(), f"U worst error = {err.max():.2f} x tolerance"
+    d = got["diag"]
+    if ref["gap"] > 1e-3 * max(1.0, abs(ref["S"].min())):
+        assert d["argmin"] == ref["argmin"]
+    assert close(d["S_min"], ref["S"].min(), 1.0)
+    assert abs(d["eta"] - ref["eta"]) <= 2e-3 * ref["eta"]
+    assert d["nonfinite"] == 0 and d["n"] == n0 + p.n_iter
+    return dict(ref=ref, u_err=float(err.max()))
+
+
+KERNELS = [pytest.param(0, id="tile"), pytest.param(4, id="thread")]
+
+
+# ------------------------------------------------------------------------------------------
+# Philox integers and drawn controls
+# ------------------------------------------------------------------------------------------
+def test_philox_bit_exact(B, O):
+    rng = np.random.default_rng(0)
+    for seed, n, tag in [(0, 0, 0), (0, 0, 1), (2**63 + 12345, 7, 0), (0xFFFFFFFFFFFFFFFF, 0xFFFFFFFF, 1),
+                         (int(rng.integers(0, 2**62)), int(rng.integers(0, 2**31)), 0)]:
+        K, T = 67, 33
+        w = B.debug_philox(seed, n, K, T, tag)
+        key = (seed & 0xFFFFFFFF, seed >> 32)
+        for k, t in [(0, 0), (5, 3), (66, 32), (17, 0), (0, 31)] + [tuple(x) for x in rng.integers(0, 33, size=(20, 2))]:
+            assert tuple(int(x) for x in w[k, t]) == O.philox((t, n, k, tag), key)
+
+
+def test_philox_matches_curand_layout(B):
+    """Second, stateful library pin: the counter layout (t, n, k, tag) is cuRAND's Philox state
+    layout, so torch's CUDA generator is not needed -- compare against the KAT directly."""
+    w = B.debug_philox(0, 0, 1, 1, 0)
+    assert [int(x) for x in w[0, 0]] == [0x6627e8d5, 0xe169c58d, 0xbc57ac4c, 0x9b00dbd8]
+
+
+@pytest.mark.parametrize("flags", [0, 2], ids=["fast", "precise"])
+def test_sampled_controls_match_oracle(B, O, flags):
+    p = scenes.default_params(K=300, T=40, seed=99)
+    U0 = np.tile([0.5, -0.1], (40, 1)).astype(np.float32)
+    u, a = B.debug_sample_controls(p, 3, U0, flags)
+    ref = O.iteration(p, 3, np.zeros(4), np.zeros(4), np.zeros((0, 5)), U0, want_samples=True)["u"]
+    floors = np.array([p.v_max, p.delta_max])
+    tol = 2e-6 if flags else 1e-5          # absolute, well inside the 1e-4 relative budget
+    assert np.abs(u - ref).max() <= tol
+    assert close(u, ref, floors).all()
+    a_ref = np.array([O.alpha(p, 3, k) for k in range(p.K)])
+    assert np.abs(a - a_ref).max() <= 1e-6
+    # clamping produces exact bound values on both sides at the same places
+    assert np.array_equal(u[..., 0] == p.v_max, ref[..., 0] == p.v_max)
+
+
+# ------------------------------------------------------------------------------------------
+# BASELINE.json configs
+# ------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("kernel", KERNELS)
+@pytest.mark.parametrize("precise", [0, 2], ids=["fast", "precise"])
+def test_cfg0(B, O, kernel, precise):
+    sc = scenes.scene_cfg0(0)
+    got = gpu_solve(B, sc, sc.params, kernel | precise)
+    check_against_oracle(O, got, sc, sc.params)
+
+
+@pytest.mark.parametrize("kernel", KERNELS)
+@pytest.mark.parametrize("seed", [0, 1, 2])
+def test_cfg1(B, O, kernel, seed):
+    sc = scenes.scene_cfg1(seed)
+    got = gpu_solve(B, sc, sc.params, kernel)
+    check_against_oracle(O, got, sc, sc.params)
+
+
+@pytest.mark.parametrize("kernel", KERNELS)
+def test_cfg2_three_iterations_moving_obstacles(B, O, kernel):
+    sc = scenes.scene_cfg2(0)
+    got = gpu_solve(B, sc, sc.params, kernel)
+    check_against_oracle(O, got, sc, sc.params)
+
+
+def test_cfg2_warm_nominal_and_counter(B, O):
+    sc = scenes.scene_cfg2(1)
+    p = sc.params.with_(K=4096, n_iter=2)
+    rng = np.random.default_rng(5)
+    U0 = np.stack([rng.uniform(-1.5, 1.5, p.T), rng.uniform(-0.4, 0.4, p.T)], axis=1).astype(np.float32)
+    got = gpu_solve(B, sc, p, 0, n0=1000, U0=U0)
+    check_against_oracle(O, got, sc, p, n0=1000, U0=U0)
+
+
+# ------------------------------------------------------------------------------------------
+# edge cases: ragged tiles, tiny horizons, obstacle counts, geometry variants
+# ------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("kernel", KERNELS)
+@pytest.mark.parametrize("K,T", [(1, 1), (1, 30), (17, 7), (129, 13), (1000, 50), (2049, 100), (333, 61)])
+def test_ragged_sizes(B, O, kernel, K, T):
+    sc = scenes.scene_static(3, 8, K=K, T=T)
+    got = gpu_solve(B, sc, sc.params, kernel)
+    check_against_oracle(O, got, sc, sc.params)
+
+
+@pytest.mark.parametrize("kernel", KERNELS)
+@pytest.mark.parametrize("n_obs", [0, 1, 7, 9, 32, 64])
+def test_obstacle_counts(B, O, kernel, n_obs):
+    sc = scenes.scene_static(4, n_obs, K=512, T=50)
+    got = gpu_solve(B, sc, sc.params, kernel, max_obstacles=64 if n_obs else 0)
+    check_against_oracle(O, got, sc, sc.params)
+
+
+@pytest.mark.parametrize("kernel", KERNELS)
+def test_geometry_variants(B, O, kernel):
+    sc = scenes.scene_cfg2(2)
+    # off-axle hitch, four discs, asymmetric bounds, other temperature
+    p = sc.params.with_(K=1024, T=40, n_iter=1, Lh=1.15, L1=3.23, L2=2.9,
+                        discs=((0, 1.5), (0, -0.5), (1, -1.0), (1, -2.5)), disc_radius=1.1,
+                        v_min=-1.0, v_max=2.5, delta_min=-0.5, delta_max=0.7, lam=5.0, dt=0.04)
+    got = gpu_solve(B, sc, p, kernel)
+    check_against_oracle(O, got, sc, p)
+    # one disc, vehicle starting inside an obstacle's inflated disc (h < 0 path)
+    p1 = sc.params.with_(K=512, T=20, n_iter=1, discs=((0, 0.0),))
+    sc1 = scenes.Scene(sc.x0, sc.goal, np.vstack([sc.obstacles, [[sc.x0[0] + 1.0, sc.x0[1], 1.0, 0.0, 0.0]]]).astype(np.float32).astype(np.float64), p1)
+    got = gpu_solve(B, sc1, p1, kernel)
+    check_against_oracle(O, got, sc1, p1)
+
+
+@pytest.mark.parametrize("kernel", KERNELS)
+def test_degenerate_noise_and_temperature(B, O, kernel):
+    sc = scenes.scene_cfg1(5)
+    U0 = np.tile([0.75, 0.125], (sc.params.T, 1)).astype(np.float32)
+    # sigma = 0: all samples identical, U is a fixed point of the update (bit-exact)
+    p = sc.params.with_(K=256, sigma_v=0.0, sigma_delta=0.0)
+    got = gpu_solve(B, sc, p, kernel, U0=U0)
+    assert np.array_equal(got["U"], U0)
+    assert np.all(got["S"] == got["S"][0])
+    assert got["diag"]["eta"] == pytest.approx(256.0)
+    # lambda -> 0: U is the argmin sample's control sequence
+    p = sc.params.with_(K=256, lam=1e-6)
+    got = gpu_solve(B, sc, p, kernel, U0=U0)
+    r = check_against_oracle(O, got, sc, p, U0=U0)
+    # lambda -> infinity: plain mean
+    p = sc.params.with_(K=256, lam=1e12)
+    got = gpu_solve(B, sc, p, kernel, U0=U0)
+    check_against_oracle(O, got, sc, p, U0=U0)
+    assert got["diag"]["eta"] == pytest.approx(256.0, rel=1e-5)
+
+
+def test_all_costs_nonfinite_leaves_U(B):
+    sc = scenes.scene_cfg1(6)
+    U0 = np.tile([0.5, 0.1], (sc.params.T, 1)).astype(np.float32)
+    p = sc.params.with_(K=200, w_pos=3e38)        # every stage cost overflows fp32
+    for kernel in (0, 4):
+        got = gpu_solve(B, sc, p, kernel, U0=U0)
+        assert np.array_equal(got["U"], U0)
+        assert got["diag"]["nonfinite"] == 200 and got["diag"]["argmin"] == -1
+
+
+def test_some_costs_nonfinite_get_zero_weight(B, O):
+    sc = scenes.scene_cfg1(6)
+    # the fp32 effort term w_v v^2 overflows to inf for samples with some |v| > ~1.06; the others
+    # stay finite (huge), and the oracle's fp64 costs of the overflowing samples are larger
+    # than every finite one, so both sides put all the weight on the same sample
+    # (T = 1: with more steps the SUM of finite fp32 terms can exceed FLT_MAX while each term
+    # and the fp64 accumulator stay finite, which is a different, benign, case)
+    p = sc.params.with_(K=512, T=1, w_v=3e38)
+    for kernel in (0, 4):
+        got = gpu_solve(B, sc, p, kernel)
+        ref = O.iteration(p, 0, sc.x0, sc.goal, sc.obstacles, np.zeros((p.T, 2)))
+        n_inf = int(np.count_nonzero(~np.isfinite(got["S"])))
+        assert 0 < n_inf < p.K and got["diag"]["nonfinite"] == n_inf
+        floors = np.array([p.v_max, p.delta_max])
+        assert close(got["U"], ref["U"], floors[None, :]).all()
+        assert got["diag"]["argmin"] == ref["argmin"]
+
+
+# ------------------------------------------------------------------------------------------
+# batches, determinism, shift, closed loop
+# ------------------------------------------------------------------------------------------
+def test_batched_scenes_equal_single_scene_solves(B, O):
+    scs = [scenes.scene_cfg2(s) for s in range(3)]
+    p = scs[0].params.with_(K=2048, T=80, n_iter=2, seed=40)
+    s = B.Solver(p, 3, 8, B.FLAG_WRITE_SAMPLES)
+    for i, sc in enumerate(scs):
+        s.set_scene(sc, i)
+    s.solve()
+    for i, sc in enumerate(scs):
+        pi = p.with_(seed=40 + i)                 # scene i uses seed + i
+        single = gpu_solve(B, sc, pi, 0)
+        got = dict(U=s.get_controls(i), S=s.get_costs(i), XT=s.get_final_states(i), diag=s.get_diag(i))
+        assert np.array_equal(got["U"], single["U"]) and np.array_equal(got["S"], single["S"])
+        check_against_oracle(O, got, sc, pi)
+    s.close()
+
+
+@pytest.mark.parametrize("kernel", KERNELS)
+def test_replay_is_bit_reproducible(B, kernel):
+    sc = scenes.scene_cfg2(3)
+    p = sc.params.with_(K=8192)
+    a = gpu_solve(B, sc, p, kernel)
+    b = gpu_solve(B, sc, p, kernel)
+    for key in ("U", "S", "XT"):
+        assert np.array_equal(a[key], b[key])
+    assert a["diag"] == b["diag"]
+
+
+def test_shift_duplicates_tail(B):
+    p = scenes.default_params(K=64, T=37)
+    s = B.Solver(p, 2, 1)
+    U = np.stack([np.linspace(-1, 1, 37), np.linspace(-0.5, 0.5, 37)], axis=1).astype(np.float32)
+    s.set_nominal(U, 0)
+    s.set_nominal(U[::-1].copy(), 1)
+    s.shift()
+    got0, got1 = s.get_controls(0), s.get_controls(1)
+    assert np.array_equal(got0[:-1], U[1:]) and np.array_equal(got0[-1], U[-1])
+    assert np.array_equal(got1[:-1], U[::-1][1:]) and np.array_equal(got1[-1], U[0])
+    s.close()
+
+
+def test_closed_loop_steps_match_oracle_stepwise(B, O):
+    """CFG3 shape (shortened): graph-replayed control steps; after every step the oracle is
+    re-seeded with the library's state so each solve / plant step / shift is compared on
+    identical inputs (closed-loop trajectories of a sampled controller diverge otherwise)."""
+    sc = scenes.scene_cfg2(4)                    # moving obstacles: exercises the obstacle advance
+    p = sc.params.with_(K=2048, T=60, n_iter=1)
+    s = B.Solver(p, 1, 8)
+    s.set_scene(sc)
+    x = sc.x0.copy()
+    obs = sc.obstacles.copy()
+    U = np.zeros((p.T, 2))
+    floors = np.array([p.v_max, p.delta_max])
+    for step in range(6):
+        u0 = s.step()[0]
+        ref = O.iteration(p, step, x, sc.goal, obs, U, n_threads=8)
+        assert close(u0, ref["U"][0], floors).all()
+        x_ref, obs_ref = O.plant_step(p, x, u0.astype(np.float64), obs)
+        x_gpu = s.get_state().astype(np.float64)
+        assert np.abs(x_gpu[:2] - x_ref[:2]).max() <= 1e-5
+        dpsi = (x_gpu[2:] - x_ref[2:] + np.pi) % (2 * np.pi) - np.pi
+        assert np.abs(dpsi).max() <= 1e-5
+        obs_gpu = s.get_obstacles().astype(np.float64)
+        assert np.abs(obs_gpu - obs_ref).max() <= 1e-5
+        U_gpu = s.get_controls().astype(np.float64)
+        assert close(U_gpu, O.shift(ref["U"]), floors[None, :]).all()
+        assert s.get_diag()["n"] == step + 1
+        x, obs, U = x_gpu, obs_gpu, U_gpu        # re-seed the oracle with the library's state
+    assert s.launch_count() == 6 * 3
+    s.close()
+
+
+# ------------------------------------------------------------------------------------------
+# full bench size: sampled outputs the oracle computes one by one + properties
+# ------------------------------------------------------------------------------------------
+def test_full_size_sampled_parity(B, O):
+    sc = scenes.scene_cfg2(0)
+    p = sc.params.with_(K=1048576, T=100, n_iter=1)
+    got = gpu_solve(B, sc, p, 0)
+    rng = np.random.default_rng(1)
+    ks = np.concatenate([[0, 15, 16, p.K - 1, int(got["diag"]["argmin"])], rng.integers(0, p.K, 150)])
+    U0 = np.zeros((p.T, 2))
+    for k in ks:
+        r = O.sample(p, 0, int(k), sc.x0, sc.goal, sc.obstacles, U0)
+        assert close(got["S"][k], r["S"], 1.0), (k, got["S"][k], r["S"])
+        assert close(got["XT"][k], r["xT"], 1.0).all()
+    # properties that hold at any size
+    d = got["diag"]
+    assert np.isfinite(got["S"]).all() and d["nonfinite"] == 0
+    assert d["argmin"] == int(np.argmin(got["S"])) or got["S"][d["argmin"]] == got["S"].min()
+    assert d["S_min"] == pytest.approx(float(got["S"].min()), rel=1e-6)
+    w = np.exp(-(got["S"].astype(np.float64) - float(got["S"].min())) / p.lam)
+    assert d["eta"] == pytest.approx(w.sum(), rel=5e-3)
+    assert got["U"][:, 0].min() >= p.v_min and got["U"][:, 0].max() <= p.v_max
+    assert got["U"][:, 1].min() >= p.delta_min and got["U"][:, 1].max() <= p.delta_max
+
+
+# ------------------------------------------------------------------------------------------
+# boundary errors
+# ------------------------------------------------------------------------------------------
+def test_error_codes(B):
+    import ctypes as C
+    import torch
+    p = scenes.default_params(K=64, T=10)
+    s = B.Solver(p, 1, 2)
+    with pytest.raises(B.BrmppiError) as e:
+        s.solve()
+    assert e.value.status == B.ERR_NOT_READY
+    s.set_state([0, 0, 0, 0])
+    s.set_goal([1, 0, 0, 0])
+    with pytest.raises(B.BrmppiError) as e:
+        s.set_obstacles(np.ones((3, 5)))
+    assert e.value.status == B.ERR_TOO_MANY_OBSTACLES
+    with pytest.raises(B.BrmppiError) as e:
+        s.set_state([np.nan, 0, 0, 0])
+    assert e.value.status == B.ERR_NONFINITE_INPUT
+    with pytest.raises(B.BrmppiError) as e:
+        s.set_obstacles([[0, 0, -1.0, 0, 0]])
+    assert e.value.status == B.ERR_INVALID_ARG
+    with pytest.raises(B.BrmppiError) as e:
+        s.set_state([0, 0, 0, 0], scene=1)
+    assert e.value.status == B.ERR_INVALID_ARG
+    with pytest.raises(B.BrmppiError) as e:
+        s.set_nominal(np.tile([5.0, 0.0], (10, 1)))          # outside the control box
+    assert e.value.status == B.ERR_INVALID_ARG
+    with pytest.raises(B.BrmppiError) as e:
+        s.get_costs()                                         # FLAG_WRITE_SAMPLES not set
+    assert e.value.status == B.ERR_NOT_READY
+    s.solve()
+    assert np.isfinite(s.get_controls()).all()
+    # psi is wrapped at set_state
+    s.set_state([1.0, 2.0, 7.0, -7.0])
+    x = s.get_state()
+    assert abs(x[2] - (7.0 - 2 * np.pi)) < 1e-6 and abs(x[3] + (7.0 - 2 * np.pi)) < 1e-6
+    s.close()
+    L = B.lib()
+    bad = B.make_cparams(p.with_(lam=0.0))
+    assert L.brmppi_workspace_bytes(C.byref(bad)) == 0
+    good = B.make_cparams(p)
+    ws = torch.empty(1024, dtype=torch.uint8, device="cuda")
+    ctx = C.c_void_p()
+    ptr = (ws.data_ptr() + 255) // 256 * 256
+    assert L.brmppi_create(C.byref(good), C.c_void_p(ptr), 512, None, C.byref(ctx)) == B.ERR_WORKSPACE_TOO_SMALL
+    assert L.brmppi_create(C.byref(good), C.c_void_p(ptr + 4), 1 << 30, None, C.byref(ctx)) == B.ERR_UNALIGNED
+    assert L.brmppi_create(C.byref(bad), C.c_void_p(ptr), 1 << 30, None, C.byref(ctx)) == B.ERR_INVALID_ARG
+    assert L.brmppi_create(None, C.c_void_p(ptr), 1 << 30, None, C.byref(ctx)) == B.ERR_NULL
+    assert B.strerror(B.ERR_TOO_MANY_OBSTACLES) == "too many obstacles"
