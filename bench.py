@@ -1,0 +1,344 @@
+#!/usr/bin/env python
+"""bench.py -- BR-MPPI throughput on synthetic parking scenes (BASELINE.json's metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload cfg2]
+
+A "step" is one control-step solve of the whole hot path (DESIGN.md §2 rows a1-a8: n_iter x
+{noise, perturb+clamp, rollout, barrier-rate + costs, online-softmax reduction, update}) on one
+synthetic scene.  Default workload: BASELINE.json configs[2] (K=16384, T=80, 8 obstacles of which
+3 move, 3 iterations per control step) -- the config the north star's ">= 50 % at K >= 16384" and
+"control rate at the 8-obstacle config" are quoted on.
+
+One JSON line on stdout (rank 0).  `value` = sample-steps/s with inputs resident in HBM, device
+time from CUDA events on the solver's stream, L2 flushed between steps; `e2e` = the same metric
+through the C ABI with host buffers (set_state/goal/obstacles from pinned host memory, solve,
+get_controls back to the host) on the host clock.  `roofline` is for the rollout kernel
+(DESIGN.md §6); `cpu_baseline` is the fp64 oracle on this box's host cores (a reported baseline,
+not the target).  --impl reference times that oracle alone.
+"""
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import scenes  # noqa: E402
+
+N_SMS = 148
+ISSUE_PER_CLK_PER_SM = 128          # thread-instructions per clock per SM (4 schedulers x 32 lanes)
+SM_MAX_MHZ_FALLBACK = 1965.0
+METRIC = "brmppi_sample_steps_per_s"
+UNIT = "sample-steps/s"
+
+
+def workload(name, rank=0):
+    """Scene + params of a named workload; rank r uses scene seed r (independent replicas)."""
+    if name == "cfg0":
+        sc = scenes.scene_cfg0(rank)
+    elif name == "cfg1":
+        sc = scenes.scene_cfg1(rank)
+    elif name == "cfg2":
+        sc = scenes.scene_cfg2(rank)
+    elif name == "cfg3":
+        sc = scenes.scene_cfg3(rank)
+    else:
+        raise SystemExit(f"unknown workload {name}")
+    return sc, sc.params
+
+
+def algorithmic_instr_per_sample_step(n_obs, n_discs):
+    """SURVEY.md §8(d) / DESIGN.md §6: issue slots the method itself needs per sample-step."""
+    return 121 + 8 * n_obs * n_discs
+
+
+def measured_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        return json.load(open(path))
+    except Exception:
+        return {}
+
+
+class ClockSampler:
+    """nvidia-smi clocks + throttle reasons sampled during the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
+         "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index=0):
+        self.rows, self.proc, self.index = [], None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "100"],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([x.strip() for x in line.split(",")])
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1]))
+            except Exception:
+                continue
+            for name, val in zip(names, r[4:8]):
+                if val.lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": statistics.median(sm) if sm else None,
+                "sm_max_mhz": max(mx) if mx else None, "reasons": sorted(reasons),
+                "samples": len(sm)}
+
+
+def oracle_throughput(sc, p, seconds_target, n_threads, k_sample):
+    """Time the oracle, as it stands, on a bounded sample (k_sample of the K samples, all T steps,
+    all n_iter iterations).  Returns (sample-steps/s, seconds, description)."""
+    from oracle import oracle as O
+    O.lib()
+    ps = p.with_(K=k_sample)
+    U = np.zeros((p.T, 2))
+    t0 = time.perf_counter()
+    reps = 0
+    while True:
+        O.solve(ps, reps * p.n_iter, sc.x0, sc.goal, sc.obstacles, U, n_threads=n_threads)
+        reps += 1
+        dt = time.perf_counter() - t0
+        if dt >= seconds_target or reps >= 50:
+            break
+    work = reps * k_sample * p.T * p.n_iter
+    return work / dt, dt, f"{reps} x ({k_sample} of {p.K} samples x T={p.T} x {p.n_iter} iterations), {n_threads} thread(s)"
+
+
+def dist_setup(n_gpus):
+    """(rank, world, local_rank, dist-or-None).  Under torchrun the env carries the rendezvous."""
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if world <= 1:
+        return 0, 1, 0, None
+    import torch.distributed as dist
+    backend = os.environ.get("BRMPPI_DIST_BACKEND", "nccl")
+    dist.init_process_group(backend=backend)
+    return dist.get_rank(), dist.get_world_size(), int(os.environ.get("LOCAL_RANK", "0")), dist
+
+
+def run_reference(args):
+    """The reference arm of this tier is the oracle, timed as it stands on the host cores."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return                                      # rank 0 alone runs it; the others exit 0
+    sc, p = workload(args.workload)
+    cores = os.cpu_count() or 1
+    k_sample = min(p.K, 1024)
+    from oracle import oracle as O
+    O.lib()
+    ps = p.with_(K=k_sample)
+    U = np.zeros((p.T, 2))
+    for w in range(args.warmup):
+        O.solve(ps, w, sc.x0, sc.goal, sc.obstacles, U, n_threads=cores)
+    t0 = time.perf_counter()
+    for s in range(args.steps):
+        O.solve(ps, s, sc.x0, sc.goal, sc.obstacles, U, n_threads=cores)
+    dt = time.perf_counter() - t0
+    value = args.steps * k_sample * p.T * p.n_iter / dt
+    sample = f"each step = {k_sample} of {p.K} samples x T={p.T} x {p.n_iter} iterations, {cores} threads"
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT,
+        "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": dt / args.steps * 1e3, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": workload_config(args.workload, sc, p, 1),
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+
+
+def workload_config(name, sc, p, n_scenes_total):
+    return {"workload": f"BASELINE.json configs[{name[-1]}] ({name})", "K": p.K, "T": p.T,
+            "n_obstacles": int(len(sc.obstacles)),
+            "n_moving": int(np.count_nonzero(np.abs(sc.obstacles[:, 3:5]).sum(axis=1))) if len(sc.obstacles) else 0,
+            "n_discs": len(p.discs), "n_iter": p.n_iter, "dt": p.dt, "scenes_total": n_scenes_total,
+            "l2": "flushed between timed steps (256 MiB write); per-step CUDA-event pairs",
+            "parallelism": "independent replicas, one scene per GPU, no collective on the data path"}
+
+
+def run_ours(args):
+    import torch
+    from paper_2508_05773_b200 import brmppi as B
+
+    rank, world, local_rank, dist = dist_setup(args.gpus)
+    dev = f"cuda:{local_rank}"
+    torch.cuda.set_device(dev)
+    sc, p = workload(args.workload, rank)
+    n_obs = len(sc.obstacles)
+    solver = B.Solver(p, 1, max(n_obs, 1), 0, device=dev)
+    solver.set_scene(sc)
+    stream = solver.stream
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+
+    def barrier():
+        torch.cuda.synchronize()
+        if dist is not None:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    # ---- device-resident throughput: inputs already in HBM, CUDA events on the solver's stream
+    for _ in range(max(args.warmup, 3)):
+        solver.solve()
+    barrier()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    launches0 = solver.launch_count()
+    sampler = ClockSampler(local_rank)
+    if rank == 0:
+        sampler.start()
+    t_wall0 = time.perf_counter()
+    for a, b in ev:
+        with torch.cuda.stream(stream):
+            flush.fill_(1)                                   # L2 flush, outside the event pair
+        a.record(stream)
+        solver.solve()
+        b.record(stream)
+    barrier()
+    wall_s = time.perf_counter() - t_wall0
+    clocks = sampler.stop() if rank == 0 else None
+    launches = solver.launch_count() - launches0
+    step_ms = [a.elapsed_time(b) for a, b in ev]
+    dev_s = sum(step_ms) * 1e-3
+    t = torch.tensor([dev_s], dtype=torch.float64, device=dev)
+    if dist is not None:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    dev_s_max = float(t.item())
+    work_per_rank = args.steps * p.K * p.T * p.n_iter
+
+    # ---- end to end through the C ABI with host buffers (pinned), host clock
+    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).pin_memory().numpy()
+    hx, hg, ho = pin(sc.x0), pin(sc.goal), pin(sc.obstacles)
+    for _ in range(3):
+        solver.set_state(hx); solver.set_goal(hg); solver.set_obstacles(ho); solver.solve(); solver.get_controls()
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        solver.set_state(hx)
+        solver.set_goal(hg)
+        solver.set_obstacles(ho)
+        solver.solve()
+        U = solver.get_controls()                            # synchronises; T*2 floats back
+    barrier()
+    e2e_s = time.perf_counter() - t0
+    te = torch.tensor([e2e_s], dtype=torch.float64, device=dev)
+    if dist is not None:
+        dist.all_reduce(te, op=dist.ReduceOp.MAX)
+    e2e_s_max = float(te.item())
+    h2d = 16 + 16 + 20 * n_obs + 4
+    d2h = 8 * p.T
+
+    # ---- closed-loop control rate (CUDA-graph replay of solve + plant step + shift)
+    lat = []
+    for i in range(20 + min(args.steps, 200)):
+        t1 = time.perf_counter()
+        solver.step()
+        if i >= 20:
+            lat.append(time.perf_counter() - t1)
+    lat.sort()
+    p50, p99 = lat[len(lat) // 2], lat[min(len(lat) - 1, int(0.99 * len(lat)))]
+
+    # ---- roofline of the rollout kernel (rank 0): device time per launch from CUDA events
+    roof = None
+    if rank == 0:
+        solver.set_scene(sc)
+        solver.set_nominal(None)
+        ms_roll, ms_upd = solver.time_kernels(50)
+        instr = algorithmic_instr_per_sample_step(n_obs, len(p.discs))
+        achieved = p.K * p.T * instr / (ms_roll * 1e-3) / 1e9          # G thread-instr / s
+        mp = measured_peaks()
+        sm_max = float(mp.get("sm_max_mhz", SM_MAX_MHZ_FALLBACK))
+        peak = N_SMS * ISSUE_PER_CLK_PER_SM * sm_max * 1e6 / 1e9
+        roof = {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "Ginstr/s (thread-instructions)",
+                "frac": achieved / peak, "traffic": dram_traffic_from_profile(),
+                "kernel": "rollout_tile", "kernel_ms": ms_roll, "update_kernel_ms": ms_upd,
+                "kernel_share_of_step": ms_roll * p.n_iter / (dev_s / args.steps * 1e3),
+                "algorithmic_instr_per_sample_step": instr,
+                "peak_basis": f"{N_SMS} SMs x {ISSUE_PER_CLK_PER_SM} thread-instr/clk/SM x {sm_max:.0f} MHz "
+                              f"({'MEASURED_PEAKS.json sm_max_mhz' if 'sm_max_mhz' in mp else 'fallback clock'}); "
+                              "issue rate confirmed by brmppi_measure_peaks (DESIGN.md §6)"}
+    solver.close()
+
+    if rank != 0:
+        return
+    cpu = None
+    if world == 1 or rank == 0:
+        cores = os.cpu_count() or 1
+        v1, s1, d1 = oracle_throughput(sc, p, 6.0, 1, min(p.K, 2048))
+        vn, sn, dn = oracle_throughput(sc, p, 8.0, cores, min(p.K, 8192))
+        cpu = {"value": vn, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": dn,
+               "value_1core": v1, "sample_1core": d1}
+    value = world * work_per_rank / dev_s_max
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": max(args.warmup, 3), "ms_per_step": dev_s_max / args.steps * 1e3,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+        "data": "synthetic", "config": workload_config(args.workload, sc, p, world),
+        "solves_per_s": world * args.steps * p.n_iter / dev_s_max,
+        "control_steps_per_s": world * args.steps / dev_s_max,
+        "e2e": {"value": world * work_per_rank / e2e_s_max, "unit": UNIT, "h2d_bytes_per_step": h2d,
+                "d2h_bytes_per_step": d2h, "control_steps_per_s": world * args.steps / e2e_s_max},
+        "closed_loop": {"p50_ms": p50 * 1e3, "p99_ms": p99 * 1e3, "hz": 1.0 / p50,
+                        "what": "brmppi_step: graph replay of solve + plant step + shift, host wall clock"},
+        "gpu_launches": int(launches), "clocks": clocks, "roofline": roof, "cpu_baseline": cpu,
+        "wall_s_timed_region": wall_s,
+        "paper_context": "paper: 9.9 ms per MPPI step, >100 Hz, 5000 rollouts x H=120, 8 obstacles, JAX on an unnamed GPU (PAPER.md:5,243) -- different formulation, context only",
+    }
+    print(json.dumps(line))
+
+
+def dram_traffic_from_profile():
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the rollout kernel, from the
+    committed ncu capture (profiles/r1_rollout_tile_dram.csv: header line, then bytes)."""
+    try:
+        rows = open(os.path.join(ROOT, "profiles", "r1_rollout_tile_dram.csv")).read().strip().splitlines()
+        return float(rows[-1].split(",")[-1])
+    except Exception:
+        return None
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=20)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="cfg2", choices=["cfg0", "cfg1", "cfg2", "cfg3"])
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

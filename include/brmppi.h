@@ -148,6 +148,13 @@ int brmppi_get_costs(brmppi_ctx* ctx, int scene, float* S_out /* K */);         
 int brmppi_get_final_states(brmppi_ctx* ctx, int scene, float* X_out /* K*4 */);    /* FLAG_WRITE_SAMPLES */
 int brmppi_get_diag(brmppi_ctx* ctx, int scene, brmppi_diag* out);
 
+/* Device time of the two kernels of one MPPI iteration, for the roofline report: runs `reps`
+ * iterations of every scene OUTSIDE the captured graph with a CUDA-event pair around each kernel
+ * on the context's stream and returns the mean milliseconds per launch:
+ * out_ms[0] = rollout kernel, out_ms[1] = merge/update kernel.  Advances the iteration counter by
+ * `reps` and updates U like `reps` single-iteration solves.  Synchronises. */
+int brmppi_time_kernels(brmppi_ctx* ctx, int reps, float out_ms[2]);
+
 /* Number of kernel launches this context has enqueued so far (graph replays count the kernels
  * inside the graph). */
 unsigned long long brmppi_launch_count(const brmppi_ctx* ctx);
@@ -172,8 +179,9 @@ int brmppi_debug_sample_controls(void* cuda_stream, const brmppi_params* p, unsi
 /* Issue-rate micro-benchmarks for the roofline denominator: thread-instructions
  * per clock per SM achieved by dependent-chain-free streams of FFMA, LOP3/IADD3 (ALU pipe),
  * MUFU (XU pipe) and the FFMA+ALU mix, plus the SM count and the clock measured in-kernel.
- * out[0..7] = {ffma, alu, mufu, mix, imad_wide, n_sms, sm_mhz_measured, ffma rate cross-checked
- * on the globaltimer}. */
+ * out[0..7] = {ffma, alu, mufu, mix (ffma+lop3 interleaved), imad_wide, n_sms, sm_mhz of an idle SM,
+ * sm_mhz seen while the FFMA kernel ran}.  Rates are whole-kernel: instructions per SM / (first
+ * block start .. last block end on the globaltimer, converted with the in-kernel clock). */
 int brmppi_measure_peaks(void* cuda_stream, float out[8]);
 
 #ifdef __cplusplus

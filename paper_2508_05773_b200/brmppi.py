@@ -24,7 +24,7 @@ EXPORTS = [
     "brmppi_set_goal", "brmppi_set_obstacles", "brmppi_set_nominal", "brmppi_set_counter",
     "brmppi_reset", "brmppi_solve", "brmppi_shift", "brmppi_step", "brmppi_get_controls",
     "brmppi_get_state", "brmppi_get_obstacles", "brmppi_get_costs", "brmppi_get_final_states",
-    "brmppi_get_diag", "brmppi_launch_count", "brmppi_strerror", "brmppi_debug_philox",
+    "brmppi_get_diag", "brmppi_time_kernels", "brmppi_launch_count", "brmppi_strerror", "brmppi_debug_philox",
     "brmppi_debug_sample_controls", "brmppi_measure_peaks",
 ]
 
@@ -95,6 +95,7 @@ def lib():
         L.brmppi_get_costs.argtypes = [vp, C.c_int, _fp]
         L.brmppi_get_final_states.argtypes = [vp, C.c_int, _fp]
         L.brmppi_get_diag.argtypes = [vp, C.c_int, C.POINTER(Diag)]
+        L.brmppi_time_kernels.argtypes = [vp, C.c_int, _fp]
         L.brmppi_launch_count.argtypes = [vp]
         L.brmppi_launch_count.restype = C.c_ulonglong
         L.brmppi_strerror.argtypes = [C.c_int]
@@ -251,6 +252,12 @@ class Solver:
         _check(lib().brmppi_get_diag(self._ctx, scene, C.byref(d)))
         return dict(S_min=d.S_min, argmin=d.argmin, eta=d.eta, ess=d.ess, n=d.n, nonfinite=d.nonfinite)
 
+    def time_kernels(self, reps=20):
+        """Mean device ms per launch of (rollout kernel, merge/update kernel)."""
+        out = np.zeros(2, dtype=np.float32)
+        _check(lib().brmppi_time_kernels(self._ctx, int(reps), _p(out)))
+        return float(out[0]), float(out[1])
+
     def launch_count(self):
         return int(lib().brmppi_launch_count(self._ctx))
 
@@ -285,4 +292,4 @@ def measure_peaks():
     _check(lib().brmppi_measure_peaks(C.c_void_p(st.cuda_stream), _p(out)))
     return dict(ffma=float(out[0]), alu=float(out[1]), mufu=float(out[2]), mix=float(out[3]),
                 imad_wide=float(out[4]), n_sms=int(out[5]), sm_mhz=float(out[6]),
-                ffma_globaltimer=float(out[7]))
+                sm_mhz_under_ffma=float(out[7]))

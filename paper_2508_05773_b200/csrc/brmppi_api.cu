@@ -141,7 +141,7 @@ struct brmppi_ctx {
 
 namespace {
 
-int enqueue_iteration(brmppi_ctx* c) {
+int launch_rollout(brmppi_ctx* c) {
   const DeviceParams& d = c->d;
   const bool precise = (c->p.flags & BRMPPI_FLAG_PRECISE_MATH) != 0;
   if (c->plan.tile_kernel) {
@@ -154,11 +154,22 @@ int enqueue_iteration(brmppi_ctx* c) {
       rollout_thread_per_sample<false><<<grid, kThreadBlock, c->smem_rollout, c->stream>>>(d);
     CU(cudaGetLastError());
   }
+  return BRMPPI_OK;
+}
+
+int launch_update(brmppi_ctx* c) {
+  const DeviceParams& d = c->d;
   dim3 ugrid((unsigned)((2 * d.T + kUpdateOutputsPerBlock - 1) / kUpdateOutputsPerBlock),
              (unsigned)d.n_scenes);
   merge_update<<<ugrid, kUpdateBlock, c->smem_update, c->stream>>>(d);
   CU(cudaGetLastError());
   return BRMPPI_OK;
+}
+
+int enqueue_iteration(brmppi_ctx* c) {
+  int r = launch_rollout(c);
+  if (r) return r;
+  return launch_update(c);
 }
 
 int enqueue_solve(brmppi_ctx* c) {
@@ -490,6 +501,37 @@ int brmppi_get_diag(brmppi_ctx* c, int scene, brmppi_diag* out) {
   return r;
 }
 
+int brmppi_time_kernels(brmppi_ctx* c, int reps, float out_ms[2]) {
+  if (!c || !out_ms) return BRMPPI_ERR_NULL;
+  if (reps < 1) return BRMPPI_ERR_INVALID_ARG;
+  int r = ready(c);
+  if (r) return r;
+  cudaEvent_t ev[3];
+  for (int i = 0; i < 3; ++i) CU(cudaEventCreate(&ev[i]));
+  double acc[2] = {0.0, 0.0};
+  cudaError_t e = cudaSuccess;
+  for (int it = 0; it < reps && e == cudaSuccess && r == 0; ++it) {
+    e = cudaEventRecord(ev[0], c->stream);
+    if (e == cudaSuccess) r = launch_rollout(c);
+    if (e == cudaSuccess && r == 0) e = cudaEventRecord(ev[1], c->stream);
+    if (e == cudaSuccess && r == 0) r = launch_update(c);
+    if (e == cudaSuccess && r == 0) e = cudaEventRecord(ev[2], c->stream);
+    if (e == cudaSuccess && r == 0) e = cudaStreamSynchronize(c->stream);
+    float a = 0.f, b = 0.f;
+    if (e == cudaSuccess && r == 0) e = cudaEventElapsedTime(&a, ev[0], ev[1]);
+    if (e == cudaSuccess && r == 0) e = cudaEventElapsedTime(&b, ev[1], ev[2]);
+    acc[0] += a; acc[1] += b;
+    c->launches += 2;
+    c->n_host += 1;
+  }
+  for (int i = 0; i < 3; ++i) cudaEventDestroy(ev[i]);
+  if (r) return r;
+  if (e != cudaSuccess) return cuda_fail(e);
+  out_ms[0] = (float)(acc[0] / reps);
+  out_ms[1] = (float)(acc[1] / reps);
+  return BRMPPI_OK;
+}
+
 unsigned long long brmppi_launch_count(const brmppi_ctx* c) { return c ? c->launches : 0ull; }
 
 const char* brmppi_strerror(int status) {
@@ -582,15 +624,22 @@ int brmppi_measure_peaks(void* cuda_stream, float out[8]) {
     if (e == cudaSuccess) e = cudaMemcpyAsync(h, spans, sizeof(long long) * 3 * (size_t)blocks, cudaMemcpyDeviceToHost, s);
     if (e == cudaSuccess) e = cudaStreamSynchronize(s);
     if (e != cudaSuccess) break;
-    long long mx = 0, gmin = h[1], gmax = h[2];
+    // Rate = instructions per SM / (first block start .. last block end, on the nanosecond
+    // globaltimer) converted to SM cycles with the clock each block saw while running
+    // (clock64 span / globaltimer span).  Per-block clock64 spans alone over-estimate: blocks
+    // that win the arbitration finish early while the SM is still busy with the others.
+    long long gmin = h[1], gmax = h[2];
+    double mhz_sum = 0.0;
     for (int b = 0; b < blocks; ++b) {
-      mx = h[3 * b] > mx ? h[3 * b] : mx;
       gmin = h[3 * b + 1] < gmin ? h[3 * b + 1] : gmin;
       gmax = h[3 * b + 2] > gmax ? h[3 * b + 2] : gmax;
+      mhz_sum += (double)h[3 * b] * 1e3 / (double)(h[3 * b + 2] - h[3 * b + 1]);
     }
+    const double mhz_kernel = mhz_sum / blocks;
     wall_ns[kind] = (double)(gmax - gmin);
     const double per_thread = (double)kPeakIters * kPeakReps * kPeakChains * (kind == PEAK_MIX ? 2.0 : 1.0);
-    out[kind] = (float)(per_thread * 1024.0 / (double)mx);   // thread-instr / clk / SM
+    out[kind] = (float)(per_thread * 1024.0 / (wall_ns[kind] * 1e-3 * mhz_kernel));   // thread-instr / clk / SM
+    if (kind == PEAK_FFMA) out[7] = (float)mhz_kernel;
   }
   if (e == cudaSuccess) {
     clock_rate_kernel<<<1, 1, 0, s>>>(sink);
@@ -600,10 +649,6 @@ int brmppi_measure_peaks(void* cuda_stream, float out[8]) {
     if (e == cudaSuccess) e = cudaStreamSynchronize(s);
     out[5] = (float)prop.multiProcessorCount;
     out[6] = mhz[0];
-    // cross-check of the FFMA rate on the nanosecond globaltimer (first block start to last
-    // block end), converted with the measured clock
-    out[7] = (float)((double)kPeakIters * kPeakReps * kPeakChains * 1024.0 /
-                     (wall_ns[PEAK_FFMA] * 1e-3 * (double)mhz[0]));
   }
   free(h);
   cudaFree(spans);

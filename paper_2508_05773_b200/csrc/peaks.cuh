@@ -12,7 +12,7 @@
 
 namespace brmppi {
 
-constexpr int kPeakIters = 512;
+constexpr int kPeakIters = 2048;
 constexpr int kPeakReps = 8;       // inner repetitions per loop trip: 64 instructions per branch
 constexpr int kPeakChains = 8;
 
