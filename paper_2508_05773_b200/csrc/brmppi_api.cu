@@ -274,7 +274,7 @@ int brmppi_create(const brmppi_params* p, void* dev_workspace, size_t workspace_
   d.diag = (brmppi_diag*)(base + L.diag);
   if (p->flags & BRMPPI_FLAG_WRITE_SAMPLES) { d.S = (float*)(base + L.S); d.XT = (float*)(base + L.XT); }
 
-  c->smem_update = sizeof(float) * (size_t)c->plan.n_partials;
+  c->smem_update = 0;
   cudaError_t e = cudaSuccess;
   if (c->plan.tile_kernel) {
     c->smem_rollout = rollout_tile_smem_bytes(d, c->plan.tile);

@@ -61,7 +61,7 @@ inline TilePlan make_tile_plan(int K, int T, int n_scenes, int max_obstacles) {
   }
   if (const char* e = getenv("BRMPPI_TILE_CHUNKS")) {   // tuning knob for sweeps
     const int c = atoi(e);
-    if (c >= 2 && c <= 16 && c % 2 == 0) best_c = c;
+    if (c >= 4 && c <= 16 && c % 2 == 0) best_c = c;
   }
   tp.chunks = best_c;
   tp.chunk_len = (T + best_c - 1) / best_c;

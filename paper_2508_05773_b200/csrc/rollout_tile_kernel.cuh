@@ -41,28 +41,35 @@ rollout_tile(const __grid_constant__ DeviceParams P) {
       sVel[i] = make_float2(0.0f, 0.0f);
     }
     __syncthreads();
-    if (tid == 0) {
+    {
+      // every thread i < n_obs places obstacle i: moving obstacles first, static ones after
+      // (groups without a moving one skip the o(t) update); ranks by counting, no serial pass
       const float4 x0 = reinterpret_cast<const float4*>(P.state)[scene];
-      float4 g = reinterpret_cast<const float4*>(P.goal)[scene];
-      g.x -= x0.x; g.y -= x0.y;
-      sM->x0 = x0;
-      sM->g = g;
-      // moving obstacles first, static ones after (groups without a moving one skip o(t))
       const int n_obs = P.n_obs[scene];
       const float* ob = P.obstacles + (size_t)scene * P.max_obstacles * 5;
-      int nm = 0;
-      for (int i = 0; i < n_obs; ++i) nm += (ob[5 * i + 3] != 0.0f || ob[5 * i + 4] != 0.0f) ? 1 : 0;
-      int im = 0, is = nm;
-      for (int i = 0; i < n_obs; ++i) {
-        const bool moving = (ob[5 * i + 3] != 0.0f || ob[5 * i + 4] != 0.0f);
-        const int dst = moving ? im++ : is++;
-        const float rho = ob[5 * i + 2] + P.disc_radius;
-        sObs[dst] = make_float4(ob[5 * i + 0] - x0.x, ob[5 * i + 1] - x0.y, 1.0f / (rho * rho), -1.0f);
-        sVel[dst] = make_float2(P.dt * ob[5 * i + 3], P.dt * ob[5 * i + 4]);
+      if (tid < n_obs) {
+        int nm = 0, before_m = 0, before_s = 0;
+        for (int j = 0; j < n_obs; ++j) {
+          const bool mj = (ob[5 * j + 3] != 0.0f || ob[5 * j + 4] != 0.0f);
+          nm += mj ? 1 : 0;
+          if (j < tid) { before_m += mj ? 1 : 0; before_s += mj ? 0 : 1; }
+        }
+        const bool moving = (ob[5 * tid + 3] != 0.0f || ob[5 * tid + 4] != 0.0f);
+        const int dst = moving ? before_m : nm + before_s;
+        const float rho = ob[5 * tid + 2] + P.disc_radius;
+        sObs[dst] = make_float4(ob[5 * tid + 0] - x0.x, ob[5 * tid + 1] - x0.y, 1.0f / (rho * rho), -1.0f);
+        sVel[dst] = make_float2(P.dt * ob[5 * tid + 3], P.dt * ob[5 * tid + 4]);
+        if (tid == 0) sM->n_moving = nm;
       }
-      sM->m = CUDART_INF; sM->argmin = 0x7fffffff; sM->eta = 0.0f; sM->w2 = 0.0f; sM->nonfinite = 0;
-      sM->n_moving = nm;
-      sM->n_groups = n_obs > 0 ? (n_obs + kObsGroup - 1) / kObsGroup : 1;
+      if (tid == 0) {
+        float4 g = reinterpret_cast<const float4*>(P.goal)[scene];
+        g.x -= x0.x; g.y -= x0.y;
+        sM->x0 = x0;
+        sM->g = g;
+        sM->m = CUDART_INF; sM->argmin = 0x7fffffff; sM->eta = 0.0f; sM->w2 = 0.0f; sM->nonfinite = 0;
+        if (n_obs == 0) sM->n_moving = 0;
+        sM->n_groups = n_obs > 0 ? (n_obs + kObsGroup - 1) / kObsGroup : 1;
+      }
     }
     __syncthreads();
   }
@@ -105,22 +112,24 @@ rollout_tile(const __grid_constant__ DeviceParams P) {
       float x = 0.0f, y = 0.0f, psi1 = x0.z, psi2 = x0.w;
       pP1[0] = psi1;
       pP2[0] = psi2;
-      int next_boundary = 0, cc = 0;
-      for (int t = 0; t < T; ++t) {
-        if (t == next_boundary) { sXY[cc * kTileSamples + s] = make_float2(x, y); ++cc; next_boundary += L; }
-        const float v = pV[t], b = pP1[t + 1];
-        float s1, c1, s2, c2;
-        sincos_t<PRECISE>(psi1, &s1, &c1);
-        sincos_t<PRECISE>(psi2, &s2, &c2);
-        const float a = P.dt * v;
-        const float sb = s1 * c2 - c1 * s2;            // sin(psi1 - psi2)
-        const float cb = fmaf(c1, c2, s1 * s2);        // cos(psi1 - psi2)
-        x = fmaf(a, c1, x);
-        y = fmaf(a, s1, y);
-        psi1 += b;
-        psi2 = fmaf(a * P.inv_L2, sb, fmaf(-(b * P.Lh_over_L2), cb, psi2));
-        pP1[t + 1] = psi1;
-        pP2[t + 1] = psi2;
+      for (int cc = 0, t = 0; t < T; ++cc) {
+        sXY[cc * kTileSamples + s] = make_float2(x, y);      // chunk-boundary position
+        const int te = min(t + L, T);
+        for (; t < te; ++t) {
+          const float v = pV[t], b = pP1[t + 1];
+          float s1, c1, s2, c2;
+          sincos_t<PRECISE>(psi1, &s1, &c1);
+          sincos_t<PRECISE>(psi2, &s2, &c2);
+          const float a = P.dt * v;
+          const float sb = s1 * c2 - c1 * s2;            // sin(psi1 - psi2)
+          const float cb = fmaf(c1, c2, s1 * s2);        // cos(psi1 - psi2)
+          x = fmaf(a, c1, x);
+          y = fmaf(a, s1, y);
+          psi1 += b;
+          psi2 = fmaf(a * P.inv_L2, sb, fmaf(-(b * P.Lh_over_L2), cb, psi2));
+          pP1[t + 1] = psi1;
+          pP2[t + 1] = psi2;
+        }
       }
       sXY[P.chunks * kTileSamples + s] = make_float2(x, y);   // x_T
     }
@@ -263,8 +272,13 @@ inline TileKernel tile_kernel_for(bool precise, int n_discs) {
 }
 
 inline cudaError_t configure_rollout_tile(bool precise, int n_discs, size_t smem_bytes) {
+  cudaError_t e = cudaFuncSetAttribute(tile_kernel_for(precise, n_discs),
+                                       cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes);
+  if (e != cudaSuccess) return e;
+  // ask for the full shared-memory carve-out: residency here is limited by shared memory and
+  // registers, the kernel streams almost nothing through L1
   return cudaFuncSetAttribute(tile_kernel_for(precise, n_discs),
-                              cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes);
+                              cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
 }
 
 inline cudaError_t launch_rollout_tile(const DeviceParams& d, const TilePlan& tp, bool precise,

@@ -12,14 +12,18 @@
 namespace brmppi {
 
 constexpr int kUpdateBlock = 256;
-constexpr int kUpdateOutputsPerBlock = kUpdateBlock / 32;   // one warp per output channel
+constexpr int kUpdateOutputsPerBlock = 1;   // one CTA per output channel o = 2 t + c
 
+// One CTA per (output channel, scene): every thread takes partials p = tid, tid + 256, ...
+// (coalesced rows, all loads of a thread independent, so the kernel is two L2 round trips deep),
+// then a fixed-order block reduction.  Every CTA recomputes the global minimum itself -- P * 12
+// bytes from L2 -- rather than paying a third kernel or a grid-wide sync for it.
 __global__ void __launch_bounds__(kUpdateBlock)
 merge_update(const __grid_constant__ DeviceParams P) {
-  extern __shared__ float sScale[];                 // [n_partials]
   __shared__ double sM[kUpdateBlock / 32];
   __shared__ int sI[kUpdateBlock / 32];
-  const int scene = blockIdx.y;
+  __shared__ float sRed[4][kUpdateBlock / 32];
+  const int scene = blockIdx.y, o = blockIdx.x;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int Pn = P.n_partials;
   const double* pm = P.part_m + (size_t)scene * Pn;
@@ -42,42 +46,28 @@ merge_update(const __grid_constant__ DeviceParams P) {
     if (sM[w] < m || (sM[w] == m && sI[w] < idx)) { m = sM[w]; idx = sI[w]; }
   const bool any_finite = m < CUDART_INF;
 
+  const float* peta = P.part_eta + (size_t)scene * Pn;
+  const float* pa = P.part_A + ((size_t)scene * 2 * P.T + o) * Pn;
+  const float* pw2 = P.part_w2 + (size_t)scene * Pn;
+  const int* pnf = P.part_nonfinite + (size_t)scene * Pn;
+  const bool diag_cta = (o == 0);
+  float eta = 0.0f, acc = 0.0f, w2 = 0.0f, nf = 0.0f;
   for (int p = tid; p < Pn; p += kUpdateBlock) {
     const double mp = pm[p];
-    sScale[p] = (any_finite && mp < CUDART_INF) ? expf((float)(-(mp - m) * (double)P.inv_lambda)) : 0.0f;
+    const float c = (any_finite && mp < CUDART_INF) ? expf((float)(-(mp - m) * (double)P.inv_lambda)) : 0.0f;
+    eta = fmaf(c, peta[p], eta);
+    acc = fmaf(c, pa[p], acc);
+    if (diag_cta) { w2 = fmaf(c * c, pw2[p], w2); nf += (float)pnf[p]; }
   }
+  eta = warp_sum(eta); acc = warp_sum(acc); w2 = warp_sum(w2); nf = warp_sum(nf);
+  if (lane == 0) { sRed[0][warp] = eta; sRed[1][warp] = acc; sRed[2][warp] = w2; sRed[3][warp] = nf; }
   __syncthreads();
-
-  // one warp per output channel o = 2 t + c; lanes stride over partials (coalesced rows)
-  const int o = blockIdx.x * kUpdateOutputsPerBlock + warp;
-  const float* peta = P.part_eta + (size_t)scene * Pn;
-  float eta = 0.0f, acc = 0.0f;
-  if (o < 2 * P.T) {
-    const float* pa = P.part_A + ((size_t)scene * 2 * P.T + o) * Pn;
-    for (int p = lane; p < Pn; p += 32) {
-      const float c = sScale[p];
-      eta = fmaf(c, peta[p], eta);
-      acc = fmaf(c, pa[p], acc);
-    }
-  } else {
-    for (int p = lane; p < Pn; p += 32) eta = fmaf(sScale[p], peta[p], eta);
-  }
-  eta = warp_sum(eta);
-  acc = warp_sum(acc);
-  if (o < 2 * P.T && lane == 0 && any_finite && eta > 0.0f) P.U[(size_t)scene * 2 * P.T + o] = acc / eta;
-
-  if (blockIdx.x == 0 && warp == 0) {
-    float w2 = 0.0f, nf = 0.0f;
-    const float* pw2 = P.part_w2 + (size_t)scene * Pn;
-    const int* pnf = P.part_nonfinite + (size_t)scene * Pn;
-    for (int p = lane; p < Pn; p += 32) {
-      const float c = sScale[p];
-      w2 = fmaf(c * c, pw2[p], w2);
-      nf += (float)pnf[p];
-    }
-    w2 = warp_sum(w2);
-    nf = warp_sum(nf);
-    if (lane == 0) {
+  if (tid == 0) {
+    eta = 0.0f; acc = 0.0f; w2 = 0.0f; nf = 0.0f;
+#pragma unroll
+    for (int w = 0; w < kUpdateBlock / 32; ++w) { eta += sRed[0][w]; acc += sRed[1][w]; w2 += sRed[2][w]; nf += sRed[3][w]; }
+    if (any_finite && eta > 0.0f) P.U[(size_t)scene * 2 * P.T + o] = acc / eta;
+    if (diag_cta) {
       brmppi_diag d;
       d.S_min = any_finite ? (float)m : CUDART_INF_F;
       d.argmin = any_finite ? idx : -1;
