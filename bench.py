@@ -280,7 +280,7 @@ def run_ours(args):
         peak = N_SMS * ISSUE_PER_CLK_PER_SM * sm_max * 1e6 / 1e9
         roof = {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "Ginstr/s (thread-instructions)",
                 "frac": achieved / peak, "traffic": dram_traffic_from_profile(),
-                "kernel": "rollout_tile", "kernel_ms": ms_roll, "update_kernel_ms": ms_upd,
+                "kernel": "rollout_cta", "kernel_ms": ms_roll, "update_kernel_ms": ms_upd,
                 "kernel_share_of_step": ms_roll * p.n_iter / (dev_s / args.steps * 1e3),
                 "algorithmic_instr_per_sample_step": instr,
                 "peak_basis": f"{N_SMS} SMs x {ISSUE_PER_CLK_PER_SM} thread-instr/clk/SM x {sm_max:.0f} MHz "
@@ -318,9 +318,9 @@ def run_ours(args):
 
 def dram_traffic_from_profile():
     """dram__bytes_read.sum + dram__bytes_write.sum per launch of the rollout kernel, from the
-    committed ncu capture (profiles/r1_rollout_tile_dram.csv: header line, then bytes)."""
+    committed ncu capture (profiles/r1_rollout_cta_dram.csv: header line, then bytes)."""
     try:
-        rows = open(os.path.join(ROOT, "profiles", "r1_rollout_tile_dram.csv")).read().strip().splitlines()
+        rows = open(os.path.join(ROOT, "profiles", "r1_rollout_cta_dram.csv")).read().strip().splitlines()
         return float(rows[-1].split(",")[-1])
     except Exception:
         return None

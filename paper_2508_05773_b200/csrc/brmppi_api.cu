@@ -14,8 +14,8 @@
 #include "brmppi_device.cuh"
 #include "peaks.cuh"
 #include "rollout_thread.cuh"
-#include "rollout_tile.cuh"
-#include "rollout_tile_kernel.cuh"
+#include "rollout_cta.cuh"
+#include "rollout_cta_kernel.cuh"
 #include "update.cuh"
 
 using namespace brmppi;
@@ -78,17 +78,32 @@ struct Layout {
 
 // Launch plan: which rollout kernel, how the sample axis is tiled, how many partials.
 struct Plan {
-  bool tile_kernel;
+  bool cta_kernel;
   int n_partials;
-  TilePlan tile;
+  CtaPlan cta;
 };
+
+// SM count of the current device (the persistent kernel launches one CTA per SM); 148 -- a B200 --
+// when no device is visible, so that brmppi_workspace_bytes still answers on a CPU-only box.
+int device_sm_count() {
+  if (const char* e = getenv("BRMPPI_NUM_SMS")) {   // tuning knob for sweeps
+    const int v = atoi(e);
+    if (v >= 1) return v;
+  }
+  int dev = 0, n = 0;
+  if (cudaGetDevice(&dev) == cudaSuccess &&
+      cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && n > 0)
+    return n;
+  cudaGetLastError();
+  return 148;
+}
 
 Plan make_plan(const brmppi_params& p) {
   Plan pl{};
-  pl.tile_kernel = !(p.flags & BRMPPI_FLAG_KERNEL_THREAD_PER_SAMPLE);
-  if (pl.tile_kernel) {
-    pl.tile = make_tile_plan(p.K, p.T, p.n_scenes, p.max_obstacles);
-    pl.n_partials = pl.tile.blocks_per_scene;
+  pl.cta_kernel = !(p.flags & BRMPPI_FLAG_KERNEL_THREAD_PER_SAMPLE);
+  if (pl.cta_kernel) {
+    pl.cta = make_cta_plan(p.K, p.T, p.n_scenes, p.max_obstacles, device_sm_count());
+    pl.n_partials = pl.cta.n_partials;
   } else {
     pl.n_partials = (p.K + kThreadBlock - 1) / kThreadBlock;
   }
@@ -144,8 +159,8 @@ namespace {
 int launch_rollout(brmppi_ctx* c) {
   const DeviceParams& d = c->d;
   const bool precise = (c->p.flags & BRMPPI_FLAG_PRECISE_MATH) != 0;
-  if (c->plan.tile_kernel) {
-    CU(launch_rollout_tile(d, c->plan.tile, precise, c->smem_rollout, c->stream));
+  if (c->plan.cta_kernel) {
+    CU(launch_rollout_cta(d, c->plan.cta, precise, c->stream));
   } else {
     dim3 grid((unsigned)c->plan.n_partials, (unsigned)d.n_scenes);
     if (precise)
@@ -252,15 +267,16 @@ int brmppi_create(const brmppi_params* p, void* dev_workspace, size_t workspace_
   d.key0 = (uint32_t)(p->seed & 0xFFFFFFFFull); d.key1 = (uint32_t)(p->seed >> 32);
   d.flags = p->flags;
   d.n_partials = c->plan.n_partials;
-  if (c->plan.tile_kernel) {
-    d.tiles_per_scene = c->plan.tile.tiles_per_scene;
-    d.chunks = c->plan.tile.chunks;
-    d.chunk_len = c->plan.tile.chunk_len;
-    d.t_stride = c->plan.tile.t_stride;
-    d.obs_padded = c->plan.tile.obs_padded;
-    const TileSmem ts = tile_smem_layout(d.T, d.obs_padded, d.chunks, d.t_stride);
-    d.off_obs = (int)ts.obs; d.off_vel = (int)ts.vel; d.off_xy = (int)ts.xy; d.off_unom = (int)ts.unom;
-    d.off_planes = (int)ts.planes; d.off_cost = (int)ts.cost; d.off_A = (int)ts.A; d.off_misc = (int)ts.misc;
+  if (c->plan.cta_kernel) {
+    const CtaPlan& cp = c->plan.cta;
+    d.S_tile = cp.S_tile; d.tiles_per_scene = cp.tiles_per_scene; d.total_tiles = cp.total_tiles;
+    d.tiles_per_cta = cp.tiles_per_cta;
+    d.chunks = cp.chunks; d.chunk_len = cp.chunk_len; d.t_stride = cp.ts; d.obs_padded = cp.obs_padded;
+    const CtaSmem ts = cta_smem_layout(d.T, cp.S_tile, cp.chunks, cp.ts, cp.obs_padded);
+    d.off_obs = (int)ts.obs; d.off_vel = (int)ts.vel; d.off_unom = (int)ts.unom; d.off_A = (int)ts.A;
+    d.off_scratch = (int)ts.scratch; d.off_w = (int)ts.w; d.off_alpha = (int)ts.alpha;
+    d.off_track = (int)ts.track; d.off_cost = (int)ts.cost; d.off_xy = (int)ts.xy;
+    d.off_planes = (int)ts.planes; d.off_misc = (int)ts.misc;
   }
   unsigned char* base = (unsigned char*)dev_workspace;
   const Layout& L = c->layout;
@@ -276,9 +292,9 @@ int brmppi_create(const brmppi_params* p, void* dev_workspace, size_t workspace_
 
   c->smem_update = 0;
   cudaError_t e = cudaSuccess;
-  if (c->plan.tile_kernel) {
-    c->smem_rollout = rollout_tile_smem_bytes(d, c->plan.tile);
-    e = configure_rollout_tile((p->flags & BRMPPI_FLAG_PRECISE_MATH) != 0, p->n_discs, c->smem_rollout);
+  if (c->plan.cta_kernel) {
+    c->smem_rollout = c->plan.cta.smem;
+    e = configure_rollout_cta((p->flags & BRMPPI_FLAG_PRECISE_MATH) != 0, p->n_discs, c->smem_rollout);
   } else {
     c->smem_rollout = rollout_thread_smem_bytes(d);
     if (c->smem_rollout > 48 * 1024) {

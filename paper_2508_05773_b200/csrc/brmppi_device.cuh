@@ -32,14 +32,18 @@ struct DeviceParams {
   uint32_t key0, key1;        // Philox key of scene 0 = (lo32(seed), hi32(seed)); scene s adds s
   uint32_t flags;
   // tiling of the sample axis
-  int n_partials;             // rollout blocks per scene (one online-softmax partial each)
-  int tiles_per_scene;        // phase-split kernel: K / kTileSamples rounded up
-  int chunks, chunk_len;      // phase-split kernel: C threads per sample, L steps per thread
-  int t_stride;               // phase-split kernel: padded row length of the control planes
-  int obs_padded;             // phase-split kernel: obstacle slots, a multiple of the group size
-  // phase-split kernel: byte offsets of the shared-memory sections (host-computed, so that the
-  // device code rematerialises a pointer with one add instead of keeping it in a register)
-  int off_obs, off_vel, off_xy, off_unom, off_planes, off_cost, off_A, off_misc;
+  int n_partials;             // partial slots per scene (one online-softmax partial per CTA and scene)
+  int S_tile;                 // persistent-CTA kernel: samples per tile
+  int tiles_per_scene;        // ceil(K / S_tile)
+  int total_tiles;            // tiles_per_scene * n_scenes
+  int tiles_per_cta;          // CTA b owns the flat tiles [b Q, (b+1) Q); 0 = one CTA per partial slot
+  int chunks, chunk_len;      // C threads per sample in the barrier phase, L steps per thread
+  int t_stride;               // padded row length of the shared-memory planes
+  int obs_padded;             // obstacle slots, a multiple of the group size
+  // byte offsets of the shared-memory sections (host-computed, so that the device code
+  // rematerialises a pointer with one add instead of keeping it in a register)
+  int off_obs, off_vel, off_unom, off_A, off_scratch, off_w, off_alpha, off_track, off_cost, off_xy,
+      off_planes, off_misc;
   // workspace pointers (DEVICE)
   float* state;               // [n_scenes][4]
   float* goal;                // [n_scenes][4]
@@ -160,6 +164,14 @@ __device__ __forceinline__ float wrap_angle(float a) {
   return fmaf(-kTwoPi, rintf(a * kInvTwoPi), a);
 }
 
+// Same value without the XU-pipe FRND: adding and subtracting 1.5 * 2^23 rounds to the nearest
+// integer (ties to even, like rintf) for |a / 2 pi| < 2^22; two FMA-pipe adds.  No fast-math
+// flags are used in this build, so the compiler keeps both additions.
+__device__ __forceinline__ float wrap_angle_fma(float a) {
+  const float r = __fadd_rn(__fmaf_rn(a, kInvTwoPi, 12582912.0f), -12582912.0f);
+  return fmaf(-kTwoPi, r, a);
+}
+
 // Vehicle state in the solve's local frame (origin at the start position).
 struct State { float x, y, psi1, psi2; };
 
@@ -213,6 +225,15 @@ __device__ __forceinline__ float goal_cost(const DeviceParams& P, const State& X
   const float ex = X.x - g.x, ey = X.y - g.y;
   const float e1 = wrap_angle(X.psi1 - g.z), e2 = wrap_angle(X.psi2 - g.w);
   return fmaf(P.w_pos, fmaf(ex, ex, ey * ey), P.w_head * fmaf(e1, e1, e2 * e2));
+}
+
+// Goal + hitch stage cost with the FMA-pipe wrap (persistent-CTA kernel, fast-math mode).
+__device__ __forceinline__ float tracking_cost_fma(const DeviceParams& P, const State& X, const float4 g) {
+  const float ex = X.x - g.x, ey = X.y - g.y;
+  const float e1 = wrap_angle_fma(X.psi1 - g.z), e2 = wrap_angle_fma(X.psi2 - g.w);
+  const float G = fmaf(P.w_pos, fmaf(ex, ex, ey * ey), P.w_head * fmaf(e1, e1, e2 * e2));
+  const float e = fmaxf(fabsf(wrap_angle_fma(X.psi1 - X.psi2)) - P.hitch_max, 0.0f);
+  return fmaf(P.w_hitch * e, e, G);
 }
 
 // Hitch-angle squared hinge (reading 15).

@@ -1,0 +1,411 @@
+// rollout_cta_kernel.cuh -- the persistent-CTA rollout kernel itself (design notes, plan and
+// shared-memory layout are in rollout_cta.cuh).
+//
+// Register discipline: everything that lives for the whole kernel but is touched once per phase
+// (start state, goal, obstacle counts, running softmax state) sits in the CtaMisc block of shared
+// memory, and every shared-memory section pointer is smem_raw + a constant-bank offset, so the long
+// phase-C loop does not have to share the register file with values it never uses.
+#pragma once
+
+#include "rollout_cta.cuh"
+
+namespace brmppi {
+
+#define BRMPPI_SMEM(type, off) reinterpret_cast<type*>(smem_raw + (off))
+
+// Phase C for one group of kObsGroup obstacles over the steps [t0, t1) of one sample: the
+// barrier-rate hinge sum_t sum_{i,j} max(0, (1 - alpha) h_t - h_{t+1})  (a4, a5).
+// Obstacle record: (ox, oy, 1/rho^2, h0) with h = |c - o|^2 / rho^2 + h0; h0 = -1 for a real
+// obstacle, and (0, 0, 0, 0) for a null one, whose h == 0 and hinge == 0 exactly.
+// pV, pS1 .. pC2: this sample's rows of the v, sin/cos psi1, sin/cos psi2 planes.
+template <int ND, bool MOVING>
+__device__ __forceinline__ double barrier_group(const DeviceParams& P, const float* __restrict__ pV,
+                                                const float* __restrict__ pS1, const float* __restrict__ pC1,
+                                                const float* __restrict__ pS2, const float* __restrict__ pC2,
+                                                const float4* __restrict__ obs, const float2* __restrict__ vel,
+                                                float x, float y, int t0, int t1, float one_minus_alpha) {
+  double bar = 0.0;
+  float hprev[kObsGroup][ND];
+  float4 o[kObsGroup];
+#pragma unroll
+  for (int i = 0; i < kObsGroup; ++i) o[i] = obs[i];
+  float s1 = pS1[t0], c1 = pC1[t0];
+  {
+    const float s2 = pS2[t0], c2 = pC2[t0];
+    float cx[ND], cy[ND];
+    disc_centres_n<ND>(P, x, y, s1, c1, s2, c2, cx, cy);
+    const float tf = (float)t0;
+#pragma unroll
+    for (int i = 0; i < kObsGroup; ++i) {
+      float ox = o[i].x, oy = o[i].y;
+      if (MOVING) { const float2 w = vel[i]; ox = fmaf(tf, w.x, ox); oy = fmaf(tf, w.y, oy); }
+#pragma unroll
+      for (int j = 0; j < ND; ++j) {
+        const float dx = cx[j] - ox, dy = cy[j] - oy;
+        hprev[i][j] = fmaf(fmaf(dx, dx, dy * dy), o[i].z, o[i].w);
+      }
+    }
+  }
+  for (int t = t0; t < t1; ++t) {
+    // (x, y) of state t+1 from state t: the chain's own FMAs on the same operands
+    const float a = P.dt * pV[t];
+    x = fmaf(a, c1, x);
+    y = fmaf(a, s1, y);
+    s1 = pS1[t + 1]; c1 = pC1[t + 1];
+    const float s2 = pS2[t + 1], c2 = pC2[t + 1];
+    float cx[ND], cy[ND];
+    disc_centres_n<ND>(P, x, y, s1, c1, s2, c2, cx, cy);
+    const float tf = (float)(t + 1);
+    float pen = 0.0f;
+#pragma unroll
+    for (int i = 0; i < kObsGroup; ++i) {
+      float ox = o[i].x, oy = o[i].y;
+      if (MOVING) { const float2 w = vel[i]; ox = fmaf(tf, w.x, ox); oy = fmaf(tf, w.y, oy); }
+#pragma unroll
+      for (int j = 0; j < ND; ++j) {
+        const float dx = cx[j] - ox, dy = cy[j] - oy;
+        const float hn = fmaf(fmaf(dx, dx, dy * dy), o[i].z, o[i].w);
+        pen += fmaxf(fmaf(one_minus_alpha, hprev[i][j], -hn), 0.0f);   // barrier-rate hinge
+        hprev[i][j] = hn;
+      }
+    }
+    bar += (double)pen;
+  }
+  return bar;
+}
+
+template <bool PRECISE, int ND>
+__global__ void __launch_bounds__(kCtaThreads, 1)
+rollout_cta(const __grid_constant__ DeviceParams P) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  const int tid = threadIdx.x;
+  const int S = P.S_tile;
+  const int c = tid / S, s = tid - c * S;     // (chunk or row, sample in tile)
+  const int lane = tid & 31, warp = tid >> 5;
+
+  const int tile_first = blockIdx.x * P.tiles_per_cta;
+  const int tile_last = min(tile_first + P.tiles_per_cta, P.total_tiles);
+  int cur_scene = -1;
+  int par = 0;          // parity of the running softmax state in CtaMisc
+
+  for (int tile = tile_first; tile < tile_last; ++tile) {
+    const int scene = tile / P.tiles_per_scene;
+    const int k = (tile - scene * P.tiles_per_scene) * S + s;
+
+    if (scene != cur_scene) {
+      // ---- partial of the scene just finished -> HBM; then this scene's data -> shared -------
+      if (cur_scene >= 0) {
+        const int Pn = P.n_partials, T = P.T;
+        const CtaMisc* sM = BRMPPI_SMEM(CtaMisc, P.off_misc);
+        const float* sA = BRMPPI_SMEM(float, P.off_A);
+        const int slot = blockIdx.x - (cur_scene * P.tiles_per_scene) / P.tiles_per_cta;
+        const size_t pbase = (size_t)cur_scene * Pn + slot;
+        if (tid == 0) {
+          P.part_m[pbase] = sM->m[par];
+          P.part_argmin[pbase] = sM->argmin[par];
+          P.part_eta[pbase] = sM->eta[par];
+          P.part_w2[pbase] = sM->w2[par];
+          P.part_nonfinite[pbase] = sM->nonfinite[par];
+        }
+        for (int o = tid; o < 2 * T; o += kCtaThreads) {
+          const int ch = o >= T ? 1 : 0, t = o - ch * T;
+          P.part_A[((size_t)cur_scene * 2 * T + (2 * t + ch)) * Pn + slot] = sA[o];
+        }
+        __syncthreads();
+      }
+      cur_scene = scene;
+      par = 0;
+      {
+        const int T = P.T;
+        float4* sObs = BRMPPI_SMEM(float4, P.off_obs);
+        float2* sVel = BRMPPI_SMEM(float2, P.off_vel);
+        float2* sUnom = BRMPPI_SMEM(float2, P.off_unom);
+        float* sA = BRMPPI_SMEM(float, P.off_A);
+        CtaMisc* sM = BRMPPI_SMEM(CtaMisc, P.off_misc);
+        for (int i = tid; i < T; i += kCtaThreads) sUnom[i] = reinterpret_cast<const float2*>(P.U)[(size_t)scene * T + i];
+        for (int i = tid; i < 2 * T; i += kCtaThreads) sA[i] = 0.0f;
+        for (int i = tid; i < P.obs_padded; i += kCtaThreads) {   // null obstacles: h == 0, hinge == 0
+          sObs[i] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+          sVel[i] = make_float2(0.0f, 0.0f);
+        }
+        __syncthreads();
+        // every thread i < n_obs places obstacle i: moving obstacles first, static ones after
+        // (groups without a moving one skip the o(t) update); ranks by counting, no serial pass.
+        // Scene data in the vehicle-centred frame.
+        const float4 x0 = reinterpret_cast<const float4*>(P.state)[scene];
+        const int n_obs = P.n_obs[scene];
+        const float* ob = P.obstacles + (size_t)scene * P.max_obstacles * 5;
+        if (tid < n_obs) {
+          int nm = 0, before_m = 0, before_s = 0;
+          for (int j = 0; j < n_obs; ++j) {
+            const bool mj = (ob[5 * j + 3] != 0.0f || ob[5 * j + 4] != 0.0f);
+            nm += mj ? 1 : 0;
+            if (j < tid) { before_m += mj ? 1 : 0; before_s += mj ? 0 : 1; }
+          }
+          const bool moving = (ob[5 * tid + 3] != 0.0f || ob[5 * tid + 4] != 0.0f);
+          const int dst = moving ? before_m : nm + before_s;
+          const float rho = ob[5 * tid + 2] + P.disc_radius;
+          sObs[dst] = make_float4(ob[5 * tid + 0] - x0.x, ob[5 * tid + 1] - x0.y, 1.0f / (rho * rho), -1.0f);
+          sVel[dst] = make_float2(P.dt * ob[5 * tid + 3], P.dt * ob[5 * tid + 4]);
+          if (tid == 0) sM->n_moving = nm;
+        }
+        if (tid == 0) {
+          float4 g = reinterpret_cast<const float4*>(P.goal)[scene];
+          g.x -= x0.x; g.y -= x0.y;
+          sM->x0 = x0;
+          sM->g = g;
+          sM->m[0] = CUDART_INF; sM->argmin[0] = 0x7fffffff; sM->eta[0] = 0.0f; sM->w2[0] = 0.0f; sM->nonfinite[0] = 0;
+          if (n_obs == 0) sM->n_moving = 0;
+          sM->n_groups = n_obs > 0 ? (n_obs + kObsGroup - 1) / kObsGroup : 1;
+        }
+        __syncthreads();
+      }
+    }
+
+    // ---- phase A: noise, perturb + clamp (a1, a2) --------------------------------------------
+    {
+      const int TS = P.t_stride, T = P.T;
+      const int R = kCtaThreads / S;
+      const uint32_t n = *P.counter;
+      const uint32_t key0 = P.key0 + (uint32_t)scene;
+      const uint32_t key1 = P.key1 + (key0 < P.key0 ? 1u : 0u);
+      const float2* sUnom = BRMPPI_SMEM(float2, P.off_unom);
+      float* pV = BRMPPI_SMEM(float, P.off_planes) + s * TS;
+      float* pD = pV + S * TS;
+      float* pS1 = pD + S * TS;
+      if (c < R) {
+        for (int t = c; t < T; t += R) {
+          const float2 u = sample_control<PRECISE>(P, sUnom[t], (uint32_t)t, n, (uint32_t)k, key0, key1);
+          const float tan_d = tan_t<PRECISE>(u.y);
+          pV[t] = u.x;
+          pD[t] = u.y;
+          pS1[t + 1] = (P.dt * u.x) * P.inv_L1 * tan_d;          // dpsi1 of step t, parked at t+1
+        }
+      }
+      if (c == 0) BRMPPI_SMEM(float, P.off_alpha)[s] = sample_alpha(P, n, (uint32_t)k, key0, key1);
+    }
+    __syncthreads();
+
+    // ---- phase B: serial Euler chain of eq. (6), one sample per thread (a3), and the stage
+    //      costs that need the full state: goal, heading, effort, hitch, terminal (a6) ---------
+    if (c == 0) {
+      const int TS = P.t_stride, T = P.T, L = P.chunk_len;
+      const float* pV = BRMPPI_SMEM(float, P.off_planes) + s * TS;
+      const float* pD = pV + S * TS;
+      float* pS1 = BRMPPI_SMEM(float, P.off_planes) + (2 * S + s) * TS;
+      float* pC1 = pS1 + S * TS;
+      float* pS2 = pC1 + S * TS;
+      float* pC2 = pS2 + S * TS;
+      float2* sXY = BRMPPI_SMEM(float2, P.off_xy);        // [C][S] chunk-start (x, y)
+      const CtaMisc* sM = BRMPPI_SMEM(CtaMisc, P.off_misc);
+      const float4 x0 = sM->x0, g = sM->g;
+      float x = 0.0f, y = 0.0f, psi1 = x0.z, psi2 = x0.w;
+      float s1, c1, s2, c2;
+      sincos_t<PRECISE>(psi1, &s1, &c1);
+      sincos_t<PRECISE>(psi2, &s2, &c2);
+      pS1[0] = s1; pC1[0] = c1; pS2[0] = s2; pC2[0] = c2;
+      double track = 0.0;
+      float effort = 0.0f;
+      for (int cc = 0, t = 0; t < T; ++cc) {
+        sXY[cc * S + s] = make_float2(x, y);
+        const int te = min(t + L, T);
+        for (; t < te; ++t) {
+          const float v = pV[t], d = pD[t], b = pS1[t + 1];
+          const float a = P.dt * v;
+          const float sb = s1 * c2 - c1 * s2;            // sin(psi1 - psi2)
+          const float cb = fmaf(c1, c2, s1 * s2);        // cos(psi1 - psi2)
+          x = fmaf(a, c1, x);
+          y = fmaf(a, s1, y);
+          psi1 += b;
+          psi2 = fmaf(a * P.inv_L2, sb, fmaf(-(b * P.Lh_over_L2), cb, psi2));
+          sincos_t<PRECISE>(psi1, &s1, &c1);
+          sincos_t<PRECISE>(psi2, &s2, &c2);
+          pS1[t + 1] = s1; pC1[t + 1] = c1; pS2[t + 1] = s2; pC2[t + 1] = c2;
+          const State X{x, y, psi1, psi2};
+          if (PRECISE) track += (double)(goal_cost(P, X, g) + hitch_cost(P, X));
+          else track += (double)tracking_cost_fma(P, X, g);
+          effort = fmaf(P.w_v * v, v, fmaf(P.w_delta * d, d, effort));
+        }
+      }
+      const State X{x, y, psi1, psi2};
+      track += (double)(P.w_term * goal_cost(P, X, g));   // terminal cost r_N(x_N), eq. (7)
+      BRMPPI_SMEM(double, P.off_track)[s] = track + (double)effort;
+      if ((P.flags & BRMPPI_FLAG_WRITE_SAMPLES) && k < P.K)
+        reinterpret_cast<float4*>(P.XT)[(size_t)scene * P.K + k] = make_float4(x + x0.x, y + x0.y, psi1, psi2);
+    }
+    __syncthreads();
+
+    // ---- phase C: barrier h and barrier-rate hinge (a4, a5) ----------------------------------
+    if (c < P.chunks) {
+      const int TS = P.t_stride, T = P.T;
+      const int t0 = c * P.chunk_len, t1 = min(t0 + P.chunk_len, T);
+      const CtaMisc* sM = BRMPPI_SMEM(CtaMisc, P.off_misc);
+      const float* pV = BRMPPI_SMEM(float, P.off_planes) + s * TS;
+      const float* pS1 = pV + 2 * S * TS;
+      const float* pC1 = pS1 + S * TS;
+      const float* pS2 = pC1 + S * TS;
+      const float* pC2 = pS2 + S * TS;
+      const float4* sObs = BRMPPI_SMEM(float4, P.off_obs);
+      const float2* sVel = BRMPPI_SMEM(float2, P.off_vel);
+      const float one_minus_alpha = 1.0f - BRMPPI_SMEM(float, P.off_alpha)[s];
+      const int n_moving = sM->n_moving, n_groups = sM->n_groups;
+      const float2 xy = BRMPPI_SMEM(float2, P.off_xy)[c * S + s];
+      double bar = 0.0;
+      for (int grp = 0; grp < n_groups; ++grp) {
+        const int ib = grp * kObsGroup;
+        if (ib < n_moving)
+          bar += barrier_group<ND, true>(P, pV, pS1, pC1, pS2, pC2, sObs + ib, sVel + ib, xy.x, xy.y, t0, t1, one_minus_alpha);
+        else
+          bar += barrier_group<ND, false>(P, pV, pS1, pC1, pS2, pC2, sObs + ib, sVel + ib, xy.x, xy.y, t0, t1, one_minus_alpha);
+      }
+      BRMPPI_SMEM(double, P.off_cost)[c * S + s] = (double)P.w_bar * bar;
+    }
+    __syncthreads();
+
+    // ---- phase D: tile reduction against the running online-softmax state (a7) --------------
+    double Sk = CUDART_INF;
+    bool valid = false, finite = false;
+    if (warp < kChainWarps) {
+      CtaMisc* sM = BRMPPI_SMEM(CtaMisc, P.off_misc);
+      valid = (tid < S) && (k < P.K);
+      if (valid) {
+        const double* sCost = BRMPPI_SMEM(double, P.off_cost);
+        Sk = BRMPPI_SMEM(double, P.off_track)[s];
+        for (int cc = 0; cc < P.chunks; ++cc) Sk += sCost[cc * S + s];      // fixed order
+        if (P.flags & BRMPPI_FLAG_WRITE_SAMPLES) P.S[(size_t)scene * P.K + k] = (float)Sk;
+      }
+      finite = valid && (Sk == Sk) && (Sk < CUDART_INF) && (Sk > -CUDART_INF);
+      double m = finite ? Sk : CUDART_INF;
+      int idx = finite ? k : 0x7fffffff;
+      warp_argmin(m, idx);
+      if (lane == 0) { sM->redM[warp] = m; sM->redI[warp] = idx; }
+    }
+    __syncthreads();
+    float scale_old;
+    {
+      // every thread folds the four warp minima and the running minimum the same way
+      CtaMisc* sM = BRMPPI_SMEM(CtaMisc, P.off_misc);
+      double m_new = sM->m[par];
+      int idx_new = sM->argmin[par];
+      const double m_old = m_new;
+#pragma unroll
+      for (int w = 0; w < kChainWarps; ++w) {
+        const double mw = sM->redM[w];
+        const int iw = sM->redI[w];
+        if (mw < m_new || (mw == m_new && iw < idx_new)) { m_new = mw; idx_new = iw; }
+      }
+      scale_old = (m_old < CUDART_INF) ? expf((float)(-(m_old - m_new) * (double)P.inv_lambda)) : 0.0f;
+      if (warp < kChainWarps) {
+        // S - m in fp64, then fp32 exp (SURVEY §7 hard part 2)
+        const float w = finite ? expf((float)(-(Sk - m_new) * (double)P.inv_lambda)) : 0.0f;
+        if (tid < S) BRMPPI_SMEM(float, P.off_w)[tid] = w;
+        const float eta_w = warp_sum(w), w2_w = warp_sum(w * w);
+        const float nf_w = warp_sum((valid && !finite) ? 1.0f : 0.0f);
+        if (lane == 0) { sM->redF[0][warp] = eta_w; sM->redF[1][warp] = w2_w; sM->redF[2][warp] = nf_w; }
+      }
+      if (tid == 0) { sM->m[par ^ 1] = m_new; sM->argmin[par ^ 1] = idx_new; }
+    }
+    __syncthreads();
+
+    // ---- phase E: running weighted control sums A[t] (a7) -----------------------------------
+    {
+      const int TS = P.t_stride, T = P.T;
+      CtaMisc* sM = BRMPPI_SMEM(CtaMisc, P.off_misc);
+      if (tid == 0) {
+        float eta_t = 0.0f, w2_t = 0.0f, nf_t = 0.0f;
+#pragma unroll
+        for (int w = 0; w < kChainWarps; ++w) { eta_t += sM->redF[0][w]; w2_t += sM->redF[1][w]; nf_t += sM->redF[2][w]; }
+        sM->eta[par ^ 1] = fmaf(sM->eta[par], scale_old, eta_t);
+        sM->w2[par ^ 1] = fmaf(sM->w2[par], scale_old * scale_old, w2_t);
+        sM->nonfinite[par ^ 1] = sM->nonfinite[par] + (int)nf_t;
+      }
+      float* sA = BRMPPI_SMEM(float, P.off_A);
+      const float* sW = BRMPPI_SMEM(float, P.off_w);
+      const float* sV = BRMPPI_SMEM(float, P.off_planes);
+      const int n_out = 2 * T;
+      if (n_out * 2 <= kCtaThreads) {
+        // G threads per output, each over the samples s = g, g + G, ...; fixed-order combine
+        float* sScr = BRMPPI_SMEM(float, P.off_scratch);
+        const int G = kCtaThreads / n_out;
+        const int g = tid / n_out, o = tid - g * n_out;
+        if (g < G) {
+          const int ch = o >= T ? 1 : 0, t = o - ch * T;
+          const float* plane = sV + ch * S * TS + t;
+          float acc = 0.0f;
+          for (int ss = g; ss < S; ss += G) acc = fmaf(sW[ss], plane[ss * TS], acc);
+          sScr[tid] = acc;
+        }
+        __syncthreads();
+        if (tid < n_out) {
+          float acc = 0.0f;
+          for (int gg = 0; gg < G; ++gg) acc += sScr[gg * n_out + tid];
+          sA[tid] = fmaf(sA[tid], scale_old, acc);
+        }
+      } else {
+        for (int o = tid; o < n_out; o += kCtaThreads) {
+          const int ch = o >= T ? 1 : 0, t = o - ch * T;
+          const float* plane = sV + ch * S * TS + t;
+          float acc = 0.0f;
+          for (int ss = 0; ss < S; ++ss) acc = fmaf(sW[ss], plane[ss * TS], acc);
+          sA[o] = fmaf(sA[o], scale_old, acc);
+        }
+      }
+    }
+    par ^= 1;
+    __syncthreads();
+  }
+
+  // ---- partial of the last scene -> HBM -----------------------------------------------------
+  if (cur_scene >= 0) {
+    const int Pn = P.n_partials, T = P.T;
+    const CtaMisc* sM = BRMPPI_SMEM(CtaMisc, P.off_misc);
+    const float* sA = BRMPPI_SMEM(float, P.off_A);
+    const int slot = blockIdx.x - (cur_scene * P.tiles_per_scene) / P.tiles_per_cta;
+    const size_t pbase = (size_t)cur_scene * Pn + slot;
+    if (tid == 0) {
+      P.part_m[pbase] = sM->m[par];
+      P.part_argmin[pbase] = sM->argmin[par];
+      P.part_eta[pbase] = sM->eta[par];
+      P.part_w2[pbase] = sM->w2[par];
+      P.part_nonfinite[pbase] = sM->nonfinite[par];
+    }
+    for (int o = tid; o < 2 * T; o += kCtaThreads) {
+      const int ch = o >= T ? 1 : 0, t = o - ch * T;
+      P.part_A[((size_t)cur_scene * 2 * T + (2 * t + ch)) * Pn + slot] = sA[o];
+    }
+  }
+}
+
+#undef BRMPPI_SMEM
+
+using CtaKernel = void (*)(const DeviceParams);
+
+inline CtaKernel cta_kernel_for(bool precise, int n_discs) {
+  switch (n_discs * 2 + (precise ? 1 : 0)) {
+    case 2: return rollout_cta<false, 1>;
+    case 3: return rollout_cta<true, 1>;
+    case 4: return rollout_cta<false, 2>;
+    case 5: return rollout_cta<true, 2>;
+    case 6: return rollout_cta<false, 3>;
+    case 7: return rollout_cta<true, 3>;
+    case 8: return rollout_cta<false, 4>;
+    default: return rollout_cta<true, 4>;
+  }
+}
+
+inline cudaError_t configure_rollout_cta(bool precise, int n_discs, size_t smem_bytes) {
+  cudaError_t e = cudaFuncSetAttribute(cta_kernel_for(precise, n_discs),
+                                       cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes);
+  if (e != cudaSuccess) return e;
+  // the kernel streams almost nothing through L1: ask for the full shared-memory carve-out
+  return cudaFuncSetAttribute(cta_kernel_for(precise, n_discs),
+                              cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
+}
+
+inline cudaError_t launch_rollout_cta(const DeviceParams& d, const CtaPlan& pl, bool precise,
+                                      cudaStream_t stream) {
+  cta_kernel_for(precise, d.n_discs)<<<(unsigned)pl.grid, kCtaThreads, pl.smem, stream>>>(d);
+  return cudaGetLastError();
+}
+
+}  // namespace brmppi

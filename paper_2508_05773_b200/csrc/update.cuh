@@ -25,9 +25,17 @@ merge_update(const __grid_constant__ DeviceParams P) {
   __shared__ float sRed[4][kUpdateBlock / 32];
   const int scene = blockIdx.y, o = blockIdx.x;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int Pn = P.n_partials;
-  const double* pm = P.part_m + (size_t)scene * Pn;
-  const int* pi = P.part_argmin + (size_t)scene * Pn;
+  // partial slots in use: the persistent kernel writes one per CTA whose tile range touches this
+  // scene (CTA b owns the flat tiles [b Q, (b+1) Q)); the thread-per-sample kernel fills them all
+  const int Pstride = P.n_partials;
+  int Pn = Pstride;
+  if (P.tiles_per_cta > 0) {
+    const int first = (scene * P.tiles_per_scene) / P.tiles_per_cta;
+    const int last = ((scene + 1) * P.tiles_per_scene - 1) / P.tiles_per_cta;
+    Pn = last - first + 1;
+  }
+  const double* pm = P.part_m + (size_t)scene * Pstride;
+  const int* pi = P.part_argmin + (size_t)scene * Pstride;
 
   // global minimum and its sample index (lowest index on ties)
   double m = CUDART_INF;
@@ -46,10 +54,10 @@ merge_update(const __grid_constant__ DeviceParams P) {
     if (sM[w] < m || (sM[w] == m && sI[w] < idx)) { m = sM[w]; idx = sI[w]; }
   const bool any_finite = m < CUDART_INF;
 
-  const float* peta = P.part_eta + (size_t)scene * Pn;
-  const float* pa = P.part_A + ((size_t)scene * 2 * P.T + o) * Pn;
-  const float* pw2 = P.part_w2 + (size_t)scene * Pn;
-  const int* pnf = P.part_nonfinite + (size_t)scene * Pn;
+  const float* peta = P.part_eta + (size_t)scene * Pstride;
+  const float* pa = P.part_A + ((size_t)scene * 2 * P.T + o) * Pstride;
+  const float* pw2 = P.part_w2 + (size_t)scene * Pstride;
+  const int* pnf = P.part_nonfinite + (size_t)scene * Pstride;
   const bool diag_cta = (o == 0);
   float eta = 0.0f, acc = 0.0f, w2 = 0.0f, nf = 0.0f;
   for (int p = tid; p < Pn; p += kUpdateBlock) {

@@ -236,7 +236,11 @@ def test_batched_scenes_equal_single_scene_solves(B, O):
         pi = p.with_(seed=40 + i)                 # scene i uses seed + i
         single = gpu_solve(B, sc, pi, 0)
         got = dict(U=s.get_controls(i), S=s.get_costs(i), XT=s.get_final_states(i), diag=s.get_diag(i))
-        assert np.array_equal(got["U"], single["U"]) and np.array_equal(got["S"], single["S"])
+        # same draws and arithmetic per sample; the tiling (hence the fp32/fp64 summation order
+        # of the chunk partials and of the weighted sums) depends on the batch size
+        assert np.allclose(got["S"], single["S"], rtol=2e-6, atol=1e-5)
+        assert np.allclose(got["U"], single["U"], rtol=0, atol=2e-5)
+        assert got["diag"]["argmin"] == single["diag"]["argmin"]
         check_against_oracle(O, got, sc, pi)
     s.close()
 
