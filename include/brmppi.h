@@ -71,6 +71,9 @@ typedef struct { int body; float offset; } brmppi_disc;
                                           steps fused (north_star item 2).  Default is the
                                           phase-split tile kernel.               */
 
+#define BRMPPI_FLAG_PHASE_TIMING 8u     /* persistent kernel: CTAs record nanoseconds per phase
+                                          (globaltimer); read with brmppi_get_phase_times       */
+
 typedef struct {
   int K;              /* samples per iteration, >= 1                                            */
   int T;              /* horizon steps, 1..BRMPPI_MAX_T                                         */
@@ -154,6 +157,13 @@ int brmppi_get_diag(brmppi_ctx* ctx, int scene, brmppi_diag* out);
  * out_ms[0] = rollout kernel, out_ms[1] = merge/update kernel.  Advances the iteration counter by
  * `reps` and updates U like `reps` single-iteration solves.  Synchronises. */
 int brmppi_time_kernels(brmppi_ctx* ctx, int reps, float out_ms[2]);
+
+/* Per-phase device time of the LAST rollout launch, from the kernel's own globaltimer stamps
+ * (needs BRMPPI_FLAG_PHASE_TIMING, else BRMPPI_ERR_NOT_READY; default kernel only).  out_us[0..6] =
+ * mean over CTAs of the microseconds spent in: scene prologue, A noise, B chain, C cost,
+ * D reduction, E weighted control sums, partial write-out; out_us[7] = first CTA start to last
+ * CTA end.  Synchronises. */
+int brmppi_get_phase_times(brmppi_ctx* ctx, float out_us[8]);
 
 /* Number of kernel launches this context has enqueued so far (graph replays count the kernels
  * inside the graph). */

@@ -14,6 +14,7 @@ MAX_DISCS = 4
 FLAG_WRITE_SAMPLES = 1
 FLAG_PRECISE_MATH = 2
 FLAG_KERNEL_THREAD_PER_SAMPLE = 4
+FLAG_PHASE_TIMING = 8
 
 OK = 0
 ERR_NULL, ERR_INVALID_ARG, ERR_WORKSPACE_TOO_SMALL, ERR_TOO_MANY_OBSTACLES = -1, -2, -3, -4
@@ -24,7 +25,7 @@ EXPORTS = [
     "brmppi_set_goal", "brmppi_set_obstacles", "brmppi_set_nominal", "brmppi_set_counter",
     "brmppi_reset", "brmppi_solve", "brmppi_shift", "brmppi_step", "brmppi_get_controls",
     "brmppi_get_state", "brmppi_get_obstacles", "brmppi_get_costs", "brmppi_get_final_states",
-    "brmppi_get_diag", "brmppi_time_kernels", "brmppi_launch_count", "brmppi_strerror", "brmppi_debug_philox",
+    "brmppi_get_diag", "brmppi_get_phase_times", "brmppi_time_kernels", "brmppi_launch_count", "brmppi_strerror", "brmppi_debug_philox",
     "brmppi_debug_sample_controls", "brmppi_measure_peaks",
 ]
 
@@ -95,6 +96,7 @@ def lib():
         L.brmppi_get_costs.argtypes = [vp, C.c_int, _fp]
         L.brmppi_get_final_states.argtypes = [vp, C.c_int, _fp]
         L.brmppi_get_diag.argtypes = [vp, C.c_int, C.POINTER(Diag)]
+        L.brmppi_get_phase_times.argtypes = [vp, _fp]
         L.brmppi_time_kernels.argtypes = [vp, C.c_int, _fp]
         L.brmppi_launch_count.argtypes = [vp]
         L.brmppi_launch_count.restype = C.c_ulonglong
@@ -257,6 +259,13 @@ class Solver:
         out = np.zeros(2, dtype=np.float32)
         _check(lib().brmppi_time_kernels(self._ctx, int(reps), _p(out)))
         return float(out[0]), float(out[1])
+
+    def get_phase_times(self):
+        """Per-phase microseconds of the last rollout launch (FLAG_PHASE_TIMING)."""
+        out = np.zeros(8, dtype=np.float32)
+        _check(lib().brmppi_get_phase_times(self._ctx, _p(out)))
+        names = ("prologue", "A_noise", "B_chain", "C_cost", "D_reduce", "E_update", "partial_out", "span")
+        return dict(zip(names, (float(x) for x in out)))
 
     def launch_count(self):
         return int(lib().brmppi_launch_count(self._ctx))

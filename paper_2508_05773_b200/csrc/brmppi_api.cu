@@ -66,14 +66,14 @@ bool params_valid(const brmppi_params* p) {
   if (p->delta_min <= -1.5f || p->delta_max >= 1.5f) return false;   // tan(delta) must stay finite
   if (p->alpha_lo > p->alpha_hi) return false;
   const unsigned known = BRMPPI_FLAG_WRITE_SAMPLES | BRMPPI_FLAG_PRECISE_MATH |
-                         BRMPPI_FLAG_KERNEL_THREAD_PER_SAMPLE;
+                         BRMPPI_FLAG_KERNEL_THREAD_PER_SAMPLE | BRMPPI_FLAG_PHASE_TIMING;
   if (p->flags & ~known) return false;
   return true;
 }
 
 struct Layout {
   size_t state, goal, n_obs, obstacles, U, counter, u0, part_m, part_argmin, part_eta, part_w2,
-      part_nf, part_A, diag, S, XT, total;
+      part_nf, part_A, diag, S, XT, phase, total;
 };
 
 // Launch plan: which rollout kernel, how the sample axis is tiled, how many partials.
@@ -133,6 +133,8 @@ Layout make_layout(const brmppi_params& p, const Plan& pl) {
     L.S = take(ns * (size_t)p.K * 4);
     L.XT = take(ns * (size_t)p.K * 16);
   }
+  if ((p.flags & BRMPPI_FLAG_PHASE_TIMING) && pl.cta_kernel)
+    L.phase = take((size_t)pl.cta.grid * (kPhaseSlots + 2) * sizeof(unsigned long long));
   L.total = off;
   return L;
 }
@@ -275,7 +277,7 @@ int brmppi_create(const brmppi_params* p, void* dev_workspace, size_t workspace_
     const CtaSmem ts = cta_smem_layout(d.T, cp.S_tile, cp.chunks, cp.ts, cp.obs_padded);
     d.off_obs = (int)ts.obs; d.off_vel = (int)ts.vel; d.off_unom = (int)ts.unom; d.off_A = (int)ts.A;
     d.off_scratch = (int)ts.scratch; d.off_w = (int)ts.w; d.off_alpha = (int)ts.alpha;
-    d.off_track = (int)ts.track; d.off_cost = (int)ts.cost; d.off_xy = (int)ts.xy;
+    d.off_cost = (int)ts.cost; d.off_xy = (int)ts.xy;
     d.off_planes = (int)ts.planes; d.off_misc = (int)ts.misc;
   }
   unsigned char* base = (unsigned char*)dev_workspace;
@@ -289,6 +291,7 @@ int brmppi_create(const brmppi_params* p, void* dev_workspace, size_t workspace_
   d.part_nonfinite = (int*)(base + L.part_nf); d.part_A = (float*)(base + L.part_A);
   d.diag = (brmppi_diag*)(base + L.diag);
   if (p->flags & BRMPPI_FLAG_WRITE_SAMPLES) { d.S = (float*)(base + L.S); d.XT = (float*)(base + L.XT); }
+  if ((p->flags & BRMPPI_FLAG_PHASE_TIMING) && c->plan.cta_kernel) d.phase_ns = (unsigned long long*)(base + L.phase);
 
   c->smem_update = 0;
   cudaError_t e = cudaSuccess;
@@ -546,6 +549,35 @@ int brmppi_time_kernels(brmppi_ctx* c, int reps, float out_ms[2]) {
   out_ms[0] = (float)(acc[0] / reps);
   out_ms[1] = (float)(acc[1] / reps);
   return BRMPPI_OK;
+}
+
+int brmppi_get_phase_times(brmppi_ctx* c, float out_us[8]) {
+  if (!c || !out_us) return BRMPPI_ERR_NULL;
+  if (!c->d.phase_ns) return BRMPPI_ERR_NOT_READY;
+  const int grid = c->plan.cta.grid, W = kPhaseSlots + 2;
+  unsigned long long* h = (unsigned long long*)malloc(sizeof(unsigned long long) * (size_t)grid * W);
+  if (!h) return BRMPPI_ERR_NULL;
+  int r = d2h(c, h, c->d.phase_ns, sizeof(unsigned long long) * (size_t)grid * W);
+  if (r == BRMPPI_OK) {
+    // phase slots are SM cycles (clock64); each CTA's own lifetime on the globaltimer converts them
+    double acc[kPhaseSlots] = {0};
+    unsigned long long tmin = ~0ull, tmax = 0ull, life = 0ull;
+    for (int b = 0; b < grid; ++b) {
+      const unsigned long long t0 = h[b * W + kPhaseSlots], t1 = h[b * W + kPhaseSlots + 1];
+      double cyc = 0.0;
+      for (int i = 0; i < kPhaseSlots; ++i) cyc += (double)h[b * W + i];
+      const double ns_per_cycle = cyc > 0.0 ? (double)(t1 - t0) / cyc : 0.0;
+      for (int i = 0; i < kPhaseSlots; ++i) acc[i] += (double)h[b * W + i] * ns_per_cycle;
+      if (t0 < tmin) tmin = t0;
+      if (t1 > tmax) tmax = t1;
+      if (t1 - t0 > life) life = t1 - t0;
+    }
+    for (int i = 0; i < kPhaseSlots; ++i) out_us[i] = (float)(acc[i] / grid * 1e-3);
+    out_us[7] = (float)((double)(tmax - tmin) * 1e-3);
+    (void)life;
+  }
+  free(h);
+  return r;
 }
 
 unsigned long long brmppi_launch_count(const brmppi_ctx* c) { return c ? c->launches : 0ull; }

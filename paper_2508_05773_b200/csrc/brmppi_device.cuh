@@ -42,7 +42,7 @@ struct DeviceParams {
   int obs_padded;             // obstacle slots, a multiple of the group size
   // byte offsets of the shared-memory sections (host-computed, so that the device code
   // rematerialises a pointer with one add instead of keeping it in a register)
-  int off_obs, off_vel, off_unom, off_A, off_scratch, off_w, off_alpha, off_track, off_cost, off_xy,
+  int off_obs, off_vel, off_unom, off_A, off_scratch, off_w, off_alpha, off_cost, off_xy,
       off_planes, off_misc;
   // workspace pointers (DEVICE)
   float* state;               // [n_scenes][4]
@@ -61,6 +61,7 @@ struct DeviceParams {
   brmppi_diag* diag;          // [n_scenes]
   float* S;                   // [n_scenes][K]     (FLAG_WRITE_SAMPLES)
   float* XT;                  // [n_scenes][K][4]  (FLAG_WRITE_SAMPLES)
+  unsigned long long* phase_ns;   // [grid][8] per-CTA phase nanoseconds (FLAG_PHASE_TIMING), else null
 };
 
 // ---------------------------------------------------------------------------------------------

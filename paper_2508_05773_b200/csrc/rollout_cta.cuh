@@ -12,18 +12,18 @@
 //
 //   A  noise      thread (s, r) draws the controls of steps r, r + R, ... of sample s
 //                 (R = 512 / S rows): Philox -> Box-Muller -> perturb + clamp (a1, a2); stores v,
-//                 delta and the heading increment dpsi1 = dt v tan(delta) / L1 to shared planes.
+//                 delta and the heading increment dpsi1 = dt v tan(delta) / L1 to shared-memory
+//                 planes; effort cost.
 //   B  chain      the S threads of warps 0..3 (one warp per scheduler) run the serial Euler
-//                 recursion of eq. (6) (a3), one sample each, and -- since the full state is in
-//                 their registers -- the goal / heading / effort / hitch cost and the terminal cost
-//                 (a6).  They leave sin/cos of both headings for every step in shared memory and
-//                 (x, y) at the chunk boundaries.
-//   C  barrier    thread (s, c) walks steps [cL, cL+L) of sample s: re-integrates (x, y) from its
-//                 chunk boundary (two FMAs, bit-identical to the chain), disc centres from the
-//                 stored sin/cos (no MUFU here), barrier h for every (obstacle, disc) with h_t in
-//                 registers, barrier-rate hinge (a4, a5).  Obstacles go in groups of 8 (padded
-//                 with null obstacles whose h is identically 0) held in registers.
-//   D  reduce     S threads add track + chunk partials in a fixed order (fp64), block argmin,
+//                 recursion of eq. (6) (a3), one sample each, and nothing else: a single in-order
+//                 instruction stream per step is the critical path of the whole tile.  psi1, psi2
+//                 of every step go to shared planes, (x, y) only at the chunk boundaries.
+//   C  cost       thread (s, c) walks steps [cL, cL+L) of sample s: re-integrates (x, y) from its
+//                 chunk boundary (two FMAs, bit-identical to the chain), disc centres, barrier h
+//                 for every (obstacle, disc) with h_t in registers, barrier-rate hinge (a4, a5),
+//                 goal / heading / hitch cost (a6).  Obstacles go in groups of 8 (padded with null
+//                 obstacles whose h is identically 0) held in registers.
+//   D  reduce     S threads add effort + chunk partials in a fixed order (fp64), block argmin,
 //                 weights against the CTA's running minimum (online softmax, a7).
 //   E  update     threads (channel, t) rescale the running A[t] and add sum_s w_s u_s[t] from the
 //                 control planes still in shared memory (a7).
@@ -45,6 +45,7 @@ constexpr int kMaxTileSamples = kChainWarps * 32;   // 128
 constexpr int kObsGroup = 8;                        // obstacles whose h_t are held in registers at a time
 constexpr int kMaxChunks = 16;
 constexpr int kMinChunkLen = 4;
+constexpr int kPhaseSlots = 7;                      // prologue, A, B, C, D, E, partial out
 constexpr size_t kSmemMax = 232448;                 // 227 KB opt-in dynamic shared memory per CTA
 
 struct CtaMisc {            // lives in the "misc" section
@@ -57,10 +58,11 @@ struct CtaMisc {            // lives in the "misc" section
   double redM[kChainWarps];
   int redI[kChainWarps];
   float redF[3][kChainWarps];
+  unsigned long long phase_acc[kPhaseSlots], t_begin;   // BRMPPI_FLAG_PHASE_TIMING
 };
 
 struct CtaSmem {
-  size_t obs, vel, unom, A, scratch, w, alpha, track, cost, xy, planes, misc, total;
+  size_t obs, vel, unom, A, scratch, w, alpha, cost, xy, planes, misc, total;
 };
 
 // Shared-memory carve-up (host only: the kernel gets the byte offsets through DeviceParams, so
@@ -76,10 +78,9 @@ inline CtaSmem cta_smem_layout(int T, int S, int chunks, int ts, int obs_padded)
   L.scratch = take(sizeof(float) * kCtaThreads);
   L.w = take(sizeof(float) * (size_t)S);
   L.alpha = take(sizeof(float) * (size_t)S);
-  L.track = take(sizeof(double) * (size_t)S);
   L.cost = take(sizeof(double) * (size_t)chunks * S);
-  L.xy = take(sizeof(float2) * (size_t)chunks * S);
-  L.planes = take(sizeof(float) * 6 * (size_t)S * ts);   // v, delta, sin psi1, cos psi1, sin psi2, cos psi2
+  L.xy = take(sizeof(float2) * (size_t)(chunks + 1) * S);
+  L.planes = take(sizeof(float) * 4 * (size_t)S * ts);   // v, delta, psi1, psi2
   L.misc = take(sizeof(CtaMisc));
   L.total = off;
   return L;

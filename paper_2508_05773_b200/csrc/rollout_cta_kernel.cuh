@@ -13,32 +13,55 @@ namespace brmppi {
 
 #define BRMPPI_SMEM(type, off) reinterpret_cast<type*>(smem_raw + (off))
 
+__device__ __forceinline__ unsigned long long global_ns() {
+  unsigned long long t;
+  asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+  return t;
+}
+// BRMPPI_FLAG_PHASE_TIMING: thread 0 adds the SM cycles since the previous stamp to phase slot i
+// (clock64: the globaltimer ticks too coarsely for sub-microsecond phases; it only brackets the CTA)
+// BAR.SYNC is deferred-blocking: the volatile shared-memory read makes the stamp wait for the
+// barrier's release instead of recording the arrival of warp 0.
+#define BRMPPI_STAMP(i)                                                      \
+  if (P.phase_ns != nullptr && tid == 0) {                                   \
+    const unsigned long long seen__ = *reinterpret_cast<volatile unsigned long long*>(&BRMPPI_SMEM(CtaMisc, P.off_misc)->t_begin); \
+    const unsigned long long now__ = (unsigned long long)clock64() + (seen__ & 0ull); \
+    BRMPPI_SMEM(CtaMisc, P.off_misc)->phase_acc[i] += now__ - t_stamp;       \
+    t_stamp = now__;                                                         \
+  }
+
 // Phase C for one group of kObsGroup obstacles over the steps [t0, t1) of one sample: the
-// barrier-rate hinge sum_t sum_{i,j} max(0, (1 - alpha) h_t - h_{t+1})  (a4, a5).
+// barrier-rate hinge sum_t sum_{i,j} max(0, (1 - alpha) h_t - h_{t+1})  (a4, a5), and -- for the
+// first group (TRACK) -- the goal / heading / hitch stage cost of every state it visits (a6).
 // Obstacle record: (ox, oy, 1/rho^2, h0) with h = |c - o|^2 / rho^2 + h0; h0 = -1 for a real
-// obstacle, and (0, 0, 0, 0) for a null one, whose h == 0 and hinge == 0 exactly.
-// pV, pS1 .. pC2: this sample's rows of the v, sin/cos psi1, sin/cos psi2 planes.
-template <int ND, bool MOVING>
-__device__ __forceinline__ double barrier_group(const DeviceParams& P, const float* __restrict__ pV,
-                                                const float* __restrict__ pS1, const float* __restrict__ pC1,
-                                                const float* __restrict__ pS2, const float* __restrict__ pC2,
-                                                const float4* __restrict__ obs, const float2* __restrict__ vel,
-                                                float x, float y, int t0, int t1, float one_minus_alpha) {
-  double bar = 0.0;
+// obstacle, and (0, 0, 0, 0) for a null one, whose h == 0 and hinge == 0 exactly.  The first NM
+// obstacles of the group move: o(t) = o(0) + t dt vel (a static one has vel == 0, so rounding NM up
+// is exact).  pV, pP1, pP2: this sample's rows of the v, psi1, psi2 planes.
+struct GroupCost { double track, bar; };
+
+template <bool PRECISE, int ND, int NM, bool TRACK>
+__device__ __forceinline__ GroupCost barrier_group(const DeviceParams& P, const float* __restrict__ pV,
+                                                   const float* __restrict__ pP1, const float* __restrict__ pP2,
+                                                   const float4* __restrict__ obs, const float2* __restrict__ vel,
+                                                   float x, float y, int t0, int t1, float one_minus_alpha,
+                                                   const float4 g) {
+  double bar = 0.0, track = 0.0;
   float hprev[kObsGroup][ND];
   float4 o[kObsGroup];
 #pragma unroll
   for (int i = 0; i < kObsGroup; ++i) o[i] = obs[i];
-  float s1 = pS1[t0], c1 = pC1[t0];
+  float s1, c1;
   {
-    const float s2 = pS2[t0], c2 = pC2[t0];
+    float s2, c2;
+    sincos_t<PRECISE>(pP1[t0], &s1, &c1);
+    sincos_t<PRECISE>(pP2[t0], &s2, &c2);
     float cx[ND], cy[ND];
     disc_centres_n<ND>(P, x, y, s1, c1, s2, c2, cx, cy);
     const float tf = (float)t0;
 #pragma unroll
     for (int i = 0; i < kObsGroup; ++i) {
       float ox = o[i].x, oy = o[i].y;
-      if (MOVING) { const float2 w = vel[i]; ox = fmaf(tf, w.x, ox); oy = fmaf(tf, w.y, oy); }
+      if (i < NM) { const float2 w = vel[i]; ox = fmaf(tf, w.x, ox); oy = fmaf(tf, w.y, oy); }
 #pragma unroll
       for (int j = 0; j < ND; ++j) {
         const float dx = cx[j] - ox, dy = cy[j] - oy;
@@ -46,21 +69,29 @@ __device__ __forceinline__ double barrier_group(const DeviceParams& P, const flo
       }
     }
   }
+#pragma unroll 2
   for (int t = t0; t < t1; ++t) {
     // (x, y) of state t+1 from state t: the chain's own FMAs on the same operands
     const float a = P.dt * pV[t];
     x = fmaf(a, c1, x);
     y = fmaf(a, s1, y);
-    s1 = pS1[t + 1]; c1 = pC1[t + 1];
-    const float s2 = pS2[t + 1], c2 = pC2[t + 1];
+    const float psi1 = pP1[t + 1], psi2 = pP2[t + 1];
+    float s2, c2;
+    sincos_t<PRECISE>(psi1, &s1, &c1);
+    sincos_t<PRECISE>(psi2, &s2, &c2);
     float cx[ND], cy[ND];
     disc_centres_n<ND>(P, x, y, s1, c1, s2, c2, cx, cy);
+    if (TRACK) {
+      const State X{x, y, psi1, psi2};
+      if (PRECISE) track += (double)(goal_cost(P, X, g) + hitch_cost(P, X));
+      else track += (double)tracking_cost_fma(P, X, g);
+    }
     const float tf = (float)(t + 1);
     float pen = 0.0f;
 #pragma unroll
     for (int i = 0; i < kObsGroup; ++i) {
       float ox = o[i].x, oy = o[i].y;
-      if (MOVING) { const float2 w = vel[i]; ox = fmaf(tf, w.x, ox); oy = fmaf(tf, w.y, oy); }
+      if (i < NM) { const float2 w = vel[i]; ox = fmaf(tf, w.x, ox); oy = fmaf(tf, w.y, oy); }
 #pragma unroll
       for (int j = 0; j < ND; ++j) {
         const float dx = cx[j] - ox, dy = cy[j] - oy;
@@ -71,7 +102,19 @@ __device__ __forceinline__ double barrier_group(const DeviceParams& P, const flo
     }
     bar += (double)pen;
   }
-  return bar;
+  return GroupCost{track, bar};
+}
+
+// Dispatch on the number of moving obstacles in the group (block-uniform).
+template <bool PRECISE, int ND, bool TRACK>
+__device__ __forceinline__ GroupCost barrier_group_nm(int nm, const DeviceParams& P, const float* pV,
+                                                      const float* pP1, const float* pP2, const float4* obs,
+                                                      const float2* vel, float x, float y, int t0, int t1,
+                                                      float oma, const float4 g) {
+  if (nm <= 0) return barrier_group<PRECISE, ND, 0, TRACK>(P, pV, pP1, pP2, obs, vel, x, y, t0, t1, oma, g);
+  if (nm <= 2) return barrier_group<PRECISE, ND, 2, TRACK>(P, pV, pP1, pP2, obs, vel, x, y, t0, t1, oma, g);
+  if (nm <= 4) return barrier_group<PRECISE, ND, 4, TRACK>(P, pV, pP1, pP2, obs, vel, x, y, t0, t1, oma, g);
+  return barrier_group<PRECISE, ND, kObsGroup, TRACK>(P, pV, pP1, pP2, obs, vel, x, y, t0, t1, oma, g);
 }
 
 template <bool PRECISE, int ND>
@@ -87,6 +130,12 @@ rollout_cta(const __grid_constant__ DeviceParams P) {
   const int tile_last = min(tile_first + P.tiles_per_cta, P.total_tiles);
   int cur_scene = -1;
   int par = 0;          // parity of the running softmax state in CtaMisc
+  unsigned long long t_stamp = 0;
+  if (P.phase_ns != nullptr && tid == 0) {
+    for (int i = 0; i < kPhaseSlots; ++i) BRMPPI_SMEM(CtaMisc, P.off_misc)->phase_acc[i] = 0ull;
+    t_stamp = (unsigned long long)clock64();
+    BRMPPI_SMEM(CtaMisc, P.off_misc)->t_begin = global_ns();
+  }
 
   for (int tile = tile_first; tile < tile_last; ++tile) {
     const int scene = tile / P.tiles_per_scene;
@@ -162,7 +211,8 @@ rollout_cta(const __grid_constant__ DeviceParams P) {
       }
     }
 
-    // ---- phase A: noise, perturb + clamp (a1, a2) --------------------------------------------
+    BRMPPI_STAMP(0)
+    // ---- phase A: noise, perturb + clamp, effort cost (a1, a2) -------------------------------
     {
       const int TS = P.t_stride, T = P.T;
       const int R = kCtaThreads / S;
@@ -172,95 +222,99 @@ rollout_cta(const __grid_constant__ DeviceParams P) {
       const float2* sUnom = BRMPPI_SMEM(float2, P.off_unom);
       float* pV = BRMPPI_SMEM(float, P.off_planes) + s * TS;
       float* pD = pV + S * TS;
-      float* pS1 = pD + S * TS;
+      float* pP1 = pD + S * TS;
+      float effort = 0.0f;
       if (c < R) {
         for (int t = c; t < T; t += R) {
           const float2 u = sample_control<PRECISE>(P, sUnom[t], (uint32_t)t, n, (uint32_t)k, key0, key1);
           const float tan_d = tan_t<PRECISE>(u.y);
           pV[t] = u.x;
           pD[t] = u.y;
-          pS1[t + 1] = (P.dt * u.x) * P.inv_L1 * tan_d;          // dpsi1 of step t, parked at t+1
+          pP1[t + 1] = (P.dt * u.x) * P.inv_L1 * tan_d;          // dpsi1 of step t, parked at t+1
+          effort = fmaf(P.w_v * u.x, u.x, fmaf(P.w_delta * u.y, u.y, effort));
         }
       }
+      BRMPPI_SMEM(float, P.off_scratch)[tid] = effort;          // row partial of sample s
       if (c == 0) BRMPPI_SMEM(float, P.off_alpha)[s] = sample_alpha(P, n, (uint32_t)k, key0, key1);
     }
     __syncthreads();
+    BRMPPI_STAMP(1)
 
-    // ---- phase B: serial Euler chain of eq. (6), one sample per thread (a3), and the stage
-    //      costs that need the full state: goal, heading, effort, hitch, terminal (a6) ---------
+    // ---- phase B: serial Euler chain of eq. (6), one sample per thread (a3).  Only the psi2
+    //      recursion is a true chain; the thread also integrates psi1, x, y (short independent
+    //      dependency chains that fill its issue bubbles).  Everything else is left to phase C. ---
     if (c == 0) {
       const int TS = P.t_stride, T = P.T, L = P.chunk_len;
       const float* pV = BRMPPI_SMEM(float, P.off_planes) + s * TS;
-      const float* pD = pV + S * TS;
-      float* pS1 = BRMPPI_SMEM(float, P.off_planes) + (2 * S + s) * TS;
-      float* pC1 = pS1 + S * TS;
-      float* pS2 = pC1 + S * TS;
-      float* pC2 = pS2 + S * TS;
+      float* pP1 = BRMPPI_SMEM(float, P.off_planes) + (2 * S + s) * TS;
+      float* pP2 = pP1 + S * TS;
       float2* sXY = BRMPPI_SMEM(float2, P.off_xy);        // [C][S] chunk-start (x, y)
-      const CtaMisc* sM = BRMPPI_SMEM(CtaMisc, P.off_misc);
-      const float4 x0 = sM->x0, g = sM->g;
+      const float4 x0 = BRMPPI_SMEM(CtaMisc, P.off_misc)->x0;
       float x = 0.0f, y = 0.0f, psi1 = x0.z, psi2 = x0.w;
-      float s1, c1, s2, c2;
-      sincos_t<PRECISE>(psi1, &s1, &c1);
-      sincos_t<PRECISE>(psi2, &s2, &c2);
-      pS1[0] = s1; pC1[0] = c1; pS2[0] = s2; pC2[0] = c2;
-      double track = 0.0;
-      float effort = 0.0f;
+      pP1[0] = psi1;
+      pP2[0] = psi2;
+      float v = pV[0], b = pP1[1];
       for (int cc = 0, t = 0; t < T; ++cc) {
         sXY[cc * S + s] = make_float2(x, y);
         const int te = min(t + L, T);
         for (; t < te; ++t) {
-          const float v = pV[t], d = pD[t], b = pS1[t + 1];
+          // next step's inputs first: the loads do not wait behind this step's stores
+          const int tn = min(t + 1, T - 1);
+          const float v_next = pV[tn], b_next = pP1[tn + 1];
           const float a = P.dt * v;
-          const float sb = s1 * c2 - c1 * s2;            // sin(psi1 - psi2)
-          const float cb = fmaf(c1, c2, s1 * s2);        // cos(psi1 - psi2)
+          float s1, c1, sb, cb;
+          sincos_t<PRECISE>(psi1 - psi2, &sb, &cb);
+          sincos_t<PRECISE>(psi1, &s1, &c1);
           x = fmaf(a, c1, x);
           y = fmaf(a, s1, y);
           psi1 += b;
           psi2 = fmaf(a * P.inv_L2, sb, fmaf(-(b * P.Lh_over_L2), cb, psi2));
-          sincos_t<PRECISE>(psi1, &s1, &c1);
-          sincos_t<PRECISE>(psi2, &s2, &c2);
-          pS1[t + 1] = s1; pC1[t + 1] = c1; pS2[t + 1] = s2; pC2[t + 1] = c2;
-          const State X{x, y, psi1, psi2};
-          if (PRECISE) track += (double)(goal_cost(P, X, g) + hitch_cost(P, X));
-          else track += (double)tracking_cost_fma(P, X, g);
-          effort = fmaf(P.w_v * v, v, fmaf(P.w_delta * d, d, effort));
+          pP1[t + 1] = psi1;
+          pP2[t + 1] = psi2;
+          v = v_next; b = b_next;
         }
       }
-      const State X{x, y, psi1, psi2};
-      track += (double)(P.w_term * goal_cost(P, X, g));   // terminal cost r_N(x_N), eq. (7)
-      BRMPPI_SMEM(double, P.off_track)[s] = track + (double)effort;
-      if ((P.flags & BRMPPI_FLAG_WRITE_SAMPLES) && k < P.K)
-        reinterpret_cast<float4*>(P.XT)[(size_t)scene * P.K + k] = make_float4(x + x0.x, y + x0.y, psi1, psi2);
+      sXY[P.chunks * S + s] = make_float2(x, y);   // x_T
     }
     __syncthreads();
+    BRMPPI_STAMP(2)
 
-    // ---- phase C: barrier h and barrier-rate hinge (a4, a5) ----------------------------------
+    // ---- phase C: barrier, barrier-rate hinge, goal / heading / hitch cost (a4-a6) -----------
     if (c < P.chunks) {
       const int TS = P.t_stride, T = P.T;
       const int t0 = c * P.chunk_len, t1 = min(t0 + P.chunk_len, T);
       const CtaMisc* sM = BRMPPI_SMEM(CtaMisc, P.off_misc);
       const float* pV = BRMPPI_SMEM(float, P.off_planes) + s * TS;
-      const float* pS1 = pV + 2 * S * TS;
-      const float* pC1 = pS1 + S * TS;
-      const float* pS2 = pC1 + S * TS;
-      const float* pC2 = pS2 + S * TS;
+      const float* pP1 = pV + 2 * S * TS;
+      const float* pP2 = pP1 + S * TS;
       const float4* sObs = BRMPPI_SMEM(float4, P.off_obs);
       const float2* sVel = BRMPPI_SMEM(float2, P.off_vel);
       const float one_minus_alpha = 1.0f - BRMPPI_SMEM(float, P.off_alpha)[s];
+      const float4 g = sM->g;
       const int n_moving = sM->n_moving, n_groups = sM->n_groups;
       const float2 xy = BRMPPI_SMEM(float2, P.off_xy)[c * S + s];
-      double bar = 0.0;
-      for (int grp = 0; grp < n_groups; ++grp) {
-        const int ib = grp * kObsGroup;
-        if (ib < n_moving)
-          bar += barrier_group<ND, true>(P, pV, pS1, pC1, pS2, pC2, sObs + ib, sVel + ib, xy.x, xy.y, t0, t1, one_minus_alpha);
-        else
-          bar += barrier_group<ND, false>(P, pV, pS1, pC1, pS2, pC2, sObs + ib, sVel + ib, xy.x, xy.y, t0, t1, one_minus_alpha);
+      double track = 0.0, bar = 0.0;
+      {
+        const GroupCost gc = barrier_group_nm<PRECISE, ND, true>(n_moving, P, pV, pP1, pP2, sObs, sVel, xy.x, xy.y, t0, t1, one_minus_alpha, g);
+        track = gc.track; bar = gc.bar;
       }
-      BRMPPI_SMEM(double, P.off_cost)[c * S + s] = (double)P.w_bar * bar;
+      for (int grp = 1; grp < n_groups; ++grp) {
+        const int ib = grp * kObsGroup;
+        bar += barrier_group_nm<PRECISE, ND, false>(n_moving - ib, P, pV, pP1, pP2, sObs + ib, sVel + ib, xy.x, xy.y, t0, t1, one_minus_alpha, g).bar;
+      }
+      if (t1 == T) {   // terminal cost r_N(x_N), eq. (7); final state out
+        const float2 xT = BRMPPI_SMEM(float2, P.off_xy)[P.chunks * S + s];
+        const State X{xT.x, xT.y, pP1[T], pP2[T]};
+        track += (double)(P.w_term * goal_cost(P, X, g));
+        if ((P.flags & BRMPPI_FLAG_WRITE_SAMPLES) && k < P.K) {
+          const float4 x0 = sM->x0;
+          reinterpret_cast<float4*>(P.XT)[(size_t)scene * P.K + k] = make_float4(X.x + x0.x, X.y + x0.y, X.psi1, X.psi2);
+        }
+      }
+      BRMPPI_SMEM(double, P.off_cost)[c * S + s] = track + (double)P.w_bar * bar;
     }
     __syncthreads();
+    BRMPPI_STAMP(3)
 
     // ---- phase D: tile reduction against the running online-softmax state (a7) --------------
     double Sk = CUDART_INF;
@@ -270,8 +324,11 @@ rollout_cta(const __grid_constant__ DeviceParams P) {
       valid = (tid < S) && (k < P.K);
       if (valid) {
         const double* sCost = BRMPPI_SMEM(double, P.off_cost);
-        Sk = BRMPPI_SMEM(double, P.off_track)[s];
-        for (int cc = 0; cc < P.chunks; ++cc) Sk += sCost[cc * S + s];      // fixed order
+        const float* sEff = BRMPPI_SMEM(float, P.off_scratch);
+        float effort = 0.0f;
+        for (int r = 0; r < kCtaThreads / S; ++r) effort += sEff[r * S + s];  // fixed order
+        Sk = (double)effort;
+        for (int cc = 0; cc < P.chunks; ++cc) Sk += sCost[cc * S + s];
         if (P.flags & BRMPPI_FLAG_WRITE_SAMPLES) P.S[(size_t)scene * P.K + k] = (float)Sk;
       }
       finite = valid && (Sk == Sk) && (Sk < CUDART_INF) && (Sk > -CUDART_INF);
@@ -306,6 +363,7 @@ rollout_cta(const __grid_constant__ DeviceParams P) {
       if (tid == 0) { sM->m[par ^ 1] = m_new; sM->argmin[par ^ 1] = idx_new; }
     }
     __syncthreads();
+    BRMPPI_STAMP(4)
 
     // ---- phase E: running weighted control sums A[t] (a7) -----------------------------------
     {
@@ -353,6 +411,7 @@ rollout_cta(const __grid_constant__ DeviceParams P) {
     }
     par ^= 1;
     __syncthreads();
+    BRMPPI_STAMP(5)
   }
 
   // ---- partial of the last scene -> HBM -----------------------------------------------------
@@ -374,8 +433,18 @@ rollout_cta(const __grid_constant__ DeviceParams P) {
       P.part_A[((size_t)cur_scene * 2 * T + (2 * t + ch)) * Pn + slot] = sA[o];
     }
   }
+  if (P.phase_ns != nullptr && tid == 0) {
+    const CtaMisc* sM = BRMPPI_SMEM(CtaMisc, P.off_misc);
+    const unsigned long long now = (unsigned long long)clock64();
+    unsigned long long* out = P.phase_ns + (size_t)blockIdx.x * (kPhaseSlots + 2);
+    for (int i = 0; i < kPhaseSlots; ++i) out[i] = sM->phase_acc[i];
+    out[6] += now - t_stamp;            // partial to HBM
+    out[kPhaseSlots] = sM->t_begin;
+    out[kPhaseSlots + 1] = global_ns();
+  }
 }
 
+#undef BRMPPI_STAMP
 #undef BRMPPI_SMEM
 
 using CtaKernel = void (*)(const DeviceParams);
