@@ -145,6 +145,21 @@ def dist_setup(n_gpus):
     return dist.get_rank(), dist.get_world_size(), int(os.environ.get("LOCAL_RANK", "0")), dist
 
 
+def max_over_ranks(seconds, dist, device):
+    """Every rank's device time -> the slowest rank's (the job is as slow as its slowest GPU)."""
+    if dist is None:
+        return float(seconds)
+    import torch
+    t = torch.tensor([seconds], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_value(work_per_rank, world, seconds_max):
+    """Replicas: every rank processes `work_per_rank` units in at most `seconds_max`."""
+    return world * work_per_rank / seconds_max
+
+
 def run_reference(args):
     """The reference arm of this tier is the oracle, timed as it stands on the host cores."""
     rank = int(os.environ.get("RANK", "0"))
@@ -229,10 +244,7 @@ def run_ours(args):
     launches = solver.launch_count() - launches0
     step_ms = [a.elapsed_time(b) for a, b in ev]
     dev_s = sum(step_ms) * 1e-3
-    t = torch.tensor([dev_s], dtype=torch.float64, device=dev)
-    if dist is not None:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    dev_s_max = float(t.item())
+    dev_s_max = max_over_ranks(dev_s, dist, dev)
     work_per_rank = args.steps * p.K * p.T * p.n_iter
 
     # ---- end to end through the C ABI with host buffers (pinned), host clock
@@ -250,10 +262,7 @@ def run_ours(args):
         U = solver.get_controls()                            # synchronises; T*2 floats back
     barrier()
     e2e_s = time.perf_counter() - t0
-    te = torch.tensor([e2e_s], dtype=torch.float64, device=dev)
-    if dist is not None:
-        dist.all_reduce(te, op=dist.ReduceOp.MAX)
-    e2e_s_max = float(te.item())
+    e2e_s_max = max_over_ranks(e2e_s, dist, dev)
     h2d = 16 + 16 + 20 * n_obs + 4
     d2h = 8 * p.T
 
@@ -297,7 +306,7 @@ def run_ours(args):
         vn, sn, dn = oracle_throughput(sc, p, 8.0, cores, min(p.K, 8192))
         cpu = {"value": vn, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": dn,
                "value_1core": v1, "sample_1core": d1}
-    value = world * work_per_rank / dev_s_max
+    value = whole_job_value(work_per_rank, world, dev_s_max)
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": max(args.warmup, 3), "ms_per_step": dev_s_max / args.steps * 1e3,
@@ -305,7 +314,7 @@ def run_ours(args):
         "data": "synthetic", "config": workload_config(args.workload, sc, p, world),
         "solves_per_s": world * args.steps * p.n_iter / dev_s_max,
         "control_steps_per_s": world * args.steps / dev_s_max,
-        "e2e": {"value": world * work_per_rank / e2e_s_max, "unit": UNIT, "h2d_bytes_per_step": h2d,
+        "e2e": {"value": whole_job_value(work_per_rank, world, e2e_s_max), "unit": UNIT, "h2d_bytes_per_step": h2d,
                 "d2h_bytes_per_step": d2h, "control_steps_per_s": world * args.steps / e2e_s_max},
         "closed_loop": {"p50_ms": p50 * 1e3, "p99_ms": p99 * 1e3, "hz": 1.0 / p50,
                         "what": "brmppi_step: graph replay of solve + plant step + shift, host wall clock"},
