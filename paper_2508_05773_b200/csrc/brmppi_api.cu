@@ -275,7 +275,7 @@ int brmppi_create(const brmppi_params* p, void* dev_workspace, size_t workspace_
     d.tiles_per_cta = cp.tiles_per_cta;
     d.chunks = cp.chunks; d.chunk_len = cp.chunk_len; d.t_stride = cp.ts; d.obs_padded = cp.obs_padded;
     const CtaSmem ts = cta_smem_layout(d.T, cp.S_tile, cp.chunks, cp.ts, cp.obs_padded);
-    d.off_obs = (int)ts.obs; d.off_vel = (int)ts.vel; d.off_unom = (int)ts.unom; d.off_A = (int)ts.A;
+    d.off_obs = (int)ts.obs; d.off_vel = (int)ts.vel; d.off_raw = (int)ts.raw; d.off_A = (int)ts.A;
     d.off_scratch = (int)ts.scratch; d.off_w = (int)ts.w; d.off_alpha = (int)ts.alpha;
     d.off_cost = (int)ts.cost; d.off_xy = (int)ts.xy;
     d.off_planes = (int)ts.planes; d.off_misc = (int)ts.misc;
@@ -522,28 +522,38 @@ int brmppi_get_diag(brmppi_ctx* c, int scene, brmppi_diag* out) {
 
 int brmppi_time_kernels(brmppi_ctx* c, int reps, float out_ms[2]) {
   if (!c || !out_ms) return BRMPPI_ERR_NULL;
-  if (reps < 1) return BRMPPI_ERR_INVALID_ARG;
+  if (reps < 1 || reps > 4096) return BRMPPI_ERR_INVALID_ARG;
   int r = ready(c);
   if (r) return r;
-  cudaEvent_t ev[3];
-  for (int i = 0; i < 3; ++i) CU(cudaEventCreate(&ev[i]));
-  double acc[2] = {0.0, 0.0};
+  // All launches are enqueued back to back with an event between consecutive kernels and ONE
+  // synchronisation at the end: the stream never runs dry, so an interval is the kernel's device
+  // time plus the kernel-to-kernel gap, not the host's launch latency.  kWarm leading iterations
+  // are enqueued the same way and left out of the mean.
+  const int kWarm = 2, n_it = reps + kWarm, n_ev = 2 * n_it + 1;
+  cudaEvent_t* ev = (cudaEvent_t*)calloc((size_t)n_ev, sizeof(cudaEvent_t));
+  if (!ev) return BRMPPI_ERR_NULL;
   cudaError_t e = cudaSuccess;
-  for (int it = 0; it < reps && e == cudaSuccess && r == 0; ++it) {
-    e = cudaEventRecord(ev[0], c->stream);
-    if (e == cudaSuccess) r = launch_rollout(c);
-    if (e == cudaSuccess && r == 0) e = cudaEventRecord(ev[1], c->stream);
-    if (e == cudaSuccess && r == 0) r = launch_update(c);
-    if (e == cudaSuccess && r == 0) e = cudaEventRecord(ev[2], c->stream);
-    if (e == cudaSuccess && r == 0) e = cudaStreamSynchronize(c->stream);
-    float a = 0.f, b = 0.f;
-    if (e == cudaSuccess && r == 0) e = cudaEventElapsedTime(&a, ev[0], ev[1]);
-    if (e == cudaSuccess && r == 0) e = cudaEventElapsedTime(&b, ev[1], ev[2]);
-    acc[0] += a; acc[1] += b;
+  int made = 0;
+  for (; made < n_ev && e == cudaSuccess; ++made) e = cudaEventCreate(&ev[made]);
+  if (e == cudaSuccess) e = cudaEventRecord(ev[0], c->stream);
+  for (int it = 0; it < n_it && e == cudaSuccess && r == 0; ++it) {
+    r = launch_rollout(c);
+    if (r == 0) e = cudaEventRecord(ev[2 * it + 1], c->stream);
+    if (r == 0 && e == cudaSuccess) r = launch_update(c);
+    if (r == 0 && e == cudaSuccess) e = cudaEventRecord(ev[2 * it + 2], c->stream);
     c->launches += 2;
     c->n_host += 1;
   }
-  for (int i = 0; i < 3; ++i) cudaEventDestroy(ev[i]);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+  double acc[2] = {0.0, 0.0};
+  for (int it = kWarm; it < n_it && e == cudaSuccess && r == 0; ++it) {
+    float a = 0.f, b = 0.f;
+    e = cudaEventElapsedTime(&a, ev[2 * it], ev[2 * it + 1]);
+    if (e == cudaSuccess) e = cudaEventElapsedTime(&b, ev[2 * it + 1], ev[2 * it + 2]);
+    acc[0] += a; acc[1] += b;
+  }
+  for (int i = 0; i < made; ++i) cudaEventDestroy(ev[i]);
+  free(ev);
   if (r) return r;
   if (e != cudaSuccess) return cuda_fail(e);
   out_ms[0] = (float)(acc[0] / reps);

@@ -42,7 +42,7 @@ struct DeviceParams {
   int obs_padded;             // obstacle slots, a multiple of the group size
   // byte offsets of the shared-memory sections (host-computed, so that the device code
   // rematerialises a pointer with one add instead of keeping it in a register)
-  int off_obs, off_vel, off_unom, off_A, off_scratch, off_w, off_alpha, off_cost, off_xy,
+  int off_obs, off_vel, off_raw, off_A, off_scratch, off_w, off_alpha, off_cost, off_xy,
       off_planes, off_misc;
   // workspace pointers (DEVICE)
   float* state;               // [n_scenes][4]

@@ -157,8 +157,9 @@ rollout_cta(const __grid_constant__ DeviceParams P) {
     const int scene = tile / P.tiles_per_scene;
     const int k = (tile - scene * P.tiles_per_scene) * S + s;
 
-    if (scene != cur_scene) {
-      // ---- partial of the scene just finished -> HBM; then this scene's data -> shared -------
+    const bool new_scene = (scene != cur_scene);
+    if (new_scene) {
+      // ---- partial of the scene just finished -> HBM -------------------------------------------
       if (cur_scene >= 0) {
         const int Pn = P.n_partials, T = P.T;
         const CtaMisc* sM = BRMPPI_SMEM(CtaMisc, P.off_misc);
@@ -180,51 +181,21 @@ rollout_cta(const __grid_constant__ DeviceParams P) {
       }
       cur_scene = scene;
       par = 0;
-      {
-        const int T = P.T;
-        float4* sObs = BRMPPI_SMEM(float4, P.off_obs);
-        float2* sVel = BRMPPI_SMEM(float2, P.off_vel);
-        float2* sUnom = BRMPPI_SMEM(float2, P.off_unom);
-        float* sA = BRMPPI_SMEM(float, P.off_A);
-        CtaMisc* sM = BRMPPI_SMEM(CtaMisc, P.off_misc);
-        for (int i = tid; i < T; i += kCtaThreads) sUnom[i] = reinterpret_cast<const float2*>(P.U)[(size_t)scene * T + i];
-        for (int i = tid; i < 2 * T; i += kCtaThreads) sA[i] = 0.0f;
-        for (int i = tid; i < P.obs_padded; i += kCtaThreads) {   // null obstacles: weight 0
-          sObs[i] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
-          sVel[i] = make_float2(0.0f, 0.0f);
-        }
-        __syncthreads();
-        // every thread i < n_obs places obstacle i: moving obstacles first, static ones after
-        // (groups without a moving one skip the o(t) update); ranks by counting, no serial pass.
-        // Scene data in the vehicle-centred frame.
-        const float4 x0 = reinterpret_cast<const float4*>(P.state)[scene];
-        const int n_obs = P.n_obs[scene];
-        const float* ob = P.obstacles + (size_t)scene * P.max_obstacles * 5;
-        if (tid < n_obs) {
-          int nm = 0, before_m = 0, before_s = 0;
-          for (int j = 0; j < n_obs; ++j) {
-            const bool mj = (ob[5 * j + 3] != 0.0f || ob[5 * j + 4] != 0.0f);
-            nm += mj ? 1 : 0;
-            if (j < tid) { before_m += mj ? 1 : 0; before_s += mj ? 0 : 1; }
-          }
-          const bool moving = (ob[5 * tid + 3] != 0.0f || ob[5 * tid + 4] != 0.0f);
-          const int dst = moving ? before_m : nm + before_s;
-          const float rho = ob[5 * tid + 2] + P.disc_radius;
-          sObs[dst] = make_float4(ob[5 * tid + 0] - x0.x, ob[5 * tid + 1] - x0.y, 0.5f / (rho * rho), -(rho * rho));
-          sVel[dst] = make_float2(P.dt * ob[5 * tid + 3], P.dt * ob[5 * tid + 4]);
-          if (tid == 0) sM->n_moving = nm;
-        }
-        if (tid == 0) {
-          float4 g = reinterpret_cast<const float4*>(P.goal)[scene];
-          g.x -= x0.x; g.y -= x0.y;
-          sM->x0 = x0;
-          sM->g = g;
-          sM->m[0] = CUDART_INF; sM->argmin[0] = 0x7fffffff; sM->eta[0] = 0.0f; sM->w2[0] = 0.0f; sM->nonfinite[0] = 0;
-          if (n_obs == 0) sM->n_moving = 0;
-          sM->n_groups = n_obs > 0 ? (n_obs + kObsGroup - 1) / kObsGroup : 1;
-        }
-        __syncthreads();
+    }
+    // Scene data: the global loads are issued here and consumed after phase A, so their latency
+    // (HBM when the caller has flushed L2) hides behind the noise generation.
+    float4 x0_in = make_float4(0.f, 0.f, 0.f, 0.f), g_in = x0_in;
+    float ob_in[5] = {0.f, 0.f, 1.f, 0.f, 0.f};
+    int n_obs_in = 0;
+    if (new_scene) {
+      x0_in = reinterpret_cast<const float4*>(P.state)[scene];
+      n_obs_in = P.n_obs[scene];
+      if (tid < P.max_obstacles) {
+        const float* ob = P.obstacles + ((size_t)scene * P.max_obstacles + tid) * 5;
+#pragma unroll
+        for (int q = 0; q < 5; ++q) ob_in[q] = ob[q];
       }
+      if (tid == 0) g_in = reinterpret_cast<const float4*>(P.goal)[scene];
     }
 
     BRMPPI_STAMP(0)
@@ -235,14 +206,14 @@ rollout_cta(const __grid_constant__ DeviceParams P) {
       const uint32_t n = *P.counter;
       const uint32_t key0 = P.key0 + (uint32_t)scene;
       const uint32_t key1 = P.key1 + (key0 < P.key0 ? 1u : 0u);
-      const float2* sUnom = BRMPPI_SMEM(float2, P.off_unom);
+      const float2* Unom = reinterpret_cast<const float2*>(P.U) + (size_t)scene * T;   // read-only here
       float* pV = BRMPPI_SMEM(float, P.off_planes) + s * TS;
       float* pD = pV + S * TS;
       float* pP1 = pD + S * TS;
       float effort = 0.0f;
       if (c < R) {
         for (int t = c; t < T; t += R) {
-          const float2 u = sample_control<PRECISE>(P, sUnom[t], (uint32_t)t, n, (uint32_t)k, key0, key1);
+          const float2 u = sample_control<PRECISE>(P, __ldg(Unom + t), (uint32_t)t, n, (uint32_t)k, key0, key1);
           const float tan_d = tan_t<PRECISE>(u.y);
           pV[t] = u.x;
           pD[t] = u.y;
@@ -252,6 +223,24 @@ rollout_cta(const __grid_constant__ DeviceParams P) {
       }
       BRMPPI_SMEM(float, P.off_scratch)[tid] = effort;          // row partial of sample s
       if (c == 0) BRMPPI_SMEM(float, P.off_alpha)[s] = sample_alpha(P, n, (uint32_t)k, key0, key1);
+    }
+    if (new_scene) {
+      // stage the scene for warp kChainWarps, which sorts the obstacles while the chain runs
+      CtaMisc* sM = BRMPPI_SMEM(CtaMisc, P.off_misc);
+      float* sRaw = BRMPPI_SMEM(float, P.off_raw);
+      float* sA = BRMPPI_SMEM(float, P.off_A);
+      if (tid < P.max_obstacles) {
+#pragma unroll
+        for (int q = 0; q < 5; ++q) sRaw[5 * tid + q] = ob_in[q];
+      }
+      for (int i = tid; i < 2 * P.T; i += kCtaThreads) sA[i] = 0.0f;
+      if (tid == 0) {
+        g_in.x -= x0_in.x; g_in.y -= x0_in.y;          // vehicle-centred frame
+        sM->x0 = x0_in;
+        sM->g = g_in;
+        sM->n_obs = n_obs_in;
+        sM->m[0] = CUDART_INF; sM->argmin[0] = 0x7fffffff; sM->eta[0] = 0.0f; sM->w2[0] = 0.0f; sM->nonfinite[0] = 0;
+      }
     }
     __syncthreads();
     BRMPPI_STAMP(1)
@@ -291,6 +280,39 @@ rollout_cta(const __grid_constant__ DeviceParams P) {
         }
       }
       sXY[P.chunks * S + s] = make_float2(x, y);   // x_T
+    } else if (new_scene && warp == kChainWarps) {
+      // obstacle table for phase C, in the vehicle-centred frame: moving obstacles first, static
+      // ones after (groups without a moving one skip the o(t) update), null padding behind.
+      // Lane l ranks obstacles l and l + 32 by counting; the chain warps are busy meanwhile.
+      CtaMisc* sM = BRMPPI_SMEM(CtaMisc, P.off_misc);
+      const float* sRaw = BRMPPI_SMEM(float, P.off_raw);
+      float4* sObs = BRMPPI_SMEM(float4, P.off_obs);
+      float2* sVel = BRMPPI_SMEM(float2, P.off_vel);
+      const int n_obs = sM->n_obs;
+      const float4 x0 = sM->x0;
+      int nm = 0;
+      for (int j = 0; j < n_obs; ++j) nm += (sRaw[5 * j + 3] != 0.0f || sRaw[5 * j + 4] != 0.0f) ? 1 : 0;
+      for (int i = lane; i < P.obs_padded; i += 32) {
+        if (i < n_obs) {
+          int before_m = 0, before_s = 0;
+          for (int j = 0; j < i; ++j) {
+            const bool mj = (sRaw[5 * j + 3] != 0.0f || sRaw[5 * j + 4] != 0.0f);
+            before_m += mj ? 1 : 0; before_s += mj ? 0 : 1;
+          }
+          const bool moving = (sRaw[5 * i + 3] != 0.0f || sRaw[5 * i + 4] != 0.0f);
+          const int dst = moving ? before_m : nm + before_s;
+          const float rho = sRaw[5 * i + 2] + P.disc_radius;
+          sObs[dst] = make_float4(sRaw[5 * i + 0] - x0.x, sRaw[5 * i + 1] - x0.y, 0.5f / (rho * rho), -(rho * rho));
+          sVel[dst] = make_float2(P.dt * sRaw[5 * i + 3], P.dt * sRaw[5 * i + 4]);
+        } else {                                        // null obstacle: weight 0
+          sObs[i] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+          sVel[i] = make_float2(0.0f, 0.0f);
+        }
+      }
+      if (lane == 0) {
+        sM->n_moving = nm;
+        sM->n_groups = n_obs > 0 ? (n_obs + kObsGroup - 1) / kObsGroup : 1;
+      }
     }
     __syncthreads();
     BRMPPI_STAMP(2)
@@ -405,9 +427,17 @@ rollout_cta(const __grid_constant__ DeviceParams P) {
         if (g < G) {
           const int ch = o >= T ? 1 : 0, t = o - ch * T;
           const float* plane = sV + ch * S * TS + t;
-          float acc = 0.0f;
-          for (int ss = g; ss < S; ss += G) acc = fmaf(sW[ss], plane[ss * TS], acc);
-          sScr[tid] = acc;
+          // four independent partial sums: the shared-memory loads of consecutive samples overlap
+          float a0 = 0.0f, a1 = 0.0f, a2 = 0.0f, a3 = 0.0f;
+          int ss = g;
+          for (; ss + 3 * G < S; ss += 4 * G) {
+            a0 = fmaf(sW[ss], plane[ss * TS], a0);
+            a1 = fmaf(sW[ss + G], plane[(ss + G) * TS], a1);
+            a2 = fmaf(sW[ss + 2 * G], plane[(ss + 2 * G) * TS], a2);
+            a3 = fmaf(sW[ss + 3 * G], plane[(ss + 3 * G) * TS], a3);
+          }
+          for (; ss < S; ss += G) a0 = fmaf(sW[ss], plane[ss * TS], a0);
+          sScr[tid] = (a0 + a1) + (a2 + a3);
         }
         __syncthreads();
         if (tid < n_out) {
