@@ -335,6 +335,53 @@ def dram_traffic_from_profile():
         return None
 
 
+def run_phases(args):
+    """In-kernel phase times of one rollout launch (BRMPPI_FLAG_PHASE_TIMING), one JSON line."""
+    import torch  # noqa: F401
+    from paper_2508_05773_b200 import brmppi as B
+    sc, p = workload(args.workload)
+    s = B.Solver(p.with_(n_iter=1), 1, max(len(sc.obstacles), 1), B.FLAG_PHASE_TIMING)
+    s.set_scene(sc)
+    for _ in range(5):
+        s.solve()
+    s.synchronize()
+    print(json.dumps({"workload": args.workload, "K": p.K, "T": p.T, "n_obstacles": len(sc.obstacles),
+                      "phase_us": s.get_phase_times()}))
+    s.close()
+
+
+def run_sweep(args):
+    """BASELINE.json configs[4]: K x T x obstacle-count sweep and the 64-scene batch; one JSON line
+    per point with the rollout kernel's device time and roofline fraction."""
+    from paper_2508_05773_b200 import brmppi as B
+    peak = N_SMS * ISSUE_PER_CLK_PER_SM * float(measured_peaks().get("sm_max_mhz", SM_MAX_MHZ_FALLBACK)) * 1e6
+
+    def point(name, scs, p, n_scenes):
+        n_obs = len(scs[0].obstacles)
+        s = B.Solver(p, n_scenes, max(n_obs, 1), 0)
+        for i, sc in enumerate(scs):
+            s.set_scene(sc, i)
+        for _ in range(3):
+            s.solve()
+        s.synchronize()
+        ms_roll, ms_upd = s.time_kernels(20)
+        s.close()
+        work = n_scenes * p.K * p.T
+        instr = algorithmic_instr_per_sample_step(n_obs, len(p.discs))
+        print(json.dumps({"point": name, "K": p.K, "T": p.T, "n_obstacles": n_obs, "n_scenes": n_scenes,
+                          "rollout_us": ms_roll * 1e3, "update_us": ms_upd * 1e3,
+                          "sample_steps_per_s": work / (ms_roll * 1e-3),
+                          "frac": work * instr / (ms_roll * 1e-3) / peak}), flush=True)
+
+    for K in (1024, 16384, 131072, 1048576):
+        for T in (50, 100):
+            for n_obs in (8, 32, 64):
+                sc = scenes.scene_static(0, n_obs, K=K, T=T)
+                point("sweep", [sc], sc.params, 1)
+    batch = scenes.scene_batch(64, 16384, 80)
+    point("batch64", batch, batch[0].params.with_(seed=0), 64)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -342,8 +389,14 @@ def main():
     ap.add_argument("--warmup", type=int, default=20)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="cfg2", choices=["cfg0", "cfg1", "cfg2", "cfg3"])
+    ap.add_argument("--phases", action="store_true", help="print the rollout kernel's in-kernel phase times")
+    ap.add_argument("--sweep", action="store_true", help="run BASELINE.json configs[4] (sweep + 64-scene batch)")
     args = ap.parse_args()
-    if args.impl == "reference":
+    if args.phases:
+        run_phases(args)
+    elif args.sweep:
+        run_sweep(args)
+    elif args.impl == "reference":
         run_reference(args)
     else:
         run_ours(args)
