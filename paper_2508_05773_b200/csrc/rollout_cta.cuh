@@ -39,7 +39,10 @@
 
 namespace brmppi {
 
-constexpr int kCtaThreads = 512;
+#ifndef BRMPPI_CTA_THREADS
+#define BRMPPI_CTA_THREADS 512
+#endif
+constexpr int kCtaThreads = BRMPPI_CTA_THREADS;
 constexpr int kChainWarps = 4;                      // one per warp scheduler
 constexpr int kMaxTileSamples = kChainWarps * 32;   // 128
 constexpr int kObsGroup = 8;                        // obstacles whose h_t are held in registers at a time
