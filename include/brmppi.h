@@ -73,6 +73,8 @@ typedef struct { int body; float offset; } brmppi_disc;
 
 #define BRMPPI_FLAG_PHASE_TIMING 8u     /* persistent kernel: CTAs record nanoseconds per phase
                                           (globaltimer); read with brmppi_get_phase_times       */
+#define BRMPPI_FLAG_NO_CULL 16u         /* evaluate every (obstacle, disc, step) even where the
+                                          hinge is provably zero; same results  */
 
 typedef struct {
   int K;              /* samples per iteration, >= 1                                            */

@@ -15,6 +15,7 @@ FLAG_WRITE_SAMPLES = 1
 FLAG_PRECISE_MATH = 2
 FLAG_KERNEL_THREAD_PER_SAMPLE = 4
 FLAG_PHASE_TIMING = 8
+FLAG_NO_CULL = 16
 
 OK = 0
 ERR_NULL, ERR_INVALID_ARG, ERR_WORKSPACE_TOO_SMALL, ERR_TOO_MANY_OBSTACLES = -1, -2, -3, -4

@@ -66,7 +66,8 @@ bool params_valid(const brmppi_params* p) {
   if (p->delta_min <= -1.5f || p->delta_max >= 1.5f) return false;   // tan(delta) must stay finite
   if (p->alpha_lo > p->alpha_hi) return false;
   const unsigned known = BRMPPI_FLAG_WRITE_SAMPLES | BRMPPI_FLAG_PRECISE_MATH |
-                         BRMPPI_FLAG_KERNEL_THREAD_PER_SAMPLE | BRMPPI_FLAG_PHASE_TIMING;
+                         BRMPPI_FLAG_KERNEL_THREAD_PER_SAMPLE | BRMPPI_FLAG_PHASE_TIMING |
+                         BRMPPI_FLAG_NO_CULL;
   if (p->flags & ~known) return false;
   return true;
 }
@@ -258,6 +259,20 @@ int brmppi_create(const brmppi_params* p, void* dev_workspace, size_t workspace_
   d.n_discs = p->n_discs;
   for (int j = 0; j < p->n_discs; ++j) { d.disc_body[j] = p->discs[j].body; d.disc_offset[j] = p->discs[j].offset; }
   d.disc_radius = p->disc_radius;
+  {
+    // Speed bound of every disc centre under the Euler map of eq. (6): the rear
+    // axle moves |v| dt per step, headings turn by at most |v| dt tan|delta| / L1 (tractor) and
+    // (|v| dt / L2)(1 + |Lh| tan|delta| / L1) (trailer), and |e(psi') - e(psi)| <= |psi' - psi|.
+    const double V = std::fmax(std::fabs((double)p->v_min), std::fabs((double)p->v_max));
+    const double td = std::tan(std::fmax(std::fabs((double)p->delta_min), std::fabs((double)p->delta_max)));
+    const double w1 = V * td / p->L1, w2 = V / p->L2 * (1.0 + std::fabs((double)p->Lh) * td / p->L1);
+    const double v_hitch = V + std::fabs((double)p->Lh) * w1;
+    for (int j = 0; j < p->n_discs; ++j) {
+      const double a = p->discs[j].offset;
+      const double sp = p->discs[j].body == 0 ? V + std::fabs(a - p->Lh) * w1 : v_hitch + std::fabs(a) * w2;
+      d.disc_speed[j] = (float)(1.001 * sp);
+    }
+  }
   d.dt = p->dt; d.inv_L1 = 1.0f / p->L1; d.inv_L2 = 1.0f / p->L2; d.Lh = p->Lh;
   d.Lh_over_L1 = p->Lh / p->L1; d.Lh_over_L2 = p->Lh / p->L2;
   d.v_min = p->v_min; d.v_max = p->v_max; d.delta_min = p->delta_min; d.delta_max = p->delta_max;
@@ -275,7 +290,7 @@ int brmppi_create(const brmppi_params* p, void* dev_workspace, size_t workspace_
     d.tiles_per_cta = cp.tiles_per_cta;
     d.chunks = cp.chunks; d.chunk_len = cp.chunk_len; d.t_stride = cp.ts; d.obs_padded = cp.obs_padded;
     const CtaSmem ts = cta_smem_layout(d.T, cp.S_tile, cp.chunks, cp.ts, cp.obs_padded);
-    d.off_obs = (int)ts.obs; d.off_vel = (int)ts.vel; d.off_raw = (int)ts.raw; d.off_A = (int)ts.A;
+    d.off_obs = (int)ts.obs; d.off_vel = (int)ts.vel; d.off_spd = (int)ts.spd; d.off_raw = (int)ts.raw; d.off_A = (int)ts.A;
     d.off_scratch = (int)ts.scratch; d.off_w = (int)ts.w; d.off_alpha = (int)ts.alpha;
     d.off_cost = (int)ts.cost; d.off_xy = (int)ts.xy;
     d.off_planes = (int)ts.planes; d.off_misc = (int)ts.misc;

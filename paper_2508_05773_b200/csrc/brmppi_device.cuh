@@ -24,6 +24,7 @@ struct DeviceParams {
   int disc_body[kMaxDiscs];
   float disc_offset[kMaxDiscs];
   float disc_radius;
+  float disc_speed[kMaxDiscs];   // upper bound on the speed of each disc centre, m/s (culling)
   float dt, inv_L1, inv_L2, Lh, Lh_over_L1, Lh_over_L2;
   float v_min, v_max, delta_min, delta_max, sigma_v, sigma_delta;
   float alpha_lo, alpha_span;
@@ -42,7 +43,7 @@ struct DeviceParams {
   int obs_padded;             // obstacle slots, a multiple of the group size
   // byte offsets of the shared-memory sections (host-computed, so that the device code
   // rematerialises a pointer with one add instead of keeping it in a register)
-  int off_obs, off_vel, off_raw, off_A, off_scratch, off_w, off_alpha, off_cost, off_xy,
+  int off_obs, off_vel, off_spd, off_raw, off_A, off_scratch, off_w, off_alpha, off_cost, off_xy,
       off_planes, off_misc;
   // workspace pointers (DEVICE)
   float* state;               // [n_scenes][4]

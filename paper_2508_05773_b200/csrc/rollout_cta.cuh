@@ -65,7 +65,7 @@ struct CtaMisc {            // lives in the "misc" section
 };
 
 struct CtaSmem {
-  size_t obs, vel, raw, A, scratch, w, alpha, cost, xy, planes, misc, total;
+  size_t obs, vel, spd, raw, A, scratch, w, alpha, cost, xy, planes, misc, total;
 };
 
 // Shared-memory carve-up (host only: the kernel gets the byte offsets through DeviceParams, so
@@ -76,6 +76,7 @@ inline CtaSmem cta_smem_layout(int T, int S, int chunks, int ts, int obs_padded)
   auto take = [&](size_t b) { size_t o = off; off = (off + b + 15) / 16 * 16; return o; };
   L.obs = take(sizeof(float4) * (size_t)obs_padded);
   L.vel = take(sizeof(float2) * (size_t)obs_padded);
+  L.spd = take(sizeof(float) * (size_t)obs_padded);       // obstacle displacement per step
   L.raw = take(sizeof(float) * 5 * (size_t)obs_padded);   // obstacles as given, before sorting
   L.A = take(sizeof(float) * 2 * (size_t)T);
   L.scratch = take(sizeof(float) * kCtaThreads);

@@ -56,6 +56,7 @@ template <bool PRECISE, int ND, int NM, bool TRACK>
 __device__ __forceinline__ GroupCost barrier_group(const DeviceParams& P, const float* __restrict__ pV,
                                                    const float* __restrict__ pP1, const float* __restrict__ pP2,
                                                    const float4* __restrict__ obs, const float2* __restrict__ vel,
+                                                   const float* __restrict__ spd,
                                                    float x, float y, int t0, int t1, float one_minus_alpha,
                                                    const float4 g) {
   double bar = 0.0, track = 0.0;
@@ -82,6 +83,33 @@ __device__ __forceinline__ GroupCost barrier_group(const DeviceParams& P, const 
       }
     }
   }
+  // Exact culling: obstacle i cannot violate the rate condition anywhere in this
+  // chunk if every disc starts farther from it than d_crit plus what the two can close in the
+  // chunk; its hinge terms are then all exactly +0 and it is skipped.  The mask is the union over
+  // the warp's samples, so the skip is a uniform branch.
+  unsigned active = 0xffu;
+  if (!(P.flags & BRMPPI_FLAG_NO_CULL)) {
+    const float alpha = 1.0f - one_minus_alpha;
+    const float inv_alpha = 1.0f / alpha;
+    const float steps = (float)(t1 - t0);
+    active = 0u;
+#pragma unroll
+    for (int i = 0; i < kObsGroup; ++i) {
+      const float rho2 = -o[i].w;
+      bool act = false;
+#pragma unroll
+      for (int j = 0; j < ND; ++j) {
+        const float dl = fmaf(P.dt, P.disc_speed[j], spd[i]);   // relative displacement per step
+        const float d0 = sqrtf(fmaxf(gprev[i][j] + rho2, 0.0f));
+        const float d_crit = (dl + sqrtf(fmaf(one_minus_alpha * dl, dl, alpha * alpha * rho2))) * inv_alpha;
+        act = act || !(d0 - steps * dl >= fmaf(1.02f, d_crit, 0.05f));
+      }
+      if (o[i].z == 0.0f) act = false;          // null obstacle: weight 0
+      active |= act ? (1u << i) : 0u;
+    }
+    active = __reduce_or_sync(__activemask(), active);
+  }
+  if (!TRACK && active == 0u) return GroupCost{0.0, 0.0};
 #pragma unroll kCostUnroll
   for (int t = t0; t < t1; ++t) {
     // (x, y) of state t+1 from state t: the chain's own FMAs on the same operands
@@ -103,6 +131,7 @@ __device__ __forceinline__ GroupCost barrier_group(const DeviceParams& P, const 
     float pen = 0.0f;
 #pragma unroll
     for (int i = 0; i < kObsGroup; ++i) {
+      if (!(active & (1u << i))) continue;      // warp-uniform
       float ox = o[i].x, oy = o[i].y;
       if (i < NM) { const float2 w = vel[i]; ox = fmaf(tf, w.x, ox); oy = fmaf(tf, w.y, oy); }
       float Pi = 0.0f;
@@ -125,12 +154,12 @@ __device__ __forceinline__ GroupCost barrier_group(const DeviceParams& P, const 
 template <bool PRECISE, int ND, bool TRACK>
 __device__ __forceinline__ GroupCost barrier_group_nm(int nm, const DeviceParams& P, const float* pV,
                                                       const float* pP1, const float* pP2, const float4* obs,
-                                                      const float2* vel, float x, float y, int t0, int t1,
-                                                      float oma, const float4 g) {
-  if (nm <= 0) return barrier_group<PRECISE, ND, 0, TRACK>(P, pV, pP1, pP2, obs, vel, x, y, t0, t1, oma, g);
-  if (nm <= 2) return barrier_group<PRECISE, ND, 2, TRACK>(P, pV, pP1, pP2, obs, vel, x, y, t0, t1, oma, g);
-  if (nm <= 4) return barrier_group<PRECISE, ND, 4, TRACK>(P, pV, pP1, pP2, obs, vel, x, y, t0, t1, oma, g);
-  return barrier_group<PRECISE, ND, kObsGroup, TRACK>(P, pV, pP1, pP2, obs, vel, x, y, t0, t1, oma, g);
+                                                      const float2* vel, const float* spd, float x, float y,
+                                                      int t0, int t1, float oma, const float4 g) {
+  if (nm <= 0) return barrier_group<PRECISE, ND, 0, TRACK>(P, pV, pP1, pP2, obs, vel, spd, x, y, t0, t1, oma, g);
+  if (nm <= 2) return barrier_group<PRECISE, ND, 2, TRACK>(P, pV, pP1, pP2, obs, vel, spd, x, y, t0, t1, oma, g);
+  if (nm <= 4) return barrier_group<PRECISE, ND, 4, TRACK>(P, pV, pP1, pP2, obs, vel, spd, x, y, t0, t1, oma, g);
+  return barrier_group<PRECISE, ND, kObsGroup, TRACK>(P, pV, pP1, pP2, obs, vel, spd, x, y, t0, t1, oma, g);
 }
 
 template <bool PRECISE, int ND>
@@ -288,6 +317,7 @@ rollout_cta(const __grid_constant__ DeviceParams P) {
       const float* sRaw = BRMPPI_SMEM(float, P.off_raw);
       float4* sObs = BRMPPI_SMEM(float4, P.off_obs);
       float2* sVel = BRMPPI_SMEM(float2, P.off_vel);
+      float* sSpd = BRMPPI_SMEM(float, P.off_spd);
       const int n_obs = sM->n_obs;
       const float4 x0 = sM->x0;
       int nm = 0;
@@ -304,9 +334,12 @@ rollout_cta(const __grid_constant__ DeviceParams P) {
           const float rho = sRaw[5 * i + 2] + P.disc_radius;
           sObs[dst] = make_float4(sRaw[5 * i + 0] - x0.x, sRaw[5 * i + 1] - x0.y, 0.5f / (rho * rho), -(rho * rho));
           sVel[dst] = make_float2(P.dt * sRaw[5 * i + 3], P.dt * sRaw[5 * i + 4]);
+          // displacement per step, rounded up (culling bound)
+          sSpd[dst] = 1.0001f * P.dt * sqrtf(fmaf(sRaw[5 * i + 3], sRaw[5 * i + 3], sRaw[5 * i + 4] * sRaw[5 * i + 4]));
         } else {                                        // null obstacle: weight 0
           sObs[i] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
           sVel[i] = make_float2(0.0f, 0.0f);
+          sSpd[i] = 0.0f;
         }
       }
       if (lane == 0) {
@@ -327,18 +360,19 @@ rollout_cta(const __grid_constant__ DeviceParams P) {
       const float* pP2 = pP1 + S * TS;
       const float4* sObs = BRMPPI_SMEM(float4, P.off_obs);
       const float2* sVel = BRMPPI_SMEM(float2, P.off_vel);
+      const float* sSpd = BRMPPI_SMEM(float, P.off_spd);
       const float one_minus_alpha = 1.0f - BRMPPI_SMEM(float, P.off_alpha)[s];
       const float4 g = sM->g;
       const int n_moving = sM->n_moving, n_groups = sM->n_groups;
       const float2 xy = BRMPPI_SMEM(float2, P.off_xy)[c * S + s];
       double track = 0.0, bar = 0.0;
       {
-        const GroupCost gc = barrier_group_nm<PRECISE, ND, true>(n_moving, P, pV, pP1, pP2, sObs, sVel, xy.x, xy.y, t0, t1, one_minus_alpha, g);
+        const GroupCost gc = barrier_group_nm<PRECISE, ND, true>(n_moving, P, pV, pP1, pP2, sObs, sVel, sSpd, xy.x, xy.y, t0, t1, one_minus_alpha, g);
         track = gc.track; bar = gc.bar;
       }
       for (int grp = 1; grp < n_groups; ++grp) {
         const int ib = grp * kObsGroup;
-        bar += barrier_group_nm<PRECISE, ND, false>(n_moving - ib, P, pV, pP1, pP2, sObs + ib, sVel + ib, xy.x, xy.y, t0, t1, one_minus_alpha, g).bar;
+        bar += barrier_group_nm<PRECISE, ND, false>(n_moving - ib, P, pV, pP1, pP2, sObs + ib, sVel + ib, sSpd + ib, xy.x, xy.y, t0, t1, one_minus_alpha, g).bar;
       }
       if (t1 == T) {   // terminal cost r_N(x_N), eq. (7); final state out
         const float2 xT = BRMPPI_SMEM(float2, P.off_xy)[P.chunks * S + s];

@@ -375,3 +375,33 @@ def test_error_codes(B):
     assert L.brmppi_create(C.byref(bad), C.c_void_p(ptr), 1 << 30, None, C.byref(ctx)) == B.ERR_INVALID_ARG
     assert L.brmppi_create(None, C.c_void_p(ptr), 1 << 30, None, C.byref(ctx)) == B.ERR_NULL
     assert B.strerror(B.ERR_TOO_MANY_OBSTACLES) == "too many obstacles"
+
+
+# ------------------------------------------------------------------------------------------
+# exact culling of obstacles whose hinge is provably zero
+# ------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("make", [lambda: scenes.scene_cfg2(0), lambda: scenes.scene_cfg2(5),
+                                  lambda: scenes.scene_static(7, 64, K=2048, T=100),
+                                  lambda: scenes.scene_cfg0(3)], ids=["cfg2a", "cfg2b", "static64", "cfg0"])
+def test_culling_is_bit_exact(B, make):
+    sc = make()
+    p = sc.params.with_(K=min(sc.params.K, 4096), n_iter=2)
+    a = gpu_solve(B, sc, p, 0)
+    b = gpu_solve(B, sc, p, B.FLAG_NO_CULL)
+    for key in ("S", "XT", "U"):
+        assert np.array_equal(a[key], b[key]), key
+    assert a["diag"] == b["diag"]
+
+
+def test_culling_keeps_close_fast_obstacles(B, O):
+    """Obstacles next to the vehicle, fast pedestrians, small alpha: nothing may be culled wrongly."""
+    sc = scenes.scene_cfg2(6)
+    obs = sc.obstacles.copy()
+    obs[:4, 0:2] = sc.x0[:2] + np.array([[4.0, 3.0], [-6.0, 2.5], [9.0, -4.0], [-12.0, 5.0]])
+    obs[4:, 3:5] *= 3.0                                     # 4.5 m/s pedestrians
+    sc2 = scenes.Scene(sc.x0, sc.goal, obs.astype(np.float32).astype(np.float64), sc.params)
+    p = sc.params.with_(K=2048, n_iter=1, alpha_lo=0.02, alpha_hi=0.3)
+    a = gpu_solve(B, sc2, p, 0)
+    b = gpu_solve(B, sc2, p, B.FLAG_NO_CULL)
+    assert np.array_equal(a["S"], b["S"]) and np.array_equal(a["U"], b["U"])
+    check_against_oracle(O, a, sc2, p)
