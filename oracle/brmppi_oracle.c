@@ -50,14 +50,17 @@ static void seed_key(uint64_t seed, uint32_t key[2]) {
   key[1] = (uint32_t)(seed >> 32);
 }
 
-/* PAPER.md:89 "draws S independent noise rollouts w ~ N(0, Sigma_w)"; reading 5: Box-Muller on
- * two 23-bit uniforms of the Philox block with counter (t, n, k, 0). */
+/* PAPER.md:89 "draws S independent noise rollouts w ~ N(0, Sigma_w)"; readings 5 and 6: Box-Muller on
+ * two 23-bit uniforms.  One Philox block, counter (t >> 1, n, k, 0), serves the two steps 2m and
+ * 2m + 1: words (0, 1) for the even step, words (2, 3) for the odd one. */
 void orc_normals(uint64_t seed, uint32_t n, uint32_t k, uint32_t t, double z[2]) {
-  uint32_t key[2], ctr[4] = {t, n, k, 0u}, w[4];
+  uint32_t key[2], ctr[4] = {t >> 1, n, k, 0u}, w[4];
   seed_key(seed, key);
   orc_philox4x32_10(ctr, key, w);
-  double u1 = 1.0 - orc_uniform(w[0]); /* in (0, 1] */
-  double u2 = orc_uniform(w[1]);       /* in [0, 1) */
+  const uint32_t wa = (t & 1u) ? w[2] : w[0];
+  const uint32_t wb = (t & 1u) ? w[3] : w[1];
+  double u1 = 1.0 - orc_uniform(wa); /* in (0, 1] */
+  double u2 = orc_uniform(wb);       /* in [0, 1) */
   double r = sqrt(-2.0 * log(u1));
   z[0] = r * cos(2.0 * M_PI * u2);
   z[1] = r * sin(2.0 * M_PI * u2);

@@ -63,8 +63,9 @@ void orc_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t ou
 /* f(w) = (w >> 9) * 2^-23, in [0,1), exact in fp32 and fp64.  SURVEY §8(c) reading 5. */
 double orc_uniform(uint32_t w);
 
-/* The two standard normals of (seed, n, k, t): Philox ctr = (t, n, k, 0), words 0,1,
- * Box-Muller with u1 = 1 - f(w0), u2 = f(w1).  z[0] -> speed channel, z[1] -> steering. */
+/* The two standard normals of (seed, n, k, t): Philox ctr = (t >> 1, n, k, 0), words (0, 1) for
+ * even t and (2, 3) for odd t (readings 5, 6); Box-Muller with u1 = 1 - f(wa), u2 = f(wb).
+ * z[0] -> speed channel, z[1] -> steering. */
 void orc_normals(uint64_t seed, uint32_t n, uint32_t k, uint32_t t, double z[2]);
 
 /* alpha_k of (seed, n, k): Philox ctr = (0, n, k, 1), word 0. */

@@ -107,14 +107,12 @@ __device__ __forceinline__ float one_minus_uniform23(uint32_t w) {
   return 2.0f - __uint_as_float(0x3f800000u | (w >> 9));
 }
 
-// Box-Muller pair for (k, t) of iteration n (reading 5).  z.x -> speed channel,
-// z.y -> steering channel.  PRECISE selects libdevice logf/sincosf instead of MUFU lg2/sin/cos.
+// Box-Muller on two Philox words (reading 5).  z.x -> speed channel, z.y -> steering
+// channel.  PRECISE selects libdevice logf/sincospif instead of MUFU lg2/sin/cos.
 template <bool PRECISE>
-__device__ __forceinline__ float2 normal_pair(uint32_t t, uint32_t n, uint32_t k, uint32_t key0,
-                                              uint32_t key1) {
-  const uint4 w = philox4x32_10(t, n, k, 0u, key0, key1);
-  const float u1 = one_minus_uniform23(w.x);   // (0, 1], exact
-  const float u2 = uniform23(w.y);          // [0, 1)
+__device__ __forceinline__ float2 box_muller(uint32_t wa, uint32_t wb) {
+  const float u1 = one_minus_uniform23(wa);   // (0, 1], exact
+  const float u2 = uniform23(wb);             // [0, 1)
   float r, s, c;
   if (PRECISE) {
     r = sqrtf(-2.0f * logf(u1));
@@ -130,6 +128,15 @@ __device__ __forceinline__ float2 normal_pair(uint32_t t, uint32_t n, uint32_t k
     c = -fast_cos(a);
   }
   return make_float2(r * c, r * s);
+}
+
+// The normals of step t of sample k in iteration n: one Philox block, counter (t >> 1, n, k, 0),
+// serves steps 2m (words 0, 1) and 2m + 1 (words 2, 3) -- readings 5 and 6.
+template <bool PRECISE>
+__device__ __forceinline__ float2 normal_pair(uint32_t t, uint32_t n, uint32_t k, uint32_t key0,
+                                              uint32_t key1) {
+  const uint4 w = philox4x32_10(t >> 1, n, k, 0u, key0, key1);
+  return (t & 1u) ? box_muller<PRECISE>(w.z, w.w) : box_muller<PRECISE>(w.x, w.y);
 }
 
 // alpha_k ~ U[alpha_lo, alpha_hi), Philox counter (0, n, k, 1) word 0 (reading 8).
@@ -150,6 +157,19 @@ __device__ __forceinline__ float2 sample_control(const DeviceParams& P, float2 u
   v = fminf(fmaxf(v, P.v_min), P.v_max);
   d = fminf(fmaxf(d, P.delta_min), P.delta_max);
   return make_float2(v, d);
+}
+
+// Both steps of pair m (steps 2m and 2m + 1) from ONE Philox block: what the persistent kernel uses.
+template <bool PRECISE>
+__device__ __forceinline__ void sample_control_pair(const DeviceParams& P, float2 u_nom0, float2 u_nom1,
+                                                    uint32_t m, uint32_t n, uint32_t k, uint32_t key0,
+                                                    uint32_t key1, float2* u0, float2* u1) {
+  const uint4 w = philox4x32_10(m, n, k, 0u, key0, key1);
+  const float2 z0 = box_muller<PRECISE>(w.x, w.y), z1 = box_muller<PRECISE>(w.z, w.w);
+  u0->x = fminf(fmaxf(fmaf(P.sigma_v, z0.x, u_nom0.x), P.v_min), P.v_max);
+  u0->y = fminf(fmaxf(fmaf(P.sigma_delta, z0.y, u_nom0.y), P.delta_min), P.delta_max);
+  u1->x = fminf(fmaxf(fmaf(P.sigma_v, z1.x, u_nom1.x), P.v_min), P.v_max);
+  u1->y = fminf(fmaxf(fmaf(P.sigma_delta, z1.y, u_nom1.y), P.delta_min), P.delta_max);
 }
 
 template <bool PRECISE>

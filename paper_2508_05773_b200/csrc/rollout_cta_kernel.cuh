@@ -18,20 +18,6 @@ namespace brmppi {
 #define BRMPPI_C_UNROLL 2
 #endif
 constexpr int kCostUnroll = BRMPPI_C_UNROLL;
-// unroll factor of the noise loop: independent Philox / Box-Muller chains interleave
-#ifndef BRMPPI_A_UNROLL
-#define BRMPPI_A_UNROLL 2
-#endif
-constexpr int kNoiseUnroll = BRMPPI_A_UNROLL;
-
-// Named barriers 1..15 (0 is __syncthreads): producers arrive, consumers wait; when the barrier
-// completes, the producers' shared-memory writes are visible to the waiting threads.
-__device__ __forceinline__ void named_bar_arrive(int id, int count) {
-  asm volatile("bar.arrive %0, %1;" :: "r"(id), "r"(count) : "memory");
-}
-__device__ __forceinline__ void named_bar_sync(int id, int count) {
-  asm volatile("bar.sync %0, %1;" :: "r"(id), "r"(count) : "memory");
-}
 
 __device__ __forceinline__ unsigned long long global_ns() {
   unsigned long long t;
@@ -225,146 +211,95 @@ rollout_cta(const __grid_constant__ DeviceParams P) {
       cur_scene = scene;
       par = 0;
     }
-    // ---- phases A and B, overlapped.  Warps 4..15 ("producers") draw the noise block by block
-    //      in time order and signal each block on a named barrier; warps 0..3 run the serial chain
-    //      one block behind them.  Scene data: the global loads are issued first and consumed
-    //      after the first noise block, so their latency (HBM when the caller has flushed L2)
-    //      hides behind the Philox rounds. ---------------------------------------------------------
-    BRMPPI_STAMP(0)
-    const int n_blocks = P.chunks < kMaxNoiseBlocks ? P.chunks : kMaxNoiseBlocks;
-    const int blk_len = ((P.chunks + n_blocks - 1) / n_blocks) * P.chunk_len;   // whole chunks
-    if (warp >= kChainWarps) {
-      const int TS = P.t_stride, T = P.T;
-      const int pt = tid - 32 * kChainWarps;              // producer thread index
-      const int pr = pt / S, ps = pt - pr * S;            // (row, sample)
-      const int R = (kCtaThreads - 32 * kChainWarps) / S;
-      const int kp = k - s + ps;                          // sample index of (tile, ps)
-      float4 x0_in = make_float4(0.f, 0.f, 0.f, 0.f), g_in = x0_in;
-      float ob_in[2][5];
-      int n_obs_in = 0;
-      if (new_scene && warp == kChainWarps) {             // this warp stages and sorts the scene
-        x0_in = reinterpret_cast<const float4*>(P.state)[scene];
-        g_in = reinterpret_cast<const float4*>(P.goal)[scene];
-        n_obs_in = P.n_obs[scene];
+    // Scene data: the global loads are issued here and consumed after phase A, so their latency
+    // (HBM when the caller has flushed L2) hides behind the noise generation.
+    float4 x0_in = make_float4(0.f, 0.f, 0.f, 0.f), g_in = x0_in;
+    float ob_in[5] = {0.f, 0.f, 1.f, 0.f, 0.f};
+    int n_obs_in = 0;
+    if (new_scene) {
+      x0_in = reinterpret_cast<const float4*>(P.state)[scene];
+      n_obs_in = P.n_obs[scene];
+      if (tid < P.max_obstacles) {
+        const float* ob = P.obstacles + ((size_t)scene * P.max_obstacles + tid) * 5;
 #pragma unroll
-        for (int h = 0; h < 2; ++h) {
-          const int i = lane + 32 * h;
-#pragma unroll
-          for (int q = 0; q < 5; ++q)
-            ob_in[h][q] = i < P.max_obstacles ? P.obstacles[((size_t)scene * P.max_obstacles + i) * 5 + q] : 0.0f;
-        }
+        for (int q = 0; q < 5; ++q) ob_in[q] = ob[q];
       }
+      if (tid == 0) g_in = reinterpret_cast<const float4*>(P.goal)[scene];
+    }
+
+    BRMPPI_STAMP(0)
+    // ---- phase A: noise, perturb + clamp, effort cost (a1, a2) -------------------------------
+    {
+      const int TS = P.t_stride, T = P.T;
+      const int R = kCtaThreads / S;
       const uint32_t n = *P.counter;
       const uint32_t key0 = P.key0 + (uint32_t)scene;
       const uint32_t key1 = P.key1 + (key0 < P.key0 ? 1u : 0u);
       const float2* Unom = reinterpret_cast<const float2*>(P.U) + (size_t)scene * T;   // read-only here
-      float* pV = BRMPPI_SMEM(float, P.off_planes) + ps * TS;
+      float* pV = BRMPPI_SMEM(float, P.off_planes) + s * TS;
       float* pD = pV + S * TS;
       float* pP1 = pD + S * TS;
       float effort = 0.0f;
-      for (int blk = 0; blk < n_blocks; ++blk) {
-        const int tb = blk * blk_len, te = min(tb + blk_len, T);
-        if (pr < R) {
-#pragma unroll kNoiseUnroll
-          for (int t = tb + pr; t < te; t += R) {
-            const float2 u = sample_control<PRECISE>(P, __ldg(Unom + t), (uint32_t)t, n, (uint32_t)kp, key0, key1);
-            const float tan_d = tan_t<PRECISE>(u.y);
-            pV[t] = u.x;
-            pD[t] = u.y;
-            pP1[t + 1] = (P.dt * u.x) * P.inv_L1 * tan_d;          // dpsi1 of step t, parked at t+1
-            effort = fmaf(P.w_v * u.x, u.x, fmaf(P.w_delta * u.y, u.y, effort));
+      if (c < R) {
+#pragma unroll 2
+        for (int m = c; m < ((T + 1) >> 1); m += R) {
+          const int t = 2 * m, t1 = min(t + 1, T - 1);
+          float2 u0, u1;
+          sample_control_pair<PRECISE>(P, __ldg(Unom + t), __ldg(Unom + t1), (uint32_t)m, n, (uint32_t)k, key0, key1, &u0, &u1);
+          pV[t] = u0.x; pD[t] = u0.y;
+          pP1[t + 1] = (P.dt * u0.x) * P.inv_L1 * tan_t<PRECISE>(u0.y);
+          effort = fmaf(P.w_v * u0.x, u0.x, fmaf(P.w_delta * u0.y, u0.y, effort));
+          if (t + 1 < T) {
+            pV[t + 1] = u1.x; pD[t + 1] = u1.y;
+            pP1[t + 2] = (P.dt * u1.x) * P.inv_L1 * tan_t<PRECISE>(u1.y);
+            effort = fmaf(P.w_v * u1.x, u1.x, fmaf(P.w_delta * u1.y, u1.y, effort));
           }
         }
-        if (blk == 0 && new_scene && pt == 0) {
-          // the chain needs the start state: published with the first block
-          CtaMisc* sM = BRMPPI_SMEM(CtaMisc, P.off_misc);
-          g_in.x -= x0_in.x; g_in.y -= x0_in.y;          // vehicle-centred frame
-          sM->x0 = x0_in;
-          sM->g = g_in;
-          sM->n_obs = n_obs_in;
-          sM->m[0] = CUDART_INF; sM->argmin[0] = 0x7fffffff; sM->eta[0] = 0.0f; sM->w2[0] = 0.0f; sM->nonfinite[0] = 0;
-        }
-        named_bar_arrive(1 + blk, kCtaThreads);
       }
-      BRMPPI_SMEM(float, P.off_scratch)[pt] = effort;       // row partial of sample ps
-      if (pr == 0) BRMPPI_SMEM(float, P.off_alpha)[ps] = sample_alpha(P, n, (uint32_t)kp, key0, key1);
-      if (new_scene) {
-        float* sA = BRMPPI_SMEM(float, P.off_A);
-        for (int i = pt; i < 2 * T; i += kCtaThreads - 32 * kChainWarps) sA[i] = 0.0f;
-      }
-      if (new_scene && warp == kChainWarps) {
-        // obstacle table for phase C, in the vehicle-centred frame: moving obstacles first, static
-        // ones after (groups without a moving one skip the o(t) update), null padding behind.
-        // Lane l ranks obstacles l and l + 32 by counting.
-        CtaMisc* sM = BRMPPI_SMEM(CtaMisc, P.off_misc);
-        float* sRaw = BRMPPI_SMEM(float, P.off_raw);
-        float4* sObs = BRMPPI_SMEM(float4, P.off_obs);
-        float2* sVel = BRMPPI_SMEM(float2, P.off_vel);
-        float* sSpd = BRMPPI_SMEM(float, P.off_spd);
+      BRMPPI_SMEM(float, P.off_scratch)[tid] = effort;          // row partial of sample s
+      if (c == 0) BRMPPI_SMEM(float, P.off_alpha)[s] = sample_alpha(P, n, (uint32_t)k, key0, key1);
+    }
+    if (new_scene) {
+      // stage the scene for warp kChainWarps, which sorts the obstacles while the chain runs
+      CtaMisc* sM = BRMPPI_SMEM(CtaMisc, P.off_misc);
+      float* sRaw = BRMPPI_SMEM(float, P.off_raw);
+      float* sA = BRMPPI_SMEM(float, P.off_A);
+      if (tid < P.max_obstacles) {
 #pragma unroll
-        for (int h = 0; h < 2; ++h) {
-          const int i = lane + 32 * h;
-          if (i < P.max_obstacles) {
-#pragma unroll
-            for (int q = 0; q < 5; ++q) sRaw[5 * i + q] = ob_in[h][q];
-          }
-        }
-        __syncwarp();
-        const int n_obs = __shfl_sync(0xffffffffu, n_obs_in, 0);
-        const float x0x = __shfl_sync(0xffffffffu, x0_in.x, 0), x0y = __shfl_sync(0xffffffffu, x0_in.y, 0);
-        int nm = 0;
-        for (int j = 0; j < n_obs; ++j) nm += (sRaw[5 * j + 3] != 0.0f || sRaw[5 * j + 4] != 0.0f) ? 1 : 0;
-        for (int i = lane; i < P.obs_padded; i += 32) {
-          if (i < n_obs) {
-            int before_m = 0, before_s = 0;
-            for (int j = 0; j < i; ++j) {
-              const bool mj = (sRaw[5 * j + 3] != 0.0f || sRaw[5 * j + 4] != 0.0f);
-              before_m += mj ? 1 : 0; before_s += mj ? 0 : 1;
-            }
-            const bool moving = (sRaw[5 * i + 3] != 0.0f || sRaw[5 * i + 4] != 0.0f);
-            const int dst = moving ? before_m : nm + before_s;
-            const float rho = sRaw[5 * i + 2] + P.disc_radius;
-            sObs[dst] = make_float4(sRaw[5 * i + 0] - x0x, sRaw[5 * i + 1] - x0y, 0.5f / (rho * rho), -(rho * rho));
-            sVel[dst] = make_float2(P.dt * sRaw[5 * i + 3], P.dt * sRaw[5 * i + 4]);
-            // displacement per step, rounded up (culling bound)
-            sSpd[dst] = 1.0001f * P.dt * sqrtf(fmaf(sRaw[5 * i + 3], sRaw[5 * i + 3], sRaw[5 * i + 4] * sRaw[5 * i + 4]));
-          }
-        }
-        for (int i = n_obs + lane; i < P.obs_padded; i += 32) {   // null obstacles: weight 0
-          sObs[i] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
-          sVel[i] = make_float2(0.0f, 0.0f);
-          sSpd[i] = 0.0f;
-        }
-        if (lane == 0) {
-          sM->n_moving = nm;
-          sM->n_groups = n_obs > 0 ? (n_obs + kObsGroup - 1) / kObsGroup : 1;
-        }
+        for (int q = 0; q < 5; ++q) sRaw[5 * tid + q] = ob_in[q];
       }
-    } else {
-      // ---- phase B: serial Euler chain of eq. (6), one sample per thread (a3).  Only the psi2
-      //      recursion is a true chain; the thread also integrates psi1, x, y (short independent
-      //      dependency chains that fill its issue bubbles).  Everything else is left to phase C.
+      for (int i = tid; i < 2 * P.T; i += kCtaThreads) sA[i] = 0.0f;
+      if (tid == 0) {
+        g_in.x -= x0_in.x; g_in.y -= x0_in.y;          // vehicle-centred frame
+        sM->x0 = x0_in;
+        sM->g = g_in;
+        sM->n_obs = n_obs_in;
+        sM->m[0] = CUDART_INF; sM->argmin[0] = 0x7fffffff; sM->eta[0] = 0.0f; sM->w2[0] = 0.0f; sM->nonfinite[0] = 0;
+      }
+    }
+    __syncthreads();
+    BRMPPI_STAMP(1)
+
+    // ---- phase B: serial Euler chain of eq. (6), one sample per thread (a3).  Only the psi2
+    //      recursion is a true chain; the thread also integrates psi1, x, y (short independent
+    //      dependency chains that fill its issue bubbles).  Everything else is left to phase C. ---
+    if (c == 0) {
       const int TS = P.t_stride, T = P.T, L = P.chunk_len;
-      const bool mine = tid < S;                          // lanes beyond the tile only keep the barriers company
-      const int sc_ = mine ? tid : 0;
-      const float* pV = BRMPPI_SMEM(float, P.off_planes) + sc_ * TS;
-      float* pP1 = BRMPPI_SMEM(float, P.off_planes) + (2 * S + sc_) * TS;
+      const float* pV = BRMPPI_SMEM(float, P.off_planes) + s * TS;
+      float* pP1 = BRMPPI_SMEM(float, P.off_planes) + (2 * S + s) * TS;
       float* pP2 = pP1 + S * TS;
-      float2* sXY = BRMPPI_SMEM(float2, P.off_xy);        // [C + 1][S] chunk-start (x, y)
-      named_bar_sync(1, kCtaThreads);                     // block 0 and the start state are there
-      int blk_ready = 1;
+      float2* sXY = BRMPPI_SMEM(float2, P.off_xy);        // [C][S] chunk-start (x, y)
       const float4 x0 = BRMPPI_SMEM(CtaMisc, P.off_misc)->x0;
       float x = 0.0f, y = 0.0f, psi1 = x0.z, psi2 = x0.w;
-      if (mine) { pP1[0] = psi1; pP2[0] = psi2; }
+      pP1[0] = psi1;
+      pP2[0] = psi2;
       float v = pV[0], b = pP1[1];
       for (int cc = 0, t = 0; t < T; ++cc) {
-        if (mine) sXY[cc * S + tid] = make_float2(x, y);
+        sXY[cc * S + s] = make_float2(x, y);
         const int te = min(t + L, T);
         for (; t < te; ++t) {
-          // next step's inputs first (the loads do not wait behind this step's stores); they may
-          // lie in the next noise block
+          // next step's inputs first: the loads do not wait behind this step's stores
           const int tn = min(t + 1, T - 1);
-          if (tn >= blk_ready * blk_len && blk_ready < n_blocks) { named_bar_sync(1 + blk_ready, kCtaThreads); ++blk_ready; }
           const float v_next = pV[tn], b_next = pP1[tn + 1];
           const float a = P.dt * v;
           float s1, c1, sb, cb;
@@ -374,12 +309,49 @@ rollout_cta(const __grid_constant__ DeviceParams P) {
           y = fmaf(a, s1, y);
           psi1 += b;
           psi2 = fmaf(a * P.inv_L2, sb, fmaf(-(b * P.Lh_over_L2), cb, psi2));
-          if (mine) { pP1[t + 1] = psi1; pP2[t + 1] = psi2; }
+          pP1[t + 1] = psi1;
+          pP2[t + 1] = psi2;
           v = v_next; b = b_next;
         }
       }
-      while (blk_ready < n_blocks) { named_bar_sync(1 + blk_ready, kCtaThreads); ++blk_ready; }
-      if (mine) sXY[P.chunks * S + tid] = make_float2(x, y);   // x_T
+      sXY[P.chunks * S + s] = make_float2(x, y);   // x_T
+    } else if (new_scene && warp == kChainWarps) {
+      // obstacle table for phase C, in the vehicle-centred frame: moving obstacles first, static
+      // ones after (groups without a moving one skip the o(t) update), null padding behind.
+      // Lane l ranks obstacles l and l + 32 by counting; the chain warps are busy meanwhile.
+      CtaMisc* sM = BRMPPI_SMEM(CtaMisc, P.off_misc);
+      const float* sRaw = BRMPPI_SMEM(float, P.off_raw);
+      float4* sObs = BRMPPI_SMEM(float4, P.off_obs);
+      float2* sVel = BRMPPI_SMEM(float2, P.off_vel);
+      float* sSpd = BRMPPI_SMEM(float, P.off_spd);
+      const int n_obs = sM->n_obs;
+      const float4 x0 = sM->x0;
+      int nm = 0;
+      for (int j = 0; j < n_obs; ++j) nm += (sRaw[5 * j + 3] != 0.0f || sRaw[5 * j + 4] != 0.0f) ? 1 : 0;
+      for (int i = lane; i < P.obs_padded; i += 32) {
+        if (i < n_obs) {
+          int before_m = 0, before_s = 0;
+          for (int j = 0; j < i; ++j) {
+            const bool mj = (sRaw[5 * j + 3] != 0.0f || sRaw[5 * j + 4] != 0.0f);
+            before_m += mj ? 1 : 0; before_s += mj ? 0 : 1;
+          }
+          const bool moving = (sRaw[5 * i + 3] != 0.0f || sRaw[5 * i + 4] != 0.0f);
+          const int dst = moving ? before_m : nm + before_s;
+          const float rho = sRaw[5 * i + 2] + P.disc_radius;
+          sObs[dst] = make_float4(sRaw[5 * i + 0] - x0.x, sRaw[5 * i + 1] - x0.y, 0.5f / (rho * rho), -(rho * rho));
+          sVel[dst] = make_float2(P.dt * sRaw[5 * i + 3], P.dt * sRaw[5 * i + 4]);
+          // displacement per step, rounded up (culling bound)
+          sSpd[dst] = 1.0001f * P.dt * sqrtf(fmaf(sRaw[5 * i + 3], sRaw[5 * i + 3], sRaw[5 * i + 4] * sRaw[5 * i + 4]));
+        } else {                                        // null obstacle: weight 0
+          sObs[i] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+          sVel[i] = make_float2(0.0f, 0.0f);
+          sSpd[i] = 0.0f;
+        }
+      }
+      if (lane == 0) {
+        sM->n_moving = nm;
+        sM->n_groups = n_obs > 0 ? (n_obs + kObsGroup - 1) / kObsGroup : 1;
+      }
     }
     __syncthreads();
     BRMPPI_STAMP(2)
@@ -432,7 +404,7 @@ rollout_cta(const __grid_constant__ DeviceParams P) {
         const double* sCost = BRMPPI_SMEM(double, P.off_cost);
         const float* sEff = BRMPPI_SMEM(float, P.off_scratch);
         float effort = 0.0f;
-        for (int r = 0; r < (kCtaThreads - 32 * kChainWarps) / S; ++r) effort += sEff[r * S + s];  // fixed order
+        for (int r = 0; r < kCtaThreads / S; ++r) effort += sEff[r * S + s];  // fixed order
         Sk = (double)effort;
         for (int cc = 0; cc < P.chunks; ++cc) Sk += sCost[cc * S + s];
         if (P.flags & BRMPPI_FLAG_WRITE_SAMPLES) P.S[(size_t)scene * P.K + k] = (float)Sk;

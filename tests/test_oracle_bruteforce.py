@@ -39,9 +39,10 @@ def brute_force(p, n, x0, goal, obstacles, U):
     for k in range(K):
         alpha.append(mpf(p.alpha_lo) + (mpf(p.alpha_hi) - mpf(p.alpha_lo)) * f(philox_py((0, n, k, 1), key)[0]))
         for t in range(T):
-            w = philox_py((t, n, k, 0), key)
-            r = mp.sqrt(-2 * mp.log(1 - f(w[0])))
-            zv, zd = r * mp.cos(2 * mp.pi * f(w[1])), r * mp.sin(2 * mp.pi * f(w[1]))
+            w = philox_py((t >> 1, n, k, 0), key)       # one block per pair of steps (reading 6)
+            wa, wb = (w[2], w[3]) if t & 1 else (w[0], w[1])
+            r = mp.sqrt(-2 * mp.log(1 - f(wa)))
+            zv, zd = r * mp.cos(2 * mp.pi * f(wb)), r * mp.sin(2 * mp.pi * f(wb))
             v = min(max(mpf(U[t][0]) + mpf(p.sigma_v) * zv, mpf(p.v_min)), mpf(p.v_max))
             d = min(max(mpf(U[t][1]) + mpf(p.sigma_delta) * zd, mpf(p.delta_min)), mpf(p.delta_max))
             u[k][t] = (v, d)

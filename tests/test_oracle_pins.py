@@ -68,14 +68,17 @@ def test_philox_counter_and_key_sensitivity(O):
 def test_noise_stream_layout(O):
     """Counter layout (t, n, k, tag) and key (lo32(seed), hi32(seed)) -- DESIGN.md reading 5/7.
     orc_normals / orc_alpha must consume exactly those blocks."""
-    seed, n, k, t = 0x1234567890ABCDEF, 7, 4242, 17
-    w = O.philox((t, n, k, 0), (seed & 0xFFFFFFFF, seed >> 32))
-    u1 = 1.0 - (w[0] >> 9) / 2.0**23
-    u2 = (w[1] >> 9) / 2.0**23
-    r = math.sqrt(-2.0 * math.log(u1))
-    z = O.normals(seed, n, k, t)
-    assert z[0] == pytest.approx(r * math.cos(2 * math.pi * u2), rel=1e-14, abs=1e-15)
-    assert z[1] == pytest.approx(r * math.sin(2 * math.pi * u2), rel=1e-14, abs=1e-15)
+    seed, n, k = 0x1234567890ABCDEF, 7, 4242
+    for t in (16, 17, 0, 1):                       # one block per pair of steps (reading 6)
+        w = O.philox((t >> 1, n, k, 0), (seed & 0xFFFFFFFF, seed >> 32))
+        wa, wb = (w[2], w[3]) if t & 1 else (w[0], w[1])
+        u1 = 1.0 - (wa >> 9) / 2.0**23
+        u2 = (wb >> 9) / 2.0**23
+        r = math.sqrt(-2.0 * math.log(u1))
+        z = O.normals(seed, n, k, t)
+        assert z[0] == pytest.approx(r * math.cos(2 * math.pi * u2), rel=1e-14, abs=1e-15)
+        assert z[1] == pytest.approx(r * math.sin(2 * math.pi * u2), rel=1e-14, abs=1e-15)
+    assert not np.allclose(O.normals(seed, n, k, 16), O.normals(seed, n, k, 17))
     p = P(seed=seed, alpha_lo=0.25, alpha_hi=0.75)
     wa = O.philox((0, n, k, 1), (seed & 0xFFFFFFFF, seed >> 32))
     assert O.alpha(p, n, k) == pytest.approx(0.25 + 0.5 * ((wa[0] >> 9) / 2.0**23), rel=1e-15)
