@@ -52,7 +52,7 @@ __device__ __forceinline__ unsigned long long global_ns() {
 // pV, pP1, pP2: this sample's rows of the v, psi1, psi2 planes.
 struct GroupCost { double track, bar; };
 
-template <bool PRECISE, int ND, int NM, bool TRACK>
+template <bool PRECISE, int ND, int NM, bool TRACK, bool CULL>
 __device__ __forceinline__ GroupCost barrier_group(const DeviceParams& P, const float* __restrict__ pV,
                                                    const float* __restrict__ pP1, const float* __restrict__ pP2,
                                                    const float4* __restrict__ obs, const float2* __restrict__ vel,
@@ -88,7 +88,7 @@ __device__ __forceinline__ GroupCost barrier_group(const DeviceParams& P, const 
   // chunk; its hinge terms are then all exactly +0 and it is skipped.  The mask is the union over
   // the warp's samples, so the skip is a uniform branch.
   unsigned active = 0xffu;
-  if (!(P.flags & BRMPPI_FLAG_NO_CULL)) {
+  if (CULL && !(P.flags & BRMPPI_FLAG_NO_CULL)) {
     const float alpha = 1.0f - one_minus_alpha;
     const float inv_alpha = 1.0f / alpha;
     const float steps = (float)(t1 - t0);
@@ -109,7 +109,7 @@ __device__ __forceinline__ GroupCost barrier_group(const DeviceParams& P, const 
     }
     active = __reduce_or_sync(__activemask(), active);
   }
-  if (!TRACK && active == 0u) return GroupCost{0.0, 0.0};
+  if (CULL && !TRACK && active == 0u) return GroupCost{0.0, 0.0};
 #pragma unroll kCostUnroll
   for (int t = t0; t < t1; ++t) {
     // (x, y) of state t+1 from state t: the chain's own FMAs on the same operands
@@ -131,7 +131,7 @@ __device__ __forceinline__ GroupCost barrier_group(const DeviceParams& P, const 
     float pen = 0.0f;
 #pragma unroll
     for (int i = 0; i < kObsGroup; ++i) {
-      if (!(active & (1u << i))) continue;      // warp-uniform
+      if (CULL && !(active & (1u << i))) continue;      // warp-uniform
       float ox = o[i].x, oy = o[i].y;
       if (i < NM) { const float2 w = vel[i]; ox = fmaf(tf, w.x, ox); oy = fmaf(tf, w.y, oy); }
       float Pi = 0.0f;
@@ -151,15 +151,15 @@ __device__ __forceinline__ GroupCost barrier_group(const DeviceParams& P, const 
 }
 
 // Dispatch on the number of moving obstacles in the group (block-uniform).
-template <bool PRECISE, int ND, bool TRACK>
+template <bool PRECISE, int ND, bool TRACK, bool CULL>
 __device__ __forceinline__ GroupCost barrier_group_nm(int nm, const DeviceParams& P, const float* pV,
                                                       const float* pP1, const float* pP2, const float4* obs,
                                                       const float2* vel, const float* spd, float x, float y,
                                                       int t0, int t1, float oma, const float4 g) {
-  if (nm <= 0) return barrier_group<PRECISE, ND, 0, TRACK>(P, pV, pP1, pP2, obs, vel, spd, x, y, t0, t1, oma, g);
-  if (nm <= 2) return barrier_group<PRECISE, ND, 2, TRACK>(P, pV, pP1, pP2, obs, vel, spd, x, y, t0, t1, oma, g);
-  if (nm <= 4) return barrier_group<PRECISE, ND, 4, TRACK>(P, pV, pP1, pP2, obs, vel, spd, x, y, t0, t1, oma, g);
-  return barrier_group<PRECISE, ND, kObsGroup, TRACK>(P, pV, pP1, pP2, obs, vel, spd, x, y, t0, t1, oma, g);
+  if (nm <= 0) return barrier_group<PRECISE, ND, 0, TRACK, CULL>(P, pV, pP1, pP2, obs, vel, spd, x, y, t0, t1, oma, g);
+  if (nm <= 2) return barrier_group<PRECISE, ND, 2, TRACK, CULL>(P, pV, pP1, pP2, obs, vel, spd, x, y, t0, t1, oma, g);
+  if (nm <= 4) return barrier_group<PRECISE, ND, 4, TRACK, CULL>(P, pV, pP1, pP2, obs, vel, spd, x, y, t0, t1, oma, g);
+  return barrier_group<PRECISE, ND, kObsGroup, TRACK, CULL>(P, pV, pP1, pP2, obs, vel, spd, x, y, t0, t1, oma, g);
 }
 
 template <bool PRECISE, int ND>
@@ -372,13 +372,18 @@ rollout_cta(const __grid_constant__ DeviceParams P) {
       const int n_moving = sM->n_moving, n_groups = sM->n_groups;
       const float2 xy = BRMPPI_SMEM(float2, P.off_xy)[c * S + s];
       double track = 0.0, bar = 0.0;
-      {
-        const GroupCost gc = barrier_group_nm<PRECISE, ND, true>(n_moving, P, pV, pP1, pP2, sObs, sVel, sSpd, xy.x, xy.y, t0, t1, one_minus_alpha, g);
+      if (n_groups == 1) {
+        // a single group of obstacles: the culling test (a square root per obstacle and disc at
+        // every chunk start, a uniform branch per obstacle and step) costs more than it saves
+        const GroupCost gc = barrier_group_nm<PRECISE, ND, true, false>(n_moving, P, pV, pP1, pP2, sObs, sVel, sSpd, xy.x, xy.y, t0, t1, one_minus_alpha, g);
         track = gc.track; bar = gc.bar;
-      }
-      for (int grp = 1; grp < n_groups; ++grp) {
-        const int ib = grp * kObsGroup;
-        bar += barrier_group_nm<PRECISE, ND, false>(n_moving - ib, P, pV, pP1, pP2, sObs + ib, sVel + ib, sSpd + ib, xy.x, xy.y, t0, t1, one_minus_alpha, g).bar;
+      } else {
+        const GroupCost gc = barrier_group_nm<PRECISE, ND, true, true>(n_moving, P, pV, pP1, pP2, sObs, sVel, sSpd, xy.x, xy.y, t0, t1, one_minus_alpha, g);
+        track = gc.track; bar = gc.bar;
+        for (int grp = 1; grp < n_groups; ++grp) {
+          const int ib = grp * kObsGroup;
+          bar += barrier_group_nm<PRECISE, ND, false, true>(n_moving - ib, P, pV, pP1, pP2, sObs + ib, sVel + ib, sSpd + ib, xy.x, xy.y, t0, t1, one_minus_alpha, g).bar;
+        }
       }
       if (t1 == T) {   // terminal cost r_N(x_N), eq. (7); final state out
         const float2 xT = BRMPPI_SMEM(float2, P.off_xy)[P.chunks * S + s];
