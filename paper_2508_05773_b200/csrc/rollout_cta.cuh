@@ -48,6 +48,7 @@ constexpr int kMaxTileSamples = kChainWarps * 32;   // 128
 constexpr int kObsGroup = 8;                        // obstacles whose h_t are held in registers at a time
 constexpr int kMaxChunks = 16;
 constexpr int kMinChunkLen = 4;
+constexpr int kMinCullChunk = 8;                    // culling pays from this chunk length on
 constexpr int kMaxNoiseBlocks = 8;                  // named barriers 1..8 hand noise blocks to the chain
 constexpr int kPhaseSlots = 7;                      // prologue, A, B, C, D, E, partial out
 constexpr size_t kSmemMax = 232448;                 // 227 KB opt-in dynamic shared memory per CTA

@@ -372,11 +372,16 @@ rollout_cta(const __grid_constant__ DeviceParams P) {
       const int n_moving = sM->n_moving, n_groups = sM->n_groups;
       const float2 xy = BRMPPI_SMEM(float2, P.off_xy)[c * S + s];
       double track = 0.0, bar = 0.0;
-      if (n_groups == 1) {
-        // a single group of obstacles: the culling test (a square root per obstacle and disc at
-        // every chunk start, a uniform branch per obstacle and step) costs more than it saves
-        const GroupCost gc = barrier_group_nm<PRECISE, ND, true, false>(n_moving, P, pV, pP1, pP2, sObs, sVel, sSpd, xy.x, xy.y, t0, t1, one_minus_alpha, g);
+      if (n_groups == 1 || P.chunk_len < kMinCullChunk) {
+        // a single group of obstacles, or short chunks: the culling test (a square root per
+        // obstacle and disc at every chunk start, a uniform branch per obstacle and step) costs
+        // more than it saves
+        GroupCost gc = barrier_group_nm<PRECISE, ND, true, false>(n_moving, P, pV, pP1, pP2, sObs, sVel, sSpd, xy.x, xy.y, t0, t1, one_minus_alpha, g);
         track = gc.track; bar = gc.bar;
+        for (int grp = 1; grp < n_groups; ++grp) {
+          const int ib = grp * kObsGroup;
+          bar += barrier_group_nm<PRECISE, ND, false, false>(n_moving - ib, P, pV, pP1, pP2, sObs + ib, sVel + ib, sSpd + ib, xy.x, xy.y, t0, t1, one_minus_alpha, g).bar;
+        }
       } else {
         const GroupCost gc = barrier_group_nm<PRECISE, ND, true, true>(n_moving, P, pV, pP1, pP2, sObs, sVel, sSpd, xy.x, xy.y, t0, t1, one_minus_alpha, g);
         track = gc.track; bar = gc.bar;
