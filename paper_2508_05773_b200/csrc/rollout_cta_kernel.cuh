@@ -236,27 +236,31 @@ rollout_cta(const __grid_constant__ DeviceParams P) {
       const uint32_t key0 = P.key0 + (uint32_t)scene;
       const uint32_t key1 = P.key1 + (key0 < P.key0 ? 1u : 0u);
       const float2* Unom = reinterpret_cast<const float2*>(P.U) + (size_t)scene * T;   // read-only here
-      float* pV = BRMPPI_SMEM(float, P.off_planes) + s * TS;
-      float* pD = pV + S * TS;
-      float* pP1 = pD + S * TS;
-      float effort = 0.0f;
-      if (c < R) {
+      // items (sample si, step pair mi) dealt round-robin over all 512 threads: item = tid,
+      // tid + 512, ...; (si, mi) = (item % S, item / S) kept up to date incrementally
+      float* planes = BRMPPI_SMEM(float, P.off_planes);
+      const int n_pairs = (T + 1) >> 1;
+      const int ds = kCtaThreads % S, dm = kCtaThreads / S;
+      const int k0 = k - s;                                  // sample index of the tile's first sample
+      int si = s, mi = c;
+      (void)R;
 #pragma unroll 2
-        for (int m = c; m < ((T + 1) >> 1); m += R) {
-          const int t = 2 * m, t1 = min(t + 1, T - 1);
-          float2 u0, u1;
-          sample_control_pair<PRECISE>(P, __ldg(Unom + t), __ldg(Unom + t1), (uint32_t)m, n, (uint32_t)k, key0, key1, &u0, &u1);
-          pV[t] = u0.x; pD[t] = u0.y;
-          pP1[t + 1] = (P.dt * u0.x) * P.inv_L1 * tan_t<PRECISE>(u0.y);
-          effort = fmaf(P.w_v * u0.x, u0.x, fmaf(P.w_delta * u0.y, u0.y, effort));
-          if (t + 1 < T) {
-            pV[t + 1] = u1.x; pD[t + 1] = u1.y;
-            pP1[t + 2] = (P.dt * u1.x) * P.inv_L1 * tan_t<PRECISE>(u1.y);
-            effort = fmaf(P.w_v * u1.x, u1.x, fmaf(P.w_delta * u1.y, u1.y, effort));
-          }
+      for (; mi < n_pairs; ) {
+        const int t = 2 * mi, t1 = min(t + 1, T - 1);
+        float2 u0, u1;
+        sample_control_pair<PRECISE>(P, __ldg(Unom + t), __ldg(Unom + t1), (uint32_t)mi, n, (uint32_t)(k0 + si), key0, key1, &u0, &u1);
+        float* pV = planes + si * TS;
+        float* pD = pV + S * TS;
+        float* pP1 = pD + S * TS;
+        pV[t] = u0.x; pD[t] = u0.y;
+        pP1[t + 1] = (P.dt * u0.x) * P.inv_L1 * tan_t<PRECISE>(u0.y);       // dpsi1 of step t, parked at t+1
+        if (t + 1 < T) {
+          pV[t + 1] = u1.x; pD[t + 1] = u1.y;
+          pP1[t + 2] = (P.dt * u1.x) * P.inv_L1 * tan_t<PRECISE>(u1.y);
         }
+        si += ds; mi += dm;
+        if (si >= S) { si -= S; ++mi; }
       }
-      BRMPPI_SMEM(float, P.off_scratch)[tid] = effort;          // row partial of sample s
       if (c == 0) BRMPPI_SMEM(float, P.off_alpha)[s] = sample_alpha(P, n, (uint32_t)k, key0, key1);
     }
     if (new_scene) {
@@ -293,6 +297,8 @@ rollout_cta(const __grid_constant__ DeviceParams P) {
       float x = 0.0f, y = 0.0f, psi1 = x0.z, psi2 = x0.w;
       pP1[0] = psi1;
       pP2[0] = psi2;
+      const float* pD = pV + S * TS;
+      float effort = 0.0f;                                   // w_v v^2 + w_delta delta^2 summed over the horizon
       float v = pV[0], b = pP1[1];
       for (int cc = 0, t = 0; t < T; ++cc) {
         sXY[cc * S + s] = make_float2(x, y);
@@ -301,6 +307,8 @@ rollout_cta(const __grid_constant__ DeviceParams P) {
           // next step's inputs first: the loads do not wait behind this step's stores
           const int tn = min(t + 1, T - 1);
           const float v_next = pV[tn], b_next = pP1[tn + 1];
+          const float d = pD[t];
+          effort = fmaf(P.w_v * v, v, fmaf(P.w_delta * d, d, effort));
           const float a = P.dt * v;
           float s1, c1, sb, cb;
           sincos_t<PRECISE>(psi1 - psi2, &sb, &cb);
@@ -315,6 +323,7 @@ rollout_cta(const __grid_constant__ DeviceParams P) {
         }
       }
       sXY[P.chunks * S + s] = make_float2(x, y);   // x_T
+      BRMPPI_SMEM(float, P.off_scratch)[s] = effort;
     } else if (new_scene && warp == kChainWarps) {
       // obstacle table for phase C, in the vehicle-centred frame: moving obstacles first, static
       // ones after (groups without a moving one skip the o(t) update), null padding behind.
@@ -412,10 +421,7 @@ rollout_cta(const __grid_constant__ DeviceParams P) {
       valid = (tid < S) && (k < P.K);
       if (valid) {
         const double* sCost = BRMPPI_SMEM(double, P.off_cost);
-        const float* sEff = BRMPPI_SMEM(float, P.off_scratch);
-        float effort = 0.0f;
-        for (int r = 0; r < kCtaThreads / S; ++r) effort += sEff[r * S + s];  // fixed order
-        Sk = (double)effort;
+        Sk = (double)BRMPPI_SMEM(float, P.off_scratch)[s];                   // effort, from the chain
         for (int cc = 0; cc < P.chunks; ++cc) Sk += sCost[cc * S + s];
         if (P.flags & BRMPPI_FLAG_WRITE_SAMPLES) P.S[(size_t)scene * P.K + k] = (float)Sk;
       }
