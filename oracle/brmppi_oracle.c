@@ -107,6 +107,18 @@ double orc_barrier(const orc_params* p, const double c[2], const double o[2], do
   return (dx * dx + dy * dy) / (rho * rho) - 1.0;
 }
 
+/* Eq. (16): obstacle frame p' = R(-theta_o)(c - o), semi-axes inflated by the
+ * vehicle disc radius, exponent e >= 2 (even e in the paper: 4 for parked cars, 2 for pedestrians;
+ * |.| makes odd or fractional e well defined too).  se = (cx, cy, m_x, m_y, theta, vx, vy, e). */
+double orc_barrier_se(const orc_params* p, const double c[2], const double o[2], const double* se) {
+  double ct = cos(se[4]), st = sin(se[4]);
+  double dx = c[0] - o[0], dy = c[1] - o[1];
+  double xp = ct * dx + st * dy;
+  double yp = -st * dx + ct * dy;
+  double ax = se[2] + p->disc_radius, ay = se[3] + p->disc_radius;
+  return pow(fabs(xp) / ax, se[7]) + pow(fabs(yp) / ay, se[7]) - 1.0;
+}
+
 double orc_goal_cost(const orc_params* p, const double x[4], const double g[4]) {
   double ex = x[0] - g[0], ey = x[1] - g[1];
   double e1 = orc_wrap(x[2] - g[2]), e2 = orc_wrap(x[3] - g[3]);
@@ -120,13 +132,14 @@ static void obstacle_at(const orc_params* p, const double* obstacles, int i, int
   o[1] = ob[1] + (double)t * p->dt * ob[4];
 }
 
-double orc_rollout(const orc_params* p, const double x0[4], const double goal[4], int n_obs,
-                   const double* obstacles, const double* u, double alpha, double xT[4],
-                   double* traj, double* pen_out) {
+double orc_rollout_se(const orc_params* p, const double x0[4], const double goal[4], int n_obs,
+                      const double* obstacles, int n_se, const double* se, const double* u,
+                      double alpha, double xT[4], double* traj, double* pen_out) {
   const int T = p->T, D = p->n_discs;
   double X[4] = {x0[0], x0[1], x0[2], x0[3]};
   double S = 0.0, pen_total = 0.0;
   double* hprev = (double*)malloc(sizeof(double) * (size_t)(n_obs > 0 ? n_obs : 1) * ORC_MAX_DISCS);
+  double* hprev_se = (double*)malloc(sizeof(double) * (size_t)(n_se > 0 ? n_se : 1) * ORC_MAX_DISCS);
 
   /* h at (x_0, o(0)) */
   for (int i = 0; i < n_obs; ++i) {
@@ -136,6 +149,14 @@ double orc_rollout(const orc_params* p, const double x0[4], const double goal[4]
       double c[2];
       orc_disc_centre(p, X, j, c);
       hprev[i * ORC_MAX_DISCS + j] = orc_barrier(p, c, o, obstacles[5 * i + 2]);
+    }
+  }
+  for (int i = 0; i < n_se; ++i) {   /* super-ellipse obstacles, same pairing of state and time */
+    double o[2] = {se[8 * i + 0], se[8 * i + 1]};
+    for (int j = 0; j < D; ++j) {
+      double c[2];
+      orc_disc_centre(p, X, j, c);
+      hprev_se[i * ORC_MAX_DISCS + j] = orc_barrier_se(p, c, o, se + 8 * i);
     }
   }
   if (traj) memcpy(traj, X, sizeof(X));
@@ -161,6 +182,18 @@ double orc_rollout(const orc_params* p, const double x0[4], const double goal[4]
         hprev[i * ORC_MAX_DISCS + j] = hn;
       }
     }
+    for (int i = 0; i < n_se; ++i) {
+      double o[2] = {se[8 * i + 0] + (double)(t + 1) * p->dt * se[8 * i + 5],
+                     se[8 * i + 1] + (double)(t + 1) * p->dt * se[8 * i + 6]};
+      for (int j = 0; j < D; ++j) {
+        double c[2];
+        orc_disc_centre(p, Xn, j, c);
+        double hn = orc_barrier_se(p, c, o, se + 8 * i);
+        double viol = (1.0 - alpha) * hprev_se[i * ORC_MAX_DISCS + j] - hn;
+        if (viol > 0.0) pen += viol;
+        hprev_se[i * ORC_MAX_DISCS + j] = hn;
+      }
+    }
     pen_total += pen;
 
     /* stage cost on (x_{t+1}, u_t) (reading 3); hitch: squared hinge at hitch_max (reading 15) */
@@ -176,7 +209,14 @@ double orc_rollout(const orc_params* p, const double x0[4], const double goal[4]
   memcpy(xT, X, sizeof(X));
   if (pen_out) *pen_out = pen_total;
   free(hprev);
+  free(hprev_se);
   return S;
+}
+
+double orc_rollout(const orc_params* p, const double x0[4], const double goal[4], int n_obs,
+                   const double* obstacles, const double* u, double alpha, double xT[4],
+                   double* traj, double* pen_out) {
+  return orc_rollout_se(p, x0, goal, n_obs, obstacles, 0, NULL, u, alpha, xT, traj, pen_out);
 }
 
 int orc_weights_update(int K, int T, double lambda, const double* S, const double* u,
@@ -217,12 +257,14 @@ typedef struct {
   const double *x0, *goal, *obstacles, *U_in;
   int n_obs, k_begin, k_end;
   double *S, *XT, *u_all;
+  int n_se;
+  const double* se;
 } sample_job;
 
 /* Sample k of iteration n: draw alpha_k and the perturbed, clamped controls, roll out. */
-double orc_sample(const orc_params* p, uint32_t n, uint32_t k, const double x0[4],
-                  const double goal[4], int n_obs, const double* obstacles, const double* U_in,
-                  double* u /* T*2 */, double xT[4]) {
+double orc_sample_se(const orc_params* p, uint32_t n, uint32_t k, const double x0[4],
+                     const double goal[4], int n_obs, const double* obstacles, int n_se,
+                     const double* se, const double* U_in, double* u /* T*2 */, double xT[4]) {
   const int T = p->T;
   double alpha = orc_alpha(p, n, k);
   for (int t = 0; t < T; ++t) {
@@ -232,21 +274,28 @@ double orc_sample(const orc_params* p, uint32_t n, uint32_t k, const double x0[4
     u[2 * t + 0] = clampd(U_in[2 * t + 0] + p->sigma_v * z[0], p->v_min, p->v_max);
     u[2 * t + 1] = clampd(U_in[2 * t + 1] + p->sigma_delta * z[1], p->delta_min, p->delta_max);
   }
-  return orc_rollout(p, x0, goal, n_obs, obstacles, u, alpha, xT, NULL, NULL);
+  return orc_rollout_se(p, x0, goal, n_obs, obstacles, n_se, se, u, alpha, xT, NULL, NULL);
+}
+
+double orc_sample(const orc_params* p, uint32_t n, uint32_t k, const double x0[4],
+                  const double goal[4], int n_obs, const double* obstacles, const double* U_in,
+                  double* u /* T*2 */, double xT[4]) {
+  return orc_sample_se(p, n, k, x0, goal, n_obs, obstacles, 0, NULL, U_in, u, xT);
 }
 
 static void* sample_worker(void* arg) {
   sample_job* job = (sample_job*)arg;
   const int T = job->p->T;
   for (int k = job->k_begin; k < job->k_end; ++k)
-    job->S[k] = orc_sample(job->p, job->n, (uint32_t)k, job->x0, job->goal, job->n_obs,
-                           job->obstacles, job->U_in, job->u_all + (size_t)k * 2 * T,
-                           job->XT + 4 * (size_t)k);
+    job->S[k] = orc_sample_se(job->p, job->n, (uint32_t)k, job->x0, job->goal, job->n_obs,
+                              job->obstacles, job->n_se, job->se, job->U_in,
+                              job->u_all + (size_t)k * 2 * T, job->XT + 4 * (size_t)k);
   return NULL;
 }
 
-int orc_iteration(const orc_params* p, uint32_t n, const double x0[4], const double goal[4],
-                  int n_obs, const double* obstacles, const double* U_in, double* U_out,
+int orc_iteration_se(const orc_params* p, uint32_t n, const double x0[4], const double goal[4],
+                     int n_obs, const double* obstacles, int n_se, const double* se,
+                     const double* U_in, double* U_out,
                   double* S, double* XT, double* u_all, double* w, int* argmin, double* gap,
                   double* eta, int n_threads) {
   const int K = p->K, T = p->T;
@@ -263,7 +312,7 @@ int orc_iteration(const orc_params* p, uint32_t n, const double x0[4], const dou
   for (int i = 0; i < n_threads; ++i) {
     jobs[i] = (sample_job){p, n, x0, goal, obstacles, U_nom, n_obs,
                            (int)((long long)K * i / n_threads),
-                           (int)((long long)K * (i + 1) / n_threads), S_buf, XT_buf, u_buf};
+                           (int)((long long)K * (i + 1) / n_threads), S_buf, XT_buf, u_buf, n_se, se};
   }
   if (n_threads == 1) {
     sample_worker(&jobs[0]);
@@ -281,6 +330,22 @@ int orc_iteration(const orc_params* p, uint32_t n, const double x0[4], const dou
   if (!XT) free(XT_buf);
   if (!u_all) free(u_buf);
   return nonfinite;
+}
+
+int orc_iteration(const orc_params* p, uint32_t n, const double x0[4], const double goal[4],
+                  int n_obs, const double* obstacles, const double* U_in, double* U_out,
+                  double* S, double* XT, double* u_all, double* w, int* argmin, double* gap,
+                  double* eta, int n_threads) {
+  return orc_iteration_se(p, n, x0, goal, n_obs, obstacles, 0, NULL, U_in, U_out, S, XT, u_all, w,
+                          argmin, gap, eta, n_threads);
+}
+
+/* Super-ellipse obstacles advance like discs: centre += dt * velocity (orientation fixed). */
+void orc_advance_se(const orc_params* p, int n_se, double* se) {
+  for (int i = 0; i < n_se; ++i) {
+    se[8 * i + 0] += p->dt * se[8 * i + 5];
+    se[8 * i + 1] += p->dt * se[8 * i + 6];
+  }
 }
 
 void orc_shift(int T, double* U) {

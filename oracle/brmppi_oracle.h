@@ -25,6 +25,8 @@
  *                              step, receding sample => 0, stationary inside => T*alpha*|h|
  *   weights / update / shift . pinned: positivity, sum to 1, shift invariance, permutation
  *                              invariance, lambda->0 argmin, lambda->inf mean, sigma=0 fixed point
+ *   super-ellipse barrier .... pinned: boundary points, e = 2 & m_x = m_y reduces to the disc barrier,
+ *                              rotation covariance, corner value, brute force with super-ellipses
  *   whole solve .............. pinned: brute force (independent mpmath transcription) K<=8, T<=5
  *   cost weights, disc placement, hinge shapes (linear barrier hinge, squared hitch hinge),
  *   scene generators ......... PARITY UNPINNED by the paper (never printed there); fixed by the
@@ -84,6 +86,11 @@ void orc_disc_centre(const orc_params* p, const double x[4], int j, double c[2])
 /* h = ||c - o||^2 / (R + r_v)^2 - 1 for disc centre c and obstacle centre o, radius R. */
 double orc_barrier(const orc_params* p, const double c[2], const double o[2], double R);
 
+/* Super-ellipse barrier, eq. (16) PAPER.md:216-221 (NEXT row 2 of SURVEY §8(f)):
+ *   h = |x'/(m_x + r_v)|^e + |y'/(m_y + r_v)|^e - 1,  (x', y') = R(-theta)(c - o).
+ * se = (cx, cy, m_x, m_y, theta, vx, vy, e); o = the obstacle centre at the step in question. */
+double orc_barrier_se(const orc_params* p, const double c[2], const double o[2], const double* se);
+
 /* G(x) = w_pos ||p - g_p||^2 + w_head (wrap(psi1-g_psi1)^2 + wrap(psi2-g_psi2)^2). */
 double orc_goal_cost(const orc_params* p, const double x[4], const double goal[4]);
 
@@ -127,6 +134,20 @@ int orc_iteration(const orc_params* p, uint32_t n, const double x0[4], const dou
                   int n_obs, const double* obstacles, const double* U_in, double* U_out,
                   double* S, double* XT, double* u_all, double* w, int* argmin, double* gap,
                   double* eta, int n_threads);
+
+/* The same three calls with n_se super-ellipse obstacles (8 doubles each, layout above) next to the
+ * discs; the barrier-rate hinge sums over both kinds.  The calls above are these with n_se = 0. */
+double orc_rollout_se(const orc_params* p, const double x0[4], const double goal[4], int n_obs,
+                      const double* obstacles, int n_se, const double* se, const double* u,
+                      double alpha, double xT[4], double* traj, double* pen_out);
+double orc_sample_se(const orc_params* p, uint32_t n, uint32_t k, const double x0[4],
+                     const double goal[4], int n_obs, const double* obstacles, int n_se,
+                     const double* se, const double* U_in, double* u, double xT[4]);
+int orc_iteration_se(const orc_params* p, uint32_t n, const double x0[4], const double goal[4],
+                     int n_obs, const double* obstacles, int n_se, const double* se,
+                     const double* U_in, double* U_out, double* S, double* XT, double* u_all,
+                     double* w, int* argmin, double* gap, double* eta, int n_threads);
+void orc_advance_se(const orc_params* p, int n_se, double* se);
 
 /* Warm-start shift: U[t] = U[t+1] for t < T-1; U[T-1] unchanged (reading 4). */
 void orc_shift(int T, double* U);

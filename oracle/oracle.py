@@ -79,6 +79,19 @@ def lib():
         L.orc_iteration.argtypes = [C.POINTER(_Params), C.c_uint32, _dp, _dp, C.c_int, _dp, _dp,
                                     _dp, _dp, _dp, _dp, _dp, C.POINTER(C.c_int), _dp, _dp, C.c_int]
         L.orc_iteration.restype = C.c_int
+        L.orc_barrier_se.argtypes = [C.POINTER(_Params), _dp, _dp, _dp]
+        L.orc_barrier_se.restype = C.c_double
+        L.orc_rollout_se.argtypes = [C.POINTER(_Params), _dp, _dp, C.c_int, _dp, C.c_int, _dp, _dp,
+                                     C.c_double, _dp, _dp, _dp]
+        L.orc_rollout_se.restype = C.c_double
+        L.orc_sample_se.argtypes = [C.POINTER(_Params), C.c_uint32, C.c_uint32, _dp, _dp, C.c_int, _dp,
+                                    C.c_int, _dp, _dp, _dp, _dp]
+        L.orc_sample_se.restype = C.c_double
+        L.orc_iteration_se.argtypes = [C.POINTER(_Params), C.c_uint32, _dp, _dp, C.c_int, _dp, C.c_int, _dp,
+                                       _dp, _dp, _dp, _dp, _dp, _dp, C.POINTER(C.c_int), _dp, _dp, C.c_int]
+        L.orc_iteration_se.restype = C.c_int
+        L.orc_advance_se.argtypes = [C.POINTER(_Params), C.c_int, _dp]
+        L.orc_advance_se.restype = None
         L.orc_shift.argtypes = [C.c_int, _dp]
         L.orc_shift.restype = None
         L.orc_plant_step.argtypes = [C.POINTER(_Params), _dp, _dp, C.c_int, _dp]
@@ -168,7 +181,20 @@ def goal_cost(p, x, goal):
     return lib().orc_goal_cost(C.byref(cp), _ptr(x), _ptr(goal))
 
 
-def rollout(p, x0, goal, obstacles, u, alpha_k, want_traj=False):
+def _se(superellipses):
+    """(n, 8) float64: cx, cy, m_x, m_y, theta, vx, vy, e."""
+    if superellipses is None:
+        return np.zeros((0, 8))
+    return _d(superellipses).reshape(-1, 8)
+
+
+def barrier_se(p, c, o, se):
+    cp = _cparams(p)
+    c, o, se = _d(c, (2,)), _d(o, (2,)), _d(se, (8,))
+    return lib().orc_barrier_se(C.byref(cp), _ptr(c), _ptr(o), _ptr(se))
+
+
+def rollout(p, x0, goal, obstacles, u, alpha_k, want_traj=False, superellipses=None):
     """One sample.  Returns dict(S, xT, pen, traj)."""
     cp = _cparams(p)
     x0, goal = _d(x0, (4,)), _d(goal, (4,))
@@ -177,13 +203,14 @@ def rollout(p, x0, goal, obstacles, u, alpha_k, want_traj=False):
     xT = np.zeros(4)
     traj = np.zeros((p.T + 1, 4)) if want_traj else None
     pen = C.c_double(0.0)
-    S = lib().orc_rollout(C.byref(cp), _ptr(x0), _ptr(goal), obstacles.shape[0], _ptr(obstacles),
-                          _ptr(u), float(alpha_k), _ptr(xT), _ptr(traj) if want_traj else None,
-                          C.cast(C.byref(pen), _dp))
+    se = _se(superellipses)
+    S = lib().orc_rollout_se(C.byref(cp), _ptr(x0), _ptr(goal), obstacles.shape[0], _ptr(obstacles),
+                             se.shape[0], _ptr(se), _ptr(u), float(alpha_k), _ptr(xT),
+                             _ptr(traj) if want_traj else None, C.cast(C.byref(pen), _dp))
     return dict(S=S, xT=xT, pen=pen.value, traj=traj)
 
 
-def sample(p, n, k, x0, goal, obstacles, U_in):
+def sample(p, n, k, x0, goal, obstacles, U_in, superellipses=None):
     """Sample k of iteration n alone: dict(S, xT, u)."""
     cp = _cparams(p)
     x0, goal = _d(x0, (4,)), _d(goal, (4,))
@@ -191,8 +218,9 @@ def sample(p, n, k, x0, goal, obstacles, U_in):
     U_in = _d(U_in, (p.T, 2))
     u = np.zeros((p.T, 2))
     xT = np.zeros(4)
-    S = lib().orc_sample(C.byref(cp), int(n), int(k), _ptr(x0), _ptr(goal), obstacles.shape[0],
-                         _ptr(obstacles), _ptr(U_in), _ptr(u), _ptr(xT))
+    se = _se(superellipses)
+    S = lib().orc_sample_se(C.byref(cp), int(n), int(k), _ptr(x0), _ptr(goal), obstacles.shape[0],
+                            _ptr(obstacles), se.shape[0], _ptr(se), _ptr(U_in), _ptr(u), _ptr(xT))
     return dict(S=S, xT=xT, u=u)
 
 
@@ -213,7 +241,7 @@ def weights_update(S, u, lam):
     return dict(U=U, w=w, argmin=am.value, gap=gap.value, eta=eta.value, nonfinite=nf)
 
 
-def iteration(p, n, x0, goal, obstacles, U_in, n_threads=1, want_samples=False):
+def iteration(p, n, x0, goal, obstacles, U_in, n_threads=1, want_samples=False, superellipses=None):
     """One MPPI iteration with global counter n.  Returns dict(U, S, XT, argmin, gap, eta,
     nonfinite[, u, w])."""
     cp = _cparams(p)
@@ -229,8 +257,9 @@ def iteration(p, n, x0, goal, obstacles, U_in, n_threads=1, want_samples=False):
     am = C.c_int(0)
     gap = C.c_double(0.0)
     eta = C.c_double(0.0)
-    nf = lib().orc_iteration(C.byref(cp), int(n), _ptr(x0), _ptr(goal), obstacles.shape[0],
-                             _ptr(obstacles), _ptr(U_in), _ptr(U), _ptr(S), _ptr(XT),
+    se = _se(superellipses)
+    nf = lib().orc_iteration_se(C.byref(cp), int(n), _ptr(x0), _ptr(goal), obstacles.shape[0],
+                             _ptr(obstacles), se.shape[0], _ptr(se), _ptr(U_in), _ptr(U), _ptr(S), _ptr(XT),
                              _ptr(u) if want_samples else None, _ptr(w) if want_samples else None,
                              C.byref(am), C.cast(C.byref(gap), _dp), C.cast(C.byref(eta), _dp),
                              int(n_threads))
@@ -240,16 +269,23 @@ def iteration(p, n, x0, goal, obstacles, U_in, n_threads=1, want_samples=False):
     return out
 
 
-def solve(p, n0, x0, goal, obstacles, U_in, n_threads=1):
+def solve(p, n0, x0, goal, obstacles, U_in, n_threads=1, superellipses=None):
     """p.n_iter iterations starting at counter n0, no shift in between (CFG2).  Returns the list
     of per-iteration results; the last one's U is the solve's output."""
     U = _d(U_in, (p.T, 2)).copy()
     outs = []
     for it in range(p.n_iter):
-        r = iteration(p, n0 + it, x0, goal, obstacles, U, n_threads=n_threads)
+        r = iteration(p, n0 + it, x0, goal, obstacles, U, n_threads=n_threads, superellipses=superellipses)
         U = r["U"]
         outs.append(r)
     return outs
+
+
+def advance_se(p, superellipses):
+    cp = _cparams(p)
+    se = _se(superellipses).copy()
+    lib().orc_advance_se(C.byref(cp), se.shape[0], _ptr(se))
+    return se
 
 
 def shift(U):

@@ -28,7 +28,7 @@ def wrap(a):
     return a - 2 * mp.pi * mp.nint(a / (2 * mp.pi))
 
 
-def brute_force(p, n, x0, goal, obstacles, U):
+def brute_force(p, n, x0, goal, obstacles, U, superellipses=()):
     K, T, D = p.K, p.T, len(p.discs)
     key = (p.seed & M32, p.seed >> 32)
     f = lambda w: mp.mpf(w >> 9) / 2**23
@@ -67,7 +67,20 @@ def brute_force(p, n, x0, goal, obstacles, U):
         oy = mpf(float(obstacles[i][1])) + t * mpf(p.dt) * mpf(float(obstacles[i][4]))
         rho = mpf(float(obstacles[i][2])) + mpf(p.disc_radius)
         return ((cx - ox) ** 2 + (cy - oy) ** 2) / rho**2 - 1
-    H = [[[[h(k, t, i, j) for j in range(D)] for i in range(len(obstacles))] for t in range(T + 1)] for k in range(K)]
+    def h_se(k, t, i, j):      # eq. (16)
+        x, y, p1, p2 = X[k][t]
+        body, off = p.discs[j]
+        ang = p1 if body == 0 else p2
+        cx = x - mpf(p.Lh) * mp.cos(p1) + mpf(off) * mp.cos(ang)
+        cy = y - mpf(p.Lh) * mp.sin(p1) + mpf(off) * mp.sin(ang)
+        ocx, ocy, mx, my, th, vx, vy, e = (mpf(float(a)) for a in superellipses[i])
+        dx, dy = cx - (ocx + t * mpf(p.dt) * vx), cy - (ocy + t * mpf(p.dt) * vy)
+        xp = mp.cos(th) * dx + mp.sin(th) * dy
+        yp = -mp.sin(th) * dx + mp.cos(th) * dy
+        return abs(xp / (mx + mpf(p.disc_radius))) ** e + abs(yp / (my + mpf(p.disc_radius))) ** e - 1
+    H = [[[[h(k, t, i, j) for j in range(D)] for i in range(len(obstacles))] +
+          [[h_se(k, t, i, j) for j in range(D)] for i in range(len(superellipses))]
+          for t in range(T + 1)] for k in range(K)]
     # 4. costs from the tables
     def G(s):
         return mpf(p.w_pos) * ((s[0] - mpf(float(goal[0]))) ** 2 + (s[1] - mpf(float(goal[1]))) ** 2) + \
@@ -75,7 +88,7 @@ def brute_force(p, n, x0, goal, obstacles, U):
     S = []
     for k in range(K):
         bar = sum(max(mpf(0), (1 - alpha[k]) * H[k][t][i][j] - H[k][t + 1][i][j])
-                  for t in range(T) for i in range(len(obstacles)) for j in range(D))
+                  for t in range(T) for i in range(len(obstacles) + len(superellipses)) for j in range(D))
         track = sum(G(X[k][t + 1]) for t in range(T))
         effort = sum(mpf(p.w_v) * u[k][t][0] ** 2 + mpf(p.w_delta) * u[k][t][1] ** 2 for t in range(T))
         hitch = sum(mpf(p.w_hitch) * max(mpf(0), abs(wrap(X[k][t + 1][2] - X[k][t + 1][3])) - mpf(p.hitch_max)) ** 2
@@ -89,7 +102,7 @@ def brute_force(p, n, x0, goal, obstacles, U):
     return dict(S=S, U=Unew, XT=[X[k][T] for k in range(K)], argmin=S.index(smin))
 
 
-@pytest.mark.parametrize("case", [0, 1, 2])
+@pytest.mark.parametrize("case", [0, 1, 2, 3])
 def test_oracle_matches_bruteforce(O, case):
     sc = scenes.scene_cfg0(case)
     if case == 0:
@@ -101,14 +114,21 @@ def test_oracle_matches_bruteforce(O, case):
         obs = np.array([[3.0, 0.5, 1.0, -1.0, 0.25], [-5.0, 1.0, 1.5, 0.0, 0.0]], dtype=np.float32).astype(float)
         x0 = np.array([0.5, -0.25, 0.4, -0.9], dtype=np.float32).astype(float)
         U = np.array([[1.0, 0.2], [-0.5, -0.3], [1.9, 0.55], [0.0, 0.0]], dtype=np.float32).astype(float)
+    elif case == 3:   # super-ellipse obstacles: a rotated parked car (e = 4) under the trailer's path, a walking pedestrian (e = 2)
+        p = sc.params.with_(K=6, T=5, seed=5, dt=0.2)
+        obs = sc.obstacles
+        x0, U = sc.x0, np.array([[-1.5, 0.1]] * 5, dtype=np.float32).astype(float)
+        se = np.array([[-9.0, 2.5, 2.25, 0.9, 0.6, 0.0, 0.0, 4.0], [-3.0, -2.0, 0.4, 0.4, 0.0, 0.3, 1.2, 2.0]], dtype=np.float32).astype(float)
     else:             # large hitch angle and headings near +-pi (wrap paths active)
         p = sc.params.with_(K=5, T=3, seed=77, sigma_v=1.0, sigma_delta=0.5, dt=0.5)
         obs = sc.obstacles
         x0 = np.array([1.0, 2.0, 3.0, -2.9], dtype=np.float32).astype(float)
         U = np.array([[-1.0, 0.5]] * 3, dtype=np.float32).astype(float)
+    if case != 3:
+        se = np.zeros((0, 8))
     n = 4
-    ref = brute_force(p, n, x0, sc.goal, obs, U)
-    got = O.iteration(p, n, x0, sc.goal, obs, U)
+    ref = brute_force(p, n, x0, sc.goal, obs, U, [tuple(r) for r in se])
+    got = O.iteration(p, n, x0, sc.goal, obs, U, superellipses=se)
     assert got["argmin"] == ref["argmin"]
     for k in range(p.K):
         assert abs(got["S"][k] - ref["S"][k]) <= 1e-12 * max(1, abs(ref["S"][k]))
