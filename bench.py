@@ -48,6 +48,8 @@ def workload(name, rank=0):
         sc = scenes.scene_cfg1(rank)
     elif name == "cfg2":
         sc = scenes.scene_cfg2(rank)
+    elif name == "cfg2se":
+        sc = scenes.scene_cfg2_superellipse(rank)
     elif name == "cfg3":
         sc = scenes.scene_cfg3(rank)
     else:
@@ -55,9 +57,15 @@ def workload(name, rank=0):
     return sc, sc.params
 
 
-def algorithmic_instr_per_sample_step(n_obs, n_discs):
-    """SURVEY.md §8(d) / DESIGN.md §6: issue slots the method itself needs per sample-step."""
-    return 121 + 8 * n_obs * n_discs
+def algorithmic_instr_per_sample_step(n_obs, n_discs, superellipses=None):
+    """SURVEY.md §8(d) / DESIGN.md §6: issue slots the method itself needs per sample-step.
+    Discs: 8 per (obstacle, disc).  Super-ellipses (eq. 16): 2 differences, 4 for the rotation and
+    scaling, 4 (e = 4) or 2 (e = 2) for the powers and their sum, rate argument, max, accumulate."""
+    n = 121 + 8 * n_obs * n_discs
+    if superellipses is not None:
+        for row in superellipses:
+            n += (13 if int(round(row[7])) == 4 else 11) * n_discs
+    return n
 
 
 def measured_peaks():
@@ -194,8 +202,11 @@ def run_reference(args):
 
 
 def workload_config(name, sc, p, n_scenes_total):
-    return {"workload": f"BASELINE.json configs[{name[-1]}] ({name})", "K": p.K, "T": p.T,
+    label = "BASELINE.json configs[2] with the paper's super-ellipse obstacles, eq. (16) (cfg2se)" if name == "cfg2se" \
+        else f"BASELINE.json configs[{name[-1]}] ({name})"
+    return {"workload": label, "K": p.K, "T": p.T,
             "n_obstacles": int(len(sc.obstacles)),
+            "n_superellipses": 0 if sc.superellipses is None else int(len(sc.superellipses)),
             "n_moving": int(np.count_nonzero(np.abs(sc.obstacles[:, 3:5]).sum(axis=1))) if len(sc.obstacles) else 0,
             "n_discs": len(p.discs), "n_iter": p.n_iter, "dt": p.dt, "scenes_total": n_scenes_total,
             "l2": "flushed between timed steps (256 MiB write); per-step CUDA-event pairs",
@@ -211,7 +222,8 @@ def run_ours(args):
     torch.cuda.set_device(dev)
     sc, p = workload(args.workload, rank)
     n_obs = len(sc.obstacles)
-    solver = B.Solver(p, 1, max(n_obs, 1), 0, device=dev)
+    n_se = 0 if sc.superellipses is None else len(sc.superellipses)
+    solver = B.Solver(p, 1, max(n_obs, 1), 0, device=dev, max_superellipses=n_se)
     solver.set_scene(sc)
     stream = solver.stream
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
@@ -249,20 +261,23 @@ def run_ours(args):
     # ---- end to end through the C ABI with host buffers (pinned), host clock
     pin = lambda a: torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).pin_memory().numpy()
     hx, hg, ho = pin(sc.x0), pin(sc.goal), pin(sc.obstacles)
+    hs = None if n_se == 0 else sc.superellipses
+    def set_inputs():
+        solver.set_state(hx); solver.set_goal(hg); solver.set_obstacles(ho)
+        if hs is not None:
+            solver.set_superellipses(hs)
     for _ in range(3):
-        solver.set_state(hx); solver.set_goal(hg); solver.set_obstacles(ho); solver.solve(); solver.get_controls()
+        set_inputs(); solver.solve(); solver.get_controls()
     barrier()
     t0 = time.perf_counter()
     for _ in range(args.steps):
-        solver.set_state(hx)
-        solver.set_goal(hg)
-        solver.set_obstacles(ho)
+        set_inputs()
         solver.solve()
         U = solver.get_controls()                            # synchronises; T*2 floats back
     barrier()
     e2e_s = time.perf_counter() - t0
     e2e_s_max = max_over_ranks(e2e_s, dist, dev)
-    h2d = 16 + 16 + 20 * n_obs + 4
+    h2d = 16 + 16 + 20 * n_obs + 4 + (32 * n_se + 4 if n_se else 0)
     d2h = 8 * p.T
 
     # ---- closed-loop control rate (CUDA-graph replay of solve + plant step + shift)
@@ -282,7 +297,7 @@ def run_ours(args):
         solver.set_scene(sc)
         solver.set_nominal(None)
         ms_roll, ms_upd = solver.time_kernels(50)
-        instr = algorithmic_instr_per_sample_step(n_obs, len(p.discs))
+        instr = algorithmic_instr_per_sample_step(n_obs, len(p.discs), sc.superellipses)
         achieved = p.K * p.T * instr / (ms_roll * 1e-3) / 1e9          # G thread-instr / s
         mp = measured_peaks()
         sm_max = float(mp.get("sm_max_mhz", SM_MAX_MHZ_FALLBACK))
@@ -340,7 +355,8 @@ def run_phases(args):
     import torch  # noqa: F401
     from paper_2508_05773_b200 import brmppi as B
     sc, p = workload(args.workload)
-    s = B.Solver(p.with_(n_iter=1), 1, max(len(sc.obstacles), 1), B.FLAG_PHASE_TIMING)
+    n_se = 0 if sc.superellipses is None else len(sc.superellipses)
+    s = B.Solver(p.with_(n_iter=1), 1, max(len(sc.obstacles), 1), B.FLAG_PHASE_TIMING, max_superellipses=n_se)
     s.set_scene(sc)
     for _ in range(5):
         s.solve()
@@ -388,7 +404,7 @@ def main():
     ap.add_argument("--steps", type=int, default=200)
     ap.add_argument("--warmup", type=int, default=20)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="cfg2", choices=["cfg0", "cfg1", "cfg2", "cfg3"])
+    ap.add_argument("--workload", default="cfg2", choices=["cfg0", "cfg1", "cfg2", "cfg2se", "cfg3"])
     ap.add_argument("--phases", action="store_true", help="print the rollout kernel's in-kernel phase times")
     ap.add_argument("--sweep", action="store_true", help="run BASELINE.json configs[4] (sweep + 64-scene batch)")
     args = ap.parse_args()

@@ -59,6 +59,13 @@ typedef enum {
  * centre at rollout step t is (cx + t dt vx, cy + t dt vy).  radius > 0. */
 typedef struct { float cx, cy, radius, vx, vy; } brmppi_obstacle;
 
+/* Super-ellipse obstacle, eq. (16): centre (cx, cy), semi-axes (mx, my) along
+ * the obstacle's own axes, orientation theta (rad), constant velocity (vx, vy) of the centre.
+ *   h = (x'/(mx + r_v))^e + (y'/(my + r_v))^e - 1,  (x', y') = R(-theta)(c - centre(t)).
+ * exponent e: 4 (parked cars in the paper) or 2 (pedestrians); other values are rejected.  The
+ * barrier-rate hinge sums over discs and super-ellipses alike.  Default kernel only. */
+typedef struct { float cx, cy, mx, my, theta, vx, vy; int exponent; } brmppi_superellipse;
+
 /* Vehicle disc: body 0 = tractor axis (psi1), 1 = trailer axis (psi2); offset in metres from the
  * hitch point p_h = (x - Lh cos psi1, y - Lh sin psi1) along that axis. */
 typedef struct { int body; float offset; } brmppi_disc;
@@ -92,10 +99,12 @@ typedef struct {
   float w_pos, w_head, w_v, w_delta, w_hitch, hitch_max, w_bar, w_term, lambda;
   unsigned long long seed;
   unsigned int flags;
+  int max_superellipses;  /* capacity per scene, 0..BRMPPI_MAX_SUPERELLIPSES                     */
 } brmppi_params;
 
 #define BRMPPI_MAX_T 512
 #define BRMPPI_MAX_OBSTACLES 64
+#define BRMPPI_MAX_SUPERELLIPSES 16
 
 typedef struct brmppi_ctx brmppi_ctx;   /* opaque, library-owned host object */
 
@@ -126,6 +135,9 @@ int brmppi_set_state(brmppi_ctx* ctx, int scene, const float x[4]);
 int brmppi_set_goal(brmppi_ctx* ctx, int scene, const float g[4]);
 /* Obstacles of one scene at rollout time 0; 0 <= n <= max_obstacles (NULL allowed when n = 0). */
 int brmppi_set_obstacles(brmppi_ctx* ctx, int scene, int n, const brmppi_obstacle* obstacles);
+/* Super-ellipse obstacles of one scene at rollout time 0; 0 <= n <= max_superellipses (NULL allowed
+ * when n = 0).  mx, my > 0; exponent 2 or 4 (else BRMPPI_ERR_INVALID_ARG). */
+int brmppi_set_superellipses(brmppi_ctx* ctx, int scene, int n, const brmppi_superellipse* obstacles);
 /* Nominal control sequence U[T][2] = (v, delta) per step; NULL = zeros.  Values must lie in
  * the control box (else BRMPPI_ERR_INVALID_ARG). */
 int brmppi_set_nominal(brmppi_ctx* ctx, int scene, const float* U);
@@ -149,6 +161,7 @@ int brmppi_step(brmppi_ctx* ctx, float* u0_out);
 int brmppi_get_controls(brmppi_ctx* ctx, int scene, float* U_out /* T*2 */);
 int brmppi_get_state(brmppi_ctx* ctx, int scene, float x_out[4]);
 int brmppi_get_obstacles(brmppi_ctx* ctx, int scene, int* n_out, brmppi_obstacle* out /* max_obstacles */);
+int brmppi_get_superellipses(brmppi_ctx* ctx, int scene, int* n_out, brmppi_superellipse* out /* max_superellipses */);
 int brmppi_get_costs(brmppi_ctx* ctx, int scene, float* S_out /* K */);             /* FLAG_WRITE_SAMPLES */
 int brmppi_get_final_states(brmppi_ctx* ctx, int scene, float* X_out /* K*4 */);    /* FLAG_WRITE_SAMPLES */
 int brmppi_get_diag(brmppi_ctx* ctx, int scene, brmppi_diag* out);

@@ -23,7 +23,7 @@ ERR_NONFINITE_INPUT, ERR_NOT_READY, ERR_CUDA, ERR_UNALIGNED = -5, -6, -7, -8
 
 EXPORTS = [
     "brmppi_workspace_bytes", "brmppi_create", "brmppi_destroy", "brmppi_set_state",
-    "brmppi_set_goal", "brmppi_set_obstacles", "brmppi_set_nominal", "brmppi_set_counter",
+    "brmppi_set_goal", "brmppi_set_obstacles", "brmppi_set_superellipses", "brmppi_get_superellipses", "brmppi_set_nominal", "brmppi_set_counter",
     "brmppi_reset", "brmppi_solve", "brmppi_shift", "brmppi_step", "brmppi_get_controls",
     "brmppi_get_state", "brmppi_get_obstacles", "brmppi_get_costs", "brmppi_get_final_states",
     "brmppi_get_diag", "brmppi_get_phase_times", "brmppi_time_kernels", "brmppi_launch_count", "brmppi_strerror", "brmppi_debug_philox",
@@ -34,6 +34,11 @@ EXPORTS = [
 class Obstacle(C.Structure):
     _fields_ = [("cx", C.c_float), ("cy", C.c_float), ("radius", C.c_float),
                 ("vx", C.c_float), ("vy", C.c_float)]
+
+
+class Superellipse(C.Structure):
+    _fields_ = [("cx", C.c_float), ("cy", C.c_float), ("mx", C.c_float), ("my", C.c_float),
+                ("theta", C.c_float), ("vx", C.c_float), ("vy", C.c_float), ("exponent", C.c_int)]
 
 
 class Disc(C.Structure):
@@ -52,7 +57,7 @@ class CParams(C.Structure):
                 ("w_pos", C.c_float), ("w_head", C.c_float), ("w_v", C.c_float),
                 ("w_delta", C.c_float), ("w_hitch", C.c_float), ("hitch_max", C.c_float),
                 ("w_bar", C.c_float), ("w_term", C.c_float), ("lam", C.c_float),
-                ("seed", C.c_ulonglong), ("flags", C.c_uint)]
+                ("seed", C.c_ulonglong), ("flags", C.c_uint), ("max_superellipses", C.c_int)]
 
 
 class Diag(C.Structure):
@@ -85,6 +90,8 @@ def lib():
         L.brmppi_set_state.argtypes = [vp, C.c_int, _fp]
         L.brmppi_set_goal.argtypes = [vp, C.c_int, _fp]
         L.brmppi_set_obstacles.argtypes = [vp, C.c_int, C.c_int, C.POINTER(Obstacle)]
+        L.brmppi_set_superellipses.argtypes = [vp, C.c_int, C.c_int, C.POINTER(Superellipse)]
+        L.brmppi_get_superellipses.argtypes = [vp, C.c_int, C.POINTER(C.c_int), C.POINTER(Superellipse)]
         L.brmppi_set_nominal.argtypes = [vp, C.c_int, _fp]
         L.brmppi_set_counter.argtypes = [vp, C.c_uint]
         L.brmppi_reset.argtypes = [vp]
@@ -119,7 +126,7 @@ def _check(status):
         raise BrmppiError(status, strerror(status))
 
 
-def make_cparams(p, n_scenes=1, max_obstacles=8, flags=0) -> CParams:
+def make_cparams(p, n_scenes=1, max_obstacles=8, flags=0, max_superellipses=0) -> CParams:
     """scenes.Params (plain data) -> brmppi_params."""
     c = CParams()
     c.K, c.T, c.n_iter, c.n_scenes = int(p.K), int(p.T), int(p.n_iter), int(n_scenes)
@@ -131,6 +138,7 @@ def make_cparams(p, n_scenes=1, max_obstacles=8, flags=0) -> CParams:
                  "w_delta", "w_hitch", "hitch_max", "w_bar", "w_term", "lam"):
         setattr(c, name, float(getattr(p, name)))
     c.seed, c.flags = int(p.seed) & 0xFFFFFFFFFFFFFFFF, int(flags)
+    c.max_superellipses = int(max_superellipses)
     return c
 
 
@@ -146,7 +154,8 @@ def _p(a):
 class Solver:
     """One brmppi_ctx plus the torch-owned workspace and stream it lives on."""
 
-    def __init__(self, params, n_scenes=1, max_obstacles=8, flags=0, stream=None, device="cuda:0"):
+    def __init__(self, params, n_scenes=1, max_obstacles=8, flags=0, stream=None, device="cuda:0",
+                 max_superellipses=0):
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("brmppi needs a CUDA device (there is no CPU fallback)")
@@ -154,7 +163,8 @@ class Solver:
         self.device = torch.device(device)
         torch.cuda.set_device(self.device)
         self.params = params
-        self.cparams = make_cparams(params, n_scenes, max_obstacles, flags)
+        self.cparams = make_cparams(params, n_scenes, max_obstacles, flags, max_superellipses)
+        self.max_superellipses = int(max_superellipses)
         self.n_scenes, self.K, self.T = int(n_scenes), int(params.K), int(params.T)
         self.max_obstacles = int(max_obstacles)
         L = lib()
@@ -194,6 +204,20 @@ class Solver:
         ptr = obs.ctypes.data_as(C.POINTER(Obstacle)) if n else None
         _check(lib().brmppi_set_obstacles(self._ctx, scene, n, ptr))
 
+    def set_superellipses(self, superellipses, scene=0):
+        """rows (cx, cy, mx, my, theta, vx, vy, exponent)"""
+        se = np.asarray(superellipses, dtype=np.float64).reshape(-1, 8)
+        arr = (Superellipse * max(len(se), 1))()
+        for i, r in enumerate(se):
+            arr[i] = Superellipse(*[float(x) for x in r[:7]], int(round(r[7])))
+        _check(lib().brmppi_set_superellipses(self._ctx, scene, len(se), arr if len(se) else None))
+
+    def get_superellipses(self, scene=0):
+        n = C.c_int(0)
+        arr = (Superellipse * max(self.max_superellipses, 1))()
+        _check(lib().brmppi_get_superellipses(self._ctx, scene, C.byref(n), arr))
+        return np.array([[a.cx, a.cy, a.mx, a.my, a.theta, a.vx, a.vy, a.exponent] for a in arr[:n.value]]).reshape(-1, 8)
+
     def set_nominal(self, U=None, scene=0):
         _check(lib().brmppi_set_nominal(self._ctx, scene, None if U is None else _p(_f32(U, (self.T, 2)))))
 
@@ -207,6 +231,9 @@ class Solver:
         self.set_state(scene_obj.x0, scene)
         self.set_goal(scene_obj.goal, scene)
         self.set_obstacles(scene_obj.obstacles, scene)
+        if self.max_superellipses > 0:
+            se = getattr(scene_obj, "superellipses", None)
+            self.set_superellipses(np.zeros((0, 8)) if se is None else se, scene)
 
     # ---- work ---------------------------------------------------------------------------
     def solve(self):

@@ -50,6 +50,8 @@ bool params_valid(const brmppi_params* p) {
   if (p->n_iter < 1 || p->n_scenes < 1 || p->n_scenes > 65535) return false;
   if ((long long)p->K * p->n_scenes > 0x7fffffffLL) return false;
   if (p->max_obstacles < 0 || p->max_obstacles > BRMPPI_MAX_OBSTACLES) return false;
+  if (p->max_superellipses < 0 || p->max_superellipses > BRMPPI_MAX_SUPERELLIPSES) return false;
+  if (p->max_superellipses > 0 && (p->flags & BRMPPI_FLAG_KERNEL_THREAD_PER_SAMPLE)) return false;   // default kernel only
   if (p->n_discs < 1 || p->n_discs > BRMPPI_MAX_DISCS) return false;
   for (int j = 0; j < p->n_discs; ++j) {
     if (p->discs[j].body != 0 && p->discs[j].body != 1) return false;
@@ -73,7 +75,7 @@ bool params_valid(const brmppi_params* p) {
 }
 
 struct Layout {
-  size_t state, goal, n_obs, obstacles, U, counter, u0, part_m, part_argmin, part_eta, part_w2,
+  size_t state, goal, n_obs, obstacles, n_se, se, U, counter, u0, part_m, part_argmin, part_eta, part_w2,
       part_nf, part_A, diag, S, XT, phase, total;
 };
 
@@ -103,7 +105,7 @@ Plan make_plan(const brmppi_params& p) {
   Plan pl{};
   pl.cta_kernel = !(p.flags & BRMPPI_FLAG_KERNEL_THREAD_PER_SAMPLE);
   if (pl.cta_kernel) {
-    pl.cta = make_cta_plan(p.K, p.T, p.n_scenes, p.max_obstacles, device_sm_count());
+    pl.cta = make_cta_plan(p.K, p.T, p.n_scenes, p.max_obstacles, p.max_superellipses, device_sm_count());
     pl.n_partials = pl.cta.n_partials;
   } else {
     pl.n_partials = (p.K + kThreadBlock - 1) / kThreadBlock;
@@ -120,6 +122,8 @@ Layout make_layout(const brmppi_params& p, const Plan& pl) {
   L.goal = take(ns * 16);
   L.n_obs = take(ns * 4);
   L.obstacles = take(ns * (size_t)(p.max_obstacles > 0 ? p.max_obstacles : 1) * 20);
+  L.n_se = take(ns * 4);
+  L.se = take(ns * (size_t)(p.max_superellipses > 0 ? p.max_superellipses : 1) * 32);
   L.U = take(ns * T * 8);
   L.counter = take(4);
   L.u0 = take(ns * 8);
@@ -289,7 +293,8 @@ int brmppi_create(const brmppi_params* p, void* dev_workspace, size_t workspace_
     d.S_tile = cp.S_tile; d.tiles_per_scene = cp.tiles_per_scene; d.total_tiles = cp.total_tiles;
     d.tiles_per_cta = cp.tiles_per_cta;
     d.chunks = cp.chunks; d.chunk_len = cp.chunk_len; d.t_stride = cp.ts; d.obs_padded = cp.obs_padded;
-    const CtaSmem ts = cta_smem_layout(d.T, cp.S_tile, cp.chunks, cp.ts, cp.obs_padded);
+    const CtaSmem ts = cta_smem_layout(d.T, cp.S_tile, cp.chunks, cp.ts, cp.obs_padded, cp.se_padded);
+    d.se_padded = cp.se_padded; d.off_se = (int)ts.se;
     d.off_obs = (int)ts.obs; d.off_vel = (int)ts.vel; d.off_spd = (int)ts.spd; d.off_raw = (int)ts.raw; d.off_A = (int)ts.A;
     d.off_scratch = (int)ts.scratch; d.off_w = (int)ts.w; d.off_alpha = (int)ts.alpha;
     d.off_cost = (int)ts.cost; d.off_xy = (int)ts.xy;
@@ -299,6 +304,7 @@ int brmppi_create(const brmppi_params* p, void* dev_workspace, size_t workspace_
   const Layout& L = c->layout;
   d.state = (float*)(base + L.state); d.goal = (float*)(base + L.goal);
   d.n_obs = (int*)(base + L.n_obs); d.obstacles = (float*)(base + L.obstacles);
+  d.n_se = (int*)(base + L.n_se); d.se = (float*)(base + L.se); d.max_superellipses = p->max_superellipses;
   d.U = (float*)(base + L.U); d.counter = (uint32_t*)(base + L.counter);
   d.u0_applied = (float*)(base + L.u0);
   d.part_m = (double*)(base + L.part_m); d.part_argmin = (int*)(base + L.part_argmin);
@@ -395,6 +401,28 @@ int brmppi_set_obstacles(brmppi_ctx* c, int scene, int n, const brmppi_obstacle*
     CU(cudaMemcpyAsync(c->d.obstacles + (size_t)scene * c->p.max_obstacles * 5, obs,
                        sizeof(brmppi_obstacle) * (size_t)n, cudaMemcpyHostToDevice, c->stream));
   CU(cudaMemcpyAsync(c->d.n_obs + scene, &n, sizeof(int), cudaMemcpyHostToDevice, c->stream));
+  return BRMPPI_OK;
+}
+
+int brmppi_set_superellipses(brmppi_ctx* c, int scene, int n, const brmppi_superellipse* se) {
+  int r = check_scene(c, scene);
+  if (r) return r;
+  if (n < 0) return BRMPPI_ERR_INVALID_ARG;
+  if (n > c->p.max_superellipses) return BRMPPI_ERR_TOO_MANY_OBSTACLES;
+  if (n > 0 && !se) return BRMPPI_ERR_NULL;
+  float rec[BRMPPI_MAX_SUPERELLIPSES][8];
+  for (int i = 0; i < n; ++i) {
+    if (!finite_all(&se[i].cx, 7)) return BRMPPI_ERR_NONFINITE_INPUT;
+    if (!(se[i].mx > 0.f) || !(se[i].my > 0.f)) return BRMPPI_ERR_INVALID_ARG;
+    if (se[i].exponent != 2 && se[i].exponent != 4) return BRMPPI_ERR_INVALID_ARG;
+    memcpy(rec[i], &se[i].cx, 7 * sizeof(float));
+    rec[i][7] = (float)se[i].exponent;
+  }
+  if (n > 0)
+    CU(cudaMemcpyAsync(c->d.se + (size_t)scene * c->p.max_superellipses * 8, rec, sizeof(float) * 8 * (size_t)n,
+                       cudaMemcpyHostToDevice, c->stream));
+  CU(cudaMemcpyAsync(c->d.n_se + scene, &n, sizeof(int), cudaMemcpyHostToDevice, c->stream));
+  CU(cudaStreamSynchronize(c->stream));     // rec is a stack buffer
   return BRMPPI_OK;
 }
 
@@ -507,6 +535,21 @@ int brmppi_get_obstacles(brmppi_ctx* c, int scene, int* n_out, brmppi_obstacle* 
   if (out && *n_out > 0)
     return d2h(c, out, c->d.obstacles + (size_t)scene * c->p.max_obstacles * 5,
                sizeof(brmppi_obstacle) * (size_t)*n_out);
+  return BRMPPI_OK;
+}
+
+int brmppi_get_superellipses(brmppi_ctx* c, int scene, int* n_out, brmppi_superellipse* out) {
+  int r = check_scene(c, scene);
+  if (r) return r;
+  if (!n_out) return BRMPPI_ERR_NULL;
+  r = d2h(c, n_out, c->d.n_se + scene, sizeof(int));
+  if (r) return r;
+  if (out && *n_out > 0) {
+    float rec[BRMPPI_MAX_SUPERELLIPSES][8];
+    r = d2h(c, rec, c->d.se + (size_t)scene * c->p.max_superellipses * 8, sizeof(float) * 8 * (size_t)*n_out);
+    if (r) return r;
+    for (int i = 0; i < *n_out; ++i) { memcpy(&out[i].cx, rec[i], 7 * sizeof(float)); out[i].exponent = (int)rec[i][7]; }
+  }
   return BRMPPI_OK;
 }
 

@@ -20,7 +20,7 @@ constexpr float kInvTwoPi = 0.15915494309189535f;
 // Everything a kernel needs, passed by value as a __grid_constant__ parameter (constant bank,
 // so scalar weights fold into FFMA operands without a load).
 struct DeviceParams {
-  int K, T, n_scenes, max_obstacles, n_discs;
+  int K, T, n_scenes, max_obstacles, n_discs, max_superellipses;
   int disc_body[kMaxDiscs];
   float disc_offset[kMaxDiscs];
   float disc_radius;
@@ -41,6 +41,8 @@ struct DeviceParams {
   int chunks, chunk_len;      // C threads per sample in the barrier phase, L steps per thread
   int t_stride;               // padded row length of the shared-memory planes
   int obs_padded;             // obstacle slots, a multiple of the group size
+  int se_padded;              // super-ellipse slots, a multiple of kSeGroup (0 if none)
+  int off_se;                 // shared-memory section of the super-ellipse table
   // byte offsets of the shared-memory sections (host-computed, so that the device code
   // rematerialises a pointer with one add instead of keeping it in a register)
   int off_obs, off_vel, off_spd, off_raw, off_A, off_scratch, off_w, off_alpha, off_cost, off_xy,
@@ -50,6 +52,8 @@ struct DeviceParams {
   float* goal;                // [n_scenes][4]
   int* n_obs;                 // [n_scenes]
   float* obstacles;           // [n_scenes][max_obstacles][5]
+  int* n_se;                  // [n_scenes]
+  float* se;                  // [n_scenes][max_superellipses][8]: cx, cy, mx, my, theta, vx, vy, exponent
   float* U;                   // [n_scenes][T][2]
   uint32_t* counter;          // global iteration counter n
   float* u0_applied;          // [n_scenes][2]  control applied by the last plant step

@@ -46,6 +46,7 @@ constexpr int kCtaThreads = BRMPPI_CTA_THREADS;
 constexpr int kChainWarps = 4;                      // one per warp scheduler
 constexpr int kMaxTileSamples = kChainWarps * 32;   // 128
 constexpr int kObsGroup = 8;                        // obstacles whose h_t are held in registers at a time
+constexpr int kSeGroup = 4;                         // super-ellipses whose h_t are held in registers at a time
 constexpr int kMaxChunks = 16;
 constexpr int kMinChunkLen = 4;
 constexpr int kMinCullChunk = 8;                    // culling pays from this chunk length on
@@ -58,7 +59,7 @@ struct CtaMisc {            // lives in the "misc" section
   int argmin[2];
   float eta[2], w2[2];
   int nonfinite[2];
-  int n_obs, n_moving, n_groups;
+  int n_obs, n_moving, n_groups, n_se_groups;
   float4 x0, g;             // start state; goal in the vehicle-centred frame
   double redM[kChainWarps];
   int redI[kChainWarps];
@@ -67,12 +68,12 @@ struct CtaMisc {            // lives in the "misc" section
 };
 
 struct CtaSmem {
-  size_t obs, vel, spd, raw, A, scratch, w, alpha, cost, xy, planes, misc, total;
+  size_t obs, vel, spd, raw, se, A, scratch, w, alpha, cost, xy, planes, misc, total;
 };
 
 // Shared-memory carve-up (host only: the kernel gets the byte offsets through DeviceParams, so
 // that a section pointer is smem_raw + a constant-bank offset instead of a live register).
-inline CtaSmem cta_smem_layout(int T, int S, int chunks, int ts, int obs_padded) {
+inline CtaSmem cta_smem_layout(int T, int S, int chunks, int ts, int obs_padded, int se_padded) {
   CtaSmem L{};
   size_t off = 0;
   auto take = [&](size_t b) { size_t o = off; off = (off + b + 15) / 16 * 16; return o; };
@@ -80,6 +81,7 @@ inline CtaSmem cta_smem_layout(int T, int S, int chunks, int ts, int obs_padded)
   L.vel = take(sizeof(float2) * (size_t)obs_padded);
   L.spd = take(sizeof(float) * (size_t)obs_padded);       // obstacle displacement per step
   L.raw = take(sizeof(float) * 5 * (size_t)obs_padded);   // obstacles as given, before sorting
+  L.se = take(sizeof(float) * 12 * (size_t)se_padded);    // SeRecord per super-ellipse
   L.A = take(sizeof(float) * 2 * (size_t)T);
   L.scratch = take(sizeof(float) * kCtaThreads);
   L.w = take(sizeof(float) * (size_t)S);
@@ -94,7 +96,7 @@ inline CtaSmem cta_smem_layout(int T, int S, int chunks, int ts, int obs_padded)
 
 struct CtaPlan {
   int S_tile, tiles_per_scene, total_tiles, grid, tiles_per_cta, chunks, chunk_len, ts, obs_padded,
-      n_partials;
+      se_padded, n_partials;
   size_t smem;
 };
 
@@ -115,19 +117,20 @@ inline void cta_chunking(int T, int S, int* chunks, int* chunk_len) {
   *chunks = (T + L - 1) / L;
 }
 
-inline size_t cta_smem_bytes(int T, int S, int obs_padded, int* chunks, int* chunk_len, int* ts) {
+inline size_t cta_smem_bytes(int T, int S, int obs_padded, int se_padded, int* chunks, int* chunk_len, int* ts) {
   cta_chunking(T, S, chunks, chunk_len);
   *ts = (T + 1) | 1;                     // T+1 entries per row, odd length: conflict-free planes
-  return cta_smem_layout(T, S, *chunks, *ts, obs_padded).total;
+  return cta_smem_layout(T, S, *chunks, *ts, obs_padded, se_padded).total;
 }
 
-inline CtaPlan make_cta_plan(int K, int T, int n_scenes, int max_obstacles, int n_sms) {
+inline CtaPlan make_cta_plan(int K, int T, int n_scenes, int max_obstacles, int max_superellipses, int n_sms) {
   CtaPlan pl{};
   pl.obs_padded = max_obstacles > 0 ? (max_obstacles + kObsGroup - 1) / kObsGroup * kObsGroup : kObsGroup;
+  pl.se_padded = (max_superellipses + kSeGroup - 1) / kSeGroup * kSeGroup;
   // largest tile that fits in shared memory
   int s_max = K < kMaxTileSamples ? K : kMaxTileSamples;
   int c, l, ts;
-  while (s_max > 1 && cta_smem_bytes(T, s_max, pl.obs_padded, &c, &l, &ts) > kSmemMax) --s_max;
+  while (s_max > 1 && cta_smem_bytes(T, s_max, pl.obs_padded, pl.se_padded, &c, &l, &ts) > kSmemMax) --s_max;
   if (const char* e = getenv("BRMPPI_MAX_TILE")) {   // tuning knob for sweeps
     const int v = atoi(e);
     if (v >= 1 && v < s_max) s_max = v;
@@ -150,7 +153,7 @@ inline CtaPlan make_cta_plan(int K, int T, int n_scenes, int max_obstacles, int 
   int np = (pl.tiles_per_scene + pl.tiles_per_cta - 2) / pl.tiles_per_cta + 1;
   if (np > pl.grid) np = pl.grid;
   pl.n_partials = np;
-  pl.smem = cta_smem_bytes(T, pl.S_tile, pl.obs_padded, &pl.chunks, &pl.chunk_len, &pl.ts);
+  pl.smem = cta_smem_bytes(T, pl.S_tile, pl.obs_padded, pl.se_padded, &pl.chunks, &pl.chunk_len, &pl.ts);
   return pl;
 }
 

@@ -150,6 +150,77 @@ __device__ __forceinline__ GroupCost barrier_group(const DeviceParams& P, const 
   return GroupCost{track, bar};
 }
 
+// Super-ellipse obstacles (eq. (16)), kSeGroup at a time:
+//   (x', y') = R(-theta)(c - o(t)),  h = (x'/(m_x + r_v))^e + (y'/(m_y + r_v))^e - 1,  e = 2 or 4,
+// and the same barrier-rate hinge as for discs.  The record holds the rows of R(-theta) divided by
+// the inflated semi-axes, so u = x'/a_x and v = y'/a_y cost two FMA-pipe instructions each.
+// Per (obstacle, disc): 2 subtractions, 4 for (u, v), 4 for u^4 + v^4 - 1 (2 for e = 2), rate
+// argument, |.|-add, accumulate = 13 (11).  A null record has weight 0.
+struct SeRecord { float ox, oy, a11, a12, a21, a22, wx, wy, e4, half_w, pad0, pad1; };
+static_assert(sizeof(SeRecord) == 48, "SeRecord layout");
+
+template <bool PRECISE, int ND>
+__device__ __forceinline__ double se_group(const DeviceParams& P, const float* __restrict__ pV,
+                                           const float* __restrict__ pP1, const float* __restrict__ pP2,
+                                           const SeRecord* __restrict__ rec, float x, float y, int t0, int t1,
+                                           float one_minus_alpha) {
+  double bar = 0.0;
+  float hprev[kSeGroup][ND];
+  float s1, c1;
+  {
+    float s2, c2;
+    sincos_t<PRECISE>(pP1[t0], &s1, &c1);
+    sincos_t<PRECISE>(pP2[t0], &s2, &c2);
+    float cx[ND], cy[ND];
+    disc_centres_n<ND>(P, x, y, s1, c1, s2, c2, cx, cy);
+    const float tf = (float)t0;
+#pragma unroll
+    for (int i = 0; i < kSeGroup; ++i) {
+      const SeRecord r = rec[i];
+      const float ox = fmaf(tf, r.wx, r.ox), oy = fmaf(tf, r.wy, r.oy);
+#pragma unroll
+      for (int j = 0; j < ND; ++j) {
+        const float dx = cx[j] - ox, dy = cy[j] - oy;
+        const float u = fmaf(r.a11, dx, r.a12 * dy), v = fmaf(r.a21, dx, r.a22 * dy);
+        const float u2 = u * u, v2 = v * v;
+        hprev[i][j] = r.e4 != 0.0f ? fmaf(u2, u2, fmaf(v2, v2, -1.0f)) : fmaf(u, u, fmaf(v, v, -1.0f));
+      }
+    }
+  }
+  float tf = (float)t0;
+  for (int t = t0; t < t1; ++t) {
+    const float a = P.dt * pV[t];
+    x = fmaf(a, c1, x);
+    y = fmaf(a, s1, y);
+    float s2, c2;
+    sincos_t<PRECISE>(pP1[t + 1], &s1, &c1);
+    sincos_t<PRECISE>(pP2[t + 1], &s2, &c2);
+    float cx[ND], cy[ND];
+    disc_centres_n<ND>(P, x, y, s1, c1, s2, c2, cx, cy);
+    tf += 1.0f;
+    float pen = 0.0f;
+#pragma unroll
+    for (int i = 0; i < kSeGroup; ++i) {
+      const SeRecord r = rec[i];
+      const float ox = fmaf(tf, r.wx, r.ox), oy = fmaf(tf, r.wy, r.oy);
+      float Pi = 0.0f;
+#pragma unroll
+      for (int j = 0; j < ND; ++j) {
+        const float dx = cx[j] - ox, dy = cy[j] - oy;
+        const float u = fmaf(r.a11, dx, r.a12 * dy), v = fmaf(r.a21, dx, r.a22 * dy);
+        const float u2 = u * u, v2 = v * v;
+        const float hn = r.e4 != 0.0f ? fmaf(u2, u2, fmaf(v2, v2, -1.0f)) : fmaf(u, u, fmaf(v, v, -1.0f));   // obstacle-uniform
+        const float z = fmaf(one_minus_alpha, hprev[i][j], -hn);
+        Pi += z + fabsf(z);                                       // 2 max(0, z), exactly
+        hprev[i][j] = hn;
+      }
+      pen = fmaf(r.half_w, Pi, pen);
+    }
+    bar += (double)pen;
+  }
+  return bar;
+}
+
 // Dispatch on the number of moving obstacles in the group (block-uniform).
 template <bool PRECISE, int ND, bool TRACK, bool CULL>
 __device__ __forceinline__ GroupCost barrier_group_nm(int nm, const DeviceParams& P, const float* pV,
@@ -357,9 +428,28 @@ rollout_cta(const __grid_constant__ DeviceParams P) {
           sSpd[i] = 0.0f;
         }
       }
+      // super-ellipse table: rows of R(-theta) over the inflated semi-axes; null records weigh 0
+      const int n_se = P.max_superellipses > 0 ? P.n_se[scene] : 0;
+      SeRecord* sSE = BRMPPI_SMEM(SeRecord, P.off_se);
+      for (int i = lane; i < P.se_padded; i += 32) {
+        SeRecord r = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+        if (i < n_se) {
+          const float* q = P.se + ((size_t)scene * P.max_superellipses + i) * 8;
+          float st, ct;
+          sincosf(q[4], &st, &ct);
+          const float iax = 1.0f / (q[2] + P.disc_radius), iay = 1.0f / (q[3] + P.disc_radius);
+          r.ox = q[0] - x0.x; r.oy = q[1] - x0.y;
+          r.a11 = ct * iax; r.a12 = st * iax; r.a21 = -st * iay; r.a22 = ct * iay;
+          r.wx = P.dt * q[5]; r.wy = P.dt * q[6];
+          r.e4 = q[7] == 4.0f ? 1.0f : 0.0f;
+          r.half_w = 0.5f;
+        }
+        sSE[i] = r;
+      }
       if (lane == 0) {
         sM->n_moving = nm;
         sM->n_groups = n_obs > 0 ? (n_obs + kObsGroup - 1) / kObsGroup : 1;
+        sM->n_se_groups = (n_se + kSeGroup - 1) / kSeGroup;
       }
     }
     __syncthreads();
@@ -399,6 +489,8 @@ rollout_cta(const __grid_constant__ DeviceParams P) {
           bar += barrier_group_nm<PRECISE, ND, false, true>(n_moving - ib, P, pV, pP1, pP2, sObs + ib, sVel + ib, sSpd + ib, xy.x, xy.y, t0, t1, one_minus_alpha, g).bar;
         }
       }
+      for (int grp = 0; grp < sM->n_se_groups; ++grp)
+        bar += se_group<PRECISE, ND>(P, pV, pP1, pP2, BRMPPI_SMEM(SeRecord, P.off_se) + grp * kSeGroup, xy.x, xy.y, t0, t1, one_minus_alpha);
       if (t1 == T) {   // terminal cost r_N(x_N), eq. (7); final state out
         const float2 xT = BRMPPI_SMEM(float2, P.off_xy)[P.chunks * S + s];
         const State X{xT.x, xT.y, pP1[T], pP2[T]};

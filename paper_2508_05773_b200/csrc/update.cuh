@@ -118,6 +118,12 @@ __global__ void __launch_bounds__(kShiftBlock) shift_plant(const __grid_constant
       ob[0] = fmaf(P.dt, ob[3], ob[0]);
       ob[1] = fmaf(P.dt, ob[4], ob[1]);
     }
+    const int n_se = P.max_superellipses > 0 ? P.n_se[scene] : 0;
+    for (int i = tid; i < n_se; i += kShiftBlock) {
+      float* q = P.se + ((size_t)scene * P.max_superellipses + i) * 8;
+      q[0] = fmaf(P.dt, q[5], q[0]);
+      q[1] = fmaf(P.dt, q[6], q[1]);
+    }
   }
   float2 next[kShiftMaxPerThread];
 #pragma unroll

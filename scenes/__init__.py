@@ -3,8 +3,8 @@ and to the CUDA library.  This module holds DATA RECIPES ONLY -- none of the met
 (no kinematics, no barrier, no costs, no random-number mapping used by the solver).  It imports
 neither `oracle/` nor `paper_2508_05773_b200/`."""
 from .params import Params, default_params
-from .parking import (Scene, scene_cfg0, scene_cfg1, scene_cfg2, scene_cfg3, scene_static,
+from .parking import (Scene, scene_cfg0, scene_cfg1, scene_cfg2, scene_cfg2_superellipse, scene_cfg3, scene_static,
                       scene_batch, vehicle_disc_centres)
 
 __all__ = ["Params", "default_params", "Scene", "scene_cfg0", "scene_cfg1", "scene_cfg2",
-           "scene_cfg3", "scene_static", "scene_batch", "vehicle_disc_centres"]
+           "scene_cfg2_superellipse", "scene_cfg3", "scene_static", "scene_batch", "vehicle_disc_centres"]

@@ -26,6 +26,7 @@ class Scene:
     params: Params
     name: str = ""
     goal_next: np.ndarray = None   # second waypoint of a forward-then-reverse schedule (CFG2)
+    superellipses: np.ndarray = None   # (M, 8): cx, cy, m_x, m_y, theta, vx, vy, exponent (eq. 16)
 
 
 def _r32(a):
@@ -109,6 +110,24 @@ def scene_cfg2(seed: int = 0) -> Scene:
     fwd[0] += 6.0 * np.cos(bay[2])
     fwd[1] += 6.0 * np.sin(bay[2])
     return Scene(s.x0, _r32(fwd), obs, s.params, f"cfg2/seed{seed}", goal_next=bay)
+
+
+def scene_cfg2_superellipse(seed: int = 0) -> Scene:
+    """CFG2 with the paper's obstacle models: the five static obstacles
+    become parked cars -- super-ellipses with e = 4, semi-axes 2.25 x 0.9 m (a 4.5 x 1.8 m car),
+    orientation U[-pi, pi), centre where CFG2's generator would put a disc of the car's
+    circumscribed radius -- and the three pedestrians super-ellipses with e = 2, m_x = m_y = 0.4 m,
+    same constant velocities as in CFG2."""
+    s = scene_cfg2(seed)
+    rng = np.random.default_rng(3000 + seed)
+    half_len, half_wid = 2.25, 0.9
+    rad = float(np.hypot(half_len, half_wid))
+    cars = _draw_obstacles(rng, 5, 20.0, rad, rad, [s.x0[:3], s.goal_next[:3], s.goal[:3]], s.params.disc_radius + 1.0)
+    se = [[c[0], c[1], half_len, half_wid, rng.uniform(-np.pi, np.pi), 0.0, 0.0, 4.0] for c in cars]
+    for o in s.obstacles[5:]:
+        se.append([o[0], o[1], o[2], o[2], 0.0, o[3], o[4], 2.0])
+    return Scene(s.x0, s.goal, np.zeros((0, 5)), s.params, f"cfg2se/seed{seed}", goal_next=s.goal_next,
+                 superellipses=_r32(se))
 
 
 def scene_cfg3(seed: int = 0) -> Scene:

@@ -405,3 +405,94 @@ def test_culling_keeps_close_fast_obstacles(B, O):
     b = gpu_solve(B, sc2, p, B.FLAG_NO_CULL)
     assert np.array_equal(a["S"], b["S"]) and np.array_equal(a["U"], b["U"])
     check_against_oracle(O, a, sc2, p)
+
+
+# ------------------------------------------------------------------------------------------
+# super-ellipse obstacles, eq. (16)
+# ------------------------------------------------------------------------------------------
+def gpu_solve_se(B, sc, p, se, flags=0, n0=0, U0=None, max_se=None):
+    n_obs = len(sc.obstacles)
+    s = B.Solver(p, 1, max(n_obs, 1), flags | B.FLAG_WRITE_SAMPLES, max_superellipses=max_se or max(len(se), 1))
+    s.set_state(sc.x0); s.set_goal(sc.goal); s.set_obstacles(sc.obstacles); s.set_superellipses(se)
+    s.set_nominal(U0)
+    s.set_counter(n0)
+    s.solve()
+    out = dict(U=s.get_controls(), S=s.get_costs(), XT=s.get_final_states(), diag=s.get_diag())
+    s.close()
+    return out
+
+
+def check_se(O, got, sc, p, se, n0=0, U0=None):
+    U = np.zeros((p.T, 2)) if U0 is None else np.asarray(U0, dtype=np.float64)
+    ref = O.solve(p, n0, sc.x0, sc.goal, sc.obstacles, U, n_threads=8, superellipses=se)[-1]
+    okS = close(got["S"], ref["S"], 1.0)
+    assert okS.all(), f"S_k: {np.count_nonzero(~okS)} of {p.K} off, worst {np.abs(got['S'] - ref['S']).max()}"
+    assert close(got["XT"], ref["XT"], 1.0).all()
+    floors = np.array([p.v_max, p.delta_max])
+    err = np.abs(got["U"] - ref["U"]) / (RTOL * np.maximum(np.abs(ref["U"]), floors[None, :]))
+    assert err.max() <= 1.0, f"U worst error = {err.max():.2f} x tolerance"
+    if ref["gap"] > 1e-3 * max(1.0, abs(ref["S"].min())):
+        assert got["diag"]["argmin"] == ref["argmin"]
+
+
+@pytest.mark.parametrize("seed", [0, 1, 2])
+@pytest.mark.parametrize("precise", [0, 2], ids=["fast", "precise"])
+def test_superellipse_scene(B, O, seed, precise):
+    sc = scenes.scene_cfg2_superellipse(seed)
+    p = sc.params.with_(K=4096, n_iter=2)
+    got = gpu_solve_se(B, sc, p, sc.superellipses, precise)
+    check_se(O, got, sc, p, sc.superellipses)
+
+
+@pytest.mark.parametrize("n_se", [1, 3, 4, 5, 16])
+def test_superellipse_counts_and_discs_together(B, O, n_se):
+    sc = scenes.scene_cfg2(3)                                   # 8 discs (3 moving) stay
+    rng = np.random.default_rng(n_se)
+    se = np.array([[sc.x0[0] + rng.uniform(-15, 15), sc.x0[1] + rng.uniform(-15, 15), rng.uniform(0.5, 2.5),
+                    rng.uniform(0.4, 1.2), rng.uniform(-3, 3), rng.uniform(-1, 1), rng.uniform(-1, 1),
+                    4.0 if i % 3 else 2.0] for i in range(n_se)], dtype=np.float32).astype(np.float64)
+    p = sc.params.with_(K=1000, T=61, n_iter=1)
+    got = gpu_solve_se(B, sc, p, se, max_se=16)
+    check_se(O, got, sc, p, se)
+
+
+def test_superellipse_e2_matches_disc_path(B):
+    sc = scenes.scene_cfg2(2)
+    p = sc.params.with_(K=2048, n_iter=1)
+    a = gpu_solve(B, sc, p, 0)
+    se = np.array([[o[0], o[1], o[2], o[2], 0.3 * i, o[3], o[4], 2.0] for i, o in enumerate(sc.obstacles)])
+    sc2 = scenes.Scene(sc.x0, sc.goal, np.zeros((0, 5)), p)
+    b = gpu_solve_se(B, sc2, p, se)
+    assert np.allclose(a["S"], b["S"], rtol=1e-5, atol=1e-3)
+    assert np.allclose(a["U"], b["U"], atol=1e-4) and a["diag"]["argmin"] == b["diag"]["argmin"]
+
+
+def test_superellipse_closed_loop_and_errors(B, O):
+    sc = scenes.scene_cfg2_superellipse(4)
+    p = sc.params.with_(K=2048, T=60, n_iter=1)
+    s = B.Solver(p, 1, 1, 0, max_superellipses=8)
+    s.set_scene(sc)
+    x, se, U = sc.x0.copy(), sc.superellipses.copy(), np.zeros((p.T, 2))
+    floors = np.array([p.v_max, p.delta_max])
+    for step in range(4):
+        u0 = s.step()[0]
+        ref = O.iteration(p, step, x, sc.goal, np.zeros((0, 5)), U, n_threads=8, superellipses=se)
+        assert close(u0, ref["U"][0], floors).all()
+        se_ref = O.advance_se(p, se)
+        se_gpu = s.get_superellipses()
+        assert np.abs(se_gpu - se_ref).max() <= 1e-5
+        x, se, U = s.get_state().astype(np.float64), se_gpu.astype(np.float64), s.get_controls().astype(np.float64)
+    with pytest.raises(B.BrmppiError) as e:
+        s.set_superellipses(np.tile(sc.superellipses[0], (9, 1)))
+    assert e.value.status == B.ERR_TOO_MANY_OBSTACLES
+    bad = sc.superellipses[:1].copy(); bad[0, 7] = 3
+    with pytest.raises(B.BrmppiError) as e:
+        s.set_superellipses(bad)
+    assert e.value.status == B.ERR_INVALID_ARG
+    bad = sc.superellipses[:1].copy(); bad[0, 2] = 0.0
+    with pytest.raises(B.BrmppiError) as e:
+        s.set_superellipses(bad)
+    assert e.value.status == B.ERR_INVALID_ARG
+    s.close()
+    with pytest.raises(B.BrmppiError):                          # default kernel only
+        B.Solver(p, 1, 1, B.FLAG_KERNEL_THREAD_PER_SAMPLE, max_superellipses=4)
