@@ -159,12 +159,12 @@ __device__ __forceinline__ GroupCost barrier_group(const DeviceParams& P, const 
 struct SeRecord { float ox, oy, a11, a12, a21, a22, wx, wy, e4, half_w, pad0, pad1; };
 static_assert(sizeof(SeRecord) == 48, "SeRecord layout");
 
-template <bool PRECISE, int ND>
-__device__ __forceinline__ double se_group(const DeviceParams& P, const float* __restrict__ pV,
-                                           const float* __restrict__ pP1, const float* __restrict__ pP2,
-                                           const SeRecord* __restrict__ rec, float x, float y, int t0, int t1,
-                                           float one_minus_alpha) {
-  double bar = 0.0;
+template <bool PRECISE, int ND, bool TRACK>
+__device__ __forceinline__ GroupCost se_group(const DeviceParams& P, const float* __restrict__ pV,
+                                              const float* __restrict__ pP1, const float* __restrict__ pP2,
+                                              const SeRecord* __restrict__ rec, float x, float y, int t0, int t1,
+                                              float one_minus_alpha, const float4 g) {
+  double bar = 0.0, track = 0.0;
   float hprev[kSeGroup][ND];
   float s1, c1;
   {
@@ -192,11 +192,17 @@ __device__ __forceinline__ double se_group(const DeviceParams& P, const float* _
     const float a = P.dt * pV[t];
     x = fmaf(a, c1, x);
     y = fmaf(a, s1, y);
+    const float psi1 = pP1[t + 1], psi2 = pP2[t + 1];
     float s2, c2;
-    sincos_t<PRECISE>(pP1[t + 1], &s1, &c1);
-    sincos_t<PRECISE>(pP2[t + 1], &s2, &c2);
+    sincos_t<PRECISE>(psi1, &s1, &c1);
+    sincos_t<PRECISE>(psi2, &s2, &c2);
     float cx[ND], cy[ND];
     disc_centres_n<ND>(P, x, y, s1, c1, s2, c2, cx, cy);
+    if (TRACK) {   // scenes without disc obstacles: the first super-ellipse group carries the stage cost
+      const State X{x, y, psi1, psi2};
+      if (PRECISE) track += (double)(goal_cost(P, X, g) + hitch_cost(P, X));
+      else track += (double)tracking_cost_fma(P, X, g);
+    }
     tf += 1.0f;
     float pen = 0.0f;
 #pragma unroll
@@ -218,7 +224,7 @@ __device__ __forceinline__ double se_group(const DeviceParams& P, const float* _
     }
     bar += (double)pen;
   }
-  return bar;
+  return GroupCost{track, bar};
 }
 
 // Dispatch on the number of moving obstacles in the group (block-uniform).
@@ -471,26 +477,36 @@ rollout_cta(const __grid_constant__ DeviceParams P) {
       const int n_moving = sM->n_moving, n_groups = sM->n_groups;
       const float2 xy = BRMPPI_SMEM(float2, P.off_xy)[c * S + s];
       double track = 0.0, bar = 0.0;
-      if (n_groups == 1 || P.chunk_len < kMinCullChunk) {
-        // a single group of obstacles, or short chunks: the culling test (a square root per
-        // obstacle and disc at every chunk start, a uniform branch per obstacle and step) costs
-        // more than it saves
-        GroupCost gc = barrier_group_nm<PRECISE, ND, true, false>(n_moving, P, pV, pP1, pP2, sObs, sVel, sSpd, xy.x, xy.y, t0, t1, one_minus_alpha, g);
+      const int n_se_groups = sM->n_se_groups;
+      const SeRecord* sSE = BRMPPI_SMEM(SeRecord, P.off_se);
+      if (sM->n_obs == 0 && n_se_groups > 0) {
+        // no disc obstacles: the first super-ellipse group carries the stage cost
+        const GroupCost gc = se_group<PRECISE, ND, true>(P, pV, pP1, pP2, sSE, xy.x, xy.y, t0, t1, one_minus_alpha, g);
         track = gc.track; bar = gc.bar;
-        for (int grp = 1; grp < n_groups; ++grp) {
-          const int ib = grp * kObsGroup;
-          bar += barrier_group_nm<PRECISE, ND, false, false>(n_moving - ib, P, pV, pP1, pP2, sObs + ib, sVel + ib, sSpd + ib, xy.x, xy.y, t0, t1, one_minus_alpha, g).bar;
-        }
+        for (int grp = 1; grp < n_se_groups; ++grp)
+          bar += se_group<PRECISE, ND, false>(P, pV, pP1, pP2, sSE + grp * kSeGroup, xy.x, xy.y, t0, t1, one_minus_alpha, g).bar;
       } else {
-        const GroupCost gc = barrier_group_nm<PRECISE, ND, true, true>(n_moving, P, pV, pP1, pP2, sObs, sVel, sSpd, xy.x, xy.y, t0, t1, one_minus_alpha, g);
-        track = gc.track; bar = gc.bar;
-        for (int grp = 1; grp < n_groups; ++grp) {
-          const int ib = grp * kObsGroup;
-          bar += barrier_group_nm<PRECISE, ND, false, true>(n_moving - ib, P, pV, pP1, pP2, sObs + ib, sVel + ib, sSpd + ib, xy.x, xy.y, t0, t1, one_minus_alpha, g).bar;
+        if (n_groups == 1 || P.chunk_len < kMinCullChunk) {
+          // a single group of obstacles, or short chunks: the culling test (a square root per
+          // obstacle and disc at every chunk start, a uniform branch per obstacle and step) costs
+          // more than it saves
+          GroupCost gc = barrier_group_nm<PRECISE, ND, true, false>(n_moving, P, pV, pP1, pP2, sObs, sVel, sSpd, xy.x, xy.y, t0, t1, one_minus_alpha, g);
+          track = gc.track; bar = gc.bar;
+          for (int grp = 1; grp < n_groups; ++grp) {
+            const int ib = grp * kObsGroup;
+            bar += barrier_group_nm<PRECISE, ND, false, false>(n_moving - ib, P, pV, pP1, pP2, sObs + ib, sVel + ib, sSpd + ib, xy.x, xy.y, t0, t1, one_minus_alpha, g).bar;
+          }
+        } else {
+          const GroupCost gc = barrier_group_nm<PRECISE, ND, true, true>(n_moving, P, pV, pP1, pP2, sObs, sVel, sSpd, xy.x, xy.y, t0, t1, one_minus_alpha, g);
+          track = gc.track; bar = gc.bar;
+          for (int grp = 1; grp < n_groups; ++grp) {
+            const int ib = grp * kObsGroup;
+            bar += barrier_group_nm<PRECISE, ND, false, true>(n_moving - ib, P, pV, pP1, pP2, sObs + ib, sVel + ib, sSpd + ib, xy.x, xy.y, t0, t1, one_minus_alpha, g).bar;
+          }
         }
+        for (int grp = 0; grp < n_se_groups; ++grp)
+          bar += se_group<PRECISE, ND, false>(P, pV, pP1, pP2, sSE + grp * kSeGroup, xy.x, xy.y, t0, t1, one_minus_alpha, g).bar;
       }
-      for (int grp = 0; grp < sM->n_se_groups; ++grp)
-        bar += se_group<PRECISE, ND>(P, pV, pP1, pP2, BRMPPI_SMEM(SeRecord, P.off_se) + grp * kSeGroup, xy.x, xy.y, t0, t1, one_minus_alpha);
       if (t1 == T) {   // terminal cost r_N(x_N), eq. (7); final state out
         const float2 xT = BRMPPI_SMEM(float2, P.off_xy)[P.chunks * S + s];
         const State X{xT.x, xT.y, pP1[T], pP2[T]};
