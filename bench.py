@@ -133,7 +133,8 @@ def oracle_throughput(sc, p, seconds_target, n_threads, k_sample):
     t0 = time.perf_counter()
     reps = 0
     while True:
-        O.solve(ps, reps * p.n_iter, sc.x0, sc.goal, sc.obstacles, U, n_threads=n_threads)
+        O.solve(ps, reps * p.n_iter, sc.x0, sc.goal, sc.obstacles, U, n_threads=n_threads,
+                superellipses=sc.superellipses)
         reps += 1
         dt = time.perf_counter() - t0
         if dt >= seconds_target or reps >= 50:
@@ -181,10 +182,10 @@ def run_reference(args):
     ps = p.with_(K=k_sample)
     U = np.zeros((p.T, 2))
     for w in range(args.warmup):
-        O.solve(ps, w, sc.x0, sc.goal, sc.obstacles, U, n_threads=cores)
+        O.solve(ps, w, sc.x0, sc.goal, sc.obstacles, U, n_threads=cores, superellipses=sc.superellipses)
     t0 = time.perf_counter()
     for s in range(args.steps):
-        O.solve(ps, s, sc.x0, sc.goal, sc.obstacles, U, n_threads=cores)
+        O.solve(ps, s, sc.x0, sc.goal, sc.obstacles, U, n_threads=cores, superellipses=sc.superellipses)
     dt = time.perf_counter() - t0
     value = args.steps * k_sample * p.T * p.n_iter / dt
     sample = f"each step = {k_sample} of {p.K} samples x T={p.T} x {p.n_iter} iterations, {cores} threads"
