@@ -279,12 +279,20 @@ __device__ __forceinline__ float hitch_cost(const DeviceParams& P, const State& 
 
 // Lexicographic (value, index) minimum over a warp; non-finite values never win.
 __device__ __forceinline__ void warp_argmin(double& m, int& idx) {
-#pragma unroll
-  for (int o = 16; o > 0; o >>= 1) {
-    const double om = __shfl_xor_sync(0xffffffffu, m, o);
-    const int oi = __shfl_xor_sync(0xffffffffu, idx, o);
-    if (om < m || (om == m && oi < idx)) { m = om; idx = oi; }
-  }
+  // Three warp-wide integer minima (REDUX) instead of five shuffle rounds on a (double, int)
+  // pair: the double becomes an order-preserving 64-bit key (NaN never occurs here: non-finite
+  // costs were replaced by +inf), compared high word first, then low word, then the index.
+  const unsigned long long b = (unsigned long long)__double_as_longlong(m);
+  const unsigned long long key = (b >> 63) ? ~b : (b | 0x8000000000000000ull);
+  const unsigned hi = (unsigned)(key >> 32), lo = (unsigned)key;
+  const unsigned min_hi = __reduce_min_sync(0xffffffffu, hi);
+  const unsigned min_lo = __reduce_min_sync(0xffffffffu, hi == min_hi ? lo : 0xffffffffu);
+  const bool is_min = (hi == min_hi) && (lo == min_lo);
+  const unsigned min_idx = __reduce_min_sync(0xffffffffu, is_min ? (unsigned)idx : 0xffffffffu);
+  const unsigned long long mk = ((unsigned long long)min_hi << 32) | min_lo;
+  const unsigned long long mb = (mk >> 63) ? (mk & 0x7fffffffffffffffull) : ~mk;
+  m = __longlong_as_double((long long)mb);
+  idx = (int)min_idx;
 }
 
 __device__ __forceinline__ float warp_sum(float v) {
