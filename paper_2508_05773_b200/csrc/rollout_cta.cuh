@@ -10,19 +10,20 @@
 // 512 threads takes a tile of S samples (S = ceil(K / #SMs) when that fits in shared memory: 111
 // at K = 16384, i.e. the whole problem is ONE balanced wave) and runs, per tile:
 //
-//   A  noise      thread (s, r) draws the controls of steps r, r + R, ... of sample s
-//                 (R = 512 / S rows): Philox -> Box-Muller -> perturb + clamp (a1, a2); stores v,
+//   A  noise      the (sample, step-pair) items are dealt round-robin over all 512 threads: one
+//                 Philox block per pair of steps -> Box-Muller -> perturb + clamp (a1, a2); stores v,
 //                 delta and the heading increment dpsi1 = dt v tan(delta) / L1 to shared-memory
-//                 planes; effort cost.
+//                 planes.
 //   B  chain      the S threads of warps 0..3 (one warp per scheduler) run the serial Euler
-//                 recursion of eq. (6) (a3), one sample each, and nothing else: a single in-order
-//                 instruction stream per step is the critical path of the whole tile.  psi1, psi2
-//                 of every step go to shared planes, (x, y) only at the chunk boundaries.
+//                 recursion of eq. (6) (a3), one sample each, and little else (the effort cost
+//                 rides along): a single in-order instruction stream per step is the critical
+//                 path of the whole tile.  psi1, psi2 of every step go to shared planes, (x, y)
+//                 only at the chunk boundaries.  Warp 4 sorts the obstacle tables meanwhile.
 //   C  cost       thread (s, c) walks steps [cL, cL+L) of sample s: re-integrates (x, y) from its
 //                 chunk boundary (two FMAs, bit-identical to the chain), disc centres, barrier h
 //                 for every (obstacle, disc) with h_t in registers, barrier-rate hinge (a4, a5),
 //                 goal / heading / hitch cost (a6).  Obstacles go in groups of 8 (padded with null
-//                 obstacles whose h is identically 0) held in registers.
+//                 obstacles of weight 0) held in registers; super-ellipses in groups of 4.
 //   D  reduce     S threads add effort + chunk partials in a fixed order (fp64), block argmin,
 //                 weights against the CTA's running minimum (online softmax, a7).
 //   E  update     threads (channel, t) rescale the running A[t] and add sum_s w_s u_s[t] from the
@@ -50,7 +51,6 @@ constexpr int kSeGroup = 4;                         // super-ellipses whose h_t 
 constexpr int kMaxChunks = 16;
 constexpr int kMinChunkLen = 4;
 constexpr int kMinCullChunk = 8;                    // culling pays from this chunk length on
-constexpr int kMaxNoiseBlocks = 8;                  // named barriers 1..8 hand noise blocks to the chain
 constexpr int kPhaseSlots = 7;                      // prologue, A, B, C, D, E, partial out
 constexpr size_t kSmemMax = 232448;                 // 227 KB opt-in dynamic shared memory per CTA
 

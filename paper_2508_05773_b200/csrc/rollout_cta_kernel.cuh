@@ -305,7 +305,7 @@ rollout_cta(const __grid_constant__ DeviceParams P) {
     }
 
     BRMPPI_STAMP(0)
-    // ---- phase A: noise, perturb + clamp, effort cost (a1, a2) -------------------------------
+    // ---- phase A: noise, perturb + clamp (a1, a2) ---------------------------------------------
     {
       const int TS = P.t_stride, T = P.T;
       const int R = kCtaThreads / S;
