@@ -100,6 +100,8 @@ typedef struct {
   unsigned long long seed;
   unsigned int flags;
   int max_superellipses;  /* capacity per scene, 0..BRMPPI_MAX_SUPERELLIPSES                     */
+  float hitch_kappa;      /* >= 0: the hitch-angle hinge starts at hitch_max - hitch_kappa |v|
+                             (eq. (18)); 0 = fixed limit                        */
 } brmppi_params;
 
 #define BRMPPI_MAX_T 512

@@ -196,8 +196,9 @@ double orc_rollout_se(const orc_params* p, const double x0[4], const double goal
     }
     pen_total += pen;
 
-    /* stage cost on (x_{t+1}, u_t) (reading 3); hitch: squared hinge at hitch_max (reading 15) */
-    double hitch = fabs(orc_wrap(Xn[2] - Xn[3])) - p->hitch_max;
+    /* stage cost on (x_{t+1}, u_t) (reading 3); hitch: squared hinge beyond the velocity-dependent
+     * limit Delta_theta_max - kappa |v| of eq. (18) (reading 15, kappa = 0 in CFG0-4) */
+    double hitch = fabs(orc_wrap(Xn[2] - Xn[3])) - (p->hitch_max - p->hitch_kappa * fabs(v));
     if (hitch < 0.0) hitch = 0.0;
     S += orc_goal_cost(p, Xn, goal) + p->w_v * v * v + p->w_delta * d * d +
          p->w_hitch * hitch * hitch + p->w_bar * pen;

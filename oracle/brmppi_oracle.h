@@ -56,6 +56,7 @@ typedef struct {
   double sigma_v, sigma_delta;
   double alpha_lo, alpha_hi;
   double w_pos, w_head, w_v, w_delta, w_hitch, hitch_max, w_bar, w_term, lambda;
+  double hitch_kappa;     /* hitch limit = hitch_max - hitch_kappa |v| (eq. (18)) */
   uint64_t seed;          /* Philox key = (lo32(seed), hi32(seed))                     */
 } orc_params;
 

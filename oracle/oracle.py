@@ -36,7 +36,7 @@ class _Params(C.Structure):
                 ("alpha_lo", C.c_double), ("alpha_hi", C.c_double),
                 ("w_pos", C.c_double), ("w_head", C.c_double), ("w_v", C.c_double),
                 ("w_delta", C.c_double), ("w_hitch", C.c_double), ("hitch_max", C.c_double),
-                ("w_bar", C.c_double), ("w_term", C.c_double), ("lam", C.c_double),
+                ("w_bar", C.c_double), ("w_term", C.c_double), ("lam", C.c_double), ("hitch_kappa", C.c_double),
                 ("seed", C.c_uint64)]
 
 
@@ -109,7 +109,7 @@ def _cparams(p) -> _Params:
         s.disc_offset[j] = float(off)
     for name in ("disc_radius", "dt", "L1", "L2", "Lh", "v_min", "v_max", "delta_min",
                  "delta_max", "sigma_v", "sigma_delta", "alpha_lo", "alpha_hi", "w_pos", "w_head",
-                 "w_v", "w_delta", "w_hitch", "hitch_max", "w_bar", "w_term", "lam"):
+                 "w_v", "w_delta", "w_hitch", "hitch_max", "w_bar", "w_term", "lam", "hitch_kappa"):
         setattr(s, name, float(getattr(p, name)))
     s.seed = int(p.seed) & 0xFFFFFFFFFFFFFFFF
     return s

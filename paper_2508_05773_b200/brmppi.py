@@ -57,7 +57,8 @@ class CParams(C.Structure):
                 ("w_pos", C.c_float), ("w_head", C.c_float), ("w_v", C.c_float),
                 ("w_delta", C.c_float), ("w_hitch", C.c_float), ("hitch_max", C.c_float),
                 ("w_bar", C.c_float), ("w_term", C.c_float), ("lam", C.c_float),
-                ("seed", C.c_ulonglong), ("flags", C.c_uint), ("max_superellipses", C.c_int)]
+                ("seed", C.c_ulonglong), ("flags", C.c_uint), ("max_superellipses", C.c_int),
+                ("hitch_kappa", C.c_float)]
 
 
 class Diag(C.Structure):
@@ -139,6 +140,7 @@ def make_cparams(p, n_scenes=1, max_obstacles=8, flags=0, max_superellipses=0) -
         setattr(c, name, float(getattr(p, name)))
     c.seed, c.flags = int(p.seed) & 0xFFFFFFFFFFFFFFFF, int(flags)
     c.max_superellipses = int(max_superellipses)
+    c.hitch_kappa = float(getattr(p, "hitch_kappa", 0.0))
     return c
 
 

@@ -64,6 +64,7 @@ bool params_valid(const brmppi_params* p) {
   if (!finite_all(f, (int)(sizeof(f) / sizeof(f[0])))) return false;
   if (!(p->dt > 0.f) || !(p->L1 > 0.f) || !(p->L2 > 0.f) || !(p->lambda > 0.f)) return false;
   if (p->disc_radius < 0.f || p->sigma_v < 0.f || p->sigma_delta < 0.f) return false;
+  if (!std::isfinite(p->hitch_kappa) || p->hitch_kappa < 0.f) return false;
   if (p->v_min > p->v_max || p->delta_min > p->delta_max) return false;
   if (p->delta_min <= -1.5f || p->delta_max >= 1.5f) return false;   // tan(delta) must stay finite
   if (p->alpha_lo > p->alpha_hi) return false;
@@ -283,7 +284,7 @@ int brmppi_create(const brmppi_params* p, void* dev_workspace, size_t workspace_
   d.sigma_v = p->sigma_v; d.sigma_delta = p->sigma_delta;
   d.alpha_lo = p->alpha_lo; d.alpha_span = p->alpha_hi - p->alpha_lo;
   d.w_pos = p->w_pos; d.w_head = p->w_head; d.w_v = p->w_v; d.w_delta = p->w_delta;
-  d.w_hitch = p->w_hitch; d.hitch_max = p->hitch_max; d.w_bar = p->w_bar; d.w_term = p->w_term;
+  d.w_hitch = p->w_hitch; d.hitch_max = p->hitch_max; d.hitch_kappa = p->hitch_kappa; d.w_bar = p->w_bar; d.w_term = p->w_term;
   d.inv_lambda = 1.0f / p->lambda;
   d.key0 = (uint32_t)(p->seed & 0xFFFFFFFFull); d.key1 = (uint32_t)(p->seed >> 32);
   d.flags = p->flags;

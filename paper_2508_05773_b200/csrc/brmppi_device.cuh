@@ -28,7 +28,7 @@ struct DeviceParams {
   float dt, inv_L1, inv_L2, Lh, Lh_over_L1, Lh_over_L2;
   float v_min, v_max, delta_min, delta_max, sigma_v, sigma_delta;
   float alpha_lo, alpha_span;
-  float w_pos, w_head, w_v, w_delta, w_hitch, hitch_max, w_bar, w_term;
+  float w_pos, w_head, w_v, w_delta, w_hitch, hitch_max, hitch_kappa, w_bar, w_term;
   float inv_lambda;
   uint32_t key0, key1;        // Philox key of scene 0 = (lo32(seed), hi32(seed)); scene s adds s
   uint32_t flags;
@@ -263,17 +263,17 @@ __device__ __forceinline__ float goal_cost(const DeviceParams& P, const State& X
 }
 
 // Goal + hitch stage cost with the FMA-pipe wrap (persistent-CTA kernel, fast-math mode).
-__device__ __forceinline__ float tracking_cost_fma(const DeviceParams& P, const State& X, const float4 g) {
+__device__ __forceinline__ float tracking_cost_fma(const DeviceParams& P, const State& X, const float4 g, float v) {
   const float ex = X.x - g.x, ey = X.y - g.y;
   const float e1 = wrap_angle_fma(X.psi1 - g.z), e2 = wrap_angle_fma(X.psi2 - g.w);
   const float G = fmaf(P.w_pos, fmaf(ex, ex, ey * ey), P.w_head * fmaf(e1, e1, e2 * e2));
-  const float e = fmaxf(fabsf(wrap_angle_fma(X.psi1 - X.psi2)) - P.hitch_max, 0.0f);
+  const float e = fmaxf(fabsf(wrap_angle_fma(X.psi1 - X.psi2)) - fmaf(-P.hitch_kappa, fabsf(v), P.hitch_max), 0.0f);
   return fmaf(P.w_hitch * e, e, G);
 }
 
 // Hitch-angle squared hinge (reading 15).
-__device__ __forceinline__ float hitch_cost(const DeviceParams& P, const State& X) {
-  const float e = fmaxf(fabsf(wrap_angle(X.psi1 - X.psi2)) - P.hitch_max, 0.0f);
+__device__ __forceinline__ float hitch_cost(const DeviceParams& P, const State& X, float v) {
+  const float e = fmaxf(fabsf(wrap_angle(X.psi1 - X.psi2)) - fmaf(-P.hitch_kappa, fabsf(v), P.hitch_max), 0.0f);
   return P.w_hitch * e * e;
 }
 

@@ -113,7 +113,8 @@ __device__ __forceinline__ GroupCost barrier_group(const DeviceParams& P, const 
 #pragma unroll kCostUnroll
   for (int t = t0; t < t1; ++t) {
     // (x, y) of state t+1 from state t: the chain's own FMAs on the same operands
-    const float a = P.dt * pV[t];
+    const float v_t = pV[t];
+    const float a = P.dt * v_t;
     x = fmaf(a, c1, x);
     y = fmaf(a, s1, y);
     const float psi1 = pP1[t + 1], psi2 = pP2[t + 1];
@@ -124,8 +125,8 @@ __device__ __forceinline__ GroupCost barrier_group(const DeviceParams& P, const 
     disc_centres_n<ND>(P, x, y, s1, c1, s2, c2, cx, cy);
     if (TRACK) {
       const State X{x, y, psi1, psi2};
-      if (PRECISE) track += (double)(goal_cost(P, X, g) + hitch_cost(P, X));
-      else track += (double)tracking_cost_fma(P, X, g);
+      if (PRECISE) track += (double)(goal_cost(P, X, g) + hitch_cost(P, X, v_t));
+      else track += (double)tracking_cost_fma(P, X, g, v_t);
     }
     const float tf = (float)(t + 1);
     float pen = 0.0f;
@@ -189,7 +190,8 @@ __device__ __forceinline__ GroupCost se_group(const DeviceParams& P, const float
   }
   float tf = (float)t0;
   for (int t = t0; t < t1; ++t) {
-    const float a = P.dt * pV[t];
+    const float v_t = pV[t];
+    const float a = P.dt * v_t;
     x = fmaf(a, c1, x);
     y = fmaf(a, s1, y);
     const float psi1 = pP1[t + 1], psi2 = pP2[t + 1];
@@ -200,8 +202,8 @@ __device__ __forceinline__ GroupCost se_group(const DeviceParams& P, const float
     disc_centres_n<ND>(P, x, y, s1, c1, s2, c2, cx, cy);
     if (TRACK) {   // scenes without disc obstacles: the first super-ellipse group carries the stage cost
       const State X{x, y, psi1, psi2};
-      if (PRECISE) track += (double)(goal_cost(P, X, g) + hitch_cost(P, X));
-      else track += (double)tracking_cost_fma(P, X, g);
+      if (PRECISE) track += (double)(goal_cost(P, X, g) + hitch_cost(P, X, v_t));
+      else track += (double)tracking_cost_fma(P, X, g, v_t);
     }
     tf += 1.0f;
     float pen = 0.0f;

@@ -96,7 +96,7 @@ rollout_thread_per_sample(const __grid_constant__ DeviceParams P) {
         }
       }
       const float stage = goal_cost(P, Xn, g) + fmaf(P.w_v * u.x, u.x, P.w_delta * u.y * u.y) +
-                          hitch_cost(P, Xn);
+                          hitch_cost(P, Xn, u.x);
       track += (double)stage;
       bar += (double)pen;
       X = Xn;

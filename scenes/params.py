@@ -41,6 +41,7 @@ class Params:
     w_delta: float = 0.1
     w_hitch: float = 10.0
     hitch_max: float = 1.2
+    hitch_kappa: float = 0.0      # velocity-dependent hitch limit hitch_max - kappa |v| (eq. 18); 0 = fixed limit
     w_bar: float = 1.0e3
     w_term: float = 10.0
     lam: float = 1.0

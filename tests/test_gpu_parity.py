@@ -496,3 +496,16 @@ def test_superellipse_closed_loop_and_errors(B, O):
     s.close()
     with pytest.raises(B.BrmppiError):                          # default kernel only
         B.Solver(p, 1, 1, B.FLAG_KERNEL_THREAD_PER_SAMPLE, max_superellipses=4)
+
+
+@pytest.mark.parametrize("kernel", KERNELS)
+def test_velocity_dependent_hitch_limit(B, O, kernel):
+    """hitch_kappa > 0 (eq. 18): start jackknifed so that the hinge is active for most samples."""
+    sc = scenes.scene_cfg1(7)
+    x0 = sc.x0.copy(); x0[3] = x0[2] - 1.0                     # hitch angle 1.0 rad
+    sc2 = scenes.Scene(np.asarray(x0, dtype=np.float32).astype(np.float64), sc.goal, sc.obstacles, sc.params)
+    p = sc.params.with_(K=1024, hitch_kappa=0.2, hitch_max=1.1)
+    got = gpu_solve(B, sc2, p, kernel)
+    check_against_oracle(O, got, sc2, p)
+    base = gpu_solve(B, sc2, p.with_(hitch_kappa=0.0), kernel)
+    assert (got["S"] >= base["S"] - 1e-3).all() and (got["S"] > base["S"] + 1e-2).any()

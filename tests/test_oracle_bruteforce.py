@@ -91,7 +91,7 @@ def brute_force(p, n, x0, goal, obstacles, U, superellipses=()):
                   for t in range(T) for i in range(len(obstacles) + len(superellipses)) for j in range(D))
         track = sum(G(X[k][t + 1]) for t in range(T))
         effort = sum(mpf(p.w_v) * u[k][t][0] ** 2 + mpf(p.w_delta) * u[k][t][1] ** 2 for t in range(T))
-        hitch = sum(mpf(p.w_hitch) * max(mpf(0), abs(wrap(X[k][t + 1][2] - X[k][t + 1][3])) - mpf(p.hitch_max)) ** 2
+        hitch = sum(mpf(p.w_hitch) * max(mpf(0), abs(wrap(X[k][t + 1][2] - X[k][t + 1][3])) - (mpf(p.hitch_max) - mpf(p.hitch_kappa) * abs(u[k][t][0]))) ** 2
                     for t in range(T))
         S.append(track + effort + hitch + mpf(p.w_bar) * bar + mpf(p.w_term) * G(X[k][T]))
     # 5. normalised softmax weights and update
@@ -120,7 +120,7 @@ def test_oracle_matches_bruteforce(O, case):
         x0, U = sc.x0, np.array([[-1.5, 0.1]] * 5, dtype=np.float32).astype(float)
         se = np.array([[-9.0, 2.5, 2.25, 0.9, 0.6, 0.0, 0.0, 4.0], [-3.0, -2.0, 0.4, 0.4, 0.0, 0.3, 1.2, 2.0]], dtype=np.float32).astype(float)
     else:             # large hitch angle and headings near +-pi (wrap paths active)
-        p = sc.params.with_(K=5, T=3, seed=77, sigma_v=1.0, sigma_delta=0.5, dt=0.5)
+        p = sc.params.with_(K=5, T=3, seed=77, sigma_v=1.0, sigma_delta=0.5, dt=0.5, hitch_kappa=0.15)   # eq. (18) limit active
         obs = sc.obstacles
         x0 = np.array([1.0, 2.0, 3.0, -2.9], dtype=np.float32).astype(float)
         U = np.array([[-1.0, 0.5]] * 3, dtype=np.float32).astype(float)

@@ -462,3 +462,21 @@ def test_shift_and_plant(O):
     assert x[2] == pytest.approx(-math.pi + 0.24, abs=1e-12)
     assert x[0] == pytest.approx(0.5 * 2.0 * math.cos(math.pi - 0.01))
     np.testing.assert_allclose(ob[0], [1.125, 1.75, 0.5, 0.25, -0.5])
+
+
+def test_velocity_dependent_hitch_limit(O):
+    """Eq. (18): the hitch hinge starts at hitch_max - kappa |v|.  One step with
+    delta = 0 from a hitch angle of 1.0 rad: psi1 stays, psi2 moves by dt (v / L2) sin(beta)."""
+    p = P(T=1, dt=0.1, w_pos=0.0, w_head=0.0, w_v=0.0, w_delta=0.0, w_term=0.0, w_hitch=10.0, hitch_max=1.2)
+    x0 = [0.0, 0.0, 1.0, 0.0]
+    for v in (2.0, -2.0, 0.5):
+        beta1 = 1.0 - p.dt * (v / p.L2) * math.sin(1.0)              # hitch angle after the step (fp32-rounded dt)
+        for kappa in (0.0, 0.05, 0.2):
+            pk = p.with_(hitch_kappa=kappa)
+            r = O.rollout(pk, x0, [0, 0, 0, 0], np.zeros((0, 5)), [[v, 0.0]], 0.5)
+            lim = pk.hitch_max - pk.hitch_kappa * abs(v)              # parameters are fp32-rounded doubles
+            want = pk.w_hitch * max(0.0, abs(beta1) - lim) ** 2
+            assert r["S"] == pytest.approx(want, rel=1e-9, abs=1e-12), (v, kappa)
+    # kappa = 0.2, |v| = 2: limit 0.8 < 0.9...: active; kappa = 0: inactive
+    assert O.rollout(p.with_(hitch_kappa=0.2), x0, [0, 0, 0, 0], np.zeros((0, 5)), [[2.0, 0.0]], 0.5)["S"] > 0
+    assert O.rollout(p, x0, [0, 0, 0, 0], np.zeros((0, 5)), [[2.0, 0.0]], 0.5)["S"] == 0.0
