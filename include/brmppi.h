@@ -168,12 +168,13 @@ int brmppi_get_costs(brmppi_ctx* ctx, int scene, float* S_out /* K */);         
 int brmppi_get_final_states(brmppi_ctx* ctx, int scene, float* X_out /* K*4 */);    /* FLAG_WRITE_SAMPLES */
 int brmppi_get_diag(brmppi_ctx* ctx, int scene, brmppi_diag* out);
 
-/* Device time of the two kernels of one MPPI iteration, for the roofline report: enqueues
- * `reps` (+2 warm-up) iterations of every scene OUTSIDE the captured graph, back to back, with a
- * CUDA event between consecutive kernels on the context's stream, synchronises once and returns
- * the mean milliseconds per launch (kernel + kernel-to-kernel gap): out_ms[0] = rollout kernel,
- * out_ms[1] = merge/update kernel.  Advances the iteration counter by reps + 2 and updates U like
- * that many single-iteration solves.  1 <= reps <= 4096. */
+/* Device time of the two kernels of one MPPI iteration, for the roofline report.  OUTSIDE the
+ * captured graph, on the context's stream, enqueues back to back and synchronises once: `reps` (+2
+ * warm-up) rollout launches of every scene between two CUDA events, then `reps` (+2) update
+ * launches between two events.  Returns mean milliseconds per launch (kernel + kernel-to-kernel
+ * gap, as between graph nodes): out_ms[0] = rollout kernel, out_ms[1] = merge/update kernel.
+ * Leaves U as ONE iteration from the current state would, and advances the iteration counter by
+ * reps + 2.  1 <= reps <= 4096. */
 int brmppi_time_kernels(brmppi_ctx* ctx, int reps, float out_ms[2]);
 
 /* Per-phase device time of the LAST rollout launch, from the kernel's own globaltimer stamps

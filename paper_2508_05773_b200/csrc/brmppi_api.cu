@@ -584,39 +584,40 @@ int brmppi_time_kernels(brmppi_ctx* c, int reps, float out_ms[2]) {
   if (reps < 1 || reps > 4096) return BRMPPI_ERR_INVALID_ARG;
   int r = ready(c);
   if (r) return r;
-  // All launches are enqueued back to back with an event between consecutive kernels and ONE
-  // synchronisation at the end: the stream never runs dry, so an interval is the kernel's device
-  // time plus the kernel-to-kernel gap, not the host's launch latency.  kWarm leading iterations
-  // are enqueued the same way and left out of the mean.
-  const int kWarm = 2, n_it = reps + kWarm, n_ev = 2 * n_it + 1;
-  cudaEvent_t* ev = (cudaEvent_t*)calloc((size_t)n_ev, sizeof(cudaEvent_t));
-  if (!ev) return BRMPPI_ERR_NULL;
+  // Two trains of launches, everything enqueued back to back with ONE synchronisation at the end so
+  // that the stream never runs dry: `reps` rollout launches between two events, then `reps` update
+  // launches between two events (the update is a pure function of the partials, so repeating it
+  // leaves U as one iteration would).  A train's mean is the kernel's device time plus the
+  // kernel-to-kernel gap, as inside the captured graph; an event between every two kernels would
+  // add its own drain-and-timestamp gap (about 3 us here) to each interval.  kWarm leading
+  // launches of each train are left out.
+  const int kWarm = 2;
+  cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
   cudaError_t e = cudaSuccess;
   int made = 0;
-  for (; made < n_ev && e == cudaSuccess; ++made) e = cudaEventCreate(&ev[made]);
-  if (e == cudaSuccess) e = cudaEventRecord(ev[0], c->stream);
-  for (int it = 0; it < n_it && e == cudaSuccess && r == 0; ++it) {
-    r = launch_rollout(c);
-    if (r == 0) e = cudaEventRecord(ev[2 * it + 1], c->stream);
-    if (r == 0 && e == cudaSuccess) r = launch_update(c);
-    if (r == 0 && e == cudaSuccess) e = cudaEventRecord(ev[2 * it + 2], c->stream);
-    c->launches += 2;
+  for (; made < 4 && e == cudaSuccess; ++made) e = cudaEventCreate(&ev[made]);
+  for (int it = 0; it < reps + kWarm && e == cudaSuccess && r == 0; ++it) {
+    if (it == kWarm) e = cudaEventRecord(ev[0], c->stream);
+    if (e == cudaSuccess) r = launch_rollout(c);
+    c->launches += 1;
+  }
+  if (e == cudaSuccess && r == 0) e = cudaEventRecord(ev[1], c->stream);
+  for (int it = 0; it < reps + kWarm && e == cudaSuccess && r == 0; ++it) {
+    if (it == kWarm) e = cudaEventRecord(ev[2], c->stream);
+    if (e == cudaSuccess) r = launch_update(c);
+    c->launches += 1;
     c->n_host += 1;
   }
+  if (e == cudaSuccess && r == 0) e = cudaEventRecord(ev[3], c->stream);
   if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
-  double acc[2] = {0.0, 0.0};
-  for (int it = kWarm; it < n_it && e == cudaSuccess && r == 0; ++it) {
-    float a = 0.f, b = 0.f;
-    e = cudaEventElapsedTime(&a, ev[2 * it], ev[2 * it + 1]);
-    if (e == cudaSuccess) e = cudaEventElapsedTime(&b, ev[2 * it + 1], ev[2 * it + 2]);
-    acc[0] += a; acc[1] += b;
-  }
+  float roll = 0.f, upd = 0.f;
+  if (e == cudaSuccess && r == 0) e = cudaEventElapsedTime(&roll, ev[0], ev[1]);
+  if (e == cudaSuccess && r == 0) e = cudaEventElapsedTime(&upd, ev[2], ev[3]);
   for (int i = 0; i < made; ++i) cudaEventDestroy(ev[i]);
-  free(ev);
   if (r) return r;
   if (e != cudaSuccess) return cuda_fail(e);
-  out_ms[0] = (float)(acc[0] / reps);
-  out_ms[1] = (float)(acc[1] / reps);
+  out_ms[0] = roll / (float)reps;
+  out_ms[1] = upd / (float)reps;
   return BRMPPI_OK;
 }
 
