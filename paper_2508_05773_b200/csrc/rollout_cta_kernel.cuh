@@ -60,10 +60,29 @@ __device__ __forceinline__ GroupCost barrier_group(const DeviceParams& P, const 
                                                    float x, float y, int t0, int t1, float one_minus_alpha,
                                                    const float4 g) {
   double bar = 0.0, track = 0.0;
-  float gprev[kObsGroup][ND];
-  float4 o[kObsGroup];
+  // obstacles in pairs (2p, 2p+1): negated centres, -rho^2, -1/rho^2 and g of the previous state
+  constexpr int NP = kObsGroup / 2;
+  f32x2 nox[NP], noy[NP], mrho2[NP], nw[NP], gprev[NP][ND];
+  {
+    // the table is pair-interleaved (see the sorting warp), so a pair arrives as one 64-bit register
+    const ulonglong2* q = reinterpret_cast<const ulonglong2*>(obs);
 #pragma unroll
-  for (int i = 0; i < kObsGroup; ++i) o[i] = obs[i];
+    for (int p = 0; p < NP; ++p) {
+      const ulonglong2 a = q[2 * p], b = q[2 * p + 1];
+      nox[p] = a.x; noy[p] = a.y; nw[p] = b.x; mrho2[p] = b.y;
+    }
+  }
+  const f32x2 noma = pack2(-one_minus_alpha, -one_minus_alpha);
+  // centre of pair p at step tf: moving obstacles are o(0) + tf vel (a6), negated exactly
+  auto centres = [&](int p, float tf, f32x2& ex, f32x2& ey) {
+    ex = nox[p]; ey = noy[p];
+    if (2 * p < NM) {
+      const ulonglong2 w = reinterpret_cast<const ulonglong2*>(vel)[p];
+      const f32x2 tf2 = pack2(tf, tf);
+      ex = fma2(tf2, w.x, ex);
+      ey = fma2(tf2, w.y, ey);
+    }
+  };
   float s1, c1;
   {
     float s2, c2;
@@ -71,15 +90,15 @@ __device__ __forceinline__ GroupCost barrier_group(const DeviceParams& P, const 
     sincos_t<PRECISE>(pP2[t0], &s2, &c2);
     float cx[ND], cy[ND];
     disc_centres_n<ND>(P, x, y, s1, c1, s2, c2, cx, cy);
-    const float tf = (float)t0;
+    const float tfp = (float)t0;
 #pragma unroll
-    for (int i = 0; i < kObsGroup; ++i) {
-      float ox = o[i].x, oy = o[i].y;
-      if (i < NM) { const float2 w = vel[i]; ox = fmaf(tf, w.x, ox); oy = fmaf(tf, w.y, oy); }
+    for (int p = 0; p < NP; ++p) {
+      f32x2 ex, ey;
+      centres(p, tfp, ex, ey);
 #pragma unroll
       for (int j = 0; j < ND; ++j) {
-        const float dx = cx[j] - ox, dy = cy[j] - oy;
-        gprev[i][j] = fmaf(dx, dx, fmaf(dy, dy, o[i].w));
+        const f32x2 dx = add2(pack2(cx[j], cx[j]), ex), dy = add2(pack2(cy[j], cy[j]), ey);
+        gprev[p][j] = fma2(dx, dx, fma2(dy, dy, mrho2[p]));
       }
     }
   }
@@ -95,16 +114,21 @@ __device__ __forceinline__ GroupCost barrier_group(const DeviceParams& P, const 
     active = 0u;
 #pragma unroll
     for (int i = 0; i < kObsGroup; ++i) {
-      const float rho2 = -o[i].w;
+      float ra, rb, wa, wb;
+      unpack2(mrho2[i >> 1], ra, rb);
+      unpack2(nw[i >> 1], wa, wb);
+      const float rho2 = -((i & 1) ? rb : ra);
       bool act = false;
 #pragma unroll
       for (int j = 0; j < ND; ++j) {
+        float ga, gb;
+        unpack2(gprev[i >> 1][j], ga, gb);
         const float dl = fmaf(P.dt, P.disc_speed[j], spd[i]);   // relative displacement per step
-        const float d0 = sqrtf(fmaxf(gprev[i][j] + rho2, 0.0f));
+        const float d0 = sqrtf(fmaxf(((i & 1) ? gb : ga) + rho2, 0.0f));
         const float d_crit = (dl + sqrtf(fmaf(one_minus_alpha * dl, dl, alpha * alpha * rho2))) * inv_alpha;
         act = act || !(d0 - steps * dl >= fmaf(1.02f, d_crit, 0.05f));
       }
-      if (o[i].z == 0.0f) act = false;          // null obstacle: weight 0
+      if (((i & 1) ? wb : wa) == 0.0f) act = false;          // null obstacle: weight 0
       active |= act ? (1u << i) : 0u;
     }
     active = __reduce_or_sync(__activemask(), active);
@@ -128,25 +152,27 @@ __device__ __forceinline__ GroupCost barrier_group(const DeviceParams& P, const 
       if (PRECISE) track += (double)(goal_cost(P, X, g) + hitch_cost(P, X, v_t));
       else track += (double)tracking_cost_fma(P, X, g, v_t);
     }
-    const float tf = (float)(t + 1);
-    float pen = 0.0f;
+    const float tfp = (float)(t + 1);
+    f32x2 pen = pack2(0.0f, 0.0f);
 #pragma unroll
-    for (int i = 0; i < kObsGroup; ++i) {
-      if (CULL && !(active & (1u << i))) continue;      // warp-uniform
-      float ox = o[i].x, oy = o[i].y;
-      if (i < NM) { const float2 w = vel[i]; ox = fmaf(tf, w.x, ox); oy = fmaf(tf, w.y, oy); }
-      float Pi = 0.0f;
+    for (int p = 0; p < NP; ++p) {
+      if (CULL && !(active & (3u << (2 * p)))) continue;      // warp-uniform
+      f32x2 ex, ey;
+      centres(p, tfp, ex, ey);
 #pragma unroll
       for (int j = 0; j < ND; ++j) {
-        const float dx = cx[j] - ox, dy = cy[j] - oy;
-        const float gn = fmaf(dx, dx, fmaf(dy, dy, o[i].w));
-        const float z = fmaf(one_minus_alpha, gprev[i][j], -gn);
-        Pi += z + fabsf(z);                                       // 2 max(0, z), exactly
-        gprev[i][j] = gn;
+        const f32x2 dx = add2(pack2(cx[j], cx[j]), ex), dy = add2(pack2(cy[j], cy[j]), ey);
+        const f32x2 gn = fma2(dx, dx, fma2(dy, dy, mrho2[p]));
+        const f32x2 zn = fma2(gprev[p][j], noma, gn);             // g_{t+1} - (1-alpha) g_t = -z
+        float za, zb;
+        unpack2(zn, za, zb);
+        pen = fma2(nw[p], pack2(fminf(za, 0.0f), fminf(zb, 0.0f)), pen);   // + max(0, z) / rho^2
+        gprev[p][j] = gn;
       }
-      pen = fmaf(o[i].z, Pi, pen);
     }
-    bar += (double)pen;
+    float pa, pb;
+    unpack2(pen, pa, pb);
+    bar += (double)(pa + pb);
   }
   return GroupCost{track, bar};
 }
@@ -406,6 +432,9 @@ rollout_cta(const __grid_constant__ DeviceParams P) {
     } else if (new_scene && warp == kChainWarps) {
       // obstacle table for phase C, in the vehicle-centred frame: moving obstacles first, static
       // ones after (groups without a moving one skip the o(t) update), null padding behind.
+      // Obstacles 2p and 2p+1 are interleaved field by field -- (-ox, -ox'), (-oy, -oy'),
+      // (-1/rho^2, ..), (-rho^2, ..); velocities (-dt vx, ..), (-dt vy, ..) -- so that phase C
+      // loads each pair of fields as one packed f32x2 operand.
       // Lane l ranks obstacles l and l + 32 by counting; the chain warps are busy meanwhile.
       CtaMisc* sM = BRMPPI_SMEM(CtaMisc, P.off_misc);
       const float* sRaw = BRMPPI_SMEM(float, P.off_raw);
@@ -426,13 +455,21 @@ rollout_cta(const __grid_constant__ DeviceParams P) {
           const bool moving = (sRaw[5 * i + 3] != 0.0f || sRaw[5 * i + 4] != 0.0f);
           const int dst = moving ? before_m : nm + before_s;
           const float rho = sRaw[5 * i + 2] + P.disc_radius;
-          sObs[dst] = make_float4(sRaw[5 * i + 0] - x0.x, sRaw[5 * i + 1] - x0.y, 0.5f / (rho * rho), -(rho * rho));
-          sVel[dst] = make_float2(P.dt * sRaw[5 * i + 3], P.dt * sRaw[5 * i + 4]);
+          float* ob = reinterpret_cast<float*>(sObs) + (dst >> 1) * 8 + (dst & 1);
+          ob[0] = -(sRaw[5 * i + 0] - x0.x);
+          ob[2] = -(sRaw[5 * i + 1] - x0.y);
+          ob[4] = -2.0f * (0.5f / (rho * rho));
+          ob[6] = -(rho * rho);
+          float* vl = reinterpret_cast<float*>(sVel) + (dst >> 1) * 4 + (dst & 1);
+          vl[0] = -(P.dt * sRaw[5 * i + 3]);
+          vl[2] = -(P.dt * sRaw[5 * i + 4]);
           // displacement per step, rounded up (culling bound)
           sSpd[dst] = 1.0001f * P.dt * sqrtf(fmaf(sRaw[5 * i + 3], sRaw[5 * i + 3], sRaw[5 * i + 4] * sRaw[5 * i + 4]));
         } else {                                        // null obstacle: weight 0
-          sObs[i] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
-          sVel[i] = make_float2(0.0f, 0.0f);
+          float* ob = reinterpret_cast<float*>(sObs) + (i >> 1) * 8 + (i & 1);
+          ob[0] = 0.0f; ob[2] = 0.0f; ob[4] = 0.0f; ob[6] = 0.0f;
+          float* vl = reinterpret_cast<float*>(sVel) + (i >> 1) * 4 + (i & 1);
+          vl[0] = 0.0f; vl[2] = 0.0f;
           sSpd[i] = 0.0f;
         }
       }
