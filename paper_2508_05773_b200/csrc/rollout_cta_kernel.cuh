@@ -41,14 +41,18 @@ __device__ __forceinline__ unsigned long long global_ns() {
 // first group (TRACK) -- the goal / heading / hitch stage cost of every state it visits (a6).
 //
 // Arithmetic form.  With rho = R + r_v and g = |c - o|^2 - rho^2 (so h = g / rho^2):
-//     max(0, (1-alpha) h_t - h_{t+1}) = (1 / (2 rho^2)) (z + |z|),   z = (1-alpha) g_t - g_{t+1},
-// i.e. per (obstacle, disc): 2 subtractions, 2 FMAs for g, 1 FMA for z, 1 add with an |.| operand
-// modifier and 1 accumulate -- seven FMA-pipe instructions, no FMNMX on the half-rate ALU pipe and
-// no per-evaluation multiply by 1/rho^2 (that factor is applied once per obstacle and step).
-// Measured on B200: 7.6-8.7 issue slots per evaluation against 9.7-11.5 for the h / fmaxf form.
-// Obstacle record: (ox, oy, 1/(2 rho^2), -rho^2); a null (padding) obstacle is (0, 0, 0, 0): its
-// weight is 0, so it adds exactly 0.  The first NM obstacles of the group move:
-// o(t) = o(0) + t dt vel (a static one has vel == 0, so rounding NM up is exact).
+//     max(0, (1-alpha) h_t - h_{t+1}) = -(1 / rho^2) min(0, zn),   zn = g_{t+1} - (1-alpha) g_t.
+// Obstacles are taken two at a time on packed f32x2 operands (add/fma.rn.f32x2: each half rounds
+// like the scalar instruction, one issue slot for the pair): per (obstacle pair, disc) 2 packed
+// subtractions, 2 packed FMAs for g, 1 for zn, 2 scalar FMNMX, 1 packed accumulate -- 8 issue
+// slots for two evaluations against 14 for the scalar z + |z| form (166 instead of 250
+// instructions per step at 8 obstacles x 3 discs; phase C of CFG2 13.9 -> 12.6 us).
+// The table (written by the sorting warp) interleaves obstacles 2p and 2p+1 field by field, already
+// negated -- (-ox, -ox'), (-oy, -oy'), (-1/rho^2, ..), (-rho^2, ..) -- so every packed operand is
+// one 64-bit shared-memory load; built from scalars, ptxas re-packs them with two MOVs per use.
+// A null (padding) obstacle is all zeros: its weight is 0, so it adds exactly 0.  The first NM
+// obstacles of the group move: o(t) = o(0) + t dt vel (a static one has vel == 0, so rounding NM
+// up is exact).
 // pV, pP1, pP2: this sample's rows of the v, psi1, psi2 planes.
 struct GroupCost { double track, bar; };
 
