@@ -368,3 +368,100 @@ void orc_plant_step(const orc_params* p, double x0[4], const double u0[2], int n
     obstacles[5 * i + 1] += p->dt * obstacles[5 * i + 4];
   }
 }
+
+/* ------------------------------------------------------------------------------------------
+ * Hitch-angle stabiliser, Sec. V-D, reading 28.
+ * ---------------------------------------------------------------------------------------- */
+
+/* Eq. (18). */
+double orc_hitch_barrier(const orc_params* p, const double x[4], double v) {
+  double beta = orc_wrap(x[2] - x[3]);
+  return p->hitch_max - p->hitch_kappa * fabs(v) - fabs(beta);
+}
+
+/* psi1dot - psi2dot of the reduced eq. (6). */
+static double hitch_rate(const orc_params* p, double beta, double v, double delta) {
+  double td = tan(delta);
+  double psi1dot = (v / p->L1) * td;
+  double psi2dot = (v / p->L2) * (sin(beta) - (p->Lh / p->L1) * cos(beta) * td);
+  return psi1dot - psi2dot;
+}
+
+double orc_hitch_rate_cond(const orc_params* p, const double x[4], const double u[2]) {
+  double beta = orc_wrap(x[2] - x[3]);
+  double s = (beta >= 0.0) ? 1.0 : -1.0;
+  return -s * p->dt * hitch_rate(p, beta, u[0], u[1]) + p->hitch_alpha * orc_hitch_barrier(p, x, u[0]);
+}
+
+void orc_hitch_constraint(const orc_params* p, const double x[4], const double u_ref[2],
+                          double* c0, double a[2]) {
+  double beta = orc_wrap(x[2] - x[3]);
+  double s = (beta >= 0.0) ? 1.0 : -1.0;
+  double v = u_ref[0], delta = u_ref[1];
+  double td = tan(delta), cd = cos(delta);
+  double sgn_v = (v > 0.0) ? 1.0 : ((v < 0.0) ? -1.0 : 0.0);
+  /* d betadot / d v      = tan(delta)/L1 - (sin beta - (Lh/L1) cos beta tan(delta))/L2
+   * d betadot / d delta  = v (1/L1 + Lh cos beta/(L1 L2)) / cos^2(delta)                   */
+  double dv = td / p->L1 - (sin(beta) - (p->Lh / p->L1) * cos(beta) * td) / p->L2;
+  double dd = v * (1.0 / p->L1 + p->Lh * cos(beta) / (p->L1 * p->L2)) / (cd * cd);
+  *c0 = orc_hitch_rate_cond(p, x, u_ref);
+  a[0] = -s * p->dt * dv - p->hitch_alpha * p->hitch_kappa * sgn_v;
+  a[1] = -s * p->dt * dd;
+}
+
+int orc_hitch_filter(const orc_params* p, const double x[4], const double u_ref[2], double u_out[2]) {
+  const double lo[2] = {p->v_min, p->delta_min}, hi[2] = {p->v_max, p->delta_max};
+  const double q[2] = {p->hitch_qv, p->hitch_qdelta};
+  double c0, a[2];
+  orc_hitch_constraint(p, x, u_ref, &c0, a);
+
+  /* Constraint lines n . u = r: the half-plane boundary and the four box edges. */
+  double n[5][2] = {{a[0], a[1]}, {1, 0}, {1, 0}, {0, 1}, {0, 1}};
+  double r[5] = {a[0] * u_ref[0] + a[1] * u_ref[1] - c0, lo[0], hi[0], lo[1], hi[1]};
+
+  /* Candidates: the unconstrained minimiser, its Q-projection on each line, every pairwise
+   * intersection of lines.  The minimiser of a strictly convex QP is the minimiser over the
+   * affine hull of its active constraints, hence one of these. */
+  double cand[16][2];
+  int nc = 0;
+  cand[nc][0] = u_ref[0]; cand[nc][1] = u_ref[1]; ++nc;
+  for (int i = 0; i < 5; ++i) {
+    double nqn = n[i][0] * n[i][0] / q[0] + n[i][1] * n[i][1] / q[1];
+    if (nqn == 0.0) continue;
+    double mu = (r[i] - n[i][0] * u_ref[0] - n[i][1] * u_ref[1]) / nqn;
+    cand[nc][0] = u_ref[0] + mu * n[i][0] / q[0];
+    cand[nc][1] = u_ref[1] + mu * n[i][1] / q[1];
+    ++nc;
+  }
+  for (int i = 0; i < 5; ++i)
+    for (int j = i + 1; j < 5; ++j) {
+      double det = n[i][0] * n[j][1] - n[i][1] * n[j][0];
+      if (det == 0.0) continue;
+      cand[nc][0] = (r[i] * n[j][1] - n[i][1] * r[j]) / det;
+      cand[nc][1] = (n[i][0] * r[j] - r[i] * n[j][0]) / det;
+      ++nc;
+    }
+
+  const double eps = 1e-12;
+  double scale = fabs(c0) + fabs(a[0]) * (hi[0] - lo[0]) + fabs(a[1]) * (hi[1] - lo[1]) + 1e-300;
+  int best = -1;
+  double best_J = 0.0;
+  for (int m = 0; m < nc; ++m) {
+    double v = cand[m][0], d = cand[m][1];
+    if (v < lo[0] - eps * (hi[0] - lo[0]) || v > hi[0] + eps * (hi[0] - lo[0])) continue;
+    if (d < lo[1] - eps * (hi[1] - lo[1]) || d > hi[1] + eps * (hi[1] - lo[1])) continue;
+    double g = c0 + a[0] * (v - u_ref[0]) + a[1] * (d - u_ref[1]);
+    if (g < -eps * scale) continue;
+    double J = q[0] * (v - u_ref[0]) * (v - u_ref[0]) + q[1] * (d - u_ref[1]) * (d - u_ref[1]);
+    if (best < 0 || J < best_J) { best = m; best_J = J; }
+  }
+  double uc[2];
+  for (int i = 0; i < 2; ++i) uc[i] = fmin(fmax(u_ref[i], lo[i]), hi[i]);
+  if (best < 0) {
+    for (int i = 0; i < 2; ++i) u_out[i] = (a[i] > 0.0) ? hi[i] : ((a[i] < 0.0) ? lo[i] : uc[i]);
+    return 2;
+  }
+  for (int i = 0; i < 2; ++i) u_out[i] = fmin(fmax(cand[best][i], lo[i]), hi[i]);
+  double g_ref = c0 + a[0] * (uc[0] - u_ref[0]) + a[1] * (uc[1] - u_ref[1]);
+  return (g_ref >= 0.0) ? 0 : 1;
+}

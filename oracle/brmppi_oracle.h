@@ -15,6 +15,8 @@
  *   stage + terminal cost structure, eq. (7) ...... PAPER.md:135
  *   quadratic tracking / heading / effort terms ... PAPER.md:202
  *   hitch-angle limit ............................. PAPER.md:231-235
+ *   hitch-angle stabiliser: barrier (18), CBF-QP .. PAPER.md:229-239 with (3) PAPER.md:66-76
+ *                                                   (reading 28)
  *
  * Pin status (tests/test_oracle_*.py, all `-m "not gpu"`):
  *   philox4x32_10 ............ pinned: published known-answer vectors + cuRAND header constants
@@ -27,6 +29,11 @@
  *                              invariance, lambda->0 argmin, lambda->inf mean, sigma=0 fixed point
  *   super-ellipse barrier .... pinned: boundary points, e = 2 & m_x = m_y reduces to the disc barrier,
  *                              rotation covariance, corner value, brute force with super-ellipses
+ *   hitch stabiliser ......... pinned: hand value of (18); rate condition == exact discrete condition (2)
+ *                              through the pinned Euler step; gradient by finite differences; QP against
+ *                              scipy SLSQP, a dense grid search and the halfspace-projection closed form;
+ *                              closed-loop forward invariance of |hitch| <= limit under a jackknifing
+ *                              reference.  The linearisation in u about u_ref is reading 28, not the paper's.
  *   whole solve .............. pinned: brute force (independent mpmath transcription) K<=8, T<=5
  *   cost weights, disc placement, hinge shapes (linear barrier hinge, squared hitch hinge),
  *   scene generators ......... PARITY UNPINNED by the paper (never printed there); fixed by the
@@ -57,6 +64,8 @@ typedef struct {
   double alpha_lo, alpha_hi;
   double w_pos, w_head, w_v, w_delta, w_hitch, hitch_max, w_bar, w_term, lambda;
   double hitch_kappa;     /* hitch limit = hitch_max - hitch_kappa |v| (eq. (18)) */
+  double hitch_alpha;     /* alpha of condition (3) in the hitch stabiliser, in (0, 1] */
+  double hitch_qv, hitch_qdelta;  /* Q_h = diag(q_v, q_delta) > 0 of the CBF-QP     */
   uint64_t seed;          /* Philox key = (lo32(seed), hi32(seed))                     */
 } orc_params;
 
@@ -156,6 +165,31 @@ void orc_shift(int T, double* U);
 /* Plant step: x0 <- Euler(x0, u0), psi wrapped to [-pi, pi); obstacles advanced by dt * vel. */
 void orc_plant_step(const orc_params* p, double x0[4], const double u0[2], int n_obs,
                     double* obstacles);
+
+/* ---- hitch-angle stabiliser, Sec. V-D (reading 28) ----------- */
+
+/* Eq. (18): h_h = hitch_max - hitch_kappa |v| - |wrap(psi1 - psi2)|.  The reduced model has the speed
+ * as an input, so "v(x)" is the speed applied over the step; |v| because the vehicle reverses. */
+double orc_hitch_barrier(const orc_params* p, const double x[4], double v);
+
+/* c(u) = [h_h(x_{k+1}) - h_h(x_k)] + alpha h_h(x_k) with |.| of the hitch angle expanded to first
+ * order about x_k, i.e. the left side minus the right side of (3) in the sign of reading 1:
+ *   c(u) = -s dt betadot(x_k, u) + hitch_alpha (hitch_max - hitch_kappa |v| - |beta|),
+ * beta = wrap(psi1 - psi2), s = +1 if beta >= 0 else -1, betadot = psi1dot - psi2dot of eq. (6). */
+double orc_hitch_rate_cond(const orc_params* p, const double x[4], const double u[2]);
+
+/* First-order Taylor expansion of c in u about u_ref (the model is not affine in (v, delta)):
+ * c(u) ~ *c0 + a . (u - u_ref).  d|v|/dv at v = 0 is taken as 0. */
+void orc_hitch_constraint(const orc_params* p, const double x[4], const double u_ref[2],
+                          double* c0, double a[2]);
+
+/* u* = argmin_{u in box} q_v (v - v_ref)^2 + q_delta (delta - delta_ref)^2
+ *      s.t. c0 + a . (u - u_ref) >= 0
+ * solved by enumerating the active sets of the five constraints.  Returns 0 if the constraint is
+ * inactive (u* = u_ref clamped into the box), 1 if it is active, 2 if box and half-plane do not
+ * intersect; then u* is the point of the box with the largest a . u (coordinates with a_i = 0 keep
+ * the clamped reference). */
+int orc_hitch_filter(const orc_params* p, const double x[4], const double u_ref[2], double u_out[2]);
 
 #ifdef __cplusplus
 }

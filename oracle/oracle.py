@@ -37,6 +37,7 @@ class _Params(C.Structure):
                 ("w_pos", C.c_double), ("w_head", C.c_double), ("w_v", C.c_double),
                 ("w_delta", C.c_double), ("w_hitch", C.c_double), ("hitch_max", C.c_double),
                 ("w_bar", C.c_double), ("w_term", C.c_double), ("lam", C.c_double), ("hitch_kappa", C.c_double),
+                ("hitch_alpha", C.c_double), ("hitch_qv", C.c_double), ("hitch_qdelta", C.c_double),
                 ("seed", C.c_uint64)]
 
 
@@ -96,6 +97,14 @@ def lib():
         L.orc_shift.restype = None
         L.orc_plant_step.argtypes = [C.POINTER(_Params), _dp, _dp, C.c_int, _dp]
         L.orc_plant_step.restype = None
+        L.orc_hitch_barrier.argtypes = [C.POINTER(_Params), _dp, C.c_double]
+        L.orc_hitch_barrier.restype = C.c_double
+        L.orc_hitch_rate_cond.argtypes = [C.POINTER(_Params), _dp, _dp]
+        L.orc_hitch_rate_cond.restype = C.c_double
+        L.orc_hitch_constraint.argtypes = [C.POINTER(_Params), _dp, _dp, _dp, _dp]
+        L.orc_hitch_constraint.restype = None
+        L.orc_hitch_filter.argtypes = [C.POINTER(_Params), _dp, _dp, _dp]
+        L.orc_hitch_filter.restype = C.c_int
         _lib = L
     return _lib
 
@@ -109,7 +118,8 @@ def _cparams(p) -> _Params:
         s.disc_offset[j] = float(off)
     for name in ("disc_radius", "dt", "L1", "L2", "Lh", "v_min", "v_max", "delta_min",
                  "delta_max", "sigma_v", "sigma_delta", "alpha_lo", "alpha_hi", "w_pos", "w_head",
-                 "w_v", "w_delta", "w_hitch", "hitch_max", "w_bar", "w_term", "lam", "hitch_kappa"):
+                 "w_v", "w_delta", "w_hitch", "hitch_max", "w_bar", "w_term", "lam", "hitch_kappa",
+                 "hitch_alpha", "hitch_qv", "hitch_qdelta"):
         setattr(s, name, float(getattr(p, name)))
     s.seed = int(p.seed) & 0xFFFFFFFFFFFFFFFF
     return s
@@ -301,3 +311,28 @@ def plant_step(p, x0, u0, obstacles):
     obs = _d(obstacles).reshape(-1, 5).copy()
     lib().orc_plant_step(C.byref(cp), _ptr(x), _ptr(u0), obs.shape[0], _ptr(obs))
     return x, obs
+
+
+def hitch_barrier(p, x, v):
+    """eq. (18), PAPER.md:233."""
+    return lib().orc_hitch_barrier(C.byref(_cparams(p)), _ptr(_d(x, (4,))), float(v))
+
+
+def hitch_rate_cond(p, x, u):
+    return lib().orc_hitch_rate_cond(C.byref(_cparams(p)), _ptr(_d(x, (4,))), _ptr(_d(u, (2,))))
+
+
+def hitch_constraint(p, x, u_ref):
+    """(c0, a): c(u) ~ c0 + a . (u - u_ref), reading 28."""
+    c0 = C.c_double()
+    a = np.zeros(2)
+    lib().orc_hitch_constraint(C.byref(_cparams(p)), _ptr(_d(x, (4,))), _ptr(_d(u_ref, (2,))),
+                               C.byref(c0), _ptr(a))
+    return c0.value, a
+
+
+def hitch_filter(p, x, u_ref):
+    """CBF-QP of Sec. V-D: (u*, status)."""
+    u = np.zeros(2)
+    st = lib().orc_hitch_filter(C.byref(_cparams(p)), _ptr(_d(x, (4,))), _ptr(_d(u_ref, (2,))), _ptr(u))
+    return u, int(st)

@@ -42,6 +42,11 @@ class Params:
     w_hitch: float = 10.0
     hitch_max: float = 1.2
     hitch_kappa: float = 0.0      # velocity-dependent hitch limit hitch_max - kappa |v| (eq. 18); 0 = fixed limit
+    # hitch-angle stabiliser, Sec. V-D (reading 28); off by default
+    hitch_filter: int = 0         # 1: brmppi_step passes U[0] through the CBF-QP before the plant step
+    hitch_alpha: float = 0.5      # alpha of condition (3), in (0, 1]
+    hitch_qv: float = 1.0         # Q_h = diag(q_v, q_delta)
+    hitch_qdelta: float = 1.0
     w_bar: float = 1.0e3
     w_term: float = 10.0
     lam: float = 1.0
