@@ -102,6 +102,11 @@ typedef struct {
   int max_superellipses;  /* capacity per scene, 0..BRMPPI_MAX_SUPERELLIPSES                     */
   float hitch_kappa;      /* >= 0: the hitch-angle hinge starts at hitch_max - hitch_kappa |v|
                              (eq. (18)); 0 = fixed limit                        */
+  /* Hitch-angle stabiliser, Sec. V-D (reading 28).                    */
+  int hitch_filter;       /* 0 = off; 1 = brmppi_step passes U[0] through the CBF-QP below before
+                             it is applied to the plant.  Never changes U itself.                 */
+  float hitch_alpha;      /* alpha of condition (3), in (0, 1]         (read only if hitch_filter) */
+  float hitch_qv, hitch_qdelta;   /* Q_h = diag(q_v, q_delta), both > 0 (read only if hitch_filter) */
 } brmppi_params;
 
 #define BRMPPI_MAX_T 512
@@ -167,6 +172,11 @@ int brmppi_get_superellipses(brmppi_ctx* ctx, int scene, int* n_out, brmppi_supe
 int brmppi_get_costs(brmppi_ctx* ctx, int scene, float* S_out /* K */);             /* FLAG_WRITE_SAMPLES */
 int brmppi_get_final_states(brmppi_ctx* ctx, int scene, float* X_out /* K*4 */);    /* FLAG_WRITE_SAMPLES */
 int brmppi_get_diag(brmppi_ctx* ctx, int scene, brmppi_diag* out);
+/* What the hitch-angle stabiliser did in the last brmppi_step: u_ref = the BR-MPPI control U[0] it was
+ * given, *status = 0 (rate constraint inactive, applied control = u_ref), 1 (active), 2 (no control in
+ * the box satisfies the constraint; the least-violating one was applied).  With hitch_filter = 0 the
+ * status is always 0.  HOST pointers; synchronises. */
+int brmppi_get_hitch_filter(brmppi_ctx* ctx, int scene, float u_ref[2], int* status);
 
 /* Device time of the two kernels of one MPPI iteration, for the roofline report.  OUTSIDE the
  * captured graph, on the context's stream, enqueues back to back and synchronises once: `reps` (+2
@@ -211,6 +221,21 @@ int brmppi_debug_sample_controls(void* cuda_stream, const brmppi_params* p, unsi
  * out[0..7] = {ffma, alu, mufu, mix (ffma+lop3 interleaved), imad_wide, n_sms, sm_mhz of an idle SM,
  * sm_mhz seen while the FFMA kernel ran}.  Rates are whole-kernel: instructions per SM / (first
  * block start .. last block end on the globaltimer, converted with the in-kernel clock). */
+/* Hitch-angle stabiliser on its own, for n independent (state, reference control) pairs
+ * (Sec. V-D).  With beta = wrap(psi1 - psi2), s = sign(beta) (+1 at 0) and
+ *   h_h = hitch_max - hitch_kappa |v| - |beta|                                          eq. (18)
+ *   c(u) = -s dt (psi1dot - psi2dot)(x, u) + hitch_alpha h_h        condition (3), sign of reading 1
+ * the constraint is c expanded to first order in u about u_ref (reading 28: the reduced model is not
+ * affine in (v, delta)), and
+ *   u* = argmin q_v (v - v_ref)^2 + q_delta (delta - delta_ref)^2
+ *        s.t. c(u_ref) + grad c(u_ref) . (u - u_ref) >= 0,  v_min <= v <= v_max,  delta_min <= delta <= delta_max.
+ * x: HOST [n][4] states (x, y, psi1, psi2); u_ref: HOST [n][2]; u_out: HOST [n][2]; status_out: HOST
+ * [n] or NULL, values as in brmppi_get_hitch_filter.  Uses p->dt, L1, L2, Lh, the control box and the
+ * hitch_* fields (hitch_filter itself is ignored).  Allocates and frees its own device scratch;
+ * synchronises the stream.  n = 0 is a no-op. */
+int brmppi_hitch_filter(void* cuda_stream, const brmppi_params* p, int n, const float* x,
+                        const float* u_ref, float* u_out, int* status_out);
+
 int brmppi_measure_peaks(void* cuda_stream, float out[8]);
 
 #ifdef __cplusplus

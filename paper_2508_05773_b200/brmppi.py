@@ -27,7 +27,7 @@ EXPORTS = [
     "brmppi_reset", "brmppi_solve", "brmppi_shift", "brmppi_step", "brmppi_get_controls",
     "brmppi_get_state", "brmppi_get_obstacles", "brmppi_get_costs", "brmppi_get_final_states",
     "brmppi_get_diag", "brmppi_get_phase_times", "brmppi_time_kernels", "brmppi_launch_count", "brmppi_strerror", "brmppi_debug_philox",
-    "brmppi_debug_sample_controls", "brmppi_measure_peaks",
+    "brmppi_debug_sample_controls", "brmppi_measure_peaks", "brmppi_get_hitch_filter", "brmppi_hitch_filter",
 ]
 
 
@@ -58,7 +58,8 @@ class CParams(C.Structure):
                 ("w_delta", C.c_float), ("w_hitch", C.c_float), ("hitch_max", C.c_float),
                 ("w_bar", C.c_float), ("w_term", C.c_float), ("lam", C.c_float),
                 ("seed", C.c_ulonglong), ("flags", C.c_uint), ("max_superellipses", C.c_int),
-                ("hitch_kappa", C.c_float)]
+                ("hitch_kappa", C.c_float), ("hitch_filter", C.c_int), ("hitch_alpha", C.c_float),
+                ("hitch_qv", C.c_float), ("hitch_qdelta", C.c_float)]
 
 
 class Diag(C.Structure):
@@ -114,6 +115,8 @@ def lib():
         L.brmppi_debug_philox.argtypes = [vp, C.c_ulonglong, C.c_uint, C.c_int, C.c_int, C.c_uint, vp]
         L.brmppi_debug_sample_controls.argtypes = [vp, C.POINTER(CParams), C.c_uint, _fp, vp, vp]
         L.brmppi_measure_peaks.argtypes = [vp, _fp]
+        L.brmppi_get_hitch_filter.argtypes = [vp, C.c_int, _fp, C.POINTER(C.c_int)]
+        L.brmppi_hitch_filter.argtypes = [vp, C.POINTER(CParams), C.c_int, _fp, _fp, _fp, C.POINTER(C.c_int)]
         _lib = L
     return _lib
 
@@ -141,6 +144,10 @@ def make_cparams(p, n_scenes=1, max_obstacles=8, flags=0, max_superellipses=0) -
     c.seed, c.flags = int(p.seed) & 0xFFFFFFFFFFFFFFFF, int(flags)
     c.max_superellipses = int(max_superellipses)
     c.hitch_kappa = float(getattr(p, "hitch_kappa", 0.0))
+    c.hitch_filter = int(getattr(p, "hitch_filter", 0))
+    c.hitch_alpha = float(getattr(p, "hitch_alpha", 0.5))
+    c.hitch_qv = float(getattr(p, "hitch_qv", 1.0))
+    c.hitch_qdelta = float(getattr(p, "hitch_qdelta", 1.0))
     return c
 
 
@@ -284,6 +291,13 @@ class Solver:
         _check(lib().brmppi_get_diag(self._ctx, scene, C.byref(d)))
         return dict(S_min=d.S_min, argmin=d.argmin, eta=d.eta, ess=d.ess, n=d.n, nonfinite=d.nonfinite)
 
+    def get_hitch_filter(self, scene=0):
+        """(u_ref, status) of the hitch-angle stabiliser in the last step()."""
+        u = np.zeros(2, dtype=np.float32)
+        st = C.c_int()
+        _check(lib().brmppi_get_hitch_filter(self._ctx, scene, _p(u), C.byref(st)))
+        return u, int(st.value)
+
     def time_kernels(self, reps=20):
         """Mean device ms per launch of (rollout kernel, merge/update kernel)."""
         out = np.zeros(2, dtype=np.float32)
@@ -322,6 +336,22 @@ def debug_sample_controls(params, n, U_nominal=None, flags=0):
     _check(lib().brmppi_debug_sample_controls(C.c_void_p(st.cuda_stream), C.byref(cp), int(n), Un,
                                               C.c_void_p(u.data_ptr()), C.c_void_p(a.data_ptr())))
     return u.cpu().numpy().reshape(params.K, params.T, 2), a.cpu().numpy()
+
+
+def hitch_filter(params, x, u_ref):
+    """Hitch-angle stabiliser (Sec. V-D) for n (state, reference control) pairs: (u[n][2], status[n])."""
+    import torch
+    x = _f32(x).reshape(-1, 4)
+    r = _f32(u_ref).reshape(-1, 2)
+    n = x.shape[0]
+    assert r.shape[0] == n
+    cp = make_cparams(params, 1, 0, 0)
+    u = np.zeros((n, 2), dtype=np.float32)
+    status = np.zeros(n, dtype=np.int32)
+    st = torch.cuda.current_stream()
+    _check(lib().brmppi_hitch_filter(C.c_void_p(st.cuda_stream), C.byref(cp), n, _p(x), _p(r), _p(u),
+                                     status.ctypes.data_as(C.POINTER(C.c_int))))
+    return u, status
 
 
 def measure_peaks():

@@ -43,6 +43,13 @@ bool finite_all(const float* v, int n) {
   return true;
 }
 
+bool hitch_params_valid(const brmppi_params* p) {
+  const float f[] = {p->hitch_alpha, p->hitch_qv, p->hitch_qdelta, p->hitch_max, p->hitch_kappa};
+  if (!finite_all(f, 5)) return false;
+  return p->hitch_alpha > 0.f && p->hitch_alpha <= 1.f && p->hitch_qv > 0.f && p->hitch_qdelta > 0.f &&
+         p->hitch_kappa >= 0.f;
+}
+
 bool params_valid(const brmppi_params* p) {
   if (!p) return false;
   if (p->K < 1 || p->K > (1 << 27)) return false;
@@ -65,6 +72,8 @@ bool params_valid(const brmppi_params* p) {
   if (!(p->dt > 0.f) || !(p->L1 > 0.f) || !(p->L2 > 0.f) || !(p->lambda > 0.f)) return false;
   if (p->disc_radius < 0.f || p->sigma_v < 0.f || p->sigma_delta < 0.f) return false;
   if (!std::isfinite(p->hitch_kappa) || p->hitch_kappa < 0.f) return false;
+  if (p->hitch_filter != 0 && p->hitch_filter != 1) return false;
+  if (p->hitch_filter && !hitch_params_valid(p)) return false;
   if (p->v_min > p->v_max || p->delta_min > p->delta_max) return false;
   if (p->delta_min <= -1.5f || p->delta_max >= 1.5f) return false;   // tan(delta) must stay finite
   if (p->alpha_lo > p->alpha_hi) return false;
@@ -77,7 +86,7 @@ bool params_valid(const brmppi_params* p) {
 
 struct Layout {
   size_t state, goal, n_obs, obstacles, n_se, se, U, counter, u0, part_m, part_argmin, part_eta, part_w2,
-      part_nf, part_A, diag, S, XT, phase, total;
+      part_nf, part_A, diag, S, XT, phase, hitch, total;
 };
 
 // Launch plan: which rollout kernel, how the sample axis is tiled, how many partials.
@@ -128,6 +137,7 @@ Layout make_layout(const brmppi_params& p, const Plan& pl) {
   L.U = take(ns * T * 8);
   L.counter = take(4);
   L.u0 = take(ns * 8);
+  L.hitch = take(ns * 16);
   L.part_m = take(ns * P * 8);
   L.part_argmin = take(ns * P * 4);
   L.part_eta = take(ns * P * 4);
@@ -286,6 +296,8 @@ int brmppi_create(const brmppi_params* p, void* dev_workspace, size_t workspace_
   d.w_pos = p->w_pos; d.w_head = p->w_head; d.w_v = p->w_v; d.w_delta = p->w_delta;
   d.w_hitch = p->w_hitch; d.hitch_max = p->hitch_max; d.hitch_kappa = p->hitch_kappa; d.w_bar = p->w_bar; d.w_term = p->w_term;
   d.inv_lambda = 1.0f / p->lambda;
+  d.hitch_filter = p->hitch_filter; d.hitch_alpha = p->hitch_alpha;
+  d.hitch_qv = p->hitch_qv; d.hitch_qdelta = p->hitch_qdelta;
   d.key0 = (uint32_t)(p->seed & 0xFFFFFFFFull); d.key1 = (uint32_t)(p->seed >> 32);
   d.flags = p->flags;
   d.n_partials = c->plan.n_partials;
@@ -308,6 +320,7 @@ int brmppi_create(const brmppi_params* p, void* dev_workspace, size_t workspace_
   d.n_se = (int*)(base + L.n_se); d.se = (float*)(base + L.se); d.max_superellipses = p->max_superellipses;
   d.U = (float*)(base + L.U); d.counter = (uint32_t*)(base + L.counter);
   d.u0_applied = (float*)(base + L.u0);
+  d.hitch_ref = (float*)(base + L.hitch);
   d.part_m = (double*)(base + L.part_m); d.part_argmin = (int*)(base + L.part_argmin);
   d.part_eta = (float*)(base + L.part_eta); d.part_w2 = (float*)(base + L.part_w2);
   d.part_nonfinite = (int*)(base + L.part_nf); d.part_A = (float*)(base + L.part_A);
@@ -709,6 +722,58 @@ int brmppi_debug_sample_controls(void* cuda_stream, const brmppi_params* p, unsi
   }
   if (e == cudaSuccess) e = cudaStreamSynchronize(s);
   cudaFree(dU);
+  if (e != cudaSuccess) return cuda_fail(e);
+  return BRMPPI_OK;
+}
+
+int brmppi_get_hitch_filter(brmppi_ctx* c, int scene, float u_ref[2], int* status) {
+  int r = check_scene(c, scene);
+  if (r) return r;
+  if (!u_ref || !status) return BRMPPI_ERR_NULL;
+  float h[4];
+  r = d2h(c, h, c->d.hitch_ref + (size_t)scene * 4, sizeof(h));
+  if (r) return r;
+  u_ref[0] = h[0]; u_ref[1] = h[1];
+  memcpy(status, &h[2], sizeof(int));
+  return BRMPPI_OK;
+}
+
+int brmppi_hitch_filter(void* cuda_stream, const brmppi_params* p, int n, const float* x,
+                        const float* u_ref, float* u_out, int* status_out) {
+  if (!p) return BRMPPI_ERR_NULL;
+  if (n < 0) return BRMPPI_ERR_INVALID_ARG;
+  const float f[] = {p->dt, p->L1, p->L2, p->Lh, p->v_min, p->v_max, p->delta_min, p->delta_max};
+  if (!finite_all(f, 8) || !hitch_params_valid(p) || !(p->dt > 0.f) || !(p->L1 > 0.f) || !(p->L2 > 0.f) ||
+      p->v_min > p->v_max || p->delta_min > p->delta_max || p->delta_min <= -1.5f || p->delta_max >= 1.5f)
+    return BRMPPI_ERR_INVALID_ARG;
+  if (n == 0) return BRMPPI_OK;
+  if (!x || !u_ref || !u_out) return BRMPPI_ERR_NULL;
+  cudaStream_t s = (cudaStream_t)cuda_stream;
+  DeviceParams d;
+  memset(&d, 0, sizeof(d));
+  d.dt = p->dt; d.inv_L1 = 1.0f / p->L1; d.inv_L2 = 1.0f / p->L2; d.Lh = p->Lh;
+  d.Lh_over_L1 = p->Lh / p->L1; d.Lh_over_L2 = p->Lh / p->L2;
+  d.v_min = p->v_min; d.v_max = p->v_max; d.delta_min = p->delta_min; d.delta_max = p->delta_max;
+  d.hitch_max = p->hitch_max; d.hitch_kappa = p->hitch_kappa; d.hitch_alpha = p->hitch_alpha;
+  d.hitch_qv = p->hitch_qv; d.hitch_qdelta = p->hitch_qdelta;
+  // one scratch allocation: x [n][4] | u_ref [n][2] | u_out [n][2] | status [n]
+  const size_t N = (size_t)n;
+  unsigned char* buf = nullptr;
+  CU(cudaMalloc((void**)&buf, N * 36));
+  float4* dx = (float4*)buf;
+  float2* dr = (float2*)(buf + N * 16);
+  float2* du = (float2*)(buf + N * 24);
+  int* ds = (int*)(buf + N * 32);
+  cudaError_t e = cudaMemcpyAsync(dx, x, N * 16, cudaMemcpyHostToDevice, s);
+  if (e == cudaSuccess) e = cudaMemcpyAsync(dr, u_ref, N * 8, cudaMemcpyHostToDevice, s);
+  if (e == cudaSuccess) {
+    hitch_filter_batch<<<(unsigned)((N + 127) / 128), 128, 0, s>>>(d, n, dx, dr, du, ds);
+    e = cudaGetLastError();
+  }
+  if (e == cudaSuccess) e = cudaMemcpyAsync(u_out, du, N * 8, cudaMemcpyDeviceToHost, s);
+  if (e == cudaSuccess && status_out) e = cudaMemcpyAsync(status_out, ds, N * 4, cudaMemcpyDeviceToHost, s);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+  cudaFree(buf);
   if (e != cudaSuccess) return cuda_fail(e);
   return BRMPPI_OK;
 }

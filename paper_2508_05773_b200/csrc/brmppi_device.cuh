@@ -30,6 +30,8 @@ struct DeviceParams {
   float alpha_lo, alpha_span;
   float w_pos, w_head, w_v, w_delta, w_hitch, hitch_max, hitch_kappa, w_bar, w_term;
   float inv_lambda;
+  int hitch_filter;            // 1: shift_plant passes U[0] through the CBF-QP of Sec. V-D
+  float hitch_alpha, hitch_qv, hitch_qdelta;
   uint32_t key0, key1;        // Philox key of scene 0 = (lo32(seed), hi32(seed)); scene s adds s
   uint32_t flags;
   // tiling of the sample axis
@@ -57,6 +59,7 @@ struct DeviceParams {
   float* U;                   // [n_scenes][T][2]
   uint32_t* counter;          // global iteration counter n
   float* u0_applied;          // [n_scenes][2]  control applied by the last plant step
+  float* hitch_ref;           // [n_scenes][4]  (v_ref, delta_ref, status as int bits, 0) of the last plant step
   double* part_m;             // [n_scenes][P]  block minimum of S (fp64)
   int* part_argmin;           // [n_scenes][P]
   float* part_eta;            // [n_scenes][P]

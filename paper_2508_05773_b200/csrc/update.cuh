@@ -8,6 +8,7 @@
 #pragma once
 
 #include "brmppi_device.cuh"
+#include "hitch_filter.cuh"
 
 namespace brmppi {
 
@@ -103,8 +104,12 @@ __global__ void __launch_bounds__(kShiftBlock) shift_plant(const __grid_constant
   float2* U = reinterpret_cast<float2*>(P.U) + (size_t)scene * T;
   if (PLANT) {
     if (tid == 0) {
-      const float2 u0 = U[0];
+      const float2 u_ref = U[0];
       float4 x = reinterpret_cast<float4*>(P.state)[scene];
+      float2 u0 = u_ref;
+      int status = 0;
+      if (P.hitch_filter) u0 = hitch_filter(P, x.z, x.w, u_ref, &status);   // Sec. V-D
+      reinterpret_cast<float4*>(P.hitch_ref)[scene] = make_float4(u_ref.x, u_ref.y, __int_as_float(status), 0.0f);
       float s1, c1, s2, c2;
       sincosf(x.z, &s1, &c1);
       sincosf(x.w, &s2, &c2);
