@@ -236,6 +236,22 @@ int brmppi_debug_sample_controls(void* cuda_stream, const brmppi_params* p, unsi
 int brmppi_hitch_filter(void* cuda_stream, const brmppi_params* p, int n, const float* x,
                         const float* u_ref, float* u_out, int* status_out);
 
+#define BRMPPI_PROJECT_MAX_NO 8
+/* Closed-form projection of BR-MPPI, eq. (11)-(12), for n independent problems:
+ *   min_z ||z - z_des||_W^2 + rho/2 (||z - z_lo||^2 + ||z_hi - z||^2)   s.t.  A z = b,
+ *   z* = M^-1 [ p - A^T (A M^-1 A^T)^-1 (A M^-1 p - b) ],  M = W + rho I,  p = W z_des + rho/2 (z_hi + z_lo),
+ * with z = [u_proj (2), u_proj^alpha (n_o)], d = 2 + n_o, 1 <= n_o <= BRMPPI_PROJECT_MAX_NO.
+ * A: [n][n_o][d] row-major; b: [n][n_o]; z_des: [n][d]; z_out: [n][d] -- HOST pointers if
+ * device_ptrs == 0 (copied in and out through scratch the call allocates and frees), DEVICE pointers,
+ * 16-byte aligned, if device_ptrs == 1 (nothing is allocated; asynchronous on the stream).
+ * w (the diagonal of W, all > 0), z_lo, z_hi: HOST [d], shared by all problems; rho >= 0.
+ * A must have full row rank (A M^-1 A^T is factorised by Cholesky without pivoting); a rank-deficient
+ * problem yields non-finite values in its own z_out row only.  How (9) builds A and b inside a rollout
+ * is not part of this call.  n = 0 is a no-op. */
+int brmppi_project(void* cuda_stream, int n, int n_o, const float* A, const float* b, const float* z_des,
+                   const float* w, float rho, const float* z_lo, const float* z_hi, float* z_out,
+                   int device_ptrs);
+
 int brmppi_measure_peaks(void* cuda_stream, float out[8]);
 
 #ifdef __cplusplus

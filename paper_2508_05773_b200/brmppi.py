@@ -27,7 +27,7 @@ EXPORTS = [
     "brmppi_reset", "brmppi_solve", "brmppi_shift", "brmppi_step", "brmppi_get_controls",
     "brmppi_get_state", "brmppi_get_obstacles", "brmppi_get_costs", "brmppi_get_final_states",
     "brmppi_get_diag", "brmppi_get_phase_times", "brmppi_time_kernels", "brmppi_launch_count", "brmppi_strerror", "brmppi_debug_philox",
-    "brmppi_debug_sample_controls", "brmppi_measure_peaks", "brmppi_get_hitch_filter", "brmppi_hitch_filter",
+    "brmppi_debug_sample_controls", "brmppi_measure_peaks", "brmppi_get_hitch_filter", "brmppi_hitch_filter", "brmppi_project",
 ]
 
 
@@ -115,6 +115,7 @@ def lib():
         L.brmppi_debug_philox.argtypes = [vp, C.c_ulonglong, C.c_uint, C.c_int, C.c_int, C.c_uint, vp]
         L.brmppi_debug_sample_controls.argtypes = [vp, C.POINTER(CParams), C.c_uint, _fp, vp, vp]
         L.brmppi_measure_peaks.argtypes = [vp, _fp]
+        L.brmppi_project.argtypes = [vp, C.c_int, C.c_int, vp, vp, vp, _fp, C.c_float, _fp, _fp, vp, C.c_int]
         L.brmppi_get_hitch_filter.argtypes = [vp, C.c_int, _fp, C.POINTER(C.c_int)]
         L.brmppi_hitch_filter.argtypes = [vp, C.POINTER(CParams), C.c_int, _fp, _fp, _fp, C.POINTER(C.c_int)]
         _lib = L
@@ -352,6 +353,30 @@ def hitch_filter(params, x, u_ref):
     _check(lib().brmppi_hitch_filter(C.c_void_p(st.cuda_stream), C.byref(cp), n, _p(x), _p(r), _p(u),
                                      status.ctypes.data_as(C.POINTER(C.c_int))))
     return u, status
+
+
+def project(A, b, z_des, w, rho, z_lo, z_hi):
+    """Closed-form projection (12) for a batch.  numpy arrays -> HOST-pointer call, returns numpy [n][d];
+    torch CUDA tensors (float32, contiguous) -> DEVICE-pointer call on the current stream, returns a tensor."""
+    import torch
+    st = torch.cuda.current_stream()
+    on_device = isinstance(A, torch.Tensor)
+    n, n_o, d = A.shape
+    w, z_lo, z_hi = _f32(w, (d,)), _f32(z_lo, (d,)), _f32(z_hi, (d,))
+    if on_device:
+        for t in (A, b, z_des):
+            assert t.is_cuda and t.dtype == torch.float32 and t.is_contiguous()
+        out = torch.empty((n, d), dtype=torch.float32, device=A.device)
+        ptr = lambda t: C.c_void_p(t.data_ptr())
+        _check(lib().brmppi_project(C.c_void_p(st.cuda_stream), n, n_o, ptr(A), ptr(b), ptr(z_des), _p(w),
+                                    float(rho), _p(z_lo), _p(z_hi), ptr(out), 1))
+        return out
+    A, b, z_des = _f32(A), _f32(b, (n, n_o)), _f32(z_des, (n, d))
+    out = np.zeros((n, d), dtype=np.float32)
+    ptr = lambda a: C.c_void_p(a.ctypes.data)
+    _check(lib().brmppi_project(C.c_void_p(st.cuda_stream), n, n_o, ptr(A), ptr(b), ptr(z_des), _p(w),
+                                float(rho), _p(z_lo), _p(z_hi), ptr(out), 0))
+    return out
 
 
 def measure_peaks():

@@ -10,7 +10,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libbrmppi.so")
 SOURCES = ["brmppi_api.cu"]
-HEADERS = ["brmppi_device.cuh", "rollout_thread.cuh", "rollout_cta.cuh", "rollout_cta_kernel.cuh", "update.cuh", "peaks.cuh",
+HEADERS = ["brmppi_device.cuh", "rollout_thread.cuh", "rollout_cta.cuh", "rollout_cta_kernel.cuh", "update.cuh", "peaks.cuh", "hitch_filter.cuh", "project.cuh",
            os.path.join("..", "..", "include", "brmppi.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-shared", "--use_fast_math=false", "-Xptxas", "-v"]

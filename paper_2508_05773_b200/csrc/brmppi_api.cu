@@ -17,6 +17,7 @@
 #include "rollout_cta.cuh"
 #include "rollout_cta_kernel.cuh"
 #include "update.cuh"
+#include "project.cuh"
 
 using namespace brmppi;
 
@@ -772,6 +773,49 @@ int brmppi_hitch_filter(void* cuda_stream, const brmppi_params* p, int n, const 
   }
   if (e == cudaSuccess) e = cudaMemcpyAsync(u_out, du, N * 8, cudaMemcpyDeviceToHost, s);
   if (e == cudaSuccess && status_out) e = cudaMemcpyAsync(status_out, ds, N * 4, cudaMemcpyDeviceToHost, s);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+  cudaFree(buf);
+  if (e != cudaSuccess) return cuda_fail(e);
+  return BRMPPI_OK;
+}
+
+int brmppi_project(void* cuda_stream, int n, int n_o, const float* A, const float* b, const float* z_des,
+                   const float* w, float rho, const float* z_lo, const float* z_hi, float* z_out,
+                   int device_ptrs) {
+  if (n < 0 || n_o < 1 || n_o > BRMPPI_PROJECT_MAX_NO || (device_ptrs != 0 && device_ptrs != 1))
+    return BRMPPI_ERR_INVALID_ARG;
+  if (!w || !z_lo || !z_hi) return BRMPPI_ERR_NULL;
+  const int d = n_o + 2;
+  if (!finite_all(w, d) || !finite_all(z_lo, d) || !finite_all(z_hi, d) || !std::isfinite(rho) || rho < 0.f)
+    return BRMPPI_ERR_INVALID_ARG;
+  ProjConst pc;
+  memset(&pc, 0, sizeof(pc));
+  for (int j = 0; j < d; ++j) {
+    if (!(w[j] > 0.f)) return BRMPPI_ERR_INVALID_ARG;
+    pc.w[j] = w[j]; pc.lo[j] = z_lo[j]; pc.hi[j] = z_hi[j];
+  }
+  pc.rho = rho;
+  if (n == 0) return BRMPPI_OK;
+  if (!A || !b || !z_des || !z_out) return BRMPPI_ERR_NULL;
+  cudaStream_t s = (cudaStream_t)cuda_stream;
+  if (device_ptrs) {
+    CU(launch_project_dyn(n_o, n, A, b, z_des, pc, z_out, s));
+    return BRMPPI_OK;
+  }
+  const size_t N = (size_t)n, nA = N * n_o * d, nb = N * n_o, nz = N * d;
+  float* buf = nullptr;
+  CU(cudaMalloc((void**)&buf, sizeof(float) * (nA + nb + 2 * nz + 12)));
+  // sections kept 16-byte aligned
+  auto up4 = [](size_t x) { return (x + 3) & ~(size_t)3; };
+  float* dA = buf;
+  float* db = dA + up4(nA);
+  float* dz = db + up4(nb);
+  float* dout = dz + up4(nz);
+  cudaError_t e = cudaMemcpyAsync(dA, A, sizeof(float) * nA, cudaMemcpyHostToDevice, s);
+  if (e == cudaSuccess) e = cudaMemcpyAsync(db, b, sizeof(float) * nb, cudaMemcpyHostToDevice, s);
+  if (e == cudaSuccess) e = cudaMemcpyAsync(dz, z_des, sizeof(float) * nz, cudaMemcpyHostToDevice, s);
+  if (e == cudaSuccess) e = launch_project_dyn(n_o, n, dA, db, dz, pc, dout, s);
+  if (e == cudaSuccess) e = cudaMemcpyAsync(z_out, dout, sizeof(float) * nz, cudaMemcpyDeviceToHost, s);
   if (e == cudaSuccess) e = cudaStreamSynchronize(s);
   cudaFree(buf);
   if (e != cudaSuccess) return cuda_fail(e);

@@ -1,0 +1,102 @@
+"""Parity of brmppi_project (eq. (11)-(12)) through the C ABI against oracle/projection.py
+on the same seeded (9)-shaped problems.
+
+Tolerance (derived): fp32 Cholesky solves S nu = r with relative error ~ cond(S) eps_32; the
+recipe's S = A M^-1 A^T has cond(S) <= ~2e3, so |z - z_ref| <= 1e-4 max(|z_ref|, 1) holds with a margin of
+about two; a problem is compared at 1e-4 * max(1, cond(S) / 1e3).  The equality constraint itself is
+checked in fp64 on the fp32 result: |A z - b| <= 2e-5 (1 + |A| |z|)."""
+import numpy as np
+import pytest
+
+from scenes.projection import projection_batch
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def B():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("GPU tests need a CUDA device; there is no CPU fallback")
+    from paper_2508_05773_b200 import brmppi
+    brmppi.lib()
+    return brmppi
+
+
+@pytest.fixture(scope="module")
+def OP():
+    from oracle import projection
+    return projection
+
+
+def check(OP, z, P, idx):
+    Minv = 1.0 / (P["w"] + P["rho"])
+    worst = 0.0
+    for i in idx:
+        ref = OP.project(P["A"][i], P["b"][i], P["z_des"][i], P["w"], P["rho"], P["z_lo"], P["z_hi"])
+        cond = np.linalg.cond((P["A"][i] * Minv[None, :]) @ P["A"][i].T)
+        tol = 1e-4 * max(1.0, cond / 1e3)
+        zi = z[i].astype(np.float64)
+        err = np.abs(zi - ref) / np.maximum(np.abs(ref), 1.0)
+        assert err.max() <= tol, (i, err.max(), cond)
+        worst = max(worst, err.max() / tol)
+        res = np.abs(P["A"][i] @ zi - P["b"][i])
+        assert np.all(res <= 2e-5 * (1.0 + np.abs(P["A"][i]) @ np.abs(zi))), (i, res)
+    return worst
+
+
+@pytest.mark.parametrize("n_o", [1, 2, 3, 4, 5, 6, 7, 8])
+@pytest.mark.parametrize("n", [1, 127, 129, 1000])
+def test_host_pointers_match_oracle(B, OP, n_o, n):
+    P = projection_batch(1000 * n_o + n, n, n_o, dense=(n % 2 == 0))
+    z = B.project(P["A"], P["b"], P["z_des"], P["w"], P["rho"], P["z_lo"], P["z_hi"])
+    assert z.shape == (n, n_o + 2) and np.isfinite(z).all()
+    check(OP, z, P, range(n))
+
+
+def test_device_pointers_full_size_sampled(B, OP):
+    """The paper's per-solve count: 5000 rollouts x 120 steps = 600 000 projections with eight obstacles
+    (PAPER.md:243), device-resident, sampled rows against the oracle; host- and device-pointer calls agree
+    bit for bit."""
+    import torch
+    n, n_o = 600_000, 8
+    P = projection_batch(7, n, n_o)
+    dev = lambda a: torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).cuda()
+    z = B.project(dev(P["A"]), dev(P["b"]), dev(P["z_des"]), P["w"], P["rho"], P["z_lo"], P["z_hi"])
+    torch.cuda.synchronize()
+    z = z.cpu().numpy()
+    assert np.isfinite(z).all()
+    idx = np.concatenate([[0, 1, 127, 128, n - 129, n - 128, n - 1], np.random.default_rng(0).integers(0, n, 300)])
+    check(OP, z, P, idx)
+    sl = slice(n - 1000, n)
+    z_host = B.project(P["A"][sl], P["b"][sl], P["z_des"][sl], P["w"], P["rho"], P["z_lo"], P["z_hi"])
+    # same arithmetic per problem whatever its position in the CTA
+    assert np.array_equal(z_host, z[sl])
+
+
+def test_rho_zero_and_large(B, OP):
+    P = projection_batch(5, 256, 4)
+    for rho in (0.0, 50.0):
+        P["rho"] = rho
+        z = B.project(P["A"], P["b"], P["z_des"], P["w"], rho, P["z_lo"], P["z_hi"])
+        check(OP, z, P, range(256))
+
+
+def test_edge_cases_and_errors(B):
+    P = projection_batch(1, 4, 3)
+    z = B.project(P["A"][:0], P["b"][:0], P["z_des"][:0], P["w"], P["rho"], P["z_lo"], P["z_hi"])   # n = 0
+    assert z.shape == (0, 5)
+    # a rank-deficient problem (two equal rows) spoils its own row only
+    A = P["A"].copy()
+    A[2, 1] = A[2, 0]
+    z = B.project(A, P["b"], P["z_des"], P["w"], P["rho"], P["z_lo"], P["z_hi"])
+    z_ok = B.project(P["A"], P["b"], P["z_des"], P["w"], P["rho"], P["z_lo"], P["z_hi"])
+    assert np.array_equal(z[[0, 1, 3]], z_ok[[0, 1, 3]])
+    with pytest.raises(B.BrmppiError):
+        B.project(np.zeros((2, 9, 11)), np.zeros((2, 9)), np.zeros((2, 11)), np.ones(11), 0.1, -np.ones(11), np.ones(11))
+    w_bad = P["w"].copy()
+    w_bad[1] = 0.0
+    with pytest.raises(B.BrmppiError):
+        B.project(P["A"], P["b"], P["z_des"], w_bad, P["rho"], P["z_lo"], P["z_hi"])
+    with pytest.raises(B.BrmppiError):
+        B.project(P["A"], P["b"], P["z_des"], P["w"], -1.0, P["z_lo"], P["z_hi"])
