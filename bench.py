@@ -399,6 +399,58 @@ def run_sweep(args):
     point("batch64", batch, batch[0].params.with_(seed=0), 64)
 
 
+def run_project(args):
+    """The closed-form projection (12) on its own (brmppi_project, NEXT row 1's kernel): the paper's per-solve
+    count, 5000 rollouts x 120 steps = 600 000 problems with N_o = 8, device-resident, L2
+    flushed between timed launches; one JSON line with the HBM roofline, the oracle beside it."""
+    import time
+    import numpy as np
+    import torch
+    from paper_2508_05773_b200 import brmppi as B
+    from scenes.projection import projection_batch
+    n, n_o = 600_000, 8
+    d = n_o + 2
+    P = projection_batch(7, n, n_o)
+    dev = lambda a: torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).cuda()
+    A, b, zd = dev(P["A"]), dev(P["b"]), dev(P["z_des"])
+    call = lambda: B.project(A, b, zd, P["w"], P["rho"], P["z_lo"], P["z_hi"])
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+    for _ in range(max(args.warmup, 3)):
+        call()
+    ms = []
+    for _ in range(args.steps):
+        flush.fill_(1)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        call()
+        e1.record()
+        torch.cuda.synchronize()
+        ms.append(e0.elapsed_time(e1))
+    t = float(np.mean(ms)) * 1e-3
+    bytes_alg = n * 4 * (n_o * d + n_o + 2 * d)          # A, b, z_des in; z out
+    mp = measured_peaks()
+    peak = float(mp.get("hbm_gbs", 6500.0))
+    from oracle import projection as OP
+    m = 20000
+    t0 = time.perf_counter()
+    for i in range(m):
+        OP.project(P["A"][i], P["b"][i], P["z_des"][i], P["w"], P["rho"], P["z_lo"], P["z_hi"])
+    t_cpu = time.perf_counter() - t0
+    print(json.dumps({
+        "metric": "brmppi_projections_per_s", "value": n / t, "unit": "projections/s", "n_gpus": 1,
+        "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": t * 1e3, "higher_is_better": True,
+        "dtype": "f32", "data": "synthetic",
+        "config": {"workload": "eq. (12), 5000 x 120 problems, N_o = 8 (PAPER.md:243)", "n": n, "n_o": n_o,
+                   "l2": "flushed between timed launches (256 MiB write)"},
+        "gpu_launches": args.steps,
+        "roofline": {"bound": "hbm", "achieved": bytes_alg / t / 1e9, "peak": peak, "unit": "GB/s",
+                     "frac": bytes_alg / t / 1e9 / peak, "traffic": None, "kernel": "project_batch_bulk<8> (persistent; its last CTA takes the 64-problem tail)",
+                     "algorithmic_bytes_per_problem": bytes_alg // n,
+                     "peak_basis": "MEASURED_PEAKS.json hbm_gbs" if "hbm_gbs" in mp else "fallback 6500 GB/s"},
+        "cpu_baseline": {"value": m / t_cpu, "unit": "projections/s", "cores": 1, "kind": "oracle",
+                         "sample": f"first {m} of the {n} problems, oracle/projection.py"}}))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -408,8 +460,11 @@ def main():
     ap.add_argument("--workload", default="cfg2", choices=["cfg0", "cfg1", "cfg2", "cfg2se", "cfg3"])
     ap.add_argument("--phases", action="store_true", help="print the rollout kernel's in-kernel phase times")
     ap.add_argument("--sweep", action="store_true", help="run BASELINE.json configs[4] (sweep + 64-scene batch)")
+    ap.add_argument("--project", action="store_true", help="time the closed-form projection (12) on its own")
     args = ap.parse_args()
-    if args.phases:
+    if args.project:
+        run_project(args)
+    elif args.phases:
         run_phases(args)
     elif args.sweep:
         run_sweep(args)

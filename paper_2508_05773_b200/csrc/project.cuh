@@ -33,27 +33,26 @@ struct ProjSmem {
 // Copy `rows` rows of `len` contiguous words from global (rows back to back) to shared rows of `stride`.
 __device__ __forceinline__ void proj_stage_in(float* dst, const float* __restrict__ src, int rows, int len, int stride) {
   const int total = rows * len;
+#pragma unroll 8
   for (int i = threadIdx.x; i < total; i += kProjBlock) {
     const int r = i / len, c = i - r * len;
     dst[r * stride + c] = __ldg(src + i);
   }
 }
 
+// `rows` (<= 128) problems starting at problem `first`, by the whole CTA, through `smem` (ProjSmem<NO>::words).
 template <int NO>
-__global__ void __launch_bounds__(kProjBlock) project_batch(int n, const float* __restrict__ A, const float* __restrict__ b,
-                                                            const float* __restrict__ z_des,
-                                                            const __grid_constant__ ProjConst C, float* __restrict__ z_out) {
+__device__ __forceinline__ void project_block_generic(float* smem, size_t first, int rows, const float* __restrict__ A,
+                                                      const float* __restrict__ b, const float* __restrict__ z_des,
+                                                      const ProjConst& C, float* __restrict__ z_out) {
   using SM = ProjSmem<NO>;
   constexpr int D = SM::D;
-  extern __shared__ float smem[];
   float* sA = smem;
   float* sB = sA + kProjBlock * SM::strideA;
   float* sZ = sB + kProjBlock * SM::strideB;
-  const int first = blockIdx.x * kProjBlock;
-  const int rows = min(kProjBlock, n - first);
-  proj_stage_in(sA, A + (size_t)first * (NO * D), rows, NO * D, SM::strideA);
-  proj_stage_in(sB, b + (size_t)first * NO, rows, NO, SM::strideB);
-  proj_stage_in(sZ, z_des + (size_t)first * D, rows, D, SM::strideZ);
+  proj_stage_in(sA, A + first * (NO * D), rows, NO * D, SM::strideA);
+  proj_stage_in(sB, b + first * NO, rows, NO, SM::strideB);
+  proj_stage_in(sZ, z_des + first * D, rows, D, SM::strideZ);
   __syncthreads();
   const int t = threadIdx.x;
   if (t < rows) {
@@ -124,11 +123,21 @@ __global__ void __launch_bounds__(kProjBlock) project_batch(int n, const float* 
   }
   __syncthreads();
   const int total = rows * D;
-  float* out = z_out + (size_t)first * D;
+  float* out = z_out + first * D;
+#pragma unroll 4
   for (int i = threadIdx.x; i < total; i += kProjBlock) {
     const int r = i / D, c = i - r * D;
     out[i] = sZ[r * SM::strideZ + c];
   }
+}
+
+template <int NO>
+__global__ void __launch_bounds__(kProjBlock) project_batch(int n, const float* __restrict__ A, const float* __restrict__ b,
+                                                            const float* __restrict__ z_des,
+                                                            const __grid_constant__ ProjConst C, float* __restrict__ z_out) {
+  extern __shared__ float smem[];
+  const size_t first = (size_t)blockIdx.x * kProjBlock;
+  project_block_generic<NO>(smem, first, min(kProjBlock, n - (int)first), A, b, z_des, C, z_out);
 }
 
 
@@ -148,13 +157,45 @@ struct ProjBulkSmem {
   static constexpr int strideA = ((rowA / 4) | 1) * 4;      // odd number of 16-byte slots
   static constexpr int offB = kProjBlock * strideA;         // words
   static constexpr int offZ = offB + kProjBlock * NO;
-  static constexpr int offBar = offZ + kProjBlock * D;      // 8-byte aligned: all terms are even
-  static constexpr int bytes = (offBar + 2) * 4;
+  static constexpr int offOut = (offZ + kProjBlock * D + 31) & ~31;   // two z-out buffers, 128-byte aligned
+  static constexpr int outWords = (kProjBlock * D + 31) & ~31;
+  static constexpr int offBar = offOut + 2 * outWords;      // one mbarrier
+  static constexpr int bulk_words = offBar + 2;
+  static constexpr int words = bulk_words > ProjSmem<NO>::words ? bulk_words : ProjSmem<NO>::words;
+  static constexpr int bytes = words * 4;
   static constexpr unsigned tx = kProjBlock * (rowA + NO + D) * 4;
 };
 
+// Loads of one full block into one stage; called by every thread (thread t copies row t of A).
 template <int NO>
-__global__ void __launch_bounds__(kProjBlock) project_batch_bulk(const float* __restrict__ A, const float* __restrict__ b,
+__device__ __forceinline__ void proj_issue_loads(float* st, uint32_t bar, size_t first, const float* __restrict__ A,
+                                                 const float* __restrict__ b, const float* __restrict__ z_des) {
+  using SM = ProjBulkSmem<NO>;
+  const int t = threadIdx.x;
+  if (t == 0)
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(SM::tx) : "memory");
+  __syncwarp();
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+               ::"r"(proj_smem_u32(st + t * SM::strideA)), "l"(A + (first + t) * SM::rowA), "r"(SM::rowA * 4), "r"(bar)
+               : "memory");
+  if (t == 0) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(proj_smem_u32(st + SM::offB)), "l"(b + first * NO), "r"(kProjBlock * NO * 4), "r"(bar) : "memory");
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(proj_smem_u32(st + SM::offZ)), "l"(z_des + first * SM::D), "r"(kProjBlock * SM::D * 4), "r"(bar)
+                 : "memory");
+  }
+}
+
+// Persistent: CTA c of the first gridDim.x - 1 takes the full blocks c, c + P, c + 2P, ... (P = gridDim.x - 1).
+// A thread keeps its whole problem in registers, so the load stage is free again as soon as every thread has
+// read its rows: the loads of the CTA's next block are issued right then and are in flight during the whole
+// computation of the current one (one stage of 52 KB instead of two -> three CTAs per SM at N_o = 8).  z goes
+// out through two small buffers so that a bulk store may still be reading one while the next is written.
+// The last CTA takes the ragged tail (n_tail < 128 problems) through the generic path.
+template <int NO>
+__global__ void __launch_bounds__(kProjBlock) project_batch_bulk(int full_blocks, int n_tail, const float* __restrict__ A,
+                                                                 const float* __restrict__ b,
                                                                  const float* __restrict__ z_des,
                                                                  const __grid_constant__ ProjConst C,
                                                                  float* __restrict__ z_out) {
@@ -163,110 +204,120 @@ __global__ void __launch_bounds__(kProjBlock) project_batch_bulk(const float* __
   constexpr int D = SM::D;
   extern __shared__ __align__(128) float smem[];
   const int t = threadIdx.x;
-  const size_t first = (size_t)blockIdx.x * kProjBlock;
-  const uint32_t bar = proj_smem_u32(smem + SM::offBar);
+  const int P = (int)gridDim.x - 1;
+  if ((int)blockIdx.x == P) {
+    if (n_tail > 0)
+      project_block_generic<NO>(smem, (size_t)full_blocks * kProjBlock, n_tail, A, b, z_des, C, z_out);
+    return;
+  }
+  const uint32_t bar0 = proj_smem_u32(smem + SM::offBar);
   if (t == 0) {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(bar));
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(bar0));
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(SM::tx) : "memory");
   }
   __syncthreads();
-  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
-               ::"r"(proj_smem_u32(smem + t * SM::strideA)), "l"(A + (first + t) * SM::rowA), "r"(SM::rowA * 4), "r"(bar)
-               : "memory");
-  if (t == 0) {
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
-                 ::"r"(proj_smem_u32(smem + SM::offB)), "l"(b + first * NO), "r"(kProjBlock * NO * 4), "r"(bar) : "memory");
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
-                 ::"r"(proj_smem_u32(smem + SM::offZ)), "l"(z_des + first * D), "r"(kProjBlock * D * 4), "r"(bar) : "memory");
-  }
-  {
-    uint32_t done = 0;
-    while (!done)
-      asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], 0; selp.u32 %0, 1, 0, p; }"
-                   : "=r"(done) : "r"(bar) : "memory");
-  }
-  float minv[D], y[D], a[NO][D];
-  float* zrow = smem + SM::offZ + t * D;
+  int blk = blockIdx.x;
+  if (blk < full_blocks) proj_issue_loads<NO>(smem, bar0, (size_t)blk * kProjBlock, A, b, z_des);
+  float* const st = smem;
+  for (int it = 0; blk < full_blocks; ++it, blk += P) {
+    {
+      const uint32_t parity = (uint32_t)it & 1u;
+      uint32_t done = 0;
+      while (!done)
+        asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }"
+                     : "=r"(done) : "r"(bar0), "r"(parity) : "memory");
+    }
+    float minv[D], y[D], a[NO][D];
+    const float* zrow = st + SM::offZ + t * D;
+    float* const orow = smem + SM::offOut + (it & 1) * SM::outWords + t * D;
 #pragma unroll
-  for (int j = 0; j < D; j += 2) {
-    const float2 zd = *reinterpret_cast<const float2*>(zrow + j);
-    minv[j] = 1.0f / (C.w[j] + C.rho);
-    minv[j + 1] = 1.0f / (C.w[j + 1] + C.rho);
-    y[j] = fmaf(C.w[j], zd.x, 0.5f * C.rho * (C.hi[j] + C.lo[j])) * minv[j];
-    y[j + 1] = fmaf(C.w[j + 1], zd.y, 0.5f * C.rho * (C.hi[j + 1] + C.lo[j + 1])) * minv[j + 1];
-  }
-#pragma unroll
-  for (int q = 0; q < SM::rowA / 4; ++q) {
-    const float4 v = *reinterpret_cast<const float4*>(smem + t * SM::strideA + 4 * q);
-    a[(4 * q) / D][(4 * q) % D] = v.x;
-    a[(4 * q + 1) / D][(4 * q + 1) % D] = v.y;
-    a[(4 * q + 2) / D][(4 * q + 2) % D] = v.z;
-    a[(4 * q + 3) / D][(4 * q + 3) % D] = v.w;
-  }
-  float nu[NO];
-#pragma unroll
-  for (int i = 0; i < NO; i += 2) {
-    const float2 bb = *reinterpret_cast<const float2*>(smem + SM::offB + t * NO + i);
-    float a0 = -bb.x, a1 = -bb.y;
-#pragma unroll
-    for (int j = 0; j < D; ++j) { a0 = fmaf(a[i][j], y[j], a0); a1 = fmaf(a[i + 1][j], y[j], a1); }
-    nu[i] = a0; nu[i + 1] = a1;
-  }
-  float S[NO][NO];
-#pragma unroll
-  for (int i = 0; i < NO; ++i)
-#pragma unroll
-    for (int k = 0; k <= i; ++k) {
-      float acc = 0.0f;
-#pragma unroll
-      for (int j = 0; j < D; ++j) acc = fmaf(a[i][j] * minv[j], a[k][j], acc);
-      S[i][k] = acc;
+    for (int j = 0; j < D; j += 2) {
+      const float2 zd = *reinterpret_cast<const float2*>(zrow + j);
+      minv[j] = 1.0f / (C.w[j] + C.rho);
+      minv[j + 1] = 1.0f / (C.w[j + 1] + C.rho);
+      y[j] = fmaf(C.w[j], zd.x, 0.5f * C.rho * (C.hi[j] + C.lo[j])) * minv[j];
+      y[j + 1] = fmaf(C.w[j + 1], zd.y, 0.5f * C.rho * (C.hi[j + 1] + C.lo[j + 1])) * minv[j + 1];
     }
 #pragma unroll
-  for (int k = 0; k < NO; ++k) {
-    float dkk = S[k][k];
+    for (int q = 0; q < SM::rowA / 4; ++q) {
+      const float4 v = *reinterpret_cast<const float4*>(st + t * SM::strideA + 4 * q);
+      a[(4 * q) / D][(4 * q) % D] = v.x;
+      a[(4 * q + 1) / D][(4 * q + 1) % D] = v.y;
+      a[(4 * q + 2) / D][(4 * q + 2) % D] = v.z;
+      a[(4 * q + 3) / D][(4 * q + 3) % D] = v.w;
+    }
+    float nu[NO];
 #pragma unroll
-    for (int m = 0; m < k; ++m) dkk = fmaf(-S[k][m], S[k][m], dkk);
-    const float inv = rsqrtf(dkk);
-    S[k][k] = inv;
+    for (int i = 0; i < NO; i += 2) {
+      const float2 bb = *reinterpret_cast<const float2*>(st + SM::offB + t * NO + i);
+      nu[i] = -bb.x; nu[i + 1] = -bb.y;
+    }
+    // every thread holds its problem in registers: hand the stage back and start the next block's loads; the
+    // z-out buffer written below was last read by the bulk store of iteration it - 2
+    if (t == 0) asm volatile("cp.async.bulk.wait_group.read 1;" ::: "memory");
+    __syncthreads();
+    if (blk + P < full_blocks) proj_issue_loads<NO>(smem, bar0, (size_t)(blk + P) * kProjBlock, A, b, z_des);
 #pragma unroll
-    for (int i = k + 1; i < NO; ++i) {
-      float v = S[i][k];
+    for (int i = 0; i < NO; ++i)
 #pragma unroll
-      for (int m = 0; m < k; ++m) v = fmaf(-S[i][m], S[k][m], v);
-      S[i][k] = v * inv;
+      for (int j = 0; j < D; ++j) nu[i] = fmaf(a[i][j], y[j], nu[i]);
+    float S[NO][NO];
+#pragma unroll
+    for (int i = 0; i < NO; ++i)
+#pragma unroll
+      for (int k = 0; k <= i; ++k) {
+        float acc = 0.0f;
+#pragma unroll
+        for (int j = 0; j < D; ++j) acc = fmaf(a[i][j] * minv[j], a[k][j], acc);
+        S[i][k] = acc;
+      }
+#pragma unroll
+    for (int k = 0; k < NO; ++k) {
+      float dkk = S[k][k];
+#pragma unroll
+      for (int m = 0; m < k; ++m) dkk = fmaf(-S[k][m], S[k][m], dkk);
+      const float inv = rsqrtf(dkk);
+      S[k][k] = inv;
+#pragma unroll
+      for (int i = k + 1; i < NO; ++i) {
+        float v = S[i][k];
+#pragma unroll
+        for (int m = 0; m < k; ++m) v = fmaf(-S[i][m], S[k][m], v);
+        S[i][k] = v * inv;
+      }
+    }
+#pragma unroll
+    for (int i = 0; i < NO; ++i) {
+      float v = nu[i];
+#pragma unroll
+      for (int m = 0; m < i; ++m) v = fmaf(-S[i][m], nu[m], v);
+      nu[i] = v * S[i][i];
+    }
+#pragma unroll
+    for (int i = NO - 1; i >= 0; --i) {
+      float v = nu[i];
+#pragma unroll
+      for (int m = i + 1; m < NO; ++m) v = fmaf(-S[m][i], nu[m], v);
+      nu[i] = v * S[i][i];
+    }
+#pragma unroll
+    for (int j = 0; j < D; j += 2) {
+      float c0 = 0.0f, c1 = 0.0f;
+#pragma unroll
+      for (int i = 0; i < NO; ++i) { c0 = fmaf(a[i][j], nu[i], c0); c1 = fmaf(a[i][j + 1], nu[i], c1); }
+      *reinterpret_cast<float2*>(orow + j) = make_float2(fmaf(-minv[j], c0, y[j]), fmaf(-minv[j + 1], c1, y[j + 1]));
+    }
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // generic-proxy writes -> visible to the bulk store
+    __syncthreads();
+    if (t == 0) {
+      asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;"
+                   ::"l"(z_out + (size_t)blk * kProjBlock * D),
+                     "r"(proj_smem_u32(smem + SM::offOut + (it & 1) * SM::outWords)), "r"(kProjBlock * D * 4)
+                   : "memory");
+      asm volatile("cp.async.bulk.commit_group;" ::: "memory");
     }
   }
-#pragma unroll
-  for (int i = 0; i < NO; ++i) {
-    float v = nu[i];
-#pragma unroll
-    for (int m = 0; m < i; ++m) v = fmaf(-S[i][m], nu[m], v);
-    nu[i] = v * S[i][i];
-  }
-#pragma unroll
-  for (int i = NO - 1; i >= 0; --i) {
-    float v = nu[i];
-#pragma unroll
-    for (int m = i + 1; m < NO; ++m) v = fmaf(-S[m][i], nu[m], v);
-    nu[i] = v * S[i][i];
-  }
-#pragma unroll
-  for (int j = 0; j < D; j += 2) {
-    float c0 = 0.0f, c1 = 0.0f;
-#pragma unroll
-    for (int i = 0; i < NO; ++i) { c0 = fmaf(a[i][j], nu[i], c0); c1 = fmaf(a[i][j + 1], nu[i], c1); }
-    *reinterpret_cast<float2*>(zrow + j) = make_float2(fmaf(-minv[j], c0, y[j]), fmaf(-minv[j + 1], c1, y[j + 1]));
-  }
-  asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // generic-proxy writes -> visible to the bulk store
-  __syncthreads();
-  if (t == 0) {
-    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;"
-                 ::"l"(z_out + first * D), "r"(proj_smem_u32(smem + SM::offZ)), "r"(kProjBlock * D * 4) : "memory");
-    asm volatile("cp.async.bulk.commit_group;" ::: "memory");
-    asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
-  }
+  if (t == 0) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");   // smem must outlive the last store's read
 }
 
 template <int NO>
@@ -281,15 +332,21 @@ inline cudaError_t launch_project(int n, const float* A, const float* b, const f
     const bool aligned = (((uintptr_t)A | (uintptr_t)b | (uintptr_t)z_des | (uintptr_t)z_out) & 15u) == 0;
     if (full > 0 && aligned) {
       using SMB = ProjBulkSmem<NO>;
-      e = cudaFuncSetAttribute(project_batch_bulk<NO>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMB::bytes);
-      if (e != cudaSuccess) return e;
-      project_batch_bulk<NO><<<(unsigned)full, kProjBlock, SMB::bytes, s>>>(A, b, z_des, C, z_out);
-      e = cudaGetLastError();
-      if (e != cudaSuccess) return e;
-      const size_t done = (size_t)full * kProjBlock;
-      n -= (int)done;
-      if (n == 0) return cudaSuccess;
-      A += done * NO * D; b += done * NO; z_des += done * D; z_out += done * D;
+      static int persistent_ctas = 0;        // resident CTAs of this kernel on the current device
+      if (persistent_ctas == 0) {
+        e = cudaFuncSetAttribute(project_batch_bulk<NO>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMB::bytes);
+        if (e != cudaSuccess) return e;
+        int dev = 0, sms = 0, per_sm = 0;
+        if ((e = cudaGetDevice(&dev)) != cudaSuccess) return e;
+        if ((e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return e;
+        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, project_batch_bulk<NO>, kProjBlock, SMB::bytes);
+        if (e != cudaSuccess) return e;
+        persistent_ctas = sms * (per_sm > 0 ? per_sm : 1);
+      }
+      // P persistent CTAs for the full blocks + one CTA for the ragged tail, all resident in one wave
+      const int P = full < persistent_ctas - 1 ? full : persistent_ctas - 1;
+      project_batch_bulk<NO><<<(unsigned)(P + 1), kProjBlock, SMB::bytes, s>>>(full, n - full * kProjBlock, A, b, z_des, C, z_out);
+      return cudaGetLastError();
     }
   }
   const size_t bytes = sizeof(float) * ProjSmem<NO>::words;
