@@ -323,7 +323,7 @@ __global__ void __launch_bounds__(kProjBlock) project_batch_bulk(int full_blocks
 template <int NO>
 inline cudaError_t launch_project(int n, const float* A, const float* b, const float* z_des, const ProjConst& C,
                                   float* z_out, cudaStream_t s) {
-  constexpr int D = NO + 2;
+  [[maybe_unused]] constexpr int D = NO + 2;
   cudaError_t e;
   if constexpr (NO % 2 == 0) {
     // full 128-problem blocks through the bulk-copy kernel (needs 16-byte aligned arrays), the tail through
