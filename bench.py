@@ -430,6 +430,14 @@ def run_project(args):
     bytes_alg = n * 4 * (n_o * d + n_o + 2 * d)          # A, b, z_des in; z out
     mp = measured_peaks()
     peak = float(mp.get("hbm_gbs", 6500.0))
+    # end to end through the C ABI with HOST buffers: the call copies A, b, z_des in and z out itself
+    hA, hb, hz = (np.ascontiguousarray(P[k], dtype=np.float32) for k in ("A", "b", "z_des"))
+    B.project(hA, hb, hz, P["w"], P["rho"], P["z_lo"], P["z_hi"])
+    reps = 3
+    t0 = time.perf_counter()
+    for _ in range(reps):
+        B.project(hA, hb, hz, P["w"], P["rho"], P["z_lo"], P["z_hi"])
+    t_e2e = (time.perf_counter() - t0) / reps
     from oracle import projection as OP
     m = 20000
     t0 = time.perf_counter()
@@ -443,6 +451,9 @@ def run_project(args):
         "config": {"workload": "eq. (12), 5000 x 120 problems, N_o = 8 (PAPER.md:243)", "n": n, "n_o": n_o,
                    "l2": "flushed between timed launches (256 MiB write)"},
         "gpu_launches": args.steps,
+        "e2e": {"value": n / t_e2e, "unit": "projections/s", "h2d_bytes_per_step": int(hA.nbytes + hb.nbytes + hz.nbytes),
+                "d2h_bytes_per_step": int(hz.nbytes), "what": "brmppi_project with host pointers (pageable numpy arrays; "
+                "the call allocates and frees its device scratch), host wall clock"},
         "roofline": {"bound": "hbm", "achieved": bytes_alg / t / 1e9, "peak": peak, "unit": "GB/s",
                      "frac": bytes_alg / t / 1e9 / peak, "traffic": None, "kernel": "project_batch_bulk<8> (persistent; its last CTA takes the 64-problem tail)",
                      "algorithmic_bytes_per_problem": bytes_alg // n,
