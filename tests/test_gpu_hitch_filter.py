@@ -159,3 +159,30 @@ def test_filter_off_is_unchanged(B):
     assert out[0][2] == 0 and out[1][2] == 0
     assert np.array_equal(out[0][0], out[1][0]) and np.array_equal(out[0][0], out[0][1])
     assert np.array_equal(out[0][3], out[1][3])
+
+
+def test_closed_loop_keeps_the_hitch_limit(B):
+    """PAPER.md:235 on the GPU path: 220 graph-replayed control steps of CFG3 from a nearly jackknifed start
+    with a hitch limit of 0.6 rad.  Without the stabiliser BR-MPPI's own control overshoots the limit; with it
+    the hitch angle stays within the linearisation remainder of reading 28 (tests/test_oracle_hitch_filter.py
+    derives the 0.02 rad)."""
+    sc = scenes.scene_cfg3(0)
+    worst = {}
+    for hf in (0, 1):
+        p = sc.params.with_(hitch_filter=hf, hitch_max=0.6, hitch_alpha=0.3)
+        s = B.Solver(p, 1, 8)
+        s.set_scene(sc)
+        x = sc.x0.copy()
+        x[3] = x[2] - 0.55
+        s.set_state(x)
+        w, active = 0.0, 0
+        for _ in range(220):
+            s.step()
+            st = s.get_state().astype(np.float64)
+            w = max(w, abs((st[2] - st[3] + np.pi) % (2 * np.pi) - np.pi))
+            active += s.get_hitch_filter()[1] == 1
+        worst[hf] = (w, active)
+        s.close()
+    assert worst[0][1] == 0 and worst[1][1] > 10
+    assert worst[1][0] <= 0.6 + 0.02
+    assert worst[0][0] > worst[1][0] + 0.03          # the unfiltered run does overshoot
