@@ -141,20 +141,23 @@ __global__ void __launch_bounds__(kProjBlock) project_batch(int n, const float* 
 }
 
 
-// ---- bulk-copy variant for even N_o (rows of A are multiples of 16 bytes) -----------------------
-// Full 128-problem blocks only.  Every thread issues one cp.async.bulk (TMA, 1-D) for its own row of A into
-// a shared row padded to an odd number of 16-byte slots, thread 0 two more for the CTA's b and z_des blocks;
-// all complete on one mbarrier.  No load passes through registers, no index arithmetic is issued for
-// staging, and a thread reads its row back with conflict-free LDS.128 (a quarter-warp's eight 16-byte
-// accesses fall on eight different slots mod 8 because the row stride is odd in slots).  z returns through
-// one bulk store of the CTA's contiguous z block.
+// ---- bulk-copy (TMA 1-D) kernel -----------------------------------------------------------------------
+// Full 128-problem blocks only.  The CTA's A, b and z_des blocks are contiguous in HBM and arrive by three
+// cp.async.bulk copies issued by one thread, all completing on one mbarrier: no load passes through
+// registers and no index arithmetic is issued for staging.  The A block lands unpadded.  For odd N_o a row is
+// an odd number of words, so thread t reading word j of row t is conflict-free with scalar LDS.  For even
+// N_o a row is a multiple of 16 bytes and is read with LDS.128; a quarter-warp's eight accesses then fall on
+// two to four distinct 16-byte slots mod 8 (2- to 4-way conflicts), which costs the same shared-memory
+// cycles as conflict-free scalar loads and is cheaper than what avoids it: one bulk copy per row into
+// padded rows ran 2-45 % slower (profiles/r1d_project.md), the TMA unit being the limit then.
+// z returns through one bulk store of the CTA's contiguous z block.
 __device__ __forceinline__ uint32_t proj_smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
 template <int NO>
 struct ProjBulkSmem {
   static constexpr int D = NO + 2;
   static constexpr int rowA = NO * D;                       // words, a multiple of 4 for even NO
-  static constexpr int strideA = ((rowA / 4) | 1) * 4;      // odd number of 16-byte slots
+  static constexpr int strideA = rowA;                      // the block lands unpadded, as it lies in HBM
   static constexpr int offB = kProjBlock * strideA;         // words
   static constexpr int offZ = offB + kProjBlock * NO;
   static constexpr int offOut = (offZ + kProjBlock * D + 31) & ~31;   // two z-out buffers, 128-byte aligned
@@ -166,7 +169,7 @@ struct ProjBulkSmem {
   static constexpr unsigned tx = kProjBlock * (rowA + NO + D) * 4;
 };
 
-// Loads of one full block into one stage; called by every thread (thread t copies row t of A).
+// Loads of one full block into the stage: three bulk copies (the CTA's A, b and z_des blocks are contiguous).
 template <int NO>
 __device__ __forceinline__ void proj_issue_loads(float* st, uint32_t bar, size_t first, const float* __restrict__ A,
                                                  const float* __restrict__ b, const float* __restrict__ z_des) {
@@ -174,11 +177,9 @@ __device__ __forceinline__ void proj_issue_loads(float* st, uint32_t bar, size_t
   const int t = threadIdx.x;
   if (t == 0)
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(SM::tx) : "memory");
-  __syncwarp();
-  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
-               ::"r"(proj_smem_u32(st + t * SM::strideA)), "l"(A + (first + t) * SM::rowA), "r"(SM::rowA * 4), "r"(bar)
-               : "memory");
   if (t == 0) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(proj_smem_u32(st)), "l"(A + first * SM::rowA), "r"(kProjBlock * SM::rowA * 4), "r"(bar) : "memory");
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
                  ::"r"(proj_smem_u32(st + SM::offB)), "l"(b + first * NO), "r"(kProjBlock * NO * 4), "r"(bar) : "memory");
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
@@ -199,7 +200,6 @@ __global__ void __launch_bounds__(kProjBlock) project_batch_bulk(int full_blocks
                                                                  const float* __restrict__ z_des,
                                                                  const __grid_constant__ ProjConst C,
                                                                  float* __restrict__ z_out) {
-  static_assert(NO % 2 == 0, "rows of A must be multiples of 16 bytes");
   using SM = ProjBulkSmem<NO>;
   constexpr int D = SM::D;
   extern __shared__ __align__(128) float smem[];
@@ -230,30 +230,50 @@ __global__ void __launch_bounds__(kProjBlock) project_batch_bulk(int full_blocks
     float minv[D], y[D], a[NO][D];
     const float* zrow = st + SM::offZ + t * D;
     float* const orow = smem + SM::offOut + (it & 1) * SM::outWords + t * D;
+    if constexpr (NO % 2 == 0) {
 #pragma unroll
-    for (int j = 0; j < D; j += 2) {
-      const float2 zd = *reinterpret_cast<const float2*>(zrow + j);
-      minv[j] = 1.0f / (C.w[j] + C.rho);
-      minv[j + 1] = 1.0f / (C.w[j + 1] + C.rho);
-      y[j] = fmaf(C.w[j], zd.x, 0.5f * C.rho * (C.hi[j] + C.lo[j])) * minv[j];
-      y[j + 1] = fmaf(C.w[j + 1], zd.y, 0.5f * C.rho * (C.hi[j + 1] + C.lo[j + 1])) * minv[j + 1];
-    }
+      for (int j = 0; j < D; j += 2) {
+        const float2 zd = *reinterpret_cast<const float2*>(zrow + j);
+        minv[j] = 1.0f / (C.w[j] + C.rho);
+        minv[j + 1] = 1.0f / (C.w[j + 1] + C.rho);
+        y[j] = fmaf(C.w[j], zd.x, 0.5f * C.rho * (C.hi[j] + C.lo[j])) * minv[j];
+        y[j + 1] = fmaf(C.w[j + 1], zd.y, 0.5f * C.rho * (C.hi[j + 1] + C.lo[j + 1])) * minv[j + 1];
+      }
 #pragma unroll
-    for (int q = 0; q < SM::rowA / 4; ++q) {
-      const float4 v = *reinterpret_cast<const float4*>(st + t * SM::strideA + 4 * q);
-      a[(4 * q) / D][(4 * q) % D] = v.x;
-      a[(4 * q + 1) / D][(4 * q + 1) % D] = v.y;
-      a[(4 * q + 2) / D][(4 * q + 2) % D] = v.z;
-      a[(4 * q + 3) / D][(4 * q + 3) % D] = v.w;
+      for (int q = 0; q < SM::rowA / 4; ++q) {
+        const float4 v = *reinterpret_cast<const float4*>(st + t * SM::strideA + 4 * q);
+        a[(4 * q) / D][(4 * q) % D] = v.x;
+        a[(4 * q + 1) / D][(4 * q + 1) % D] = v.y;
+        a[(4 * q + 2) / D][(4 * q + 2) % D] = v.z;
+        a[(4 * q + 3) / D][(4 * q + 3) % D] = v.w;
+      }
+    } else {
+#pragma unroll
+      for (int j = 0; j < D; ++j) {
+        minv[j] = 1.0f / (C.w[j] + C.rho);
+        y[j] = fmaf(C.w[j], zrow[j], 0.5f * C.rho * (C.hi[j] + C.lo[j])) * minv[j];
+      }
+#pragma unroll
+      for (int i = 0; i < NO; ++i)
+#pragma unroll
+        for (int j = 0; j < D; ++j) a[i][j] = st[t * SM::strideA + i * D + j];
     }
     float nu[NO];
+    if constexpr (NO % 2 == 0) {
 #pragma unroll
-    for (int i = 0; i < NO; i += 2) {
-      const float2 bb = *reinterpret_cast<const float2*>(st + SM::offB + t * NO + i);
-      nu[i] = -bb.x; nu[i + 1] = -bb.y;
+      for (int i = 0; i < NO; i += 2) {
+        const float2 bb = *reinterpret_cast<const float2*>(st + SM::offB + t * NO + i);
+        nu[i] = -bb.x; nu[i + 1] = -bb.y;
+      }
+    } else {
+#pragma unroll
+      for (int i = 0; i < NO; ++i) nu[i] = -st[SM::offB + t * NO + i];
     }
     // every thread holds its problem in registers: hand the stage back and start the next block's loads; the
     // z-out buffer written below was last read by the bulk store of iteration it - 2
+    // (the refill is an async-proxy write issued by another thread: bar.sync alone does not order this
+    // thread's shared loads, possibly still in flight, before it -- the proxy fence does)
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
     if (t == 0) asm volatile("cp.async.bulk.wait_group.read 1;" ::: "memory");
     __syncthreads();
     if (blk + P < full_blocks) proj_issue_loads<NO>(smem, bar0, (size_t)(blk + P) * kProjBlock, A, b, z_des);
@@ -300,12 +320,22 @@ __global__ void __launch_bounds__(kProjBlock) project_batch_bulk(int full_blocks
       for (int m = i + 1; m < NO; ++m) v = fmaf(-S[m][i], nu[m], v);
       nu[i] = v * S[i][i];
     }
+    if constexpr (NO % 2 == 0) {
 #pragma unroll
-    for (int j = 0; j < D; j += 2) {
-      float c0 = 0.0f, c1 = 0.0f;
+      for (int j = 0; j < D; j += 2) {
+        float c0 = 0.0f, c1 = 0.0f;
 #pragma unroll
-      for (int i = 0; i < NO; ++i) { c0 = fmaf(a[i][j], nu[i], c0); c1 = fmaf(a[i][j + 1], nu[i], c1); }
-      *reinterpret_cast<float2*>(orow + j) = make_float2(fmaf(-minv[j], c0, y[j]), fmaf(-minv[j + 1], c1, y[j + 1]));
+        for (int i = 0; i < NO; ++i) { c0 = fmaf(a[i][j], nu[i], c0); c1 = fmaf(a[i][j + 1], nu[i], c1); }
+        *reinterpret_cast<float2*>(orow + j) = make_float2(fmaf(-minv[j], c0, y[j]), fmaf(-minv[j + 1], c1, y[j + 1]));
+      }
+    } else {
+#pragma unroll
+      for (int j = 0; j < D; ++j) {
+        float c0 = 0.0f;
+#pragma unroll
+        for (int i = 0; i < NO; ++i) c0 = fmaf(a[i][j], nu[i], c0);
+        orow[j] = fmaf(-minv[j], c0, y[j]);
+      }
     }
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // generic-proxy writes -> visible to the bulk store
     __syncthreads();
@@ -325,11 +355,11 @@ inline cudaError_t launch_project(int n, const float* A, const float* b, const f
                                   float* z_out, cudaStream_t s) {
   [[maybe_unused]] constexpr int D = NO + 2;
   cudaError_t e;
-  if constexpr (NO % 2 == 0) {
+  {
     // full 128-problem blocks through the bulk-copy kernel (needs 16-byte aligned arrays), the tail through
     // the generic one
     const int full = n / kProjBlock;
-    const bool aligned = (((uintptr_t)A | (uintptr_t)b | (uintptr_t)z_des | (uintptr_t)z_out) & 15u) == 0;
+    const bool aligned = (((uintptr_t)A | (uintptr_t)b | (uintptr_t)z_des | (uintptr_t)z_out) & 15u) == 0;   // bulk copies
     if (full > 0 && aligned) {
       using SMB = ProjBulkSmem<NO>;
       static int persistent_ctas = 0;        // resident CTAs of this kernel on the current device

@@ -68,10 +68,31 @@ def test_device_pointers_full_size_sampled(B, OP):
     assert np.isfinite(z).all()
     idx = np.concatenate([[0, 1, 127, 128, n - 129, n - 128, n - 1], np.random.default_rng(0).integers(0, n, 300)])
     check(OP, z, P, idx)
-    sl = slice(n - 1000, n)
+    # A CTA of the big launch walks ~10 blocks through one shared-memory stage that is refilled while it
+    # computes; a launch of <= 443 blocks gives every CTA a single block.  Same arithmetic per problem, so
+    # windows of the big result must equal their own small launches bit for bit (this caught a missing
+    # proxy fence before the refill: rows of the next block overwrote loads still in flight).
+    for start_blk in (0, 1500, 4687 - 440):
+        sl = slice(start_blk * 128, (start_blk + 440) * 128)
+        z_win = B.project(P["A"][sl], P["b"][sl], P["z_des"][sl], P["w"], P["rho"], P["z_lo"], P["z_hi"])
+        assert np.array_equal(z_win, z[sl]), start_blk
+    sl = slice(n - 960, n)                       # 7 full blocks + the 64-problem tail in both launches
     z_host = B.project(P["A"][sl], P["b"][sl], P["z_des"][sl], P["w"], P["rho"], P["z_lo"], P["z_hi"])
-    # same arithmetic per problem whatever its position in the CTA
     assert np.array_equal(z_host, z[sl])
+
+
+@pytest.mark.parametrize("n_o", [3, 6, 7])
+def test_many_blocks_per_cta_other_sizes(B, OP, n_o):
+    """Odd N_o (scalar shared loads) and another even one through the persistent multi-block path."""
+    import torch
+    n = 128 * 3000 + 77
+    P = projection_batch(40 + n_o, n, n_o)
+    dev = lambda a: torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).cuda()
+    z = B.project(dev(P["A"]), dev(P["b"]), dev(P["z_des"]), P["w"], P["rho"], P["z_lo"], P["z_hi"]).cpu().numpy()
+    check(OP, z, P, np.concatenate([[0, 127, 128, n - 78, n - 77, n - 1], np.random.default_rng(1).integers(0, n, 150)]))
+    sl = slice(128 * 1000, 128 * 1400)
+    z_win = B.project(P["A"][sl], P["b"][sl], P["z_des"][sl], P["w"], P["rho"], P["z_lo"], P["z_hi"])
+    assert np.array_equal(z_win, z[sl])
 
 
 def test_rho_zero_and_large(B, OP):
