@@ -3,10 +3,12 @@
 // z = [u_proj (2), u_proj^alpha (N_o)], A is N_o x d with d = 2 + N_o, W diagonal.  One thread per problem
 // with everything in registers (N_o is a template parameter, all loops unroll): y = M^-1 p, r = A y - b,
 // S = A M^-1 A^T by its lower triangle, Cholesky S = L L^T in place, two triangular solves, z = y - M^-1 A^T nu.
-// A 128-thread CTA takes 128 consecutive problems; their A, b, z_des blocks are contiguous in HBM and are
-// staged through shared memory with coalesced 16-byte loads, rows padded to an odd stride so that thread
-// i reading word j of its own row hits bank (i * stride + j) mod 32 without conflict; z goes back the same
-// way.  432 B and ~1.5 kflop per problem at N_o = 8: HBM-bound.
+// A 128-thread CTA takes 128 consecutive problems, whose A, b, z_des blocks are contiguous in HBM.  Two paths:
+// project_batch_bulk (below; persistent CTAs, TMA bulk copies, every full block of a 16-byte aligned call)
+// and project_block_generic (coalesced LDG into odd-stride shared rows; the ragged tail and unaligned
+// pointers).  Both run the same arithmetic in the same order, so a problem's result does not depend on the
+// path or on its position.  432 B and ~1 k instructions per problem at N_o = 8: HBM-bound on paper
+// (DESIGN.md 6.9).
 #pragma once
 #include <cuda_runtime.h>
 #include <cstdint>
