@@ -341,11 +341,11 @@ def run_ours(args):
     print(json.dumps(line))
 
 
-def dram_traffic_from_profile():
-    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the rollout kernel, from the
-    committed ncu capture (profiles/r1_rollout_cta_dram.csv: header line, then bytes)."""
+def dram_traffic_from_profile(name="r1_rollout_cta_dram.csv"):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the
+    committed ncu capture (profiles/<name>: header line, then bytes)."""
     try:
-        rows = open(os.path.join(ROOT, "profiles", "r1_rollout_cta_dram.csv")).read().strip().splitlines()
+        rows = open(os.path.join(ROOT, "profiles", name)).read().strip().splitlines()
         return float(rows[-1].split(",")[-1])
     except Exception:
         return None
@@ -455,7 +455,7 @@ def run_project(args):
                 "d2h_bytes_per_step": int(hz.nbytes), "what": "brmppi_project with host pointers (pageable numpy arrays; "
                 "the call allocates and frees its device scratch), host wall clock"},
         "roofline": {"bound": "hbm", "achieved": bytes_alg / t / 1e9, "peak": peak, "unit": "GB/s",
-                     "frac": bytes_alg / t / 1e9 / peak, "traffic": None, "kernel": "project_batch_bulk<8> (persistent; its last CTA takes the 64-problem tail)",
+                     "frac": bytes_alg / t / 1e9 / peak, "traffic": dram_traffic_from_profile("r1d_project_dram.csv"), "kernel": "project_batch_bulk<8> (persistent; its last CTA takes the 64-problem tail)",
                      "algorithmic_bytes_per_problem": bytes_alg // n,
                      "peak_basis": "MEASURED_PEAKS.json hbm_gbs" if "hbm_gbs" in mp else "fallback 6500 GB/s"},
         "cpu_baseline": {"value": m / t_cpu, "unit": "projections/s", "cores": 1, "kind": "oracle",
