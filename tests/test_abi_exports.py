@@ -70,6 +70,45 @@ def test_host_only_calls(lib_path):
     assert lib.brmppi_create(None, None, 0, None, C.byref(ctx)) == brmppi.ERR_NULL
 
 
+def test_new_entry_points_validate_before_touching_cuda(lib_path):
+    """brmppi_project / brmppi_hitch_filter: argument errors and the n = 0 no-op are decided on the host."""
+    import numpy as np
+    import scenes
+    from paper_2508_05773_b200 import brmppi
+    lib = C.CDLL(lib_path)
+    fp = C.POINTER(C.c_float)
+    lib.brmppi_project.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, fp, C.c_float,
+                                   fp, fp, C.c_void_p, C.c_int]
+    ones = (C.c_float * 10)(*([1.0] * 10))
+    lo = (C.c_float * 10)(*([-1.0] * 10))
+    assert lib.brmppi_project(None, 0, 8, None, None, None, ones, 0.1, lo, ones, None, 0) == brmppi.OK       # n = 0
+    assert lib.brmppi_project(None, 0, 8, None, None, None, ones, 0.1, lo, ones, None, 1) == brmppi.OK
+    assert lib.brmppi_project(None, 4, 9, None, None, None, ones, 0.1, lo, ones, None, 0) == brmppi.ERR_INVALID_ARG
+    assert lib.brmppi_project(None, 4, 0, None, None, None, ones, 0.1, lo, ones, None, 0) == brmppi.ERR_INVALID_ARG
+    assert lib.brmppi_project(None, -1, 8, None, None, None, ones, 0.1, lo, ones, None, 0) == brmppi.ERR_INVALID_ARG
+    assert lib.brmppi_project(None, 4, 8, None, None, None, ones, -0.1, lo, ones, None, 0) == brmppi.ERR_INVALID_ARG
+    assert lib.brmppi_project(None, 4, 8, None, None, None, ones, 0.1, lo, ones, None, 2) == brmppi.ERR_INVALID_ARG
+    assert lib.brmppi_project(None, 4, 8, None, None, None, lo, 0.1, lo, ones, None, 0) == brmppi.ERR_INVALID_ARG   # w <= 0
+    assert lib.brmppi_project(None, 4, 8, None, None, None, None, 0.1, lo, ones, None, 0) == brmppi.ERR_NULL
+    assert lib.brmppi_project(None, 4, 8, None, None, None, ones, 0.1, lo, ones, None, 0) == brmppi.ERR_NULL        # A
+    lib.brmppi_hitch_filter.argtypes = [C.c_void_p, C.POINTER(brmppi.CParams), C.c_int, fp, fp, fp, C.POINTER(C.c_int)]
+    p = scenes.default_params()
+    good = brmppi.make_cparams(p, 1, 0, 0)
+    assert lib.brmppi_hitch_filter(None, C.byref(good), 0, None, None, None, None) == brmppi.OK                 # n = 0
+    assert lib.brmppi_hitch_filter(None, None, 0, None, None, None, None) == brmppi.ERR_NULL
+    assert lib.brmppi_hitch_filter(None, C.byref(good), -1, None, None, None, None) == brmppi.ERR_INVALID_ARG
+    assert lib.brmppi_hitch_filter(None, C.byref(good), 3, None, None, None, None) == brmppi.ERR_NULL
+    for kw in (dict(hitch_alpha=0.0), dict(hitch_alpha=1.1), dict(hitch_qv=0.0), dict(hitch_qdelta=-2.0), dict(dt=0.0)):
+        bad = brmppi.make_cparams(p.with_(**kw), 1, 0, 0)
+        assert lib.brmppi_hitch_filter(None, C.byref(bad), 0, None, None, None, None) == brmppi.ERR_INVALID_ARG, kw
+    # the stabiliser's parameters are validated by brmppi_create only when it is switched on
+    lib.brmppi_workspace_bytes.restype = C.c_size_t
+    lib.brmppi_workspace_bytes.argtypes = [C.POINTER(brmppi.CParams)]
+    assert lib.brmppi_workspace_bytes(C.byref(brmppi.make_cparams(p.with_(hitch_filter=0, hitch_alpha=0.0), 1, 8, 0))) > 0
+    assert lib.brmppi_workspace_bytes(C.byref(brmppi.make_cparams(p.with_(hitch_filter=1, hitch_alpha=0.0), 1, 8, 0))) == 0
+    assert lib.brmppi_workspace_bytes(C.byref(brmppi.make_cparams(p.with_(hitch_filter=2), 1, 8, 0))) == 0
+
+
 def test_no_cpu_fallback_without_a_device():
     import torch
     if torch.cuda.is_available():
