@@ -121,3 +121,18 @@ def test_edge_cases_and_errors(B):
         B.project(P["A"], P["b"], P["z_des"], w_bad, P["rho"], P["z_lo"], P["z_hi"])
     with pytest.raises(B.BrmppiError):
         B.project(P["A"], P["b"], P["z_des"], P["w"], -1.0, P["z_lo"], P["z_hi"])
+
+
+def test_unaligned_device_pointers_take_the_generic_path(B, OP):
+    """Views that start one problem into an odd-N_o batch are not 16-byte aligned (63, 7 and 9 words per
+    problem): no bulk copy is legal, the call falls back to the LDG kernel and must still be right."""
+    import torch
+    n, n_o = 700, 7
+    P = projection_batch(9, n, n_o)
+    dev = lambda a: torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).cuda()
+    A, b, zd = dev(P["A"]), dev(P["b"]), dev(P["z_des"])
+    assert A[1:].data_ptr() % 16 != 0 and A[1:].is_contiguous()
+    z_all = B.project(A, b, zd, P["w"], P["rho"], P["z_lo"], P["z_hi"]).cpu().numpy()
+    z_view = B.project(A[1:], b[1:], zd[1:], P["w"], P["rho"], P["z_lo"], P["z_hi"]).cpu().numpy()
+    assert np.array_equal(z_view, z_all[1:])          # same arithmetic on both paths
+    check(OP, z_all, P, range(0, n, 5))
