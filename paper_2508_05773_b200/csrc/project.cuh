@@ -364,16 +364,18 @@ inline cudaError_t launch_project(int n, const float* A, const float* b, const f
     const bool aligned = (((uintptr_t)A | (uintptr_t)b | (uintptr_t)z_des | (uintptr_t)z_out) & 15u) == 0;   // bulk copies
     if (full > 0 && aligned) {
       using SMB = ProjBulkSmem<NO>;
-      static int persistent_ctas = 0;        // resident CTAs of this kernel on the current device
-      if (persistent_ctas == 0) {
+      static int persistent_ctas = 0, cached_dev = -1;   // resident CTAs of this kernel on device cached_dev
+      int dev = 0;
+      if ((e = cudaGetDevice(&dev)) != cudaSuccess) return e;
+      if (dev != cached_dev) {                            // (the attribute is per device, like the SM count)
         e = cudaFuncSetAttribute(project_batch_bulk<NO>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMB::bytes);
         if (e != cudaSuccess) return e;
-        int dev = 0, sms = 0, per_sm = 0;
-        if ((e = cudaGetDevice(&dev)) != cudaSuccess) return e;
+        int sms = 0, per_sm = 0;
         if ((e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return e;
         e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, project_batch_bulk<NO>, kProjBlock, SMB::bytes);
         if (e != cudaSuccess) return e;
         persistent_ctas = sms * (per_sm > 0 ? per_sm : 1);
+        cached_dev = dev;
       }
       // P persistent CTAs for the full blocks + one CTA for the ragged tail, all resident in one wave
       const int P = full < persistent_ctas - 1 ? full : persistent_ctas - 1;
