@@ -648,8 +648,8 @@ int brmppi_get_phase_times(brmppi_ctx* c, float out_us[8]) {
     unsigned long long tmin = ~0ull, tmax = 0ull, life = 0ull;
     for (int b = 0; b < grid; ++b) {
       const unsigned long long t0 = h[b * W + kPhaseSlots], t1 = h[b * W + kPhaseSlots + 1];
-      double cyc = 0.0;
-      for (int i = 0; i < kPhaseSlots; ++i) cyc += (double)h[b * W + i];
+      double cyc = 0.0;   // the chain slot runs under the cost slot: not part of the CTA's timeline sum
+      for (int i = 0; i < kPhaseSlots; ++i) if (i != kChainSlot) cyc += (double)h[b * W + i];
       const double ns_per_cycle = cyc > 0.0 ? (double)(t1 - t0) / cyc : 0.0;
       for (int i = 0; i < kPhaseSlots; ++i) acc[i] += (double)h[b * W + i] * ns_per_cycle;
       if (t0 < tmin) tmin = t0;

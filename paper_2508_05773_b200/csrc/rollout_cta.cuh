@@ -44,14 +44,18 @@ namespace brmppi {
 #define BRMPPI_CTA_THREADS 512
 #endif
 constexpr int kCtaThreads = BRMPPI_CTA_THREADS;
-constexpr int kChainWarps = 4;                      // one per warp scheduler
+constexpr int kCtaWarps = kCtaThreads / 32;
+constexpr int kChainWarps = 4;                      // one per warp scheduler: the LAST four warps of the CTA
 constexpr int kMaxTileSamples = kChainWarps * 32;   // 128
+constexpr int kChainFirstThread = kCtaThreads - kMaxTileSamples;   // chain thread of sample s: this + s
+constexpr int kWorkerThreads = kChainFirstThread;   // threads that only generate noise and evaluate costs
 constexpr int kObsGroup = 8;                        // obstacles whose h_t are held in registers at a time
 constexpr int kSeGroup = 4;                         // super-ellipses whose h_t are held in registers at a time
 constexpr int kMaxChunks = 16;
 constexpr int kMinChunkLen = 4;
 constexpr int kMinCullChunk = 8;                    // culling pays from this chunk length on
-constexpr int kPhaseSlots = 7;                      // prologue, A, B, C, D, E, partial out
+constexpr int kPhaseSlots = 7;                      // prologue, A, chain (runs under C), B + C, D, E, partial out
+constexpr int kChainSlot = 2;
 constexpr size_t kSmemMax = 232448;                 // 227 KB opt-in dynamic shared memory per CTA
 
 struct CtaMisc {            // lives in the "misc" section
@@ -65,6 +69,10 @@ struct CtaMisc {            // lives in the "misc" section
   int redI[kChainWarps];
   float redF[3][kChainWarps];
   unsigned long long phase_acc[kPhaseSlots], t_begin;   // BRMPPI_FLAG_PHASE_TIMING
+  // chunk hand-off from the chain warps to the cost threads (one phase per tile): bar_chunk[c]
+  // completes when every chain thread has stored the headings of steps <= (c + 1) L and the
+  // (x, y) at the start of chunk c + 1; bar_table when warp 0 has written the obstacle tables
+  unsigned long long bar_chunk[kMaxChunks], bar_table;
 };
 
 struct CtaSmem {
@@ -103,7 +111,8 @@ struct CtaPlan {
 // C threads per sample, L = ceil(T / C) steps per thread.  A thread evaluates L + 1 barrier
 // sets (h at its first state plus L new ones); with threads to spare the smallest L wins.
 inline void cta_chunking(int T, int S, int* chunks, int* chunk_len) {
-  int cmax = kCtaThreads / S;
+  // chunks 0 .. C-2 go to the worker threads, the last chunk to the chain threads once the chain is done
+  int cmax = kWorkerThreads / S + 1;
   if (cmax > kMaxChunks) cmax = kMaxChunks;
   if (cmax < 1) cmax = 1;
   if (const char* e = getenv("BRMPPI_MAX_CHUNKS")) {   // tuning knob for sweeps

@@ -36,6 +36,23 @@ __device__ __forceinline__ unsigned long long global_ns() {
     t_stamp = now__;                                                         \
   }
 
+// mbarrier hand-off (chain warps -> cost threads), CTA scope.  One phase per tile: the waiter passes
+// the parity of the tile it is in.
+__device__ __forceinline__ uint32_t smem_addr(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint32_t bar, int count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {   // release: this thread's earlier shared stores are visible to the waiter
+  asm volatile("mbarrier.arrive.release.cta.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+  uint32_t done;
+  do {
+    asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.acquire.cta.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }"
+                 : "=r"(done) : "r"(bar), "r"(parity) : "memory");
+  } while (!done);
+}
+
 // Phase C for one group of kObsGroup obstacles over the steps [t0, t1) of one sample: the
 // barrier-rate hinge sum_t sum_{i,j} max(0, (1 - alpha) h_t - h_{t+1})  (a4, a5), and -- for the
 // first group (TRACK) -- the goal / heading / hitch stage cost of every state it visits (a6).
@@ -284,7 +301,14 @@ rollout_cta(const __grid_constant__ DeviceParams P) {
   const int tile_last = min(tile_first + P.tiles_per_cta, P.total_tiles);
   int cur_scene = -1;
   int par = 0;          // parity of the running softmax state in CtaMisc
+  uint32_t tile_parity = 0;   // phase parity of the hand-off barriers (one phase per tile)
   unsigned long long t_stamp = 0;
+  if (tid == 0) {
+    CtaMisc* sM = BRMPPI_SMEM(CtaMisc, P.off_misc);
+    for (int i = 0; i < kMaxChunks; ++i) mbar_init(smem_addr(&sM->bar_chunk[i]), kMaxTileSamples);
+    mbar_init(smem_addr(&sM->bar_table), 32);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
   if (P.phase_ns != nullptr && tid == 0) {
     for (int i = 0; i < kPhaseSlots; ++i) BRMPPI_SMEM(CtaMisc, P.off_misc)->phase_acc[i] = 0ull;
     t_stamp = (unsigned long long)clock64();
@@ -323,15 +347,29 @@ rollout_cta(const __grid_constant__ DeviceParams P) {
     // Scene data: the global loads are issued here and consumed after phase A, so their latency
     // (HBM when the caller has flushed L2) hides behind the noise generation.
     float4 x0_in = make_float4(0.f, 0.f, 0.f, 0.f), g_in = x0_in;
-    float ob_in[5] = {0.f, 0.f, 1.f, 0.f, 0.f};
-    int n_obs_in = 0;
+    float ob_in[2][5] = {{0.f, 0.f, 1.f, 0.f, 0.f}, {0.f, 0.f, 1.f, 0.f, 0.f}};   // warp 0: obstacles lane, lane + 32
+    float4 se_in[2] = {x0_in, x0_in};                                          // warp 0: super-ellipse `lane`
+    int n_obs_in = 0, n_se_in = 0;
     if (new_scene) {
       x0_in = reinterpret_cast<const float4*>(P.state)[scene];
       n_obs_in = P.n_obs[scene];
-      if (tid < P.max_obstacles) {
-        const float* ob = P.obstacles + ((size_t)scene * P.max_obstacles + tid) * 5;
+      if (warp == 0) {
 #pragma unroll
-        for (int q = 0; q < 5; ++q) ob_in[q] = ob[q];
+        for (int h = 0; h < 2; ++h) {
+          const int i = lane + 32 * h;
+          if (i < P.max_obstacles) {
+            const float* ob = P.obstacles + ((size_t)scene * P.max_obstacles + i) * 5;
+#pragma unroll
+            for (int q = 0; q < 5; ++q) ob_in[h][q] = ob[q];
+          }
+        }
+        if (P.max_superellipses > 0) {
+          n_se_in = P.n_se[scene];
+          if (lane < P.max_superellipses) {
+            const float4* q = reinterpret_cast<const float4*>(P.se + ((size_t)scene * P.max_superellipses + lane) * 8);
+            se_in[0] = q[0]; se_in[1] = q[1];
+          }
+        }
       }
       if (tid == 0) g_in = reinterpret_cast<const float4*>(P.goal)[scene];
     }
@@ -373,14 +411,8 @@ rollout_cta(const __grid_constant__ DeviceParams P) {
       if (c == 0) BRMPPI_SMEM(float, P.off_alpha)[s] = sample_alpha(P, n, (uint32_t)k, key0, key1);
     }
     if (new_scene) {
-      // stage the scene for warp kChainWarps, which sorts the obstacles while the chain runs
       CtaMisc* sM = BRMPPI_SMEM(CtaMisc, P.off_misc);
-      float* sRaw = BRMPPI_SMEM(float, P.off_raw);
       float* sA = BRMPPI_SMEM(float, P.off_A);
-      if (tid < P.max_obstacles) {
-#pragma unroll
-        for (int q = 0; q < 5; ++q) sRaw[5 * tid + q] = ob_in[q];
-      }
       for (int i = tid; i < 2 * P.T; i += kCtaThreads) sA[i] = 0.0f;
       if (tid == 0) {
         g_in.x -= x0_in.x; g_in.y -= x0_in.y;          // vehicle-centred frame
@@ -393,119 +425,157 @@ rollout_cta(const __grid_constant__ DeviceParams P) {
     __syncthreads();
     BRMPPI_STAMP(1)
 
-    // ---- phase B: serial Euler chain of eq. (6), one sample per thread (a3).  Only the psi2
-    //      recursion is a true chain; the thread also integrates psi1, x, y (short independent
-    //      dependency chains that fill its issue bubbles).  Everything else is left to phase C. ---
-    if (c == 0) {
-      const int TS = P.t_stride, T = P.T, L = P.chunk_len;
-      const float* pV = BRMPPI_SMEM(float, P.off_planes) + s * TS;
-      float* pP1 = BRMPPI_SMEM(float, P.off_planes) + (2 * S + s) * TS;
-      float* pP2 = pP1 + S * TS;
-      float2* sXY = BRMPPI_SMEM(float2, P.off_xy);        // [C][S] chunk-start (x, y)
-      const float4 x0 = BRMPPI_SMEM(CtaMisc, P.off_misc)->x0;
-      float x = 0.0f, y = 0.0f, psi1 = x0.z, psi2 = x0.w;
-      pP1[0] = psi1;
-      pP2[0] = psi2;
-      const float* pD = pV + S * TS;
-      float effort = 0.0f;                                   // w_v v^2 + w_delta delta^2 summed over the horizon
-      float v = pV[0], b = pP1[1];
-      for (int cc = 0, t = 0; t < T; ++cc) {
-        sXY[cc * S + s] = make_float2(x, y);
-        const int te = min(t + L, T);
-        for (; t < te; ++t) {
-          // next step's inputs first: the loads do not wait behind this step's stores
-          const int tn = min(t + 1, T - 1);
-          const float v_next = pV[tn], b_next = pP1[tn + 1];
-          const float d = pD[t];
-          effort = fmaf(P.w_v * v, v, fmaf(P.w_delta * d, d, effort));
-          const float a = P.dt * v;
-          float s1, c1, sb, cb;
-          sincos_t<PRECISE>(psi1 - psi2, &sb, &cb);
-          sincos_t<PRECISE>(psi1, &s1, &c1);
-          x = fmaf(a, c1, x);
-          y = fmaf(a, s1, y);
-          psi1 += b;
-          psi2 = fmaf(a * P.inv_L2, sb, fmaf(-(b * P.Lh_over_L2), cb, psi2));
-          pP1[t + 1] = psi1;
-          pP2[t + 1] = psi2;
-          v = v_next; b = b_next;
-        }
-      }
-      sXY[P.chunks * S + s] = make_float2(x, y);   // x_T
-      BRMPPI_SMEM(float, P.off_scratch)[s] = effort;
-    } else if (new_scene && warp == kChainWarps) {
-      // obstacle table for phase C, in the vehicle-centred frame: moving obstacles first, static
-      // ones after (groups without a moving one skip the o(t) update), null padding behind.
-      // Obstacles 2p and 2p+1 are interleaved field by field -- (-ox, -ox'), (-oy, -oy'),
-      // (-1/rho^2, ..), (-rho^2, ..); velocities (-dt vx, ..), (-dt vy, ..) -- so that phase C
-      // loads each pair of fields as one packed f32x2 operand.
-      // Lane l ranks obstacles l and l + 32 by counting; the chain warps are busy meanwhile.
+    // ---- phase B: serial Euler chain of eq. (6), one sample per thread (a3), on the CTA's LAST four
+    //      warps -- one per scheduler, and the ones the arbiter prefers (highest warp id first), so
+    //      the in-order chain keeps its issue slots while the cost threads of the chunks already
+    //      handed over run underneath it.  Only the psi2 recursion is a true chain; the thread also
+    //      integrates psi1, x, y (short independent dependency chains that fill its issue
+    //      bubbles).  After every chunk of L steps the chain threads arrive on bar_chunk[chunk]. ---
+    const int k0 = k - s;                                    // sample index of the tile's first sample
+    if (warp >= kCtaWarps - kChainWarps) {
       CtaMisc* sM = BRMPPI_SMEM(CtaMisc, P.off_misc);
-      const float* sRaw = BRMPPI_SMEM(float, P.off_raw);
-      float4* sObs = BRMPPI_SMEM(float4, P.off_obs);
-      float2* sVel = BRMPPI_SMEM(float2, P.off_vel);
-      float* sSpd = BRMPPI_SMEM(float, P.off_spd);
-      const int n_obs = sM->n_obs;
-      const float4 x0 = sM->x0;
-      int nm = 0;
-      for (int j = 0; j < n_obs; ++j) nm += (sRaw[5 * j + 3] != 0.0f || sRaw[5 * j + 4] != 0.0f) ? 1 : 0;
-      for (int i = lane; i < P.obs_padded; i += 32) {
-        if (i < n_obs) {
-          int before_m = 0, before_s = 0;
-          for (int j = 0; j < i; ++j) {
-            const bool mj = (sRaw[5 * j + 3] != 0.0f || sRaw[5 * j + 4] != 0.0f);
-            before_m += mj ? 1 : 0; before_s += mj ? 0 : 1;
+      const int sc = tid - kChainFirstThread;
+      const int n_handoff = P.chunks - 1;                    // the last chunk stays with the chain threads
+      if (sc < S) {
+        const int TS = P.t_stride, T = P.T, L = P.chunk_len;
+        const float* pV = BRMPPI_SMEM(float, P.off_planes) + sc * TS;
+        float* pP1 = BRMPPI_SMEM(float, P.off_planes) + (2 * S + sc) * TS;
+        float* pP2 = pP1 + S * TS;
+        float2* sXY = BRMPPI_SMEM(float2, P.off_xy);        // [C][S] chunk-start (x, y)
+        const float4 x0 = sM->x0;
+        float x = 0.0f, y = 0.0f, psi1 = x0.z, psi2 = x0.w;
+        pP1[0] = psi1;
+        pP2[0] = psi2;
+        const float* pD = pV + S * TS;
+        float effort = 0.0f;                                   // w_v v^2 + w_delta delta^2 summed over the horizon
+        float v = pV[0], b = pP1[1];
+        const long long t_chain = (P.phase_ns != nullptr && sc == 0) ? clock64() : 0ll;
+        for (int cc = 0, t = 0; t < T; ++cc) {
+          sXY[cc * S + sc] = make_float2(x, y);
+          const int te = min(t + L, T);
+          for (; t < te; ++t) {
+            // next step's inputs first: the loads do not wait behind this step's stores
+            const int tn = min(t + 1, T - 1);
+            const float v_next = pV[tn], b_next = pP1[tn + 1];
+            const float d = pD[t];
+            effort = fmaf(P.w_v * v, v, fmaf(P.w_delta * d, d, effort));
+            const float a = P.dt * v;
+            float s1, c1, sb, cb;
+            sincos_t<PRECISE>(psi1 - psi2, &sb, &cb);
+            sincos_t<PRECISE>(psi1, &s1, &c1);
+            x = fmaf(a, c1, x);
+            y = fmaf(a, s1, y);
+            psi1 += b;
+            psi2 = fmaf(a * P.inv_L2, sb, fmaf(-(b * P.Lh_over_L2), cb, psi2));
+            pP1[t + 1] = psi1;
+            pP2[t + 1] = psi2;
+            v = v_next; b = b_next;
           }
-          const bool moving = (sRaw[5 * i + 3] != 0.0f || sRaw[5 * i + 4] != 0.0f);
-          const int dst = moving ? before_m : nm + before_s;
-          const float rho = sRaw[5 * i + 2] + P.disc_radius;
-          float* ob = reinterpret_cast<float*>(sObs) + (dst >> 1) * 8 + (dst & 1);
-          ob[0] = -(sRaw[5 * i + 0] - x0.x);
-          ob[2] = -(sRaw[5 * i + 1] - x0.y);
-          ob[4] = -2.0f * (0.5f / (rho * rho));
-          ob[6] = -(rho * rho);
-          float* vl = reinterpret_cast<float*>(sVel) + (dst >> 1) * 4 + (dst & 1);
-          vl[0] = -(P.dt * sRaw[5 * i + 3]);
-          vl[2] = -(P.dt * sRaw[5 * i + 4]);
-          // displacement per step, rounded up (culling bound)
-          sSpd[dst] = 1.0001f * P.dt * sqrtf(fmaf(sRaw[5 * i + 3], sRaw[5 * i + 3], sRaw[5 * i + 4] * sRaw[5 * i + 4]));
-        } else {                                        // null obstacle: weight 0
+          if (cc < n_handoff) mbar_arrive(smem_addr(&sM->bar_chunk[cc]));
+        }
+        sXY[P.chunks * S + sc] = make_float2(x, y);   // x_T
+        BRMPPI_SMEM(float, P.off_scratch)[sc] = effort;
+        if (P.phase_ns != nullptr && sc == 0) sM->phase_acc[kChainSlot] += (unsigned long long)(clock64() - t_chain);
+      } else {
+        for (int cc = 0; cc < n_handoff; ++cc) mbar_arrive(smem_addr(&sM->bar_chunk[cc]));
+      }
+    } else if (warp == 0) {
+      // While the chain runs its first chunk (nothing else is ready yet), warp 0 writes the scene's
+      // obstacle tables.
+      CtaMisc* sM = BRMPPI_SMEM(CtaMisc, P.off_misc);
+      if (new_scene) {
+        // obstacle table for phase C, in the vehicle-centred frame: moving obstacles first, static
+        // ones after (groups without a moving one skip the o(t) update), null padding behind.
+        // Obstacles 2p and 2p+1 are interleaved field by field -- (-ox, -ox'), (-oy, -oy'),
+        // (-1/rho^2, ..), (-rho^2, ..); velocities (-dt vx, ..), (-dt vy, ..) -- so that phase C
+        // loads each pair of fields as one packed f32x2 operand.
+        // Lane l holds obstacles l and l + 32 in registers and ranks them with two ballots.
+        float4* sObs = BRMPPI_SMEM(float4, P.off_obs);
+        float2* sVel = BRMPPI_SMEM(float2, P.off_vel);
+        float* sSpd = BRMPPI_SMEM(float, P.off_spd);
+        const int n_obs = n_obs_in;
+        const unsigned lt = (1u << lane) - 1u;
+        bool val[2], mov[2];
+        unsigned bv[2], bm[2];
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+          val[h] = lane + 32 * h < n_obs;
+          mov[h] = val[h] && (ob_in[h][3] != 0.0f || ob_in[h][4] != 0.0f);
+          bv[h] = __ballot_sync(0xffffffffu, val[h]);
+          bm[h] = __ballot_sync(0xffffffffu, mov[h]);
+        }
+        const int nm = __popc(bm[0]) + __popc(bm[1]);
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+          if (val[h]) {
+            const int before_m = (h ? __popc(bm[0]) : 0) + __popc(bm[h] & lt);
+            const int before_s = (h ? __popc(bv[0] & ~bm[0]) : 0) + __popc(bv[h] & ~bm[h] & lt);
+            const int dst = mov[h] ? before_m : nm + before_s;
+            const float rho = ob_in[h][2] + P.disc_radius;
+            float* ob = reinterpret_cast<float*>(sObs) + (dst >> 1) * 8 + (dst & 1);
+            ob[0] = -(ob_in[h][0] - x0_in.x);
+            ob[2] = -(ob_in[h][1] - x0_in.y);
+            ob[4] = -2.0f * (0.5f / (rho * rho));
+            ob[6] = -(rho * rho);
+            float* vl = reinterpret_cast<float*>(sVel) + (dst >> 1) * 4 + (dst & 1);
+            vl[0] = -(P.dt * ob_in[h][3]);
+            vl[2] = -(P.dt * ob_in[h][4]);
+            // displacement per step, rounded up (culling bound)
+            sSpd[dst] = 1.0001f * P.dt * sqrtf(fmaf(ob_in[h][3], ob_in[h][3], ob_in[h][4] * ob_in[h][4]));
+          }
+        }
+        for (int i = n_obs + lane; i < P.obs_padded; i += 32) {   // null obstacles: weight 0
           float* ob = reinterpret_cast<float*>(sObs) + (i >> 1) * 8 + (i & 1);
           ob[0] = 0.0f; ob[2] = 0.0f; ob[4] = 0.0f; ob[6] = 0.0f;
           float* vl = reinterpret_cast<float*>(sVel) + (i >> 1) * 4 + (i & 1);
           vl[0] = 0.0f; vl[2] = 0.0f;
           sSpd[i] = 0.0f;
         }
-      }
-      // super-ellipse table: rows of R(-theta) over the inflated semi-axes; null records weigh 0
-      const int n_se = P.max_superellipses > 0 ? P.n_se[scene] : 0;
-      SeRecord* sSE = BRMPPI_SMEM(SeRecord, P.off_se);
-      for (int i = lane; i < P.se_padded; i += 32) {
-        SeRecord r = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
-        if (i < n_se) {
-          const float* q = P.se + ((size_t)scene * P.max_superellipses + i) * 8;
-          float st, ct;
-          sincosf(q[4], &st, &ct);
-          const float iax = 1.0f / (q[2] + P.disc_radius), iay = 1.0f / (q[3] + P.disc_radius);
-          r.ox = q[0] - x0.x; r.oy = q[1] - x0.y;
-          r.a11 = ct * iax; r.a12 = st * iax; r.a21 = -st * iay; r.a22 = ct * iay;
-          r.wx = P.dt * q[5]; r.wy = P.dt * q[6];
-          r.e4 = q[7] == 4.0f ? 1.0f : 0.0f;
-          r.half_w = 0.5f;
+        // super-ellipse table: rows of R(-theta) over the inflated semi-axes; null records weigh 0
+        const int n_se = n_se_in;
+        SeRecord* sSE = BRMPPI_SMEM(SeRecord, P.off_se);
+        if (lane < P.se_padded) {
+          SeRecord r = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+          if (lane < n_se) {
+            float st, ct;
+            sincosf(se_in[1].x, &st, &ct);
+            const float iax = 1.0f / (se_in[0].z + P.disc_radius), iay = 1.0f / (se_in[0].w + P.disc_radius);
+            r.ox = se_in[0].x - x0_in.x; r.oy = se_in[0].y - x0_in.y;
+            r.a11 = ct * iax; r.a12 = st * iax; r.a21 = -st * iay; r.a22 = ct * iay;
+            r.wx = P.dt * se_in[1].y; r.wy = P.dt * se_in[1].z;
+            r.e4 = se_in[1].w == 4.0f ? 1.0f : 0.0f;
+            r.half_w = 0.5f;
+          }
+          sSE[lane] = r;
         }
-        sSE[i] = r;
+        if (lane == 0) {
+          sM->n_moving = nm;
+          sM->n_groups = n_obs > 0 ? (n_obs + kObsGroup - 1) / kObsGroup : 1;
+          sM->n_se_groups = (n_se + kSeGroup - 1) / kSeGroup;
+        }
       }
-      if (lane == 0) {
-        sM->n_moving = nm;
-        sM->n_groups = n_obs > 0 ? (n_obs + kObsGroup - 1) / kObsGroup : 1;
-        sM->n_se_groups = (n_se + kSeGroup - 1) / kSeGroup;
+      mbar_arrive(smem_addr(&sM->bar_table));    // every tile, so that the barrier's phase follows the tile count
+    }
+
+    // ---- phase C: barrier, barrier-rate hinge, goal / heading / hitch cost (a4-a6).  Worker thread
+    //      (chunk, sample) = (tid / S, tid % S) takes chunks 0 .. C-2 as soon as the chain has handed
+    //      the chunk over; the chain thread of a sample takes its last chunk. -------------------------
+    int cq = -1, sq = 0;
+    {
+      const int n_worker_items = (P.chunks - 1) * S;
+      if (tid < n_worker_items) { cq = c; sq = s; }
+      else if (tid >= kChainFirstThread && tid - kChainFirstThread < S) { cq = P.chunks - 1; sq = tid - kChainFirstThread; }
+      if (cq >= 0) {
+        CtaMisc* sMb = BRMPPI_SMEM(CtaMisc, P.off_misc);
+        mbar_wait(smem_addr(&sMb->bar_table), tile_parity);
+        if (tid < n_worker_items) {   // warp-uniform: the latest chunk any lane of this warp works on
+          const int last = min((warp << 5) + 31, n_worker_items - 1);
+          mbar_wait(smem_addr(&sMb->bar_chunk[last / S]), tile_parity);
+        }
       }
     }
-    __syncthreads();
-    BRMPPI_STAMP(2)
-
-    // ---- phase C: barrier, barrier-rate hinge, goal / heading / hitch cost (a4-a6) -----------
-    if (c < P.chunks) {
+    if (cq >= 0) {
+      const int c = cq, s = sq, k = k0 + sq;     // this thread's (chunk, sample in tile, sample index)
       const int TS = P.t_stride, T = P.T;
       const int t0 = c * P.chunk_len, t1 = min(t0 + P.chunk_len, T);
       const CtaMisc* sM = BRMPPI_SMEM(CtaMisc, P.off_misc);
@@ -663,6 +733,7 @@ rollout_cta(const __grid_constant__ DeviceParams P) {
       }
     }
     par ^= 1;
+    tile_parity ^= 1u;
     __syncthreads();
     BRMPPI_STAMP(5)
   }
