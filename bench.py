@@ -357,13 +357,14 @@ def run_phases(args):
     from paper_2508_05773_b200 import brmppi as B
     sc, p = workload(args.workload)
     n_se = 0 if sc.superellipses is None else len(sc.superellipses)
-    s = B.Solver(p.with_(n_iter=1), 1, max(len(sc.obstacles), 1), B.FLAG_PHASE_TIMING, max_superellipses=n_se)
+    s = B.Solver(p.with_(n_iter=1), 1, max(len(sc.obstacles), 1), B.FLAG_PHASE_TIMING | (B.FLAG_NO_CULL if args.no_cull else 0),
+                 max_superellipses=n_se)
     s.set_scene(sc)
     for _ in range(5):
         s.solve()
     s.synchronize()
     print(json.dumps({"workload": args.workload, "K": p.K, "T": p.T, "n_obstacles": len(sc.obstacles),
-                      "phase_us": s.get_phase_times()}))
+                      "no_cull": bool(args.no_cull), "phase_us": s.get_phase_times()}))
     s.close()
 
 
@@ -472,6 +473,7 @@ def main():
     ap.add_argument("--phases", action="store_true", help="print the rollout kernel's in-kernel phase times")
     ap.add_argument("--sweep", action="store_true", help="run BASELINE.json configs[4] (sweep + 64-scene batch)")
     ap.add_argument("--project", action="store_true", help="time the closed-form projection (12) on its own")
+    ap.add_argument("--no-cull", action="store_true", help="evaluate every (obstacle, disc, step): BRMPPI_FLAG_NO_CULL")
     args = ap.parse_args()
     if args.project:
         run_project(args)

@@ -273,7 +273,11 @@ int brmppi_create(const brmppi_params* p, void* dev_workspace, size_t workspace_
   memset(&d, 0, sizeof(d));
   d.K = p->K; d.T = p->T; d.n_scenes = p->n_scenes; d.max_obstacles = p->max_obstacles;
   d.n_discs = p->n_discs;
-  for (int j = 0; j < p->n_discs; ++j) { d.disc_body[j] = p->discs[j].body; d.disc_offset[j] = p->discs[j].offset; }
+  for (int j = 0; j < p->n_discs; ++j) {
+    d.disc_body[j] = p->discs[j].body; d.disc_offset[j] = p->discs[j].offset;
+    d.disc_a1[j] = p->discs[j].body == 0 ? p->discs[j].offset : 0.0f;
+    d.disc_a2[j] = p->discs[j].body == 0 ? 0.0f : p->discs[j].offset;
+  }
   d.disc_radius = p->disc_radius;
   {
     // Speed bound of every disc centre under the Euler map of eq. (6): the rear
@@ -309,7 +313,7 @@ int brmppi_create(const brmppi_params* p, void* dev_workspace, size_t workspace_
     d.chunks = cp.chunks; d.chunk_len = cp.chunk_len; d.t_stride = cp.ts; d.obs_padded = cp.obs_padded;
     const CtaSmem ts = cta_smem_layout(d.T, cp.S_tile, cp.chunks, cp.ts, cp.obs_padded, cp.se_padded);
     d.se_padded = cp.se_padded; d.off_se = (int)ts.se;
-    d.off_obs = (int)ts.obs; d.off_vel = (int)ts.vel; d.off_spd = (int)ts.spd; d.off_raw = (int)ts.raw; d.off_A = (int)ts.A;
+    d.off_obs = (int)ts.obs; d.off_vel = (int)ts.vel; d.off_thr = (int)ts.thr; d.off_A = (int)ts.A;
     d.off_scratch = (int)ts.scratch; d.off_w = (int)ts.w; d.off_alpha = (int)ts.alpha;
     d.off_cost = (int)ts.cost; d.off_xy = (int)ts.xy;
     d.off_planes = (int)ts.planes; d.off_misc = (int)ts.misc;

@@ -23,6 +23,7 @@ struct DeviceParams {
   int K, T, n_scenes, max_obstacles, n_discs, max_superellipses;
   int disc_body[kMaxDiscs];
   float disc_offset[kMaxDiscs];
+  float disc_a1[kMaxDiscs], disc_a2[kMaxDiscs];   // offset on the tractor axis / on the trailer axis (one is 0)
   float disc_radius;
   float disc_speed[kMaxDiscs];   // upper bound on the speed of each disc centre, m/s (culling)
   float dt, inv_L1, inv_L2, Lh, Lh_over_L1, Lh_over_L2;
@@ -47,7 +48,7 @@ struct DeviceParams {
   int off_se;                 // shared-memory section of the super-ellipse table
   // byte offsets of the shared-memory sections (host-computed, so that the device code
   // rematerialises a pointer with one add instead of keeping it in a register)
-  int off_obs, off_vel, off_spd, off_raw, off_A, off_scratch, off_w, off_alpha, off_cost, off_xy,
+  int off_obs, off_vel, off_thr, off_A, off_scratch, off_w, off_alpha, off_cost, off_xy,
       off_planes, off_misc;
   // workspace pointers (DEVICE)
   float* state;               // [n_scenes][4]
@@ -260,9 +261,9 @@ __device__ __forceinline__ void disc_centres_n(const DeviceParams& P, float x, f
   const float hx = fmaf(-P.Lh, c1, x), hy = fmaf(-P.Lh, s1, y);
 #pragma unroll
   for (int j = 0; j < ND; ++j) {
-    const bool trailer = P.disc_body[j] != 0;
-    cx[j] = fmaf(P.disc_offset[j], trailer ? c2 : c1, hx);
-    cy[j] = fmaf(P.disc_offset[j], trailer ? s2 : s1, hy);
+    // one of the two coefficients is zero: the same value as offset * (body axis), without a select
+    cx[j] = fmaf(P.disc_a1[j], c1, fmaf(P.disc_a2[j], c2, hx));
+    cy[j] = fmaf(P.disc_a1[j], s1, fmaf(P.disc_a2[j], s2, hy));
   }
 }
 

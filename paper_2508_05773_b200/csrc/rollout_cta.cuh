@@ -49,11 +49,11 @@ constexpr int kChainWarps = 4;                      // one per warp scheduler: t
 constexpr int kMaxTileSamples = kChainWarps * 32;   // 128
 constexpr int kChainFirstThread = kCtaThreads - kMaxTileSamples;   // chain thread of sample s: this + s
 constexpr int kWorkerThreads = kChainFirstThread;   // threads that only generate noise and evaluate costs
+constexpr int kTableWarp = kCtaWarps - kChainWarps - 1;   // writes the obstacle tables of a scene
 constexpr int kObsGroup = 8;                        // obstacles whose h_t are held in registers at a time
 constexpr int kSeGroup = 4;                         // super-ellipses whose h_t are held in registers at a time
 constexpr int kMaxChunks = 16;
 constexpr int kMinChunkLen = 4;
-constexpr int kMinCullChunk = 8;                    // culling pays from this chunk length on
 constexpr int kPhaseSlots = 7;                      // prologue, A, chain (runs under C), B + C, D, E, partial out
 constexpr int kChainSlot = 2;
 constexpr size_t kSmemMax = 232448;                 // 227 KB opt-in dynamic shared memory per CTA
@@ -63,7 +63,8 @@ struct CtaMisc {            // lives in the "misc" section
   int argmin[2];
   float eta[2], w2[2];
   int nonfinite[2];
-  int n_obs, n_moving, n_groups, n_se_groups;
+  int n_obs, n_groups, n_se_groups;
+  unsigned moving_groups;   // bit g: some obstacle of group g moves
   float4 x0, g;             // start state; goal in the vehicle-centred frame
   double redM[kChainWarps];
   int redI[kChainWarps];
@@ -71,12 +72,12 @@ struct CtaMisc {            // lives in the "misc" section
   unsigned long long phase_acc[kPhaseSlots], t_begin;   // BRMPPI_FLAG_PHASE_TIMING
   // chunk hand-off from the chain warps to the cost threads (one phase per tile): bar_chunk[c]
   // completes when every chain thread has stored the headings of steps <= (c + 1) L and the
-  // (x, y) at the start of chunk c + 1; bar_table when warp 0 has written the obstacle tables
-  unsigned long long bar_chunk[kMaxChunks], bar_table;
+  // (x, y) at the start of chunk c + 1
+  unsigned long long bar_chunk[kMaxChunks];
 };
 
 struct CtaSmem {
-  size_t obs, vel, spd, raw, se, A, scratch, w, alpha, cost, xy, planes, misc, total;
+  size_t obs, vel, thr, se, A, scratch, w, alpha, cost, xy, planes, misc, total;
 };
 
 // Shared-memory carve-up (host only: the kernel gets the byte offsets through DeviceParams, so
@@ -87,8 +88,7 @@ inline CtaSmem cta_smem_layout(int T, int S, int chunks, int ts, int obs_padded,
   auto take = [&](size_t b) { size_t o = off; off = (off + b + 15) / 16 * 16; return o; };
   L.obs = take(sizeof(float4) * (size_t)obs_padded);
   L.vel = take(sizeof(float2) * (size_t)obs_padded);
-  L.spd = take(sizeof(float) * (size_t)obs_padded);       // obstacle displacement per step
-  L.raw = take(sizeof(float) * 5 * (size_t)obs_padded);   // obstacles as given, before sorting
+  L.thr = take(sizeof(float) * kMaxDiscs * (size_t)obs_padded);   // culling thresholds per (obstacle, disc)
   L.se = take(sizeof(float) * 12 * (size_t)se_padded);    // SeRecord per super-ellipse
   L.A = take(sizeof(float) * 2 * (size_t)T);
   L.scratch = take(sizeof(float) * kCtaThreads);

@@ -50,6 +50,7 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
   do {
     asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.acquire.cta.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }"
                  : "=r"(done) : "r"(bar), "r"(parity) : "memory");
+    if (!done) __nanosleep(32);     // waiting warps must not take issue slots from the chain and the table warp
   } while (!done);
 }
 
@@ -60,62 +61,62 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
 // Arithmetic form.  With rho = R + r_v and g = |c - o|^2 - rho^2 (so h = g / rho^2):
 //     max(0, (1-alpha) h_t - h_{t+1}) = -(1 / rho^2) min(0, zn),   zn = g_{t+1} - (1-alpha) g_t.
 // Obstacles are taken two at a time on packed f32x2 operands (add/fma.rn.f32x2: each half rounds
-// like the scalar instruction, one issue slot for the pair): per (obstacle pair, disc) 2 packed
-// subtractions, 2 packed FMAs for g, 1 for zn, 2 scalar FMNMX, 1 packed accumulate -- 8 issue
-// slots for two evaluations against 14 for the scalar z + |z| form (166 instead of 250
-// instructions per step at 8 obstacles x 3 discs; phase C of CFG2 13.9 -> 12.6 us).
-// The table (written by the sorting warp) interleaves obstacles 2p and 2p+1 field by field, already
+// like the scalar instruction): per (obstacle pair, disc) 2 packed subtractions, 2 packed FMAs for
+// g, 1 for zn, 2 scalar FMNMX, 1 packed accumulate.
+// The table (written by warp 0) interleaves obstacles 2p and 2p+1 field by field, already
 // negated -- (-ox, -ox'), (-oy, -oy'), (-1/rho^2, ..), (-rho^2, ..) -- so every packed operand is
 // one 64-bit shared-memory load; built from scalars, ptxas re-packs them with two MOVs per use.
-// A null (padding) obstacle is all zeros: its weight is 0, so it adds exactly 0.  The first NM
-// obstacles of the group move: o(t) = o(0) + t dt vel (a static one has vel == 0, so rounding NM
-// up is exact).
+// A null (padding) obstacle is all zeros: its weight is 0, so it adds exactly 0.  MOVING: some
+// obstacle of the group moves, o(t) = o(0) + t dt vel (a static one has vel == 0, so the update is
+// exact for it too).
+//
+// Exact culling.  thr[i][j] (warp 0, once per scene) is the value of g above which
+// disc j cannot violate the rate condition against obstacle i anywhere in a chunk, for ANY alpha the
+// sampler can draw (alpha >= alpha_lo gives the largest critical distance): every hinge term of the
+// pair is then exactly +0 and the pair of obstacles is skipped for the chunk.  The mask is the union
+// over the warp's samples, so the skip is a uniform branch.
 // pV, pP1, pP2: this sample's rows of the v, psi1, psi2 planes.
 struct GroupCost { double track, bar; };
 
-template <bool PRECISE, int ND, int NM, bool TRACK, bool CULL>
-__device__ __forceinline__ GroupCost barrier_group(const DeviceParams& P, const float* __restrict__ pV,
-                                                   const float* __restrict__ pP1, const float* __restrict__ pP2,
-                                                   const float4* __restrict__ obs, const float2* __restrict__ vel,
-                                                   const float* __restrict__ spd,
-                                                   float x, float y, int t0, int t1, float one_minus_alpha,
-                                                   const float4 g) {
+// One chunk of one sample with the first NACT obstacle pairs of the group evaluated (the others are
+// culled for this chunk): loads those pairs, g at the chunk's first state, then the step loop --
+// straight-line code, so g_t / g_{t+1} swap registers across the two unrolled steps without moves,
+// and a chunk that needs one pair does not carry the registers of four.
+template <bool PRECISE, int ND, bool MOVING, bool TRACK, int NACT>
+__device__ __forceinline__ GroupCost hinge_chunk(const DeviceParams& P, const float* __restrict__ pV,
+                                                 const float* __restrict__ pP1, const float* __restrict__ pP2,
+                                                 const float4* __restrict__ obs, const float2* __restrict__ vel,
+                                                 float x, float y, int t0, int t1, float one_minus_alpha,
+                                                 const float4 g) {
   double bar = 0.0, track = 0.0;
+  constexpr int NA = NACT > 0 ? NACT : 1;
   // obstacles in pairs (2p, 2p+1): negated centres, -rho^2, -1/rho^2 and g of the previous state
-  constexpr int NP = kObsGroup / 2;
-  f32x2 nox[NP], noy[NP], mrho2[NP], nw[NP], gprev[NP][ND];
-  {
-    // the table is pair-interleaved (see the sorting warp), so a pair arrives as one 64-bit register
+  f32x2 nox[NA], noy[NA], mrho2[NA], nw[NA], gprev[NA][ND];
+  const f32x2 noma = pack2(-one_minus_alpha, -one_minus_alpha);
+  float s1, c1;
+  sincos_t<PRECISE>(pP1[t0], &s1, &c1);
+  if (NACT > 0) {
+    // the table is pair-interleaved (see the table warp), so a pair arrives as one 64-bit register
     const ulonglong2* q = reinterpret_cast<const ulonglong2*>(obs);
 #pragma unroll
-    for (int p = 0; p < NP; ++p) {
+    for (int p = 0; p < NACT; ++p) {
       const ulonglong2 a = q[2 * p], b = q[2 * p + 1];
       nox[p] = a.x; noy[p] = a.y; nw[p] = b.x; mrho2[p] = b.y;
     }
-  }
-  const f32x2 noma = pack2(-one_minus_alpha, -one_minus_alpha);
-  // centre of pair p at step tf: moving obstacles are o(0) + tf vel (a6), negated exactly
-  auto centres = [&](int p, float tf, f32x2& ex, f32x2& ey) {
-    ex = nox[p]; ey = noy[p];
-    if (2 * p < NM) {
-      const ulonglong2 w = reinterpret_cast<const ulonglong2*>(vel)[p];
-      const f32x2 tf2 = pack2(tf, tf);
-      ex = fma2(tf2, w.x, ex);
-      ey = fma2(tf2, w.y, ey);
-    }
-  };
-  float s1, c1;
-  {
     float s2, c2;
-    sincos_t<PRECISE>(pP1[t0], &s1, &c1);
     sincos_t<PRECISE>(pP2[t0], &s2, &c2);
     float cx[ND], cy[ND];
     disc_centres_n<ND>(P, x, y, s1, c1, s2, c2, cx, cy);
     const float tfp = (float)t0;
 #pragma unroll
-    for (int p = 0; p < NP; ++p) {
-      f32x2 ex, ey;
-      centres(p, tfp, ex, ey);
+    for (int p = 0; p < NACT; ++p) {
+      f32x2 ex = nox[p], ey = noy[p];
+      if (MOVING) {   // o(t) = o(0) + t dt vel, negated exactly (a static obstacle has vel == 0)
+        const ulonglong2 w = reinterpret_cast<const ulonglong2*>(vel)[p];
+        const f32x2 tf2 = pack2(tfp, tfp);
+        ex = fma2(tf2, w.x, ex);
+        ey = fma2(tf2, w.y, ey);
+      }
 #pragma unroll
       for (int j = 0; j < ND; ++j) {
         const f32x2 dx = add2(pack2(cx[j], cx[j]), ex), dy = add2(pack2(cy[j], cy[j]), ey);
@@ -123,38 +124,6 @@ __device__ __forceinline__ GroupCost barrier_group(const DeviceParams& P, const 
       }
     }
   }
-  // Exact culling: obstacle i cannot violate the rate condition anywhere in this
-  // chunk if every disc starts farther from it than d_crit plus what the two can close in the
-  // chunk; its hinge terms are then all exactly +0 and it is skipped.  The mask is the union over
-  // the warp's samples, so the skip is a uniform branch.
-  unsigned active = 0xffu;
-  if (CULL && !(P.flags & BRMPPI_FLAG_NO_CULL)) {
-    const float alpha = 1.0f - one_minus_alpha;
-    const float inv_alpha = 1.0f / alpha;
-    const float steps = (float)(t1 - t0);
-    active = 0u;
-#pragma unroll
-    for (int i = 0; i < kObsGroup; ++i) {
-      float ra, rb, wa, wb;
-      unpack2(mrho2[i >> 1], ra, rb);
-      unpack2(nw[i >> 1], wa, wb);
-      const float rho2 = -((i & 1) ? rb : ra);
-      bool act = false;
-#pragma unroll
-      for (int j = 0; j < ND; ++j) {
-        float ga, gb;
-        unpack2(gprev[i >> 1][j], ga, gb);
-        const float dl = fmaf(P.dt, P.disc_speed[j], spd[i]);   // relative displacement per step
-        const float d0 = sqrtf(fmaxf(((i & 1) ? gb : ga) + rho2, 0.0f));
-        const float d_crit = (dl + sqrtf(fmaf(one_minus_alpha * dl, dl, alpha * alpha * rho2))) * inv_alpha;
-        act = act || !(d0 - steps * dl >= fmaf(1.02f, d_crit, 0.05f));
-      }
-      if (((i & 1) ? wb : wa) == 0.0f) act = false;          // null obstacle: weight 0
-      active |= act ? (1u << i) : 0u;
-    }
-    active = __reduce_or_sync(__activemask(), active);
-  }
-  if (CULL && !TRACK && active == 0u) return GroupCost{0.0, 0.0};
 #pragma unroll kCostUnroll
   for (int t = t0; t < t1; ++t) {
     // (x, y) of state t+1 from state t: the chain's own FMAs on the same operands
@@ -163,39 +132,99 @@ __device__ __forceinline__ GroupCost barrier_group(const DeviceParams& P, const 
     x = fmaf(a, c1, x);
     y = fmaf(a, s1, y);
     const float psi1 = pP1[t + 1], psi2 = pP2[t + 1];
-    float s2, c2;
     sincos_t<PRECISE>(psi1, &s1, &c1);
-    sincos_t<PRECISE>(psi2, &s2, &c2);
-    float cx[ND], cy[ND];
-    disc_centres_n<ND>(P, x, y, s1, c1, s2, c2, cx, cy);
     if (TRACK) {
       const State X{x, y, psi1, psi2};
       if (PRECISE) track += (double)(goal_cost(P, X, g) + hitch_cost(P, X, v_t));
       else track += (double)tracking_cost_fma(P, X, g, v_t);
     }
-    const float tfp = (float)(t + 1);
-    f32x2 pen = pack2(0.0f, 0.0f);
+    if (NACT > 0) {
+      float s2, c2;
+      sincos_t<PRECISE>(psi2, &s2, &c2);
+      float cx[ND], cy[ND];
+      disc_centres_n<ND>(P, x, y, s1, c1, s2, c2, cx, cy);
+      const float tfp = (float)(t + 1);
+      f32x2 pen = pack2(0.0f, 0.0f);
+#pragma unroll
+      for (int p = 0; p < NACT; ++p) {
+        f32x2 ex = nox[p], ey = noy[p];
+        if (MOVING) {
+          const ulonglong2 w = reinterpret_cast<const ulonglong2*>(vel)[p];
+          const f32x2 tf2 = pack2(tfp, tfp);
+          ex = fma2(tf2, w.x, ex);
+          ey = fma2(tf2, w.y, ey);
+        }
+#pragma unroll
+        for (int j = 0; j < ND; ++j) {
+          const f32x2 dx = add2(pack2(cx[j], cx[j]), ex), dy = add2(pack2(cy[j], cy[j]), ey);
+          const f32x2 gn = fma2(dx, dx, fma2(dy, dy, mrho2[p]));
+          const f32x2 zn = fma2(gprev[p][j], noma, gn);             // g_{t+1} - (1-alpha) g_t = -z
+          float za, zb;
+          unpack2(zn, za, zb);
+          pen = fma2(nw[p], pack2(fminf(za, 0.0f), fminf(zb, 0.0f)), pen);   // + max(0, z) / rho^2
+          gprev[p][j] = gn;
+        }
+      }
+      float pa, pb;
+      unpack2(pen, pa, pb);
+      bar += (double)(pa + pb);
+    }
+  }
+  return GroupCost{track, bar};
+}
+
+template <bool PRECISE, int ND, bool MOVING, bool TRACK>
+__device__ __forceinline__ GroupCost barrier_group(const DeviceParams& P, const float* __restrict__ pV,
+                                                   const float* __restrict__ pP1, const float* __restrict__ pP2,
+                                                   const float4* __restrict__ obs, const float2* __restrict__ vel,
+                                                   const float* __restrict__ thr,
+                                                   float x, float y, int t0, int t1, float one_minus_alpha,
+                                                   const float4 g) {
+  constexpr int NP = kObsGroup / 2;
+  // pairs to evaluate in this chunk: 1 + the highest pair any sample of the warp needs (the table is
+  // ordered by how close an obstacle is to its threshold at the start state, so the needed pairs are
+  // mostly a prefix; evaluating a culled pair in between adds exact zeros)
+  int n_act = NP;
+  if (!(P.flags & BRMPPI_FLAG_NO_CULL)) {
+    float s1, c1, s2, c2;
+    sincos_t<PRECISE>(pP1[t0], &s1, &c1);
+    sincos_t<PRECISE>(pP2[t0], &s2, &c2);
+    float cx[ND], cy[ND];
+    disc_centres_n<ND>(P, x, y, s1, c1, s2, c2, cx, cy);
+    const float tfp = (float)t0;
+    unsigned mine = 0u;
 #pragma unroll
     for (int p = 0; p < NP; ++p) {
-      if (CULL && !(active & (3u << (2 * p)))) continue;      // warp-uniform
-      f32x2 ex, ey;
-      centres(p, tfp, ex, ey);
+      const ulonglong2 a = reinterpret_cast<const ulonglong2*>(obs)[2 * p];
+      const f32x2 mr = reinterpret_cast<const ulonglong2*>(obs)[2 * p + 1].y;
+      f32x2 ex = a.x, ey = a.y;
+      if (MOVING) {
+        const ulonglong2 w = reinterpret_cast<const ulonglong2*>(vel)[p];
+        const f32x2 tf2 = pack2(tfp, tfp);
+        ex = fma2(tf2, w.x, ex);
+        ey = fma2(tf2, w.y, ey);
+      }
+      bool far = true;
 #pragma unroll
       for (int j = 0; j < ND; ++j) {
         const f32x2 dx = add2(pack2(cx[j], cx[j]), ex), dy = add2(pack2(cy[j], cy[j]), ey);
-        const f32x2 gn = fma2(dx, dx, fma2(dy, dy, mrho2[p]));
-        const f32x2 zn = fma2(gprev[p][j], noma, gn);             // g_{t+1} - (1-alpha) g_t = -z
-        float za, zb;
-        unpack2(zn, za, zb);
-        pen = fma2(nw[p], pack2(fminf(za, 0.0f), fminf(zb, 0.0f)), pen);   // + max(0, z) / rho^2
-        gprev[p][j] = gn;
+        float ga, gb;
+        unpack2(fma2(dx, dx, fma2(dy, dy, mr)), ga, gb);
+        far = far && (ga >= thr[(2 * p) * kMaxDiscs + j]) && (gb >= thr[(2 * p + 1) * kMaxDiscs + j]);   // NaN: not far
       }
+      mine |= far ? 0u : (1u << p);
     }
-    float pa, pb;
-    unpack2(pen, pa, pb);
-    bar += (double)(pa + pb);
+    n_act = 32 - __clz((int)__reduce_or_sync(__activemask(), mine));
   }
-  return GroupCost{track, bar};
+#define BRMPPI_CHUNK(N) return hinge_chunk<PRECISE, ND, MOVING, TRACK, N>(P, pV, pP1, pP2, obs, vel, x, y, t0, t1, one_minus_alpha, g)
+  switch (n_act) {
+    case 0: if (TRACK) BRMPPI_CHUNK(0); return GroupCost{0.0, 0.0};
+    case 1: BRMPPI_CHUNK(1);
+    case 2: BRMPPI_CHUNK(2);
+    case 3: BRMPPI_CHUNK(3);
+    default: BRMPPI_CHUNK(4);
+  }
+#undef BRMPPI_CHUNK
 }
 
 // Super-ellipse obstacles (eq. (16)), kSeGroup at a time:
@@ -276,16 +305,14 @@ __device__ __forceinline__ GroupCost se_group(const DeviceParams& P, const float
   return GroupCost{track, bar};
 }
 
-// Dispatch on the number of moving obstacles in the group (block-uniform).
-template <bool PRECISE, int ND, bool TRACK, bool CULL>
-__device__ __forceinline__ GroupCost barrier_group_nm(int nm, const DeviceParams& P, const float* pV,
+// Dispatch on whether any obstacle of the group moves (block-uniform).
+template <bool PRECISE, int ND, bool TRACK>
+__device__ __forceinline__ GroupCost barrier_group_mv(bool moving, const DeviceParams& P, const float* pV,
                                                       const float* pP1, const float* pP2, const float4* obs,
-                                                      const float2* vel, const float* spd, float x, float y,
+                                                      const float2* vel, const float* thr, float x, float y,
                                                       int t0, int t1, float oma, const float4 g) {
-  if (nm <= 0) return barrier_group<PRECISE, ND, 0, TRACK, CULL>(P, pV, pP1, pP2, obs, vel, spd, x, y, t0, t1, oma, g);
-  if (nm <= 2) return barrier_group<PRECISE, ND, 2, TRACK, CULL>(P, pV, pP1, pP2, obs, vel, spd, x, y, t0, t1, oma, g);
-  if (nm <= 4) return barrier_group<PRECISE, ND, 4, TRACK, CULL>(P, pV, pP1, pP2, obs, vel, spd, x, y, t0, t1, oma, g);
-  return barrier_group<PRECISE, ND, kObsGroup, TRACK, CULL>(P, pV, pP1, pP2, obs, vel, spd, x, y, t0, t1, oma, g);
+  if (!moving) return barrier_group<PRECISE, ND, false, TRACK>(P, pV, pP1, pP2, obs, vel, thr, x, y, t0, t1, oma, g);
+  return barrier_group<PRECISE, ND, true, TRACK>(P, pV, pP1, pP2, obs, vel, thr, x, y, t0, t1, oma, g);
 }
 
 template <bool PRECISE, int ND>
@@ -306,7 +333,6 @@ rollout_cta(const __grid_constant__ DeviceParams P) {
   if (tid == 0) {
     CtaMisc* sM = BRMPPI_SMEM(CtaMisc, P.off_misc);
     for (int i = 0; i < kMaxChunks; ++i) mbar_init(smem_addr(&sM->bar_chunk[i]), kMaxTileSamples);
-    mbar_init(smem_addr(&sM->bar_table), 32);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   if (P.phase_ns != nullptr && tid == 0) {
@@ -353,7 +379,7 @@ rollout_cta(const __grid_constant__ DeviceParams P) {
     if (new_scene) {
       x0_in = reinterpret_cast<const float4*>(P.state)[scene];
       n_obs_in = P.n_obs[scene];
-      if (warp == 0) {
+      if (warp == kTableWarp) {
 #pragma unroll
         for (int h = 0; h < 2; ++h) {
           const int i = lane + 32 * h;
@@ -387,9 +413,14 @@ rollout_cta(const __grid_constant__ DeviceParams P) {
       // tid + 512, ...; (si, mi) = (item % S, item / S) kept up to date incrementally
       float* planes = BRMPPI_SMEM(float, P.off_planes);
       const int n_pairs = (T + 1) >> 1;
-      const int ds = kCtaThreads % S, dm = kCtaThreads / S;
+      // On a tile that starts a scene the table warp writes the obstacle tables instead (below), and
+      // the other 480 threads share the items.
+      const int n_noise = new_scene ? kCtaThreads - 32 : kCtaThreads;
+      const int nid = (new_scene && warp > kTableWarp) ? tid - 32 : tid;
+      const int ds = n_noise % S, dm = n_noise / S;
       const int k0 = k - s;                                  // sample index of the tile's first sample
-      int si = s, mi = c;
+      int mi = nid / S, si = nid - mi * S;
+      if (new_scene && warp == kTableWarp) mi = n_pairs;
       (void)R;
 #pragma unroll 2
       for (; mi < n_pairs; ) {
@@ -409,6 +440,127 @@ rollout_cta(const __grid_constant__ DeviceParams P) {
         if (si >= S) { si -= S; ++mi; }
       }
       if (c == 0) BRMPPI_SMEM(float, P.off_alpha)[s] = sample_alpha(P, n, (uint32_t)k, key0, key1);
+    }
+    if (new_scene && warp == kTableWarp) {
+      // The scene's obstacle tables, by the one warp that generates no noise on this tile.
+      CtaMisc* sM = BRMPPI_SMEM(CtaMisc, P.off_misc);
+      // obstacle table for phase C, in the vehicle-centred frame, ordered by how close an obstacle is
+      // to its culling threshold at the start state (the obstacles a chunk has to evaluate are then
+      // mostly the first pairs of the table), null padding behind.
+      // Obstacles 2p and 2p+1 are interleaved field by field -- (-ox, -ox'), (-oy, -oy'),
+      // (-1/rho^2, ..), (-rho^2, ..); velocities (-dt vx, ..), (-dt vy, ..) -- so that phase C
+      // loads each pair of fields as one packed f32x2 operand.
+      // Lane l holds obstacles l and l + 32 in registers and ranks them by counting over shuffles.
+      //
+      // Culling thresholds: with Dl the largest change of the centre distance per
+      // step and d_crit(alpha) = (Dl + sqrt((1 - alpha) Dl^2 + alpha^2 rho^2)) / alpha, largest at
+      // alpha_lo, the pair (obstacle, disc) has all its hinge terms exactly 0 over a chunk of L steps
+      // when it starts at distance d0 >= L Dl + 1.02 d_crit + 0.05, i.e. g0 = d0^2 - rho^2 >= thr.
+      float4* sObs = BRMPPI_SMEM(float4, P.off_obs);
+      float2* sVel = BRMPPI_SMEM(float2, P.off_vel);
+      float* sThr = BRMPPI_SMEM(float, P.off_thr);
+      const int n_obs = n_obs_in;
+      const float a_lo = P.alpha_lo;
+      const float steps = (float)P.chunk_len;
+      // (sort keys and thresholds only have to be on the safe side, not exact: MUFU approximations,
+      // with their 1e-6 relative error covered by the 1.00001 factors)
+      float dcx[kMaxDiscs], dcy[kMaxDiscs];                // disc centres at the start state
+      {
+        const float s1 = fast_sin(x0_in.z), c1 = fast_cos(x0_in.z), s2 = fast_sin(x0_in.w), c2 = fast_cos(x0_in.w);
+#pragma unroll
+        for (int j = 0; j < kMaxDiscs; ++j) {
+          dcx[j] = fmaf(P.disc_a1[j], c1, fmaf(P.disc_a2[j], c2, -P.Lh * c1));
+          dcy[j] = fmaf(P.disc_a1[j], s1, fmaf(P.disc_a2[j], s2, -P.Lh * s1));
+        }
+      }
+      const float inv_a_lo = a_lo > 0.0f ? 1.00001f * fast_rcp(a_lo) : 0.0f;
+      bool val[2], mov[2];
+      float key[2], th[2][kMaxDiscs];
+#pragma unroll
+      for (int h = 0; h < 2; ++h) {
+        val[h] = lane + 32 * h < n_obs;
+        mov[h] = val[h] && (ob_in[h][3] != 0.0f || ob_in[h][4] != 0.0f);
+        const float ox = ob_in[h][0] - x0_in.x, oy = ob_in[h][1] - x0_in.y;
+        const float rho = ob_in[h][2] + P.disc_radius;
+        // obstacle displacement per step, rounded up
+        const float spd = 1.0001f * P.dt * fast_sqrt(fmaf(ob_in[h][3], ob_in[h][3], ob_in[h][4] * ob_in[h][4]));
+        key[h] = CUDART_INF_F;
+#pragma unroll
+        for (int j = 0; j < kMaxDiscs; ++j) {
+          float t = CUDART_INF_F;
+          if (a_lo > 0.0f) {
+            const float dl = fmaf(P.dt, P.disc_speed[j], spd);
+            const float d_crit = (dl + 1.00001f * fast_sqrt(fmaf((1.0f - a_lo) * dl, dl, a_lo * a_lo * rho * rho))) * inv_a_lo;
+            const float r_cull = fmaf(steps, dl, fmaf(1.02f, d_crit, 0.05f));
+            t = fmaf(1.00001f * r_cull, r_cull, -(rho * rho));
+          }
+          th[h][j] = t;
+          if (j < P.n_discs) {
+            const float ex = dcx[j] - ox, ey = dcy[j] - oy;
+            const float margin = fmaf(ex, ex, fmaf(ey, ey, -(rho * rho))) - t;
+            key[h] = fminf(key[h], a_lo > 0.0f ? margin : fmaf(ex, ex, ey * ey));
+          }
+        }
+      }
+      int rank[2] = {0, 0};
+      for (int j = 0; j < n_obs; ++j) {
+        const float kj = __shfl_sync(0xffffffffu, (j >> 5) ? key[1] : key[0], j & 31);
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+          const int i = lane + 32 * h;
+          rank[h] += (kj < key[h] || (kj == key[h] && j < i)) ? 1 : 0;   // j sorts before i
+        }
+      }
+      unsigned moving_groups = 0u;
+#pragma unroll
+      for (int h = 0; h < 2; ++h) {
+        if (val[h]) {
+          const int dst = rank[h];
+          const float rho = ob_in[h][2] + P.disc_radius;
+          float* ob = reinterpret_cast<float*>(sObs) + (dst >> 1) * 8 + (dst & 1);
+          ob[0] = -(ob_in[h][0] - x0_in.x);
+          ob[2] = -(ob_in[h][1] - x0_in.y);
+          ob[4] = -2.0f * (0.5f / (rho * rho));
+          ob[6] = -(rho * rho);
+          float* vl = reinterpret_cast<float*>(sVel) + (dst >> 1) * 4 + (dst & 1);
+          vl[0] = -(P.dt * ob_in[h][3]);
+          vl[2] = -(P.dt * ob_in[h][4]);
+#pragma unroll
+          for (int j = 0; j < kMaxDiscs; ++j) sThr[dst * kMaxDiscs + j] = th[h][j];
+          if (mov[h]) moving_groups |= 1u << (dst / kObsGroup);
+        }
+      }
+      moving_groups = __reduce_or_sync(0xffffffffu, moving_groups);
+      for (int i = n_obs + lane; i < P.obs_padded; i += 32) {   // null obstacles: weight 0, never "near"
+        float* ob = reinterpret_cast<float*>(sObs) + (i >> 1) * 8 + (i & 1);
+        ob[0] = 0.0f; ob[2] = 0.0f; ob[4] = 0.0f; ob[6] = 0.0f;
+        float* vl = reinterpret_cast<float*>(sVel) + (i >> 1) * 4 + (i & 1);
+        vl[0] = 0.0f; vl[2] = 0.0f;
+#pragma unroll
+        for (int j = 0; j < kMaxDiscs; ++j) sThr[i * kMaxDiscs + j] = -CUDART_INF_F;
+      }
+      // super-ellipse table: rows of R(-theta) over the inflated semi-axes; null records weigh 0
+      const int n_se = n_se_in;
+      SeRecord* sSE = BRMPPI_SMEM(SeRecord, P.off_se);
+      if (lane < P.se_padded) {
+        SeRecord r = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+        if (lane < n_se) {
+          float st, ct;
+          sincosf(se_in[1].x, &st, &ct);
+          const float iax = 1.0f / (se_in[0].z + P.disc_radius), iay = 1.0f / (se_in[0].w + P.disc_radius);
+          r.ox = se_in[0].x - x0_in.x; r.oy = se_in[0].y - x0_in.y;
+          r.a11 = ct * iax; r.a12 = st * iax; r.a21 = -st * iay; r.a22 = ct * iay;
+          r.wx = P.dt * se_in[1].y; r.wy = P.dt * se_in[1].z;
+          r.e4 = se_in[1].w == 4.0f ? 1.0f : 0.0f;
+          r.half_w = 0.5f;
+        }
+        sSE[lane] = r;
+      }
+      if (lane == 0) {
+        sM->moving_groups = moving_groups;
+        sM->n_groups = n_obs > 0 ? (n_obs + kObsGroup - 1) / kObsGroup : 1;
+        sM->n_se_groups = (n_se + kSeGroup - 1) / kSeGroup;
+      }
     }
     if (new_scene) {
       CtaMisc* sM = BRMPPI_SMEM(CtaMisc, P.off_misc);
@@ -479,82 +631,6 @@ rollout_cta(const __grid_constant__ DeviceParams P) {
       } else {
         for (int cc = 0; cc < n_handoff; ++cc) mbar_arrive(smem_addr(&sM->bar_chunk[cc]));
       }
-    } else if (warp == 0) {
-      // While the chain runs its first chunk (nothing else is ready yet), warp 0 writes the scene's
-      // obstacle tables.
-      CtaMisc* sM = BRMPPI_SMEM(CtaMisc, P.off_misc);
-      if (new_scene) {
-        // obstacle table for phase C, in the vehicle-centred frame: moving obstacles first, static
-        // ones after (groups without a moving one skip the o(t) update), null padding behind.
-        // Obstacles 2p and 2p+1 are interleaved field by field -- (-ox, -ox'), (-oy, -oy'),
-        // (-1/rho^2, ..), (-rho^2, ..); velocities (-dt vx, ..), (-dt vy, ..) -- so that phase C
-        // loads each pair of fields as one packed f32x2 operand.
-        // Lane l holds obstacles l and l + 32 in registers and ranks them with two ballots.
-        float4* sObs = BRMPPI_SMEM(float4, P.off_obs);
-        float2* sVel = BRMPPI_SMEM(float2, P.off_vel);
-        float* sSpd = BRMPPI_SMEM(float, P.off_spd);
-        const int n_obs = n_obs_in;
-        const unsigned lt = (1u << lane) - 1u;
-        bool val[2], mov[2];
-        unsigned bv[2], bm[2];
-#pragma unroll
-        for (int h = 0; h < 2; ++h) {
-          val[h] = lane + 32 * h < n_obs;
-          mov[h] = val[h] && (ob_in[h][3] != 0.0f || ob_in[h][4] != 0.0f);
-          bv[h] = __ballot_sync(0xffffffffu, val[h]);
-          bm[h] = __ballot_sync(0xffffffffu, mov[h]);
-        }
-        const int nm = __popc(bm[0]) + __popc(bm[1]);
-#pragma unroll
-        for (int h = 0; h < 2; ++h) {
-          if (val[h]) {
-            const int before_m = (h ? __popc(bm[0]) : 0) + __popc(bm[h] & lt);
-            const int before_s = (h ? __popc(bv[0] & ~bm[0]) : 0) + __popc(bv[h] & ~bm[h] & lt);
-            const int dst = mov[h] ? before_m : nm + before_s;
-            const float rho = ob_in[h][2] + P.disc_radius;
-            float* ob = reinterpret_cast<float*>(sObs) + (dst >> 1) * 8 + (dst & 1);
-            ob[0] = -(ob_in[h][0] - x0_in.x);
-            ob[2] = -(ob_in[h][1] - x0_in.y);
-            ob[4] = -2.0f * (0.5f / (rho * rho));
-            ob[6] = -(rho * rho);
-            float* vl = reinterpret_cast<float*>(sVel) + (dst >> 1) * 4 + (dst & 1);
-            vl[0] = -(P.dt * ob_in[h][3]);
-            vl[2] = -(P.dt * ob_in[h][4]);
-            // displacement per step, rounded up (culling bound)
-            sSpd[dst] = 1.0001f * P.dt * sqrtf(fmaf(ob_in[h][3], ob_in[h][3], ob_in[h][4] * ob_in[h][4]));
-          }
-        }
-        for (int i = n_obs + lane; i < P.obs_padded; i += 32) {   // null obstacles: weight 0
-          float* ob = reinterpret_cast<float*>(sObs) + (i >> 1) * 8 + (i & 1);
-          ob[0] = 0.0f; ob[2] = 0.0f; ob[4] = 0.0f; ob[6] = 0.0f;
-          float* vl = reinterpret_cast<float*>(sVel) + (i >> 1) * 4 + (i & 1);
-          vl[0] = 0.0f; vl[2] = 0.0f;
-          sSpd[i] = 0.0f;
-        }
-        // super-ellipse table: rows of R(-theta) over the inflated semi-axes; null records weigh 0
-        const int n_se = n_se_in;
-        SeRecord* sSE = BRMPPI_SMEM(SeRecord, P.off_se);
-        if (lane < P.se_padded) {
-          SeRecord r = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
-          if (lane < n_se) {
-            float st, ct;
-            sincosf(se_in[1].x, &st, &ct);
-            const float iax = 1.0f / (se_in[0].z + P.disc_radius), iay = 1.0f / (se_in[0].w + P.disc_radius);
-            r.ox = se_in[0].x - x0_in.x; r.oy = se_in[0].y - x0_in.y;
-            r.a11 = ct * iax; r.a12 = st * iax; r.a21 = -st * iay; r.a22 = ct * iay;
-            r.wx = P.dt * se_in[1].y; r.wy = P.dt * se_in[1].z;
-            r.e4 = se_in[1].w == 4.0f ? 1.0f : 0.0f;
-            r.half_w = 0.5f;
-          }
-          sSE[lane] = r;
-        }
-        if (lane == 0) {
-          sM->n_moving = nm;
-          sM->n_groups = n_obs > 0 ? (n_obs + kObsGroup - 1) / kObsGroup : 1;
-          sM->n_se_groups = (n_se + kSeGroup - 1) / kSeGroup;
-        }
-      }
-      mbar_arrive(smem_addr(&sM->bar_table));    // every tile, so that the barrier's phase follows the tile count
     }
 
     // ---- phase C: barrier, barrier-rate hinge, goal / heading / hitch cost (a4-a6).  Worker thread
@@ -567,7 +643,6 @@ rollout_cta(const __grid_constant__ DeviceParams P) {
       else if (tid >= kChainFirstThread && tid - kChainFirstThread < S) { cq = P.chunks - 1; sq = tid - kChainFirstThread; }
       if (cq >= 0) {
         CtaMisc* sMb = BRMPPI_SMEM(CtaMisc, P.off_misc);
-        mbar_wait(smem_addr(&sMb->bar_table), tile_parity);
         if (tid < n_worker_items) {   // warp-uniform: the latest chunk any lane of this warp works on
           const int last = min((warp << 5) + 31, n_worker_items - 1);
           mbar_wait(smem_addr(&sMb->bar_chunk[last / S]), tile_parity);
@@ -584,10 +659,10 @@ rollout_cta(const __grid_constant__ DeviceParams P) {
       const float* pP2 = pP1 + S * TS;
       const float4* sObs = BRMPPI_SMEM(float4, P.off_obs);
       const float2* sVel = BRMPPI_SMEM(float2, P.off_vel);
-      const float* sSpd = BRMPPI_SMEM(float, P.off_spd);
       const float one_minus_alpha = 1.0f - BRMPPI_SMEM(float, P.off_alpha)[s];
       const float4 g = sM->g;
-      const int n_moving = sM->n_moving, n_groups = sM->n_groups;
+      const unsigned moving_groups = sM->moving_groups;
+      const int n_groups = sM->n_groups;
       const float2 xy = BRMPPI_SMEM(float2, P.off_xy)[c * S + s];
       double track = 0.0, bar = 0.0;
       const int n_se_groups = sM->n_se_groups;
@@ -599,23 +674,12 @@ rollout_cta(const __grid_constant__ DeviceParams P) {
         for (int grp = 1; grp < n_se_groups; ++grp)
           bar += se_group<PRECISE, ND, false>(P, pV, pP1, pP2, sSE + grp * kSeGroup, xy.x, xy.y, t0, t1, one_minus_alpha, g).bar;
       } else {
-        if (n_groups == 1 || P.chunk_len < kMinCullChunk) {
-          // a single group of obstacles, or short chunks: the culling test (a square root per
-          // obstacle and disc at every chunk start, a uniform branch per obstacle and step) costs
-          // more than it saves
-          GroupCost gc = barrier_group_nm<PRECISE, ND, true, false>(n_moving, P, pV, pP1, pP2, sObs, sVel, sSpd, xy.x, xy.y, t0, t1, one_minus_alpha, g);
-          track = gc.track; bar = gc.bar;
-          for (int grp = 1; grp < n_groups; ++grp) {
-            const int ib = grp * kObsGroup;
-            bar += barrier_group_nm<PRECISE, ND, false, false>(n_moving - ib, P, pV, pP1, pP2, sObs + ib, sVel + ib, sSpd + ib, xy.x, xy.y, t0, t1, one_minus_alpha, g).bar;
-          }
-        } else {
-          const GroupCost gc = barrier_group_nm<PRECISE, ND, true, true>(n_moving, P, pV, pP1, pP2, sObs, sVel, sSpd, xy.x, xy.y, t0, t1, one_minus_alpha, g);
-          track = gc.track; bar = gc.bar;
-          for (int grp = 1; grp < n_groups; ++grp) {
-            const int ib = grp * kObsGroup;
-            bar += barrier_group_nm<PRECISE, ND, false, true>(n_moving - ib, P, pV, pP1, pP2, sObs + ib, sVel + ib, sSpd + ib, xy.x, xy.y, t0, t1, one_minus_alpha, g).bar;
-          }
+        const float* sThr = BRMPPI_SMEM(float, P.off_thr);
+        const GroupCost gc = barrier_group_mv<PRECISE, ND, true>((moving_groups & 1u) != 0u, P, pV, pP1, pP2, sObs, sVel, sThr, xy.x, xy.y, t0, t1, one_minus_alpha, g);
+        track = gc.track; bar = gc.bar;
+        for (int grp = 1; grp < n_groups; ++grp) {
+          const int ib = grp * kObsGroup;
+          bar += barrier_group_mv<PRECISE, ND, false>(((moving_groups >> grp) & 1u) != 0u, P, pV, pP1, pP2, sObs + ib, sVel + ib, sThr + ib * kMaxDiscs, xy.x, xy.y, t0, t1, one_minus_alpha, g).bar;
         }
         for (int grp = 0; grp < n_se_groups; ++grp)
           bar += se_group<PRECISE, ND, false>(P, pV, pP1, pP2, sSE + grp * kSeGroup, xy.x, xy.y, t0, t1, one_minus_alpha, g).bar;
