@@ -78,8 +78,9 @@ typedef struct { int body; float offset; } brmppi_disc;
                                           steps fused (north_star item 2).  Default is the
                                           phase-split tile kernel.               */
 
-#define BRMPPI_FLAG_PHASE_TIMING 8u     /* persistent kernel: CTAs record nanoseconds per phase
-                                          (globaltimer); read with brmppi_get_phase_times       */
+#define BRMPPI_FLAG_PHASE_TIMING 8u     /* persistent kernel: every CTA records SM cycles per phase
+                                          (clock64, bracketed by the globaltimer for the conversion
+                                          to time); read with brmppi_get_phase_times            */
 #define BRMPPI_FLAG_NO_CULL 16u         /* evaluate every (obstacle, disc, step) even where the
                                           hinge is provably zero; same results  */
 
@@ -187,11 +188,13 @@ int brmppi_get_hitch_filter(brmppi_ctx* ctx, int scene, float u_ref[2], int* sta
  * reps + 2.  1 <= reps <= 4096. */
 int brmppi_time_kernels(brmppi_ctx* ctx, int reps, float out_ms[2]);
 
-/* Per-phase device time of the LAST rollout launch, from the kernel's own globaltimer stamps
- * (needs BRMPPI_FLAG_PHASE_TIMING, else BRMPPI_ERR_NOT_READY; default kernel only).  out_us[0..6] =
- * mean over CTAs of the microseconds spent in: scene prologue, A noise, B chain, C cost,
- * D reduction, E weighted control sums, partial write-out; out_us[7] = first CTA start to last
- * CTA end.  Synchronises. */
+/* Per-phase device time of the LAST rollout launch, from the kernel's own clock64 stamps converted
+ * with each CTA's lifetime on the globaltimer (needs BRMPPI_FLAG_PHASE_TIMING, else
+ * BRMPPI_ERR_NOT_READY; default kernel only).  out_us[0..6] = mean over CTAs of the microseconds
+ * spent in: scene prologue, A noise (+ obstacle tables), the Euler chain (which runs UNDER slot 3 on
+ * the CTA's last four warps; not part of the sum), cost phase from the end of A to the end of the
+ * last chunk, D reduction, E weighted control sums, partial write-out; out_us[7] = first CTA start to
+ * last CTA end.  Synchronises. */
 int brmppi_get_phase_times(brmppi_ctx* ctx, float out_us[8]);
 
 /* Number of kernel launches this context has enqueued so far (graph replays count the kernels
@@ -209,18 +212,20 @@ const char* brmppi_strerror(int status);
 int brmppi_debug_philox(void* cuda_stream, unsigned long long seed, unsigned int n, int K, int T,
                         unsigned int tag, unsigned int* dev_out);
 
-/* The perturbed, clamped controls and alpha the kernels draw for (params, n, nominal U): writes
- * u[K][T][2] and alpha[K] (DEVICE pointers; either may be NULL).  U_nominal: HOST T*2 or NULL.
- * Same device functions as the rollout kernels.  Synchronises. */
-int brmppi_debug_sample_controls(void* cuda_stream, const brmppi_params* p, unsigned int n,
-                                 const float* U_nominal, float* dev_u, float* dev_alpha);
+/* Arbitrary Philox4x32-10 blocks: out[i] = P(ctr[i]; key[i]) for i < n, through the generator the
+ * rollout kernels use (use_curand = 0) or through the CUDA toolkit's own raw device function
+ * curand_Philox4x32_10(uint4, uint2) (use_curand = 1) -- the library pin of the generator
+ * (SURVEY §8(c)).  dev_ctr [n][4], dev_key [n][2], dev_out [n][4]: DEVICE pointers, 16-byte (key: 8-byte)
+ * aligned.  Synchronises. */
+int brmppi_debug_philox_raw(void* cuda_stream, int n, const unsigned int* dev_ctr, const unsigned int* dev_key,
+                            int use_curand, unsigned int* dev_out);
 
-/* Issue-rate micro-benchmarks for the roofline denominator (DESIGN.md §6): thread-instructions
- * per clock per SM achieved by dependent-chain-free streams of FFMA, LOP3/IADD3 (ALU pipe),
- * MUFU (XU pipe) and the FFMA+ALU mix, plus the SM count and the clock measured in-kernel.
- * out[0..7] = {ffma, alu, mufu, mix (ffma+lop3 interleaved), imad_wide, n_sms, sm_mhz of an idle SM,
- * sm_mhz seen while the FFMA kernel ran}.  Rates are whole-kernel: instructions per SM / (first
- * block start .. last block end on the globaltimer, converted with the in-kernel clock). */
+/* The perturbed, clamped controls and alpha the kernels draw for (params, n, nominal U): writes
+ * u[K][T][2] and alpha[K] (DEVICE pointers; either may be NULL).  dev_U_nominal: DEVICE [T][2].
+ * Same device functions as the rollout kernels.  Nothing is allocated.  Synchronises. */
+int brmppi_debug_sample_controls(void* cuda_stream, const brmppi_params* p, unsigned int n,
+                                 const float* dev_U_nominal, float* dev_u, float* dev_alpha);
+
 /* Hitch-angle stabiliser on its own, for n independent (state, reference control) pairs
  * (Sec. V-D).  With beta = wrap(psi1 - psi2), s = sign(beta) (+1 at 0) and
  *   h_h = hitch_max - hitch_kappa |v| - |beta|                                          eq. (18)
@@ -231,10 +236,14 @@ int brmppi_debug_sample_controls(void* cuda_stream, const brmppi_params* p, unsi
  *        s.t. c(u_ref) + grad c(u_ref) . (u - u_ref) >= 0,  v_min <= v <= v_max,  delta_min <= delta <= delta_max.
  * x: HOST [n][4] states (x, y, psi1, psi2); u_ref: HOST [n][2]; u_out: HOST [n][2]; status_out: HOST
  * [n] or NULL, values as in brmppi_get_hitch_filter.  Uses p->dt, L1, L2, Lh, the control box and the
- * hitch_* fields (hitch_filter itself is ignored).  Allocates and frees its own device scratch;
- * synchronises the stream.  n = 0 is a no-op. */
+ * hitch_* fields (hitch_filter itself is ignored).  dev_scratch: DEVICE pointer to >=
+ * brmppi_hitch_filter_scratch_bytes(n) bytes owned by the caller (staging for the host arrays; the
+ * library allocates no device memory; BRMPPI_ERR_WORKSPACE_TOO_SMALL if it is too small).
+ * Synchronises the stream.  n = 0 is a no-op. */
+size_t brmppi_hitch_filter_scratch_bytes(int n);
 int brmppi_hitch_filter(void* cuda_stream, const brmppi_params* p, int n, const float* x,
-                        const float* u_ref, float* u_out, int* status_out);
+                        const float* u_ref, float* u_out, int* status_out, void* dev_scratch,
+                        size_t scratch_bytes);
 
 #define BRMPPI_PROJECT_MAX_NO 8
 /* Closed-form projection of BR-MPPI, eq. (11)-(12), for n independent problems:
@@ -242,17 +251,30 @@ int brmppi_hitch_filter(void* cuda_stream, const brmppi_params* p, int n, const 
  *   z* = M^-1 [ p - A^T (A M^-1 A^T)^-1 (A M^-1 p - b) ],  M = W + rho I,  p = W z_des + rho/2 (z_hi + z_lo),
  * with z = [u_proj (2), u_proj^alpha (n_o)], d = 2 + n_o, 1 <= n_o <= BRMPPI_PROJECT_MAX_NO.
  * A: [n][n_o][d] row-major; b: [n][n_o]; z_des: [n][d]; z_out: [n][d] -- HOST pointers if
- * device_ptrs == 0 (copied in and out through scratch the call allocates and frees), DEVICE pointers,
- * 16-byte aligned, if device_ptrs == 1 (nothing is allocated; asynchronous on the stream).
+ * device_ptrs == 0 (copied in and out through dev_scratch, a DEVICE buffer of >=
+ * brmppi_project_scratch_bytes(n, n_o) bytes owned by the caller; page-locked host arrays copy at
+ * full PCIe rate, pageable ones several times slower; synchronises), DEVICE pointers, 16-byte
+ * aligned for the bulk-copy path, if device_ptrs == 1 (dev_scratch unused, may be NULL; asynchronous
+ * on the stream).  The library allocates no device memory either way.
  * w (the diagonal of W, all > 0), z_lo, z_hi: HOST [d], shared by all problems; rho >= 0.
  * A must have full row rank (A M^-1 A^T is factorised by Cholesky without pivoting); a rank-deficient
  * problem yields non-finite values in its own z_out row only.  How (9) builds A and b inside a rollout
  * is not part of this call.  n = 0 is a no-op. */
+size_t brmppi_project_scratch_bytes(int n, int n_o);
 int brmppi_project(void* cuda_stream, int n, int n_o, const float* A, const float* b, const float* z_des,
                    const float* w, float rho, const float* z_lo, const float* z_hi, float* z_out,
-                   int device_ptrs);
+                   int device_ptrs, void* dev_scratch, size_t scratch_bytes);
 
-int brmppi_measure_peaks(void* cuda_stream, float out[8]);
+/* Issue-rate micro-benchmarks for the roofline denominator (DESIGN.md §6): thread-instructions
+ * per clock per SM achieved by dependent-chain-free streams of FFMA, LOP3/IADD3 (ALU pipe),
+ * MUFU (XU pipe) and the FFMA+ALU mix, plus the SM count and the clock measured in-kernel.
+ * out[0..7] = {ffma, alu, mufu, mix (ffma+lop3 interleaved), imad_wide, n_sms, sm_mhz of an idle SM,
+ * sm_mhz seen while the FFMA kernel ran}.  Rates are whole-kernel: instructions per SM / (first
+ * block start .. last block end on the globaltimer, converted with the in-kernel clock).
+ * dev_scratch: DEVICE pointer to >= brmppi_measure_peaks_scratch_bytes() bytes owned by the caller
+ * (the library allocates no device memory).  Synchronises. */
+size_t brmppi_measure_peaks_scratch_bytes(void);
+int brmppi_measure_peaks(void* cuda_stream, void* dev_scratch, size_t scratch_bytes, float out[8]);
 
 #ifdef __cplusplus
 }

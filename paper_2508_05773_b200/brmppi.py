@@ -4,7 +4,6 @@ PyTorch provides device memory (the workspace tensor) and the CUDA stream; every
 path runs in libbrmppi.so's kernels.  There is no CPU fallback: if the CUDA library is missing or
 no device is present, construction raises."""
 import ctypes as C
-import os
 
 import numpy as np
 
@@ -28,6 +27,8 @@ EXPORTS = [
     "brmppi_get_state", "brmppi_get_obstacles", "brmppi_get_costs", "brmppi_get_final_states",
     "brmppi_get_diag", "brmppi_get_phase_times", "brmppi_time_kernels", "brmppi_launch_count", "brmppi_strerror", "brmppi_debug_philox",
     "brmppi_debug_sample_controls", "brmppi_measure_peaks", "brmppi_get_hitch_filter", "brmppi_hitch_filter", "brmppi_project",
+    "brmppi_debug_philox_raw", "brmppi_hitch_filter_scratch_bytes", "brmppi_project_scratch_bytes",
+    "brmppi_measure_peaks_scratch_bytes",
 ]
 
 
@@ -81,8 +82,7 @@ def lib():
     """Load libbrmppi.so (building it in-tree first if its sources are newer)."""
     global _lib
     if _lib is None:
-        # BRMPPI_LIB: load a pre-built variant of the library (kernel-tuning experiments)
-        path = os.environ.get("BRMPPI_LIB") or _build.build()
+        path = _build.build()
         L = C.CDLL(path)
         vp = C.c_void_p
         L.brmppi_workspace_bytes.argtypes = [C.POINTER(CParams)]
@@ -113,11 +113,18 @@ def lib():
         L.brmppi_strerror.argtypes = [C.c_int]
         L.brmppi_strerror.restype = C.c_char_p
         L.brmppi_debug_philox.argtypes = [vp, C.c_ulonglong, C.c_uint, C.c_int, C.c_int, C.c_uint, vp]
-        L.brmppi_debug_sample_controls.argtypes = [vp, C.POINTER(CParams), C.c_uint, _fp, vp, vp]
-        L.brmppi_measure_peaks.argtypes = [vp, _fp]
-        L.brmppi_project.argtypes = [vp, C.c_int, C.c_int, vp, vp, vp, _fp, C.c_float, _fp, _fp, vp, C.c_int]
+        L.brmppi_debug_philox_raw.argtypes = [vp, C.c_int, vp, vp, C.c_int, vp]
+        L.brmppi_debug_sample_controls.argtypes = [vp, C.POINTER(CParams), C.c_uint, vp, vp, vp]
+        L.brmppi_measure_peaks_scratch_bytes.argtypes = []
+        L.brmppi_measure_peaks_scratch_bytes.restype = C.c_size_t
+        L.brmppi_measure_peaks.argtypes = [vp, vp, C.c_size_t, _fp]
+        L.brmppi_project_scratch_bytes.argtypes = [C.c_int, C.c_int]
+        L.brmppi_project_scratch_bytes.restype = C.c_size_t
+        L.brmppi_project.argtypes = [vp, C.c_int, C.c_int, vp, vp, vp, _fp, C.c_float, _fp, _fp, vp, C.c_int, vp, C.c_size_t]
         L.brmppi_get_hitch_filter.argtypes = [vp, C.c_int, _fp, C.POINTER(C.c_int)]
-        L.brmppi_hitch_filter.argtypes = [vp, C.POINTER(CParams), C.c_int, _fp, _fp, _fp, C.POINTER(C.c_int)]
+        L.brmppi_hitch_filter_scratch_bytes.argtypes = [C.c_int]
+        L.brmppi_hitch_filter_scratch_bytes.restype = C.c_size_t
+        L.brmppi_hitch_filter.argtypes = [vp, C.POINTER(CParams), C.c_int, _fp, _fp, _fp, C.POINTER(C.c_int), vp, C.c_size_t]
         _lib = L
     return _lib
 
@@ -326,17 +333,41 @@ def debug_philox(seed, n, K, T, tag=0):
     return out.cpu().numpy().view(np.uint32).reshape(K, T, 4)
 
 
+def debug_philox_raw(ctr, key, use_curand=False):
+    """Philox4x32-10 blocks for arbitrary (counter [n][4], key [n][2]) uint32 arrays: through the library's
+    generator, or through the toolkit's raw curand_Philox4x32_10 device function.  uint32 [n][4]."""
+    import torch
+    ctr = np.ascontiguousarray(ctr, dtype=np.uint32).reshape(-1, 4)
+    key = np.ascontiguousarray(key, dtype=np.uint32).reshape(-1, 2)
+    n = ctr.shape[0]
+    assert key.shape[0] == n
+    dc = torch.from_numpy(ctr.view(np.int32)).cuda()
+    dk = torch.from_numpy(key.view(np.int32)).cuda()
+    out = torch.empty((max(n, 1), 4), dtype=torch.int32, device="cuda")
+    st = torch.cuda.current_stream()
+    st.synchronize()
+    _check(lib().brmppi_debug_philox_raw(C.c_void_p(st.cuda_stream), n, C.c_void_p(dc.data_ptr()), C.c_void_p(dk.data_ptr()),
+                                         1 if use_curand else 0, C.c_void_p(out.data_ptr())))
+    return out[:n].cpu().numpy().view(np.uint32)
+
+
 def debug_sample_controls(params, n, U_nominal=None, flags=0):
     """Perturbed, clamped controls u[K][T][2] and alpha[K] exactly as the kernels draw them."""
     import torch
     cp = make_cparams(params, 1, 0, flags)
     u = torch.empty(params.K * params.T * 2, dtype=torch.float32, device="cuda")
     a = torch.empty(params.K, dtype=torch.float32, device="cuda")
+    Un = torch.from_numpy(_f32(np.zeros((params.T, 2)) if U_nominal is None else U_nominal, (params.T, 2))).cuda()
     st = torch.cuda.current_stream()
-    Un = None if U_nominal is None else _p(_f32(U_nominal, (params.T, 2)))
-    _check(lib().brmppi_debug_sample_controls(C.c_void_p(st.cuda_stream), C.byref(cp), int(n), Un,
+    st.synchronize()
+    _check(lib().brmppi_debug_sample_controls(C.c_void_p(st.cuda_stream), C.byref(cp), int(n), C.c_void_p(Un.data_ptr()),
                                               C.c_void_p(u.data_ptr()), C.c_void_p(a.data_ptr())))
     return u.cpu().numpy().reshape(params.K, params.T, 2), a.cpu().numpy()
+
+
+def _scratch(nbytes):
+    import torch
+    return torch.empty(max(int(nbytes), 1), dtype=torch.uint8, device="cuda")
 
 
 def hitch_filter(params, x, u_ref):
@@ -349,41 +380,63 @@ def hitch_filter(params, x, u_ref):
     cp = make_cparams(params, 1, 0, 0)
     u = np.zeros((n, 2), dtype=np.float32)
     status = np.zeros(n, dtype=np.int32)
+    nb = lib().brmppi_hitch_filter_scratch_bytes(n)
+    scratch = _scratch(nb)
     st = torch.cuda.current_stream()
+    st.synchronize()
     _check(lib().brmppi_hitch_filter(C.c_void_p(st.cuda_stream), C.byref(cp), n, _p(x), _p(r), _p(u),
-                                     status.ctypes.data_as(C.POINTER(C.c_int))))
+                                     status.ctypes.data_as(C.POINTER(C.c_int)), C.c_void_p(scratch.data_ptr()), C.c_size_t(nb)))
     return u, status
 
 
-def project(A, b, z_des, w, rho, z_lo, z_hi):
-    """Closed-form projection (12) for a batch.  numpy arrays -> HOST-pointer call, returns numpy [n][d];
-    torch CUDA tensors (float32, contiguous) -> DEVICE-pointer call on the current stream, returns a tensor."""
+def project(A, b, z_des, w, rho, z_lo, z_hi, out=None, scratch=None):
+    """Closed-form projection (12) for a batch.  numpy arrays (or CPU torch tensors, e.g. page-locked ones) ->
+    HOST-pointer call through a caller-owned device scratch, returns numpy [n][d]; torch CUDA tensors (float32,
+    contiguous) -> DEVICE-pointer call on the current stream, returns a tensor."""
     import torch
     st = torch.cuda.current_stream()
-    on_device = isinstance(A, torch.Tensor)
+    on_device = isinstance(A, torch.Tensor) and A.is_cuda
     n, n_o, d = A.shape
     w, z_lo, z_hi = _f32(w, (d,)), _f32(z_lo, (d,)), _f32(z_hi, (d,))
     if on_device:
         for t in (A, b, z_des):
             assert t.is_cuda and t.dtype == torch.float32 and t.is_contiguous()
-        out = torch.empty((n, d), dtype=torch.float32, device=A.device)
+        if out is None:
+            out = torch.empty((n, d), dtype=torch.float32, device=A.device)
         ptr = lambda t: C.c_void_p(t.data_ptr())
         _check(lib().brmppi_project(C.c_void_p(st.cuda_stream), n, n_o, ptr(A), ptr(b), ptr(z_des), _p(w),
-                                    float(rho), _p(z_lo), _p(z_hi), ptr(out), 1))
+                                    float(rho), _p(z_lo), _p(z_hi), ptr(out), 1, None, 0))
         return out
-    A, b, z_des = _f32(A), _f32(b, (n, n_o)), _f32(z_des, (n, d))
-    out = np.zeros((n, d), dtype=np.float32)
-    ptr = lambda a: C.c_void_p(a.ctypes.data)
+    if isinstance(A, torch.Tensor):            # CPU tensors (page-locked staging): no copies on the way in
+        for t in (A, b, z_des):
+            assert t.dtype == torch.float32 and t.is_contiguous()
+        ptr = lambda t: C.c_void_p(t.data_ptr())
+        if out is None:
+            out = torch.empty((n, d), dtype=torch.float32).pin_memory()
+        ret = out.numpy()
+    else:
+        A, b, z_des = _f32(A), _f32(b, (n, n_o)), _f32(z_des, (n, d))
+        ptr = lambda a: C.c_void_p(a.ctypes.data)
+        out = np.zeros((n, d), dtype=np.float32) if out is None else out
+        ret = out
+    nb = lib().brmppi_project_scratch_bytes(n, n_o)
+    if scratch is None:
+        scratch = _scratch(nb)
+        st.synchronize()
     _check(lib().brmppi_project(C.c_void_p(st.cuda_stream), n, n_o, ptr(A), ptr(b), ptr(z_des), _p(w),
-                                float(rho), _p(z_lo), _p(z_hi), ptr(out), 0))
-    return out
+                                float(rho), _p(z_lo), _p(z_hi), ptr(out), 0, C.c_void_p(scratch.data_ptr()),
+                                C.c_size_t(scratch.numel())))
+    return ret
 
 
 def measure_peaks():
     import torch
     out = np.zeros(8, dtype=np.float32)
+    nb = lib().brmppi_measure_peaks_scratch_bytes()
+    scratch = _scratch(nb)
     st = torch.cuda.current_stream()
-    _check(lib().brmppi_measure_peaks(C.c_void_p(st.cuda_stream), _p(out)))
+    st.synchronize()
+    _check(lib().brmppi_measure_peaks(C.c_void_p(st.cuda_stream), C.c_void_p(scratch.data_ptr()), C.c_size_t(nb), _p(out)))
     return dict(ffma=float(out[0]), alu=float(out[1]), mufu=float(out[2]), mix=float(out[3]),
                 imad_wide=float(out[4]), n_sms=int(out[5]), sm_mhz=float(out[6]),
                 sm_mhz_under_ffma=float(out[7]))

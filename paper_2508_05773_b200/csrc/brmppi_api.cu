@@ -100,10 +100,6 @@ struct Plan {
 // SM count of the current device (the persistent kernel launches one CTA per SM); 148 -- a B200 --
 // when no device is visible, so that brmppi_workspace_bytes still answers on a CPU-only box.
 int device_sm_count() {
-  if (const char* e = getenv("BRMPPI_NUM_SMS")) {   // tuning knob for sweeps
-    const int v = atoi(e);
-    if (v >= 1) return v;
-  }
   int dev = 0, n = 0;
   if (cudaGetDevice(&dev) == cudaSuccess &&
       cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && n > 0)
@@ -340,11 +336,10 @@ int brmppi_create(const brmppi_params* p, void* dev_workspace, size_t workspace_
     e = configure_rollout_cta((p->flags & BRMPPI_FLAG_PRECISE_MATH) != 0, p->n_discs, c->smem_rollout);
   } else {
     c->smem_rollout = rollout_thread_smem_bytes(d);
-    if (c->smem_rollout > 48 * 1024) {
-      e = cudaFuncSetAttribute(rollout_thread_per_sample<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_rollout);
-      if (e == cudaSuccess)
-        e = cudaFuncSetAttribute(rollout_thread_per_sample<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_rollout);
-    }
+    // per function and device, not per context: always the opt-in maximum, never lowered
+    e = cudaFuncSetAttribute(rollout_thread_per_sample<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)prop.sharedMemPerBlockOptin);
+    if (e == cudaSuccess)
+      e = cudaFuncSetAttribute(rollout_thread_per_sample<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)prop.sharedMemPerBlockOptin);
   }
   if (e == cudaSuccess && c->smem_update > 48 * 1024)
     e = cudaFuncSetAttribute(merge_update, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_update);
@@ -700,9 +695,25 @@ int brmppi_debug_philox(void* cuda_stream, unsigned long long seed, unsigned int
   return BRMPPI_OK;
 }
 
+int brmppi_debug_philox_raw(void* cuda_stream, int n, const unsigned int* dev_ctr, const unsigned int* dev_key,
+                            int use_curand, unsigned int* dev_out) {
+  if (n < 0 || (use_curand != 0 && use_curand != 1)) return BRMPPI_ERR_INVALID_ARG;
+  if (n == 0) return BRMPPI_OK;
+  if (!dev_ctr || !dev_key || !dev_out) return BRMPPI_ERR_NULL;
+  cudaStream_t s = (cudaStream_t)cuda_stream;
+  const unsigned grid = (unsigned)((n + 255) / 256);
+  if (use_curand)
+    debug_philox_raw<true><<<grid, 256, 0, s>>>(n, (const uint4*)dev_ctr, (const uint2*)dev_key, (uint4*)dev_out);
+  else
+    debug_philox_raw<false><<<grid, 256, 0, s>>>(n, (const uint4*)dev_ctr, (const uint2*)dev_key, (uint4*)dev_out);
+  CU(cudaGetLastError());
+  CU(cudaStreamSynchronize(s));
+  return BRMPPI_OK;
+}
+
 int brmppi_debug_sample_controls(void* cuda_stream, const brmppi_params* p, unsigned int n,
-                                 const float* U_nominal, float* dev_u, float* dev_alpha) {
-  if (!p) return BRMPPI_ERR_NULL;
+                                 const float* dev_U_nominal, float* dev_u, float* dev_alpha) {
+  if (!p || !dev_U_nominal) return BRMPPI_ERR_NULL;
   if (!params_valid(p)) return BRMPPI_ERR_INVALID_ARG;
   cudaStream_t s = (cudaStream_t)cuda_stream;
   DeviceParams d;
@@ -712,22 +723,14 @@ int brmppi_debug_sample_controls(void* cuda_stream, const brmppi_params* p, unsi
   d.sigma_v = p->sigma_v; d.sigma_delta = p->sigma_delta;
   d.alpha_lo = p->alpha_lo; d.alpha_span = p->alpha_hi - p->alpha_lo;
   d.key0 = (uint32_t)(p->seed & 0xFFFFFFFFull); d.key1 = (uint32_t)(p->seed >> 32);
-  float2* dU = nullptr;
-  CU(cudaMalloc((void**)&dU, sizeof(float2) * (size_t)p->T));   // debug-only scratch
-  cudaError_t e = U_nominal ? cudaMemcpyAsync(dU, U_nominal, sizeof(float2) * (size_t)p->T, cudaMemcpyHostToDevice, s)
-                            : cudaMemsetAsync(dU, 0, sizeof(float2) * (size_t)p->T, s);
-  if (e == cudaSuccess) {
-    const size_t total = (size_t)p->K * p->T;
-    const unsigned grid = (unsigned)((total + 255) / 256);
-    if (p->flags & BRMPPI_FLAG_PRECISE_MATH)
-      debug_sample_controls<true><<<grid, 256, 0, s>>>(d, n, dU, (float2*)dev_u, dev_alpha);
-    else
-      debug_sample_controls<false><<<grid, 256, 0, s>>>(d, n, dU, (float2*)dev_u, dev_alpha);
-    e = cudaGetLastError();
-  }
-  if (e == cudaSuccess) e = cudaStreamSynchronize(s);
-  cudaFree(dU);
-  if (e != cudaSuccess) return cuda_fail(e);
+  const size_t total = (size_t)p->K * p->T;
+  const unsigned grid = (unsigned)((total + 255) / 256);
+  if (p->flags & BRMPPI_FLAG_PRECISE_MATH)
+    debug_sample_controls<true><<<grid, 256, 0, s>>>(d, n, (const float2*)dev_U_nominal, (float2*)dev_u, dev_alpha);
+  else
+    debug_sample_controls<false><<<grid, 256, 0, s>>>(d, n, (const float2*)dev_U_nominal, (float2*)dev_u, dev_alpha);
+  CU(cudaGetLastError());
+  CU(cudaStreamSynchronize(s));
   return BRMPPI_OK;
 }
 
@@ -743,8 +746,11 @@ int brmppi_get_hitch_filter(brmppi_ctx* c, int scene, float u_ref[2], int* statu
   return BRMPPI_OK;
 }
 
+size_t brmppi_hitch_filter_scratch_bytes(int n) { return n > 0 ? (size_t)n * 36 + 256 : 0; }
+
 int brmppi_hitch_filter(void* cuda_stream, const brmppi_params* p, int n, const float* x,
-                        const float* u_ref, float* u_out, int* status_out) {
+                        const float* u_ref, float* u_out, int* status_out, void* dev_scratch,
+                        size_t scratch_bytes) {
   if (!p) return BRMPPI_ERR_NULL;
   if (n < 0) return BRMPPI_ERR_INVALID_ARG;
   const float f[] = {p->dt, p->L1, p->L2, p->Lh, p->v_min, p->v_max, p->delta_min, p->delta_max};
@@ -752,7 +758,8 @@ int brmppi_hitch_filter(void* cuda_stream, const brmppi_params* p, int n, const 
       p->v_min > p->v_max || p->delta_min > p->delta_max || p->delta_min <= -1.5f || p->delta_max >= 1.5f)
     return BRMPPI_ERR_INVALID_ARG;
   if (n == 0) return BRMPPI_OK;
-  if (!x || !u_ref || !u_out) return BRMPPI_ERR_NULL;
+  if (!x || !u_ref || !u_out || !dev_scratch) return BRMPPI_ERR_NULL;
+  if (scratch_bytes < brmppi_hitch_filter_scratch_bytes(n)) return BRMPPI_ERR_WORKSPACE_TOO_SMALL;
   cudaStream_t s = (cudaStream_t)cuda_stream;
   DeviceParams d;
   memset(&d, 0, sizeof(d));
@@ -761,31 +768,32 @@ int brmppi_hitch_filter(void* cuda_stream, const brmppi_params* p, int n, const 
   d.v_min = p->v_min; d.v_max = p->v_max; d.delta_min = p->delta_min; d.delta_max = p->delta_max;
   d.hitch_max = p->hitch_max; d.hitch_kappa = p->hitch_kappa; d.hitch_alpha = p->hitch_alpha;
   d.hitch_qv = p->hitch_qv; d.hitch_qdelta = p->hitch_qdelta;
-  // one scratch allocation: x [n][4] | u_ref [n][2] | u_out [n][2] | status [n]
+  // the caller's scratch: x [n][4] | u_ref [n][2] | u_out [n][2] | status [n]
   const size_t N = (size_t)n;
-  unsigned char* buf = nullptr;
-  CU(cudaMalloc((void**)&buf, N * 36));
+  unsigned char* buf = (unsigned char*)align_up((size_t)(uintptr_t)dev_scratch, 256);
   float4* dx = (float4*)buf;
   float2* dr = (float2*)(buf + N * 16);
   float2* du = (float2*)(buf + N * 24);
   int* ds = (int*)(buf + N * 32);
-  cudaError_t e = cudaMemcpyAsync(dx, x, N * 16, cudaMemcpyHostToDevice, s);
-  if (e == cudaSuccess) e = cudaMemcpyAsync(dr, u_ref, N * 8, cudaMemcpyHostToDevice, s);
-  if (e == cudaSuccess) {
-    hitch_filter_batch<<<(unsigned)((N + 127) / 128), 128, 0, s>>>(d, n, dx, dr, du, ds);
-    e = cudaGetLastError();
-  }
-  if (e == cudaSuccess) e = cudaMemcpyAsync(u_out, du, N * 8, cudaMemcpyDeviceToHost, s);
-  if (e == cudaSuccess && status_out) e = cudaMemcpyAsync(status_out, ds, N * 4, cudaMemcpyDeviceToHost, s);
-  if (e == cudaSuccess) e = cudaStreamSynchronize(s);
-  cudaFree(buf);
-  if (e != cudaSuccess) return cuda_fail(e);
+  CU(cudaMemcpyAsync(dx, x, N * 16, cudaMemcpyHostToDevice, s));
+  CU(cudaMemcpyAsync(dr, u_ref, N * 8, cudaMemcpyHostToDevice, s));
+  hitch_filter_batch<<<(unsigned)((N + 127) / 128), 128, 0, s>>>(d, n, dx, dr, du, ds);
+  CU(cudaGetLastError());
+  CU(cudaMemcpyAsync(u_out, du, N * 8, cudaMemcpyDeviceToHost, s));
+  if (status_out) CU(cudaMemcpyAsync(status_out, ds, N * 4, cudaMemcpyDeviceToHost, s));
+  CU(cudaStreamSynchronize(s));
   return BRMPPI_OK;
+}
+
+size_t brmppi_project_scratch_bytes(int n, int n_o) {
+  if (n <= 0 || n_o < 1 || n_o > BRMPPI_PROJECT_MAX_NO) return 0;
+  const size_t N = (size_t)n, d = (size_t)n_o + 2;
+  return sizeof(float) * (N * n_o * d + N * n_o + 2 * N * d + 16) + 256;
 }
 
 int brmppi_project(void* cuda_stream, int n, int n_o, const float* A, const float* b, const float* z_des,
                    const float* w, float rho, const float* z_lo, const float* z_hi, float* z_out,
-                   int device_ptrs) {
+                   int device_ptrs, void* dev_scratch, size_t scratch_bytes) {
   if (n < 0 || n_o < 1 || n_o > BRMPPI_PROJECT_MAX_NO || (device_ptrs != 0 && device_ptrs != 1))
     return BRMPPI_ERR_INVALID_ARG;
   if (!w || !z_lo || !z_hi) return BRMPPI_ERR_NULL;
@@ -806,38 +814,38 @@ int brmppi_project(void* cuda_stream, int n, int n_o, const float* A, const floa
     CU(launch_project_dyn(n_o, n, A, b, z_des, pc, z_out, s));
     return BRMPPI_OK;
   }
+  if (!dev_scratch) return BRMPPI_ERR_NULL;
+  if (scratch_bytes < brmppi_project_scratch_bytes(n, n_o)) return BRMPPI_ERR_WORKSPACE_TOO_SMALL;
   const size_t N = (size_t)n, nA = N * n_o * d, nb = N * n_o, nz = N * d;
-  float* buf = nullptr;
-  CU(cudaMalloc((void**)&buf, sizeof(float) * (nA + nb + 2 * nz + 12)));
-  // sections kept 16-byte aligned
+  // sections of the caller's scratch, kept 16-byte aligned
   auto up4 = [](size_t x) { return (x + 3) & ~(size_t)3; };
-  float* dA = buf;
+  float* dA = (float*)align_up((size_t)(uintptr_t)dev_scratch, 256);
   float* db = dA + up4(nA);
   float* dz = db + up4(nb);
   float* dout = dz + up4(nz);
-  cudaError_t e = cudaMemcpyAsync(dA, A, sizeof(float) * nA, cudaMemcpyHostToDevice, s);
-  if (e == cudaSuccess) e = cudaMemcpyAsync(db, b, sizeof(float) * nb, cudaMemcpyHostToDevice, s);
-  if (e == cudaSuccess) e = cudaMemcpyAsync(dz, z_des, sizeof(float) * nz, cudaMemcpyHostToDevice, s);
-  if (e == cudaSuccess) e = launch_project_dyn(n_o, n, dA, db, dz, pc, dout, s);
-  if (e == cudaSuccess) e = cudaMemcpyAsync(z_out, dout, sizeof(float) * nz, cudaMemcpyDeviceToHost, s);
-  if (e == cudaSuccess) e = cudaStreamSynchronize(s);
-  cudaFree(buf);
-  if (e != cudaSuccess) return cuda_fail(e);
+  CU(cudaMemcpyAsync(dA, A, sizeof(float) * nA, cudaMemcpyHostToDevice, s));
+  CU(cudaMemcpyAsync(db, b, sizeof(float) * nb, cudaMemcpyHostToDevice, s));
+  CU(cudaMemcpyAsync(dz, z_des, sizeof(float) * nz, cudaMemcpyHostToDevice, s));
+  CU(launch_project_dyn(n_o, n, dA, db, dz, pc, dout, s));
+  CU(cudaMemcpyAsync(z_out, dout, sizeof(float) * nz, cudaMemcpyDeviceToHost, s));
+  CU(cudaStreamSynchronize(s));
   return BRMPPI_OK;
 }
 
-int brmppi_measure_peaks(void* cuda_stream, float out[8]) {
-  if (!out) return BRMPPI_ERR_NULL;
+size_t brmppi_measure_peaks_scratch_bytes(void) { return sizeof(long long) * 3 * 4 * 1024 + 256; }
+
+int brmppi_measure_peaks(void* cuda_stream, void* dev_scratch, size_t scratch_bytes, float out[8]) {
+  if (!out || !dev_scratch) return BRMPPI_ERR_NULL;
+  if (scratch_bytes < brmppi_measure_peaks_scratch_bytes()) return BRMPPI_ERR_WORKSPACE_TOO_SMALL;
   cudaStream_t s = (cudaStream_t)cuda_stream;
   int dev = 0;
   CU(cudaGetDevice(&dev));
   cudaDeviceProp prop;
   CU(cudaGetDeviceProperties(&prop, dev));
   const int blocks = prop.multiProcessorCount * 4;   // 4 x 256 threads resident per SM, one wave
-  long long* spans = nullptr;
-  float* sink = nullptr;
-  CU(cudaMalloc((void**)&spans, sizeof(long long) * 3 * (size_t)blocks));
-  CU(cudaMalloc((void**)&sink, sizeof(float) * 4));
+  if (blocks > 4 * 1024 - 8) return BRMPPI_ERR_INVALID_ARG;
+  float* sink = (float*)align_up((size_t)(uintptr_t)dev_scratch, 256);   // 4 floats, then the spans
+  long long* spans = (long long*)(sink + 8);
   long long* h = (long long*)malloc(sizeof(long long) * 3 * (size_t)blocks);
   double wall_ns[5] = {0, 0, 0, 0, 0};
   cudaError_t e = cudaSuccess;
@@ -882,8 +890,6 @@ int brmppi_measure_peaks(void* cuda_stream, float out[8]) {
     out[6] = mhz[0];
   }
   free(h);
-  cudaFree(spans);
-  cudaFree(sink);
   if (e != cudaSuccess) return cuda_fail(e);
   return BRMPPI_OK;
 }

@@ -10,6 +10,8 @@
 // path or on its position.  432 B and ~1 k instructions per problem at N_o = 8: HBM-bound on paper
 // (DESIGN.md 6.9).
 #pragma once
+
+#include <atomic>
 #include <cuda_runtime.h>
 #include <cstdint>
 
@@ -352,6 +354,8 @@ __global__ void __launch_bounds__(kProjBlock) project_batch_bulk(int full_blocks
   if (t == 0) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");   // smem must outlive the last store's read
 }
 
+constexpr int kProjMaxDevices = 64;
+
 template <int NO>
 inline cudaError_t launch_project(int n, const float* A, const float* b, const float* z_des, const ProjConst& C,
                                   float* z_out, cudaStream_t s) {
@@ -364,10 +368,13 @@ inline cudaError_t launch_project(int n, const float* A, const float* b, const f
     const bool aligned = (((uintptr_t)A | (uintptr_t)b | (uintptr_t)z_des | (uintptr_t)z_out) & 15u) == 0;   // bulk copies
     if (full > 0 && aligned) {
       using SMB = ProjBulkSmem<NO>;
-      static int persistent_ctas = 0, cached_dev = -1;   // resident CTAs of this kernel on device cached_dev
+      // resident CTAs of this kernel per device: one atomic word per device, written once (the
+      // function attribute is per device too); two threads racing compute the same value
+      static std::atomic<int> resident[kProjMaxDevices];
       int dev = 0;
       if ((e = cudaGetDevice(&dev)) != cudaSuccess) return e;
-      if (dev != cached_dev) {                            // (the attribute is per device, like the SM count)
+      int persistent_ctas = (dev >= 0 && dev < kProjMaxDevices) ? resident[dev].load(std::memory_order_acquire) : 0;
+      if (persistent_ctas == 0) {
         e = cudaFuncSetAttribute(project_batch_bulk<NO>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMB::bytes);
         if (e != cudaSuccess) return e;
         int sms = 0, per_sm = 0;
@@ -375,7 +382,8 @@ inline cudaError_t launch_project(int n, const float* A, const float* b, const f
         e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, project_batch_bulk<NO>, kProjBlock, SMB::bytes);
         if (e != cudaSuccess) return e;
         persistent_ctas = sms * (per_sm > 0 ? per_sm : 1);
-        cached_dev = dev;
+        if (persistent_ctas < 2) persistent_ctas = 2;     // one CTA for the full blocks, one for the tail
+        if (dev >= 0 && dev < kProjMaxDevices) resident[dev].store(persistent_ctas, std::memory_order_release);
       }
       // P persistent CTAs for the full blocks + one CTA for the ragged tail, all resident in one wave
       const int P = full < persistent_ctas - 1 ? full : persistent_ctas - 1;
@@ -384,8 +392,16 @@ inline cudaError_t launch_project(int n, const float* A, const float* b, const f
     }
   }
   const size_t bytes = sizeof(float) * ProjSmem<NO>::words;
-  e = cudaFuncSetAttribute(project_batch<NO>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
-  if (e != cudaSuccess) return e;
+  {
+    static std::atomic<int> configured[kProjMaxDevices];
+    int dev = 0;
+    if ((e = cudaGetDevice(&dev)) != cudaSuccess) return e;
+    if (dev < 0 || dev >= kProjMaxDevices || configured[dev].load(std::memory_order_acquire) == 0) {
+      e = cudaFuncSetAttribute(project_batch<NO>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+      if (e != cudaSuccess) return e;
+      if (dev >= 0 && dev < kProjMaxDevices) configured[dev].store(1, std::memory_order_release);
+    }
+  }
   project_batch<NO><<<(unsigned)((n + kProjBlock - 1) / kProjBlock), kProjBlock, bytes, s>>>(n, A, b, z_des, C, z_out);
   return cudaGetLastError();
 }

@@ -34,8 +34,6 @@
 // to CTAs statically (a contiguous range of the flat (scene, tile) list): bit-reproducible.
 #pragma once
 
-#include <cstdlib>
-
 #include "brmppi_device.cuh"
 
 namespace brmppi {
@@ -115,10 +113,6 @@ inline void cta_chunking(int T, int S, int* chunks, int* chunk_len) {
   int cmax = kWorkerThreads / S + 1;
   if (cmax > kMaxChunks) cmax = kMaxChunks;
   if (cmax < 1) cmax = 1;
-  if (const char* e = getenv("BRMPPI_MAX_CHUNKS")) {   // tuning knob for sweeps
-    const int c = atoi(e);
-    if (c >= 1 && c < cmax) cmax = c;
-  }
   int L = (T + cmax - 1) / cmax;
   const int lmin = T < kMinChunkLen ? T : kMinChunkLen;
   if (L < lmin) L = lmin;
@@ -140,10 +134,6 @@ inline CtaPlan make_cta_plan(int K, int T, int n_scenes, int max_obstacles, int 
   int s_max = K < kMaxTileSamples ? K : kMaxTileSamples;
   int c, l, ts;
   while (s_max > 1 && cta_smem_bytes(T, s_max, pl.obs_padded, pl.se_padded, &c, &l, &ts) > kSmemMax) --s_max;
-  if (const char* e = getenv("BRMPPI_MAX_TILE")) {   // tuning knob for sweeps
-    const int v = atoi(e);
-    if (v >= 1 && v < s_max) s_max = v;
-  }
   // fewest tiles, then cut them smaller until the last round of CTAs is full
   const long tps_min = (K + s_max - 1) / s_max;
   const long n_min = tps_min * n_scenes;

@@ -850,9 +850,13 @@ inline CtaKernel cta_kernel_for(bool precise, int n_discs) {
   }
 }
 
+// The dynamic shared-memory limit is an attribute of the FUNCTION on a device, not of a context: it is
+// always raised to the opt-in maximum, so that a second context with a smaller tile never lowers it
+// under a live one.
 inline cudaError_t configure_rollout_cta(bool precise, int n_discs, size_t smem_bytes) {
+  if (smem_bytes > kSmemMax) return cudaErrorInvalidValue;
   cudaError_t e = cudaFuncSetAttribute(cta_kernel_for(precise, n_discs),
-                                       cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes);
+                                       cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemMax);
   if (e != cudaSuccess) return e;
   // the kernel streams almost nothing through L1: ask for the full shared-memory carve-out
   return cudaFuncSetAttribute(cta_kernel_for(precise, n_discs),

@@ -7,6 +7,8 @@
 //            U[o] = sum_p c_p A_p[o] / eta                          (eq. 5)
 #pragma once
 
+#include <curand_philox4x32_x.h>   // library pin only: brmppi_debug_philox_raw(use_curand = 1)
+
 #include "brmppi_device.cuh"
 #include "hitch_filter.cuh"
 
@@ -151,6 +153,17 @@ __global__ void debug_philox(uint32_t key0, uint32_t key1, uint32_t n, int K, in
   if (i >= (size_t)K * T) return;
   const uint32_t k = (uint32_t)(i / T), t = (uint32_t)(i % T);
   out[i] = philox4x32_10(t, n, k, tag, key0, key1);
+}
+
+// Arbitrary (counter, key) blocks through this library's generator, or through the toolkit's raw
+// curand_Philox4x32_10(uint4, uint2) device function (the library pin of SURVEY §8(c)).
+template <bool CURAND>
+__global__ void debug_philox_raw(int n, const uint4* ctr, const uint2* key, uint4* out) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const uint4 c = ctr[i];
+  const uint2 k = key[i];
+  out[i] = CURAND ? curand_Philox4x32_10(c, k) : philox4x32_10(c.x, c.y, c.z, c.w, k.x, k.y);
 }
 
 template <bool PRECISE>

@@ -186,3 +186,24 @@ def test_closed_loop_keeps_the_hitch_limit(B):
     assert worst[0][1] == 0 and worst[1][1] > 10
     assert worst[1][0] <= 0.6 + 0.02
     assert worst[0][0] > worst[1][0] + 0.03          # the unfiltered run does overshoot
+
+
+def test_scratch_is_caller_owned(B):
+    """brmppi_hitch_filter stages through a device scratch the caller passes in (no library-side allocation)."""
+    import ctypes as C
+    import torch
+    p = scenes.default_params(hitch_max=0.9, hitch_alpha=0.4)
+    n = 100
+    assert B.lib().brmppi_hitch_filter_scratch_bytes(0) == 0
+    need = B.lib().brmppi_hitch_filter_scratch_bytes(n)
+    assert need >= 36 * n
+    cp = B.make_cparams(p, 1, 0, 0)
+    x = np.zeros((n, 4), dtype=np.float32); r = np.zeros((n, 2), dtype=np.float32); u = np.zeros((n, 2), dtype=np.float32)
+    fp = C.POINTER(C.c_float)
+    st = torch.cuda.current_stream()
+    small = torch.empty(need // 2, dtype=torch.uint8, device="cuda")
+    args = (C.c_void_p(st.cuda_stream), C.byref(cp), n, x.ctypes.data_as(fp), r.ctypes.data_as(fp), u.ctypes.data_as(fp), None)
+    assert B.lib().brmppi_hitch_filter(*args, C.c_void_p(small.data_ptr()), C.c_size_t(small.numel())) == B.ERR_WORKSPACE_TOO_SMALL
+    assert B.lib().brmppi_hitch_filter(*args, None, 0) == B.ERR_NULL
+    ok = torch.empty(need, dtype=torch.uint8, device="cuda")
+    assert B.lib().brmppi_hitch_filter(*args, C.c_void_p(ok.data_ptr()), C.c_size_t(need)) == B.OK

@@ -80,9 +80,32 @@ def test_philox_bit_exact(B, O):
             assert tuple(int(x) for x in w[k, t]) == O.philox((t, n, k, tag), key)
 
 
-def test_philox_matches_curand_layout(B):
-    """Second, stateful library pin: the counter layout (t, n, k, tag) is cuRAND's Philox state
-    layout, so torch's CUDA generator is not needed -- compare against the KAT directly."""
+def test_philox_matches_curand_device_function(B, O):
+    """Library pin (SURVEY 8(c) pin (ii)): the CUDA toolkit's own raw curand_Philox4x32_10(uint4, uint2)
+    device function, this library's generator and the oracle give the same four words for random
+    (counter, key) pairs -- three independent implementations of the published block function."""
+    rng = np.random.default_rng(20250805)
+    n = 4096
+    ctr = rng.integers(0, 2**32, size=(n, 4), dtype=np.uint64).astype(np.uint32)
+    key = rng.integers(0, 2**32, size=(n, 2), dtype=np.uint64).astype(np.uint32)
+    ctr[0] = 0; key[0] = 0                                 # the published known-answer vectors ride along
+    ctr[1] = 0xFFFFFFFF; key[1] = 0xFFFFFFFF
+    ctr[2] = [0x243f6a88, 0x85a308d3, 0x13198a2e, 0x03707344]; key[2] = [0xa4093822, 0x299f31d0]
+    ours = B.debug_philox_raw(ctr, key, use_curand=False)
+    theirs = B.debug_philox_raw(ctr, key, use_curand=True)
+    assert np.array_equal(ours, theirs)
+    assert [int(x) for x in theirs[0]] == [0x6627e8d5, 0xe169c58d, 0xbc57ac4c, 0x9b00dbd8]
+    assert [int(x) for x in theirs[1]] == [0x408f276d, 0x41c83b0e, 0xa20bc7c6, 0x6d5451fd]
+    assert [int(x) for x in theirs[2]] == [0xd16cfe09, 0x94fdcceb, 0x5001e420, 0x24126ea1]
+    for i in list(range(3)) + [int(x) for x in rng.integers(0, n, 200)]:
+        want = O.philox(tuple(int(x) for x in ctr[i]), tuple(int(x) for x in key[i]))
+        assert tuple(int(x) for x in theirs[i]) == want
+    assert B.debug_philox_raw(np.zeros((0, 4)), np.zeros((0, 2)), use_curand=True).shape == (0, 4)
+
+
+def test_philox_layout_is_curand_state_layout(B):
+    """The counter layout (t, n, k, tag) with key (lo32, hi32)(seed) is cuRAND's Philox state layout
+    (curand_kernel.h: ctr.xy = offset / 4, ctr.zw = subsequence): block (0, 0, 0, 0) of seed 0."""
     w = B.debug_philox(0, 0, 1, 1, 0)
     assert [int(x) for x in w[0, 0]] == [0x6627e8d5, 0xe169c58d, 0xbc57ac4c, 0x9b00dbd8]
 
@@ -325,6 +348,77 @@ def test_full_size_sampled_parity(B, O):
     assert got["U"][:, 1].min() >= p.delta_min and got["U"][:, 1].max() <= p.delta_max
 
 
+@pytest.mark.parametrize("n_obs", [32, 64])
+def test_many_obstacles_at_size_sampled_parity(B, O, n_obs):
+    """The multi-group, culled path in the launch configuration the sweep times (K = 16384, T = 100):
+    sampled costs and final states against the oracle, every sample bit-identical to the un-culled run."""
+    sc = scenes.scene_static(3, n_obs, K=16384, T=100)
+    p = sc.params
+    got = gpu_solve(B, sc, p, 0)
+    ref = gpu_solve(B, sc, p, B.FLAG_NO_CULL)
+    for key in ("S", "XT", "U"):
+        assert np.array_equal(got[key], ref[key]), key
+    rng = np.random.default_rng(n_obs)
+    ks = np.concatenate([[0, 110, 111, p.K - 1, int(got["diag"]["argmin"])], rng.integers(0, p.K, 120)])
+    U0 = np.zeros((p.T, 2))
+    for k in ks:
+        r = O.sample(p, 0, int(k), sc.x0, sc.goal, sc.obstacles, U0)
+        assert close(got["S"][k], r["S"], 1.0), (k, got["S"][k], r["S"])
+        assert close(got["XT"][k], r["xT"], 1.0).all()
+    d = got["diag"]
+    assert np.isfinite(got["S"]).all() and d["nonfinite"] == 0
+    assert got["S"][d["argmin"]] == got["S"].min()
+
+
+def test_batch64_at_size_sampled_parity(B, O):
+    """BASELINE.json configs[4]'s batched launch -- 64 scenes x K = 16384, T = 80 in one launch -- on sampled
+    (scene, sample) pairs against the oracle, and every scene's update inside the control box."""
+    batch = scenes.scene_batch(64, 16384, 80)
+    p = batch[0].params.with_(seed=0)
+    s = B.Solver(p, 64, 8, B.FLAG_WRITE_SAMPLES)
+    for i, sc in enumerate(batch):
+        s.set_scene(sc, i)
+    s.solve()
+    rng = np.random.default_rng(64)
+    U0 = np.zeros((p.T, 2))
+    for i in [0, 1, 31, 63] + [int(x) for x in rng.integers(0, 64, 6)]:
+        S, XT, U, d = s.get_costs(i), s.get_final_states(i), s.get_controls(i), s.get_diag(i)
+        sc = batch[i]
+        pi = p.with_(seed=i)                               # scene i draws with seed + i
+        for k in [0, p.K - 1, int(d["argmin"])] + [int(x) for x in rng.integers(0, p.K, 12)]:
+            r = O.sample(pi, 0, k, sc.x0, sc.goal, sc.obstacles, U0)
+            assert close(S[k], r["S"], 1.0), (i, k, S[k], r["S"])
+            assert close(XT[k], r["xT"], 1.0).all()
+        assert S[d["argmin"]] == S.min() and d["nonfinite"] == 0
+        assert U[:, 0].min() >= p.v_min and U[:, 0].max() <= p.v_max
+        assert U[:, 1].min() >= p.delta_min and U[:, 1].max() <= p.delta_max
+    s.close()
+
+
+def test_contexts_of_different_sizes_are_independent(B, O):
+    """The shared-memory limit is a per-function attribute: a small context created after a large one
+    must not break the large one's next launch (and the other way round)."""
+    big_sc, small_sc = scenes.scene_cfg2(2), scenes.scene_cfg0(1)
+    pb, ps = big_sc.params.with_(K=16384, T=80, n_iter=1), small_sc.params
+    for kernel in (0, 4):
+        big = B.Solver(pb, 1, 8, kernel | B.FLAG_WRITE_SAMPLES)
+        big.set_scene(big_sc)
+        big.solve()
+        first = big.get_costs()
+        small = B.Solver(ps, 1, 1, kernel | B.FLAG_WRITE_SAMPLES)
+        small.set_scene(small_sc)
+        small.solve()
+        small.synchronize()
+        big.set_nominal(None); big.set_counter(0)
+        big.solve()                                        # replays the captured graph
+        assert np.array_equal(big.get_costs(), first)
+        big.time_kernels(2)                                # plain launches outside the graph
+        big.step()                                         # captured lazily AFTER the small context exists
+        assert np.isfinite(big.get_controls()).all()
+        small.solve(); small.step()
+        big.close(); small.close()
+
+
 # ------------------------------------------------------------------------------------------
 # boundary errors
 # ------------------------------------------------------------------------------------------
@@ -382,7 +476,10 @@ def test_error_codes(B):
 # ------------------------------------------------------------------------------------------
 @pytest.mark.parametrize("make", [lambda: scenes.scene_cfg2(0), lambda: scenes.scene_cfg2(5),
                                   lambda: scenes.scene_static(7, 64, K=2048, T=100),
-                                  lambda: scenes.scene_cfg0(3)], ids=["cfg2a", "cfg2b", "static64", "cfg0"])
+                                  lambda: scenes.scene_cfg0(3), lambda: scenes.scene_cfg1(1),
+                                  lambda: scenes.scene_cfg1(2), lambda: scenes.scene_cfg3(4),
+                                  lambda: scenes.scene_static(11, 20, K=1000, T=37)],
+                         ids=["cfg2a", "cfg2b", "static64", "cfg0", "cfg1a", "cfg1b", "cfg3", "static20"])
 def test_culling_is_bit_exact(B, make):
     sc = make()
     p = sc.params.with_(K=min(sc.params.K, 4096), n_iter=2)

@@ -1,10 +1,13 @@
 """Parity of brmppi_project (eq. (11)-(12)) through the C ABI against oracle/projection.py
 on the same seeded (9)-shaped problems.
 
-Tolerance (derived): fp32 Cholesky solves S nu = r with relative error ~ cond(S) eps_32; the
-recipe's S = A M^-1 A^T has cond(S) <= ~2e3, so |z - z_ref| <= 1e-4 max(|z_ref|, 1) holds with a margin of
-about two; a problem is compared at 1e-4 * max(1, cond(S) / 1e3).  The equality constraint itself is
-checked in fp64 on the fp32 result: |A z - b| <= 2e-5 (1 + |A| |z|)."""
+Tolerance: the flat |z - z_ref| <= 1e-4 max(|z_ref|, 1) of the north star for every (9)-shaped problem of the
+recipe (A = [L_g h | diag(h)]; measured on 3000 problems per N_o: worst error 2.0e-5 at N_o = 7 although
+cond(S) of S = A M^-1 A^T reaches 7e4 -- Cholesky's error follows the diagonally scaled condition number,
+which the diag(h) block keeps small; table in DESIGN.md 6.9).  A DENSE random A is not what (9) produces; the
+call accepts it, and there fp32 Cholesky loses cond(S) eps_32 (2.6e-4 seen at cond 2e4), so those cases are
+compared at 1e-4 max(1, cond(S) / 1e3).  The equality constraint itself is checked in fp64 on the fp32
+result: |A z - b| <= 2e-5 (1 + |A| |z|)."""
 import numpy as np
 import pytest
 
@@ -29,16 +32,17 @@ def OP():
     return projection
 
 
-def check(OP, z, P, idx):
+def check(OP, z, P, idx, dense=False):
     Minv = 1.0 / (P["w"] + P["rho"])
     worst = 0.0
     for i in idx:
         ref = OP.project(P["A"][i], P["b"][i], P["z_des"][i], P["w"], P["rho"], P["z_lo"], P["z_hi"])
-        cond = np.linalg.cond((P["A"][i] * Minv[None, :]) @ P["A"][i].T)
-        tol = 1e-4 * max(1.0, cond / 1e3)
+        tol = 1e-4
+        if dense:
+            tol *= max(1.0, np.linalg.cond((P["A"][i] * Minv[None, :]) @ P["A"][i].T) / 1e3)
         zi = z[i].astype(np.float64)
         err = np.abs(zi - ref) / np.maximum(np.abs(ref), 1.0)
-        assert err.max() <= tol, (i, err.max(), cond)
+        assert err.max() <= tol, (i, err.max())
         worst = max(worst, err.max() / tol)
         res = np.abs(P["A"][i] @ zi - P["b"][i])
         assert np.all(res <= 2e-5 * (1.0 + np.abs(P["A"][i]) @ np.abs(zi))), (i, res)
@@ -48,10 +52,11 @@ def check(OP, z, P, idx):
 @pytest.mark.parametrize("n_o", [1, 2, 3, 4, 5, 6, 7, 8])
 @pytest.mark.parametrize("n", [1, 127, 129, 1000])
 def test_host_pointers_match_oracle(B, OP, n_o, n):
-    P = projection_batch(1000 * n_o + n, n, n_o, dense=(n % 2 == 0))
+    dense = (n % 2 == 0)
+    P = projection_batch(1000 * n_o + n, n, n_o, dense=dense)
     z = B.project(P["A"], P["b"], P["z_des"], P["w"], P["rho"], P["z_lo"], P["z_hi"])
     assert z.shape == (n, n_o + 2) and np.isfinite(z).all()
-    check(OP, z, P, range(n))
+    check(OP, z, P, range(n), dense=dense)
 
 
 def test_device_pointers_full_size_sampled(B, OP):
@@ -136,3 +141,37 @@ def test_unaligned_device_pointers_take_the_generic_path(B, OP):
     z_view = B.project(A[1:], b[1:], zd[1:], P["w"], P["rho"], P["z_lo"], P["z_hi"]).cpu().numpy()
     assert np.array_equal(z_view, z_all[1:])          # same arithmetic on both paths
     check(OP, z_all, P, range(0, n, 5))
+
+
+def test_caller_owned_scratch_and_pinned_staging(B, OP):
+    """The host-pointer form stages through a device scratch the CALLER owns (the library allocates no device
+    memory): too small -> BRMPPI_ERR_WORKSPACE_TOO_SMALL, NULL -> BRMPPI_ERR_NULL; page-locked host tensors go
+    through the same call and give the same bits as numpy arrays."""
+    import ctypes as C
+    import torch
+    n, n_o = 300, 5
+    P = projection_batch(21, n, n_o)
+    need = B.lib().brmppi_project_scratch_bytes(n, n_o)
+    assert need >= 4 * (n * n_o * (n_o + 2) + n * n_o + 2 * n * (n_o + 2))
+    assert B.lib().brmppi_project_scratch_bytes(0, n_o) == 0 and B.lib().brmppi_project_scratch_bytes(n, 9) == 0
+    z_np = B.project(P["A"], P["b"], P["z_des"], P["w"], P["rho"], P["z_lo"], P["z_hi"])
+    small = torch.empty(need // 2, dtype=torch.uint8, device="cuda")
+    with pytest.raises(B.BrmppiError) as e:
+        B.project(P["A"], P["b"], P["z_des"], P["w"], P["rho"], P["z_lo"], P["z_hi"], scratch=small)
+    assert e.value.status == B.ERR_WORKSPACE_TOO_SMALL
+    A = np.ascontiguousarray(P["A"], dtype=np.float32)
+    st = torch.cuda.current_stream()
+    f = lambda a: np.ascontiguousarray(a, dtype=np.float32)
+    w, lo, hi = f(P["w"]), f(P["z_lo"]), f(P["z_hi"])
+    fp = C.POINTER(C.c_float)
+    out = np.zeros((n, n_o + 2), dtype=np.float32)
+    b_, z_ = f(P["b"]), f(P["z_des"])
+    r = B.lib().brmppi_project(C.c_void_p(st.cuda_stream), n, n_o, C.c_void_p(A.ctypes.data), C.c_void_p(b_.ctypes.data),
+                               C.c_void_p(z_.ctypes.data), w.ctypes.data_as(fp), float(P["rho"]), lo.ctypes.data_as(fp),
+                               hi.ctypes.data_as(fp), C.c_void_p(out.ctypes.data), 0, None, 0)
+    assert r == B.ERR_NULL
+    pin = lambda a: torch.from_numpy(f(a)).pin_memory()
+    big = torch.empty(need, dtype=torch.uint8, device="cuda")
+    z_pin = B.project(pin(P["A"]), pin(P["b"]), pin(P["z_des"]), P["w"], P["rho"], P["z_lo"], P["z_hi"], scratch=big)
+    assert np.array_equal(z_pin, z_np)
+    check(OP, z_np, P, range(0, n, 3))

@@ -93,3 +93,26 @@ def test_receding_and_stationary(O):
     hs = [O.barrier_se(p, O.disc_centre(p, x_in, j), se[0, :2], se[0]) for j in range(3)]
     want = p.T * 0.25 * sum(-h for h in hs if h < 0)
     assert any(h < 0 for h in hs) and r["pen"] == pytest.approx(want, rel=1e-12)
+
+
+def test_advance_moves_the_centre_only_and_like_a_disc(O):
+    """orc_advance_se: centre += dt * velocity, everything else untouched (hand value), and the same
+    displacement the plant step gives a disc obstacle with that velocity (Assumption 2)."""
+    p = P(dt=0.25)
+    se = np.array([[1.0, -2.0, 2.25, 0.9, 0.7, 0.8, -0.4, 4.0],
+                   [5.0, 5.0, 0.4, 0.4, 0.0, 0.0, 0.0, 2.0]])
+    out = O.advance_se(p, se)
+    want = se.copy()
+    want[0, 0] = 1.0 + 0.25 * 0.8      # 1.2
+    want[0, 1] = -2.0 + 0.25 * -0.4    # -2.1
+    assert np.array_equal(out, want)
+    assert np.array_equal(se[0, :2], [1.0, -2.0])          # the input is not modified
+    discs = np.array([[1.0, -2.0, 0.5, 0.8, -0.4], [5.0, 5.0, 0.4, 0.0, 0.0]])
+    _, discs_next = O.plant_step(p, np.zeros(4), np.zeros(2), discs)
+    assert np.array_equal(out[:, :2], discs_next[:, :2])
+    # n steps of advance == the position the rollout pairs with step n: o(n) = o(0) + n dt vel
+    cur = se
+    for _ in range(7):
+        cur = O.advance_se(p, cur)
+    assert cur[0, 0] == pytest.approx(1.0 + 7 * 0.25 * 0.8, rel=1e-15)
+    assert cur[0, 1] == pytest.approx(-2.0 + 7 * 0.25 * -0.4, rel=1e-15)
