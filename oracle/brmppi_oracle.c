@@ -465,3 +465,266 @@ int orc_hitch_filter(const orc_params* p, const double x[4], const double u_ref[
   double g_ref = c0 + a[0] * (uc[0] - u_ref[0]) + a[1] * (uc[1] - u_ref[1]);
   return (g_ref >= 0.0) ? 0 : 1;
 }
+
+/* ------------------------------------------------------------------------------------------
+ * The projected rollout: BR-MPPI proper, Sec. V-A; readings in the header.
+ * ---------------------------------------------------------------------------------------- */
+
+/* Eq. (12). */
+int orc_project(int m, int d, const double* A, const double* b, const double* z_des, const double* w,
+                double rho, const double* z_lo, const double* z_hi, double* z_out) {
+  double Minv[2 + ORC_PROJ_MAX_NO], pvec[2 + ORC_PROJ_MAX_NO], y[2 + ORC_PROJ_MAX_NO];
+  double S[ORC_PROJ_MAX_NO][ORC_PROJ_MAX_NO], r[ORC_PROJ_MAX_NO], nu[ORC_PROJ_MAX_NO], diag0[ORC_PROJ_MAX_NO];
+  int dropped_row[ORC_PROJ_MAX_NO], dropped = 0;
+  for (int j = 0; j < d; ++j) {
+    Minv[j] = 1.0 / (w[j] + rho);                                /* M = W + rho I, diagonal        */
+    pvec[j] = w[j] * z_des[j] + 0.5 * rho * (z_hi[j] + z_lo[j]); /* p = W z_des + rho/2 (z_hi+z_lo) */
+    y[j] = Minv[j] * pvec[j];                                    /* M^-1 p                          */
+  }
+  for (int i = 0; i < m; ++i) {
+    double acc = -b[i];
+    for (int j = 0; j < d; ++j) acc += A[i * d + j] * y[j];
+    r[i] = acc;                                                  /* A M^-1 p - b                    */
+    for (int k = 0; k < m; ++k) {
+      double s = 0.0;
+      for (int j = 0; j < d; ++j) s += A[i * d + j] * Minv[j] * A[k * d + j];
+      S[i][k] = s;                                               /* A M^-1 A^T                      */
+    }
+    diag0[i] = S[i][i];
+  }
+  /* Cholesky S = L L^T in place (lower triangle), then L w = r, L^T nu = w */
+  for (int k = 0; k < m; ++k) {
+    double dkk = S[k][k];
+    for (int q = 0; q < k; ++q) dkk -= S[k][q] * S[k][q];
+    dropped_row[k] = !(dkk > 1e-14 * diag0[k]);
+    if (dropped_row[k]) {
+      ++dropped;
+      S[k][k] = 1.0;
+      for (int i = k + 1; i < m; ++i) S[i][k] = 0.0;
+      for (int q = 0; q < k; ++q) S[k][q] = 0.0;
+      r[k] = 0.0;
+      continue;
+    }
+    S[k][k] = sqrt(dkk);
+    for (int i = k + 1; i < m; ++i) {
+      double v = S[i][k];
+      for (int q = 0; q < k; ++q) v -= S[i][q] * S[k][q];
+      S[i][k] = v / S[k][k];
+    }
+  }
+  for (int i = 0; i < m; ++i) {
+    double v = r[i];
+    for (int q = 0; q < i; ++q) v -= S[i][q] * nu[q];
+    nu[i] = v / S[i][i];
+  }
+  for (int i = m - 1; i >= 0; --i) {
+    double v = nu[i];
+    for (int q = i + 1; q < m; ++q) v -= S[q][i] * nu[q];
+    nu[i] = v / S[i][i];
+    if (dropped_row[i]) nu[i] = 0.0;
+  }
+  for (int j = 0; j < d; ++j) {
+    double acc = pvec[j];
+    for (int i = 0; i < m; ++i) acc -= A[i * d + j] * nu[i];
+    z_out[j] = Minv[j] * acc;                                    /* M^-1 (p - A^T nu)               */
+  }
+  return dropped;
+}
+
+/* u~^alpha draws: counter (t, n, k, 2 + (i >> 2)); Box-Muller on (w0, w1) and (w2, w3). */
+void orc_ualpha_normals(uint64_t seed, uint32_t n, uint32_t k, uint32_t t, int n_obs, double* zeta) {
+  uint32_t key[2];
+  seed_key(seed, key);
+  for (int q = 0; 4 * q < n_obs; ++q) {
+    uint32_t ctr[4] = {t, n, k, 2u + (uint32_t)q}, w[4];
+    orc_philox4x32_10(ctr, key, w);
+    double z4[4];
+    for (int h = 0; h < 2; ++h) {
+      double u1 = 1.0 - orc_uniform(w[2 * h]);
+      double u2 = orc_uniform(w[2 * h + 1]);
+      double rr = sqrt(-2.0 * log(u1));
+      z4[2 * h + 0] = rr * cos(2.0 * M_PI * u2);
+      z4[2 * h + 1] = rr * sin(2.0 * M_PI * u2);
+    }
+    for (int e = 0; e < 4 && 4 * q + e < n_obs; ++e) zeta[4 * q + e] = z4[e];
+  }
+}
+
+/* Row i of (9): h_i on the closest disc, L_g h_i = grad_x h_i . dt G(x), L_f h_i from the
+ * obstacle's predicted motion. */
+void orc_barrier_row(const orc_params* p, const double x[4], const double* ob, int t, double* h_out,
+                     int* jstar, double Lg[2], double* Lf) {
+  double o[2] = {ob[0] + (double)t * p->dt * ob[3], ob[1] + (double)t * p->dt * ob[4]};
+  double rho = ob[2] + p->disc_radius;
+  int jbest = 0;
+  double hbest = 0.0, cbest[2] = {0.0, 0.0};
+  for (int j = 0; j < p->n_discs; ++j) {
+    double c[2];
+    orc_disc_centre(p, x, j, c);
+    double h = orc_barrier(p, c, o, ob[2]);
+    if (j == 0 || h < hbest) { hbest = h; jbest = j; cbest[0] = c[0]; cbest[1] = c[1]; }
+  }
+  double psi1 = x[2], psi2 = x[3], beta = psi1 - psi2;
+  /* grad of h wrt the disc centre, then the chain rule through c(x) = p_h + a e(psi_body),
+   * p_h = (x - Lh cos psi1, y - Lh sin psi1) */
+  double gx = 2.0 * (cbest[0] - o[0]) / (rho * rho), gy = 2.0 * (cbest[1] - o[1]) / (rho * rho);
+  double a = p->disc_offset[jbest];
+  double dc1x = p->Lh * sin(psi1), dc1y = -p->Lh * cos(psi1);   /* d p_h / d psi1 */
+  double dc2x = 0.0, dc2y = 0.0;
+  if (p->disc_body[jbest] == 0) { dc1x += -a * sin(psi1); dc1y += a * cos(psi1); }
+  else { dc2x = -a * sin(psi2); dc2y = a * cos(psi2); }
+  double dh_dx = gx, dh_dy = gy;
+  double dh_dpsi1 = gx * dc1x + gy * dc1y;
+  double dh_dpsi2 = gx * dc2x + gy * dc2y;
+  /* columns of G(x): d/dv = (cos psi1, sin psi1, 0, sin(beta)/L2), d/domega = (0, 0, 1/L1, -(Lh/(L1 L2)) cos beta) */
+  Lg[0] = p->dt * (dh_dx * cos(psi1) + dh_dy * sin(psi1) + dh_dpsi2 * sin(beta) / p->L2);
+  Lg[1] = p->dt * (dh_dpsi1 / p->L1 - dh_dpsi2 * (p->Lh / (p->L1 * p->L2)) * cos(beta));
+  *Lf = -p->dt * (gx * ob[3] + gy * ob[4]);
+  *h_out = hbest;
+  *jstar = jbest;
+}
+
+void orc_affine_step(const orc_params* p, const double x[4], const double w[2], double xn[4]) {
+  double psi1 = x[2], psi2 = x[3], beta = psi1 - psi2;
+  xn[0] = x[0] + p->dt * w[0] * cos(psi1);
+  xn[1] = x[1] + p->dt * w[0] * sin(psi1);
+  xn[2] = psi1 + p->dt * w[1] / p->L1;
+  xn[3] = psi2 + p->dt * (w[0] * sin(beta) - (p->Lh / p->L1) * w[1] * cos(beta)) / p->L2;
+}
+
+double orc_rollout_projected(const orc_params* p, const orc_proj_params* pp, const double x0[4],
+                             const double goal[4], int n_obs, const double* obstacles, const double* u,
+                             const double* ualpha, double alpha0, double xT[4], double* traj,
+                             double* z_all, double* alpha_all, double* Ab_all) {
+  const int T = p->T, d = 2 + n_obs;
+  double X[4] = {x0[0], x0[1], x0[2], x0[3]};
+  double alpha[ORC_PROJ_MAX_NO], S = 0.0;
+  double wdiag[2 + ORC_PROJ_MAX_NO], zlo[2 + ORC_PROJ_MAX_NO], zhi[2 + ORC_PROJ_MAX_NO];
+  double vabs = fmax(fabs(p->v_min), fabs(p->v_max));
+  double omega_max = vabs * tan(fmax(fabs(p->delta_min), fabs(p->delta_max)));
+  wdiag[0] = pp->q_v; wdiag[1] = pp->q_omega;
+  zlo[0] = p->v_min; zhi[0] = p->v_max; zlo[1] = -omega_max; zhi[1] = omega_max;
+  for (int i = 0; i < n_obs; ++i) {
+    alpha[i] = alpha0;
+    wdiag[2 + i] = pp->q_alpha; zlo[2 + i] = -pp->ualpha_max; zhi[2 + i] = pp->ualpha_max;
+  }
+  if (traj) memcpy(traj, X, sizeof(X));
+  if (alpha_all) memcpy(alpha_all, alpha, sizeof(double) * (size_t)n_obs);
+
+  for (int t = 0; t < T; ++t) {
+    /* z_des = [w_des; u~^alpha], w_des = (v~, v~ tan delta~) */
+    double zdes[2 + ORC_PROJ_MAX_NO], A[ORC_PROJ_MAX_NO * (2 + ORC_PROJ_MAX_NO)], b[ORC_PROJ_MAX_NO];
+    double z[2 + ORC_PROJ_MAX_NO];
+    zdes[0] = u[2 * t + 0];
+    zdes[1] = u[2 * t + 0] * tan(u[2 * t + 1]);
+    memset(A, 0, sizeof(A));
+    for (int i = 0; i < n_obs; ++i) {
+      double h, Lg[2], Lf;
+      int jstar;
+      zdes[2 + i] = ualpha[t * n_obs + i];
+      orc_barrier_row(p, X, obstacles + 5 * i, t, &h, &jstar, Lg, &Lf);
+      /* (9): L_g h u + h u^alpha = -alpha h - L_f h */
+      A[i * d + 0] = Lg[0]; A[i * d + 1] = Lg[1]; A[i * d + 2 + i] = h;
+      b[i] = -alpha[i] * h - Lf;
+      if (Ab_all) {
+        double* q = Ab_all + ((size_t)t * n_obs + i) * 4;
+        q[0] = Lg[0]; q[1] = Lg[1]; q[2] = h; q[3] = b[i];
+      }
+    }
+    if (n_obs > 0) orc_project(n_obs, d, A, b, zdes, wdiag, pp->rho, zlo, zhi, z);
+    else {                                                   /* no constraint: the soft-bounded minimiser M^-1 p */
+      for (int j = 0; j < 2; ++j) z[j] = (wdiag[j] * zdes[j] + 0.5 * pp->rho * (zhi[j] + zlo[j])) / (wdiag[j] + pp->rho);
+    }
+    if (z_all) memcpy(z_all + (size_t)t * d, z, sizeof(double) * (size_t)d);
+    /* x_{tau+1} from the projected input, alpha_{tau+1} = alpha_tau + u^alpha_proj */
+    double Xn[4];
+    orc_affine_step(p, X, z, Xn);
+    for (int i = 0; i < n_obs; ++i) alpha[i] += z[2 + i];
+    /* stage cost on (x_{tau+1}, projected input) */
+    double hitch = fabs(orc_wrap(Xn[2] - Xn[3])) - (p->hitch_max - p->hitch_kappa * fabs(z[0]));
+    if (hitch < 0.0) hitch = 0.0;
+    double ca = 0.0;
+    for (int i = 0; i < n_obs; ++i) {
+      double h, Lg[2], Lf;
+      int jstar;
+      orc_barrier_row(p, Xn, obstacles + 5 * i, t + 1, &h, &jstar, Lg, &Lf);
+      if (h < pp->h_buffer && alpha[i] > 0.0) ca += alpha[i] * alpha[i];
+    }
+    S += orc_goal_cost(p, Xn, goal) + p->w_v * z[0] * z[0] + p->w_delta * z[1] * z[1] +
+         p->w_hitch * hitch * hitch + pp->w_alpha * ca;
+    memcpy(X, Xn, sizeof(X));
+    if (traj) memcpy(traj + 4 * (t + 1), X, sizeof(X));
+    if (alpha_all) memcpy(alpha_all + (size_t)(t + 1) * n_obs, alpha, sizeof(double) * (size_t)n_obs);
+  }
+  S += p->w_term * orc_goal_cost(p, X, goal);
+  memcpy(xT, X, sizeof(X));
+  return S;
+}
+
+double orc_sample_projected(const orc_params* p, const orc_proj_params* pp, uint32_t n, uint32_t k,
+                            const double x0[4], const double goal[4], int n_obs, const double* obstacles,
+                            const double* U_in, double* u, double xT[4]) {
+  const int T = p->T;
+  double alpha0 = orc_alpha(p, n, k);
+  double* ua = (double*)malloc(sizeof(double) * (size_t)T * (size_t)(n_obs > 0 ? n_obs : 1));
+  for (int t = 0; t < T; ++t) {
+    double z[2], zeta[ORC_PROJ_MAX_NO];
+    orc_normals(p->seed, n, k, (uint32_t)t, z);
+    u[2 * t + 0] = clampd(U_in[2 * t + 0] + p->sigma_v * z[0], p->v_min, p->v_max);
+    u[2 * t + 1] = clampd(U_in[2 * t + 1] + p->sigma_delta * z[1], p->delta_min, p->delta_max);
+    orc_ualpha_normals(p->seed, n, k, (uint32_t)t, n_obs, zeta);
+    for (int i = 0; i < n_obs; ++i) ua[t * n_obs + i] = pp->sigma_ualpha * zeta[i];
+  }
+  double S = orc_rollout_projected(p, pp, x0, goal, n_obs, obstacles, u, ua, alpha0, xT, NULL, NULL, NULL, NULL);
+  free(ua);
+  return S;
+}
+
+typedef struct {
+  sample_job base;
+  const orc_proj_params* pp;
+} proj_job;
+
+static void* proj_worker(void* arg) {
+  proj_job* job = (proj_job*)arg;
+  const sample_job* b = &job->base;
+  const int T = b->p->T;
+  for (int k = b->k_begin; k < b->k_end; ++k)
+    b->S[k] = orc_sample_projected(b->p, job->pp, b->n, (uint32_t)k, b->x0, b->goal, b->n_obs, b->obstacles,
+                                   b->U_in, b->u_all + (size_t)k * 2 * T, b->XT + 4 * (size_t)k);
+  return NULL;
+}
+
+int orc_iteration_projected(const orc_params* p, const orc_proj_params* pp, uint32_t n, const double x0[4],
+                            const double goal[4], int n_obs, const double* obstacles, const double* U_in,
+                            double* U_out, double* S, double* XT, double* u_all, double* w, int* argmin,
+                            double* gap, double* eta, int n_threads) {
+  const int K = p->K, T = p->T;
+  double* S_buf = S ? S : (double*)malloc(sizeof(double) * (size_t)K);
+  double* XT_buf = XT ? XT : (double*)malloc(sizeof(double) * 4 * (size_t)K);
+  double* u_buf = u_all ? u_all : (double*)malloc(sizeof(double) * 2 * (size_t)T * (size_t)K);
+  double* U_nom = (double*)malloc(sizeof(double) * 2 * (size_t)T);
+  memcpy(U_nom, U_in, sizeof(double) * 2 * (size_t)T);
+  if (n_threads < 1) n_threads = 1;
+  if (n_threads > K) n_threads = K;
+  proj_job* jobs = (proj_job*)malloc(sizeof(proj_job) * (size_t)n_threads);
+  pthread_t* tids = (pthread_t*)malloc(sizeof(pthread_t) * (size_t)n_threads);
+  for (int i = 0; i < n_threads; ++i) {
+    jobs[i].base = (sample_job){p, n, x0, goal, obstacles, U_nom, n_obs, (int)((long long)K * i / n_threads),
+                                (int)((long long)K * (i + 1) / n_threads), S_buf, XT_buf, u_buf, 0, NULL};
+    jobs[i].pp = pp;
+  }
+  if (n_threads == 1) proj_worker(&jobs[0]);
+  else {
+    for (int i = 0; i < n_threads; ++i) pthread_create(&tids[i], NULL, proj_worker, &jobs[i]);
+    for (int i = 0; i < n_threads; ++i) pthread_join(tids[i], NULL);
+  }
+  if (U_out != U_in) memcpy(U_out, U_nom, sizeof(double) * 2 * (size_t)T);
+  /* eq. (5) on the sampled u~ with the projected rollouts' costs */
+  int nonfinite = orc_weights_update(K, T, p->lambda, S_buf, u_buf, U_out, w, argmin, gap, eta);
+  free(jobs); free(tids); free(U_nom);
+  if (!S) free(S_buf);
+  if (!XT) free(XT_buf);
+  if (!u_all) free(u_buf);
+  return nonfinite;
+}

@@ -34,6 +34,11 @@
  *                              scipy SLSQP, a dense grid search and the halfspace-projection closed form;
  *                              closed-loop forward invariance of |hitch| <= limit under a jackknifing
  *                              reference.  The linearisation in u about u_ref is reading 28, not the paper's.
+ *   projected rollout ........ pinned: (12) against the numpy form, KKT residuals and scipy SLSQP; A z* = b at
+ *                              every (k, t); N_o = 1 scalar closed form; rho = 0 == pinv projection; rho -> inf
+ *                              pulls to the centre of the bounds; rows of (9) against finite differences of h
+ *                              through the pinned Euler step; far obstacle => u untouched; mpmath brute
+ *                              force K<=4, T<=4.  The alpha cost's FORM is parity unpinned (reference [1] only).
  *   whole solve .............. pinned: brute force (independent mpmath transcription) K<=8, T<=5
  *   cost weights, disc placement, hinge shapes (linear barrier hinge, squared hitch hinge),
  *   scene generators ......... PARITY UNPINNED by the paper (never printed there); fixed by the
@@ -190,6 +195,81 @@ void orc_hitch_constraint(const orc_params* p, const double x[4], const double u
  * intersect; then u* is the point of the box with the largest a . u (coordinates with a_i = 0 keep
  * the clamped reference). */
 int orc_hitch_filter(const orc_params* p, const double x[4], const double u_ref[2], double u_out[2]);
+
+/* ---- the projected rollout: BR-MPPI proper, Sec. V-A (reading 30) ------
+ *
+ * At every prediction step the sampled inputs are projected onto the barrier-rate EQUALITY (9)
+ *     L_f h_i(x) + L_g h_i(x) u = -(alpha_i + u^alpha_i) h_i(x),   i = 1..N_o,
+ * by the closed form (12) of the soft-bounded weighted minimum-norm problem (11); the projected input
+ * drives the model, the projected auxiliary input drives alpha_i.
+ *
+ * Readings taken for the reduced model (the paper's own model is the 7-state one):
+ *  - inputs: the reduced eq. (6) is driftless and affine in w = (v, omega), omega := v tan(delta):
+ *      x' = x + dt G(x) w,  G = [cos psi1, 0; sin psi1, 0; 0, 1/L1; sin(beta)/L2, -(Lh/(L1 L2)) cos(beta)],
+ *    so f = 0, g = dt G and (9) is exact-affine in z = [w; u^alpha].  Sampled (v~, delta~) (perturbed and
+ *    clamped as in the penalty path) give w_des = (v~, v~ tan delta~).
+ *  - one constraint per obstacle, on the vehicle disc with the smallest h at x_tau
+ *    (lowest index on ties): h_i = min_j h_ij.
+ *  - L_g h_i = grad_x h_i . dt G(x);  L_f h_i = -(2/rho_i^2)(c - o_i) . dt vel_i: the obstacle's predicted
+ *    motion (time-varying safe set), zero for a static one.
+ *  - alpha_{i,0} = alpha_k for every obstacle (reading 8's per-sample draw), alpha_{i,tau+1} = alpha_{i,tau}
+ *    + u^alpha_proj,i; u~^alpha_{i,tau} = sigma_ualpha zeta, zeta ~ N(0,1) from Philox counter
+ *    (t, n, k, 2 + (i >> 2)), Box-Muller on words (0,1) -> zeta_0, zeta_1 and (2,3) -> zeta_2, zeta_3,
+ *    obstacle i takes zeta_{i & 3}.
+ *  - W = Diag(q_v, q_omega, q_alpha ... q_alpha);  z_lo / z_hi = (v_min, -omega_max, -ualpha_max ...) /
+ *    (v_max, omega_max, ualpha_max ...), omega_max = max|v| tan(max|delta|).
+ *  - stage cost on (x_{tau+1}, projected input): goal + heading + w_v v_p^2 + w_delta omega_p^2 + hitch
+ *    hinge + w_alpha sum_i [h_i(x_{tau+1}, o_i(tau+1)) < h_buffer] max(0, alpha_{i,tau+1})^2 -- the
+ *    "cost that motivates negative alpha within a buffer zone" (its exact form is in the
+ *    paper's reference [1] only: PARITY UNPINNED).  No hinge penalty: the projection replaces it.
+ *  - update (5) averages the SAMPLED u~ (PAPER.md:95 prints u~, not u_proj) with weights from the
+ *    projected rollouts' costs.
+ * Pins: tests/test_oracle_projected.py.
+ */
+typedef struct {
+  double q_v, q_omega, q_alpha;   /* W = Diag(Q1, Q2), Q1 = diag(q_v, q_omega), Q2 = q_alpha I */
+  double rho;                     /* soft-bound weight of (11a), >= 0                                          */
+  double sigma_ualpha;            /* standard deviation of the sampled auxiliary inputs          */
+  double ualpha_max;              /* u^alpha in [-ualpha_max, ualpha_max]: the z_lo / z_hi of (11)              */
+  double w_alpha, h_buffer;       /* cost on alpha where h < h_buffer                            */
+} orc_proj_params;
+
+#define ORC_PROJ_MAX_NO 8
+
+/* Eq. (12): z* = M^-1 [p - A^T (A M^-1 A^T)^-1 (A M^-1 p - b)], M = W + rho I,
+ * p = W z_des + rho/2 (z_hi + z_lo); A is m x d row-major, W = diag(w).  The m x m system is solved by
+ * Cholesky; a row whose pivot is not above 1e-14 times its own diagonal entry is dropped (multiplier 0).
+ * Returns the number of dropped rows. */
+int orc_project(int m, int d, const double* A, const double* b, const double* z_des, const double* w,
+                double rho, const double* z_lo, const double* z_hi, double* z_out);
+
+/* zeta[i], i < n_obs: the standard normals behind u~^alpha_{i,t} of sample k in iteration n. */
+void orc_ualpha_normals(uint64_t seed, uint32_t n, uint32_t k, uint32_t t, int n_obs, double* zeta);
+
+/* Row i of (9) at state x and step t: h = min_j h_ij(x, o(t)) (*jstar = its disc), Lg[2] = L_g h,
+ * *Lf = L_f h.  obstacle = (cx, cy, R, vx, vy) at rollout time 0. */
+void orc_barrier_row(const orc_params* p, const double x[4], const double* obstacle, int t, double* h,
+                     int* jstar, double Lg[2], double* Lf);
+
+/* x' = x + dt G(x) w, w = (v, omega). */
+void orc_affine_step(const orc_params* p, const double x[4], const double w[2], double x_next[4]);
+
+/* One projected rollout.  u[T][2]: sampled, clamped (v~, delta~); ualpha[T][n_obs]: sampled u~^alpha;
+ * alpha0: initial alpha of every obstacle.  Optional outputs (NULL to skip): traj[(T+1)][4],
+ * z_all[T][2 + n_obs] (projected z*), alpha_all[(T+1)][n_obs], Ab_all[T][n_obs][4] = (Lg0, Lg1, h, b). */
+double orc_rollout_projected(const orc_params* p, const orc_proj_params* pp, const double x0[4],
+                             const double goal[4], int n_obs, const double* obstacles, const double* u,
+                             const double* ualpha, double alpha0, double xT[4], double* traj,
+                             double* z_all, double* alpha_all, double* Ab_all);
+
+double orc_sample_projected(const orc_params* p, const orc_proj_params* pp, uint32_t n, uint32_t k,
+                            const double x0[4], const double goal[4], int n_obs, const double* obstacles,
+                            const double* U_in, double* u /* T*2 */, double xT[4]);
+
+int orc_iteration_projected(const orc_params* p, const orc_proj_params* pp, uint32_t n, const double x0[4],
+                            const double goal[4], int n_obs, const double* obstacles, const double* U_in,
+                            double* U_out, double* S, double* XT, double* u_all, double* w, int* argmin,
+                            double* gap, double* eta, int n_threads);
 
 #ifdef __cplusplus
 }

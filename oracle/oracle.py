@@ -41,6 +41,12 @@ class _Params(C.Structure):
                 ("seed", C.c_uint64)]
 
 
+class _ProjParams(C.Structure):
+    _fields_ = [("q_v", C.c_double), ("q_omega", C.c_double), ("q_alpha", C.c_double), ("rho", C.c_double),
+                ("sigma_ualpha", C.c_double), ("ualpha_max", C.c_double), ("w_alpha", C.c_double),
+                ("h_buffer", C.c_double)]
+
+
 _lib = None
 _dp = C.POINTER(C.c_double)
 _u32p = C.POINTER(C.c_uint32)
@@ -105,8 +111,35 @@ def lib():
         L.orc_hitch_constraint.restype = None
         L.orc_hitch_filter.argtypes = [C.POINTER(_Params), _dp, _dp, _dp]
         L.orc_hitch_filter.restype = C.c_int
+        PP = C.POINTER(_ProjParams)
+        ip = C.POINTER(C.c_int)
+        L.orc_project.argtypes = [C.c_int, C.c_int, _dp, _dp, _dp, _dp, C.c_double, _dp, _dp, _dp]
+        L.orc_project.restype = C.c_int
+        L.orc_ualpha_normals.argtypes = [C.c_uint64, C.c_uint32, C.c_uint32, C.c_uint32, C.c_int, _dp]
+        L.orc_ualpha_normals.restype = None
+        L.orc_barrier_row.argtypes = [C.POINTER(_Params), _dp, _dp, C.c_int, _dp, ip, _dp, _dp]
+        L.orc_barrier_row.restype = None
+        L.orc_affine_step.argtypes = [C.POINTER(_Params), _dp, _dp, _dp]
+        L.orc_affine_step.restype = None
+        L.orc_rollout_projected.argtypes = [C.POINTER(_Params), PP, _dp, _dp, C.c_int, _dp, _dp, _dp, C.c_double,
+                                            _dp, _dp, _dp, _dp, _dp]
+        L.orc_rollout_projected.restype = C.c_double
+        L.orc_sample_projected.argtypes = [C.POINTER(_Params), PP, C.c_uint32, C.c_uint32, _dp, _dp, C.c_int, _dp,
+                                           _dp, _dp, _dp]
+        L.orc_sample_projected.restype = C.c_double
+        L.orc_iteration_projected.argtypes = [C.POINTER(_Params), PP, C.c_uint32, _dp, _dp, C.c_int, _dp, _dp,
+                                              _dp, _dp, _dp, _dp, _dp, ip, _dp, _dp, C.c_int]
+        L.orc_iteration_projected.restype = C.c_int
         _lib = L
     return _lib
+
+
+def _pparams(p) -> _ProjParams:
+    s = _ProjParams()
+    s.q_v, s.q_omega, s.q_alpha, s.rho = float(p.proj_qv), float(p.proj_qomega), float(p.proj_qalpha), float(p.proj_rho)
+    s.sigma_ualpha, s.ualpha_max = float(p.sigma_ualpha), float(p.ualpha_max)
+    s.w_alpha, s.h_buffer = float(p.w_alpha), float(p.h_buffer)
+    return s
 
 
 def _cparams(p) -> _Params:
@@ -336,3 +369,85 @@ def hitch_filter(p, x, u_ref):
     u = np.zeros(2)
     st = lib().orc_hitch_filter(C.byref(_cparams(p)), _ptr(_d(x, (4,))), _ptr(_d(u_ref, (2,))), _ptr(u))
     return u, int(st)
+
+
+# ---- projected rollout, Sec. V-A ---------------------------------------------
+def project(A, b, z_des, w, rho, z_lo, z_hi):
+    """Eq. (12) by the C oracle: (z*, number of dropped rows)."""
+    A = _d(A)
+    m, d = A.shape
+    z = np.zeros(d)
+    dropped = lib().orc_project(m, d, _ptr(A), _ptr(_d(b, (m,))), _ptr(_d(z_des, (d,))), _ptr(_d(w, (d,))),
+                                float(rho), _ptr(_d(z_lo, (d,))), _ptr(_d(z_hi, (d,))), _ptr(z))
+    return z, int(dropped)
+
+
+def ualpha_normals(seed, n, k, t, n_obs):
+    z = np.zeros(max(n_obs, 1))
+    lib().orc_ualpha_normals(int(seed) & 0xFFFFFFFFFFFFFFFF, int(n), int(k), int(t), int(n_obs), _ptr(z))
+    return z[:n_obs]
+
+
+def barrier_row(p, x, obstacle, t):
+    """(h, active disc, L_g h [2], L_f h) of one obstacle at state x, step t."""
+    h, Lf, j = C.c_double(), C.c_double(), C.c_int()
+    Lg = np.zeros(2)
+    lib().orc_barrier_row(C.byref(_cparams(p)), _ptr(_d(x, (4,))), _ptr(_d(obstacle, (5,))), int(t), C.byref(h),
+                          C.byref(j), _ptr(Lg), C.byref(Lf))
+    return h.value, j.value, Lg, Lf.value
+
+
+def affine_step(p, x, w):
+    xn = np.zeros(4)
+    lib().orc_affine_step(C.byref(_cparams(p)), _ptr(_d(x, (4,))), _ptr(_d(w, (2,))), _ptr(xn))
+    return xn
+
+
+def rollout_projected(p, x0, goal, obstacles, u, ualpha, alpha0):
+    obs = _d(obstacles).reshape(-1, 5)
+    n_obs, T = obs.shape[0], p.T
+    u = _d(u, (T, 2))
+    ua = _d(ualpha).reshape(T, n_obs) if n_obs else np.zeros((T, 1))
+    xT, traj = np.zeros(4), np.zeros((T + 1, 4))
+    z = np.zeros((T, 2 + n_obs))
+    al = np.zeros((T + 1, max(n_obs, 1)))
+    Ab = np.zeros((T, max(n_obs, 1), 4))
+    S = lib().orc_rollout_projected(C.byref(_cparams(p)), C.byref(_pparams(p)), _ptr(_d(x0, (4,))), _ptr(_d(goal, (4,))),
+                                    n_obs, _ptr(obs), _ptr(u), _ptr(ua), float(alpha0), _ptr(xT), _ptr(traj), _ptr(z),
+                                    _ptr(al), _ptr(Ab))
+    return dict(S=S, xT=xT, traj=traj, z=z, alpha=al[:, :n_obs], Ab=Ab[:, :n_obs])
+
+
+def sample_projected(p, n, k, x0, goal, obstacles, U_in):
+    obs = _d(obstacles).reshape(-1, 5)
+    u, xT = np.zeros((p.T, 2)), np.zeros(4)
+    S = lib().orc_sample_projected(C.byref(_cparams(p)), C.byref(_pparams(p)), int(n), int(k), _ptr(_d(x0, (4,))),
+                                   _ptr(_d(goal, (4,))), obs.shape[0], _ptr(obs), _ptr(_d(U_in, (p.T, 2))), _ptr(u), _ptr(xT))
+    return dict(S=S, u=u, xT=xT)
+
+
+def iteration_projected(p, n, x0, goal, obstacles, U_in, n_threads=1, want_samples=False):
+    obs = _d(obstacles).reshape(-1, 5)
+    K, T = p.K, p.T
+    U_out, S, XT, w = np.zeros((T, 2)), np.zeros(K), np.zeros((K, 4)), np.zeros(K)
+    u_all = np.zeros((K, T, 2))
+    argmin, gap, eta = C.c_int(), C.c_double(), C.c_double()
+    nonfinite = lib().orc_iteration_projected(C.byref(_cparams(p)), C.byref(_pparams(p)), int(n), _ptr(_d(x0, (4,))),
+                                              _ptr(_d(goal, (4,))), obs.shape[0], _ptr(obs), _ptr(_d(U_in, (T, 2))),
+                                              _ptr(U_out), _ptr(S), _ptr(XT), _ptr(u_all), _ptr(w), C.byref(argmin),
+                                              C.byref(gap), C.byref(eta), int(n_threads))
+    out = dict(U=U_out, S=S, XT=XT, w=w, argmin=argmin.value, gap=gap.value, eta=eta.value, nonfinite=nonfinite)
+    if want_samples:
+        out["u"] = u_all
+    return out
+
+
+def solve_projected(p, n0, x0, goal, obstacles, U_in, n_threads=1):
+    """n_iter projected iterations from counter n0; list of per-iteration results."""
+    U = _d(U_in, (p.T, 2)).copy()
+    outs = []
+    for it in range(p.n_iter):
+        r = iteration_projected(p, n0 + it, x0, goal, obstacles, U, n_threads=n_threads)
+        U = r["U"].copy()
+        outs.append(r)
+    return outs

@@ -47,6 +47,15 @@ class Params:
     hitch_alpha: float = 0.5      # alpha of condition (3), in (0, 1]
     hitch_qv: float = 1.0         # Q_h = diag(q_v, q_delta)
     hitch_qdelta: float = 1.0
+    # projected rollout, Sec. V-A (reading 30); read only in projected mode
+    proj_qv: float = 1.0          # W = Diag(Q1, Q2): Q1 = diag(proj_qv, proj_qomega), Q2 = proj_qalpha I
+    proj_qomega: float = 4.0
+    proj_qalpha: float = 0.5
+    proj_rho: float = 0.25        # soft-bound weight rho of (11a)
+    sigma_ualpha: float = 0.3     # standard deviation of the sampled auxiliary inputs u~^alpha
+    ualpha_max: float = 1.0       # u^alpha in [-ualpha_max, ualpha_max]
+    w_alpha: float = 10.0         # cost on positive alpha inside the buffer zone h < h_buffer
+    h_buffer: float = 0.5
     w_bar: float = 1.0e3
     w_term: float = 10.0
     lam: float = 1.0
