@@ -52,16 +52,48 @@ def workload(name, rank=0):
         sc = scenes.scene_cfg2_superellipse(rank)
     elif name == "cfg3":
         sc = scenes.scene_cfg3(rank)
+    elif name == "cfg2proj":      # CFG2 solved by BR-MPPI proper: projection (9)-(12) inside the rollout
+        sc = scenes.scene_cfg2(rank)
+    elif name == "paperproj":     # the paper's own size: 5000 rollouts x H = 120 (T_s = 0.04 s) x 8 obstacles
+        sc = scenes.scene_cfg2(rank)
+        sc.params = sc.params.with_(K=5000, T=120, dt=0.04, n_iter=1)
     else:
         raise SystemExit(f"unknown workload {name}")
     return sc, sc.params
 
 
-def algorithmic_instr_per_sample_step(n_obs, n_discs, superellipses=None):
+PROJECTED = ("cfg2proj", "paperproj")
+
+
+def solver_flags(B, name, no_cull=False):
+    return (B.FLAG_PROJECTED if name in PROJECTED else 0) | (B.FLAG_NO_CULL if no_cull else 0)
+
+
+def oracle_solve(O, name, ps, n0, sc, U, n_threads):
+    if name in PROJECTED:
+        return O.solve_projected(ps, n0, sc.x0, sc.goal, sc.obstacles, U, n_threads=n_threads)
+    return O.solve(ps, n0, sc.x0, sc.goal, sc.obstacles, U, n_threads=n_threads, superellipses=sc.superellipses)
+
+
+def projected_instr_per_sample_step(n_obs, n_discs):
+    """issue slots of one projected sample-step.  150 fixed (control noise, perturb + clamp,
+    model step, tracking cost); 64 per Philox block of auxiliary-input normals (one per four obstacles);
+    16 + 10 D per row of (9) (obstacle position, D disc barriers, closest disc, gradient, L_g h, L_f h, b);
+    the projection (12): y, r, S = A M^-1 A^T from its rank-2-plus-diagonal form, Cholesky, two triangular
+    solves, z*, alpha update."""
+    N = n_obs
+    chol = N * (N - 1) // 2 + sum((N - 1 - c) * (c + 1) for c in range(N)) + 3 * N
+    proj = 14 + 4 * N + N * (N + 1) + chol + (N * (N - 1) + 2 * N) + (4 * N + 2) + 3 * N
+    return 150 + 64 * ((N + 3) // 4) + N * (16 + 10 * n_discs) + proj
+
+
+def algorithmic_instr_per_sample_step(n_obs, n_discs, superellipses=None, philox_per_step=1.0):
     """SURVEY.md §8(d) / DESIGN.md §6: issue slots the method itself needs per sample-step.
     Discs: 8 per (obstacle, disc).  Super-ellipses (eq. 16): 2 differences, 4 for the rotation and
-    scaling, 4 (e = 4) or 2 (e = 2) for the powers and their sum, rate argument, max, accumulate."""
-    n = 121 + 8 * n_obs * n_discs
+    scaling, 4 (e = 4) or 2 (e = 2) for the powers and their sum, rate argument, max, accumulate.
+    philox_per_step: the survey's 121 charges one Philox block (40 slots) per step; reading 6 draws one block
+    per PAIR of steps (0.5 -> 101 fixed slots)."""
+    n = 121 - int(round(40 * (1.0 - philox_per_step))) + 8 * n_obs * n_discs
     if superellipses is not None:
         for row in superellipses:
             n += (13 if int(round(row[7])) == 4 else 11) * n_discs
@@ -123,7 +155,7 @@ class ClockSampler:
                 "samples": len(sm)}
 
 
-def oracle_throughput(sc, p, seconds_target, n_threads, k_sample):
+def oracle_throughput(sc, p, seconds_target, n_threads, k_sample, name="cfg2"):
     """Time the oracle, as it stands, on a bounded sample (k_sample of the K samples, all T steps,
     all n_iter iterations).  Returns (sample-steps/s, seconds, description)."""
     from oracle import oracle as O
@@ -133,8 +165,7 @@ def oracle_throughput(sc, p, seconds_target, n_threads, k_sample):
     t0 = time.perf_counter()
     reps = 0
     while True:
-        O.solve(ps, reps * p.n_iter, sc.x0, sc.goal, sc.obstacles, U, n_threads=n_threads,
-                superellipses=sc.superellipses)
+        oracle_solve(O, name, ps, reps * p.n_iter, sc, U, n_threads)
         reps += 1
         dt = time.perf_counter() - t0
         if dt >= seconds_target or reps >= 50:
@@ -182,10 +213,10 @@ def run_reference(args):
     ps = p.with_(K=k_sample)
     U = np.zeros((p.T, 2))
     for w in range(args.warmup):
-        O.solve(ps, w, sc.x0, sc.goal, sc.obstacles, U, n_threads=cores, superellipses=sc.superellipses)
+        oracle_solve(O, args.workload, ps, w, sc, U, cores)
     t0 = time.perf_counter()
     for s in range(args.steps):
-        O.solve(ps, s, sc.x0, sc.goal, sc.obstacles, U, n_threads=cores, superellipses=sc.superellipses)
+        oracle_solve(O, args.workload, ps, s, sc, U, cores)
     dt = time.perf_counter() - t0
     value = args.steps * k_sample * p.T * p.n_iter / dt
     sample = f"each step = {k_sample} of {p.K} samples x T={p.T} x {p.n_iter} iterations, {cores} threads"
@@ -203,8 +234,10 @@ def run_reference(args):
 
 
 def workload_config(name, sc, p, n_scenes_total):
-    label = "BASELINE.json configs[2] with the paper's super-ellipse obstacles, eq. (16) (cfg2se)" if name == "cfg2se" \
-        else f"BASELINE.json configs[{name[-1]}] ({name})"
+    label = {"cfg2se": "BASELINE.json configs[2] with the paper's super-ellipse obstacles, eq. (16) (cfg2se)",
+             "cfg2proj": "BASELINE.json configs[2] solved by BR-MPPI proper: projection (9)-(12) inside the rollout (cfg2proj)",
+             "paperproj": "the paper's size, 5000 rollouts x H = 120 x 8 obstacles (PAPER.md:243), projected rollout of the reduced model (paperproj)",
+             }.get(name, f"BASELINE.json configs[{name[-1]}] ({name})")
     return {"workload": label, "K": p.K, "T": p.T,
             "n_obstacles": int(len(sc.obstacles)),
             "n_superellipses": 0 if sc.superellipses is None else int(len(sc.superellipses)),
@@ -214,17 +247,14 @@ def workload_config(name, sc, p, n_scenes_total):
             "parallelism": "independent replicas, one scene per GPU, no collective on the data path"}
 
 
-def run_ours(args):
-    import torch
-    from paper_2508_05773_b200 import brmppi as B
-
-    rank, world, local_rank, dist = dist_setup(args.gpus)
-    dev = f"cuda:{local_rank}"
-    torch.cuda.set_device(dev)
-    sc, p = workload(args.workload, rank)
+def measure(B, torch, name, rank, steps, warmup, dist, dev, local_rank, closed_loop_steps, with_clocks):
+    """One workload on this rank: device-resident throughput (CUDA events on the solver's stream, L2 flushed
+    between steps), end to end through the C ABI with pinned host buffers, closed-loop brmppi_step latency,
+    kernel times by CUDA events (with and without culling)."""
+    sc, p = workload(name, rank)
     n_obs = len(sc.obstacles)
     n_se = 0 if sc.superellipses is None else len(sc.superellipses)
-    solver = B.Solver(p, 1, max(n_obs, 1), 0, device=dev, max_superellipses=n_se)
+    solver = B.Solver(p, 1, max(n_obs, 1), solver_flags(B, name), device=dev, max_superellipses=n_se)
     solver.set_scene(sc)
     stream = solver.stream
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
@@ -235,14 +265,13 @@ def run_ours(args):
             dist.barrier()
             torch.cuda.synchronize()
 
-    # ---- device-resident throughput: inputs already in HBM, CUDA events on the solver's stream
-    for _ in range(max(args.warmup, 3)):
+    for _ in range(max(warmup, 3)):
         solver.solve()
     barrier()
-    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
     launches0 = solver.launch_count()
-    sampler = ClockSampler(local_rank)
-    if rank == 0:
+    sampler = ClockSampler(local_rank) if with_clocks else None
+    if sampler:
         sampler.start()
     t_wall0 = time.perf_counter()
     for a, b in ev:
@@ -254,15 +283,14 @@ def run_ours(args):
     barrier()
     wall_s = time.perf_counter() - t_wall0
     launches = solver.launch_count() - launches0
-    step_ms = [a.elapsed_time(b) for a, b in ev]
-    dev_s = sum(step_ms) * 1e-3
+    dev_s = sum(a.elapsed_time(b) for a, b in ev) * 1e-3
     dev_s_max = max_over_ranks(dev_s, dist, dev)
-    work_per_rank = args.steps * p.K * p.T * p.n_iter
 
     # ---- end to end through the C ABI with host buffers (pinned), host clock
     pin = lambda a: torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).pin_memory().numpy()
     hx, hg, ho = pin(sc.x0), pin(sc.goal), pin(sc.obstacles)
     hs = None if n_se == 0 else sc.superellipses
+
     def set_inputs():
         solver.set_state(hx); solver.set_goal(hg); solver.set_obstacles(ho)
         if hs is not None:
@@ -271,84 +299,173 @@ def run_ours(args):
         set_inputs(); solver.solve(); solver.get_controls()
     barrier()
     t0 = time.perf_counter()
-    for _ in range(args.steps):
+    for _ in range(steps):
         set_inputs()
         solver.solve()
-        U = solver.get_controls()                            # synchronises; T*2 floats back
+        solver.get_controls()                                # synchronises; T*2 floats back
     barrier()
-    e2e_s = time.perf_counter() - t0
-    e2e_s_max = max_over_ranks(e2e_s, dist, dev)
+    e2e_s_max = max_over_ranks(time.perf_counter() - t0, dist, dev)
     h2d = 16 + 16 + 20 * n_obs + 4 + (32 * n_se + 4 if n_se else 0)
     d2h = 8 * p.T
 
     # ---- closed-loop control rate (CUDA-graph replay of solve + plant step + shift)
     lat = []
-    for i in range(20 + min(args.steps, 200)):
+    for i in range(20 + closed_loop_steps):
         t1 = time.perf_counter()
         solver.step()
         if i >= 20:
             lat.append(time.perf_counter() - t1)
-    clocks = sampler.stop() if rank == 0 else None   # sampled across all three timed regions
+    clocks = sampler.stop() if sampler else None             # sampled across all three timed regions
     lat.sort()
     p50, p99 = lat[len(lat) // 2], lat[min(len(lat) - 1, int(0.99 * len(lat)))]
 
-    # ---- roofline of the rollout kernel (rank 0): device time per launch from CUDA events
+    # ---- kernel times (rank 0): device time per launch from CUDA events on the solver's stream
     roof = None
     if rank == 0:
         solver.set_scene(sc)
         solver.set_nominal(None)
         ms_roll, ms_upd = solver.time_kernels(50)
-        instr = algorithmic_instr_per_sample_step(n_obs, len(p.discs), sc.superellipses)
-        achieved = p.K * p.T * instr / (ms_roll * 1e-3) / 1e9          # G thread-instr / s
+        ms_nocull = None
+        if name not in PROJECTED:                            # the same launch with every (obstacle, disc, step) evaluated
+            s2 = B.Solver(p, 1, max(n_obs, 1), solver_flags(B, name, no_cull=True), device=dev, max_superellipses=n_se)
+            s2.set_scene(sc)
+            for _ in range(3):
+                s2.solve()
+            s2.set_scene(sc); s2.set_nominal(None)
+            ms_nocull = s2.time_kernels(50)[0]
+            s2.close()
         mp = measured_peaks()
         sm_max = float(mp.get("sm_max_mhz", SM_MAX_MHZ_FALLBACK))
         peak = N_SMS * ISSUE_PER_CLK_PER_SM * sm_max * 1e6 / 1e9
+        if name in PROJECTED:
+            instr = projected_instr_per_sample_step(n_obs, len(p.discs))
+            instr_pair = instr
+        else:
+            instr = algorithmic_instr_per_sample_step(n_obs, len(p.discs), sc.superellipses)
+            instr_pair = algorithmic_instr_per_sample_step(n_obs, len(p.discs), sc.superellipses, philox_per_step=0.5)
+        achieved = p.K * p.T * instr / (ms_roll * 1e-3) / 1e9          # G thread-instr / s
+        traffic, traffic_source = dram_traffic_from_profile()
         roof = {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "Ginstr/s (thread-instructions)",
-                "frac": achieved / peak, "traffic": dram_traffic_from_profile(),
-                "kernel": "rollout_cta", "kernel_ms": ms_roll, "update_kernel_ms": ms_upd,
-                "kernel_share_of_step": ms_roll * p.n_iter / (dev_s / args.steps * 1e3),
+                "frac": achieved / peak, "traffic": traffic if name == "cfg2" else None,
+                "traffic_source": traffic_source if name == "cfg2" else None,
+                "kernel": "rollout_projected" if name in PROJECTED else "rollout_cta",
+                "kernel_ms": ms_roll, "update_kernel_ms": ms_upd,
+                "kernel_share_of_step": ms_roll * p.n_iter / (dev_s / steps * 1e3),
                 "algorithmic_instr_per_sample_step": instr,
+                "frac_with_one_philox_block_per_step_pair": p.K * p.T * instr_pair / (ms_roll * 1e-3) / 1e9 / peak,
+                "algorithmic_instr_per_sample_step_pair_blocks": instr_pair,
+                "kernel_ms_no_cull": ms_nocull,
+                "frac_no_cull": None if ms_nocull is None else p.K * p.T * instr / (ms_nocull * 1e-3) / 1e9 / peak,
+                "culling": None if ms_nocull is None else "exact (bit-identical results, DESIGN.md 6.5): frac counts "
+                           "every (obstacle, disc, step) the method defines as useful work; frac_no_cull is the same "
+                           "launch with all of them executed (BRMPPI_FLAG_NO_CULL)",
                 "peak_basis": f"{N_SMS} SMs x {ISSUE_PER_CLK_PER_SM} thread-instr/clk/SM x {sm_max:.0f} MHz "
                               f"({'MEASURED_PEAKS.json sm_max_mhz' if 'sm_max_mhz' in mp else 'fallback clock'}); "
                               "issue rate confirmed by brmppi_measure_peaks (DESIGN.md §6)"}
     solver.close()
+    del flush
+    return dict(sc=sc, p=p, dev_s=dev_s, dev_s_max=dev_s_max, e2e_s_max=e2e_s_max, h2d=h2d, d2h=d2h, p50=p50, p99=p99,
+                launches=int(launches), clocks=clocks, roof=roof, wall_s=wall_s, steps=steps)
 
+
+def record(name, m, world):
+    """Compact record of a secondary workload for the `others` key of the JSON line."""
+    p, steps = m["p"], m["steps"]
+    work = steps * p.K * p.T * p.n_iter
+    r = m["roof"] or {}
+    return {"workload": name, "K": p.K, "T": p.T, "n_obstacles": int(len(m["sc"].obstacles)), "n_iter": p.n_iter, "steps": steps,
+            "value": world * work / m["dev_s_max"], "unit": UNIT, "ms_per_step": m["dev_s_max"] / steps * 1e3,
+            "e2e_value": world * work / m["e2e_s_max"],
+            "closed_loop_p50_ms": m["p50"] * 1e3, "closed_loop_p99_ms": m["p99"] * 1e3, "closed_loop_hz": 1.0 / m["p50"],
+            "kernel": r.get("kernel"), "kernel_ms": r.get("kernel_ms"), "update_kernel_ms": r.get("update_kernel_ms"),
+            "frac": r.get("frac"), "kernel_ms_no_cull": r.get("kernel_ms_no_cull"), "frac_no_cull": r.get("frac_no_cull"),
+            "algorithmic_instr_per_sample_step": r.get("algorithmic_instr_per_sample_step"), "gpu_launches": m["launches"]}
+
+
+def batch64_record(B):
+    """BASELINE.json configs[4]'s batched launch: 64 scenes x K = 16384, T = 80, 8 obstacles in one launch."""
+    batch = scenes.scene_batch(64, 16384, 80)
+    p = batch[0].params.with_(seed=0)
+    s = B.Solver(p, 64, 8, 0)
+    for i, sc in enumerate(batch):
+        s.set_scene(sc, i)
+    for _ in range(3):
+        s.solve()
+    s.synchronize()
+    ms_roll, ms_upd = s.time_kernels(10)
+    s.close()
+    work = 64 * p.K * p.T
+    instr = algorithmic_instr_per_sample_step(8, len(p.discs))
+    peak = N_SMS * ISSUE_PER_CLK_PER_SM * float(measured_peaks().get("sm_max_mhz", SM_MAX_MHZ_FALLBACK)) * 1e6
+    return {"workload": "batch64", "n_scenes": 64, "K": p.K, "T": p.T, "n_obstacles": 8, "kernel_ms": ms_roll,
+            "update_kernel_ms": ms_upd, "value": work / ((ms_roll + ms_upd) * 1e-3), "unit": UNIT,
+            "frac": work * instr / (ms_roll * 1e-3) / peak}
+
+
+def run_ours(args):
+    import torch
+    from paper_2508_05773_b200 import brmppi as B
+
+    rank, world, local_rank, dist = dist_setup(args.gpus)
+    dev = f"cuda:{local_rank}"
+    torch.cuda.set_device(dev)
+    m = measure(B, torch, args.workload, rank, args.steps, args.warmup, dist, dev, local_rank,
+                min(args.steps, 200), with_clocks=(rank == 0))
     if rank != 0:
         return
-    cpu = None
-    if world == 1 or rank == 0:
-        cores = os.cpu_count() or 1
-        v1, s1, d1 = oracle_throughput(sc, p, 6.0, 1, min(p.K, 2048))
-        vn, sn, dn = oracle_throughput(sc, p, 8.0, cores, min(p.K, 8192))
-        cpu = {"value": vn, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": dn,
-               "value_1core": v1, "sample_1core": d1}
-    value = whole_job_value(work_per_rank, world, dev_s_max)
+    sc, p = m["sc"], m["p"]
+    work_per_rank = args.steps * p.K * p.T * p.n_iter
+    # the other BASELINE.json configs, the 64-scene batch and the projected rollout: N = 1 only, shorter runs
+    others = []
+    if world == 1 and not args.no_others:
+        for name in ("cfg0", "cfg1", "cfg2", "cfg3", "cfg2se", "cfg2proj", "paperproj"):
+            if name != args.workload:
+                steps_o = 20 if name in PROJECTED else 50
+                others.append(record(name, measure(B, torch, name, 0, steps_o, 5, None, dev, local_rank, 100, False), 1))
+        others.append(batch64_record(B))
+    cores = os.cpu_count() or 1
+    v1, s1, d1 = oracle_throughput(sc, p, 6.0, 1, min(p.K, 2048), args.workload)
+    vn, sn, dn = oracle_throughput(sc, p, 8.0, cores, min(p.K, 8192), args.workload)
+    cpu = {"value": vn, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": dn,
+           "value_1core": v1, "sample_1core": d1}
+    dev_s_max, e2e_s_max = m["dev_s_max"], m["e2e_s_max"]
     line = {
-        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-        "warmup": max(args.warmup, 3), "ms_per_step": dev_s_max / args.steps * 1e3,
+        "metric": METRIC, "value": whole_job_value(work_per_rank, world, dev_s_max), "unit": UNIT, "n_gpus": world,
+        "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": dev_s_max / args.steps * 1e3,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
         "data": "synthetic", "config": workload_config(args.workload, sc, p, world),
         "solves_per_s": world * args.steps * p.n_iter / dev_s_max,
         "control_steps_per_s": world * args.steps / dev_s_max,
-        "e2e": {"value": whole_job_value(work_per_rank, world, e2e_s_max), "unit": UNIT, "h2d_bytes_per_step": h2d,
-                "d2h_bytes_per_step": d2h, "control_steps_per_s": world * args.steps / e2e_s_max},
-        "closed_loop": {"p50_ms": p50 * 1e3, "p99_ms": p99 * 1e3, "hz": 1.0 / p50,
+        "e2e": {"value": whole_job_value(work_per_rank, world, e2e_s_max), "unit": UNIT, "h2d_bytes_per_step": m["h2d"],
+                "d2h_bytes_per_step": m["d2h"], "control_steps_per_s": world * args.steps / e2e_s_max},
+        "closed_loop": {"p50_ms": m["p50"] * 1e3, "p99_ms": m["p99"] * 1e3, "hz": 1.0 / m["p50"],
                         "what": "brmppi_step: graph replay of solve + plant step + shift, host wall clock"},
-        "gpu_launches": int(launches), "clocks": clocks, "roofline": roof, "cpu_baseline": cpu,
-        "wall_s_timed_region": wall_s,
-        "paper_context": "paper: 9.9 ms per MPPI step, >100 Hz, 5000 rollouts x H=120, 8 obstacles, JAX on an unnamed GPU (PAPER.md:5,243) -- different formulation, context only",
+        "gpu_launches": m["launches"], "clocks": m["clocks"], "roofline": m["roof"], "cpu_baseline": cpu,
+        "wall_s_timed_region": m["wall_s"], "others": others,
+        "paper_context": "paper: 9.9 ms per MPPI step, >100 Hz, 5000 rollouts x H=120, 8 obstacles, JAX on an unnamed GPU (PAPER.md:5,243) -- full formulation (7-state model, contouring cost), context only; the `paperproj` record under `others` is the same size solved by this library's projected rollout of the reduced model",
     }
     print(json.dumps(line))
 
 
-def dram_traffic_from_profile(name="r1_rollout_cta_dram.csv"):
-    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the
-    committed ncu capture (profiles/<name>: header line, then bytes)."""
+def spawn_ranks(args):
+    """`python bench.py --gpus N` without a torchrun environment: start the N ranks here (one process per GPU)."""
+    import socket
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    raise SystemExit(subprocess.call(cmd))
+
+
+def dram_traffic_from_profile(name="r2_rollout_cta_dram.csv"):
+    """(dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, where it comes from):
+    NOT measured in this run -- read from the committed ncu capture profiles/<name> (header line, then bytes)."""
     try:
         rows = open(os.path.join(ROOT, "profiles", name)).read().strip().splitlines()
-        return float(rows[-1].split(",")[-1])
+        return float(rows[-1].split(",")[-1]), f"profiles/{name} (committed ncu --set full capture, not this run)"
     except Exception:
-        return None
+        return None, None
 
 
 def run_phases(args):
@@ -431,13 +548,17 @@ def run_project(args):
     bytes_alg = n * 4 * (n_o * d + n_o + 2 * d)          # A, b, z_des in; z out
     mp = measured_peaks()
     peak = float(mp.get("hbm_gbs", 6500.0))
-    # end to end through the C ABI with HOST buffers: the call copies A, b, z_des in and z out itself
-    hA, hb, hz = (np.ascontiguousarray(P[k], dtype=np.float32) for k in ("A", "b", "z_des"))
-    B.project(hA, hb, hz, P["w"], P["rho"], P["z_lo"], P["z_hi"])
-    reps = 3
+    # end to end through the C ABI with HOST buffers (page-locked) and a caller-owned device scratch: the call
+    # copies A, b, z_des in and z out itself
+    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).pin_memory()
+    hA, hb, hz = pin(P["A"]), pin(P["b"]), pin(P["z_des"])
+    hout = torch.empty((n, d), dtype=torch.float32).pin_memory()
+    scratch = torch.empty(B.lib().brmppi_project_scratch_bytes(n, n_o), dtype=torch.uint8, device="cuda")
+    B.project(hA, hb, hz, P["w"], P["rho"], P["z_lo"], P["z_hi"], out=hout, scratch=scratch)
+    reps = 5
     t0 = time.perf_counter()
     for _ in range(reps):
-        B.project(hA, hb, hz, P["w"], P["rho"], P["z_lo"], P["z_hi"])
+        B.project(hA, hb, hz, P["w"], P["rho"], P["z_lo"], P["z_hi"], out=hout, scratch=scratch)
     t_e2e = (time.perf_counter() - t0) / reps
     from oracle import projection as OP
     m = 20000
@@ -452,11 +573,12 @@ def run_project(args):
         "config": {"workload": "eq. (12), 5000 x 120 problems, N_o = 8 (PAPER.md:243)", "n": n, "n_o": n_o,
                    "l2": "flushed between timed launches (256 MiB write)"},
         "gpu_launches": args.steps,
-        "e2e": {"value": n / t_e2e, "unit": "projections/s", "h2d_bytes_per_step": int(hA.nbytes + hb.nbytes + hz.nbytes),
-                "d2h_bytes_per_step": int(hz.nbytes), "what": "brmppi_project with host pointers (pageable numpy arrays; "
-                "the call allocates and frees its device scratch), host wall clock"},
+        "e2e": {"value": n / t_e2e, "unit": "projections/s", "h2d_bytes_per_step": int(4 * (hA.numel() + hb.numel() + hz.numel())),
+                "d2h_bytes_per_step": int(4 * hout.numel()), "what": "brmppi_project with page-locked host pointers and a "
+                "caller-owned device scratch, host wall clock"},
         "roofline": {"bound": "hbm", "achieved": bytes_alg / t / 1e9, "peak": peak, "unit": "GB/s",
-                     "frac": bytes_alg / t / 1e9 / peak, "traffic": dram_traffic_from_profile("r1d_project_dram.csv"), "kernel": "project_batch_bulk<8> (persistent; its last CTA takes the 64-problem tail)",
+                     "frac": bytes_alg / t / 1e9 / peak, "traffic": dram_traffic_from_profile("r1d_project_dram.csv")[0],
+                     "traffic_source": dram_traffic_from_profile("r1d_project_dram.csv")[1], "kernel": "project_batch_bulk<8> (persistent; its last CTA takes the 64-problem tail)",
                      "algorithmic_bytes_per_problem": bytes_alg // n,
                      "peak_basis": "MEASURED_PEAKS.json hbm_gbs" if "hbm_gbs" in mp else "fallback 6500 GB/s"},
         "cpu_baseline": {"value": m / t_cpu, "unit": "projections/s", "cores": 1, "kind": "oracle",
@@ -469,12 +591,15 @@ def main():
     ap.add_argument("--steps", type=int, default=200)
     ap.add_argument("--warmup", type=int, default=20)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="cfg2", choices=["cfg0", "cfg1", "cfg2", "cfg2se", "cfg3"])
+    ap.add_argument("--workload", default="cfg2", choices=["cfg0", "cfg1", "cfg2", "cfg2se", "cfg3", "cfg2proj", "paperproj"])
+    ap.add_argument("--no-others", action="store_true", help="skip the secondary workloads of the `others` key")
     ap.add_argument("--phases", action="store_true", help="print the rollout kernel's in-kernel phase times")
     ap.add_argument("--sweep", action="store_true", help="run BASELINE.json configs[4] (sweep + 64-scene batch)")
     ap.add_argument("--project", action="store_true", help="time the closed-form projection (12) on its own")
     ap.add_argument("--no-cull", action="store_true", help="evaluate every (obstacle, disc, step): BRMPPI_FLAG_NO_CULL")
     args = ap.parse_args()
+    if args.gpus > 1 and int(os.environ.get("WORLD_SIZE", "1")) <= 1 and not (args.project or args.phases or args.sweep):
+        spawn_ranks(args)          # reference arm included: rank 0 runs it, the others exit 0
     if args.project:
         run_project(args)
     elif args.phases:

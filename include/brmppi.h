@@ -81,6 +81,12 @@ typedef struct { int body; float offset; } brmppi_disc;
 #define BRMPPI_FLAG_PHASE_TIMING 8u     /* persistent kernel: every CTA records SM cycles per phase
                                           (clock64, bracketed by the globaltimer for the conversion
                                           to time); read with brmppi_get_phase_times            */
+#define BRMPPI_FLAG_PROJECTED 32u       /* BR-MPPI proper (Sec. V-A): every sampled input is
+                                          projected onto the barrier-rate equality (9) by the closed form
+                                          (12) inside the rollout; per-obstacle alpha_i driven by the projected
+                                          auxiliary input; no hinge penalty (w_bar is not read).  Readings:
+                                          DESIGN.md reading 30.  max_obstacles <= BRMPPI_PROJECT_MAX_NO, no
+                                          super-ellipses; one thread per sample.                            */
 #define BRMPPI_FLAG_NO_CULL 16u         /* evaluate every (obstacle, disc, step) even where the
                                           hinge is provably zero; same results  */
 
@@ -108,11 +114,18 @@ typedef struct {
                              it is applied to the plant.  Never changes U itself.                 */
   float hitch_alpha;      /* alpha of condition (3), in (0, 1]         (read only if hitch_filter) */
   float hitch_qv, hitch_qdelta;   /* Q_h = diag(q_v, q_delta), both > 0 (read only if hitch_filter) */
+  /* Projected rollout (read only with BRMPPI_FLAG_PROJECTED).  z = [v, omega = v tan(delta), u^alpha_1..N_o]:
+   * W = Diag(Q1, Q2) with Q1 = diag(proj_qv, proj_qomega), Q2 = proj_qalpha I (all > 0), soft-bound weight
+   * proj_rho >= 0 of (11a); bounds z_lo / z_hi = (v_min, -omega_max, -ualpha_max ..) / (v_max, omega_max,
+   * ualpha_max ..), omega_max = max|v| tan(max|delta|); sampled u~^alpha ~ N(0, sigma_ualpha^2); stage cost
+   * w_alpha * sum_i [h_i < h_buffer] max(0, alpha_i)^2.                                       */
+  float proj_qv, proj_qomega, proj_qalpha, proj_rho, sigma_ualpha, ualpha_max, w_alpha, h_buffer;
 } brmppi_params;
 
 #define BRMPPI_MAX_T 512
 #define BRMPPI_MAX_OBSTACLES 64
 #define BRMPPI_MAX_SUPERELLIPSES 16
+#define BRMPPI_PROJECT_MAX_NO 8     /* obstacles (rows of (9)) the projection handles */
 
 typedef struct brmppi_ctx brmppi_ctx;   /* opaque, library-owned host object */
 
@@ -245,7 +258,6 @@ int brmppi_hitch_filter(void* cuda_stream, const brmppi_params* p, int n, const 
                         const float* u_ref, float* u_out, int* status_out, void* dev_scratch,
                         size_t scratch_bytes);
 
-#define BRMPPI_PROJECT_MAX_NO 8
 /* Closed-form projection of BR-MPPI, eq. (11)-(12), for n independent problems:
  *   min_z ||z - z_des||_W^2 + rho/2 (||z - z_lo||^2 + ||z_hi - z||^2)   s.t.  A z = b,
  *   z* = M^-1 [ p - A^T (A M^-1 A^T)^-1 (A M^-1 p - b) ],  M = W + rho I,  p = W z_des + rho/2 (z_hi + z_lo),

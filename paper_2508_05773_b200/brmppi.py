@@ -15,6 +15,7 @@ FLAG_PRECISE_MATH = 2
 FLAG_KERNEL_THREAD_PER_SAMPLE = 4
 FLAG_PHASE_TIMING = 8
 FLAG_NO_CULL = 16
+FLAG_PROJECTED = 32
 
 OK = 0
 ERR_NULL, ERR_INVALID_ARG, ERR_WORKSPACE_TOO_SMALL, ERR_TOO_MANY_OBSTACLES = -1, -2, -3, -4
@@ -60,7 +61,9 @@ class CParams(C.Structure):
                 ("w_bar", C.c_float), ("w_term", C.c_float), ("lam", C.c_float),
                 ("seed", C.c_ulonglong), ("flags", C.c_uint), ("max_superellipses", C.c_int),
                 ("hitch_kappa", C.c_float), ("hitch_filter", C.c_int), ("hitch_alpha", C.c_float),
-                ("hitch_qv", C.c_float), ("hitch_qdelta", C.c_float)]
+                ("hitch_qv", C.c_float), ("hitch_qdelta", C.c_float),
+                ("proj_qv", C.c_float), ("proj_qomega", C.c_float), ("proj_qalpha", C.c_float), ("proj_rho", C.c_float),
+                ("sigma_ualpha", C.c_float), ("ualpha_max", C.c_float), ("w_alpha", C.c_float), ("h_buffer", C.c_float)]
 
 
 class Diag(C.Structure):
@@ -156,6 +159,9 @@ def make_cparams(p, n_scenes=1, max_obstacles=8, flags=0, max_superellipses=0) -
     c.hitch_alpha = float(getattr(p, "hitch_alpha", 0.5))
     c.hitch_qv = float(getattr(p, "hitch_qv", 1.0))
     c.hitch_qdelta = float(getattr(p, "hitch_qdelta", 1.0))
+    for name, default in (("proj_qv", 1.0), ("proj_qomega", 4.0), ("proj_qalpha", 0.5), ("proj_rho", 0.25),
+                          ("sigma_ualpha", 0.3), ("ualpha_max", 1.0), ("w_alpha", 10.0), ("h_buffer", 0.5)):
+        setattr(c, name, float(getattr(p, name, default)))
     return c
 
 

@@ -14,6 +14,7 @@
 #include "brmppi_device.cuh"
 #include "peaks.cuh"
 #include "rollout_thread.cuh"
+#include "rollout_projected.cuh"
 #include "rollout_cta.cuh"
 #include "rollout_cta_kernel.cuh"
 #include "update.cuh"
@@ -80,8 +81,16 @@ bool params_valid(const brmppi_params* p) {
   if (p->alpha_lo > p->alpha_hi) return false;
   const unsigned known = BRMPPI_FLAG_WRITE_SAMPLES | BRMPPI_FLAG_PRECISE_MATH |
                          BRMPPI_FLAG_KERNEL_THREAD_PER_SAMPLE | BRMPPI_FLAG_PHASE_TIMING |
-                         BRMPPI_FLAG_NO_CULL;
+                         BRMPPI_FLAG_NO_CULL | BRMPPI_FLAG_PROJECTED;
   if (p->flags & ~known) return false;
+  if (p->flags & BRMPPI_FLAG_PROJECTED) {
+    if (p->max_obstacles > BRMPPI_PROJECT_MAX_NO || p->max_superellipses > 0) return false;
+    const float q[] = {p->proj_qv, p->proj_qomega, p->proj_qalpha, p->proj_rho, p->sigma_ualpha, p->ualpha_max,
+                       p->w_alpha, p->h_buffer};
+    if (!finite_all(q, 8)) return false;
+    if (!(p->proj_qv > 0.f) || !(p->proj_qomega > 0.f) || !(p->proj_qalpha > 0.f)) return false;
+    if (p->proj_rho < 0.f || p->sigma_ualpha < 0.f || p->ualpha_max < 0.f || p->w_alpha < 0.f) return false;
+  }
   return true;
 }
 
@@ -110,7 +119,7 @@ int device_sm_count() {
 
 Plan make_plan(const brmppi_params& p) {
   Plan pl{};
-  pl.cta_kernel = !(p.flags & BRMPPI_FLAG_KERNEL_THREAD_PER_SAMPLE);
+  pl.cta_kernel = !(p.flags & (BRMPPI_FLAG_KERNEL_THREAD_PER_SAMPLE | BRMPPI_FLAG_PROJECTED));
   if (pl.cta_kernel) {
     pl.cta = make_cta_plan(p.K, p.T, p.n_scenes, p.max_obstacles, p.max_superellipses, device_sm_count());
     pl.n_partials = pl.cta.n_partials;
@@ -176,6 +185,10 @@ int launch_rollout(brmppi_ctx* c) {
   const bool precise = (c->p.flags & BRMPPI_FLAG_PRECISE_MATH) != 0;
   if (c->plan.cta_kernel) {
     CU(launch_rollout_cta(d, c->plan.cta, precise, c->stream));
+  } else if (c->p.flags & BRMPPI_FLAG_PROJECTED) {
+    dim3 grid((unsigned)c->plan.n_partials, (unsigned)d.n_scenes);
+    projected_kernel_for(precise, d.max_obstacles)<<<grid, kThreadBlock, c->smem_rollout, c->stream>>>(d);
+    CU(cudaGetLastError());
   } else {
     dim3 grid((unsigned)c->plan.n_partials, (unsigned)d.n_scenes);
     if (precise)
@@ -299,6 +312,8 @@ int brmppi_create(const brmppi_params* p, void* dev_workspace, size_t workspace_
   d.inv_lambda = 1.0f / p->lambda;
   d.hitch_filter = p->hitch_filter; d.hitch_alpha = p->hitch_alpha;
   d.hitch_qv = p->hitch_qv; d.hitch_qdelta = p->hitch_qdelta;
+  d.proj_qv = p->proj_qv; d.proj_qomega = p->proj_qomega; d.proj_qalpha = p->proj_qalpha; d.proj_rho = p->proj_rho;
+  d.sigma_ualpha = p->sigma_ualpha; d.ualpha_max = p->ualpha_max; d.w_alpha = p->w_alpha; d.h_buffer = p->h_buffer;
   d.key0 = (uint32_t)(p->seed & 0xFFFFFFFFull); d.key1 = (uint32_t)(p->seed >> 32);
   d.flags = p->flags;
   d.n_partials = c->plan.n_partials;
@@ -337,7 +352,11 @@ int brmppi_create(const brmppi_params* p, void* dev_workspace, size_t workspace_
   } else {
     c->smem_rollout = rollout_thread_smem_bytes(d);
     // per function and device, not per context: always the opt-in maximum, never lowered
-    e = cudaFuncSetAttribute(rollout_thread_per_sample<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)prop.sharedMemPerBlockOptin);
+    if (p->flags & BRMPPI_FLAG_PROJECTED)
+      e = cudaFuncSetAttribute(projected_kernel_for((p->flags & BRMPPI_FLAG_PRECISE_MATH) != 0, p->max_obstacles),
+                               cudaFuncAttributeMaxDynamicSharedMemorySize, (int)prop.sharedMemPerBlockOptin);
+    if (e == cudaSuccess)
+      e = cudaFuncSetAttribute(rollout_thread_per_sample<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)prop.sharedMemPerBlockOptin);
     if (e == cudaSuccess)
       e = cudaFuncSetAttribute(rollout_thread_per_sample<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)prop.sharedMemPerBlockOptin);
   }

@@ -33,6 +33,7 @@ struct DeviceParams {
   float inv_lambda;
   int hitch_filter;            // 1: shift_plant passes U[0] through the CBF-QP of Sec. V-D
   float hitch_alpha, hitch_qv, hitch_qdelta;
+  float proj_qv, proj_qomega, proj_qalpha, proj_rho, sigma_ualpha, ualpha_max, w_alpha, h_buffer;   // BRMPPI_FLAG_PROJECTED
   uint32_t key0, key1;        // Philox key of scene 0 = (lo32(seed), hi32(seed)); scene s adds s
   uint32_t flags;
   // tiling of the sample axis

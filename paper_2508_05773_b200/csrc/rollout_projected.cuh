@@ -1,0 +1,266 @@
+// rollout_projected.cuh -- BR-MPPI proper (Sec. V-A): at every
+// prediction step the sampled inputs are PROJECTED onto the barrier-rate equality (9) by the closed form
+// (12), the projected input drives the model, the projected auxiliary input drives alpha_i.  Selected by
+// BRMPPI_FLAG_PROJECTED; readings in DESIGN.md (reading 30).
+//
+// One thread per sample, NO = obstacle capacity as a template parameter so that everything -- the rows
+// of (9), the N_o x N_o matrix A M^-1 A^T, its Cholesky factor -- lives in registers.  Nothing of a step
+// touches HBM: A and b are built from the state, not streamed.
+//
+// What (9) looks like for the reduced model: with the inputs w = (v, omega), omega = v tan(delta), the model
+// is x' = x + dt G(x) w, so row i is   L_g h_i . w + h_i u^alpha_i = -alpha_i h_i - L_f h_i,
+//   A = [ L_g h (N_o x 2) | diag(h) ],   M = diag(q_v + rho, q_omega + rho, q_alpha + rho ...),
+// and S = A M^-1 A^T = G' M_u^-1 G'^T + diag(h_i^2 / m_alpha) needs three multiply-adds per entry.
+//
+// The serial chain per step is long (about 1100 instructions, eight obstacle rows of independent work
+// in it), so a warp brings its own instruction-level parallelism; 128-thread CTAs put one warp on each
+// scheduler of an SM.
+#pragma once
+
+#include "rollout_thread.cuh"
+
+namespace brmppi {
+
+// The four standard normals of Philox block (t, n, k, tag): Box-Muller on words (0,1) and (2,3).
+template <bool PRECISE>
+__device__ __forceinline__ void normals4(uint32_t t, uint32_t n, uint32_t k, uint32_t tag, uint32_t key0,
+                                         uint32_t key1, float (&z)[4]) {
+  const uint4 w = philox4x32_10(t, n, k, tag, key0, key1);
+  const float2 a = box_muller<PRECISE>(w.x, w.y), b = box_muller<PRECISE>(w.z, w.w);
+  z[0] = a.x; z[1] = a.y; z[2] = b.x; z[3] = b.y;
+}
+
+// Rows of (9) for all obstacles at state X, step t: h_i on the closest disc (lowest index on ties),
+// L_g h_i (2), L_f h_i.  Obstacle i: sObs = (ox, oy, 1/rho^2, -) in the vehicle frame, sVel = dt vel.
+template <bool PRECISE, int NO>
+__device__ __forceinline__ void barrier_rows(const DeviceParams& P, const State& X, int n_obs, float tf,
+                                             const float4* __restrict__ sObs, const float2* __restrict__ sVel,
+                                             float (&h)[NO], float (&g0)[NO], float (&g1)[NO], float (&lf)[NO]) {
+  float s1, c1, s2, c2;
+  sincos_t<PRECISE>(X.psi1, &s1, &c1);
+  sincos_t<PRECISE>(X.psi2, &s2, &c2);
+  float cx[kMaxDiscs], cy[kMaxDiscs];
+  disc_centres(P, X, s1, c1, s2, c2, cx, cy);
+  const float sb = s1 * c2 - c1 * s2, cb = fmaf(c1, c2, s1 * s2);   // sin / cos (psi1 - psi2)
+  // d c_j / d psi1 and d c_j / d psi2 (c = p_h + a e(psi_body), p_h = (x - Lh cos psi1, y - Lh sin psi1))
+  float d1x[kMaxDiscs], d1y[kMaxDiscs], d2x[kMaxDiscs], d2y[kMaxDiscs];
+#pragma unroll
+  for (int j = 0; j < kMaxDiscs; ++j) {
+    const float a1 = P.disc_a1[j] - P.Lh, a2 = P.disc_a2[j];
+    d1x[j] = -a1 * s1; d1y[j] = a1 * c1;
+    d2x[j] = -a2 * s2; d2y[j] = a2 * c2;
+  }
+#pragma unroll
+  for (int i = 0; i < NO; ++i) {
+    if (i < n_obs) {
+      const float4 o = sObs[i];
+      const float2 w = sVel[i];
+      const float ox = fmaf(tf, w.x, o.x), oy = fmaf(tf, w.y, o.y);                 // o(t)
+      float hb = 0.0f, ex = 0.0f, ey = 0.0f, b1x = 0.0f, b1y = 0.0f, b2x = 0.0f, b2y = 0.0f;
+#pragma unroll
+      for (int j = 0; j < kMaxDiscs; ++j) {
+        if (j < P.n_discs) {
+          const float dx = cx[j] - ox, dy = cy[j] - oy;
+          const float hj = fmaf(fmaf(dx, dx, dy * dy), o.z, -1.0f);
+          if (j == 0 || hj < hb) { hb = hj; ex = dx; ey = dy; b1x = d1x[j]; b1y = d1y[j]; b2x = d2x[j]; b2y = d2y[j]; }
+        }
+      }
+      const float gx = 2.0f * ex * o.z, gy = 2.0f * ey * o.z;                       // grad_c h
+      const float dpsi1 = fmaf(gx, b1x, gy * b1y), dpsi2 = fmaf(gx, b2x, gy * b2y);
+      h[i] = hb;
+      g0[i] = P.dt * fmaf(gx, c1, fmaf(gy, s1, dpsi2 * sb * P.inv_L2));
+      g1[i] = P.dt * fmaf(dpsi1, P.inv_L1, -(dpsi2 * P.Lh_over_L1 * P.inv_L2) * cb);
+      lf[i] = -fmaf(gx, w.x, gy * w.y);                                             // w = dt vel
+    } else {
+      h[i] = 1.0f; g0[i] = 0.0f; g1[i] = 0.0f; lf[i] = 0.0f;
+    }
+  }
+}
+
+template <bool PRECISE, int NO>
+__global__ void __launch_bounds__(kThreadBlock)
+rollout_projected(const __grid_constant__ DeviceParams P) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  // same layout as rollout_thread_per_sample
+  const int T = P.T;
+  float4* sObs = reinterpret_cast<float4*>(smem_raw);
+  float2* sVel = reinterpret_cast<float2*>(sObs + P.max_obstacles);
+  float2* sU = sVel + P.max_obstacles;
+  double* sRedM = reinterpret_cast<double*>(sU + T);
+  int* sRedI = reinterpret_cast<int*>(sRedM + 4);
+  float* sRedF = reinterpret_cast<float*>(sRedI + 4);
+  float* sA = sRedF + 12;
+
+  const int scene = blockIdx.y;
+  const int tid = threadIdx.x;
+  const int k = blockIdx.x * kThreadBlock + tid;
+  const bool valid = k < P.K;
+  const uint32_t n = *P.counter;
+  const uint32_t key0 = P.key0 + (uint32_t)scene;
+  const uint32_t key1 = P.key1 + (key0 < P.key0 ? 1u : 0u);
+
+  const float4 x0 = reinterpret_cast<const float4*>(P.state)[scene];
+  float4 g = reinterpret_cast<const float4*>(P.goal)[scene];
+  g.x -= x0.x; g.y -= x0.y;                     // vehicle-centred frame
+  const int n_obs = min(P.n_obs[scene], NO);
+  for (int i = tid; i < T; i += kThreadBlock)
+    sU[i] = reinterpret_cast<const float2*>(P.U)[scene * T + i];
+  for (int i = tid; i < n_obs; i += kThreadBlock) {
+    const float* ob = P.obstacles + ((size_t)scene * P.max_obstacles + i) * 5;
+    const float rho = ob[2] + P.disc_radius;
+    sObs[i] = make_float4(ob[0] - x0.x, ob[1] - x0.y, 1.0f / (rho * rho), 0.0f);
+    sVel[i] = make_float2(P.dt * ob[3], P.dt * ob[4]);
+  }
+  __syncthreads();
+
+  double S = CUDART_INF;
+  if (valid) {
+    // M^-1 (diagonal), the soft-bound part of p, bounds: PAPER.md:185-192
+    const float mv = 1.0f / (P.proj_qv + P.proj_rho), mw = 1.0f / (P.proj_qomega + P.proj_rho),
+                ma = 1.0f / (P.proj_qalpha + P.proj_rho);
+    const float pv0 = 0.5f * P.proj_rho * (P.v_max + P.v_min);        // rho/2 (z_hi + z_lo): 0 for omega, u^alpha
+    State X{0.0f, 0.0f, x0.z, x0.w};
+    float alpha[NO];
+    {
+      const float a0 = sample_alpha(P, n, (uint32_t)k, key0, key1);
+#pragma unroll
+      for (int i = 0; i < NO; ++i) alpha[i] = a0;
+    }
+    float h[NO], g0[NO], g1[NO], lf[NO];
+    barrier_rows<PRECISE, NO>(P, X, n_obs, 0.0f, sObs, sVel, h, g0, g1, lf);
+    double cost = 0.0;
+    for (int t = 0; t < T; ++t) {
+      // z_des = [w_des; u~^alpha], w_des = (v~, v~ tan delta~)
+      const float2 u = sample_control<PRECISE>(P, sU[t], (uint32_t)t, n, (uint32_t)k, key0, key1);
+      float ua[NO];
+#pragma unroll
+      for (int q = 0; 4 * q < NO; ++q) {
+        if (4 * q < n_obs) {
+          float z4[4];
+          normals4<PRECISE>((uint32_t)t, n, (uint32_t)k, 2u + (uint32_t)q, key0, key1, z4);
+#pragma unroll
+          for (int e = 0; e < 4; ++e)
+            if (4 * q + e < NO) ua[4 * q + e] = P.sigma_ualpha * z4[e];
+        } else {
+#pragma unroll
+          for (int e = 0; e < 4; ++e)
+            if (4 * q + e < NO) ua[4 * q + e] = 0.0f;
+        }
+      }
+      // y = M^-1 p, p = W z_des + rho/2 (z_hi + z_lo)
+      const float yv = fmaf(P.proj_qv, u.x, pv0) * mv;
+      const float yw = (P.proj_qomega * (u.x * tan_t<PRECISE>(u.y))) * mw;
+      float ya[NO], r[NO];
+#pragma unroll
+      for (int i = 0; i < NO; ++i) {
+        ya[i] = (P.proj_qalpha * ua[i]) * ma;
+        // (9): L_g h w + h u^alpha = b,  b = -alpha h - L_f h;  r = A y - b.  A null row (i >= n_obs) is
+        // u^alpha_i = y_i: r = 0, it changes nothing.
+        const float b = i < n_obs ? -fmaf(alpha[i], h[i], lf[i]) : ya[i];
+        r[i] = fmaf(g0[i], yv, fmaf(g1[i], yw, fmaf(h[i], ya[i], -b)));
+      }
+      // S = A M^-1 A^T (lower triangle), Cholesky in place with 1 / L_kk on the diagonal
+      float Sm[NO][NO];
+#pragma unroll
+      for (int i = 0; i < NO; ++i) {
+        const float a0 = g0[i] * mv, a1 = g1[i] * mw;
+#pragma unroll
+        for (int c = 0; c <= i; ++c) Sm[i][c] = fmaf(a0, g0[c], a1 * g1[c]);
+        Sm[i][i] = fmaf(h[i] * ma, h[i], Sm[i][i]);
+      }
+      bool drop[NO];
+#pragma unroll
+      for (int c = 0; c < NO; ++c) {
+        const float d0 = Sm[c][c];
+        float dkk = d0;
+#pragma unroll
+        for (int m = 0; m < c; ++m) dkk = fmaf(-Sm[c][m], Sm[c][m], dkk);
+        drop[c] = !(dkk > 1e-6f * d0);            // a row that adds nothing new is dropped (multiplier 0)
+        const float inv = drop[c] ? 0.0f : rsqrtf(dkk);
+        Sm[c][c] = inv;
+#pragma unroll
+        for (int i = c + 1; i < NO; ++i) {
+          float v = Sm[i][c];
+#pragma unroll
+          for (int m = 0; m < c; ++m) v = fmaf(-Sm[i][m], Sm[c][m], v);
+          Sm[i][c] = v * inv;
+        }
+        if (drop[c]) {
+#pragma unroll
+          for (int m = 0; m < c; ++m) Sm[c][m] = 0.0f;
+        }
+      }
+#pragma unroll
+      for (int i = 0; i < NO; ++i) {              // L w = r
+        float v = r[i];
+#pragma unroll
+        for (int m = 0; m < i; ++m) v = fmaf(-Sm[i][m], r[m], v);
+        r[i] = v * Sm[i][i];
+      }
+#pragma unroll
+      for (int i = NO - 1; i >= 0; --i) {         // L^T nu = w
+        float v = r[i];
+#pragma unroll
+        for (int m = i + 1; m < NO; ++m) v = fmaf(-Sm[m][i], r[m], v);
+        r[i] = v * Sm[i][i];
+      }
+      // z* = y - M^-1 A^T nu
+      float gv = 0.0f, gw = 0.0f;
+#pragma unroll
+      for (int i = 0; i < NO; ++i) { gv = fmaf(g0[i], r[i], gv); gw = fmaf(g1[i], r[i], gw); }
+      const float vp = fmaf(-mv, gv, yv), wp = fmaf(-mw, gw, yw);
+#pragma unroll
+      for (int i = 0; i < NO; ++i)
+        if (i < n_obs) alpha[i] += fmaf(-ma * h[i], r[i], ya[i]);   // alpha_{tau+1} = alpha_tau + u^alpha_proj
+      // x_{tau+1} = x_tau + dt G(x_tau) w_proj
+      {
+        float s1, c1, s2, c2;
+        sincos_t<PRECISE>(X.psi1, &s1, &c1);
+        sincos_t<PRECISE>(X.psi2, &s2, &c2);
+        const float sb = s1 * c2 - c1 * s2, cb = fmaf(c1, c2, s1 * s2);
+        const float a = P.dt * vp;
+        State N;
+        N.x = fmaf(a, c1, X.x);
+        N.y = fmaf(a, s1, X.y);
+        N.psi1 = fmaf(P.dt * wp, P.inv_L1, X.psi1);
+        N.psi2 = fmaf(P.dt * P.inv_L2, fmaf(vp, sb, -(P.Lh_over_L1 * wp) * cb), X.psi2);
+        X = N;
+      }
+      // rows of (9) at the new state: the alpha cost now, A and b of the next step
+      barrier_rows<PRECISE, NO>(P, X, n_obs, (float)(t + 1), sObs, sVel, h, g0, g1, lf);
+      float ca = 0.0f;
+#pragma unroll
+      for (int i = 0; i < NO; ++i)
+        if (i < n_obs && h[i] < P.h_buffer && alpha[i] > 0.0f) ca = fmaf(alpha[i], alpha[i], ca);
+      const float stage = goal_cost(P, X, g) + fmaf(P.w_v * vp, vp, P.w_delta * wp * wp) + hitch_cost(P, X, vp) +
+                          P.w_alpha * ca;
+      cost += (double)stage;
+    }
+    S = cost + (double)(P.w_term * goal_cost(P, X, g));
+    if (P.flags & BRMPPI_FLAG_WRITE_SAMPLES) {
+      P.S[(size_t)scene * P.K + k] = (float)S;
+      reinterpret_cast<float4*>(P.XT)[(size_t)scene * P.K + k] =
+          make_float4(X.x + x0.x, X.y + x0.y, X.psi1, X.psi2);
+    }
+  }
+  // eq. (5) averages the SAMPLED u~ with the projected rollouts' weights
+  thread_kernel_epilogue<PRECISE>(P, sU, sRedM, sRedI, sRedF, sA, S, valid, k, scene, n, key0, key1);
+}
+
+using ProjectedKernel = void (*)(const DeviceParams);
+
+inline ProjectedKernel projected_kernel_for(bool precise, int max_obstacles) {
+  const int cap = max_obstacles <= 1 ? 1 : max_obstacles <= 2 ? 2 : max_obstacles <= 4 ? 4 : 8;
+  switch (cap * 2 + (precise ? 1 : 0)) {
+    case 2: return rollout_projected<false, 1>;
+    case 3: return rollout_projected<true, 1>;
+    case 4: return rollout_projected<false, 2>;
+    case 5: return rollout_projected<true, 2>;
+    case 8: return rollout_projected<false, 4>;
+    case 9: return rollout_projected<true, 4>;
+    case 16: return rollout_projected<false, 8>;
+    default: return rollout_projected<true, 8>;
+  }
+}
+
+}  // namespace brmppi

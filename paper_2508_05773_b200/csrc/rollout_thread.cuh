@@ -18,6 +18,55 @@ namespace brmppi {
 
 constexpr int kThreadBlock = 128;
 
+// Block partial of the online softmax (a7) for the one-thread-per-sample kernels: block minimum,
+// weights, eta, and the weighted control sums with the sampled controls regenerated from the
+// counter-based generator (nothing per sample is kept in memory).  All kThreadBlock threads call it.
+template <bool PRECISE>
+__device__ __forceinline__ void thread_kernel_epilogue(const DeviceParams& P, const float2* sU, double* sRedM,
+                                                       int* sRedI, float* sRedF, float* sA, double S, bool valid,
+                                                       int k, int scene, uint32_t n, uint32_t key0, uint32_t key1) {
+  const int T = P.T;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const bool finite = valid && (S == S) && (S < CUDART_INF) && (S > -CUDART_INF);
+  double m = finite ? S : CUDART_INF;
+  int idx = finite ? k : 0x7fffffff;
+  warp_argmin(m, idx);
+  if (lane == 0) { sRedM[warp] = m; sRedI[warp] = idx; }
+  __syncthreads();
+  m = sRedM[0]; idx = sRedI[0];
+#pragma unroll
+  for (int w = 1; w < 4; ++w)
+    if (sRedM[w] < m || (sRedM[w] == m && sRedI[w] < idx)) { m = sRedM[w]; idx = sRedI[w]; }
+  // S - m in fp64, then fp32 exp (SURVEY §7 hard part 2)
+  const float wk = finite ? expf((float)(-(S - m) * (double)P.inv_lambda)) : 0.0f;
+  float eta = warp_sum(wk), w2 = warp_sum(wk * wk);
+  float nf = warp_sum((valid && !finite) ? 1.0f : 0.0f);
+  if (lane == 0) { sRedF[warp] = eta; sRedF[4 + warp] = w2; sRedF[8 + warp] = nf; }
+
+  // weighted control sums: regenerate u_k[t] from the counter-based generator
+  for (int t = 0; t < T; ++t) {
+    float2 u = make_float2(0.0f, 0.0f);
+    if (finite) u = sample_control<PRECISE>(P, sU[t], (uint32_t)t, n, (uint32_t)k, key0, key1);
+    const float av = warp_sum(wk * u.x), ad = warp_sum(wk * u.y);
+    if (lane == 0) { sA[warp * 2 * T + 2 * t] = av; sA[warp * 2 * T + 2 * t + 1] = ad; }
+  }
+  __syncthreads();
+
+  const int P_n = P.n_partials;
+  const size_t pbase = (size_t)scene * P_n + blockIdx.x;
+  if (tid == 0) {
+    P.part_m[pbase] = m;
+    P.part_argmin[pbase] = idx;
+    P.part_eta[pbase] = (sRedF[0] + sRedF[1]) + (sRedF[2] + sRedF[3]);
+    P.part_w2[pbase] = (sRedF[4] + sRedF[5]) + (sRedF[6] + sRedF[7]);
+    P.part_nonfinite[pbase] = (int)((sRedF[8] + sRedF[9]) + (sRedF[10] + sRedF[11]));
+  }
+  for (int o = tid; o < 2 * T; o += kThreadBlock) {
+    const float a = (sA[o] + sA[2 * T + o]) + (sA[4 * T + o] + sA[6 * T + o]);   // fixed order
+    P.part_A[((size_t)scene * 2 * T + o) * P_n + blockIdx.x] = a;
+  }
+}
+
 template <bool PRECISE>
 __global__ void __launch_bounds__(kThreadBlock)
 rollout_thread_per_sample(const __grid_constant__ DeviceParams P) {
@@ -111,45 +160,7 @@ rollout_thread_per_sample(const __grid_constant__ DeviceParams P) {
     }
   }
 
-  // ---- block partial of the online softmax (a7) -----------------------------------------
-  const bool finite = valid && (S == S) && (S < CUDART_INF) && (S > -CUDART_INF);
-  double m = finite ? S : CUDART_INF;
-  int idx = finite ? k : 0x7fffffff;
-  warp_argmin(m, idx);
-  if (lane == 0) { sRedM[warp] = m; sRedI[warp] = idx; }
-  __syncthreads();
-  m = sRedM[0]; idx = sRedI[0];
-#pragma unroll
-  for (int w = 1; w < 4; ++w)
-    if (sRedM[w] < m || (sRedM[w] == m && sRedI[w] < idx)) { m = sRedM[w]; idx = sRedI[w]; }
-  // S - m in fp64, then fp32 exp (SURVEY §7 hard part 2)
-  const float wk = finite ? expf((float)(-(S - m) * (double)P.inv_lambda)) : 0.0f;
-  float eta = warp_sum(wk), w2 = warp_sum(wk * wk);
-  float nf = warp_sum((valid && !finite) ? 1.0f : 0.0f);
-  if (lane == 0) { sRedF[warp] = eta; sRedF[4 + warp] = w2; sRedF[8 + warp] = nf; }
-
-  // weighted control sums: regenerate u_k[t] from the counter-based generator
-  for (int t = 0; t < T; ++t) {
-    float2 u = make_float2(0.0f, 0.0f);
-    if (finite) u = sample_control<PRECISE>(P, sU[t], (uint32_t)t, n, (uint32_t)k, key0, key1);
-    const float av = warp_sum(wk * u.x), ad = warp_sum(wk * u.y);
-    if (lane == 0) { sA[warp * 2 * T + 2 * t] = av; sA[warp * 2 * T + 2 * t + 1] = ad; }
-  }
-  __syncthreads();
-
-  const int P_n = P.n_partials;
-  const size_t pbase = (size_t)scene * P_n + blockIdx.x;
-  if (tid == 0) {
-    P.part_m[pbase] = m;
-    P.part_argmin[pbase] = idx;
-    P.part_eta[pbase] = (sRedF[0] + sRedF[1]) + (sRedF[2] + sRedF[3]);
-    P.part_w2[pbase] = (sRedF[4] + sRedF[5]) + (sRedF[6] + sRedF[7]);
-    P.part_nonfinite[pbase] = (int)((sRedF[8] + sRedF[9]) + (sRedF[10] + sRedF[11]));
-  }
-  for (int o = tid; o < 2 * T; o += kThreadBlock) {
-    const float a = (sA[o] + sA[2 * T + o]) + (sA[4 * T + o] + sA[6 * T + o]);   // fixed order
-    P.part_A[((size_t)scene * 2 * T + o) * P_n + blockIdx.x] = a;
-  }
+  thread_kernel_epilogue<PRECISE>(P, sU, sRedM, sRedI, sRedF, sA, S, valid, k, scene, n, key0, key1);
 }
 
 inline size_t rollout_thread_smem_bytes(const DeviceParams& P) {
