@@ -350,7 +350,7 @@ int brmppi_create(const brmppi_params* p, void* dev_workspace, size_t workspace_
     c->smem_rollout = c->plan.cta.smem;
     e = configure_rollout_cta((p->flags & BRMPPI_FLAG_PRECISE_MATH) != 0, p->n_discs, c->smem_rollout);
   } else {
-    c->smem_rollout = rollout_thread_smem_bytes(d);
+    c->smem_rollout = (p->flags & BRMPPI_FLAG_PROJECTED) ? rollout_projected_smem_bytes(d) : rollout_thread_smem_bytes(d);
     // per function and device, not per context: always the opt-in maximum, never lowered
     if (p->flags & BRMPPI_FLAG_PROJECTED)
       e = cudaFuncSetAttribute(projected_kernel_for((p->flags & BRMPPI_FLAG_PRECISE_MATH) != 0, p->max_obstacles),

@@ -31,7 +31,9 @@ __device__ __forceinline__ void normals4(uint32_t t, uint32_t n, uint32_t k, uin
 }
 
 // Rows of (9) for all obstacles at state X, step t: h_i on the closest disc (lowest index on ties),
-// L_g h_i (2), L_f h_i.  Obstacle i: sObs = (ox, oy, 1/rho^2, -) in the vehicle frame, sVel = dt vel.
+// L_g h_i (2), L_f h_i.  Obstacle i: sObs = (ox, oy, 1/rho^2, -) in the vehicle frame, sVel = dt vel; the
+// table is padded to NO entries with null obstacles (1/rho^2 = 0), so the loop has no branch: a null row
+// comes out as h = 1, L_g h = 0, L_f h = 0.
 template <bool PRECISE, int NO>
 __device__ __forceinline__ void barrier_rows(const DeviceParams& P, const State& X, int n_obs, float tf,
                                              const float4* __restrict__ sObs, const float2* __restrict__ sVel,
@@ -42,38 +44,28 @@ __device__ __forceinline__ void barrier_rows(const DeviceParams& P, const State&
   float cx[kMaxDiscs], cy[kMaxDiscs];
   disc_centres(P, X, s1, c1, s2, c2, cx, cy);
   const float sb = s1 * c2 - c1 * s2, cb = fmaf(c1, c2, s1 * s2);   // sin / cos (psi1 - psi2)
-  // d c_j / d psi1 and d c_j / d psi2 (c = p_h + a e(psi_body), p_h = (x - Lh cos psi1, y - Lh sin psi1))
-  float d1x[kMaxDiscs], d1y[kMaxDiscs], d2x[kMaxDiscs], d2y[kMaxDiscs];
-#pragma unroll
-  for (int j = 0; j < kMaxDiscs; ++j) {
-    const float a1 = P.disc_a1[j] - P.Lh, a2 = P.disc_a2[j];
-    d1x[j] = -a1 * s1; d1y[j] = a1 * c1;
-    d2x[j] = -a2 * s2; d2y[j] = a2 * c2;
-  }
 #pragma unroll
   for (int i = 0; i < NO; ++i) {
-    if (i < n_obs) {
-      const float4 o = sObs[i];
-      const float2 w = sVel[i];
-      const float ox = fmaf(tf, w.x, o.x), oy = fmaf(tf, w.y, o.y);                 // o(t)
-      float hb = 0.0f, ex = 0.0f, ey = 0.0f, b1x = 0.0f, b1y = 0.0f, b2x = 0.0f, b2y = 0.0f;
+    const float4 o = sObs[i];
+    const float2 w = sVel[i];
+    const float ox = fmaf(tf, w.x, o.x), oy = fmaf(tf, w.y, o.y);                 // o(t)
+    // closest disc: h_j, the offset c_j - o, and the disc's lever arms on the two headings
+    // (d c_j / d psi1 = (a1_j - Lh)(-sin psi1, cos psi1), d c_j / d psi2 = a2_j (-sin psi2, cos psi2))
+    float hb = CUDART_INF_F, ex = 0.0f, ey = 0.0f, l1 = 0.0f, l2 = 0.0f;
 #pragma unroll
-      for (int j = 0; j < kMaxDiscs; ++j) {
-        if (j < P.n_discs) {
-          const float dx = cx[j] - ox, dy = cy[j] - oy;
-          const float hj = fmaf(fmaf(dx, dx, dy * dy), o.z, -1.0f);
-          if (j == 0 || hj < hb) { hb = hj; ex = dx; ey = dy; b1x = d1x[j]; b1y = d1y[j]; b2x = d2x[j]; b2y = d2y[j]; }
-        }
-      }
-      const float gx = 2.0f * ex * o.z, gy = 2.0f * ey * o.z;                       // grad_c h
-      const float dpsi1 = fmaf(gx, b1x, gy * b1y), dpsi2 = fmaf(gx, b2x, gy * b2y);
-      h[i] = hb;
-      g0[i] = P.dt * fmaf(gx, c1, fmaf(gy, s1, dpsi2 * sb * P.inv_L2));
-      g1[i] = P.dt * fmaf(dpsi1, P.inv_L1, -(dpsi2 * P.Lh_over_L1 * P.inv_L2) * cb);
-      lf[i] = -fmaf(gx, w.x, gy * w.y);                                             // w = dt vel
-    } else {
-      h[i] = 1.0f; g0[i] = 0.0f; g1[i] = 0.0f; lf[i] = 0.0f;
+    for (int j = 0; j < kMaxDiscs; ++j) {
+      const float dx = cx[j] - ox, dy = cy[j] - oy;
+      const float hj = j < P.n_discs ? fmaf(fmaf(dx, dx, dy * dy), o.z, -1.0f) : CUDART_INF_F;
+      const bool take = hj < hb;
+      hb = take ? hj : hb; ex = take ? dx : ex; ey = take ? dy : ey;
+      l1 = take ? P.disc_a1[j] - P.Lh : l1; l2 = take ? P.disc_a2[j] : l2;
     }
+    const float gx = 2.0f * ex * o.z, gy = 2.0f * ey * o.z;                       // grad_c h
+    const float dpsi1 = l1 * fmaf(gy, c1, -gx * s1), dpsi2 = l2 * fmaf(gy, c2, -gx * s2);
+    h[i] = i < n_obs ? hb : 1.0f;
+    g0[i] = P.dt * fmaf(gx, c1, fmaf(gy, s1, dpsi2 * sb * P.inv_L2));
+    g1[i] = P.dt * fmaf(dpsi1, P.inv_L1, -(dpsi2 * P.Lh_over_L1 * P.inv_L2) * cb);
+    lf[i] = -fmaf(gx, w.x, gy * w.y);                                             // w = dt vel
   }
 }
 
@@ -81,11 +73,11 @@ template <bool PRECISE, int NO>
 __global__ void __launch_bounds__(kThreadBlock)
 rollout_projected(const __grid_constant__ DeviceParams P) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  // same layout as rollout_thread_per_sample
+  // layout of rollout_thread_per_sample with NO obstacle slots
   const int T = P.T;
   float4* sObs = reinterpret_cast<float4*>(smem_raw);
-  float2* sVel = reinterpret_cast<float2*>(sObs + P.max_obstacles);
-  float2* sU = sVel + P.max_obstacles;
+  float2* sVel = reinterpret_cast<float2*>(sObs + NO);
+  float2* sU = sVel + NO;
   double* sRedM = reinterpret_cast<double*>(sU + T);
   int* sRedI = reinterpret_cast<int*>(sRedM + 4);
   float* sRedF = reinterpret_cast<float*>(sRedI + 4);
@@ -105,11 +97,16 @@ rollout_projected(const __grid_constant__ DeviceParams P) {
   const int n_obs = min(P.n_obs[scene], NO);
   for (int i = tid; i < T; i += kThreadBlock)
     sU[i] = reinterpret_cast<const float2*>(P.U)[scene * T + i];
-  for (int i = tid; i < n_obs; i += kThreadBlock) {
-    const float* ob = P.obstacles + ((size_t)scene * P.max_obstacles + i) * 5;
-    const float rho = ob[2] + P.disc_radius;
-    sObs[i] = make_float4(ob[0] - x0.x, ob[1] - x0.y, 1.0f / (rho * rho), 0.0f);
-    sVel[i] = make_float2(P.dt * ob[3], P.dt * ob[4]);
+  for (int i = tid; i < NO; i += kThreadBlock) {
+    if (i < n_obs) {
+      const float* ob = P.obstacles + ((size_t)scene * P.max_obstacles + i) * 5;
+      const float rho = ob[2] + P.disc_radius;
+      sObs[i] = make_float4(ob[0] - x0.x, ob[1] - x0.y, 1.0f / (rho * rho), 0.0f);
+      sVel[i] = make_float2(P.dt * ob[3], P.dt * ob[4]);
+    } else {                                                 // null obstacle: no gradient, no motion
+      sObs[i] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+      sVel[i] = make_float2(0.0f, 0.0f);
+    }
   }
   __syncthreads();
 
@@ -129,22 +126,35 @@ rollout_projected(const __grid_constant__ DeviceParams P) {
     float h[NO], g0[NO], g1[NO], lf[NO];
     barrier_rows<PRECISE, NO>(P, X, n_obs, 0.0f, sObs, sVel, h, g0, g1, lf);
     double cost = 0.0;
+    // The draws of step t + 1 do not depend on the state: they are generated during step t, so that the long
+    // Philox / Box-Muller chains fill the issue slots the Cholesky chain leaves empty.
+    float2 u_next = sample_control<PRECISE>(P, sU[0], 0u, n, (uint32_t)k, key0, key1);
+    float ua_next[NO];
+#pragma unroll
+    for (int q = 0; 4 * q < NO; ++q) {
+      float z4[4];
+      normals4<PRECISE>(0u, n, (uint32_t)k, 2u + (uint32_t)q, key0, key1, z4);
+#pragma unroll
+      for (int e = 0; e < 4; ++e)
+        if (4 * q + e < NO) ua_next[4 * q + e] = P.sigma_ualpha * z4[e];
+    }
+#pragma unroll 1
     for (int t = 0; t < T; ++t) {
       // z_des = [w_des; u~^alpha], w_des = (v~, v~ tan delta~)
-      const float2 u = sample_control<PRECISE>(P, sU[t], (uint32_t)t, n, (uint32_t)k, key0, key1);
+      const float2 u = u_next;
       float ua[NO];
 #pragma unroll
-      for (int q = 0; 4 * q < NO; ++q) {
-        if (4 * q < n_obs) {
+      for (int i = 0; i < NO; ++i) ua[i] = ua_next[i];
+      {
+        const uint32_t tn = (uint32_t)min(t + 1, T - 1);
+        u_next = sample_control<PRECISE>(P, sU[tn], tn, n, (uint32_t)k, key0, key1);
+#pragma unroll
+        for (int q = 0; 4 * q < NO; ++q) {
           float z4[4];
-          normals4<PRECISE>((uint32_t)t, n, (uint32_t)k, 2u + (uint32_t)q, key0, key1, z4);
+          normals4<PRECISE>(tn, n, (uint32_t)k, 2u + (uint32_t)q, key0, key1, z4);
 #pragma unroll
           for (int e = 0; e < 4; ++e)
-            if (4 * q + e < NO) ua[4 * q + e] = P.sigma_ualpha * z4[e];
-        } else {
-#pragma unroll
-          for (int e = 0; e < 4; ++e)
-            if (4 * q + e < NO) ua[4 * q + e] = 0.0f;
+            if (4 * q + e < NO) ua_next[4 * q + e] = P.sigma_ualpha * z4[e];
         }
       }
       // y = M^-1 p, p = W z_des + rho/2 (z_hi + z_lo)
@@ -185,10 +195,9 @@ rollout_projected(const __grid_constant__ DeviceParams P) {
           for (int m = 0; m < c; ++m) v = fmaf(-Sm[i][m], Sm[c][m], v);
           Sm[i][c] = v * inv;
         }
-        if (drop[c]) {
+        const float keep = drop[c] ? 0.0f : 1.0f;
 #pragma unroll
-          for (int m = 0; m < c; ++m) Sm[c][m] = 0.0f;
-        }
+        for (int m = 0; m < c; ++m) Sm[c][m] *= keep;
       }
 #pragma unroll
       for (int i = 0; i < NO; ++i) {              // L w = r
@@ -245,6 +254,11 @@ rollout_projected(const __grid_constant__ DeviceParams P) {
   }
   // eq. (5) averages the SAMPLED u~ with the projected rollouts' weights
   thread_kernel_epilogue<PRECISE>(P, sU, sRedM, sRedI, sRedF, sA, S, valid, k, scene, n, key0, key1);
+}
+
+inline size_t rollout_projected_smem_bytes(const DeviceParams& P) {
+  return sizeof(float4) * BRMPPI_PROJECT_MAX_NO + sizeof(float2) * BRMPPI_PROJECT_MAX_NO + sizeof(float2) * P.T +
+         sizeof(double) * 4 + sizeof(int) * 4 + sizeof(float) * 12 + sizeof(float) * 4 * 2 * P.T;
 }
 
 using ProjectedKernel = void (*)(const DeviceParams);
