@@ -367,7 +367,8 @@ int brmppi_create(const brmppi_params* p, void* dev_workspace, size_t workspace_
   // zero: n_obs, U, counter, diag, u0 (state/goal stay unset until the caller provides them)
   if (e == cudaSuccess) e = cudaMemsetAsync(base, 0, L.part_m, c->stream);
   if (e == cudaSuccess) e = cudaMemsetAsync(base + L.diag, 0, (size_t)p->n_scenes * sizeof(brmppi_diag), c->stream);
-  if (e == cudaSuccess) e = cudaMallocHost((void**)&c->pinned_u0, sizeof(float) * 2 * (size_t)p->n_scenes);
+  if (e == cudaSuccess) e = cudaHostAlloc((void**)&c->pinned_u0, sizeof(float) * 2 * (size_t)p->n_scenes, cudaHostAllocMapped);
+  if (e == cudaSuccess) e = cudaHostGetDevicePointer((void**)&d.u0_host, c->pinned_u0, 0);
   if (e != cudaSuccess) {
     free(c->state_set); free(c->goal_set);
     delete c;
@@ -523,10 +524,10 @@ int brmppi_step(brmppi_ctx* c, float* u0_out) {
     r = capture(c, &c->step_graph, [&] {
       int rr = enqueue_solve(c);
       if (rr) return rr;
+      // the plant step writes the applied control straight into the page-locked host buffer (mapped
+      // under unified addressing): the graph needs no copy node, the sync below makes it visible
       shift_plant<true><<<(unsigned)c->p.n_scenes, kShiftBlock, 0, c->stream>>>(c->d);
       CU(cudaGetLastError());
-      CU(cudaMemcpyAsync(c->pinned_u0, c->d.u0_applied, sizeof(float) * 2 * (size_t)c->p.n_scenes,
-                         cudaMemcpyDeviceToHost, c->stream));
       return (int)BRMPPI_OK;
     });
     if (r) return r;

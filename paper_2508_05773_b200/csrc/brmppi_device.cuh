@@ -61,6 +61,7 @@ struct DeviceParams {
   float* U;                   // [n_scenes][T][2]
   uint32_t* counter;          // global iteration counter n
   float* u0_applied;          // [n_scenes][2]  control applied by the last plant step
+  float* u0_host;             // the same, in page-locked HOST memory the device writes directly (brmppi_step's result)
   float* hitch_ref;           // [n_scenes][4]  (v_ref, delta_ref, status as int bits, 0) of the last plant step
   double* part_m;             // [n_scenes][P]  block minimum of S (fp64)
   int* part_argmin;           // [n_scenes][P]

@@ -118,6 +118,7 @@ __global__ void __launch_bounds__(kShiftBlock) shift_plant(const __grid_constant
       const State N = kinematic_step(P, State{x.x, x.y, x.z, x.w}, s1, c1, s2, c2, u0.x, tanf(u0.y));
       reinterpret_cast<float4*>(P.state)[scene] = make_float4(N.x, N.y, wrap_angle(N.psi1), wrap_angle(N.psi2));
       reinterpret_cast<float2*>(P.u0_applied)[scene] = u0;
+      if (P.u0_host != nullptr) reinterpret_cast<float2*>(P.u0_host)[scene] = u0;   // zero-copy: no D2H node in the step graph
     }
     const int n_obs = P.n_obs[scene];
     for (int i = tid; i < n_obs; i += kShiftBlock) {
