@@ -493,20 +493,25 @@ def run_sweep(args):
 
     def point(name, scs, p, n_scenes):
         n_obs = len(scs[0].obstacles)
-        s = B.Solver(p, n_scenes, max(n_obs, 1), 0)
-        for i, sc in enumerate(scs):
-            s.set_scene(sc, i)
-        for _ in range(3):
-            s.solve()
-        s.synchronize()
-        ms_roll, ms_upd = s.time_kernels(20)
-        s.close()
+        times = {}
+        for label, flags in (("cull", 0), ("no_cull", B.FLAG_NO_CULL)):
+            s = B.Solver(p, n_scenes, max(n_obs, 1), flags)
+            for i, sc in enumerate(scs):
+                s.set_scene(sc, i)
+            for _ in range(3):
+                s.solve()
+            s.synchronize()
+            times[label] = s.time_kernels(20)
+            s.close()
+        ms_roll, ms_upd = times["cull"]
         work = n_scenes * p.K * p.T
         instr = algorithmic_instr_per_sample_step(n_obs, len(p.discs))
         print(json.dumps({"point": name, "K": p.K, "T": p.T, "n_obstacles": n_obs, "n_scenes": n_scenes,
                           "rollout_us": ms_roll * 1e3, "update_us": ms_upd * 1e3,
                           "sample_steps_per_s": work / (ms_roll * 1e-3),
-                          "frac": work * instr / (ms_roll * 1e-3) / peak}), flush=True)
+                          "frac": work * instr / (ms_roll * 1e-3) / peak,
+                          "rollout_us_no_cull": times["no_cull"][0] * 1e3,
+                          "frac_no_cull": work * instr / (times["no_cull"][0] * 1e-3) / peak}), flush=True)
 
     for K in (1024, 16384, 131072, 1048576):
         for T in (50, 100):
@@ -596,11 +601,19 @@ def main():
     ap.add_argument("--phases", action="store_true", help="print the rollout kernel's in-kernel phase times")
     ap.add_argument("--sweep", action="store_true", help="run BASELINE.json configs[4] (sweep + 64-scene batch)")
     ap.add_argument("--project", action="store_true", help="time the closed-form projection (12) on its own")
+    ap.add_argument("--peaks", action="store_true", help="issue-rate micro-benchmarks (brmppi_measure_peaks): the dispatch-cost table")
     ap.add_argument("--no-cull", action="store_true", help="evaluate every (obstacle, disc, step): BRMPPI_FLAG_NO_CULL")
     args = ap.parse_args()
     if args.gpus > 1 and int(os.environ.get("WORLD_SIZE", "1")) <= 1 and not (args.project or args.phases or args.sweep):
         spawn_ranks(args)          # reference arm included: rank 0 runs it, the others exit 0
-    if args.project:
+    if args.peaks:
+        from paper_2508_05773_b200 import brmppi as B
+        pk = B.measure_peaks()
+        pk["unit"] = "thread-instructions per clock per SM (128 = one warp instruction per clock per scheduler)"
+        pk["cycles_per_warp_instruction_per_scheduler"] = {k: round(128.0 / v, 3) for k, v in pk.items()
+                                                           if isinstance(v, float) and k not in ("sm_mhz", "sm_mhz_under_ffma") and v > 0}
+        print(json.dumps(pk))
+    elif args.project:
         run_project(args)
     elif args.phases:
         run_phases(args)

@@ -280,13 +280,15 @@ int brmppi_project(void* cuda_stream, int n, int n_o, const float* A, const floa
 /* Issue-rate micro-benchmarks for the roofline denominator: thread-instructions
  * per clock per SM achieved by dependent-chain-free streams of FFMA, LOP3/IADD3 (ALU pipe),
  * MUFU (XU pipe) and the FFMA+ALU mix, plus the SM count and the clock measured in-kernel.
- * out[0..7] = {ffma, alu, mufu, mix (ffma+lop3 interleaved), imad_wide, n_sms, sm_mhz of an idle SM,
- * sm_mhz seen while the FFMA kernel ran}.  Rates are whole-kernel: instructions per SM / (first
- * block start .. last block end on the globaltimer, converted with the in-kernel clock).
+ * out[0..7] = {ffma, alu (lop3), mufu, mix (ffma+lop3 interleaved), imad_wide, n_sms, sm_mhz of an idle SM,
+ * sm_mhz seen while the FFMA kernel ran}; out[8..15] = {fmnmx, ffma2 (packed f32x2, two operands shared),
+ * ffma2 with three distinct 64-bit register operands, fadd2, ffma+fmnmx interleaved, ffma2+fmnmx interleaved,
+ * imad.lo, imad.hi} -- the dispatch-cost table of DESIGN.md 6.1.  Rates are whole-kernel: instructions per
+ * SM / (first block start .. last block end on the globaltimer, converted with the in-kernel clock).
  * dev_scratch: DEVICE pointer to >= brmppi_measure_peaks_scratch_bytes() bytes owned by the caller
  * (the library allocates no device memory).  Synchronises. */
 size_t brmppi_measure_peaks_scratch_bytes(void);
-int brmppi_measure_peaks(void* cuda_stream, void* dev_scratch, size_t scratch_bytes, float out[8]);
+int brmppi_measure_peaks(void* cuda_stream, void* dev_scratch, size_t scratch_bytes, float out[16]);
 
 #ifdef __cplusplus
 }

@@ -437,7 +437,7 @@ def project(A, b, z_des, w, rho, z_lo, z_hi, out=None, scratch=None):
 
 def measure_peaks():
     import torch
-    out = np.zeros(8, dtype=np.float32)
+    out = np.zeros(16, dtype=np.float32)
     nb = lib().brmppi_measure_peaks_scratch_bytes()
     scratch = _scratch(nb)
     st = torch.cuda.current_stream()
@@ -445,4 +445,6 @@ def measure_peaks():
     _check(lib().brmppi_measure_peaks(C.c_void_p(st.cuda_stream), C.c_void_p(scratch.data_ptr()), C.c_size_t(nb), _p(out)))
     return dict(ffma=float(out[0]), alu=float(out[1]), mufu=float(out[2]), mix=float(out[3]),
                 imad_wide=float(out[4]), n_sms=int(out[5]), sm_mhz=float(out[6]),
-                sm_mhz_under_ffma=float(out[7]))
+                sm_mhz_under_ffma=float(out[7]), fmnmx=float(out[8]), ffma2=float(out[9]),
+                ffma2_distinct_operands=float(out[10]), fadd2=float(out[11]), ffma_fmnmx_mix=float(out[12]),
+                ffma2_fmnmx_mix=float(out[13]), imad_lo=float(out[14]), imad_hi=float(out[15]))

@@ -245,6 +245,12 @@ int capture(brmppi_ctx* c, cudaGraphExec_t* exec, F&& body) {
 
 }  // namespace
 
+template <int KIND>
+static cudaError_t launch_peak(int blocks, cudaStream_t s, long long* spans, float* sink) {
+  peak_kernel<KIND><<<blocks, 256, 0, s>>>(1.0f, spans, sink);
+  return cudaGetLastError();
+}
+
 extern "C" {
 
 size_t brmppi_workspace_bytes(const brmppi_params* p) {
@@ -854,7 +860,7 @@ int brmppi_project(void* cuda_stream, int n, int n_o, const float* A, const floa
 
 size_t brmppi_measure_peaks_scratch_bytes(void) { return sizeof(long long) * 3 * 4 * 1024 + 256; }
 
-int brmppi_measure_peaks(void* cuda_stream, void* dev_scratch, size_t scratch_bytes, float out[8]) {
+int brmppi_measure_peaks(void* cuda_stream, void* dev_scratch, size_t scratch_bytes, float out[16]) {
   if (!out || !dev_scratch) return BRMPPI_ERR_NULL;
   if (scratch_bytes < brmppi_measure_peaks_scratch_bytes()) return BRMPPI_ERR_WORKSPACE_TOO_SMALL;
   cudaStream_t s = (cudaStream_t)cuda_stream;
@@ -867,18 +873,27 @@ int brmppi_measure_peaks(void* cuda_stream, void* dev_scratch, size_t scratch_by
   float* sink = (float*)align_up((size_t)(uintptr_t)dev_scratch, 256);   // 4 floats, then the spans
   long long* spans = (long long*)(sink + 8);
   long long* h = (long long*)malloc(sizeof(long long) * 3 * (size_t)blocks);
-  double wall_ns[5] = {0, 0, 0, 0, 0};
+  if (!h) return BRMPPI_ERR_NULL;
+  // where each kind's rate goes in out[]: 0..4 as before, 5..7 = SM count and clocks, 8..15 = the rest
+  const int slot[PEAK_KINDS] = {0, 1, 2, 3, 4, 8, 9, 10, 11, 12, 13, 14, 15};
   cudaError_t e = cudaSuccess;
-  for (int kind = 0; kind < 5 && e == cudaSuccess; ++kind) {
+  for (int kind = 0; kind < PEAK_KINDS && e == cudaSuccess; ++kind) {
     for (int rep = 0; rep < 3 && e == cudaSuccess; ++rep) {   // last repetition is the one kept
       switch (kind) {
-        case PEAK_FFMA: peak_kernel<PEAK_FFMA><<<blocks, 256, 0, s>>>(1.0f, spans, sink); break;
-        case PEAK_ALU: peak_kernel<PEAK_ALU><<<blocks, 256, 0, s>>>(1.0f, spans, sink); break;
-        case PEAK_MUFU: peak_kernel<PEAK_MUFU><<<blocks, 256, 0, s>>>(1.0f, spans, sink); break;
-        case PEAK_MIX: peak_kernel<PEAK_MIX><<<blocks, 256, 0, s>>>(1.0f, spans, sink); break;
-        default: peak_kernel<PEAK_IMAD_WIDE><<<blocks, 256, 0, s>>>(1.0f, spans, sink); break;
+        case PEAK_FFMA: e = launch_peak<PEAK_FFMA>(blocks, s, spans, sink); break;
+        case PEAK_ALU: e = launch_peak<PEAK_ALU>(blocks, s, spans, sink); break;
+        case PEAK_MUFU: e = launch_peak<PEAK_MUFU>(blocks, s, spans, sink); break;
+        case PEAK_MIX: e = launch_peak<PEAK_MIX>(blocks, s, spans, sink); break;
+        case PEAK_IMAD_WIDE: e = launch_peak<PEAK_IMAD_WIDE>(blocks, s, spans, sink); break;
+        case PEAK_FMNMX: e = launch_peak<PEAK_FMNMX>(blocks, s, spans, sink); break;
+        case PEAK_FFMA2: e = launch_peak<PEAK_FFMA2>(blocks, s, spans, sink); break;
+        case PEAK_FFMA2_DISTINCT: e = launch_peak<PEAK_FFMA2_DISTINCT>(blocks, s, spans, sink); break;
+        case PEAK_FADD2: e = launch_peak<PEAK_FADD2>(blocks, s, spans, sink); break;
+        case PEAK_FFMA_FMNMX: e = launch_peak<PEAK_FFMA_FMNMX>(blocks, s, spans, sink); break;
+        case PEAK_FFMA2_FMNMX: e = launch_peak<PEAK_FFMA2_FMNMX>(blocks, s, spans, sink); break;
+        case PEAK_IMAD_LO: e = launch_peak<PEAK_IMAD_LO>(blocks, s, spans, sink); break;
+        default: e = launch_peak<PEAK_IMAD_HI>(blocks, s, spans, sink); break;
       }
-      e = cudaGetLastError();
     }
     if (e == cudaSuccess) e = cudaMemcpyAsync(h, spans, sizeof(long long) * 3 * (size_t)blocks, cudaMemcpyDeviceToHost, s);
     if (e == cudaSuccess) e = cudaStreamSynchronize(s);
@@ -895,9 +910,9 @@ int brmppi_measure_peaks(void* cuda_stream, void* dev_scratch, size_t scratch_by
       mhz_sum += (double)h[3 * b] * 1e3 / (double)(h[3 * b + 2] - h[3 * b + 1]);
     }
     const double mhz_kernel = mhz_sum / blocks;
-    wall_ns[kind] = (double)(gmax - gmin);
-    const double per_thread = (double)kPeakIters * kPeakReps * kPeakChains * (kind == PEAK_MIX ? 2.0 : 1.0);
-    out[kind] = (float)(per_thread * 1024.0 / (wall_ns[kind] * 1e-3 * mhz_kernel));   // thread-instr / clk / SM
+    const double wall_ns = (double)(gmax - gmin);
+    const double per_thread = (double)kPeakIters * kPeakReps * kPeakChains * peak_instr_per_slot(kind);
+    out[slot[kind]] = (float)(per_thread * 1024.0 / (wall_ns * 1e-3 * mhz_kernel));   // thread-instr / clk / SM
     if (kind == PEAK_FFMA) out[7] = (float)mhz_kernel;
   }
   if (e == cudaSuccess) {
