@@ -447,6 +447,48 @@ def run_ours(args):
     print(json.dumps(line))
 
 
+def run_sharded(args):
+    """K-sharded solve: the K samples of ONE solve split over the ranks, one 8 + 2T-float record
+    per rank and iteration all-gathered over NCCL.  Strong scaling: total work is fixed as N grows."""
+    import torch
+    from paper_2508_05773_b200 import brmppi as B
+    from paper_2508_05773_b200 import sharded
+    import torch.distributed as dist
+    if not dist.is_initialized():
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1"); os.environ.setdefault("MASTER_PORT", "29655")
+        os.environ.setdefault("RANK", "0"); os.environ.setdefault("WORLD_SIZE", "1")
+        dist.init_process_group(backend=os.environ.get("BRMPPI_DIST_BACKEND", "nccl"))
+    rank, world = dist.get_rank(), dist.get_world_size()
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    dev = f"cuda:{local_rank}"
+    torch.cuda.set_device(dev)
+    sc, p = workload(args.workload, 0)                       # every rank solves the SAME scene
+    s = sharded.ShardedSolver(B, p, dist, 1, max(len(sc.obstacles), 1), solver_flags(B, args.workload), device=dev)
+    s.set_scene(sc)
+    for _ in range(max(args.warmup, 3)):
+        s.solve()
+    torch.cuda.synchronize(); dist.barrier(); torch.cuda.synchronize()
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    a.record(s.solver.stream)
+    for _ in range(args.steps):
+        s.solve()
+    b.record(s.solver.stream)
+    torch.cuda.synchronize(); dist.barrier(); torch.cuda.synchronize()
+    dev_s = max_over_ranks(a.elapsed_time(b) * 1e-3, dist, dev)
+    U = s.get_controls()
+    s.close()
+    if rank == 0:
+        work = args.steps * p.K * p.T * p.n_iter
+        print(json.dumps({"metric": METRIC, "value": work / dev_s, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+                          "warmup": max(args.warmup, 3), "ms_per_step": dev_s / args.steps * 1e3, "higher_is_better": True,
+                          "scaling": "strong", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+                          "config": dict(workload_config(args.workload, sc, p, 1),
+                                         parallelism=f"K sharded over {world} rank(s): {p.K // world} samples per rank, one "
+                                                     f"{4 * (8 + 2 * p.T)}-byte record per rank and iteration all-gathered (NCCL)"),
+                          "gpu_launches": int(args.steps * p.n_iter * 3), "U0": [float(x) for x in U[0]]}))
+    dist.destroy_process_group()
+
+
 def spawn_ranks(args):
     """`python bench.py --gpus N` without a torchrun environment: start the N ranks here (one process per GPU)."""
     import socket
@@ -601,6 +643,7 @@ def main():
     ap.add_argument("--phases", action="store_true", help="print the rollout kernel's in-kernel phase times")
     ap.add_argument("--sweep", action="store_true", help="run BASELINE.json configs[4] (sweep + 64-scene batch)")
     ap.add_argument("--project", action="store_true", help="time the closed-form projection (12) on its own")
+    ap.add_argument("--sharded", action="store_true", help="K-sharded solve over the ranks (strong scaling) instead of replicas")
     ap.add_argument("--peaks", action="store_true", help="issue-rate micro-benchmarks (brmppi_measure_peaks): the dispatch-cost table")
     ap.add_argument("--no-cull", action="store_true", help="evaluate every (obstacle, disc, step): BRMPPI_FLAG_NO_CULL")
     args = ap.parse_args()
@@ -621,6 +664,8 @@ def main():
         run_sweep(args)
     elif args.impl == "reference":
         run_reference(args)
+    elif args.sharded:
+        run_sharded(args)
     else:
         run_ours(args)
 

@@ -120,6 +120,8 @@ typedef struct {
    * ualpha_max ..), omega_max = max|v| tan(max|delta|); sampled u~^alpha ~ N(0, sigma_ualpha^2); stage cost
    * w_alpha * sum_i [h_i < h_buffer] max(0, alpha_i)^2.                                       */
   float proj_qv, proj_qomega, proj_qalpha, proj_rho, sigma_ualpha, ualpha_max, w_alpha, h_buffer;
+  int k_offset;       /* global index of this context's first sample, >= 0: sample k of the context draws the noise
+                         of sample k_offset + k and reports that index as argmin (K-sharded solves); 0 otherwise */
 } brmppi_params;
 
 #define BRMPPI_MAX_T 512
@@ -171,6 +173,21 @@ int brmppi_reset(brmppi_ctx* ctx);
  * Asynchronous on the stream.  A sample with non-finite cost gets weight 0; if all K are
  * non-finite U is left unchanged (diag.nonfinite == K). */
 int brmppi_solve(brmppi_ctx* ctx);
+/* K-sharded solve.  The online-softmax state (m, eta, A[2T]) of
+ * eq. (5) is associative, so G contexts (on G GPUs, or on one) can each own K/G of the samples of ONE solve:
+ * same seed, state, goal, obstacles and nominal in every context, k_offset = first global sample index.
+ * One MPPI iteration is then, on every shard:
+ *   brmppi_shard_export(ctx, dev_record)   rollout of this shard's samples, its partials merged into ONE
+ *                                          record of brmppi_shard_words(ctx) floats (per scene: m as fp64 in
+ *                                          words 0-1, argmin, eta, sum w^2, nonfinite, 2 unused, A[2T]);
+ *   (the caller gathers the G records in shard order: an all-gather of 4 (8 + 2T) bytes per scene and rank)
+ *   brmppi_shard_import(ctx, G, dev_records)  merges them, writes U and the diagnostics, counter + 1.
+ * Every shard merges the same records in the same order, so U is bit-identical on all of them.  dev_record /
+ * dev_records: DEVICE pointers, 8-byte aligned, owned by the caller.  Asynchronous on the stream. */
+size_t brmppi_shard_words(const brmppi_ctx* ctx);
+int brmppi_shard_export(brmppi_ctx* ctx, float* dev_record);
+int brmppi_shard_import(brmppi_ctx* ctx, int n_shards, const float* dev_records);
+
 /* Warm-start shift U[t] <- U[t+1], last element kept (reading 4).  Asynchronous. */
 int brmppi_shift(brmppi_ctx* ctx);
 /* One closed-loop control step as a single CUDA-graph replay: solve; apply U[0] to the

@@ -29,7 +29,7 @@ EXPORTS = [
     "brmppi_get_diag", "brmppi_get_phase_times", "brmppi_time_kernels", "brmppi_launch_count", "brmppi_strerror", "brmppi_debug_philox",
     "brmppi_debug_sample_controls", "brmppi_measure_peaks", "brmppi_get_hitch_filter", "brmppi_hitch_filter", "brmppi_project",
     "brmppi_debug_philox_raw", "brmppi_hitch_filter_scratch_bytes", "brmppi_project_scratch_bytes",
-    "brmppi_measure_peaks_scratch_bytes",
+    "brmppi_measure_peaks_scratch_bytes", "brmppi_shard_words", "brmppi_shard_export", "brmppi_shard_import",
 ]
 
 
@@ -63,7 +63,8 @@ class CParams(C.Structure):
                 ("hitch_kappa", C.c_float), ("hitch_filter", C.c_int), ("hitch_alpha", C.c_float),
                 ("hitch_qv", C.c_float), ("hitch_qdelta", C.c_float),
                 ("proj_qv", C.c_float), ("proj_qomega", C.c_float), ("proj_qalpha", C.c_float), ("proj_rho", C.c_float),
-                ("sigma_ualpha", C.c_float), ("ualpha_max", C.c_float), ("w_alpha", C.c_float), ("h_buffer", C.c_float)]
+                ("sigma_ualpha", C.c_float), ("ualpha_max", C.c_float), ("w_alpha", C.c_float), ("h_buffer", C.c_float),
+                ("k_offset", C.c_int)]
 
 
 class Diag(C.Structure):
@@ -102,6 +103,10 @@ def lib():
         L.brmppi_reset.argtypes = [vp]
         L.brmppi_solve.argtypes = [vp]
         L.brmppi_shift.argtypes = [vp]
+        L.brmppi_shard_words.argtypes = [vp]
+        L.brmppi_shard_words.restype = C.c_size_t
+        L.brmppi_shard_export.argtypes = [vp, vp]
+        L.brmppi_shard_import.argtypes = [vp, C.c_int, vp]
         L.brmppi_step.argtypes = [vp, _fp]
         L.brmppi_get_controls.argtypes = [vp, C.c_int, _fp]
         L.brmppi_get_state.argtypes = [vp, C.c_int, _fp]
@@ -141,7 +146,7 @@ def _check(status):
         raise BrmppiError(status, strerror(status))
 
 
-def make_cparams(p, n_scenes=1, max_obstacles=8, flags=0, max_superellipses=0) -> CParams:
+def make_cparams(p, n_scenes=1, max_obstacles=8, flags=0, max_superellipses=0, k_offset=0) -> CParams:
     """scenes.Params (plain data) -> brmppi_params."""
     c = CParams()
     c.K, c.T, c.n_iter, c.n_scenes = int(p.K), int(p.T), int(p.n_iter), int(n_scenes)
@@ -162,6 +167,7 @@ def make_cparams(p, n_scenes=1, max_obstacles=8, flags=0, max_superellipses=0) -
     for name, default in (("proj_qv", 1.0), ("proj_qomega", 4.0), ("proj_qalpha", 0.5), ("proj_rho", 0.25),
                           ("sigma_ualpha", 0.3), ("ualpha_max", 1.0), ("w_alpha", 10.0), ("h_buffer", 0.5)):
         setattr(c, name, float(getattr(p, name, default)))
+    c.k_offset = int(k_offset)
     return c
 
 
@@ -178,7 +184,7 @@ class Solver:
     """One brmppi_ctx plus the torch-owned workspace and stream it lives on."""
 
     def __init__(self, params, n_scenes=1, max_obstacles=8, flags=0, stream=None, device="cuda:0",
-                 max_superellipses=0):
+                 max_superellipses=0, k_offset=0):
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("brmppi needs a CUDA device (there is no CPU fallback)")
@@ -186,7 +192,7 @@ class Solver:
         self.device = torch.device(device)
         torch.cuda.set_device(self.device)
         self.params = params
-        self.cparams = make_cparams(params, n_scenes, max_obstacles, flags, max_superellipses)
+        self.cparams = make_cparams(params, n_scenes, max_obstacles, flags, max_superellipses, k_offset)
         self.max_superellipses = int(max_superellipses)
         self.n_scenes, self.K, self.T = int(n_scenes), int(params.K), int(params.T)
         self.max_obstacles = int(max_obstacles)
@@ -264,6 +270,20 @@ class Solver:
 
     def shift(self):
         _check(lib().brmppi_shift(self._ctx))
+
+    # ---- K-sharded solves -------------------------------------------------------
+    def shard_words(self):
+        return int(lib().brmppi_shard_words(self._ctx))
+
+    def shard_export(self, record):
+        """Rollout of this context's samples, merged into one record (float32 CUDA tensor of shard_words())."""
+        assert record.is_cuda and record.is_contiguous() and record.numel() >= self.shard_words()
+        _check(lib().brmppi_shard_export(self._ctx, C.c_void_p(record.data_ptr())))
+
+    def shard_import(self, records, n_shards):
+        """Merge n_shards records (float32 CUDA tensor [n_shards][shard_words()], in shard order) into U."""
+        assert records.is_cuda and records.is_contiguous() and records.numel() >= n_shards * self.shard_words()
+        _check(lib().brmppi_shard_import(self._ctx, int(n_shards), C.c_void_p(records.data_ptr())))
 
     def step(self):
         u0 = np.zeros((self.n_scenes, 2), dtype=np.float32)

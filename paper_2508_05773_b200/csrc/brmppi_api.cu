@@ -58,6 +58,7 @@ bool params_valid(const brmppi_params* p) {
   if (p->T < 1 || p->T > BRMPPI_MAX_T) return false;
   if (p->n_iter < 1 || p->n_scenes < 1 || p->n_scenes > 65535) return false;
   if ((long long)p->K * p->n_scenes > 0x7fffffffLL) return false;
+  if (p->k_offset < 0 || (long long)p->k_offset + p->K > 0x7fffffffLL) return false;
   if (p->max_obstacles < 0 || p->max_obstacles > BRMPPI_MAX_OBSTACLES) return false;
   if (p->max_superellipses < 0 || p->max_superellipses > BRMPPI_MAX_SUPERELLIPSES) return false;
   if (p->max_superellipses > 0 && (p->flags & BRMPPI_FLAG_KERNEL_THREAD_PER_SAMPLE)) return false;   // default kernel only
@@ -204,7 +205,7 @@ int launch_update(brmppi_ctx* c) {
   const DeviceParams& d = c->d;
   dim3 ugrid((unsigned)((2 * d.T + kUpdateOutputsPerBlock - 1) / kUpdateOutputsPerBlock),
              (unsigned)d.n_scenes);
-  merge_update<<<ugrid, kUpdateBlock, c->smem_update, c->stream>>>(d);
+  merge_update<kMergeLocal><<<ugrid, kUpdateBlock, c->smem_update, c->stream>>>(d, nullptr, 0);
   CU(cudaGetLastError());
   return BRMPPI_OK;
 }
@@ -287,7 +288,7 @@ int brmppi_create(const brmppi_params* p, void* dev_workspace, size_t workspace_
   DeviceParams& d = c->d;
   memset(&d, 0, sizeof(d));
   d.K = p->K; d.T = p->T; d.n_scenes = p->n_scenes; d.max_obstacles = p->max_obstacles;
-  d.n_discs = p->n_discs;
+  d.n_discs = p->n_discs; d.k_offset = p->k_offset;
   for (int j = 0; j < p->n_discs; ++j) {
     d.disc_body[j] = p->discs[j].body; d.disc_offset[j] = p->discs[j].offset;
     d.disc_a1[j] = p->discs[j].body == 0 ? p->discs[j].offset : 0.0f;
@@ -367,7 +368,7 @@ int brmppi_create(const brmppi_params* p, void* dev_workspace, size_t workspace_
       e = cudaFuncSetAttribute(rollout_thread_per_sample<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)prop.sharedMemPerBlockOptin);
   }
   if (e == cudaSuccess && c->smem_update > 48 * 1024)
-    e = cudaFuncSetAttribute(merge_update, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_update);
+    e = cudaFuncSetAttribute(merge_update<kMergeLocal>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_update);
   if (e == cudaSuccess && (c->smem_rollout > prop.sharedMemPerBlockOptin || c->smem_update > prop.sharedMemPerBlockOptin))
     e = cudaErrorInvalidValue;
   // zero: n_obs, U, counter, diag, u0 (state/goal stay unset until the caller provides them)
@@ -510,6 +511,36 @@ int brmppi_solve(brmppi_ctx* c) {
   }
   c->launches += 2ull * (unsigned)c->p.n_iter;
   c->n_host += (unsigned)c->p.n_iter;
+  return BRMPPI_OK;
+}
+
+size_t brmppi_shard_words(const brmppi_ctx* c) {
+  return c ? (size_t)c->p.n_scenes * (size_t)(kShardHeader + 2 * c->p.T) : 0;
+}
+
+int brmppi_shard_export(brmppi_ctx* c, float* dev_shard) {
+  if (!c || !dev_shard) return BRMPPI_ERR_NULL;
+  if ((uintptr_t)dev_shard % 8 != 0) return BRMPPI_ERR_UNALIGNED;
+  int r = ready(c);
+  if (r) return r;
+  r = launch_rollout(c);
+  if (r) return r;
+  dim3 ugrid((unsigned)(2 * c->d.T), (unsigned)c->d.n_scenes);
+  merge_update<kMergeExport><<<ugrid, kUpdateBlock, 0, c->stream>>>(c->d, dev_shard, 0);
+  CU(cudaGetLastError());
+  c->launches += 2;
+  return BRMPPI_OK;
+}
+
+int brmppi_shard_import(brmppi_ctx* c, int n_shards, const float* dev_shards) {
+  if (!c || !dev_shards) return BRMPPI_ERR_NULL;
+  if (n_shards < 1) return BRMPPI_ERR_INVALID_ARG;
+  if ((uintptr_t)dev_shards % 8 != 0) return BRMPPI_ERR_UNALIGNED;
+  dim3 ugrid((unsigned)(2 * c->d.T), (unsigned)c->d.n_scenes);
+  merge_update<kMergeImport><<<ugrid, kUpdateBlock, 0, c->stream>>>(c->d, const_cast<float*>(dev_shards), n_shards);
+  CU(cudaGetLastError());
+  c->launches += 1;
+  c->n_host += 1;
   return BRMPPI_OK;
 }
 

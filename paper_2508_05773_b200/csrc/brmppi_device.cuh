@@ -21,6 +21,7 @@ constexpr float kInvTwoPi = 0.15915494309189535f;
 // so scalar weights fold into FFMA operands without a load).
 struct DeviceParams {
   int K, T, n_scenes, max_obstacles, n_discs, max_superellipses;
+  int k_offset;               // global index of this context's first sample (Philox counter, argmin): K-sharded solves
   int disc_body[kMaxDiscs];
   float disc_offset[kMaxDiscs];
   float disc_a1[kMaxDiscs], disc_a2[kMaxDiscs];   // offset on the tractor axis / on the trailer axis (one is 0)

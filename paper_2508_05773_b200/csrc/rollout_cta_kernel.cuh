@@ -426,7 +426,7 @@ rollout_cta(const __grid_constant__ DeviceParams P) {
       for (; mi < n_pairs; ) {
         const int t = 2 * mi, t1 = min(t + 1, T - 1);
         float2 u0, u1;
-        sample_control_pair<PRECISE>(P, __ldg(Unom + t), __ldg(Unom + t1), (uint32_t)mi, n, (uint32_t)(k0 + si), key0, key1, &u0, &u1);
+        sample_control_pair<PRECISE>(P, __ldg(Unom + t), __ldg(Unom + t1), (uint32_t)mi, n, (uint32_t)(k0 + si + P.k_offset), key0, key1, &u0, &u1);
         float* pV = planes + si * TS;
         float* pD = pV + S * TS;
         float* pP1 = pD + S * TS;
@@ -439,7 +439,7 @@ rollout_cta(const __grid_constant__ DeviceParams P) {
         si += ds; mi += dm;
         if (si >= S) { si -= S; ++mi; }
       }
-      if (c == 0) BRMPPI_SMEM(float, P.off_alpha)[s] = sample_alpha(P, n, (uint32_t)k, key0, key1);
+      if (c == 0) BRMPPI_SMEM(float, P.off_alpha)[s] = sample_alpha(P, n, (uint32_t)(k + P.k_offset), key0, key1);
     }
     if (new_scene && warp == kTableWarp) {
       // The scene's obstacle tables, by the one warp that generates no noise on this tile.
@@ -712,7 +712,7 @@ rollout_cta(const __grid_constant__ DeviceParams P) {
       }
       finite = valid && (Sk == Sk) && (Sk < CUDART_INF) && (Sk > -CUDART_INF);
       double m = finite ? Sk : CUDART_INF;
-      int idx = finite ? k : 0x7fffffff;
+      int idx = finite ? k + P.k_offset : 0x7fffffff;     // global sample index (K-sharded solves)
       warp_argmin(m, idx);
       if (lane == 0) { sM->redM[warp] = m; sM->redI[warp] = idx; }
     }

@@ -119,7 +119,7 @@ rollout_projected(const __grid_constant__ DeviceParams P) {
     State X{0.0f, 0.0f, x0.z, x0.w};
     float alpha[NO];
     {
-      const float a0 = sample_alpha(P, n, (uint32_t)k, key0, key1);
+      const float a0 = sample_alpha(P, n, (uint32_t)(k + P.k_offset), key0, key1);
 #pragma unroll
       for (int i = 0; i < NO; ++i) alpha[i] = a0;
     }
@@ -128,12 +128,12 @@ rollout_projected(const __grid_constant__ DeviceParams P) {
     double cost = 0.0;
     // The draws of step t + 1 do not depend on the state: they are generated during step t, so that the long
     // Philox / Box-Muller chains fill the issue slots the Cholesky chain leaves empty.
-    float2 u_next = sample_control<PRECISE>(P, sU[0], 0u, n, (uint32_t)k, key0, key1);
+    float2 u_next = sample_control<PRECISE>(P, sU[0], 0u, n, (uint32_t)(k + P.k_offset), key0, key1);
     float ua_next[NO];
 #pragma unroll
     for (int q = 0; 4 * q < NO; ++q) {
       float z4[4];
-      normals4<PRECISE>(0u, n, (uint32_t)k, 2u + (uint32_t)q, key0, key1, z4);
+      normals4<PRECISE>(0u, n, (uint32_t)(k + P.k_offset), 2u + (uint32_t)q, key0, key1, z4);
 #pragma unroll
       for (int e = 0; e < 4; ++e)
         if (4 * q + e < NO) ua_next[4 * q + e] = P.sigma_ualpha * z4[e];
@@ -147,11 +147,11 @@ rollout_projected(const __grid_constant__ DeviceParams P) {
       for (int i = 0; i < NO; ++i) ua[i] = ua_next[i];
       {
         const uint32_t tn = (uint32_t)min(t + 1, T - 1);
-        u_next = sample_control<PRECISE>(P, sU[tn], tn, n, (uint32_t)k, key0, key1);
+        u_next = sample_control<PRECISE>(P, sU[tn], tn, n, (uint32_t)(k + P.k_offset), key0, key1);
 #pragma unroll
         for (int q = 0; 4 * q < NO; ++q) {
           float z4[4];
-          normals4<PRECISE>(tn, n, (uint32_t)k, 2u + (uint32_t)q, key0, key1, z4);
+          normals4<PRECISE>(tn, n, (uint32_t)(k + P.k_offset), 2u + (uint32_t)q, key0, key1, z4);
 #pragma unroll
           for (int e = 0; e < 4; ++e)
             if (4 * q + e < NO) ua_next[4 * q + e] = P.sigma_ualpha * z4[e];

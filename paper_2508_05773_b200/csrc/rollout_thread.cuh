@@ -29,7 +29,7 @@ __device__ __forceinline__ void thread_kernel_epilogue(const DeviceParams& P, co
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const bool finite = valid && (S == S) && (S < CUDART_INF) && (S > -CUDART_INF);
   double m = finite ? S : CUDART_INF;
-  int idx = finite ? k : 0x7fffffff;
+  int idx = finite ? k + P.k_offset : 0x7fffffff;       // global sample index (K-sharded solves)
   warp_argmin(m, idx);
   if (lane == 0) { sRedM[warp] = m; sRedI[warp] = idx; }
   __syncthreads();
@@ -46,7 +46,7 @@ __device__ __forceinline__ void thread_kernel_epilogue(const DeviceParams& P, co
   // weighted control sums: regenerate u_k[t] from the counter-based generator
   for (int t = 0; t < T; ++t) {
     float2 u = make_float2(0.0f, 0.0f);
-    if (finite) u = sample_control<PRECISE>(P, sU[t], (uint32_t)t, n, (uint32_t)k, key0, key1);
+    if (finite) u = sample_control<PRECISE>(P, sU[t], (uint32_t)t, n, (uint32_t)(k + P.k_offset), key0, key1);
     const float av = warp_sum(wk * u.x), ad = warp_sum(wk * u.y);
     if (lane == 0) { sA[warp * 2 * T + 2 * t] = av; sA[warp * 2 * T + 2 * t + 1] = ad; }
   }
@@ -110,7 +110,7 @@ rollout_thread_per_sample(const __grid_constant__ DeviceParams P) {
   State X{0.0f, 0.0f, x0.z, x0.w};
   float alpha = 0.0f;
   if (valid) {
-    alpha = sample_alpha(P, n, (uint32_t)k, key0, key1);
+    alpha = sample_alpha(P, n, (uint32_t)(k + P.k_offset), key0, key1);
     const float one_minus_alpha = 1.0f - alpha;
     float s1, c1, s2, c2;
     sincos_t<PRECISE>(X.psi1, &s1, &c1);
@@ -119,7 +119,7 @@ rollout_thread_per_sample(const __grid_constant__ DeviceParams P) {
     disc_centres(P, X, s1, c1, s2, c2, pcx, pcy);
     double track = 0.0, bar = 0.0;
     for (int t = 0; t < T; ++t) {
-      const float2 u = sample_control<PRECISE>(P, sU[t], (uint32_t)t, n, (uint32_t)k, key0, key1);
+      const float2 u = sample_control<PRECISE>(P, sU[t], (uint32_t)t, n, (uint32_t)(k + P.k_offset), key0, key1);
       const float tan_d = tan_t<PRECISE>(u.y);
       const State Xn = kinematic_step(P, X, s1, c1, s2, c2, u.x, tan_d);
       sincos_t<PRECISE>(Xn.psi1, &s1, &c1);

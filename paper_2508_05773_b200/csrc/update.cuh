@@ -21,31 +21,55 @@ constexpr int kUpdateOutputsPerBlock = 1;   // one CTA per output channel o = 2 
 // (coalesced rows, all loads of a thread independent, so the kernel is two L2 round trips deep),
 // then a fixed-order block reduction.  Every CTA recomputes the global minimum itself -- P * 12
 // bytes from L2 -- rather than paying a third kernel or a grid-wide sync for it.
+//
+// MODE (K-sharded solves): the online-softmax state (m, eta, A[2T]) is associative, so a
+// solve can be split over contexts / GPUs that each own a range of the samples.
+//   kMergeLocal   this context's partials -> U, diagnostics, counter + 1            (the single-GPU path)
+//   kMergeExport  this context's partials -> ONE shard record (m, argmin, eta, w2, nonfinite, A[2T]) in
+//                 `shard`, nothing else touched
+//   kMergeImport  n_shards shard records in `shard` ([n_shards][n_scenes][kShardHeader + 2T] floats, in
+//                 shard order) -> U, diagnostics, counter + 1
+// Shard record: words 0-1 = m (fp64), 2 = argmin (int), 3 = eta, 4 = sum w^2, 5 = nonfinite (int), 6-7 unused,
+// 8 + o = A[o] (o = 2t + channel).
+enum MergeMode { kMergeLocal = 0, kMergeExport = 1, kMergeImport = 2 };
+constexpr int kShardHeader = 8;
+
+template <int MODE>
 __global__ void __launch_bounds__(kUpdateBlock)
-merge_update(const __grid_constant__ DeviceParams P) {
+merge_update(const __grid_constant__ DeviceParams P, float* shard, int n_shards) {
   __shared__ double sM[kUpdateBlock / 32];
   __shared__ int sI[kUpdateBlock / 32];
   __shared__ float sRed[4][kUpdateBlock / 32];
   const int scene = blockIdx.y, o = blockIdx.x;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int words = kShardHeader + 2 * P.T;
   // partial slots in use: the persistent kernel writes one per CTA whose tile range touches this
-  // scene (CTA b owns the flat tiles [b Q, (b+1) Q)); the thread-per-sample kernel fills them all
+  // scene (CTA b owns the flat tiles [b Q, (b+1) Q)); the thread-per-sample kernels fill them all
   const int Pstride = P.n_partials;
   int Pn = Pstride;
-  if (P.tiles_per_cta > 0) {
+  if (MODE == kMergeImport) {
+    Pn = n_shards;
+  } else if (P.tiles_per_cta > 0) {
     const int first = (scene * P.tiles_per_scene) / P.tiles_per_cta;
     const int last = ((scene + 1) * P.tiles_per_scene - 1) / P.tiles_per_cta;
     Pn = last - first + 1;
   }
   const double* pm = P.part_m + (size_t)scene * Pstride;
   const int* pi = P.part_argmin + (size_t)scene * Pstride;
+  const float* peta = P.part_eta + (size_t)scene * Pstride;
+  const float* pa = P.part_A + ((size_t)scene * 2 * P.T + o) * Pstride;
+  const float* pw2 = P.part_w2 + (size_t)scene * Pstride;
+  const int* pnf = P.part_nonfinite + (size_t)scene * Pstride;
+  auto rec = [&](int p) { return shard + ((size_t)p * P.n_scenes + scene) * words; };
+  auto part_m = [&](int p) { return MODE == kMergeImport ? *reinterpret_cast<const double*>(rec(p)) : pm[p]; };
+  auto part_i = [&](int p) { return MODE == kMergeImport ? __float_as_int(rec(p)[2]) : pi[p]; };
 
   // global minimum and its sample index (lowest index on ties)
   double m = CUDART_INF;
   int idx = 0x7fffffff;
   for (int p = tid; p < Pn; p += kUpdateBlock) {
-    const double om = pm[p];
-    const int oi = pi[p];
+    const double om = part_m(p);
+    const int oi = part_i(p);
     if (om < m || (om == m && oi < idx)) { m = om; idx = oi; }
   }
   warp_argmin(m, idx);
@@ -57,18 +81,21 @@ merge_update(const __grid_constant__ DeviceParams P) {
     if (sM[w] < m || (sM[w] == m && sI[w] < idx)) { m = sM[w]; idx = sI[w]; }
   const bool any_finite = m < CUDART_INF;
 
-  const float* peta = P.part_eta + (size_t)scene * Pstride;
-  const float* pa = P.part_A + ((size_t)scene * 2 * P.T + o) * Pstride;
-  const float* pw2 = P.part_w2 + (size_t)scene * Pstride;
-  const int* pnf = P.part_nonfinite + (size_t)scene * Pstride;
   const bool diag_cta = (o == 0);
   float eta = 0.0f, acc = 0.0f, w2 = 0.0f, nf = 0.0f;
   for (int p = tid; p < Pn; p += kUpdateBlock) {
-    const double mp = pm[p];
+    const double mp = part_m(p);
     const float c = (any_finite && mp < CUDART_INF) ? expf((float)(-(mp - m) * (double)P.inv_lambda)) : 0.0f;
-    eta = fmaf(c, peta[p], eta);
-    acc = fmaf(c, pa[p], acc);
-    if (diag_cta) { w2 = fmaf(c * c, pw2[p], w2); nf += (float)pnf[p]; }
+    if (MODE == kMergeImport) {
+      const float* r = rec(p);
+      eta = fmaf(c, r[3], eta);
+      acc = fmaf(c, r[kShardHeader + o], acc);
+      if (diag_cta) { w2 = fmaf(c * c, r[4], w2); nf += (float)__float_as_int(r[5]); }
+    } else {
+      eta = fmaf(c, peta[p], eta);
+      acc = fmaf(c, pa[p], acc);
+      if (diag_cta) { w2 = fmaf(c * c, pw2[p], w2); nf += (float)pnf[p]; }
+    }
   }
   eta = warp_sum(eta); acc = warp_sum(acc); w2 = warp_sum(w2); nf = warp_sum(nf);
   if (lane == 0) { sRed[0][warp] = eta; sRed[1][warp] = acc; sRed[2][warp] = w2; sRed[3][warp] = nf; }
@@ -77,6 +104,16 @@ merge_update(const __grid_constant__ DeviceParams P) {
     eta = 0.0f; acc = 0.0f; w2 = 0.0f; nf = 0.0f;
 #pragma unroll
     for (int w = 0; w < kUpdateBlock / 32; ++w) { eta += sRed[0][w]; acc += sRed[1][w]; w2 += sRed[2][w]; nf += sRed[3][w]; }
+    if (MODE == kMergeExport) {
+      float* r = shard + (size_t)scene * words;
+      r[kShardHeader + o] = acc;
+      if (diag_cta) {
+        *reinterpret_cast<double*>(r) = m;
+        r[2] = __int_as_float(any_finite ? idx : 0x7fffffff);
+        r[3] = eta; r[4] = w2; r[5] = __int_as_float((int)nf); r[6] = 0.0f; r[7] = 0.0f;
+      }
+      return;
+    }
     if (any_finite && eta > 0.0f) P.U[(size_t)scene * 2 * P.T + o] = acc / eta;
     if (diag_cta) {
       brmppi_diag d;
