@@ -728,3 +728,189 @@ int orc_iteration_projected(const orc_params* p, const orc_proj_params* pp, uint
   if (!u_all) free(u_buf);
   return nonfinite;
 }
+
+/* ------------------------------------------------------------------------------------------
+ * The paper's own model and tracking cost: eq. (6), (13)-(15), (17);
+ * readings in the header (reading 31).
+ * ---------------------------------------------------------------------------------------- */
+
+/* eq. (6): x = [px, py, v, a, theta1, theta2, delta], u = [j, omega]; every RHS at step k. */
+void orc7_step(const orc_params* p, const orc_mpcc_params* mp, const double x[7], const double u[2], double xn[7]) {
+  double Ts = p->dt, v = x[2], a = x[3], th1 = x[4], th2 = x[5], de = x[6];
+  xn[0] = x[0] + Ts * v * cos(th1);
+  xn[1] = x[1] + Ts * v * sin(th1);
+  xn[2] = v + Ts * a;
+  xn[3] = a + Ts * u[0];
+  xn[4] = th1 + Ts * (v / p->L1) * tan(de);
+  xn[5] = th2 + Ts * (v / p->L2) * (sin(th1 - th2) - (p->Lh / p->L1) * cos(th1 - th2) * tan(de));
+  xn[6] = clampd(de + Ts * u[1], mp->delta_lo, mp->delta_hi);
+}
+
+void orc_path_eval(const orc_mpcc_params* mp, double psi, double out[4]) {
+  double L = mp->M * mp->dpsi;
+  if (psi < 0.0) psi = 0.0;
+  if (psi > L) psi = L;
+  int m = (int)floor(psi / mp->dpsi);
+  if (m > mp->M - 1) m = mp->M - 1;
+  double s = psi - m * mp->dpsi;
+  for (int c = 0; c < 4; ++c) {
+    const double* q = mp->coef + ((size_t)m * 4 + c) * 4;
+    out[c] = q[0] + s * (q[1] + s * (q[2] + s * q[3]));
+  }
+}
+
+double orc7_progress(const orc_mpcc_params* mp, const double x[7], double psi) {
+  double r[4];
+  orc_path_eval(mp, psi, r);
+  return x[2] * cos(x[4] - r[2]);
+}
+
+/* (14), (15) PAPER.md:207-210 as printed; heading errors PAPER.md:212, wrapped. */
+void orc7_errors(const orc_mpcc_params* mp, const double x[7], double psi, double e[4]) {
+  double r[4];
+  orc_path_eval(mp, psi, r);
+  double dx = x[0] - r[0], dy = x[1] - r[1];
+  e[0] = sin(r[2]) * dx - cos(r[2]) * dy;
+  e[1] = -cos(r[2]) * dx - sin(r[2]) * dy;
+  e[2] = orc_wrap(x[4] - r[2]);
+  e[3] = orc_wrap(x[5] - r[3]);
+}
+
+/* (17): hhat = h + Ts hdot + Ts^2/2 hddot along the continuous model
+ *   pdot = v e(th1), vdot = a, th1dot = W1 = (v/l1) tan(delta), th2dot = W2 = (v/l2)(sin b - k cos b tan(delta)),
+ *   deltadot = omega, b = th1 - th2, k = lh/l1,
+ * for the disc centre c = p - lh e(th1) + a_j e(th_body) and the obstacle o(t) = o0 + t Ts vel. */
+double orc7_hhat(const orc_params* p, const double x[7], const double u[2], const double* ob, int t, int j,
+                 double* h_out) {
+  double Ts = p->dt, v = x[2], a = x[3], th1 = x[4], th2 = x[5], de = x[6], om = u[1];
+  double td = tan(de), sec2 = 1.0 / (cos(de) * cos(de));
+  double b = th1 - th2, kap = p->Lh / p->L1;
+  double W1 = (v / p->L1) * td;
+  double W2 = (v / p->L2) * (sin(b) - kap * cos(b) * td);
+  double bdot = W1 - W2;
+  double W1dot = (a / p->L1) * td + (v / p->L1) * sec2 * om;
+  double W2dot = (a / p->L2) * (sin(b) - kap * cos(b) * td) +
+                 (v / p->L2) * (cos(b) * bdot + kap * sin(b) * bdot * td - kap * cos(b) * sec2 * om);
+  double e1[2] = {cos(th1), sin(th1)}, n1[2] = {-sin(th1), cos(th1)};
+  double thb = (p->disc_body[j] == 0) ? th1 : th2;
+  double Wb = (p->disc_body[j] == 0) ? W1 : W2, Wbdot = (p->disc_body[j] == 0) ? W1dot : W2dot;
+  double eb[2] = {cos(thb), sin(thb)}, nb[2] = {-sin(thb), cos(thb)};
+  double aj = p->disc_offset[j];
+  double c[2], cd[2], cdd[2];
+  for (int q = 0; q < 2; ++q) {
+    c[q] = x[q] - p->Lh * e1[q] + aj * eb[q];
+    cd[q] = v * e1[q] - p->Lh * W1 * n1[q] + aj * Wb * nb[q];
+    cdd[q] = a * e1[q] + v * W1 * n1[q] - p->Lh * (W1dot * n1[q] - W1 * W1 * e1[q]) +
+             aj * (Wbdot * nb[q] - Wb * Wb * eb[q]);
+  }
+  double o[2] = {ob[0] + (double)t * Ts * ob[3], ob[1] + (double)t * Ts * ob[4]};
+  double rho = ob[2] + p->disc_radius;
+  double d[2] = {c[0] - o[0], c[1] - o[1]}, dd[2] = {cd[0] - ob[3], cd[1] - ob[4]};
+  double h = (d[0] * d[0] + d[1] * d[1]) / (rho * rho) - 1.0;
+  double hdot = 2.0 * (d[0] * dd[0] + d[1] * dd[1]) / (rho * rho);
+  double hddot = 2.0 * (dd[0] * dd[0] + dd[1] * dd[1] + d[0] * cdd[0] + d[1] * cdd[1]) / (rho * rho);
+  if (h_out) *h_out = h;
+  return h + Ts * hdot + 0.5 * Ts * Ts * hddot;
+}
+
+static double mpcc_tracking(const orc_mpcc_params* mp, const double x[7], double psi) {
+  double e[4];
+  orc7_errors(mp, x, psi, e);
+  return mp->Qc * e[0] * e[0] + mp->Ql * e[1] * e[1] + mp->Qth1 * e[2] * e[2] + mp->Qth2 * e[3] * e[3];
+}
+
+double orc7_rollout(const orc_params* p, const orc_mpcc_params* mp, const double x0[7], double psi0, int n_obs,
+                    const double* obstacles, const double* u, double alpha, double xT[8], double* traj) {
+  const int T = p->T, D = p->n_discs;
+  double X[7], psi = psi0, S = 0.0, L = mp->M * mp->dpsi;
+  memcpy(X, x0, sizeof(X));
+  if (traj) { memcpy(traj, X, sizeof(X)); traj[7] = psi; }
+  for (int t = 0; t < T; ++t) {
+    const double* ut = u + 2 * t;
+    /* barrier-rate hinge with the predictor (17) in the place of h(x_{k+1}) */
+    double pen = 0.0;
+    for (int i = 0; i < n_obs; ++i)
+      for (int j = 0; j < D; ++j) {
+        double h, hhat = orc7_hhat(p, X, ut, obstacles + 5 * i, t, j, &h);
+        double viol = (1.0 - alpha) * h - hhat;
+        if (viol > 0.0) pen += viol;
+      }
+    double Xn[7];
+    orc7_step(p, mp, X, ut, Xn);
+    double psin = clampd(psi + p->dt * orc7_progress(mp, X, psi), 0.0, L);
+    /* stage cost (13) on (x_{k+1}, u_k, psi_{k+1}) */
+    double nu = orc7_progress(mp, Xn, psin);
+    double hitch = fabs(orc_wrap(Xn[4] - Xn[5])) - (p->hitch_max - p->hitch_kappa * fabs(Xn[2]));
+    if (hitch < 0.0) hitch = 0.0;
+    S += mpcc_tracking(mp, Xn, psin) + mp->Rj * ut[0] * ut[0] + mp->Rw * ut[1] * ut[1] +
+         mp->mu * (mp->nu_bar - nu) * (mp->nu_bar - nu) + p->w_hitch * hitch * hitch + p->w_bar * pen;
+    memcpy(X, Xn, sizeof(X));
+    psi = psin;
+    if (traj) { memcpy(traj + 8 * (t + 1), X, sizeof(X)); traj[8 * (t + 1) + 7] = psi; }
+  }
+  S += p->w_term * mpcc_tracking(mp, X, psi);
+  memcpy(xT, X, sizeof(X));
+  xT[7] = psi;
+  return S;
+}
+
+double orc7_sample(const orc_params* p, const orc_mpcc_params* mp, uint32_t n, uint32_t k, const double x0[7],
+                   double psi0, int n_obs, const double* obstacles, const double* U_in, double* u, double xT[8]) {
+  double alpha = orc_alpha(p, n, k);
+  for (int t = 0; t < p->T; ++t) {
+    double z[2];
+    orc_normals(p->seed, n, k, (uint32_t)t, z);
+    u[2 * t + 0] = clampd(U_in[2 * t + 0] + mp->sigma_j * z[0], mp->j_min, mp->j_max);
+    u[2 * t + 1] = clampd(U_in[2 * t + 1] + mp->sigma_omega * z[1], mp->omega_min, mp->omega_max);
+  }
+  return orc7_rollout(p, mp, x0, psi0, n_obs, obstacles, u, alpha, xT, NULL);
+}
+
+typedef struct {
+  const orc_params* p;
+  const orc_mpcc_params* mp;
+  uint32_t n;
+  const double *x0, *obstacles, *U_in;
+  double psi0;
+  int n_obs, k_begin, k_end;
+  double *S, *XT, *u_all;
+} mpcc_job;
+
+static void* mpcc_worker(void* arg) {
+  mpcc_job* b = (mpcc_job*)arg;
+  const int T = b->p->T;
+  for (int k = b->k_begin; k < b->k_end; ++k)
+    b->S[k] = orc7_sample(b->p, b->mp, b->n, (uint32_t)k, b->x0, b->psi0, b->n_obs, b->obstacles, b->U_in,
+                          b->u_all + (size_t)k * 2 * T, b->XT + 8 * (size_t)k);
+  return NULL;
+}
+
+int orc7_iteration(const orc_params* p, const orc_mpcc_params* mp, uint32_t n, const double x0[7], double psi0,
+                   int n_obs, const double* obstacles, const double* U_in, double* U_out, double* S, double* XT,
+                   double* u_all, double* w, int* argmin, double* gap, double* eta, int n_threads) {
+  const int K = p->K, T = p->T;
+  double* S_buf = S ? S : (double*)malloc(sizeof(double) * (size_t)K);
+  double* XT_buf = XT ? XT : (double*)malloc(sizeof(double) * 8 * (size_t)K);
+  double* u_buf = u_all ? u_all : (double*)malloc(sizeof(double) * 2 * (size_t)T * (size_t)K);
+  double* U_nom = (double*)malloc(sizeof(double) * 2 * (size_t)T);
+  memcpy(U_nom, U_in, sizeof(double) * 2 * (size_t)T);
+  if (n_threads < 1) n_threads = 1;
+  if (n_threads > K) n_threads = K;
+  mpcc_job* jobs = (mpcc_job*)malloc(sizeof(mpcc_job) * (size_t)n_threads);
+  pthread_t* tids = (pthread_t*)malloc(sizeof(pthread_t) * (size_t)n_threads);
+  for (int i = 0; i < n_threads; ++i)
+    jobs[i] = (mpcc_job){p, mp, n, x0, obstacles, U_nom, psi0, n_obs, (int)((long long)K * i / n_threads),
+                         (int)((long long)K * (i + 1) / n_threads), S_buf, XT_buf, u_buf};
+  if (n_threads == 1) mpcc_worker(&jobs[0]);
+  else {
+    for (int i = 0; i < n_threads; ++i) pthread_create(&tids[i], NULL, mpcc_worker, &jobs[i]);
+    for (int i = 0; i < n_threads; ++i) pthread_join(tids[i], NULL);
+  }
+  if (U_out != U_in) memcpy(U_out, U_nom, sizeof(double) * 2 * (size_t)T);
+  int nonfinite = orc_weights_update(K, T, p->lambda, S_buf, u_buf, U_out, w, argmin, gap, eta);
+  free(jobs); free(tids); free(U_nom);
+  if (!S) free(S_buf);
+  if (!XT) free(XT_buf);
+  if (!u_all) free(u_buf);
+  return nonfinite;
+}

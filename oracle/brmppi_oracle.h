@@ -271,6 +271,61 @@ int orc_iteration_projected(const orc_params* p, const orc_proj_params* pp, uint
                             double* U_out, double* S, double* XT, double* u_all, double* w, int* argmin,
                             double* gap, double* eta, int n_threads);
 
+/* ---- the paper's own model and tracking cost (reading 31) ------------------
+ *
+ * 7-state kinematic model with jerk and steering-rate inputs, eq. (6), state
+ * x = [p^x, p^y, v, a, theta1, theta2, delta], u = [j, omega], explicit Euler as printed; second-order Taylor
+ * predictor of the barrier, eq. (17); contouring / lag / heading / effort / progress cost,
+ * eq. (13)-(15) PAPER.md:196-212, along a reference path zeta(psi) given as cubic splines in arc length.
+ *
+ * Readings where the paper is silent:
+ *  - reference path: M cubic segments on uniform knots psi_m = m dpsi for each of (p^{x,r}, p^{y,r}, theta^{1,r},
+ *    theta^{2,r}): value = c0 + c1 s + c2 s^2 + c3 s^3, s = psi - m dpsi, m = min(floor(psi / dpsi), M - 1), psi
+ *    clamped to [0, M dpsi] ("third-order spline");
+ *  - path parameter: psi_{k+1} = clamp(psi_k + T_s nu_k), nu_k = v_k cos(theta1_k - theta^{1,r}(psi_k)) -- "the
+ *    projection velocity along the reference path";
+ *  - delta is clamped to [delta_lo, delta_hi] after its Euler update (steering stops); v and a are free;
+ *  - stage cost on (x_{k+1}, u_k, psi_{k+1}) (reading 3): Q_c e_c^2 + Q_l e_l^2 + Q_th1 e_th1^2 + Q_th2 e_th2^2
+ *    + R_j j^2 + R_w omega^2 + mu (nu_bar - nu_{k+1})^2 + the hitch hinge of reading 15 (with |v_{k+1}|)
+ *    + w_bar * sum_{i,j} max(0, (1 - alpha) h_ij(x_k, o_i(k)) - hhat_ij(x_k, u_k)): the barrier-rate condition
+ *    of the penalty path with h(x_{k+1}) replaced by the predictor (17), whose hdot and hddot are the first and
+ *    second Lie derivatives of h (disc j against obstacle i, reading 10) along the continuous model under the
+ *    sampled input -- hddot depends on omega through d(delta)/dt, not on j (relative degree 3);
+ *    terminal cost w_term * (the four tracking terms at (x_N, psi_N));
+ *  - sampled inputs: clamp(U + sigma z) on (j, omega), same noise stream as the penalty path; alpha per sample
+ *    (reading 8); update (5) on (j, omega).
+ * Pins: tests/test_oracle_mpcc.py.  The weights are never printed in the paper (PARITY UNPINNED, like the
+ * penalty path's). */
+typedef struct {
+  double j_min, j_max, omega_min, omega_max;     /* j in [-2, 2] m/s^3, omega in [-0.9, 0.9] rad/s */
+  double sigma_j, sigma_omega;
+  double delta_lo, delta_hi;
+  double Qc, Ql, Qth1, Qth2, Rj, Rw, mu, nu_bar; /* weights of (13)                                             */
+  int M;                                         /* cubic segments of the reference path                        */
+  double dpsi;                                   /* knot spacing in arc length                                  */
+  const double* coef;                            /* [M][4 components][4 coefficients c0..c3]                    */
+} orc_mpcc_params;
+
+/* eq. (6), explicit Euler, delta clamped. */
+void orc7_step(const orc_params* p, const orc_mpcc_params* mp, const double x[7], const double u[2], double xn[7]);
+/* (p^{x,r}, p^{y,r}, theta^{1,r}, theta^{2,r}) at arc length psi. */
+void orc_path_eval(const orc_mpcc_params* mp, double psi, double out[4]);
+/* nu = v cos(theta1 - theta^{1,r}(psi)). */
+double orc7_progress(const orc_mpcc_params* mp, const double x[7], double psi);
+/* (e^c, e^l, e^theta1, e^theta2) of (14), (15) and PAPER.md:212 (heading errors wrapped). */
+void orc7_errors(const orc_mpcc_params* mp, const double x[7], double psi, double e[4]);
+/* Predictor (17) for vehicle disc j against obstacle (cx, cy, R, vx, vy) at step t: returns hhat, *h = h(x). */
+double orc7_hhat(const orc_params* p, const double x[7], const double u[2], const double* obstacle, int t,
+                 int j, double* h);
+/* One rollout under sampled, clamped inputs u[T][2]; xT[8] = final state and psi; traj (optional) [(T+1)][8]. */
+double orc7_rollout(const orc_params* p, const orc_mpcc_params* mp, const double x0[7], double psi0, int n_obs,
+                    const double* obstacles, const double* u, double alpha, double xT[8], double* traj);
+double orc7_sample(const orc_params* p, const orc_mpcc_params* mp, uint32_t n, uint32_t k, const double x0[7],
+                   double psi0, int n_obs, const double* obstacles, const double* U_in, double* u, double xT[8]);
+int orc7_iteration(const orc_params* p, const orc_mpcc_params* mp, uint32_t n, const double x0[7], double psi0,
+                   int n_obs, const double* obstacles, const double* U_in, double* U_out, double* S, double* XT,
+                   double* u_all, double* w, int* argmin, double* gap, double* eta, int n_threads);
+
 #ifdef __cplusplus
 }
 #endif

@@ -47,6 +47,14 @@ class _ProjParams(C.Structure):
                 ("h_buffer", C.c_double)]
 
 
+class _MpccParams(C.Structure):
+    _fields_ = [("j_min", C.c_double), ("j_max", C.c_double), ("omega_min", C.c_double), ("omega_max", C.c_double),
+                ("sigma_j", C.c_double), ("sigma_omega", C.c_double), ("delta_lo", C.c_double), ("delta_hi", C.c_double),
+                ("Qc", C.c_double), ("Ql", C.c_double), ("Qth1", C.c_double), ("Qth2", C.c_double),
+                ("Rj", C.c_double), ("Rw", C.c_double), ("mu", C.c_double), ("nu_bar", C.c_double),
+                ("M", C.c_int), ("dpsi", C.c_double), ("coef", C.POINTER(C.c_double))]
+
+
 _lib = None
 _dp = C.POINTER(C.c_double)
 _u32p = C.POINTER(C.c_uint32)
@@ -130,6 +138,24 @@ def lib():
         L.orc_iteration_projected.argtypes = [C.POINTER(_Params), PP, C.c_uint32, _dp, _dp, C.c_int, _dp, _dp,
                                               _dp, _dp, _dp, _dp, _dp, ip, _dp, _dp, C.c_int]
         L.orc_iteration_projected.restype = C.c_int
+        MP = C.POINTER(_MpccParams)
+        L.orc7_step.argtypes = [C.POINTER(_Params), MP, _dp, _dp, _dp]
+        L.orc7_step.restype = None
+        L.orc_path_eval.argtypes = [MP, C.c_double, _dp]
+        L.orc_path_eval.restype = None
+        L.orc7_progress.argtypes = [MP, _dp, C.c_double]
+        L.orc7_progress.restype = C.c_double
+        L.orc7_errors.argtypes = [MP, _dp, C.c_double, _dp]
+        L.orc7_errors.restype = None
+        L.orc7_hhat.argtypes = [C.POINTER(_Params), _dp, _dp, _dp, C.c_int, C.c_int, _dp]
+        L.orc7_hhat.restype = C.c_double
+        L.orc7_rollout.argtypes = [C.POINTER(_Params), MP, _dp, C.c_double, C.c_int, _dp, _dp, C.c_double, _dp, _dp]
+        L.orc7_rollout.restype = C.c_double
+        L.orc7_sample.argtypes = [C.POINTER(_Params), MP, C.c_uint32, C.c_uint32, _dp, C.c_double, C.c_int, _dp, _dp, _dp, _dp]
+        L.orc7_sample.restype = C.c_double
+        L.orc7_iteration.argtypes = [C.POINTER(_Params), MP, C.c_uint32, _dp, C.c_double, C.c_int, _dp, _dp, _dp, _dp, _dp,
+                                     _dp, _dp, ip, _dp, _dp, C.c_int]
+        L.orc7_iteration.restype = C.c_int
         _lib = L
     return _lib
 
@@ -448,6 +474,98 @@ def solve_projected(p, n0, x0, goal, obstacles, U_in, n_threads=1):
     outs = []
     for it in range(p.n_iter):
         r = iteration_projected(p, n0 + it, x0, goal, obstacles, U, n_threads=n_threads)
+        U = r["U"].copy()
+        outs.append(r)
+    return outs
+
+
+# ---- the paper's own model and tracking cost: eq. (6), (13)-(15), (17) ------------------------------
+def _mparams(p, coef, dpsi):
+    """(struct, keep-alive array): coef [M][4][4]."""
+    coef = _d(coef)
+    s = _MpccParams()
+    for name in ("j_min", "j_max", "omega_min", "omega_max", "sigma_j", "sigma_omega", "Qc", "Ql", "Qth1", "Qth2",
+                 "Rj", "Rw", "mu", "nu_bar"):
+        setattr(s, name, float(getattr(p, name)))
+    s.delta_lo, s.delta_hi = float(p.delta_min), float(p.delta_max)
+    s.M, s.dpsi = int(coef.shape[0]), float(dpsi)
+    s.coef = _ptr(coef)
+    return s, coef
+
+
+def step7(p, coef, dpsi, x, u):
+    mp, keep = _mparams(p, coef, dpsi)
+    xn = np.zeros(7)
+    lib().orc7_step(C.byref(_cparams(p)), C.byref(mp), _ptr(_d(x, (7,))), _ptr(_d(u, (2,))), _ptr(xn))
+    return xn
+
+
+def path_eval(p, coef, dpsi, psi):
+    mp, keep = _mparams(p, coef, dpsi)
+    out = np.zeros(4)
+    lib().orc_path_eval(C.byref(mp), float(psi), _ptr(out))
+    return out
+
+
+def progress7(p, coef, dpsi, x, psi):
+    mp, keep = _mparams(p, coef, dpsi)
+    return lib().orc7_progress(C.byref(mp), _ptr(_d(x, (7,))), float(psi))
+
+
+def errors7(p, coef, dpsi, x, psi):
+    mp, keep = _mparams(p, coef, dpsi)
+    e = np.zeros(4)
+    lib().orc7_errors(C.byref(mp), _ptr(_d(x, (7,))), float(psi), _ptr(e))
+    return e
+
+
+def hhat7(p, x, u, obstacle, t, j):
+    """(hhat, h) of eq. (17) for disc j against one obstacle at step t."""
+    h = C.c_double()
+    hh = lib().orc7_hhat(C.byref(_cparams(p)), _ptr(_d(x, (7,))), _ptr(_d(u, (2,))), _ptr(_d(obstacle, (5,))), int(t), int(j),
+                         C.byref(h))
+    return hh, h.value
+
+
+def rollout7(p, coef, dpsi, x0, psi0, obstacles, u, alpha):
+    mp, keep = _mparams(p, coef, dpsi)
+    obs = _d(obstacles).reshape(-1, 5)
+    xT, traj = np.zeros(8), np.zeros((p.T + 1, 8))
+    S = lib().orc7_rollout(C.byref(_cparams(p)), C.byref(mp), _ptr(_d(x0, (7,))), float(psi0), obs.shape[0], _ptr(obs),
+                           _ptr(_d(u, (p.T, 2))), float(alpha), _ptr(xT), _ptr(traj))
+    return dict(S=S, xT=xT, traj=traj)
+
+
+def sample7(p, coef, dpsi, n, k, x0, psi0, obstacles, U_in):
+    mp, keep = _mparams(p, coef, dpsi)
+    obs = _d(obstacles).reshape(-1, 5)
+    u, xT = np.zeros((p.T, 2)), np.zeros(8)
+    S = lib().orc7_sample(C.byref(_cparams(p)), C.byref(mp), int(n), int(k), _ptr(_d(x0, (7,))), float(psi0), obs.shape[0],
+                          _ptr(obs), _ptr(_d(U_in, (p.T, 2))), _ptr(u), _ptr(xT))
+    return dict(S=S, u=u, xT=xT)
+
+
+def iteration7(p, coef, dpsi, n, x0, psi0, obstacles, U_in, n_threads=1, want_samples=False):
+    mp, keep = _mparams(p, coef, dpsi)
+    obs = _d(obstacles).reshape(-1, 5)
+    K, T = p.K, p.T
+    U_out, S, XT, w = np.zeros((T, 2)), np.zeros(K), np.zeros((K, 8)), np.zeros(K)
+    u_all = np.zeros((K, T, 2))
+    argmin, gap, eta = C.c_int(), C.c_double(), C.c_double()
+    nonfinite = lib().orc7_iteration(C.byref(_cparams(p)), C.byref(mp), int(n), _ptr(_d(x0, (7,))), float(psi0), obs.shape[0],
+                                     _ptr(obs), _ptr(_d(U_in, (T, 2))), _ptr(U_out), _ptr(S), _ptr(XT), _ptr(u_all), _ptr(w),
+                                     C.byref(argmin), C.byref(gap), C.byref(eta), int(n_threads))
+    out = dict(U=U_out, S=S, XT=XT, w=w, argmin=argmin.value, gap=gap.value, eta=eta.value, nonfinite=nonfinite)
+    if want_samples:
+        out["u"] = u_all
+    return out
+
+
+def solve7(p, coef, dpsi, n0, x0, psi0, obstacles, U_in, n_threads=1):
+    U = _d(U_in, (p.T, 2)).copy()
+    outs = []
+    for it in range(p.n_iter):
+        r = iteration7(p, coef, dpsi, n0 + it, x0, psi0, obstacles, U, n_threads=n_threads)
         U = r["U"].copy()
         outs.append(r)
     return outs

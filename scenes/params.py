@@ -56,6 +56,21 @@ class Params:
     ualpha_max: float = 1.0       # u^alpha in [-ualpha_max, ualpha_max]
     w_alpha: float = 10.0         # cost on positive alpha inside the buffer zone h < h_buffer
     h_buffer: float = 0.5
+    # the paper's own model and tracking cost, eq. (6), (13)-(15), (17) (reading 31); read only in MPCC mode
+    j_min: float = -2.0           # jerk bounds, m/s^3
+    j_max: float = 2.0
+    omega_min: float = -0.9       # steering-rate bounds, rad/s
+    omega_max: float = 0.9
+    sigma_j: float = 0.8
+    sigma_omega: float = 0.3
+    Qc: float = 2.0               # weights of (13): contouring, lag, the two headings, effort, progress
+    Ql: float = 0.5
+    Qth1: float = 0.5
+    Qth2: float = 0.5
+    Rj: float = 0.01
+    Rw: float = 0.1
+    mu: float = 0.2
+    nu_bar: float = 1.5           # desired progress rate along the path, m/s
     w_bar: float = 1.0e3
     w_term: float = 10.0
     lam: float = 1.0
