@@ -87,6 +87,14 @@ typedef struct { int body; float offset; } brmppi_disc;
                                           auxiliary input; no hinge penalty (w_bar is not read).  Readings:
                                           DESIGN.md reading 30.  max_obstacles <= BRMPPI_PROJECT_MAX_NO, no
                                           super-ellipses; one thread per sample.                            */
+#define BRMPPI_FLAG_MPCC 64u            /* the paper's own model and tracking cost (DESIGN.md
+                                          reading 31): 7-state jerk / steering-rate model, eq. (6)
+                                          (PAPER.md:119-127), barrier-rate hinge on the second-order predictor (17)
+                                          (PAPER.md:221-225), contouring / lag / heading / effort / progress cost
+                                          (13)-(15) along a cubic reference path.  Controls are
+                                          (j, omega); the state is set with brmppi_set_state7 and the path with
+                                          brmppi_set_reference_path (no goal).  One thread per sample; not with
+                                          PROJECTED, super-ellipses or the hitch filter.                        */
 #define BRMPPI_FLAG_NO_CULL 16u         /* evaluate every (obstacle, disc, step) even where the
                                           hinge is provably zero; same results  */
 
@@ -122,12 +130,23 @@ typedef struct {
   float proj_qv, proj_qomega, proj_qalpha, proj_rho, sigma_ualpha, ualpha_max, w_alpha, h_buffer;
   int k_offset;       /* global index of this context's first sample, >= 0: sample k of the context draws the noise
                          of sample k_offset + k and reports that index as argmin (K-sharded solves); 0 otherwise */
+  /* The paper's own model and cost (read only with BRMPPI_FLAG_MPCC).  The sampled inputs are u = (j, omega):
+   * box [j_min, j_max] x [omega_min, omega_max], Sigma_w = diag(sigma_j^2, sigma_omega^2); the
+   * steering STATE delta is clamped to [delta_min, delta_max] after its Euler update; weights of (13): Qc
+   * (contouring), Ql (lag), Qth1 / Qth2 (headings), Rj / Rw (effort), mu (progress, against nu_bar m/s); w_hitch,
+   * hitch_max, hitch_kappa, w_bar, w_term, lambda, alpha_lo / alpha_hi as on the penalty path (w_term multiplies the
+   * four tracking terms at the final state).  v_min .. sigma_delta's control-box meaning, w_pos, w_head, w_v and
+   * w_delta are not read.  max_path_segments: capacity of the reference path, 1..BRMPPI_MAX_PATH_SEGMENTS.     */
+  float j_min, j_max, omega_min, omega_max, sigma_j, sigma_omega;
+  float Qc, Ql, Qth1, Qth2, Rj, Rw, mu, nu_bar;
+  int max_path_segments;
 } brmppi_params;
 
 #define BRMPPI_MAX_T 512
 #define BRMPPI_MAX_OBSTACLES 64
 #define BRMPPI_MAX_SUPERELLIPSES 16
 #define BRMPPI_PROJECT_MAX_NO 8     /* obstacles (rows of (9)) the projection handles */
+#define BRMPPI_MAX_PATH_SEGMENTS 256
 
 typedef struct brmppi_ctx brmppi_ctx;   /* opaque, library-owned host object */
 
@@ -152,16 +171,25 @@ int brmppi_create(const brmppi_params* p, void* dev_workspace, size_t workspace_
 /* Destroys the host object (and any captured graph).  Never frees the workspace. */
 int brmppi_destroy(brmppi_ctx* ctx);
 
-/* Vehicle state (x, y, psi1, psi2) of one scene.  psi1, psi2 are wrapped to [-pi, pi]. */
+/* Vehicle state (x, y, psi1, psi2) of one scene.  psi1, psi2 are wrapped to [-pi, pi].  Not with BRMPPI_FLAG_MPCC. */
 int brmppi_set_state(brmppi_ctx* ctx, int scene, const float x[4]);
-/* Goal pose (g_x, g_y, g_psi1, g_psi2). */
+/* BRMPPI_FLAG_MPCC: state x = (p_x, p_y, v, a, theta1, theta2, delta) of eq. (6) and the path parameter psi (arc
+ * length of the vehicle's reference point on the path, 0 <= psi <= M dpsi, else BRMPPI_ERR_INVALID_ARG; delta must
+ * lie in [delta_min, delta_max]).  theta1, theta2 are wrapped to [-pi, pi].  HOST pointer. */
+int brmppi_set_state7(brmppi_ctx* ctx, int scene, const float x[7], float psi);
+/* BRMPPI_FLAG_MPCC: reference path of one scene: M cubic segments on uniform knots of spacing dpsi > 0 in arc
+ * length, coef[M][4][4] = coefficients c0..c3 (value = c0 + s (c1 + s (c2 + s c3)), s = psi - m dpsi) of the four
+ * components (p^{x,r}, p^{y,r}, theta^{1,r}, theta^{2,r}) of segment m.  1 <= M <=
+ * max_path_segments.  HOST pointer, copied.  Set it before brmppi_set_state7 (psi is checked against M dpsi). */
+int brmppi_set_reference_path(brmppi_ctx* ctx, int scene, int M, float dpsi, const float* coef);
+/* Goal pose (g_x, g_y, g_psi1, g_psi2).  Not with BRMPPI_FLAG_MPCC. */
 int brmppi_set_goal(brmppi_ctx* ctx, int scene, const float g[4]);
 /* Obstacles of one scene at rollout time 0; 0 <= n <= max_obstacles (NULL allowed when n = 0). */
 int brmppi_set_obstacles(brmppi_ctx* ctx, int scene, int n, const brmppi_obstacle* obstacles);
 /* Super-ellipse obstacles of one scene at rollout time 0; 0 <= n <= max_superellipses (NULL allowed
  * when n = 0).  mx, my > 0; exponent 2 or 4 (else BRMPPI_ERR_INVALID_ARG). */
 int brmppi_set_superellipses(brmppi_ctx* ctx, int scene, int n, const brmppi_superellipse* obstacles);
-/* Nominal control sequence U[T][2] = (v, delta) per step; NULL = zeros.  Values must lie in
+/* Nominal control sequence U[T][2] = (v, delta) per step ((j, omega) with BRMPPI_FLAG_MPCC); NULL = zeros.  Values must lie in
  * the control box (else BRMPPI_ERR_INVALID_ARG). */
 int brmppi_set_nominal(brmppi_ctx* ctx, int scene, const float* U);
 /* Set the global iteration counter n (the Philox counter word; reading 7).  All scenes. */
@@ -191,17 +219,20 @@ int brmppi_shard_import(brmppi_ctx* ctx, int n_shards, const float* dev_records)
 /* Warm-start shift U[t] <- U[t+1], last element kept (reading 4).  Asynchronous. */
 int brmppi_shift(brmppi_ctx* ctx);
 /* One closed-loop control step as a single CUDA-graph replay: solve; apply U[0] to the
- * kinematic model (one Euler step of eq. (6), psi wrapped); advance obstacles by dt * velocity;
+ * kinematic model (one Euler step of eq. (6), psi wrapped; with BRMPPI_FLAG_MPCC the 7-state step and the
+ * path-parameter update of reading 31); advance obstacles by dt * velocity;
  * shift.  Synchronises; u0_out[n_scenes][2] receives the applied control of each scene. */
 int brmppi_step(brmppi_ctx* ctx, float* u0_out);
 
 /* Results.  All synchronise the stream. */
 int brmppi_get_controls(brmppi_ctx* ctx, int scene, float* U_out /* T*2 */);
 int brmppi_get_state(brmppi_ctx* ctx, int scene, float x_out[4]);
+int brmppi_get_state7(brmppi_ctx* ctx, int scene, float x_out[8]);   /* FLAG_MPCC: the seven states, then psi */
 int brmppi_get_obstacles(brmppi_ctx* ctx, int scene, int* n_out, brmppi_obstacle* out /* max_obstacles */);
 int brmppi_get_superellipses(brmppi_ctx* ctx, int scene, int* n_out, brmppi_superellipse* out /* max_superellipses */);
 int brmppi_get_costs(brmppi_ctx* ctx, int scene, float* S_out /* K */);             /* FLAG_WRITE_SAMPLES */
 int brmppi_get_final_states(brmppi_ctx* ctx, int scene, float* X_out /* K*4 */);    /* FLAG_WRITE_SAMPLES */
+int brmppi_get_final_states7(brmppi_ctx* ctx, int scene, float* X_out /* K*8 */);   /* FLAG_WRITE_SAMPLES | FLAG_MPCC */
 int brmppi_get_diag(brmppi_ctx* ctx, int scene, brmppi_diag* out);
 /* What the hitch-angle stabiliser did in the last brmppi_step: u_ref = the BR-MPPI control U[0] it was
  * given, *status = 0 (rate constraint inactive, applied control = u_ref), 1 (active), 2 (no control in

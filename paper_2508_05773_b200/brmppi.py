@@ -16,6 +16,7 @@ FLAG_KERNEL_THREAD_PER_SAMPLE = 4
 FLAG_PHASE_TIMING = 8
 FLAG_NO_CULL = 16
 FLAG_PROJECTED = 32
+FLAG_MPCC = 64
 
 OK = 0
 ERR_NULL, ERR_INVALID_ARG, ERR_WORKSPACE_TOO_SMALL, ERR_TOO_MANY_OBSTACLES = -1, -2, -3, -4
@@ -30,6 +31,7 @@ EXPORTS = [
     "brmppi_debug_sample_controls", "brmppi_measure_peaks", "brmppi_get_hitch_filter", "brmppi_hitch_filter", "brmppi_project",
     "brmppi_debug_philox_raw", "brmppi_hitch_filter_scratch_bytes", "brmppi_project_scratch_bytes",
     "brmppi_measure_peaks_scratch_bytes", "brmppi_shard_words", "brmppi_shard_export", "brmppi_shard_import",
+    "brmppi_set_state7", "brmppi_set_reference_path", "brmppi_get_state7", "brmppi_get_final_states7",
 ]
 
 
@@ -64,7 +66,12 @@ class CParams(C.Structure):
                 ("hitch_qv", C.c_float), ("hitch_qdelta", C.c_float),
                 ("proj_qv", C.c_float), ("proj_qomega", C.c_float), ("proj_qalpha", C.c_float), ("proj_rho", C.c_float),
                 ("sigma_ualpha", C.c_float), ("ualpha_max", C.c_float), ("w_alpha", C.c_float), ("h_buffer", C.c_float),
-                ("k_offset", C.c_int)]
+                ("k_offset", C.c_int),
+                ("j_min", C.c_float), ("j_max", C.c_float), ("omega_min", C.c_float), ("omega_max", C.c_float),
+                ("sigma_j", C.c_float), ("sigma_omega", C.c_float),
+                ("Qc", C.c_float), ("Ql", C.c_float), ("Qth1", C.c_float), ("Qth2", C.c_float),
+                ("Rj", C.c_float), ("Rw", C.c_float), ("mu", C.c_float), ("nu_bar", C.c_float),
+                ("max_path_segments", C.c_int)]
 
 
 class Diag(C.Structure):
@@ -95,6 +102,10 @@ def lib():
         L.brmppi_destroy.argtypes = [vp]
         L.brmppi_set_state.argtypes = [vp, C.c_int, _fp]
         L.brmppi_set_goal.argtypes = [vp, C.c_int, _fp]
+        L.brmppi_set_state7.argtypes = [vp, C.c_int, _fp, C.c_float]
+        L.brmppi_set_reference_path.argtypes = [vp, C.c_int, C.c_int, C.c_float, _fp]
+        L.brmppi_get_state7.argtypes = [vp, C.c_int, _fp]
+        L.brmppi_get_final_states7.argtypes = [vp, C.c_int, _fp]
         L.brmppi_set_obstacles.argtypes = [vp, C.c_int, C.c_int, C.POINTER(Obstacle)]
         L.brmppi_set_superellipses.argtypes = [vp, C.c_int, C.c_int, C.POINTER(Superellipse)]
         L.brmppi_get_superellipses.argtypes = [vp, C.c_int, C.POINTER(C.c_int), C.POINTER(Superellipse)]
@@ -146,7 +157,8 @@ def _check(status):
         raise BrmppiError(status, strerror(status))
 
 
-def make_cparams(p, n_scenes=1, max_obstacles=8, flags=0, max_superellipses=0, k_offset=0) -> CParams:
+def make_cparams(p, n_scenes=1, max_obstacles=8, flags=0, max_superellipses=0, k_offset=0,
+                 max_path_segments=64) -> CParams:
     """scenes.Params (plain data) -> brmppi_params."""
     c = CParams()
     c.K, c.T, c.n_iter, c.n_scenes = int(p.K), int(p.T), int(p.n_iter), int(n_scenes)
@@ -168,6 +180,11 @@ def make_cparams(p, n_scenes=1, max_obstacles=8, flags=0, max_superellipses=0, k
                           ("sigma_ualpha", 0.3), ("ualpha_max", 1.0), ("w_alpha", 10.0), ("h_buffer", 0.5)):
         setattr(c, name, float(getattr(p, name, default)))
     c.k_offset = int(k_offset)
+    for name, default in (("j_min", -2.0), ("j_max", 2.0), ("omega_min", -0.9), ("omega_max", 0.9), ("sigma_j", 0.8),
+                          ("sigma_omega", 0.3), ("Qc", 2.0), ("Ql", 0.5), ("Qth1", 0.5), ("Qth2", 0.5), ("Rj", 0.01),
+                          ("Rw", 0.1), ("mu", 0.2), ("nu_bar", 1.5)):
+        setattr(c, name, float(getattr(p, name, default)))
+    c.max_path_segments = int(max_path_segments)
     return c
 
 
@@ -184,7 +201,7 @@ class Solver:
     """One brmppi_ctx plus the torch-owned workspace and stream it lives on."""
 
     def __init__(self, params, n_scenes=1, max_obstacles=8, flags=0, stream=None, device="cuda:0",
-                 max_superellipses=0, k_offset=0):
+                 max_superellipses=0, k_offset=0, max_path_segments=64):
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("brmppi needs a CUDA device (there is no CPU fallback)")
@@ -192,7 +209,9 @@ class Solver:
         self.device = torch.device(device)
         torch.cuda.set_device(self.device)
         self.params = params
-        self.cparams = make_cparams(params, n_scenes, max_obstacles, flags, max_superellipses, k_offset)
+        self.cparams = make_cparams(params, n_scenes, max_obstacles, flags, max_superellipses, k_offset,
+                                    max_path_segments)
+        self.mpcc = bool(flags & FLAG_MPCC)
         self.max_superellipses = int(max_superellipses)
         self.n_scenes, self.K, self.T = int(n_scenes), int(params.K), int(params.T)
         self.max_obstacles = int(max_obstacles)
@@ -256,7 +275,21 @@ class Solver:
     def reset(self):
         _check(lib().brmppi_reset(self._ctx))
 
+    def set_reference_path(self, coef, dpsi, scene=0):
+        """FLAG_MPCC: coef [M][4][4] cubic coefficients of (p^{x,r}, p^{y,r}, theta^{1,r}, theta^{2,r})."""
+        coef = _f32(coef)
+        M = coef.shape[0]
+        _check(lib().brmppi_set_reference_path(self._ctx, scene, int(M), float(dpsi), _p(_f32(coef, (M, 4, 4)))))
+
+    def set_state7(self, x, psi, scene=0):
+        _check(lib().brmppi_set_state7(self._ctx, scene, _p(_f32(x, (7,))), float(psi)))
+
     def set_scene(self, scene_obj, scene=0):
+        if self.mpcc:                     # a scenes.PathScene
+            self.set_reference_path(scene_obj.coef, scene_obj.dpsi, scene)
+            self.set_state7(scene_obj.x0, scene_obj.psi0, scene)
+            self.set_obstacles(scene_obj.obstacles, scene)
+            return
         self.set_state(scene_obj.x0, scene)
         self.set_goal(scene_obj.goal, scene)
         self.set_obstacles(scene_obj.obstacles, scene)
@@ -303,6 +336,17 @@ class Solver:
         x = np.zeros(4, dtype=np.float32)
         _check(lib().brmppi_get_state(self._ctx, scene, _p(x)))
         return x
+
+    def get_state7(self, scene=0):
+        """FLAG_MPCC: (p_x, p_y, v, a, theta1, theta2, delta, psi)."""
+        x = np.zeros(8, dtype=np.float32)
+        _check(lib().brmppi_get_state7(self._ctx, scene, _p(x)))
+        return x
+
+    def get_final_states7(self, scene=0):
+        X = np.zeros((self.K, 8), dtype=np.float32)
+        _check(lib().brmppi_get_final_states7(self._ctx, scene, _p(X)))
+        return X
 
     def get_obstacles(self, scene=0):
         n = C.c_int(0)

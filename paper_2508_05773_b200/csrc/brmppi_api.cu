@@ -15,6 +15,7 @@
 #include "peaks.cuh"
 #include "rollout_thread.cuh"
 #include "rollout_projected.cuh"
+#include "rollout_mpcc.cuh"
 #include "rollout_cta.cuh"
 #include "rollout_cta_kernel.cuh"
 #include "update.cuh"
@@ -82,8 +83,16 @@ bool params_valid(const brmppi_params* p) {
   if (p->alpha_lo > p->alpha_hi) return false;
   const unsigned known = BRMPPI_FLAG_WRITE_SAMPLES | BRMPPI_FLAG_PRECISE_MATH |
                          BRMPPI_FLAG_KERNEL_THREAD_PER_SAMPLE | BRMPPI_FLAG_PHASE_TIMING |
-                         BRMPPI_FLAG_NO_CULL | BRMPPI_FLAG_PROJECTED;
+                         BRMPPI_FLAG_NO_CULL | BRMPPI_FLAG_PROJECTED | BRMPPI_FLAG_MPCC;
   if (p->flags & ~known) return false;
+  if (p->flags & BRMPPI_FLAG_MPCC) {
+    if ((p->flags & BRMPPI_FLAG_PROJECTED) || p->max_superellipses > 0 || p->hitch_filter) return false;
+    if (p->max_path_segments < 1 || p->max_path_segments > BRMPPI_MAX_PATH_SEGMENTS) return false;
+    const float q[] = {p->j_min, p->j_max, p->omega_min, p->omega_max, p->sigma_j, p->sigma_omega, p->Qc, p->Ql,
+                       p->Qth1, p->Qth2, p->Rj, p->Rw, p->mu, p->nu_bar};
+    if (!finite_all(q, 14)) return false;
+    if (p->j_min > p->j_max || p->omega_min > p->omega_max || p->sigma_j < 0.f || p->sigma_omega < 0.f) return false;
+  }
   if (p->flags & BRMPPI_FLAG_PROJECTED) {
     if (p->max_obstacles > BRMPPI_PROJECT_MAX_NO || p->max_superellipses > 0) return false;
     const float q[] = {p->proj_qv, p->proj_qomega, p->proj_qalpha, p->proj_rho, p->sigma_ualpha, p->ualpha_max,
@@ -97,7 +106,7 @@ bool params_valid(const brmppi_params* p) {
 
 struct Layout {
   size_t state, goal, n_obs, obstacles, n_se, se, U, counter, u0, part_m, part_argmin, part_eta, part_w2,
-      part_nf, part_A, diag, S, XT, phase, hitch, total;
+      part_nf, part_A, diag, S, XT, phase, hitch, state7, path_M, path_dpsi, path_coef, total;
 };
 
 // Launch plan: which rollout kernel, how the sample axis is tiled, how many partials.
@@ -120,7 +129,7 @@ int device_sm_count() {
 
 Plan make_plan(const brmppi_params& p) {
   Plan pl{};
-  pl.cta_kernel = !(p.flags & (BRMPPI_FLAG_KERNEL_THREAD_PER_SAMPLE | BRMPPI_FLAG_PROJECTED));
+  pl.cta_kernel = !(p.flags & (BRMPPI_FLAG_KERNEL_THREAD_PER_SAMPLE | BRMPPI_FLAG_PROJECTED | BRMPPI_FLAG_MPCC));
   if (pl.cta_kernel) {
     pl.cta = make_cta_plan(p.K, p.T, p.n_scenes, p.max_obstacles, p.max_superellipses, device_sm_count());
     pl.n_partials = pl.cta.n_partials;
@@ -145,6 +154,12 @@ Layout make_layout(const brmppi_params& p, const Plan& pl) {
   L.counter = take(4);
   L.u0 = take(ns * 8);
   L.hitch = take(ns * 16);
+  if (p.flags & BRMPPI_FLAG_MPCC) {
+    L.state7 = take(ns * 32);
+    L.path_M = take(ns * 4);
+    L.path_dpsi = take(ns * 4);
+    L.path_coef = take(ns * (size_t)p.max_path_segments * 64);
+  }
   L.part_m = take(ns * P * 8);
   L.part_argmin = take(ns * P * 4);
   L.part_eta = take(ns * P * 4);
@@ -154,7 +169,7 @@ Layout make_layout(const brmppi_params& p, const Plan& pl) {
   L.diag = take(ns * sizeof(brmppi_diag));
   if (p.flags & BRMPPI_FLAG_WRITE_SAMPLES) {
     L.S = take(ns * (size_t)p.K * 4);
-    L.XT = take(ns * (size_t)p.K * 16);
+    L.XT = take(ns * (size_t)p.K * ((p.flags & BRMPPI_FLAG_MPCC) ? 32 : 16));
   }
   if ((p.flags & BRMPPI_FLAG_PHASE_TIMING) && pl.cta_kernel)
     L.phase = take((size_t)pl.cta.grid * (kPhaseSlots + 2) * sizeof(unsigned long long));
@@ -176,6 +191,7 @@ struct brmppi_ctx {
   unsigned int n_host;          // host mirror of the device iteration counter
   cudaGraphExec_t solve_graph, step_graph;
   float* pinned_u0;             // [n_scenes][2] staging for brmppi_step
+  float* path_len;              // [n_scenes] M dpsi of the reference path (BRMPPI_FLAG_MPCC), host
   size_t smem_rollout, smem_update;
 };
 
@@ -186,6 +202,13 @@ int launch_rollout(brmppi_ctx* c) {
   const bool precise = (c->p.flags & BRMPPI_FLAG_PRECISE_MATH) != 0;
   if (c->plan.cta_kernel) {
     CU(launch_rollout_cta(d, c->plan.cta, precise, c->stream));
+  } else if (c->p.flags & BRMPPI_FLAG_MPCC) {
+    dim3 grid((unsigned)c->plan.n_partials, (unsigned)d.n_scenes);
+    if (precise)
+      rollout_mpcc<true><<<grid, kThreadBlock, c->smem_rollout, c->stream>>>(d);
+    else
+      rollout_mpcc<false><<<grid, kThreadBlock, c->smem_rollout, c->stream>>>(d);
+    CU(cudaGetLastError());
   } else if (c->p.flags & BRMPPI_FLAG_PROJECTED) {
     dim3 grid((unsigned)c->plan.n_partials, (unsigned)d.n_scenes);
     projected_kernel_for(precise, d.max_obstacles)<<<grid, kThreadBlock, c->smem_rollout, c->stream>>>(d);
@@ -284,6 +307,7 @@ int brmppi_create(const brmppi_params* p, void* dev_workspace, size_t workspace_
   c->solve_graph = nullptr;
   c->step_graph = nullptr;
   c->pinned_u0 = nullptr;
+  c->path_len = (float*)calloc((size_t)p->n_scenes, sizeof(float));
 
   DeviceParams& d = c->d;
   memset(&d, 0, sizeof(d));
@@ -313,6 +337,14 @@ int brmppi_create(const brmppi_params* p, void* dev_workspace, size_t workspace_
   d.Lh_over_L1 = p->Lh / p->L1; d.Lh_over_L2 = p->Lh / p->L2;
   d.v_min = p->v_min; d.v_max = p->v_max; d.delta_min = p->delta_min; d.delta_max = p->delta_max;
   d.sigma_v = p->sigma_v; d.sigma_delta = p->sigma_delta;
+  if (p->flags & BRMPPI_FLAG_MPCC) {
+    // the sampled inputs are (j, omega): their box and sigmas take the control slots of the sampler
+    d.v_min = p->j_min; d.v_max = p->j_max; d.delta_min = p->omega_min; d.delta_max = p->omega_max;
+    d.sigma_v = p->sigma_j; d.sigma_delta = p->sigma_omega;
+    d.dstate_lo = p->delta_min; d.dstate_hi = p->delta_max;
+    d.Qc = p->Qc; d.Ql = p->Ql; d.Qth1 = p->Qth1; d.Qth2 = p->Qth2; d.Rj = p->Rj; d.Rw = p->Rw;
+    d.mu = p->mu; d.nu_bar = p->nu_bar; d.max_path_segments = p->max_path_segments;
+  }
   d.alpha_lo = p->alpha_lo; d.alpha_span = p->alpha_hi - p->alpha_lo;
   d.w_pos = p->w_pos; d.w_head = p->w_head; d.w_v = p->w_v; d.w_delta = p->w_delta;
   d.w_hitch = p->w_hitch; d.hitch_max = p->hitch_max; d.hitch_kappa = p->hitch_kappa; d.w_bar = p->w_bar; d.w_term = p->w_term;
@@ -344,6 +376,10 @@ int brmppi_create(const brmppi_params* p, void* dev_workspace, size_t workspace_
   d.U = (float*)(base + L.U); d.counter = (uint32_t*)(base + L.counter);
   d.u0_applied = (float*)(base + L.u0);
   d.hitch_ref = (float*)(base + L.hitch);
+  if (p->flags & BRMPPI_FLAG_MPCC) {
+    d.state7 = (float*)(base + L.state7); d.path_M = (int*)(base + L.path_M);
+    d.path_dpsi = (float*)(base + L.path_dpsi); d.path_coef = (float*)(base + L.path_coef);
+  }
   d.part_m = (double*)(base + L.part_m); d.part_argmin = (int*)(base + L.part_argmin);
   d.part_eta = (float*)(base + L.part_eta); d.part_w2 = (float*)(base + L.part_w2);
   d.part_nonfinite = (int*)(base + L.part_nf); d.part_A = (float*)(base + L.part_A);
@@ -357,11 +393,17 @@ int brmppi_create(const brmppi_params* p, void* dev_workspace, size_t workspace_
     c->smem_rollout = c->plan.cta.smem;
     e = configure_rollout_cta((p->flags & BRMPPI_FLAG_PRECISE_MATH) != 0, p->n_discs, c->smem_rollout);
   } else {
-    c->smem_rollout = (p->flags & BRMPPI_FLAG_PROJECTED) ? rollout_projected_smem_bytes(d) : rollout_thread_smem_bytes(d);
+    c->smem_rollout = (p->flags & BRMPPI_FLAG_PROJECTED) ? rollout_projected_smem_bytes(d)
+                      : (p->flags & BRMPPI_FLAG_MPCC)    ? rollout_mpcc_smem_bytes(d)
+                                                         : rollout_thread_smem_bytes(d);
     // per function and device, not per context: always the opt-in maximum, never lowered
     if (p->flags & BRMPPI_FLAG_PROJECTED)
       e = cudaFuncSetAttribute(projected_kernel_for((p->flags & BRMPPI_FLAG_PRECISE_MATH) != 0, p->max_obstacles),
                                cudaFuncAttributeMaxDynamicSharedMemorySize, (int)prop.sharedMemPerBlockOptin);
+    if (e == cudaSuccess)
+      e = cudaFuncSetAttribute(rollout_mpcc<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)prop.sharedMemPerBlockOptin);
+    if (e == cudaSuccess)
+      e = cudaFuncSetAttribute(rollout_mpcc<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)prop.sharedMemPerBlockOptin);
     if (e == cudaSuccess)
       e = cudaFuncSetAttribute(rollout_thread_per_sample<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)prop.sharedMemPerBlockOptin);
     if (e == cudaSuccess)
@@ -377,7 +419,7 @@ int brmppi_create(const brmppi_params* p, void* dev_workspace, size_t workspace_
   if (e == cudaSuccess) e = cudaHostAlloc((void**)&c->pinned_u0, sizeof(float) * 2 * (size_t)p->n_scenes, cudaHostAllocMapped);
   if (e == cudaSuccess) e = cudaHostGetDevicePointer((void**)&d.u0_host, c->pinned_u0, 0);
   if (e != cudaSuccess) {
-    free(c->state_set); free(c->goal_set);
+    free(c->state_set); free(c->goal_set); free(c->path_len);
     delete c;
     return cuda_fail(e);
   }
@@ -392,6 +434,7 @@ int brmppi_destroy(brmppi_ctx* c) {
   if (c->pinned_u0) cudaFreeHost(c->pinned_u0);
   free(c->state_set);
   free(c->goal_set);
+  free(c->path_len);
   delete c;
   return BRMPPI_OK;
 }
@@ -411,6 +454,7 @@ int brmppi_set_state(brmppi_ctx* c, int scene, const float x[4]) {
   int r = check_scene(c, scene);
   if (r) return r;
   if (!x) return BRMPPI_ERR_NULL;
+  if (c->p.flags & BRMPPI_FLAG_MPCC) return BRMPPI_ERR_INVALID_ARG;
   if (!finite_all(x, 4)) return BRMPPI_ERR_NONFINITE_INPUT;
   const float v[4] = {x[0], x[1], wrap_pi(x[2]), wrap_pi(x[3])};
   CU(cudaMemcpyAsync(c->d.state + 4 * scene, v, sizeof(v), cudaMemcpyHostToDevice, c->stream));
@@ -418,10 +462,46 @@ int brmppi_set_state(brmppi_ctx* c, int scene, const float x[4]) {
   return BRMPPI_OK;
 }
 
+int brmppi_set_state7(brmppi_ctx* c, int scene, const float x[7], float psi) {
+  int r = check_scene(c, scene);
+  if (r) return r;
+  if (!x) return BRMPPI_ERR_NULL;
+  if (!(c->p.flags & BRMPPI_FLAG_MPCC)) return BRMPPI_ERR_INVALID_ARG;
+  if (!c->goal_set[scene]) return BRMPPI_ERR_NOT_READY;          // the path comes first: psi is checked against it
+  if (!finite_all(x, 7) || !std::isfinite(psi)) return BRMPPI_ERR_NONFINITE_INPUT;
+  if (psi < 0.f || psi > c->path_len[scene]) return BRMPPI_ERR_INVALID_ARG;
+  if (x[6] < c->p.delta_min || x[6] > c->p.delta_max) return BRMPPI_ERR_INVALID_ARG;
+  const float v[8] = {x[0], x[1], x[2], x[3], wrap_pi(x[4]), wrap_pi(x[5]), x[6], psi};
+  CU(cudaMemcpyAsync(c->d.state7 + 8 * scene, v, sizeof(v), cudaMemcpyHostToDevice, c->stream));
+  CU(cudaStreamSynchronize(c->stream));     // v is a stack buffer
+  c->state_set[scene] = 1;
+  return BRMPPI_OK;
+}
+
+int brmppi_set_reference_path(brmppi_ctx* c, int scene, int M, float dpsi, const float* coef) {
+  int r = check_scene(c, scene);
+  if (r) return r;
+  if (!coef) return BRMPPI_ERR_NULL;
+  if (!(c->p.flags & BRMPPI_FLAG_MPCC)) return BRMPPI_ERR_INVALID_ARG;
+  if (M < 1 || M > c->p.max_path_segments) return BRMPPI_ERR_INVALID_ARG;
+  if (!std::isfinite(dpsi) || !finite_all(coef, 16 * M)) return BRMPPI_ERR_NONFINITE_INPUT;
+  if (!(dpsi > 0.f)) return BRMPPI_ERR_INVALID_ARG;
+  CU(cudaMemcpyAsync(c->d.path_coef + (size_t)scene * c->p.max_path_segments * 16, coef, sizeof(float) * 16 * (size_t)M,
+                     cudaMemcpyHostToDevice, c->stream));
+  CU(cudaMemcpyAsync(c->d.path_M + scene, &M, sizeof(int), cudaMemcpyHostToDevice, c->stream));
+  CU(cudaMemcpyAsync(c->d.path_dpsi + scene, &dpsi, sizeof(float), cudaMemcpyHostToDevice, c->stream));
+  CU(cudaStreamSynchronize(c->stream));     // M and dpsi are stack values
+  c->path_len[scene] = (float)M * dpsi;
+  c->goal_set[scene] = 1;                   // the path stands where the goal does on the other paths
+  c->state_set[scene] = 0;                  // psi has to be given again against the new path
+  return BRMPPI_OK;
+}
+
 int brmppi_set_goal(brmppi_ctx* c, int scene, const float g[4]) {
   int r = check_scene(c, scene);
   if (r) return r;
   if (!g) return BRMPPI_ERR_NULL;
+  if (c->p.flags & BRMPPI_FLAG_MPCC) return BRMPPI_ERR_INVALID_ARG;
   if (!finite_all(g, 4)) return BRMPPI_ERR_NONFINITE_INPUT;
   CU(cudaMemcpyAsync(c->d.goal + 4 * scene, g, 16, cudaMemcpyHostToDevice, c->stream));
   c->goal_set[scene] = 1;
@@ -474,9 +554,9 @@ int brmppi_set_nominal(brmppi_ctx* c, int scene, const float* U) {
   const size_t bytes = sizeof(float) * 2 * (size_t)c->p.T;
   if (!U) { CU(cudaMemsetAsync(dst, 0, bytes, c->stream)); return BRMPPI_OK; }
   if (!finite_all(U, 2 * c->p.T)) return BRMPPI_ERR_NONFINITE_INPUT;
-  for (int t = 0; t < c->p.T; ++t) {
-    if (U[2 * t] < c->p.v_min || U[2 * t] > c->p.v_max) return BRMPPI_ERR_INVALID_ARG;
-    if (U[2 * t + 1] < c->p.delta_min || U[2 * t + 1] > c->p.delta_max) return BRMPPI_ERR_INVALID_ARG;
+  for (int t = 0; t < c->p.T; ++t) {    // c->d holds the box of the mode's controls: (v, delta) or (j, omega)
+    if (U[2 * t] < c->d.v_min || U[2 * t] > c->d.v_max) return BRMPPI_ERR_INVALID_ARG;
+    if (U[2 * t + 1] < c->d.delta_min || U[2 * t + 1] > c->d.delta_max) return BRMPPI_ERR_INVALID_ARG;
   }
   CU(cudaMemcpyAsync(dst, U, bytes, cudaMemcpyHostToDevice, c->stream));
   return BRMPPI_OK;
@@ -594,7 +674,16 @@ int brmppi_get_state(brmppi_ctx* c, int scene, float x_out[4]) {
   int r = check_scene(c, scene);
   if (r) return r;
   if (!x_out) return BRMPPI_ERR_NULL;
+  if (c->p.flags & BRMPPI_FLAG_MPCC) return BRMPPI_ERR_INVALID_ARG;
   return d2h(c, x_out, c->d.state + 4 * scene, 16);
+}
+
+int brmppi_get_state7(brmppi_ctx* c, int scene, float x_out[8]) {
+  int r = check_scene(c, scene);
+  if (r) return r;
+  if (!x_out) return BRMPPI_ERR_NULL;
+  if (!(c->p.flags & BRMPPI_FLAG_MPCC)) return BRMPPI_ERR_INVALID_ARG;
+  return d2h(c, x_out, c->d.state7 + 8 * scene, 32);
 }
 
 int brmppi_get_obstacles(brmppi_ctx* c, int scene, int* n_out, brmppi_obstacle* out) {
@@ -637,7 +726,17 @@ int brmppi_get_final_states(brmppi_ctx* c, int scene, float* X_out) {
   if (r) return r;
   if (!X_out) return BRMPPI_ERR_NULL;
   if (!(c->p.flags & BRMPPI_FLAG_WRITE_SAMPLES)) return BRMPPI_ERR_NOT_READY;
+  if (c->p.flags & BRMPPI_FLAG_MPCC) return BRMPPI_ERR_INVALID_ARG;
   return d2h(c, X_out, c->d.XT + (size_t)scene * c->p.K * 4, sizeof(float) * 4 * (size_t)c->p.K);
+}
+
+int brmppi_get_final_states7(brmppi_ctx* c, int scene, float* X_out) {
+  int r = check_scene(c, scene);
+  if (r) return r;
+  if (!X_out) return BRMPPI_ERR_NULL;
+  if (!(c->p.flags & BRMPPI_FLAG_WRITE_SAMPLES)) return BRMPPI_ERR_NOT_READY;
+  if (!(c->p.flags & BRMPPI_FLAG_MPCC)) return BRMPPI_ERR_INVALID_ARG;
+  return d2h(c, X_out, c->d.XT + (size_t)scene * c->p.K * 8, sizeof(float) * 8 * (size_t)c->p.K);
 }
 
 int brmppi_get_diag(brmppi_ctx* c, int scene, brmppi_diag* out) {
@@ -778,6 +877,10 @@ int brmppi_debug_sample_controls(void* cuda_stream, const brmppi_params* p, unsi
   d.K = p->K; d.T = p->T;
   d.v_min = p->v_min; d.v_max = p->v_max; d.delta_min = p->delta_min; d.delta_max = p->delta_max;
   d.sigma_v = p->sigma_v; d.sigma_delta = p->sigma_delta;
+  if (p->flags & BRMPPI_FLAG_MPCC) {
+    d.v_min = p->j_min; d.v_max = p->j_max; d.delta_min = p->omega_min; d.delta_max = p->omega_max;
+    d.sigma_v = p->sigma_j; d.sigma_delta = p->sigma_omega;
+  }
   d.alpha_lo = p->alpha_lo; d.alpha_span = p->alpha_hi - p->alpha_lo;
   d.key0 = (uint32_t)(p->seed & 0xFFFFFFFFull); d.key1 = (uint32_t)(p->seed >> 32);
   const size_t total = (size_t)p->K * p->T;

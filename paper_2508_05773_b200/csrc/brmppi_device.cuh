@@ -35,6 +35,10 @@ struct DeviceParams {
   int hitch_filter;            // 1: shift_plant passes U[0] through the CBF-QP of Sec. V-D
   float hitch_alpha, hitch_qv, hitch_qdelta;
   float proj_qv, proj_qomega, proj_qalpha, proj_rho, sigma_ualpha, ualpha_max, w_alpha, h_buffer;   // BRMPPI_FLAG_PROJECTED
+  // BRMPPI_FLAG_MPCC: in this mode v_min .. sigma_delta above hold the (j, omega) box and sigmas
+  float dstate_lo, dstate_hi;  // clamp of the steering STATE delta
+  float Qc, Ql, Qth1, Qth2, Rj, Rw, mu, nu_bar;
+  int max_path_segments;
   uint32_t key0, key1;        // Philox key of scene 0 = (lo32(seed), hi32(seed)); scene s adds s
   uint32_t flags;
   // tiling of the sample axis
@@ -63,6 +67,10 @@ struct DeviceParams {
   uint32_t* counter;          // global iteration counter n
   float* u0_applied;          // [n_scenes][2]  control applied by the last plant step
   float* u0_host;             // the same, in page-locked HOST memory the device writes directly (brmppi_step's result)
+  float* state7;              // [n_scenes][8]  (p_x, p_y, v, a, theta1, theta2, delta, psi)  (FLAG_MPCC)
+  int* path_M;                // [n_scenes]     cubic segments of the reference path
+  float* path_dpsi;           // [n_scenes]     knot spacing
+  float* path_coef;           // [n_scenes][max_path_segments][4][4]
   float* hitch_ref;           // [n_scenes][4]  (v_ref, delta_ref, status as int bits, 0) of the last plant step
   double* part_m;             // [n_scenes][P]  block minimum of S (fp64)
   int* part_argmin;           // [n_scenes][P]
@@ -72,7 +80,7 @@ struct DeviceParams {
   float* part_A;              // [n_scenes][2T][P]  weighted control sums, output-major
   brmppi_diag* diag;          // [n_scenes]
   float* S;                   // [n_scenes][K]     (FLAG_WRITE_SAMPLES)
-  float* XT;                  // [n_scenes][K][4]  (FLAG_WRITE_SAMPLES)
+  float* XT;                  // [n_scenes][K][4]  (FLAG_WRITE_SAMPLES); [K][8] with FLAG_MPCC
   unsigned long long* phase_ns;   // [grid][8] per-CTA phase nanoseconds (FLAG_PHASE_TIMING), else null
 };
 

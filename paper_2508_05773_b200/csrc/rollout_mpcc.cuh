@@ -1,0 +1,195 @@
+// rollout_mpcc.cuh -- the paper's own model and tracking cost (BRMPPI_FLAG_MPCC):
+// 7-state jerk / steering-rate model, eq. (6), barrier-rate hinge on the second-order Taylor
+// predictor (17), contouring / lag / heading / effort / progress cost (13)-(15)
+// along a cubic-spline reference path in arc length.  Readings: DESIGN.md reading 31.
+//
+// One thread per sample (the whole step is a serial chain: the predictor and the path parameter depend on the
+// state), everything in registers; the obstacle table, the nominal and the path's coefficient table sit in
+// shared memory.  In this mode DeviceParams' control box (v_min .. delta_max, sigma_v, sigma_delta) holds the
+// (jerk, steering-rate) box and sigmas, so the sampler and the thread-per-sample epilogue are the penalty path's.
+#pragma once
+
+#include "rollout_thread.cuh"
+
+namespace brmppi {
+
+struct State7 { float x, y, v, a, t1, t2, de, psi; };
+
+// (p^{x,r}, p^{y,r}, theta^{1,r}, theta^{2,r}) at arc length psi from the table [M][4][4] in shared memory.
+__device__ __forceinline__ float4 path_eval(const float4* __restrict__ sPath, int M, float dpsi, float inv_dpsi,
+                                            float psi) {
+  int m = (int)floorf(psi * inv_dpsi);
+  m = m > M - 1 ? M - 1 : (m < 0 ? 0 : m);
+  const float s = psi - (float)m * dpsi;
+  const float4* q = sPath + 4 * m;
+  float r[4];
+#pragma unroll
+  for (int c = 0; c < 4; ++c) {
+    const float4 k = q[c];
+    r[c] = fmaf(s, fmaf(s, fmaf(s, k.w, k.z), k.y), k.x);
+  }
+  return make_float4(r[0], r[1], r[2], r[3]);
+}
+
+// Q_c e_c^2 + Q_l e_l^2 + Q_th1 e_th1^2 + Q_th2 e_th2^2 at (X, psi); *nu = v cos(theta1 - theta^{1,r}).
+template <bool PRECISE>
+__device__ __forceinline__ float mpcc_tracking(const DeviceParams& P, const State7& X, const float4 r, float* nu) {
+  float sr, cr;
+  sincos_t<PRECISE>(r.z, &sr, &cr);
+  const float dx = X.x - r.x, dy = X.y - r.y;
+  const float ec = fmaf(sr, dx, -cr * dy);                       // (14)
+  const float el = -fmaf(cr, dx, sr * dy);                       // (15)
+  const float e1 = wrap_angle(X.t1 - r.z), e2 = wrap_angle(X.t2 - r.w);
+  float s1, c1;
+  sincos_t<PRECISE>(X.t1, &s1, &c1);
+  *nu = X.v * fmaf(c1, cr, s1 * sr);                             // v cos(theta1 - theta1r)
+  return fmaf(P.Qc * ec, ec, fmaf(P.Ql * el, el, fmaf(P.Qth1 * e1, e1, P.Qth2 * e2 * e2)));
+}
+
+template <bool PRECISE>
+__global__ void __launch_bounds__(kThreadBlock)
+rollout_mpcc(const __grid_constant__ DeviceParams P) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  // layout: obs[max_obs] float4 (ox, oy, 1/rho^2, -) | vel[max_obs] float4 (dt vx, dt vy, vx, vy) |
+  //         path[M_max][4] float4 | U_nom[T] float2 | red (4 double, 4 int, 12 float) | A_w[4][2T] float
+  const int T = P.T;
+  float4* sObs = reinterpret_cast<float4*>(smem_raw);
+  float4* sVel = sObs + P.max_obstacles;
+  float4* sPath = sVel + P.max_obstacles;
+  float2* sU = reinterpret_cast<float2*>(sPath + 4 * P.max_path_segments);
+  double* sRedM = reinterpret_cast<double*>(sU + T + (T & 1));
+  int* sRedI = reinterpret_cast<int*>(sRedM + 4);
+  float* sRedF = reinterpret_cast<float*>(sRedI + 4);
+  float* sA = sRedF + 12;
+
+  const int scene = blockIdx.y;
+  const int tid = threadIdx.x;
+  const int k = blockIdx.x * kThreadBlock + tid;
+  const bool valid = k < P.K;
+  const uint32_t n = *P.counter;
+  const uint32_t key0 = P.key0 + (uint32_t)scene;
+  const uint32_t key1 = P.key1 + (key0 < P.key0 ? 1u : 0u);
+
+  const float* s7 = P.state7 + 8 * scene;                         // px, py, v, a, theta1, theta2, delta, psi
+  const float x0 = s7[0], y0 = s7[1];
+  const int n_obs = P.n_obs[scene];
+  const int M = P.path_M[scene];
+  const float dpsi = P.path_dpsi[scene];
+  for (int i = tid; i < T; i += kThreadBlock)
+    sU[i] = reinterpret_cast<const float2*>(P.U)[scene * T + i];
+  for (int i = tid; i < n_obs; i += kThreadBlock) {
+    const float* ob = P.obstacles + ((size_t)scene * P.max_obstacles + i) * 5;
+    const float rho = ob[2] + P.disc_radius;
+    sObs[i] = make_float4(ob[0] - x0, ob[1] - y0, 1.0f / (rho * rho), 0.0f);   // vehicle-centred frame
+    sVel[i] = make_float4(P.dt * ob[3], P.dt * ob[4], ob[3], ob[4]);
+  }
+  for (int i = tid; i < 4 * M; i += kThreadBlock) {
+    float4 c = reinterpret_cast<const float4*>(P.path_coef)[(size_t)scene * 4 * P.max_path_segments + i];
+    const int comp = i & 3;
+    if (comp == 0) c.x -= x0;
+    if (comp == 1) c.x -= y0;
+    sPath[i] = c;
+  }
+  __syncthreads();
+
+  double S = CUDART_INF;
+  if (valid) {
+    const float inv_dpsi = 1.0f / dpsi, Lpath = (float)M * dpsi;
+    const float alpha = sample_alpha(P, n, (uint32_t)(k + P.k_offset), key0, key1);
+    const float half_dt2 = 0.5f * P.dt * P.dt;
+    State7 X{0.0f, 0.0f, s7[2], s7[3], s7[4], s7[5], s7[6], s7[7]};
+    double cost = 0.0;
+#pragma unroll 1
+    for (int t = 0; t < T; ++t) {
+      const float2 u = sample_control<PRECISE>(P, sU[t], (uint32_t)t, n, (uint32_t)(k + P.k_offset), key0, key1);   // (j, omega)
+      float s1, c1, s2, c2;
+      sincos_t<PRECISE>(X.t1, &s1, &c1);
+      sincos_t<PRECISE>(X.t2, &s2, &c2);
+      const float td = tan_t<PRECISE>(X.de), sec2 = fmaf(td, td, 1.0f);
+      const float sb = s1 * c2 - c1 * s2, cb = fmaf(c1, c2, s1 * s2);
+      // heading rates of the continuous model and their time derivatives under the sampled input
+      const float W1 = X.v * P.inv_L1 * td;
+      const float gb = fmaf(-P.Lh_over_L1 * cb, td, sb);                       // sin b - k cos b tan(delta)
+      const float W2 = X.v * P.inv_L2 * gb;
+      const float bdot = W1 - W2;
+      const float W1dot = P.inv_L1 * fmaf(X.a, td, X.v * sec2 * u.y);
+      const float gbdot = fmaf(bdot, fmaf(P.Lh_over_L1 * sb, td, cb), -P.Lh_over_L1 * cb * sec2 * u.y);
+      const float W2dot = P.inv_L2 * fmaf(X.a, gb, X.v * gbdot);
+      // barrier-rate hinge with the predictor (17): (1 - alpha) h - hhat = -(alpha h + Ts hdot + Ts^2/2 hddot)
+      float pen = 0.0f;
+      {
+        float cx[kMaxDiscs], cy[kMaxDiscs], vx[kMaxDiscs], vy[kMaxDiscs], ax[kMaxDiscs], ay[kMaxDiscs];
+#pragma unroll
+        for (int j = 0; j < kMaxDiscs; ++j) {
+          const float l1 = P.disc_a1[j] - P.Lh, l2 = P.disc_a2[j];              // lever arms on the two headings
+          cx[j] = fmaf(l1, c1, fmaf(l2, c2, X.x));
+          cy[j] = fmaf(l1, s1, fmaf(l2, s2, X.y));
+          vx[j] = fmaf(X.v, c1, fmaf(-l1 * W1, s1, -l2 * W2 * s2));
+          vy[j] = fmaf(X.v, s1, fmaf(l1 * W1, c1, l2 * W2 * c2));
+          // a e1 + v W1 n1 + l1 (W1dot n1 - W1^2 e1) + l2 (W2dot n2 - W2^2 e2)
+          const float q1 = fmaf(X.v, W1, l1 * W1dot), r1 = fmaf(-l1 * W1, W1, X.a);
+          ax[j] = fmaf(r1, c1, fmaf(-q1, s1, l2 * fmaf(-W2dot, s2, -W2 * W2 * c2)));
+          ay[j] = fmaf(r1, s1, fmaf(q1, c1, l2 * fmaf(W2dot, c2, -W2 * W2 * s2)));
+        }
+        const float tf = (float)t;
+        for (int i = 0; i < n_obs; ++i) {
+          const float4 o = sObs[i];
+          const float4 w = sVel[i];
+          const float ox = fmaf(tf, w.x, o.x), oy = fmaf(tf, w.y, o.y);
+#pragma unroll
+          for (int j = 0; j < kMaxDiscs; ++j) {
+            if (j < P.n_discs) {
+              const float dx = cx[j] - ox, dy = cy[j] - oy, ex = vx[j] - w.z, ey = vy[j] - w.w;
+              const float h = fmaf(fmaf(dx, dx, dy * dy), o.z, -1.0f);
+              const float hd = 2.0f * o.z * fmaf(dx, ex, dy * ey);
+              const float hdd = 2.0f * o.z * (fmaf(ex, ex, ey * ey) + fmaf(dx, ax[j], dy * ay[j]));
+              pen += fmaxf(-fmaf(alpha, h, fmaf(P.dt, hd, half_dt2 * hdd)), 0.0f);
+            }
+          }
+        }
+      }
+      // eq. (6), every right-hand side at step k; path parameter by the projection velocity
+      float nu;
+      {
+        const float4 r = path_eval(sPath, M, dpsi, inv_dpsi, X.psi);
+        float sr, cr;
+        sincos_t<PRECISE>(r.z, &sr, &cr);
+        nu = X.v * fmaf(c1, cr, s1 * sr);
+      }
+      State7 N;
+      N.x = fmaf(P.dt * X.v, c1, X.x);
+      N.y = fmaf(P.dt * X.v, s1, X.y);
+      N.v = fmaf(P.dt, X.a, X.v);
+      N.a = fmaf(P.dt, u.x, X.a);
+      N.t1 = fmaf(P.dt, W1, X.t1);
+      N.t2 = fmaf(P.dt, W2, X.t2);
+      N.de = fminf(fmaxf(fmaf(P.dt, u.y, X.de), P.dstate_lo), P.dstate_hi);
+      N.psi = fminf(fmaxf(fmaf(P.dt, nu, X.psi), 0.0f), Lpath);
+      X = N;
+      // stage cost (13) on (x_{k+1}, u_k, psi_{k+1})
+      float nu1;
+      const float track = mpcc_tracking<PRECISE>(P, X, path_eval(sPath, M, dpsi, inv_dpsi, X.psi), &nu1);
+      const float dn = P.nu_bar - nu1;
+      const float hl = fmaxf(fabsf(wrap_angle(X.t1 - X.t2)) - fmaf(-P.hitch_kappa, fabsf(X.v), P.hitch_max), 0.0f);
+      const float stage = track + fmaf(P.Rj * u.x, u.x, P.Rw * u.y * u.y) + P.mu * dn * dn + P.w_hitch * hl * hl;
+      cost += (double)stage + (double)P.w_bar * (double)pen;
+    }
+    float nuT;
+    S = cost + (double)(P.w_term * mpcc_tracking<PRECISE>(P, X, path_eval(sPath, M, dpsi, inv_dpsi, X.psi), &nuT));
+    if (P.flags & BRMPPI_FLAG_WRITE_SAMPLES) {
+      P.S[(size_t)scene * P.K + k] = (float)S;
+      float4* out = reinterpret_cast<float4*>(P.XT) + 2 * ((size_t)scene * P.K + k);
+      out[0] = make_float4(X.x + x0, X.y + y0, X.v, X.a);
+      out[1] = make_float4(X.t1, X.t2, X.de, X.psi);
+    }
+  }
+  thread_kernel_epilogue<PRECISE>(P, sU, sRedM, sRedI, sRedF, sA, S, valid, k, scene, n, key0, key1);
+}
+
+inline size_t rollout_mpcc_smem_bytes(const DeviceParams& P) {
+  return sizeof(float4) * 2 * (size_t)P.max_obstacles + sizeof(float4) * 4 * (size_t)P.max_path_segments +
+         sizeof(float2) * (size_t)(P.T + (P.T & 1)) + sizeof(double) * 4 + sizeof(int) * 4 + sizeof(float) * 12 +
+         sizeof(float) * 4 * 2 * (size_t)P.T;
+}
+
+}  // namespace brmppi

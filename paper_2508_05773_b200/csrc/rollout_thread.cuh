@@ -83,7 +83,7 @@ rollout_thread_per_sample(const __grid_constant__ DeviceParams P) {
   float* sA = sRedF + 12;                                              // [4][2T]
 
   const int scene = blockIdx.y;
-  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int tid = threadIdx.x;
   const int k = blockIdx.x * kThreadBlock + tid;
   const bool valid = k < P.K;
   const uint32_t n = *P.counter;

@@ -142,7 +142,32 @@ __global__ void __launch_bounds__(kShiftBlock) shift_plant(const __grid_constant
   const int scene = blockIdx.x, tid = threadIdx.x, T = P.T;
   float2* U = reinterpret_cast<float2*>(P.U) + (size_t)scene * T;
   if (PLANT) {
-    if (tid == 0) {
+    if (tid == 0 && (P.flags & BRMPPI_FLAG_MPCC)) {
+      // eq. (6) under u = (j, omega) = U[0], the path parameter by the projection velocity (reading 31)
+      const float2 u0 = U[0];
+      float* x = P.state7 + 8 * scene;
+      const float v = x[2], a = x[3], t1 = x[4], t2 = x[5], de = x[6], psi = x[7];
+      const int M = P.path_M[scene];
+      const float dpsi = P.path_dpsi[scene];
+      int m = (int)floorf(psi / dpsi);
+      m = m > M - 1 ? M - 1 : (m < 0 ? 0 : m);
+      const float s = psi - (float)m * dpsi;
+      const float* q = P.path_coef + ((size_t)scene * P.max_path_segments + m) * 16 + 8;   // theta^{1,r}
+      const float th1r = fmaf(s, fmaf(s, fmaf(s, q[3], q[2]), q[1]), q[0]);
+      float s1, c1;
+      sincosf(t1, &s1, &c1);
+      const float td = tanf(de), b = t1 - t2;
+      x[0] = fmaf(P.dt * v, c1, x[0]);
+      x[1] = fmaf(P.dt * v, s1, x[1]);
+      x[2] = fmaf(P.dt, a, v);
+      x[3] = fmaf(P.dt, u0.x, a);
+      x[4] = wrap_angle(fmaf(P.dt * v * P.inv_L1, td, t1));
+      x[5] = wrap_angle(fmaf(P.dt * v * P.inv_L2, fmaf(-P.Lh_over_L1 * td, cosf(b), sinf(b)), t2));
+      x[6] = fminf(fmaxf(fmaf(P.dt, u0.y, de), P.dstate_lo), P.dstate_hi);
+      x[7] = fminf(fmaxf(fmaf(P.dt, v * cosf(t1 - th1r), psi), 0.0f), (float)M * dpsi);
+      reinterpret_cast<float2*>(P.u0_applied)[scene] = u0;
+      if (P.u0_host != nullptr) reinterpret_cast<float2*>(P.u0_host)[scene] = u0;
+    } else if (tid == 0) {
       const float2 u_ref = U[0];
       float4 x = reinterpret_cast<float4*>(P.state)[scene];
       float2 u0 = u_ref;
