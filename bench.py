@@ -57,19 +57,29 @@ def workload(name, rank=0):
     elif name == "paperproj":     # the paper's own size: 5000 rollouts x H = 120 (T_s = 0.04 s) x 8 obstacles
         sc = scenes.scene_cfg2(rank)
         sc.params = sc.params.with_(K=5000, T=120, dt=0.04, n_iter=1)
+    elif name == "cfg2mpcc":      # CFG2's size on the paper's own model and cost: 7 states, predictor (17), cost (13)
+        sc = scenes.scene_mpcc(rank, K=16384, T=80, dt=0.05, n_obs=8, M=24)
+        sc.params = sc.params.with_(n_iter=3)
+    elif name == "papermpcc":     # the paper's own size on the paper's own model
+        sc = scenes.scene_mpcc(rank, K=5000, T=120, dt=0.04, n_obs=8, M=24)
     else:
         raise SystemExit(f"unknown workload {name}")
     return sc, sc.params
 
 
 PROJECTED = ("cfg2proj", "paperproj")
+MPCC = ("cfg2mpcc", "papermpcc")
+THREAD_PER_SAMPLE = PROJECTED + MPCC          # workloads whose rollout is a one-thread-per-sample kernel (no culling)
 
 
 def solver_flags(B, name, no_cull=False):
-    return (B.FLAG_PROJECTED if name in PROJECTED else 0) | (B.FLAG_NO_CULL if no_cull else 0)
+    return ((B.FLAG_PROJECTED if name in PROJECTED else 0) | (B.FLAG_MPCC if name in MPCC else 0) |
+            (B.FLAG_NO_CULL if no_cull else 0))
 
 
 def oracle_solve(O, name, ps, n0, sc, U, n_threads):
+    if name in MPCC:
+        return O.solve7(ps, sc.coef, sc.dpsi, n0, sc.x0, sc.psi0, sc.obstacles, U, n_threads=n_threads)
     if name in PROJECTED:
         return O.solve_projected(ps, n0, sc.x0, sc.goal, sc.obstacles, U, n_threads=n_threads)
     return O.solve(ps, n0, sc.x0, sc.goal, sc.obstacles, U, n_threads=n_threads, superellipses=sc.superellipses)
@@ -85,6 +95,16 @@ def projected_instr_per_sample_step(n_obs, n_discs):
     chol = N * (N - 1) // 2 + sum((N - 1 - c) * (c + 1) for c in range(N)) + 3 * N
     proj = 14 + 4 * N + N * (N + 1) + chol + (N * (N - 1) + 2 * N) + (4 * N + 2) + 3 * N
     return 150 + 64 * ((N + 3) // 4) + N * (16 + 10 * n_discs) + proj
+
+
+def mpcc_instr_per_sample_step(n_obs, n_discs):
+    """issue slots of one sample-step of the paper's own model and cost.  Fixed 176: noise, perturb
+    and clamp 60 (as on the penalty path); sin / cos of the two headings, tan and sec^2 of delta 11; sin / cos of the
+    hitch angle 4; W1, W2 and their time derivatives 20; Euler step (6) 12; path segment and four cubics 19;
+    tracking errors (14), (15), heading wraps, nu 26; progress, effort, hitch hinge, psi update, accumulate, loop 24.
+    Per disc 26: centre 4, velocity 8, acceleration 14.  Per obstacle 3 (position, 2 / rho^2); per (obstacle, disc)
+    21: differences 4, h 3, hdot 3, hddot 6, predictor and hinge 5."""
+    return 176 + 26 * n_discs + n_obs * (3 + 21 * n_discs)
 
 
 def algorithmic_instr_per_sample_step(n_obs, n_discs, superellipses=None, philox_per_step=1.0):
@@ -237,10 +257,12 @@ def workload_config(name, sc, p, n_scenes_total):
     label = {"cfg2se": "BASELINE.json configs[2] with the paper's super-ellipse obstacles, eq. (16) (cfg2se)",
              "cfg2proj": "BASELINE.json configs[2] solved by BR-MPPI proper: projection (9)-(12) inside the rollout (cfg2proj)",
              "paperproj": "the paper's size, 5000 rollouts x H = 120 x 8 obstacles (PAPER.md:243), projected rollout of the reduced model (paperproj)",
+             "cfg2mpcc": "BASELINE.json configs[2]'s size on the paper's own 7-state model, predictor (17) and contouring cost (13) (cfg2mpcc)",
+             "papermpcc": "the paper's size, 5000 rollouts x H = 120 x 8 obstacles (PAPER.md:243), on the paper's own 7-state model and contouring cost (papermpcc)",
              }.get(name, f"BASELINE.json configs[{name[-1]}] ({name})")
     return {"workload": label, "K": p.K, "T": p.T,
             "n_obstacles": int(len(sc.obstacles)),
-            "n_superellipses": 0 if sc.superellipses is None else int(len(sc.superellipses)),
+            "n_superellipses": 0 if getattr(sc, "superellipses", None) is None else int(len(sc.superellipses)),
             "n_moving": int(np.count_nonzero(np.abs(sc.obstacles[:, 3:5]).sum(axis=1))) if len(sc.obstacles) else 0,
             "n_discs": len(p.discs), "n_iter": p.n_iter, "dt": p.dt, "scenes_total": n_scenes_total,
             "l2": "flushed between timed steps (256 MiB write); per-step CUDA-event pairs",
@@ -253,8 +275,11 @@ def measure(B, torch, name, rank, steps, warmup, dist, dev, local_rank, closed_l
     kernel times by CUDA events (with and without culling)."""
     sc, p = workload(name, rank)
     n_obs = len(sc.obstacles)
-    n_se = 0 if sc.superellipses is None else len(sc.superellipses)
-    solver = B.Solver(p, 1, max(n_obs, 1), solver_flags(B, name), device=dev, max_superellipses=n_se)
+    se = getattr(sc, "superellipses", None)
+    n_se = 0 if se is None else len(se)
+    n_seg = sc.coef.shape[0] if name in MPCC else 1
+    solver = B.Solver(p, 1, max(n_obs, 1), solver_flags(B, name), device=dev, max_superellipses=n_se,
+                      max_path_segments=n_seg)
     solver.set_scene(sc)
     stream = solver.stream
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
@@ -288,10 +313,14 @@ def measure(B, torch, name, rank, steps, warmup, dist, dev, local_rank, closed_l
 
     # ---- end to end through the C ABI with host buffers (pinned), host clock
     pin = lambda a: torch.from_numpy(np.ascontiguousarray(a, dtype=np.float32)).pin_memory().numpy()
-    hx, hg, ho = pin(sc.x0), pin(sc.goal), pin(sc.obstacles)
-    hs = None if n_se == 0 else sc.superellipses
+    hx, ho = pin(sc.x0), pin(sc.obstacles)
+    hg = pin(sc.coef) if name in MPCC else pin(sc.goal)
+    hs = None if n_se == 0 else se
 
     def set_inputs():
+        if name in MPCC:
+            solver.set_reference_path(hg, sc.dpsi); solver.set_state7(hx, sc.psi0); solver.set_obstacles(ho)
+            return
         solver.set_state(hx); solver.set_goal(hg); solver.set_obstacles(ho)
         if hs is not None:
             solver.set_superellipses(hs)
@@ -306,6 +335,8 @@ def measure(B, torch, name, rank, steps, warmup, dist, dev, local_rank, closed_l
     barrier()
     e2e_s_max = max_over_ranks(time.perf_counter() - t0, dist, dev)
     h2d = 16 + 16 + 20 * n_obs + 4 + (32 * n_se + 4 if n_se else 0)
+    if name in MPCC:                                         # state and psi, path table with M and dpsi, obstacles
+        h2d = 32 + (64 * n_seg + 8) + 20 * n_obs + 4
     d2h = 8 * p.T
 
     # ---- closed-loop control rate (CUDA-graph replay of solve + plant step + shift)
@@ -326,7 +357,7 @@ def measure(B, torch, name, rank, steps, warmup, dist, dev, local_rank, closed_l
         solver.set_nominal(None)
         ms_roll, ms_upd = solver.time_kernels(50)
         ms_nocull = None
-        if name not in PROJECTED:                            # the same launch with every (obstacle, disc, step) evaluated
+        if name not in THREAD_PER_SAMPLE:                    # the same launch with every (obstacle, disc, step) evaluated
             s2 = B.Solver(p, 1, max(n_obs, 1), solver_flags(B, name, no_cull=True), device=dev, max_superellipses=n_se)
             s2.set_scene(sc)
             for _ in range(3):
@@ -340,15 +371,18 @@ def measure(B, torch, name, rank, steps, warmup, dist, dev, local_rank, closed_l
         if name in PROJECTED:
             instr = projected_instr_per_sample_step(n_obs, len(p.discs))
             instr_pair = instr
+        elif name in MPCC:
+            instr = mpcc_instr_per_sample_step(n_obs, len(p.discs))
+            instr_pair = instr - 20
         else:
-            instr = algorithmic_instr_per_sample_step(n_obs, len(p.discs), sc.superellipses)
-            instr_pair = algorithmic_instr_per_sample_step(n_obs, len(p.discs), sc.superellipses, philox_per_step=0.5)
+            instr = algorithmic_instr_per_sample_step(n_obs, len(p.discs), se)
+            instr_pair = algorithmic_instr_per_sample_step(n_obs, len(p.discs), se, philox_per_step=0.5)
         achieved = p.K * p.T * instr / (ms_roll * 1e-3) / 1e9          # G thread-instr / s
         traffic, traffic_source = dram_traffic_from_profile()
         roof = {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "Ginstr/s (thread-instructions)",
                 "frac": achieved / peak, "traffic": traffic if name == "cfg2" else None,
                 "traffic_source": traffic_source if name == "cfg2" else None,
-                "kernel": "rollout_projected" if name in PROJECTED else "rollout_cta",
+                "kernel": "rollout_projected" if name in PROJECTED else "rollout_mpcc" if name in MPCC else "rollout_cta",
                 "kernel_ms": ms_roll, "update_kernel_ms": ms_upd,
                 "kernel_share_of_step": ms_roll * p.n_iter / (dev_s / steps * 1e3),
                 "algorithmic_instr_per_sample_step": instr,
@@ -418,9 +452,9 @@ def run_ours(args):
     # the other BASELINE.json configs, the 64-scene batch and the projected rollout: N = 1 only, shorter runs
     others = []
     if world == 1 and not args.no_others:
-        for name in ("cfg0", "cfg1", "cfg2", "cfg3", "cfg2se", "cfg2proj", "paperproj"):
+        for name in ("cfg0", "cfg1", "cfg2", "cfg3", "cfg2se", "cfg2proj", "paperproj", "cfg2mpcc", "papermpcc"):
             if name != args.workload:
-                steps_o = 20 if name in PROJECTED else 50
+                steps_o = 20 if name in THREAD_PER_SAMPLE else 50
                 others.append(record(name, measure(B, torch, name, 0, steps_o, 5, None, dev, local_rank, 100, False), 1))
         others.append(batch64_record(B))
     cores = os.cpu_count() or 1
@@ -442,7 +476,7 @@ def run_ours(args):
                         "what": "brmppi_step: graph replay of solve + plant step + shift, host wall clock"},
         "gpu_launches": m["launches"], "clocks": m["clocks"], "roofline": m["roof"], "cpu_baseline": cpu,
         "wall_s_timed_region": m["wall_s"], "others": others,
-        "paper_context": "paper: 9.9 ms per MPPI step, >100 Hz, 5000 rollouts x H=120, 8 obstacles, JAX on an unnamed GPU (PAPER.md:5,243) -- full formulation (7-state model, contouring cost), context only; the `paperproj` record under `others` is the same size solved by this library's projected rollout of the reduced model",
+        "paper_context": "paper: 9.9 ms per MPPI step, >100 Hz, 5000 rollouts x H=120, 8 obstacles, JAX on an unnamed GPU (PAPER.md:5,243) -- full formulation (7-state model, contouring cost), context only; the `papermpcc` record under `others` is the same size on the same model and cost family (7 states, predictor (17), contouring cost; penalty form of the barrier-rate condition), `paperproj` the same size solved by the projected rollout of the reduced model",
     }
     print(json.dumps(line))
 
@@ -638,7 +672,7 @@ def main():
     ap.add_argument("--steps", type=int, default=200)
     ap.add_argument("--warmup", type=int, default=20)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="cfg2", choices=["cfg0", "cfg1", "cfg2", "cfg2se", "cfg3", "cfg2proj", "paperproj"])
+    ap.add_argument("--workload", default="cfg2", choices=["cfg0", "cfg1", "cfg2", "cfg2se", "cfg3", "cfg2proj", "paperproj", "cfg2mpcc", "papermpcc"])
     ap.add_argument("--no-others", action="store_true", help="skip the secondary workloads of the `others` key")
     ap.add_argument("--phases", action="store_true", help="print the rollout kernel's in-kernel phase times")
     ap.add_argument("--sweep", action="store_true", help="run BASELINE.json configs[4] (sweep + 64-scene batch)")

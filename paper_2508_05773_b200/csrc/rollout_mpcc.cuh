@@ -32,16 +32,16 @@ __device__ __forceinline__ float4 path_eval(const float4* __restrict__ sPath, in
 }
 
 // Q_c e_c^2 + Q_l e_l^2 + Q_th1 e_th1^2 + Q_th2 e_th2^2 at (X, psi); *nu = v cos(theta1 - theta^{1,r}).
+// s1 / c1 = sin / cos(X.t1): the caller needs them for the next step anyway.
 template <bool PRECISE>
-__device__ __forceinline__ float mpcc_tracking(const DeviceParams& P, const State7& X, const float4 r, float* nu) {
+__device__ __forceinline__ float mpcc_tracking(const DeviceParams& P, const State7& X, float s1, float c1,
+                                               const float4 r, float* nu) {
   float sr, cr;
   sincos_t<PRECISE>(r.z, &sr, &cr);
   const float dx = X.x - r.x, dy = X.y - r.y;
   const float ec = fmaf(sr, dx, -cr * dy);                       // (14)
   const float el = -fmaf(cr, dx, sr * dy);                       // (15)
   const float e1 = wrap_angle(X.t1 - r.z), e2 = wrap_angle(X.t2 - r.w);
-  float s1, c1;
-  sincos_t<PRECISE>(X.t1, &s1, &c1);
   *nu = X.v * fmaf(c1, cr, s1 * sr);                             // v cos(theta1 - theta1r)
   return fmaf(P.Qc * ec, ec, fmaf(P.Ql * el, el, fmaf(P.Qth1 * e1, e1, P.Qth2 * e2 * e2)));
 }
@@ -99,11 +99,16 @@ rollout_mpcc(const __grid_constant__ DeviceParams P) {
     const float half_dt2 = 0.5f * P.dt * P.dt;
     State7 X{0.0f, 0.0f, s7[2], s7[3], s7[4], s7[5], s7[6], s7[7]};
     double cost = 0.0;
+    float last_track = 0.0f;
+    // carried from step to step: sin / cos(theta1) and nu = v cos(theta1 - theta^{1,r}(psi)) of the current
+    // state -- the stage cost of step k - 1 evaluates the same path point and the same nu as the progress of step k
+    float s1, c1, nu;
+    sincos_t<PRECISE>(X.t1, &s1, &c1);
+    (void)mpcc_tracking<PRECISE>(P, X, s1, c1, path_eval(sPath, M, dpsi, inv_dpsi, X.psi), &nu);
 #pragma unroll 1
     for (int t = 0; t < T; ++t) {
       const float2 u = sample_control<PRECISE>(P, sU[t], (uint32_t)t, n, (uint32_t)(k + P.k_offset), key0, key1);   // (j, omega)
-      float s1, c1, s2, c2;
-      sincos_t<PRECISE>(X.t1, &s1, &c1);
+      float s2, c2;
       sincos_t<PRECISE>(X.t2, &s2, &c2);
       const float td = tan_t<PRECISE>(X.de), sec2 = fmaf(td, td, 1.0f);
       const float sb = s1 * c2 - c1 * s2, cb = fmaf(c1, c2, s1 * s2);
@@ -149,13 +154,6 @@ rollout_mpcc(const __grid_constant__ DeviceParams P) {
         }
       }
       // eq. (6), every right-hand side at step k; path parameter by the projection velocity
-      float nu;
-      {
-        const float4 r = path_eval(sPath, M, dpsi, inv_dpsi, X.psi);
-        float sr, cr;
-        sincos_t<PRECISE>(r.z, &sr, &cr);
-        nu = X.v * fmaf(c1, cr, s1 * sr);
-      }
       State7 N;
       N.x = fmaf(P.dt * X.v, c1, X.x);
       N.y = fmaf(P.dt * X.v, s1, X.y);
@@ -167,15 +165,16 @@ rollout_mpcc(const __grid_constant__ DeviceParams P) {
       N.psi = fminf(fmaxf(fmaf(P.dt, nu, X.psi), 0.0f), Lpath);
       X = N;
       // stage cost (13) on (x_{k+1}, u_k, psi_{k+1})
-      float nu1;
-      const float track = mpcc_tracking<PRECISE>(P, X, path_eval(sPath, M, dpsi, inv_dpsi, X.psi), &nu1);
-      const float dn = P.nu_bar - nu1;
+      sincos_t<PRECISE>(X.t1, &s1, &c1);
+      const float track = mpcc_tracking<PRECISE>(P, X, s1, c1, path_eval(sPath, M, dpsi, inv_dpsi, X.psi), &nu);
+      last_track = track;
+      const float dn = P.nu_bar - nu;
       const float hl = fmaxf(fabsf(wrap_angle(X.t1 - X.t2)) - fmaf(-P.hitch_kappa, fabsf(X.v), P.hitch_max), 0.0f);
       const float stage = track + fmaf(P.Rj * u.x, u.x, P.Rw * u.y * u.y) + P.mu * dn * dn + P.w_hitch * hl * hl;
       cost += (double)stage + (double)P.w_bar * (double)pen;
     }
-    float nuT;
-    S = cost + (double)(P.w_term * mpcc_tracking<PRECISE>(P, X, path_eval(sPath, M, dpsi, inv_dpsi, X.psi), &nuT));
+    // terminal cost: the tracking terms at (x_N, psi_N), which the last stage cost just evaluated
+    S = cost + (double)(P.w_term * last_track);
     if (P.flags & BRMPPI_FLAG_WRITE_SAMPLES) {
       P.S[(size_t)scene * P.K + k] = (float)S;
       float4* out = reinterpret_cast<float4*>(P.XT) + 2 * ((size_t)scene * P.K + k);
