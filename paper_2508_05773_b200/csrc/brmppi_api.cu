@@ -16,6 +16,7 @@
 #include "rollout_thread.cuh"
 #include "rollout_projected.cuh"
 #include "rollout_mpcc.cuh"
+#include "rollout_mpcc_cta.cuh"
 #include "rollout_cta.cuh"
 #include "rollout_cta_kernel.cuh"
 #include "update.cuh"
@@ -112,8 +113,10 @@ struct Layout {
 // Launch plan: which rollout kernel, how the sample axis is tiled, how many partials.
 struct Plan {
   bool cta_kernel;
+  bool mpcc_cta;          // BRMPPI_FLAG_MPCC without KERNEL_THREAD_PER_SAMPLE: the phase-split kernel of rollout_mpcc_cta.cuh
   int n_partials;
   CtaPlan cta;
+  MpccCtaPlan mpcc;
 };
 
 // SM count of the current device (the persistent kernel launches one CTA per SM); 148 -- a B200 --
@@ -130,9 +133,13 @@ int device_sm_count() {
 Plan make_plan(const brmppi_params& p) {
   Plan pl{};
   pl.cta_kernel = !(p.flags & (BRMPPI_FLAG_KERNEL_THREAD_PER_SAMPLE | BRMPPI_FLAG_PROJECTED | BRMPPI_FLAG_MPCC));
+  pl.mpcc_cta = (p.flags & BRMPPI_FLAG_MPCC) && !(p.flags & BRMPPI_FLAG_KERNEL_THREAD_PER_SAMPLE);
   if (pl.cta_kernel) {
     pl.cta = make_cta_plan(p.K, p.T, p.n_scenes, p.max_obstacles, p.max_superellipses, device_sm_count());
     pl.n_partials = pl.cta.n_partials;
+  } else if (pl.mpcc_cta) {
+    pl.mpcc = make_mpcc_cta_plan(p.K, p.T, p.n_scenes, p.max_obstacles, p.max_path_segments, device_sm_count());
+    pl.n_partials = pl.mpcc.tiles_per_scene;
   } else {
     pl.n_partials = (p.K + kThreadBlock - 1) / kThreadBlock;
   }
@@ -202,6 +209,9 @@ int launch_rollout(brmppi_ctx* c) {
   const bool precise = (c->p.flags & BRMPPI_FLAG_PRECISE_MATH) != 0;
   if (c->plan.cta_kernel) {
     CU(launch_rollout_cta(d, c->plan.cta, precise, c->stream));
+  } else if (c->plan.mpcc_cta) {
+    mpcc_cta_kernel_for(precise, d.n_discs)<<<(unsigned)c->plan.mpcc.grid, kMpccThreads, c->smem_rollout, c->stream>>>(d);
+    CU(cudaGetLastError());
   } else if (c->p.flags & BRMPPI_FLAG_MPCC) {
     dim3 grid((unsigned)c->plan.n_partials, (unsigned)d.n_scenes);
     if (precise)
@@ -368,6 +378,9 @@ int brmppi_create(const brmppi_params* p, void* dev_workspace, size_t workspace_
     d.off_cost = (int)ts.cost; d.off_xy = (int)ts.xy;
     d.off_planes = (int)ts.planes; d.off_misc = (int)ts.misc;
   }
+  if (c->plan.mpcc_cta) {
+    d.S_tile = kMpccTile; d.tiles_per_scene = c->plan.mpcc.tiles_per_scene; d.total_tiles = c->plan.mpcc.total_tiles;
+  }
   unsigned char* base = (unsigned char*)dev_workspace;
   const Layout& L = c->layout;
   d.state = (float*)(base + L.state); d.goal = (float*)(base + L.goal);
@@ -392,6 +405,10 @@ int brmppi_create(const brmppi_params* p, void* dev_workspace, size_t workspace_
   if (c->plan.cta_kernel) {
     c->smem_rollout = c->plan.cta.smem;
     e = configure_rollout_cta((p->flags & BRMPPI_FLAG_PRECISE_MATH) != 0, p->n_discs, c->smem_rollout);
+  } else if (c->plan.mpcc_cta) {
+    c->smem_rollout = c->plan.mpcc.smem;
+    e = cudaFuncSetAttribute(mpcc_cta_kernel_for((p->flags & BRMPPI_FLAG_PRECISE_MATH) != 0, p->n_discs),
+                             cudaFuncAttributeMaxDynamicSharedMemorySize, (int)prop.sharedMemPerBlockOptin);
   } else {
     c->smem_rollout = (p->flags & BRMPPI_FLAG_PROJECTED) ? rollout_projected_smem_bytes(d)
                       : (p->flags & BRMPPI_FLAG_MPCC)    ? rollout_mpcc_smem_bytes(d)

@@ -31,19 +31,103 @@ __device__ __forceinline__ float4 path_eval(const float4* __restrict__ sPath, in
   return make_float4(r[0], r[1], r[2], r[3]);
 }
 
-// Q_c e_c^2 + Q_l e_l^2 + Q_th1 e_th1^2 + Q_th2 e_th2^2 at (X, psi); *nu = v cos(theta1 - theta^{1,r}).
-// s1 / c1 = sin / cos(X.t1): the caller needs them for the next step anyway.
+// One component of the same (the chain of the phase-split kernel needs theta^{1,r} only).
+__device__ __forceinline__ float path_eval_component(const float4* __restrict__ sPath, int M, float dpsi,
+                                                     float inv_dpsi, float psi, int comp) {
+  int m = (int)floorf(psi * inv_dpsi);
+  m = m > M - 1 ? M - 1 : (m < 0 ? 0 : m);
+  const float s = psi - (float)m * dpsi;
+  const float4 k = sPath[4 * m + comp];
+  return fmaf(s, fmaf(s, fmaf(s, k.w, k.z), k.y), k.x);
+}
+
+// Q_c e_c^2 + Q_l e_l^2 + Q_th1 e_th1^2 + Q_th2 e_th2^2 at pose (x, y, t1, t2) against the path point r;
+// s1 / c1 = sin / cos(t1), sr / cr = sin / cos(r.z); *nu = v cos(theta1 - theta^{1,r}).
+__device__ __forceinline__ float mpcc_tracking_sc(const DeviceParams& P, float x, float y, float t1, float t2, float v,
+                                                  float s1, float c1, const float4 r, float sr, float cr, float* nu) {
+  const float dx = x - r.x, dy = y - r.y;
+  const float ec = fmaf(sr, dx, -cr * dy);                       // (14)
+  const float el = -fmaf(cr, dx, sr * dy);                       // (15)
+  const float e1 = wrap_angle(t1 - r.z), e2 = wrap_angle(t2 - r.w);
+  *nu = v * fmaf(c1, cr, s1 * sr);                               // v cos(theta1 - theta1r)
+  return fmaf(P.Qc * ec, ec, fmaf(P.Ql * el, el, fmaf(P.Qth1 * e1, e1, P.Qth2 * e2 * e2)));
+}
+
+// The same with sin / cos of the path heading taken here; s1 / c1 = sin / cos(X.t1): the caller needs them for the
+// next step anyway.
 template <bool PRECISE>
 __device__ __forceinline__ float mpcc_tracking(const DeviceParams& P, const State7& X, float s1, float c1,
                                                const float4 r, float* nu) {
   float sr, cr;
   sincos_t<PRECISE>(r.z, &sr, &cr);
-  const float dx = X.x - r.x, dy = X.y - r.y;
-  const float ec = fmaf(sr, dx, -cr * dy);                       // (14)
-  const float el = -fmaf(cr, dx, sr * dy);                       // (15)
-  const float e1 = wrap_angle(X.t1 - r.z), e2 = wrap_angle(X.t2 - r.w);
-  *nu = X.v * fmaf(c1, cr, s1 * sr);                             // v cos(theta1 - theta1r)
-  return fmaf(P.Qc * ec, ec, fmaf(P.Ql * el, el, fmaf(P.Qth1 * e1, e1, P.Qth2 * e2 * e2)));
+  return mpcc_tracking_sc(P, X.x, X.y, X.t1, X.t2, X.v, s1, c1, r, sr, cr, nu);
+}
+
+// Heading rates of the continuous model, W1 = theta1', W2 = theta2', and their time derivatives under the input
+// omega = delta' (sb / cb = sin / cos of the hitch angle theta1 - theta2 by the angle-difference identities).
+struct MpccRates { float W1, W2, W1dot, W2dot; };
+
+__device__ __forceinline__ MpccRates mpcc_rates(const DeviceParams& P, float v, float a, float td, float s1, float c1,
+                                                float s2, float c2, float omega) {
+  const float sec2 = fmaf(td, td, 1.0f);
+  const float sb = s1 * c2 - c1 * s2, cb = fmaf(c1, c2, s1 * s2);
+  MpccRates R;
+  R.W1 = v * P.inv_L1 * td;
+  const float gb = fmaf(-P.Lh_over_L1 * cb, td, sb);                       // sin b - k cos b tan(delta)
+  R.W2 = v * P.inv_L2 * gb;
+  const float bdot = R.W1 - R.W2;
+  R.W1dot = P.inv_L1 * fmaf(a, td, v * sec2 * omega);
+  const float gbdot = fmaf(bdot, fmaf(P.Lh_over_L1 * sb, td, cb), -P.Lh_over_L1 * cb * sec2 * omega);
+  R.W2dot = P.inv_L2 * fmaf(a, gb, v * gbdot);
+  return R;
+}
+
+// Barrier-rate hinge with the predictor (17) summed over every (obstacle, disc):
+// (1 - alpha) h - hhat = -(alpha h + Ts hdot + Ts^2/2 hddot), from the centre, velocity and acceleration of each
+// disc (lever arms a1 - l_h on e(theta1), a2 on e(theta2)) and the obstacle's constant velocity.  nd <= ND discs.
+template <int ND>
+__device__ __forceinline__ float mpcc_hinge(const DeviceParams& P, const float4* __restrict__ sObs,
+                                            const float4* __restrict__ sVel, int n_obs, int nd, float tf, float alpha,
+                                            float x, float y, float v, float a, float s1, float c1, float s2, float c2,
+                                            const MpccRates& R) {
+  const float half_dt2 = 0.5f * P.dt * P.dt;
+  float cx[ND], cy[ND], vx[ND], vy[ND], ax[ND], ay[ND];
+#pragma unroll
+  for (int j = 0; j < ND; ++j) {
+    const float l1 = P.disc_a1[j] - P.Lh, l2 = P.disc_a2[j];
+    cx[j] = fmaf(l1, c1, fmaf(l2, c2, x));
+    cy[j] = fmaf(l1, s1, fmaf(l2, s2, y));
+    vx[j] = fmaf(v, c1, fmaf(-l1 * R.W1, s1, -l2 * R.W2 * s2));
+    vy[j] = fmaf(v, s1, fmaf(l1 * R.W1, c1, l2 * R.W2 * c2));
+    // a e1 + v W1 n1 + l1 (W1dot n1 - W1^2 e1) + l2 (W2dot n2 - W2^2 e2)
+    const float q1 = fmaf(v, R.W1, l1 * R.W1dot), r1 = fmaf(-l1 * R.W1, R.W1, a);
+    ax[j] = fmaf(r1, c1, fmaf(-q1, s1, l2 * fmaf(-R.W2dot, s2, -R.W2 * R.W2 * c2)));
+    ay[j] = fmaf(r1, s1, fmaf(q1, c1, l2 * fmaf(R.W2dot, c2, -R.W2 * R.W2 * s2)));
+  }
+  float pen = 0.0f;
+  for (int i = 0; i < n_obs; ++i) {
+    const float4 o = sObs[i];
+    const float4 w = sVel[i];
+    const float ox = fmaf(tf, w.x, o.x), oy = fmaf(tf, w.y, o.y);
+#pragma unroll
+    for (int j = 0; j < ND; ++j) {
+      if (j < nd) {
+        const float dx = cx[j] - ox, dy = cy[j] - oy, ex = vx[j] - w.z, ey = vy[j] - w.w;
+        const float h = fmaf(fmaf(dx, dx, dy * dy), o.z, -1.0f);
+        const float hd = 2.0f * o.z * fmaf(dx, ex, dy * ey);
+        const float hdd = 2.0f * o.z * (fmaf(ex, ex, ey * ey) + fmaf(dx, ax[j], dy * ay[j]));
+        pen += fmaxf(-fmaf(alpha, h, fmaf(P.dt, hd, half_dt2 * hdd)), 0.0f);
+      }
+    }
+  }
+  return pen;
+}
+
+// Hitch hinge, effort and progress terms of (13) at (x_{k+1}, u_k): everything but tracking and barrier.
+__device__ __forceinline__ float mpcc_stage_rest(const DeviceParams& P, float t1, float t2, float v, float nu, float2 u) {
+  const float dn = P.nu_bar - nu;
+  const float hl = fmaxf(fabsf(wrap_angle(t1 - t2)) - fmaf(-P.hitch_kappa, fabsf(v), P.hitch_max), 0.0f);
+  return fmaf(P.Rj * u.x, u.x, P.Rw * u.y * u.y) + P.mu * dn * dn + P.w_hitch * hl * hl;
 }
 
 template <bool PRECISE>
@@ -96,7 +180,6 @@ rollout_mpcc(const __grid_constant__ DeviceParams P) {
   if (valid) {
     const float inv_dpsi = 1.0f / dpsi, Lpath = (float)M * dpsi;
     const float alpha = sample_alpha(P, n, (uint32_t)(k + P.k_offset), key0, key1);
-    const float half_dt2 = 0.5f * P.dt * P.dt;
     State7 X{0.0f, 0.0f, s7[2], s7[3], s7[4], s7[5], s7[6], s7[7]};
     double cost = 0.0;
     float last_track = 0.0f;
@@ -110,49 +193,11 @@ rollout_mpcc(const __grid_constant__ DeviceParams P) {
       const float2 u = sample_control<PRECISE>(P, sU[t], (uint32_t)t, n, (uint32_t)(k + P.k_offset), key0, key1);   // (j, omega)
       float s2, c2;
       sincos_t<PRECISE>(X.t2, &s2, &c2);
-      const float td = tan_t<PRECISE>(X.de), sec2 = fmaf(td, td, 1.0f);
-      const float sb = s1 * c2 - c1 * s2, cb = fmaf(c1, c2, s1 * s2);
-      // heading rates of the continuous model and their time derivatives under the sampled input
-      const float W1 = X.v * P.inv_L1 * td;
-      const float gb = fmaf(-P.Lh_over_L1 * cb, td, sb);                       // sin b - k cos b tan(delta)
-      const float W2 = X.v * P.inv_L2 * gb;
-      const float bdot = W1 - W2;
-      const float W1dot = P.inv_L1 * fmaf(X.a, td, X.v * sec2 * u.y);
-      const float gbdot = fmaf(bdot, fmaf(P.Lh_over_L1 * sb, td, cb), -P.Lh_over_L1 * cb * sec2 * u.y);
-      const float W2dot = P.inv_L2 * fmaf(X.a, gb, X.v * gbdot);
-      // barrier-rate hinge with the predictor (17): (1 - alpha) h - hhat = -(alpha h + Ts hdot + Ts^2/2 hddot)
-      float pen = 0.0f;
-      {
-        float cx[kMaxDiscs], cy[kMaxDiscs], vx[kMaxDiscs], vy[kMaxDiscs], ax[kMaxDiscs], ay[kMaxDiscs];
-#pragma unroll
-        for (int j = 0; j < kMaxDiscs; ++j) {
-          const float l1 = P.disc_a1[j] - P.Lh, l2 = P.disc_a2[j];              // lever arms on the two headings
-          cx[j] = fmaf(l1, c1, fmaf(l2, c2, X.x));
-          cy[j] = fmaf(l1, s1, fmaf(l2, s2, X.y));
-          vx[j] = fmaf(X.v, c1, fmaf(-l1 * W1, s1, -l2 * W2 * s2));
-          vy[j] = fmaf(X.v, s1, fmaf(l1 * W1, c1, l2 * W2 * c2));
-          // a e1 + v W1 n1 + l1 (W1dot n1 - W1^2 e1) + l2 (W2dot n2 - W2^2 e2)
-          const float q1 = fmaf(X.v, W1, l1 * W1dot), r1 = fmaf(-l1 * W1, W1, X.a);
-          ax[j] = fmaf(r1, c1, fmaf(-q1, s1, l2 * fmaf(-W2dot, s2, -W2 * W2 * c2)));
-          ay[j] = fmaf(r1, s1, fmaf(q1, c1, l2 * fmaf(W2dot, c2, -W2 * W2 * s2)));
-        }
-        const float tf = (float)t;
-        for (int i = 0; i < n_obs; ++i) {
-          const float4 o = sObs[i];
-          const float4 w = sVel[i];
-          const float ox = fmaf(tf, w.x, o.x), oy = fmaf(tf, w.y, o.y);
-#pragma unroll
-          for (int j = 0; j < kMaxDiscs; ++j) {
-            if (j < P.n_discs) {
-              const float dx = cx[j] - ox, dy = cy[j] - oy, ex = vx[j] - w.z, ey = vy[j] - w.w;
-              const float h = fmaf(fmaf(dx, dx, dy * dy), o.z, -1.0f);
-              const float hd = 2.0f * o.z * fmaf(dx, ex, dy * ey);
-              const float hdd = 2.0f * o.z * (fmaf(ex, ex, ey * ey) + fmaf(dx, ax[j], dy * ay[j]));
-              pen += fmaxf(-fmaf(alpha, h, fmaf(P.dt, hd, half_dt2 * hdd)), 0.0f);
-            }
-          }
-        }
-      }
+      const float td = tan_t<PRECISE>(X.de);
+      const MpccRates R = mpcc_rates(P, X.v, X.a, td, s1, c1, s2, c2, u.y);
+      const float W1 = R.W1, W2 = R.W2;
+      const float pen = mpcc_hinge<kMaxDiscs>(P, sObs, sVel, n_obs, P.n_discs, (float)t, alpha, X.x, X.y, X.v, X.a,
+                                              s1, c1, s2, c2, R);
       // eq. (6), every right-hand side at step k; path parameter by the projection velocity
       State7 N;
       N.x = fmaf(P.dt * X.v, c1, X.x);
@@ -168,9 +213,7 @@ rollout_mpcc(const __grid_constant__ DeviceParams P) {
       sincos_t<PRECISE>(X.t1, &s1, &c1);
       const float track = mpcc_tracking<PRECISE>(P, X, s1, c1, path_eval(sPath, M, dpsi, inv_dpsi, X.psi), &nu);
       last_track = track;
-      const float dn = P.nu_bar - nu;
-      const float hl = fmaxf(fabsf(wrap_angle(X.t1 - X.t2)) - fmaf(-P.hitch_kappa, fabsf(X.v), P.hitch_max), 0.0f);
-      const float stage = track + fmaf(P.Rj * u.x, u.x, P.Rw * u.y * u.y) + P.mu * dn * dn + P.w_hitch * hl * hl;
+      const float stage = track + mpcc_stage_rest(P, X.t1, X.t2, X.v, nu, u);
       cost += (double)stage + (double)P.w_bar * (double)pen;
     }
     // terminal cost: the tracking terms at (x_N, psi_N), which the last stage cost just evaluated

@@ -33,6 +33,12 @@ def B():
     return brmppi
 
 
+@pytest.fixture(params=[0, 4], ids=["cta", "thread"])
+def kern(request):
+    """Both rollout kernels of the mode: the phase-split CTA kernel (default) and BRMPPI_FLAG_KERNEL_THREAD_PER_SAMPLE."""
+    return request.param
+
+
 def close(a, b, floor):
     a, b = np.asarray(a, dtype=np.float64), np.asarray(b, dtype=np.float64)
     return np.abs(a - b) <= RTOL * np.maximum(np.abs(b), floor)
@@ -134,9 +140,9 @@ def check(O, got, sc, p, n0=0, U0=None):
 
 @pytest.mark.parametrize("n_obs", [0, 1, 3, 8])
 @pytest.mark.parametrize("precise", [0, 2], ids=["fast", "precise"])
-def test_mpcc_iteration_matches_oracle(B, O, n_obs, precise):
+def test_mpcc_iteration_matches_oracle(B, O, n_obs, precise, kern):
     sc = path_scene(n_obs, n_obs, K=1000, T=40)
-    ref = check(O, gpu_mpcc(B, sc, sc.params, precise), sc, sc.params)
+    ref = check(O, gpu_mpcc(B, sc, sc.params, precise | kern), sc, sc.params)
     if n_obs >= 3:      # the scene is one where the predictor's hinge is at work, not a free run
         free = O.solve7(sc.params, sc.coef, sc.dpsi, 0, sc.x0, sc.psi0, np.zeros((0, 5)), np.zeros((40, 2)), n_threads=8)[-1]
         assert (ref["S"] > free["S"] + 1e-3).mean() > 0.05
@@ -144,22 +150,22 @@ def test_mpcc_iteration_matches_oracle(B, O, n_obs, precise):
         assert ref["flat_ok"] == sc.params.K and ref["U_err_flat"] <= 1.0
 
 
-def test_ragged_sizes_and_unused_capacity(B, O):
+def test_ragged_sizes_and_unused_capacity(B, O, kern):
     """K not a multiple of the block, odd T (the Philox pair of the last step is half used), obstacle and path
     capacity larger than what is set."""
     sc = path_scene(4, 3, K=333, T=27)
-    check(O, gpu_mpcc(B, sc, sc.params, 0, max_obstacles=8), sc, sc.params)
-    s = B.Solver(sc.params, 1, 8, B.FLAG_MPCC | B.FLAG_WRITE_SAMPLES, max_path_segments=64)
+    check(O, gpu_mpcc(B, sc, sc.params, kern, max_obstacles=8), sc, sc.params)
+    s = B.Solver(sc.params, 1, 8, kern | B.FLAG_MPCC | B.FLAG_WRITE_SAMPLES, max_path_segments=64)
     s.set_scene(sc)
     s.solve()
     got = dict(U=s.get_controls(), S=s.get_costs(), XT=s.get_final_states7(), diag=s.get_diag())
     s.close()
     check(O, got, sc, sc.params)
     one = path_scene(5, 2, K=1, T=5)
-    check(O, gpu_mpcc(B, one, one.params), one, one.params)
+    check(O, gpu_mpcc(B, one, one.params, kern), one, one.params)
 
 
-def test_warm_nominal_moving_obstacles_off_axle_hitch_four_discs(B, O):
+def test_warm_nominal_moving_obstacles_off_axle_hitch_four_discs(B, O, kern):
     discs = ((0, 0.0), (0, 2.5), (1, -2.0), (1, -4.5))
     sc = path_scene(6, 6, K=800, T=50, Lh=0.75, discs=discs, nu_bar=2.5, hitch_kappa=0.05, alpha_lo=0.0, alpha_hi=1.0)
     sc.obstacles[:, 3:] = np.random.default_rng(1).uniform(-1.2, 1.2, (6, 2)).astype(np.float32)
@@ -168,12 +174,12 @@ def test_warm_nominal_moving_obstacles_off_axle_hitch_four_discs(B, O):
     x0[5] += 0.3                                  # trailer not aligned
     sc = scenes.PathScene(x0.astype(np.float32).astype(np.float64), 0.75, sc.obstacles, sc.coef, sc.dpsi, sc.params)
     U0 = np.tile([0.5, -0.2], (50, 1)).astype(np.float32)
-    check(O, gpu_mpcc(B, sc, sc.params, 0, n0=7, U0=U0), sc, sc.params, n0=7, U0=U0)
+    check(O, gpu_mpcc(B, sc, sc.params, kern, n0=7, U0=U0), sc, sc.params, n0=7, U0=U0)
     p3 = sc.params.with_(n_iter=3)
-    check(O, gpu_mpcc(B, sc, p3, 0, n0=2), sc, p3, n0=2)
+    check(O, gpu_mpcc(B, sc, p3, kern, n0=2), sc, p3, n0=2)
 
 
-def test_path_end_clamp_and_reverse(B, O):
+def test_path_end_clamp_and_reverse(B, O, kern):
     """psi pinned at both ends of the path: a start at the path's end driving forward (psi stays at M dpsi), and a
     start at psi = 0 reversing (psi stays at 0); the steering state saturates under a hard-over nominal."""
     sc = path_scene(7, 2, K=400, T=40)
@@ -181,21 +187,21 @@ def test_path_end_clamp_and_reverse(B, O):
     r_end = O.path_eval(sc.params, sc.coef, sc.dpsi, L)
     x_end = np.array([r_end[0], r_end[1], 2.0, 0.0, r_end[2], r_end[3], 0.0]).astype(np.float32).astype(np.float64)
     a = scenes.PathScene(x_end, float(np.float32(L)), sc.obstacles, sc.coef, sc.dpsi, sc.params)
-    ra = check(O, gpu_mpcc(B, a, a.params), a, a.params)
+    ra = check(O, gpu_mpcc(B, a, a.params, kern), a, a.params)
     assert (ra["XT"][:, 7] >= L - 1e-9).mean() > 0.9
     x_rev = sc.x0.copy(); x_rev[2] = -1.5
     b = scenes.PathScene(x_rev, 0.0, sc.obstacles, sc.coef, sc.dpsi, sc.params)
-    rb = check(O, gpu_mpcc(B, b, b.params), b, b.params)
+    rb = check(O, gpu_mpcc(B, b, b.params, kern), b, b.params)
     assert (rb["XT"][:, 7] == 0.0).mean() > 0.9
     U0 = np.tile([0.0, 0.9], (40, 1)).astype(np.float32)
-    rc = check(O, gpu_mpcc(B, sc, sc.params, U0=U0), sc, sc.params, U0=U0)
+    rc = check(O, gpu_mpcc(B, sc, sc.params, kern, U0=U0), sc, sc.params, U0=U0)
     assert (rc["XT"][:, 6] == sc.params.delta_max).mean() > 0.3
 
 
-def test_batch_of_scenes_with_their_own_paths(B, O):
+def test_batch_of_scenes_with_their_own_paths(B, O, kern):
     scs = [path_scene(10 + s, 2 + s, K=500, T=30) for s in range(3)]
     p = scs[0].params
-    s = B.Solver(p, 3, 8, B.FLAG_MPCC | B.FLAG_WRITE_SAMPLES, max_path_segments=16)
+    s = B.Solver(p, 3, 8, kern | B.FLAG_MPCC | B.FLAG_WRITE_SAMPLES, max_path_segments=16)
     for i, sc in enumerate(scs):
         s.set_scene(sc, i)
     s.solve()
@@ -205,14 +211,14 @@ def test_batch_of_scenes_with_their_own_paths(B, O):
     s.close()
 
 
-def test_k_offset_draws_the_global_samples(B, O):
+def test_k_offset_draws_the_global_samples(B, O, kern):
     """A context with k_offset = 384 computes samples 384..639 of the 640-sample solve: bit-identical S_k and x_T
     to the same samples of an unsharded context (same arithmetic, same draws), the oracle's argmin index."""
     sc = path_scene(3, 3, K=256, T=20)
     full = sc.params.with_(K=640)
-    whole = gpu_mpcc(B, sc, full, n0=4)
+    whole = gpu_mpcc(B, sc, full, kern, n0=4)
     ref = check(O, whole, sc, full, n0=4)
-    s = B.Solver(sc.params, 1, 3, B.FLAG_MPCC | B.FLAG_WRITE_SAMPLES, k_offset=384, max_path_segments=16)
+    s = B.Solver(sc.params, 1, 3, kern | B.FLAG_MPCC | B.FLAG_WRITE_SAMPLES, k_offset=384, max_path_segments=16)
     s.set_scene(sc)
     s.set_counter(4)
     s.solve()
@@ -224,11 +230,11 @@ def test_k_offset_draws_the_global_samples(B, O):
     s.close()
 
 
-def test_step_applies_the_plant_of_eq6_and_shifts(B, O):
+def test_step_applies_the_plant_of_eq6_and_shifts(B, O, kern):
     sc = path_scene(9, 3, K=512, T=30)
     sc.obstacles[:, 3:] = np.float32(0.5)
     p = sc.params
-    s = B.Solver(p, 1, 3, B.FLAG_MPCC, max_path_segments=16)
+    s = B.Solver(p, 1, 3, kern | B.FLAG_MPCC, max_path_segments=16)
     s.set_scene(sc)
     x, psi, obs = sc.x0.copy(), sc.psi0, sc.obstacles.copy()
     for it in range(3):
@@ -320,12 +326,12 @@ def test_argument_checks(B):
     s.close()
 
 
-def test_full_size_against_the_oracle(B, O):
+def test_full_size_against_the_oracle(B, O, kern):
     """CFG2's size in the launch configuration bench.py times (K = 16384, T = 80, 8 obstacles, the recipe's scene):
     every S_k and x_T and the update against the oracle's iteration."""
     sc = scenes.scene_mpcc(0, K=16384, T=80, dt=0.05, n_obs=8, M=24)
     p = sc.params.with_(n_iter=1)
-    s = B.Solver(p, 1, 8, B.FLAG_MPCC | B.FLAG_WRITE_SAMPLES, max_path_segments=24)
+    s = B.Solver(p, 1, 8, kern | B.FLAG_MPCC | B.FLAG_WRITE_SAMPLES, max_path_segments=24)
     s.set_scene(sc)
     s.solve()
     got = dict(U=s.get_controls(), S=s.get_costs(), XT=s.get_final_states7(), diag=s.get_diag())
