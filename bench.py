@@ -98,13 +98,15 @@ def projected_instr_per_sample_step(n_obs, n_discs):
 
 
 def mpcc_instr_per_sample_step(n_obs, n_discs):
-    """issue slots of one sample-step of the paper's own model and cost.  Fixed 176: noise, perturb
-    and clamp 60 (as on the penalty path); sin / cos of the two headings, tan and sec^2 of delta 11; sin / cos of the
-    hitch angle 4; W1, W2 and their time derivatives 20; Euler step (6) 12; path segment and four cubics 19;
-    tracking errors (14), (15), heading wraps, nu 26; progress, effort, hitch hinge, psi update, accumulate, loop 24.
-    Per disc 26: centre 4, velocity 8, acceleration 14.  Per obstacle 3 (position, 2 / rho^2); per (obstacle, disc)
-    21: differences 4, h 3, hdot 3, hddot 6, predictor and hinge 5."""
-    return 176 + 26 * n_discs + n_obs * (3 + 21 * n_discs)
+    """issue slots of one sample-step of the paper's own model and cost, with the predictor folded
+    into one quadratic form per (obstacle, disc) (rollout_mpcc.cuh: mpcc_hinge).  Fixed 203: noise, perturb and clamp
+    60 (as on the penalty path); sin / cos of the two headings, tan and sec^2 of delta 11; sin / cos of the hitch
+    angle 4; step-unit scaling 3; W1, W2 and their time derivatives 20; the six vectors every disc's velocity and
+    acceleration are affine in 24; Euler step (6) 12; path segment and four cubics 19; tracking errors (14), (15),
+    heading wraps, nu 26; progress, effort, hitch hinge, psi update, accumulate, loop 24.  Per disc 12: centre,
+    velocity, 2 v + a.  Per obstacle 2 (position); per (obstacle, disc) 16: differences 4, obstacle-velocity
+    correction 2, d.(2e + a) + |e|^2 4, |d|^2 2, alpha |d|^2 1, alpha - q / rho^2 1, max and accumulate 2."""
+    return 203 + 12 * n_discs + n_obs * (2 + 16 * n_discs)
 
 
 def algorithmic_instr_per_sample_step(n_obs, n_discs, superellipses=None, philox_per_step=1.0):

@@ -379,7 +379,9 @@ int brmppi_create(const brmppi_params* p, void* dev_workspace, size_t workspace_
     d.off_planes = (int)ts.planes; d.off_misc = (int)ts.misc;
   }
   if (c->plan.mpcc_cta) {
-    d.S_tile = kMpccTile; d.tiles_per_scene = c->plan.mpcc.tiles_per_scene; d.total_tiles = c->plan.mpcc.total_tiles;
+    const MpccCtaPlan& mp = c->plan.mpcc;
+    d.S_tile = mp.S; d.t_stride = mp.stride; d.chunks = mp.G; d.chunk_len = mp.L; d.mpcc_noise_planes = mp.noise_planes;
+    d.tiles_per_scene = mp.tiles_per_scene; d.total_tiles = mp.total_tiles;
   }
   unsigned char* base = (unsigned char*)dev_workspace;
   const Layout& L = c->layout;

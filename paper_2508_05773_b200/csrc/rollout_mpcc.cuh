@@ -82,41 +82,50 @@ __device__ __forceinline__ MpccRates mpcc_rates(const DeviceParams& P, float v, 
   return R;
 }
 
-// Barrier-rate hinge with the predictor (17) summed over every (obstacle, disc):
-// (1 - alpha) h - hhat = -(alpha h + Ts hdot + Ts^2/2 hddot), from the centre, velocity and acceleration of each
-// disc (lever arms a1 - l_h on e(theta1), a2 on e(theta2)) and the obstacle's constant velocity.  nd <= ND discs.
+// Barrier-rate hinge with the predictor (17) summed over every (obstacle, disc).  With h = |d|^2 / rho^2 - 1,
+// hdot = 2 d.e / rho^2, hddot = 2 (e.e + d.acc) / rho^2 (d = disc centre - obstacle, e = their relative velocity,
+// acc = the disc centre's acceleration):
+//   (1 - alpha) h - hhat = -(alpha h + Ts hdot + Ts^2/2 hddot) = alpha - [alpha |d|^2 + d.(2 Ts e + Ts^2 acc) + |Ts e|^2] / rho^2,
+// so everything is evaluated in step units: the caller passes vh = Ts v, ah = Ts^2 a and the rates of
+// mpcc_rates(vh, ah, ..., Ts omega) (every formula is homogeneous in Ts), the obstacle table holds Ts vel.
+// Lever arms a1 - l_h on e(theta1), a2 on e(theta2).  nd <= ND discs.
 template <int ND>
 __device__ __forceinline__ float mpcc_hinge(const DeviceParams& P, const float4* __restrict__ sObs,
                                             const float4* __restrict__ sVel, int n_obs, int nd, float tf, float alpha,
-                                            float x, float y, float v, float a, float s1, float c1, float s2, float c2,
+                                            float x, float y, float vh, float ah, float s1, float c1, float s2, float c2,
                                             const MpccRates& R) {
-  const float half_dt2 = 0.5f * P.dt * P.dt;
-  float cx[ND], cy[ND], vx[ND], vy[ND], ax[ND], ay[ND];
+  // centre, velocity and f = 2 v + acc of disc j are affine in its lever arms (l1, l2): c = p + l1 e1 + l2 e2,
+  // v = vh e1 + l1 W1 n1 + l2 W2 n2, acc = (ah e1 + vh W1 n1) + l1 (W1dot n1 - W1^2 e1) + l2 (W2dot n2 - W2^2 e2)
+  // with e = (cos, sin), n = (-sin, cos) of the two headings; the six vectors are shared by all discs
+  const float p1x = -R.W1 * s1, p1y = R.W1 * c1, p2x = -R.W2 * s2, p2y = R.W2 * c2, v0x = vh * c1, v0y = vh * s1;
+  const float f0x = fmaf(2.0f, v0x, fmaf(ah, c1, vh * p1x)), f0y = fmaf(2.0f, v0y, fmaf(ah, s1, vh * p1y));
+  const float f1x = fmaf(2.0f, p1x, fmaf(-R.W1dot, s1, -R.W1 * p1y)), f1y = fmaf(2.0f, p1y, fmaf(R.W1dot, c1, R.W1 * p1x));
+  const float f2x = fmaf(2.0f, p2x, fmaf(-R.W2dot, s2, -R.W2 * p2y)), f2y = fmaf(2.0f, p2y, fmaf(R.W2dot, c2, R.W2 * p2x));
+  float cx[ND], cy[ND], vx[ND], vy[ND], fx[ND], fy[ND];
 #pragma unroll
   for (int j = 0; j < ND; ++j) {
     const float l1 = P.disc_a1[j] - P.Lh, l2 = P.disc_a2[j];
     cx[j] = fmaf(l1, c1, fmaf(l2, c2, x));
     cy[j] = fmaf(l1, s1, fmaf(l2, s2, y));
-    vx[j] = fmaf(v, c1, fmaf(-l1 * R.W1, s1, -l2 * R.W2 * s2));
-    vy[j] = fmaf(v, s1, fmaf(l1 * R.W1, c1, l2 * R.W2 * c2));
-    // a e1 + v W1 n1 + l1 (W1dot n1 - W1^2 e1) + l2 (W2dot n2 - W2^2 e2)
-    const float q1 = fmaf(v, R.W1, l1 * R.W1dot), r1 = fmaf(-l1 * R.W1, R.W1, a);
-    ax[j] = fmaf(r1, c1, fmaf(-q1, s1, l2 * fmaf(-R.W2dot, s2, -R.W2 * R.W2 * c2)));
-    ay[j] = fmaf(r1, s1, fmaf(q1, c1, l2 * fmaf(R.W2dot, c2, -R.W2 * R.W2 * s2)));
+    vx[j] = fmaf(l1, p1x, fmaf(l2, p2x, v0x));
+    vy[j] = fmaf(l1, p1y, fmaf(l2, p2y, v0y));
+    fx[j] = fmaf(l1, f1x, fmaf(l2, f2x, f0x));
+    fy[j] = fmaf(l1, f1y, fmaf(l2, f2y, f0y));
   }
   float pen = 0.0f;
   for (int i = 0; i < n_obs; ++i) {
     const float4 o = sObs[i];
-    const float4 w = sVel[i];
+    const float4 w = sVel[i];                                  // (Ts vx, Ts vy, ...): the obstacle's step
     const float ox = fmaf(tf, w.x, o.x), oy = fmaf(tf, w.y, o.y);
 #pragma unroll
     for (int j = 0; j < ND; ++j) {
       if (j < nd) {
-        const float dx = cx[j] - ox, dy = cy[j] - oy, ex = vx[j] - w.z, ey = vy[j] - w.w;
-        const float h = fmaf(fmaf(dx, dx, dy * dy), o.z, -1.0f);
-        const float hd = 2.0f * o.z * fmaf(dx, ex, dy * ey);
-        const float hdd = 2.0f * o.z * (fmaf(ex, ex, ey * ey) + fmaf(dx, ax[j], dy * ay[j]));
-        pen += fmaxf(-fmaf(alpha, h, fmaf(P.dt, hd, half_dt2 * hdd)), 0.0f);
+        const float dx = cx[j] - ox, dy = cy[j] - oy, ex = vx[j] - w.x, ey = vy[j] - w.y;
+        // d.(2 e + acc) = d.(f - 2 w): the obstacle does not accelerate
+        const float gx = fmaf(-2.0f, w.x, fx[j]), gy = fmaf(-2.0f, w.y, fy[j]);
+        float q = fmaf(dx, gx, fmaf(dy, gy, fmaf(ex, ex, ey * ey)));
+        q = fmaf(alpha, fmaf(dx, dx, dy * dy), q);
+        pen += fmaxf(fmaf(-o.z, q, alpha), 0.0f);
       }
     }
   }
@@ -194,18 +203,19 @@ rollout_mpcc(const __grid_constant__ DeviceParams P) {
       float s2, c2;
       sincos_t<PRECISE>(X.t2, &s2, &c2);
       const float td = tan_t<PRECISE>(X.de);
-      const MpccRates R = mpcc_rates(P, X.v, X.a, td, s1, c1, s2, c2, u.y);
-      const float W1 = R.W1, W2 = R.W2;
-      const float pen = mpcc_hinge<kMaxDiscs>(P, sObs, sVel, n_obs, P.n_discs, (float)t, alpha, X.x, X.y, X.v, X.a,
+      // rates in step units (Ts W1 and Ts W2 are the Euler increments of the headings as well)
+      const float vh = P.dt * X.v, ah = P.dt * P.dt * X.a;
+      const MpccRates R = mpcc_rates(P, vh, ah, td, s1, c1, s2, c2, P.dt * u.y);
+      const float pen = mpcc_hinge<kMaxDiscs>(P, sObs, sVel, n_obs, P.n_discs, (float)t, alpha, X.x, X.y, vh, ah,
                                               s1, c1, s2, c2, R);
       // eq. (6), every right-hand side at step k; path parameter by the projection velocity
       State7 N;
-      N.x = fmaf(P.dt * X.v, c1, X.x);
-      N.y = fmaf(P.dt * X.v, s1, X.y);
+      N.x = fmaf(vh, c1, X.x);
+      N.y = fmaf(vh, s1, X.y);
       N.v = fmaf(P.dt, X.a, X.v);
       N.a = fmaf(P.dt, u.x, X.a);
-      N.t1 = fmaf(P.dt, W1, X.t1);
-      N.t2 = fmaf(P.dt, W2, X.t2);
+      N.t1 = X.t1 + R.W1;
+      N.t2 = X.t2 + R.W2;
       N.de = fminf(fmaxf(fmaf(P.dt, u.y, X.de), P.dstate_lo), P.dstate_hi);
       N.psi = fminf(fmaxf(fmaf(P.dt, nu, X.psi), 0.0f), Lpath);
       X = N;

@@ -165,6 +165,13 @@ def test_ragged_sizes_and_unused_capacity(B, O, kern):
     check(O, gpu_mpcc(B, one, one.params, kern), one, one.params)
 
 
+def test_long_horizon_without_control_planes(B, O):
+    """K = 19000, T = 130: full 128-sample tiles whose sampled controls no longer fit in shared memory beside the state
+    ring -- the CTA kernel's chain then draws them as it goes and the epilogue regenerates them."""
+    sc = path_scene(13, 2, K=19000, T=130, v0=0.5)
+    check(O, gpu_mpcc(B, sc, sc.params), sc, sc.params)
+
+
 def test_warm_nominal_moving_obstacles_off_axle_hitch_four_discs(B, O, kern):
     discs = ((0, 0.0), (0, 2.5), (1, -2.0), (1, -4.5))
     sc = path_scene(6, 6, K=800, T=50, Lh=0.75, discs=discs, nu_bar=2.5, hitch_kappa=0.05, alpha_lo=0.0, alpha_hi=1.0)
