@@ -25,9 +25,12 @@ constexpr int kMpccCost = kMpccThreads - kMpccTileMax; // 640 cost threads, thre
 constexpr int kMpccMaxGroups = 12;                     // cost threads per sample, at most
 constexpr int kMpccMaxRows = kMpccMaxGroups + 1;       // a chunk keeps the row after its last step too
 
-// planes of one row (one state of the horizon), each [stride] floats
-enum MpccPlane { MP_X, MP_Y, MP_V, MP_A, MP_T1, MP_T2, MP_PSI, MP_S1, MP_C1, MP_SR, MP_CR,
-                 MP_S2, MP_C2, MP_TD, MP_J, MP_W, MP_COUNT };
+// One row (one state of the horizon) is four planes of float4, each [stride]: a thread moves a state with four
+// 128-bit accesses, conflict-free (consecutive samples, consecutive 16-byte words).
+//   Q0 = (x, y, v, a)   Q1 = (sin t1, cos t1, sin t2, cos t2)   Q2 = (tan delta, t1, t2, psi)
+//   Q3 = (sin, cos of the path heading at psi, j, omega)        (j, omega only without the control planes)
+constexpr int MP_QUADS = 4;
+constexpr int MP_COUNT = 4 * MP_QUADS;                 // floats per sample and row
 
 // Tiling of one launch: S samples per tile, stride = S rounded up to a warp, G cost threads per sample, L steps per chunk.
 // noise_planes: the sampled controls of the whole horizon are drawn by all threads before the chain starts and kept
@@ -84,25 +87,26 @@ inline MpccCtaPlan make_mpcc_cta_plan(int K, int T, int n_scenes, int max_obstac
 
 // One (sample, step) item of the cost phase: everything of step t that is not the state recursion.  Returns the
 // stage cost (13) with the barrier term; *track = the four tracking terms at (x_{t+1}, psi_{t+1}).  row0 / row1:
-// plane 0 of rows t and t + 1, already offset by the sample; st = plane stride.
+// quad 0 of rows t and t + 1, already offset by the sample; st = plane stride (in float4).
 template <int ND>
 __device__ __forceinline__ double mpcc_cost_item(const DeviceParams& P, const float4* __restrict__ sObs,
                                                  const float4* __restrict__ sVel, const float4* __restrict__ sPath,
-                                                 int n_obs, int M, float dpsi, float inv_dpsi, const float* row0,
-                                                 const float* row1, int st, int t, float alpha, float2 u, float* track) {
-  const float x = row0[MP_X * st], y = row0[MP_Y * st], v = row0[MP_V * st], a = row0[MP_A * st],
-              s1 = row0[MP_S1 * st], c1 = row0[MP_C1 * st], s2 = row0[MP_S2 * st], c2 = row0[MP_C2 * st],
-              td = row0[MP_TD * st];
-  const float vh = P.dt * v, ah = P.dt * P.dt * a;                               // step units (mpcc_hinge)
-  const MpccRates R = mpcc_rates(P, vh, ah, td, s1, c1, s2, c2, P.dt * u.y);
-  const float pen = mpcc_hinge<ND>(P, sObs, sVel, n_obs, ND, (float)t, alpha, x, y, vh, ah, s1, c1, s2, c2, R);
+                                                 int n_obs, int M, float dpsi, float inv_dpsi, const float4* row0,
+                                                 const float4* row1, int st, int t, float alpha, bool u_in_row,
+                                                 float2 u, float* track) {
+  const float4 q0 = row0[0], q1 = row0[st];                                     // (x, y, v, a), (s1, c1, s2, c2)
+  const float td = row0[2 * st].x;
+  if (u_in_row) { const float4 q3 = row0[3 * st]; u = make_float2(q3.z, q3.w); }
+  const float vh = P.dt * q0.z, ah = P.dt * P.dt * q0.w;                         // step units (mpcc_hinge)
+  const MpccRates R = mpcc_rates(P, vh, ah, td, q1.x, q1.y, q1.z, q1.w, P.dt * u.y);
+  const float pen = mpcc_hinge<ND>(P, sObs, sVel, n_obs, ND, (float)t, alpha, q0.x, q0.y, vh, ah, q1.x, q1.y, q1.z,
+                                   q1.w, R);
   // stage cost (13) on (x_{t+1}, u_t, psi_{t+1}): the next row
-  const float xn = row1[MP_X * st], yn = row1[MP_Y * st], vn = row1[MP_V * st], t1n = row1[MP_T1 * st],
-              t2n = row1[MP_T2 * st], psin = row1[MP_PSI * st], s1n = row1[MP_S1 * st], c1n = row1[MP_C1 * st],
-              srn = row1[MP_SR * st], crn = row1[MP_CR * st];
+  const float4 n0 = row1[0], n1 = row1[st], n2 = row1[2 * st], n3 = row1[3 * st];
   float nu;
-  *track = mpcc_tracking_sc(P, xn, yn, t1n, t2n, vn, s1n, c1n, path_eval(sPath, M, dpsi, inv_dpsi, psin), srn, crn, &nu);
-  const float stage = *track + mpcc_stage_rest(P, t1n, t2n, vn, nu, u);
+  *track = mpcc_tracking_sc(P, n0.x, n0.y, n2.y, n2.z, n0.z, n1.x, n1.y, path_eval(sPath, M, dpsi, inv_dpsi, n2.w), n3.x,
+                            n3.y, &nu);
+  const float stage = *track + mpcc_stage_rest(P, n2.y, n2.z, n0.z, nu, u);
   return (double)stage + (double)P.w_bar * (double)pen;
 }
 
@@ -118,7 +122,7 @@ rollout_mpcc_cta(const __grid_constant__ DeviceParams P) {
   float4* sVel = reinterpret_cast<float4*>(smem_raw + lay.vel);
   float4* sPath = reinterpret_cast<float4*>(smem_raw + lay.path);
   float2* sU = reinterpret_cast<float2*>(smem_raw + lay.U);
-  float* sPlanes = reinterpret_cast<float*>(smem_raw + lay.planes);
+  float4* sPlanes = reinterpret_cast<float4*>(smem_raw + lay.planes);
   float* sNoise = reinterpret_cast<float*>(smem_raw + lay.noise);      // [T + 1][2][st]: j, omega of every step
   double* sPart = reinterpret_cast<double*>(smem_raw + lay.part);
   float* sW = reinterpret_cast<float*>(smem_raw + lay.w);
@@ -135,7 +139,7 @@ rollout_mpcc_cta(const __grid_constant__ DeviceParams P) {
   const int s = chain_range ? tid - kMpccCost : tid - grp * S;
   const bool is_chain = chain_range && s < S, is_cost = !chain_range && grp < G;
   const int n_chunks = (T + L - 1) / L;
-  const int slot_floats = (L + 1) * MP_COUNT * st, row_floats = MP_COUNT * st;
+  const int row_quads = MP_QUADS * st, slot_quads = (L + 1) * row_quads;
   const uint32_t n = *P.counter;
   if (tid == 0) {
     mbar_init(smem_addr(&bars[0]), S); mbar_init(smem_addr(&bars[1]), S);
@@ -209,10 +213,10 @@ rollout_mpcc_cta(const __grid_constant__ DeviceParams P) {
         const uint32_t gg = g + (uint32_t)c;
         const int slot = (int)(gg & 1u);
         if (gg >= 2u) mbar_wait(smem_addr(&bars[2 + slot]), ((gg >> 1) - 1u) & 1u);   // the cost threads are done with it
-        float* row = sPlanes + slot * slot_floats + s;
+        float4* row = sPlanes + slot * slot_quads + s;
         const int t_end = min(t + L, T);
 #pragma unroll 1
-        for (; t < t_end; ++t, row += row_floats) {
+        for (; t < t_end; ++t, row += row_quads) {
           float2 u;
           if (noise_planes)
             u = make_float2(sNoise[(size_t)(2 * t) * st + s], sNoise[(size_t)(2 * t + 1) * st + s]);
@@ -221,11 +225,10 @@ rollout_mpcc_cta(const __grid_constant__ DeviceParams P) {
                                          key1, &u, &u_odd);
           else
             u = u_odd;
-          row[MP_X * st] = X.x;   row[MP_Y * st] = X.y;   row[MP_V * st] = X.v;   row[MP_A * st] = X.a;
-          row[MP_T1 * st] = X.t1; row[MP_T2 * st] = X.t2; row[MP_PSI * st] = X.psi;
-          row[MP_S1 * st] = s1;   row[MP_C1 * st] = c1;   row[MP_S2 * st] = s2;   row[MP_C2 * st] = c2;
-          row[MP_SR * st] = sr;   row[MP_CR * st] = cr;   row[MP_TD * st] = td;
-          if (!noise_planes) { row[MP_J * st] = u.x; row[MP_W * st] = u.y; }
+          row[0] = make_float4(X.x, X.y, X.v, X.a);
+          row[st] = make_float4(s1, c1, s2, c2);
+          row[2 * st] = make_float4(td, X.t1, X.t2, X.psi);
+          row[3 * st] = make_float4(sr, cr, u.x, u.y);
           const float vh = P.dt * X.v;
           const float nu = X.v * fmaf(c1, cr, s1 * sr);
           const MpccRates R = mpcc_rates(P, vh, 0.0f, td, s1, c1, s2, c2, 0.0f);     // Ts W1, Ts W2 are what is used
@@ -246,9 +249,10 @@ rollout_mpcc_cta(const __grid_constant__ DeviceParams P) {
           td = tan_t<PRECISE>(X.de);
         }
         // the row after the chunk's last step: read only as a "next state"
-        row[MP_X * st] = X.x;   row[MP_Y * st] = X.y;   row[MP_V * st] = X.v;
-        row[MP_T1 * st] = X.t1; row[MP_T2 * st] = X.t2; row[MP_PSI * st] = X.psi;
-        row[MP_S1 * st] = s1;   row[MP_C1 * st] = c1;   row[MP_SR * st] = sr;   row[MP_CR * st] = cr;
+        row[0] = make_float4(X.x, X.y, X.v, X.a);
+        row[st] = make_float4(s1, c1, s2, c2);
+        row[2 * st] = make_float4(td, X.t1, X.t2, X.psi);
+        row[3 * st] = make_float4(sr, cr, 0.0f, 0.0f);
         mbar_arrive(smem_addr(&bars[slot]));
       }
       if (valid && (P.flags & BRMPPI_FLAG_WRITE_SAMPLES)) {
@@ -269,11 +273,9 @@ rollout_mpcc_cta(const __grid_constant__ DeviceParams P) {
           const int t = c * L + r;
           if (t < T) {
             float track;
-            const float* row0 = sPlanes + slot * slot_floats + r * row_floats + s;
-            const float2 u = noise_planes ? make_float2(sNoise[(size_t)(2 * t) * st + s], sNoise[(size_t)(2 * t + 1) * st + s])
-                                          : make_float2(row0[MP_J * st], row0[MP_W * st]);
-            acc += mpcc_cost_item<ND>(P, sObs, sVel, sPath, n_obs, M, dpsi, inv_dpsi, row0, row0 + row_floats, st, t,
-                                      alpha, u, &track);
+            const float4* row0 = sPlanes + slot * slot_quads + r * row_quads + s;
+            acc += mpcc_cost_item<ND>(P, sObs, sVel, sPath, n_obs, M, dpsi, inv_dpsi, row0, row0 + row_quads, st, t,
+                                      alpha, true, make_float2(0.0f, 0.0f), &track);
             if (t == T - 1) acc += (double)(P.w_term * track);       // terminal cost: the same four terms at (x_N, psi_N)
           }
         }
