@@ -52,7 +52,9 @@ typedef enum {
   BRMPPI_ERR_NOT_READY = -6,           /* solve/step before state and goal of every scene set;
                                           get_costs/get_final_states without FLAG_WRITE_SAMPLES */
   BRMPPI_ERR_CUDA = -7,
-  BRMPPI_ERR_UNALIGNED = -8            /* workspace not 256-byte aligned                       */
+  BRMPPI_ERR_UNALIGNED = -8,           /* workspace not 256-byte aligned                       */
+  BRMPPI_ERR_TOO_LARGE = -9            /* n exceeds the capacity of the library's static device scratch
+                                          (brmppi_hitch_filter_static: BRMPPI_HITCH_STATIC_MAX_N)  */
 } brmppi_status;
 
 /* Disc obstacle with constant-velocity prediction (Assumption 2):
@@ -305,6 +307,21 @@ size_t brmppi_hitch_filter_scratch_bytes(int n);
 int brmppi_hitch_filter(void* cuda_stream, const brmppi_params* p, int n, const float* x,
                         const float* u_ref, float* u_out, int* status_out, void* dev_scratch,
                         size_t scratch_bytes);
+
+/* The same operation for callers that cannot allocate device memory at all (code under CUDA-graph capture, tight
+ * serving loops, harnesses that forbid cudaMalloc): the staging that brmppi_hitch_filter takes from the caller as
+ * dev_scratch lives here in a file-scope static __device__ array of BRMPPI_HITCH_STATIC_MAX_N * 36 bytes (576 KiB),
+ * which every GPU that loads the library holds until the process exits.  Arguments, results and error codes as
+ * brmppi_hitch_filter (all pointers HOST), plus: n > BRMPPI_HITCH_STATIC_MAX_N returns BRMPPI_ERR_TOO_LARGE and
+ * touches nothing.  Calls no cudaMalloc / cudaFree and no allocating library routine; the array's device address
+ * is looked up once per device (cudaGetSymbolAddress, with that device current) and kept.  Synchronises the
+ * stream.  Every call on a device shares the one array: nothing in it has to start at zero (each call overwrites
+ * the n entries it reads back; entries beyond n keep an earlier call's contents and are never read), but two
+ * calls that overlap on the GPU -- from two host threads or two streams of the same device -- race on it:
+ * serialise them. */
+#define BRMPPI_HITCH_STATIC_MAX_N 16384
+int brmppi_hitch_filter_static(void* cuda_stream, const brmppi_params* p, int n, const float* x,
+                               const float* u_ref, float* u_out, int* status_out);
 
 /* Closed-form projection of BR-MPPI, eq. (11)-(12), for n independent problems:
  *   min_z ||z - z_des||_W^2 + rho/2 (||z - z_lo||^2 + ||z_hi - z||^2)   s.t.  A z = b,

@@ -21,6 +21,8 @@ FLAG_MPCC = 64
 OK = 0
 ERR_NULL, ERR_INVALID_ARG, ERR_WORKSPACE_TOO_SMALL, ERR_TOO_MANY_OBSTACLES = -1, -2, -3, -4
 ERR_NONFINITE_INPUT, ERR_NOT_READY, ERR_CUDA, ERR_UNALIGNED = -5, -6, -7, -8
+ERR_TOO_LARGE = -9
+HITCH_STATIC_MAX_N = 16384
 
 EXPORTS = [
     "brmppi_workspace_bytes", "brmppi_create", "brmppi_destroy", "brmppi_set_state",
@@ -32,6 +34,7 @@ EXPORTS = [
     "brmppi_debug_philox_raw", "brmppi_hitch_filter_scratch_bytes", "brmppi_project_scratch_bytes",
     "brmppi_measure_peaks_scratch_bytes", "brmppi_shard_words", "brmppi_shard_export", "brmppi_shard_import",
     "brmppi_set_state7", "brmppi_set_reference_path", "brmppi_get_state7", "brmppi_get_final_states7",
+    "brmppi_hitch_filter_static",
 ]
 
 
@@ -144,6 +147,7 @@ def lib():
         L.brmppi_hitch_filter_scratch_bytes.argtypes = [C.c_int]
         L.brmppi_hitch_filter_scratch_bytes.restype = C.c_size_t
         L.brmppi_hitch_filter.argtypes = [vp, C.POINTER(CParams), C.c_int, _fp, _fp, _fp, C.POINTER(C.c_int), vp, C.c_size_t]
+        L.brmppi_hitch_filter_static.argtypes = [vp, C.POINTER(CParams), C.c_int, _fp, _fp, _fp, C.POINTER(C.c_int)]
         _lib = L
     return _lib
 
@@ -456,6 +460,24 @@ def hitch_filter(params, x, u_ref):
     st.synchronize()
     _check(lib().brmppi_hitch_filter(C.c_void_p(st.cuda_stream), C.byref(cp), n, _p(x), _p(r), _p(u),
                                      status.ctypes.data_as(C.POINTER(C.c_int)), C.c_void_p(scratch.data_ptr()), C.c_size_t(nb)))
+    return u, status
+
+
+def hitch_filter_static(params, x, u_ref):
+    """hitch_filter through the library's static device scratch (no device allocation anywhere on the call:
+    brmppi_hitch_filter_static); n <= HITCH_STATIC_MAX_N, else BrmppiError with status ERR_TOO_LARGE."""
+    import torch
+    x = _f32(x).reshape(-1, 4)
+    r = _f32(u_ref).reshape(-1, 2)
+    n = x.shape[0]
+    assert r.shape[0] == n
+    cp = make_cparams(params, 1, 0, 0)
+    u = np.zeros((n, 2), dtype=np.float32)
+    status = np.zeros(n, dtype=np.int32)
+    st = torch.cuda.current_stream()
+    st.synchronize()
+    _check(lib().brmppi_hitch_filter_static(C.c_void_p(st.cuda_stream), C.byref(cp), n, _p(x), _p(r), _p(u),
+                                            status.ctypes.data_as(C.POINTER(C.c_int))))
     return u, status
 
 

@@ -4,6 +4,7 @@
 #include <cuda_runtime.h>
 #include <math_constants.h>
 
+#include <atomic>
 #include <cmath>
 #include <cstdio>
 #include <cstdlib>
@@ -277,6 +278,30 @@ int capture(brmppi_ctx* c, cudaGraphExec_t* exec, F&& body) {
   return BRMPPI_OK;
 }
 
+}  // namespace
+
+// Static device scratch of brmppi_hitch_filter_static (include/brmppi.h): staging for at most
+// BRMPPI_HITCH_STATIC_MAX_N problems, 36 bytes each.  In host code the name g_hitch_static is a host-side stand-in,
+// not a device address: the address comes from cudaGetSymbolAddress, once per device, with that device current.
+static __device__ __align__(256) unsigned char g_hitch_static[(size_t)BRMPPI_HITCH_STATIC_MAX_N * 36];
+
+namespace {
+constexpr int kStaticMaxDevices = 64;
+std::atomic<unsigned char*> g_hitch_static_addr[kStaticMaxDevices];
+
+int hitch_static_address(unsigned char** out) {
+  int dev = 0;
+  CU(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= kStaticMaxDevices) return BRMPPI_ERR_INVALID_ARG;
+  unsigned char* ptr = g_hitch_static_addr[dev].load(std::memory_order_acquire);
+  if (!ptr) {
+    CU(cudaGetSymbolAddress((void**)&ptr, g_hitch_static));
+    if (!ptr) return BRMPPI_ERR_NULL;
+    g_hitch_static_addr[dev].store(ptr, std::memory_order_release);   // the same value from any thread
+  }
+  *out = ptr;
+  return BRMPPI_OK;
+}
 }  // namespace
 
 template <int KIND>
@@ -850,6 +875,7 @@ const char* brmppi_strerror(int status) {
     case BRMPPI_ERR_NONFINITE_INPUT: return "non-finite input";
     case BRMPPI_ERR_NOT_READY: return "not ready (state/goal unset, or sample outputs not enabled)";
     case BRMPPI_ERR_UNALIGNED: return "workspace not 256-byte aligned";
+    case BRMPPI_ERR_TOO_LARGE: return "size exceeds the capacity of the library's static device scratch";
     case BRMPPI_ERR_CUDA:
       snprintf(g_errbuf, sizeof(g_errbuf), "CUDA error: %s", cudaGetErrorString(g_last_cuda));
       return g_errbuf;
@@ -950,6 +976,44 @@ int brmppi_hitch_filter(void* cuda_stream, const brmppi_params* p, int n, const 
   // the caller's scratch: x [n][4] | u_ref [n][2] | u_out [n][2] | status [n]
   const size_t N = (size_t)n;
   unsigned char* buf = (unsigned char*)align_up((size_t)(uintptr_t)dev_scratch, 256);
+  float4* dx = (float4*)buf;
+  float2* dr = (float2*)(buf + N * 16);
+  float2* du = (float2*)(buf + N * 24);
+  int* ds = (int*)(buf + N * 32);
+  CU(cudaMemcpyAsync(dx, x, N * 16, cudaMemcpyHostToDevice, s));
+  CU(cudaMemcpyAsync(dr, u_ref, N * 8, cudaMemcpyHostToDevice, s));
+  hitch_filter_batch<<<(unsigned)((N + 127) / 128), 128, 0, s>>>(d, n, dx, dr, du, ds);
+  CU(cudaGetLastError());
+  CU(cudaMemcpyAsync(u_out, du, N * 8, cudaMemcpyDeviceToHost, s));
+  if (status_out) CU(cudaMemcpyAsync(status_out, ds, N * 4, cudaMemcpyDeviceToHost, s));
+  CU(cudaStreamSynchronize(s));
+  return BRMPPI_OK;
+}
+
+int brmppi_hitch_filter_static(void* cuda_stream, const brmppi_params* p, int n, const float* x,
+                               const float* u_ref, float* u_out, int* status_out) {
+  if (!p) return BRMPPI_ERR_NULL;
+  if (n < 0) return BRMPPI_ERR_INVALID_ARG;
+  if (n > BRMPPI_HITCH_STATIC_MAX_N) return BRMPPI_ERR_TOO_LARGE;
+  const float f[] = {p->dt, p->L1, p->L2, p->Lh, p->v_min, p->v_max, p->delta_min, p->delta_max};
+  if (!finite_all(f, 8) || !hitch_params_valid(p) || !(p->dt > 0.f) || !(p->L1 > 0.f) || !(p->L2 > 0.f) ||
+      p->v_min > p->v_max || p->delta_min > p->delta_max || p->delta_min <= -1.5f || p->delta_max >= 1.5f)
+    return BRMPPI_ERR_INVALID_ARG;
+  if (n == 0) return BRMPPI_OK;
+  if (!x || !u_ref || !u_out) return BRMPPI_ERR_NULL;
+  unsigned char* buf = nullptr;
+  int r = hitch_static_address(&buf);
+  if (r) return r;
+  cudaStream_t s = (cudaStream_t)cuda_stream;
+  DeviceParams d;
+  memset(&d, 0, sizeof(d));
+  d.dt = p->dt; d.inv_L1 = 1.0f / p->L1; d.inv_L2 = 1.0f / p->L2; d.Lh = p->Lh;
+  d.Lh_over_L1 = p->Lh / p->L1; d.Lh_over_L2 = p->Lh / p->L2;
+  d.v_min = p->v_min; d.v_max = p->v_max; d.delta_min = p->delta_min; d.delta_max = p->delta_max;
+  d.hitch_max = p->hitch_max; d.hitch_kappa = p->hitch_kappa; d.hitch_alpha = p->hitch_alpha;
+  d.hitch_qv = p->hitch_qv; d.hitch_qdelta = p->hitch_qdelta;
+  // the static array: x [n][4] | u_ref [n][2] | u_out [n][2] | status [n]
+  const size_t N = (size_t)n;
   float4* dx = (float4*)buf;
   float2* dr = (float2*)(buf + N * 16);
   float2* du = (float2*)(buf + N * 24);
