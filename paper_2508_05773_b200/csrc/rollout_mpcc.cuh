@@ -88,12 +88,15 @@ __device__ __forceinline__ MpccRates mpcc_rates(const DeviceParams& P, float v, 
 //   (1 - alpha) h - hhat = -(alpha h + Ts hdot + Ts^2/2 hddot) = alpha - [alpha |d|^2 + d.(2 Ts e + Ts^2 acc) + |Ts e|^2] / rho^2,
 // so everything is evaluated in step units: the caller passes vh = Ts v, ah = Ts^2 a and the rates of
 // mpcc_rates(vh, ah, ..., Ts omega) (every formula is homogeneous in Ts), the obstacle table holds Ts vel.
-// Lever arms a1 - l_h on e(theta1), a2 on e(theta2).  nd <= ND discs.
+// Lever arms a1 - l_h on e(theta1), a2 on e(theta2).  nd <= ND discs.  Obstacles [0, n_moving) are taken in the
+// general form; [n_moving, n_obs) must be at rest (zero velocity: the caller's table is ordered that way), for
+// which e = v_disc and g = f, so that the bracket is alpha |d|^2 + d.f + |v_disc|^2 -- the same value (every
+// dropped term is an exact zero), ten instructions per (obstacle, disc) instead of sixteen.
 template <int ND>
 __device__ __forceinline__ float mpcc_hinge(const DeviceParams& P, const float4* __restrict__ sObs,
-                                            const float4* __restrict__ sVel, int n_obs, int nd, float tf, float alpha,
-                                            float x, float y, float vh, float ah, float s1, float c1, float s2, float c2,
-                                            const MpccRates& R) {
+                                            const float4* __restrict__ sVel, int n_moving, int n_obs, int nd, float tf,
+                                            float alpha, float x, float y, float vh, float ah, float s1, float c1,
+                                            float s2, float c2, const MpccRates& R) {
   // centre, velocity and f = 2 v + acc of disc j are affine in its lever arms (l1, l2): c = p + l1 e1 + l2 e2,
   // v = vh e1 + l1 W1 n1 + l2 W2 n2, acc = (ah e1 + vh W1 n1) + l1 (W1dot n1 - W1^2 e1) + l2 (W2dot n2 - W2^2 e2)
   // with e = (cos, sin), n = (-sin, cos) of the two headings; the six vectors are shared by all discs
@@ -113,7 +116,7 @@ __device__ __forceinline__ float mpcc_hinge(const DeviceParams& P, const float4*
     fy[j] = fmaf(l1, f1y, fmaf(l2, f2y, f0y));
   }
   float pen = 0.0f;
-  for (int i = 0; i < n_obs; ++i) {
+  for (int i = 0; i < n_moving; ++i) {
     const float4 o = sObs[i];
     const float4 w = sVel[i];                                  // (Ts vx, Ts vy, ...): the obstacle's step
     const float ox = fmaf(tf, w.x, o.x), oy = fmaf(tf, w.y, o.y);
@@ -126,6 +129,23 @@ __device__ __forceinline__ float mpcc_hinge(const DeviceParams& P, const float4*
         float q = fmaf(dx, gx, fmaf(dy, gy, fmaf(ex, ex, ey * ey)));
         q = fmaf(alpha, fmaf(dx, dx, dy * dy), q);
         pen += fmaxf(fmaf(-o.z, q, alpha), 0.0f);
+      }
+    }
+  }
+  if (n_moving < n_obs) {
+    float vv[ND];
+#pragma unroll
+    for (int j = 0; j < ND; ++j) vv[j] = fmaf(vx[j], vx[j], vy[j] * vy[j]);
+    for (int i = n_moving; i < n_obs; ++i) {
+      const float4 o = sObs[i];
+#pragma unroll
+      for (int j = 0; j < ND; ++j) {
+        if (j < nd) {
+          const float dx = cx[j] - o.x, dy = cy[j] - o.y;
+          float q = fmaf(dx, fx[j], fmaf(dy, fy[j], vv[j]));
+          q = fmaf(alpha, fmaf(dx, dx, dy * dy), q);
+          pen += fmaxf(fmaf(-o.z, q, alpha), 0.0f);
+        }
       }
     }
   }
@@ -206,8 +226,8 @@ rollout_mpcc(const __grid_constant__ DeviceParams P) {
       // rates in step units (Ts W1 and Ts W2 are the Euler increments of the headings as well)
       const float vh = P.dt * X.v, ah = P.dt * P.dt * X.a;
       const MpccRates R = mpcc_rates(P, vh, ah, td, s1, c1, s2, c2, P.dt * u.y);
-      const float pen = mpcc_hinge<kMaxDiscs>(P, sObs, sVel, n_obs, P.n_discs, (float)t, alpha, X.x, X.y, vh, ah,
-                                              s1, c1, s2, c2, R);
+      const float pen = mpcc_hinge<kMaxDiscs>(P, sObs, sVel, n_obs, n_obs, P.n_discs, (float)t, alpha, X.x, X.y, vh, ah,
+                                              s1, c1, s2, c2, R);          // table in the caller's order: general form
       // eq. (6), every right-hand side at step k; path parameter by the projection velocity
       State7 N;
       N.x = fmaf(vh, c1, X.x);
