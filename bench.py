@@ -384,7 +384,7 @@ def measure(B, torch, name, rank, steps, warmup, dist, dev, local_rank, closed_l
         roof = {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "Ginstr/s (thread-instructions)",
                 "frac": achieved / peak, "traffic": traffic if name == "cfg2" else None,
                 "traffic_source": traffic_source if name == "cfg2" else None,
-                "kernel": "rollout_projected" if name in PROJECTED else "rollout_mpcc" if name in MPCC else "rollout_cta",
+                "kernel": "rollout_projected" if name in PROJECTED else "rollout_mpcc_cta" if name in MPCC else "rollout_cta",
                 "kernel_ms": ms_roll, "update_kernel_ms": ms_upd,
                 "kernel_share_of_step": ms_roll * p.n_iter / (dev_s / steps * 1e3),
                 "algorithmic_instr_per_sample_step": instr,
@@ -392,6 +392,9 @@ def measure(B, torch, name, rank, steps, warmup, dist, dev, local_rank, closed_l
                 "algorithmic_instr_per_sample_step_pair_blocks": instr_pair,
                 "kernel_ms_no_cull": ms_nocull,
                 "frac_no_cull": None if ms_nocull is None else p.K * p.T * instr / (ms_nocull * 1e-3) / 1e9 / peak,
+                "static_obstacles": None if name not in MPCC else "obstacles at rest take a 10-instruction form of the "
+                           "predictor hinge (dropped terms are exact zeros); frac counts the general 16 per (obstacle, "
+                           "disc) for all of them, as useful work (DESIGN.md 9.2)",
                 "culling": None if ms_nocull is None else "exact (bit-identical results, DESIGN.md 6.5): frac counts "
                            "every (obstacle, disc, step) the method defines as useful work; frac_no_cull is the same "
                            "launch with all of them executed (BRMPPI_FLAG_NO_CULL)",
