@@ -5,12 +5,36 @@
  * Build:  gcc -O2 -std=c11 -fPIC -shared -o liboracle.so brmppi_oracle.c -lm -lpthread
  *         (-ffp-contract=off so that the result does not depend on FMA availability)
  */
-#include "brmppi_oracle.h"
-
 #include <math.h>
 #include <pthread.h>
+#include <stdint.h>
 #include <stdlib.h>
 #include <string.h>
+
+#ifdef ORC_FP32
+/* Reading 23: the fp32 re-run mode.  The SAME source with every `double` a `float`, libm's
+ * single-precision functions and (gcc -fsingle-precision-constant) single-precision literals: what a careful fp32
+ * implementation of these very formulas returns, rounding after every operation.  It exists only so that the tests
+ * can print the fp32 noise floor next to each tolerance (oracle/oracle32.py, tests/test_oracle_fp32_floor.py); the
+ * GPU path is never compared with it, and the fp64 build below is untouched by it.
+ * Build:  gcc -O2 -std=c11 -ffp-contract=off -DORC_FP32 -fsingle-precision-constant -fPIC -shared
+ *             -o liboracle32.so brmppi_oracle.c -lm -lpthread */
+#define double float
+#define cos cosf
+#define sin sinf
+#define tan tanf
+#define sqrt sqrtf
+#define log logf
+#define exp expf
+#define pow powf
+#define fabs fabsf
+#define fmin fminf
+#define fmax fmaxf
+#define rint rintf
+#define floor floorf
+#endif
+
+#include "brmppi_oracle.h"
 
 #ifndef M_PI
 #define M_PI 3.14159265358979323846

@@ -9,8 +9,17 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "brmppi_oracle.c")
-_LIB = os.path.join(_HERE, "liboracle.so")
+# oracle/oracle32.py executes this file a second time with _ORACLE_FP32 set: the same front-end over the fp32 re-run
+# build of the same C source (SURVEY 8(c) reading 23: prints the fp32 noise floor, never a parity reference)
+_FP32 = bool(globals().get("_ORACLE_FP32", False))
+_LIB = os.path.join(_HERE, "liboracle32.so" if _FP32 else "liboracle.so")
+_REAL_C = C.c_float if _FP32 else C.c_double
+_REAL_NP = np.float32 if _FP32 else np.float64
 ORC_MAX_DISCS = 4
+
+
+def _zeros(shape):
+    return np.zeros(shape, dtype=_REAL_NP)
 
 
 def build(force: bool = False) -> str:
@@ -19,44 +28,45 @@ def build(force: bool = False) -> str:
     stale = (not os.path.exists(_LIB)) or any(
         os.path.getmtime(f) > os.path.getmtime(_LIB) for f in (_SRC, hdr))
     if force or stale:
-        cmd = ["gcc", "-O2", "-std=c11", "-ffp-contract=off", "-fPIC", "-shared", "-o", _LIB, _SRC,
-               "-lm", "-lpthread"]
+        mode = ["-DORC_FP32", "-fsingle-precision-constant", "-Wno-overflow"] if _FP32 else []
+        cmd = ["gcc", "-O2", "-std=c11", "-ffp-contract=off"] + mode + ["-fPIC", "-shared", "-o", _LIB, _SRC,
+                                                                      "-lm", "-lpthread"]
         subprocess.check_call(cmd)
     return _LIB
 
 
 class _Params(C.Structure):
     _fields_ = [("K", C.c_int), ("T", C.c_int), ("n_discs", C.c_int),
-                ("disc_body", C.c_int * ORC_MAX_DISCS), ("disc_offset", C.c_double * ORC_MAX_DISCS),
-                ("disc_radius", C.c_double),
-                ("dt", C.c_double), ("L1", C.c_double), ("L2", C.c_double), ("Lh", C.c_double),
-                ("v_min", C.c_double), ("v_max", C.c_double),
-                ("delta_min", C.c_double), ("delta_max", C.c_double),
-                ("sigma_v", C.c_double), ("sigma_delta", C.c_double),
-                ("alpha_lo", C.c_double), ("alpha_hi", C.c_double),
-                ("w_pos", C.c_double), ("w_head", C.c_double), ("w_v", C.c_double),
-                ("w_delta", C.c_double), ("w_hitch", C.c_double), ("hitch_max", C.c_double),
-                ("w_bar", C.c_double), ("w_term", C.c_double), ("lam", C.c_double), ("hitch_kappa", C.c_double),
-                ("hitch_alpha", C.c_double), ("hitch_qv", C.c_double), ("hitch_qdelta", C.c_double),
+                ("disc_body", C.c_int * ORC_MAX_DISCS), ("disc_offset", _REAL_C * ORC_MAX_DISCS),
+                ("disc_radius", _REAL_C),
+                ("dt", _REAL_C), ("L1", _REAL_C), ("L2", _REAL_C), ("Lh", _REAL_C),
+                ("v_min", _REAL_C), ("v_max", _REAL_C),
+                ("delta_min", _REAL_C), ("delta_max", _REAL_C),
+                ("sigma_v", _REAL_C), ("sigma_delta", _REAL_C),
+                ("alpha_lo", _REAL_C), ("alpha_hi", _REAL_C),
+                ("w_pos", _REAL_C), ("w_head", _REAL_C), ("w_v", _REAL_C),
+                ("w_delta", _REAL_C), ("w_hitch", _REAL_C), ("hitch_max", _REAL_C),
+                ("w_bar", _REAL_C), ("w_term", _REAL_C), ("lam", _REAL_C), ("hitch_kappa", _REAL_C),
+                ("hitch_alpha", _REAL_C), ("hitch_qv", _REAL_C), ("hitch_qdelta", _REAL_C),
                 ("seed", C.c_uint64)]
 
 
 class _ProjParams(C.Structure):
-    _fields_ = [("q_v", C.c_double), ("q_omega", C.c_double), ("q_alpha", C.c_double), ("rho", C.c_double),
-                ("sigma_ualpha", C.c_double), ("ualpha_max", C.c_double), ("w_alpha", C.c_double),
-                ("h_buffer", C.c_double)]
+    _fields_ = [("q_v", _REAL_C), ("q_omega", _REAL_C), ("q_alpha", _REAL_C), ("rho", _REAL_C),
+                ("sigma_ualpha", _REAL_C), ("ualpha_max", _REAL_C), ("w_alpha", _REAL_C),
+                ("h_buffer", _REAL_C)]
 
 
 class _MpccParams(C.Structure):
-    _fields_ = [("j_min", C.c_double), ("j_max", C.c_double), ("omega_min", C.c_double), ("omega_max", C.c_double),
-                ("sigma_j", C.c_double), ("sigma_omega", C.c_double), ("delta_lo", C.c_double), ("delta_hi", C.c_double),
-                ("Qc", C.c_double), ("Ql", C.c_double), ("Qth1", C.c_double), ("Qth2", C.c_double),
-                ("Rj", C.c_double), ("Rw", C.c_double), ("mu", C.c_double), ("nu_bar", C.c_double),
-                ("M", C.c_int), ("dpsi", C.c_double), ("coef", C.POINTER(C.c_double))]
+    _fields_ = [("j_min", _REAL_C), ("j_max", _REAL_C), ("omega_min", _REAL_C), ("omega_max", _REAL_C),
+                ("sigma_j", _REAL_C), ("sigma_omega", _REAL_C), ("delta_lo", _REAL_C), ("delta_hi", _REAL_C),
+                ("Qc", _REAL_C), ("Ql", _REAL_C), ("Qth1", _REAL_C), ("Qth2", _REAL_C),
+                ("Rj", _REAL_C), ("Rw", _REAL_C), ("mu", _REAL_C), ("nu_bar", _REAL_C),
+                ("M", C.c_int), ("dpsi", _REAL_C), ("coef", C.POINTER(_REAL_C))]
 
 
 _lib = None
-_dp = C.POINTER(C.c_double)
+_dp = C.POINTER(_REAL_C)
 _u32p = C.POINTER(C.c_uint32)
 
 
@@ -67,41 +77,41 @@ def lib():
         L.orc_philox4x32_10.argtypes = [_u32p, _u32p, _u32p]
         L.orc_philox4x32_10.restype = None
         L.orc_uniform.argtypes = [C.c_uint32]
-        L.orc_uniform.restype = C.c_double
+        L.orc_uniform.restype = _REAL_C
         L.orc_normals.argtypes = [C.c_uint64, C.c_uint32, C.c_uint32, C.c_uint32, _dp]
         L.orc_normals.restype = None
         L.orc_alpha.argtypes = [C.POINTER(_Params), C.c_uint32, C.c_uint32]
-        L.orc_alpha.restype = C.c_double
-        L.orc_wrap.argtypes = [C.c_double]
-        L.orc_wrap.restype = C.c_double
-        L.orc_kinematic_step.argtypes = [C.POINTER(_Params), _dp, C.c_double, C.c_double, _dp]
+        L.orc_alpha.restype = _REAL_C
+        L.orc_wrap.argtypes = [_REAL_C]
+        L.orc_wrap.restype = _REAL_C
+        L.orc_kinematic_step.argtypes = [C.POINTER(_Params), _dp, _REAL_C, _REAL_C, _dp]
         L.orc_kinematic_step.restype = None
         L.orc_disc_centre.argtypes = [C.POINTER(_Params), _dp, C.c_int, _dp]
         L.orc_disc_centre.restype = None
-        L.orc_barrier.argtypes = [C.POINTER(_Params), _dp, _dp, C.c_double]
-        L.orc_barrier.restype = C.c_double
+        L.orc_barrier.argtypes = [C.POINTER(_Params), _dp, _dp, _REAL_C]
+        L.orc_barrier.restype = _REAL_C
         L.orc_goal_cost.argtypes = [C.POINTER(_Params), _dp, _dp]
-        L.orc_goal_cost.restype = C.c_double
-        L.orc_rollout.argtypes = [C.POINTER(_Params), _dp, _dp, C.c_int, _dp, _dp, C.c_double,
+        L.orc_goal_cost.restype = _REAL_C
+        L.orc_rollout.argtypes = [C.POINTER(_Params), _dp, _dp, C.c_int, _dp, _dp, _REAL_C,
                                   _dp, _dp, _dp]
-        L.orc_rollout.restype = C.c_double
+        L.orc_rollout.restype = _REAL_C
         L.orc_sample.argtypes = [C.POINTER(_Params), C.c_uint32, C.c_uint32, _dp, _dp, C.c_int, _dp,
                                  _dp, _dp, _dp]
-        L.orc_sample.restype = C.c_double
-        L.orc_weights_update.argtypes = [C.c_int, C.c_int, C.c_double, _dp, _dp, _dp, _dp,
+        L.orc_sample.restype = _REAL_C
+        L.orc_weights_update.argtypes = [C.c_int, C.c_int, _REAL_C, _dp, _dp, _dp, _dp,
                                          C.POINTER(C.c_int), _dp, _dp]
         L.orc_weights_update.restype = C.c_int
         L.orc_iteration.argtypes = [C.POINTER(_Params), C.c_uint32, _dp, _dp, C.c_int, _dp, _dp,
                                     _dp, _dp, _dp, _dp, _dp, C.POINTER(C.c_int), _dp, _dp, C.c_int]
         L.orc_iteration.restype = C.c_int
         L.orc_barrier_se.argtypes = [C.POINTER(_Params), _dp, _dp, _dp]
-        L.orc_barrier_se.restype = C.c_double
+        L.orc_barrier_se.restype = _REAL_C
         L.orc_rollout_se.argtypes = [C.POINTER(_Params), _dp, _dp, C.c_int, _dp, C.c_int, _dp, _dp,
-                                     C.c_double, _dp, _dp, _dp]
-        L.orc_rollout_se.restype = C.c_double
+                                     _REAL_C, _dp, _dp, _dp]
+        L.orc_rollout_se.restype = _REAL_C
         L.orc_sample_se.argtypes = [C.POINTER(_Params), C.c_uint32, C.c_uint32, _dp, _dp, C.c_int, _dp,
                                     C.c_int, _dp, _dp, _dp, _dp]
-        L.orc_sample_se.restype = C.c_double
+        L.orc_sample_se.restype = _REAL_C
         L.orc_iteration_se.argtypes = [C.POINTER(_Params), C.c_uint32, _dp, _dp, C.c_int, _dp, C.c_int, _dp,
                                        _dp, _dp, _dp, _dp, _dp, _dp, C.POINTER(C.c_int), _dp, _dp, C.c_int]
         L.orc_iteration_se.restype = C.c_int
@@ -111,17 +121,17 @@ def lib():
         L.orc_shift.restype = None
         L.orc_plant_step.argtypes = [C.POINTER(_Params), _dp, _dp, C.c_int, _dp]
         L.orc_plant_step.restype = None
-        L.orc_hitch_barrier.argtypes = [C.POINTER(_Params), _dp, C.c_double]
-        L.orc_hitch_barrier.restype = C.c_double
+        L.orc_hitch_barrier.argtypes = [C.POINTER(_Params), _dp, _REAL_C]
+        L.orc_hitch_barrier.restype = _REAL_C
         L.orc_hitch_rate_cond.argtypes = [C.POINTER(_Params), _dp, _dp]
-        L.orc_hitch_rate_cond.restype = C.c_double
+        L.orc_hitch_rate_cond.restype = _REAL_C
         L.orc_hitch_constraint.argtypes = [C.POINTER(_Params), _dp, _dp, _dp, _dp]
         L.orc_hitch_constraint.restype = None
         L.orc_hitch_filter.argtypes = [C.POINTER(_Params), _dp, _dp, _dp]
         L.orc_hitch_filter.restype = C.c_int
         PP = C.POINTER(_ProjParams)
         ip = C.POINTER(C.c_int)
-        L.orc_project.argtypes = [C.c_int, C.c_int, _dp, _dp, _dp, _dp, C.c_double, _dp, _dp, _dp]
+        L.orc_project.argtypes = [C.c_int, C.c_int, _dp, _dp, _dp, _dp, _REAL_C, _dp, _dp, _dp]
         L.orc_project.restype = C.c_int
         L.orc_ualpha_normals.argtypes = [C.c_uint64, C.c_uint32, C.c_uint32, C.c_uint32, C.c_int, _dp]
         L.orc_ualpha_normals.restype = None
@@ -129,31 +139,31 @@ def lib():
         L.orc_barrier_row.restype = None
         L.orc_affine_step.argtypes = [C.POINTER(_Params), _dp, _dp, _dp]
         L.orc_affine_step.restype = None
-        L.orc_rollout_projected.argtypes = [C.POINTER(_Params), PP, _dp, _dp, C.c_int, _dp, _dp, _dp, C.c_double,
+        L.orc_rollout_projected.argtypes = [C.POINTER(_Params), PP, _dp, _dp, C.c_int, _dp, _dp, _dp, _REAL_C,
                                             _dp, _dp, _dp, _dp, _dp]
-        L.orc_rollout_projected.restype = C.c_double
+        L.orc_rollout_projected.restype = _REAL_C
         L.orc_sample_projected.argtypes = [C.POINTER(_Params), PP, C.c_uint32, C.c_uint32, _dp, _dp, C.c_int, _dp,
                                            _dp, _dp, _dp]
-        L.orc_sample_projected.restype = C.c_double
+        L.orc_sample_projected.restype = _REAL_C
         L.orc_iteration_projected.argtypes = [C.POINTER(_Params), PP, C.c_uint32, _dp, _dp, C.c_int, _dp, _dp,
                                               _dp, _dp, _dp, _dp, _dp, ip, _dp, _dp, C.c_int]
         L.orc_iteration_projected.restype = C.c_int
         MP = C.POINTER(_MpccParams)
         L.orc7_step.argtypes = [C.POINTER(_Params), MP, _dp, _dp, _dp]
         L.orc7_step.restype = None
-        L.orc_path_eval.argtypes = [MP, C.c_double, _dp]
+        L.orc_path_eval.argtypes = [MP, _REAL_C, _dp]
         L.orc_path_eval.restype = None
-        L.orc7_progress.argtypes = [MP, _dp, C.c_double]
-        L.orc7_progress.restype = C.c_double
-        L.orc7_errors.argtypes = [MP, _dp, C.c_double, _dp]
+        L.orc7_progress.argtypes = [MP, _dp, _REAL_C]
+        L.orc7_progress.restype = _REAL_C
+        L.orc7_errors.argtypes = [MP, _dp, _REAL_C, _dp]
         L.orc7_errors.restype = None
         L.orc7_hhat.argtypes = [C.POINTER(_Params), _dp, _dp, _dp, C.c_int, C.c_int, _dp]
-        L.orc7_hhat.restype = C.c_double
-        L.orc7_rollout.argtypes = [C.POINTER(_Params), MP, _dp, C.c_double, C.c_int, _dp, _dp, C.c_double, _dp, _dp]
-        L.orc7_rollout.restype = C.c_double
-        L.orc7_sample.argtypes = [C.POINTER(_Params), MP, C.c_uint32, C.c_uint32, _dp, C.c_double, C.c_int, _dp, _dp, _dp, _dp]
-        L.orc7_sample.restype = C.c_double
-        L.orc7_iteration.argtypes = [C.POINTER(_Params), MP, C.c_uint32, _dp, C.c_double, C.c_int, _dp, _dp, _dp, _dp, _dp,
+        L.orc7_hhat.restype = _REAL_C
+        L.orc7_rollout.argtypes = [C.POINTER(_Params), MP, _dp, _REAL_C, C.c_int, _dp, _dp, _REAL_C, _dp, _dp]
+        L.orc7_rollout.restype = _REAL_C
+        L.orc7_sample.argtypes = [C.POINTER(_Params), MP, C.c_uint32, C.c_uint32, _dp, _REAL_C, C.c_int, _dp, _dp, _dp, _dp]
+        L.orc7_sample.restype = _REAL_C
+        L.orc7_iteration.argtypes = [C.POINTER(_Params), MP, C.c_uint32, _dp, _REAL_C, C.c_int, _dp, _dp, _dp, _dp, _dp,
                                      _dp, _dp, ip, _dp, _dp, C.c_int]
         L.orc7_iteration.restype = C.c_int
         _lib = L
@@ -185,7 +195,7 @@ def _cparams(p) -> _Params:
 
 
 def _d(a, shape=None):
-    a = np.ascontiguousarray(a, dtype=np.float64)
+    a = np.ascontiguousarray(a, dtype=_REAL_NP)
     if shape is not None:
         a = a.reshape(shape)
     return a
@@ -208,7 +218,7 @@ def uniform(w):
 
 
 def normals(seed, n, k, t):
-    z = np.zeros(2)
+    z = _zeros(2)
     lib().orc_normals(int(seed), int(n), int(k), int(t), _ptr(z))
     return z
 
@@ -225,7 +235,7 @@ def wrap(a):
 def kinematic_step(p, x, v, delta):
     cp = _cparams(p)
     x = _d(x, (4,))
-    xn = np.zeros(4)
+    xn = _zeros(4)
     lib().orc_kinematic_step(C.byref(cp), _ptr(x), float(v), float(delta), _ptr(xn))
     return xn
 
@@ -233,7 +243,7 @@ def kinematic_step(p, x, v, delta):
 def disc_centre(p, x, j):
     cp = _cparams(p)
     x = _d(x, (4,))
-    c = np.zeros(2)
+    c = _zeros(2)
     lib().orc_disc_centre(C.byref(cp), _ptr(x), int(j), _ptr(c))
     return c
 
@@ -253,7 +263,7 @@ def goal_cost(p, x, goal):
 def _se(superellipses):
     """(n, 8) float64: cx, cy, m_x, m_y, theta, vx, vy, e."""
     if superellipses is None:
-        return np.zeros((0, 8))
+        return _zeros((0, 8))
     return _d(superellipses).reshape(-1, 8)
 
 
@@ -269,9 +279,9 @@ def rollout(p, x0, goal, obstacles, u, alpha_k, want_traj=False, superellipses=N
     x0, goal = _d(x0, (4,)), _d(goal, (4,))
     obstacles = _d(obstacles).reshape(-1, 5)
     u = _d(u, (p.T, 2))
-    xT = np.zeros(4)
-    traj = np.zeros((p.T + 1, 4)) if want_traj else None
-    pen = C.c_double(0.0)
+    xT = _zeros(4)
+    traj = _zeros((p.T + 1, 4)) if want_traj else None
+    pen = _REAL_C(0.0)
     se = _se(superellipses)
     S = lib().orc_rollout_se(C.byref(cp), _ptr(x0), _ptr(goal), obstacles.shape[0], _ptr(obstacles),
                              se.shape[0], _ptr(se), _ptr(u), float(alpha_k), _ptr(xT),
@@ -285,8 +295,8 @@ def sample(p, n, k, x0, goal, obstacles, U_in, superellipses=None):
     x0, goal = _d(x0, (4,)), _d(goal, (4,))
     obstacles = _d(obstacles).reshape(-1, 5)
     U_in = _d(U_in, (p.T, 2))
-    u = np.zeros((p.T, 2))
-    xT = np.zeros(4)
+    u = _zeros((p.T, 2))
+    xT = _zeros(4)
     se = _se(superellipses)
     S = lib().orc_sample_se(C.byref(cp), int(n), int(k), _ptr(x0), _ptr(goal), obstacles.shape[0],
                             _ptr(obstacles), se.shape[0], _ptr(se), _ptr(U_in), _ptr(u), _ptr(xT))
@@ -299,11 +309,11 @@ def weights_update(S, u, lam):
     K = S.shape[0]
     u = _d(u).reshape(K, -1, 2)
     T = u.shape[1]
-    U = np.zeros((T, 2))
-    w = np.zeros(K)
+    U = _zeros((T, 2))
+    w = _zeros(K)
     am = C.c_int(0)
-    gap = C.c_double(0.0)
-    eta = C.c_double(0.0)
+    gap = _REAL_C(0.0)
+    eta = _REAL_C(0.0)
     nf = lib().orc_weights_update(K, T, float(lam), _ptr(S), _ptr(u), _ptr(U), _ptr(w),
                                   C.byref(am), C.cast(C.byref(gap), _dp),
                                   C.cast(C.byref(eta), _dp))
@@ -318,14 +328,14 @@ def iteration(p, n, x0, goal, obstacles, U_in, n_threads=1, want_samples=False, 
     x0, goal = _d(x0, (4,)), _d(goal, (4,))
     obstacles = _d(obstacles).reshape(-1, 5)
     U_in = _d(U_in, (T, 2))
-    U = np.zeros((T, 2))
-    S = np.zeros(K)
-    XT = np.zeros((K, 4))
-    u = np.zeros((K, T, 2)) if want_samples else None
-    w = np.zeros(K) if want_samples else None
+    U = _zeros((T, 2))
+    S = _zeros(K)
+    XT = _zeros((K, 4))
+    u = _zeros((K, T, 2)) if want_samples else None
+    w = _zeros(K) if want_samples else None
     am = C.c_int(0)
-    gap = C.c_double(0.0)
-    eta = C.c_double(0.0)
+    gap = _REAL_C(0.0)
+    eta = _REAL_C(0.0)
     se = _se(superellipses)
     nf = lib().orc_iteration_se(C.byref(cp), int(n), _ptr(x0), _ptr(goal), obstacles.shape[0],
                              _ptr(obstacles), se.shape[0], _ptr(se), _ptr(U_in), _ptr(U), _ptr(S), _ptr(XT),
@@ -383,8 +393,8 @@ def hitch_rate_cond(p, x, u):
 
 def hitch_constraint(p, x, u_ref):
     """(c0, a): c(u) ~ c0 + a . (u - u_ref), reading 28."""
-    c0 = C.c_double()
-    a = np.zeros(2)
+    c0 = _REAL_C()
+    a = _zeros(2)
     lib().orc_hitch_constraint(C.byref(_cparams(p)), _ptr(_d(x, (4,))), _ptr(_d(u_ref, (2,))),
                                C.byref(c0), _ptr(a))
     return c0.value, a
@@ -392,7 +402,7 @@ def hitch_constraint(p, x, u_ref):
 
 def hitch_filter(p, x, u_ref):
     """CBF-QP of Sec. V-D: (u*, status)."""
-    u = np.zeros(2)
+    u = _zeros(2)
     st = lib().orc_hitch_filter(C.byref(_cparams(p)), _ptr(_d(x, (4,))), _ptr(_d(u_ref, (2,))), _ptr(u))
     return u, int(st)
 
@@ -402,29 +412,29 @@ def project(A, b, z_des, w, rho, z_lo, z_hi):
     """Eq. (12) by the C oracle: (z*, number of dropped rows)."""
     A = _d(A)
     m, d = A.shape
-    z = np.zeros(d)
+    z = _zeros(d)
     dropped = lib().orc_project(m, d, _ptr(A), _ptr(_d(b, (m,))), _ptr(_d(z_des, (d,))), _ptr(_d(w, (d,))),
                                 float(rho), _ptr(_d(z_lo, (d,))), _ptr(_d(z_hi, (d,))), _ptr(z))
     return z, int(dropped)
 
 
 def ualpha_normals(seed, n, k, t, n_obs):
-    z = np.zeros(max(n_obs, 1))
+    z = _zeros(max(n_obs, 1))
     lib().orc_ualpha_normals(int(seed) & 0xFFFFFFFFFFFFFFFF, int(n), int(k), int(t), int(n_obs), _ptr(z))
     return z[:n_obs]
 
 
 def barrier_row(p, x, obstacle, t):
     """(h, active disc, L_g h [2], L_f h) of one obstacle at state x, step t."""
-    h, Lf, j = C.c_double(), C.c_double(), C.c_int()
-    Lg = np.zeros(2)
+    h, Lf, j = _REAL_C(), _REAL_C(), C.c_int()
+    Lg = _zeros(2)
     lib().orc_barrier_row(C.byref(_cparams(p)), _ptr(_d(x, (4,))), _ptr(_d(obstacle, (5,))), int(t), C.byref(h),
                           C.byref(j), _ptr(Lg), C.byref(Lf))
     return h.value, j.value, Lg, Lf.value
 
 
 def affine_step(p, x, w):
-    xn = np.zeros(4)
+    xn = _zeros(4)
     lib().orc_affine_step(C.byref(_cparams(p)), _ptr(_d(x, (4,))), _ptr(_d(w, (2,))), _ptr(xn))
     return xn
 
@@ -433,11 +443,11 @@ def rollout_projected(p, x0, goal, obstacles, u, ualpha, alpha0):
     obs = _d(obstacles).reshape(-1, 5)
     n_obs, T = obs.shape[0], p.T
     u = _d(u, (T, 2))
-    ua = _d(ualpha).reshape(T, n_obs) if n_obs else np.zeros((T, 1))
-    xT, traj = np.zeros(4), np.zeros((T + 1, 4))
-    z = np.zeros((T, 2 + n_obs))
-    al = np.zeros((T + 1, max(n_obs, 1)))
-    Ab = np.zeros((T, max(n_obs, 1), 4))
+    ua = _d(ualpha).reshape(T, n_obs) if n_obs else _zeros((T, 1))
+    xT, traj = _zeros(4), _zeros((T + 1, 4))
+    z = _zeros((T, 2 + n_obs))
+    al = _zeros((T + 1, max(n_obs, 1)))
+    Ab = _zeros((T, max(n_obs, 1), 4))
     S = lib().orc_rollout_projected(C.byref(_cparams(p)), C.byref(_pparams(p)), _ptr(_d(x0, (4,))), _ptr(_d(goal, (4,))),
                                     n_obs, _ptr(obs), _ptr(u), _ptr(ua), float(alpha0), _ptr(xT), _ptr(traj), _ptr(z),
                                     _ptr(al), _ptr(Ab))
@@ -446,7 +456,7 @@ def rollout_projected(p, x0, goal, obstacles, u, ualpha, alpha0):
 
 def sample_projected(p, n, k, x0, goal, obstacles, U_in):
     obs = _d(obstacles).reshape(-1, 5)
-    u, xT = np.zeros((p.T, 2)), np.zeros(4)
+    u, xT = _zeros((p.T, 2)), _zeros(4)
     S = lib().orc_sample_projected(C.byref(_cparams(p)), C.byref(_pparams(p)), int(n), int(k), _ptr(_d(x0, (4,))),
                                    _ptr(_d(goal, (4,))), obs.shape[0], _ptr(obs), _ptr(_d(U_in, (p.T, 2))), _ptr(u), _ptr(xT))
     return dict(S=S, u=u, xT=xT)
@@ -455,9 +465,9 @@ def sample_projected(p, n, k, x0, goal, obstacles, U_in):
 def iteration_projected(p, n, x0, goal, obstacles, U_in, n_threads=1, want_samples=False):
     obs = _d(obstacles).reshape(-1, 5)
     K, T = p.K, p.T
-    U_out, S, XT, w = np.zeros((T, 2)), np.zeros(K), np.zeros((K, 4)), np.zeros(K)
-    u_all = np.zeros((K, T, 2))
-    argmin, gap, eta = C.c_int(), C.c_double(), C.c_double()
+    U_out, S, XT, w = _zeros((T, 2)), _zeros(K), _zeros((K, 4)), _zeros(K)
+    u_all = _zeros((K, T, 2))
+    argmin, gap, eta = C.c_int(), _REAL_C(), _REAL_C()
     nonfinite = lib().orc_iteration_projected(C.byref(_cparams(p)), C.byref(_pparams(p)), int(n), _ptr(_d(x0, (4,))),
                                               _ptr(_d(goal, (4,))), obs.shape[0], _ptr(obs), _ptr(_d(U_in, (T, 2))),
                                               _ptr(U_out), _ptr(S), _ptr(XT), _ptr(u_all), _ptr(w), C.byref(argmin),
@@ -495,14 +505,14 @@ def _mparams(p, coef, dpsi):
 
 def step7(p, coef, dpsi, x, u):
     mp, keep = _mparams(p, coef, dpsi)
-    xn = np.zeros(7)
+    xn = _zeros(7)
     lib().orc7_step(C.byref(_cparams(p)), C.byref(mp), _ptr(_d(x, (7,))), _ptr(_d(u, (2,))), _ptr(xn))
     return xn
 
 
 def path_eval(p, coef, dpsi, psi):
     mp, keep = _mparams(p, coef, dpsi)
-    out = np.zeros(4)
+    out = _zeros(4)
     lib().orc_path_eval(C.byref(mp), float(psi), _ptr(out))
     return out
 
@@ -514,14 +524,14 @@ def progress7(p, coef, dpsi, x, psi):
 
 def errors7(p, coef, dpsi, x, psi):
     mp, keep = _mparams(p, coef, dpsi)
-    e = np.zeros(4)
+    e = _zeros(4)
     lib().orc7_errors(C.byref(mp), _ptr(_d(x, (7,))), float(psi), _ptr(e))
     return e
 
 
 def hhat7(p, x, u, obstacle, t, j):
     """(hhat, h) of eq. (17) for disc j against one obstacle at step t."""
-    h = C.c_double()
+    h = _REAL_C()
     hh = lib().orc7_hhat(C.byref(_cparams(p)), _ptr(_d(x, (7,))), _ptr(_d(u, (2,))), _ptr(_d(obstacle, (5,))), int(t), int(j),
                          C.byref(h))
     return hh, h.value
@@ -530,7 +540,7 @@ def hhat7(p, x, u, obstacle, t, j):
 def rollout7(p, coef, dpsi, x0, psi0, obstacles, u, alpha):
     mp, keep = _mparams(p, coef, dpsi)
     obs = _d(obstacles).reshape(-1, 5)
-    xT, traj = np.zeros(8), np.zeros((p.T + 1, 8))
+    xT, traj = _zeros(8), _zeros((p.T + 1, 8))
     S = lib().orc7_rollout(C.byref(_cparams(p)), C.byref(mp), _ptr(_d(x0, (7,))), float(psi0), obs.shape[0], _ptr(obs),
                            _ptr(_d(u, (p.T, 2))), float(alpha), _ptr(xT), _ptr(traj))
     return dict(S=S, xT=xT, traj=traj)
@@ -539,7 +549,7 @@ def rollout7(p, coef, dpsi, x0, psi0, obstacles, u, alpha):
 def sample7(p, coef, dpsi, n, k, x0, psi0, obstacles, U_in):
     mp, keep = _mparams(p, coef, dpsi)
     obs = _d(obstacles).reshape(-1, 5)
-    u, xT = np.zeros((p.T, 2)), np.zeros(8)
+    u, xT = _zeros((p.T, 2)), _zeros(8)
     S = lib().orc7_sample(C.byref(_cparams(p)), C.byref(mp), int(n), int(k), _ptr(_d(x0, (7,))), float(psi0), obs.shape[0],
                           _ptr(obs), _ptr(_d(U_in, (p.T, 2))), _ptr(u), _ptr(xT))
     return dict(S=S, u=u, xT=xT)
@@ -549,9 +559,9 @@ def iteration7(p, coef, dpsi, n, x0, psi0, obstacles, U_in, n_threads=1, want_sa
     mp, keep = _mparams(p, coef, dpsi)
     obs = _d(obstacles).reshape(-1, 5)
     K, T = p.K, p.T
-    U_out, S, XT, w = np.zeros((T, 2)), np.zeros(K), np.zeros((K, 8)), np.zeros(K)
-    u_all = np.zeros((K, T, 2))
-    argmin, gap, eta = C.c_int(), C.c_double(), C.c_double()
+    U_out, S, XT, w = _zeros((T, 2)), _zeros(K), _zeros((K, 8)), _zeros(K)
+    u_all = _zeros((K, T, 2))
+    argmin, gap, eta = C.c_int(), _REAL_C(), _REAL_C()
     nonfinite = lib().orc7_iteration(C.byref(_cparams(p)), C.byref(mp), int(n), _ptr(_d(x0, (7,))), float(psi0), obs.shape[0],
                                      _ptr(obs), _ptr(_d(U_in, (T, 2))), _ptr(U_out), _ptr(S), _ptr(XT), _ptr(u_all), _ptr(w),
                                      C.byref(argmin), C.byref(gap), C.byref(eta), int(n_threads))
