@@ -359,8 +359,9 @@ def measure(B, torch, name, rank, steps, warmup, dist, dev, local_rank, closed_l
         solver.set_nominal(None)
         ms_roll, ms_upd = solver.time_kernels(50)
         ms_nocull = None
-        if name not in THREAD_PER_SAMPLE:                    # the same launch with every (obstacle, disc, step) evaluated
-            s2 = B.Solver(p, 1, max(n_obs, 1), solver_flags(B, name, no_cull=True), device=dev, max_superellipses=n_se)
+        if name not in PROJECTED:                            # the same launch with every (obstacle, disc, step) evaluated
+            s2 = B.Solver(p, 1, max(n_obs, 1), solver_flags(B, name, no_cull=True), device=dev, max_superellipses=n_se,
+                          max_path_segments=n_seg)
             s2.set_scene(sc)
             for _ in range(3):
                 s2.solve()

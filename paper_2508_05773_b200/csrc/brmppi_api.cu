@@ -379,6 +379,9 @@ int brmppi_create(const brmppi_params* p, void* dev_workspace, size_t workspace_
     d.dstate_lo = p->delta_min; d.dstate_hi = p->delta_max;
     d.Qc = p->Qc; d.Ql = p->Ql; d.Qth1 = p->Qth1; d.Qth2 = p->Qth2; d.Rj = p->Rj; d.Rw = p->Rw;
     d.mu = p->mu; d.nu_bar = p->nu_bar; d.max_path_segments = p->max_path_segments;
+    d.mpcc_lmax = 0.0f;
+    for (int j = 0; j < p->n_discs; ++j)
+      d.mpcc_lmax = std::fmax(d.mpcc_lmax, std::fabs(d.disc_a1[j] - p->Lh) + std::fabs(d.disc_a2[j]));
   }
   d.alpha_lo = p->alpha_lo; d.alpha_span = p->alpha_hi - p->alpha_lo;
   d.w_pos = p->w_pos; d.w_head = p->w_head; d.w_v = p->w_v; d.w_delta = p->w_delta;

@@ -39,6 +39,7 @@ struct DeviceParams {
   float dstate_lo, dstate_hi;  // clamp of the steering STATE delta
   float Qc, Ql, Qth1, Qth2, Rj, Rw, mu, nu_bar;
   int max_path_segments;
+  float mpcc_lmax;             // longest lever of a disc centre about the reference point, |a1 - Lh| + |a2| (culling)
   int mpcc_noise_planes;       // rollout_mpcc_cta: the tile's sampled controls are kept in shared memory
   uint32_t key0, key1;        // Philox key of scene 0 = (lo32(seed), hi32(seed)); scene s adds s
   uint32_t flags;

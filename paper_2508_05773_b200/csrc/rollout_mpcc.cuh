@@ -92,11 +92,20 @@ __device__ __forceinline__ MpccRates mpcc_rates(const DeviceParams& P, float v, 
 // general form; [n_moving, n_obs) must be at rest (zero velocity: the caller's table is ordered that way), for
 // which e = v_disc and g = f, so that the bracket is alpha |d|^2 + d.f + |v_disc|^2 -- the same value (every
 // dropped term is an exact zero), ten instructions per (obstacle, disc) instead of sixteen.
+//
+// Exact culling (inv_alpha_cull > 0; the phase-split kernel unless BRMPPI_FLAG_NO_CULL): the bracket of disc j is
+// Q = alpha |d|^2 + d.g + |e|^2 >= alpha |d|^2 - |d| |g| with g = f_j - 2 Ts o', so for alpha > 0 the hinge
+// max(0, alpha - Q / rho^2) is zero whenever |d| >= rho + |g| / alpha (then alpha |d| (|d| - |g| / alpha) >=
+// alpha rho |d| >= alpha rho^2).  With D = |p - o| the distance of the vehicle's reference point, l_max the longest
+// lever (|d_j| >= D - l_max) and G = max_j (|f_jx| + |f_jy|) >= |f_j|, an obstacle contributes nothing to ANY disc
+// if D >= l_max + rho + (G + 2 |Ts o'|) / alpha.  The table carries (l_max + rho) and 2 |Ts o'| with a 0.1 % + 1 mm
+// margin that covers the fp32 rounding of the test and of Q; an obstacle is skipped only when every active lane of
+// the warp agrees (the samples of a warp sit at the same step, close together), so the result is bit-identical.
 template <int ND>
 __device__ __forceinline__ float mpcc_hinge(const DeviceParams& P, const float4* __restrict__ sObs,
                                             const float4* __restrict__ sVel, int n_moving, int n_obs, int nd, float tf,
                                             float alpha, float x, float y, float vh, float ah, float s1, float c1,
-                                            float s2, float c2, const MpccRates& R) {
+                                            float s2, float c2, const MpccRates& R, float inv_alpha_cull = 0.0f) {
   // centre, velocity and f = 2 v + acc of disc j are affine in its lever arms (l1, l2): c = p + l1 e1 + l2 e2,
   // v = vh e1 + l1 W1 n1 + l2 W2 n2, acc = (ah e1 + vh W1 n1) + l1 (W1dot n1 - W1^2 e1) + l2 (W2dot n2 - W2^2 e2)
   // with e = (cos, sin), n = (-sin, cos) of the two headings; the six vectors are shared by all discs
@@ -115,11 +124,23 @@ __device__ __forceinline__ float mpcc_hinge(const DeviceParams& P, const float4*
     fx[j] = fmaf(l1, f1x, fmaf(l2, f2x, f0x));
     fy[j] = fmaf(l1, f1y, fmaf(l2, f2y, f0y));
   }
+  const bool cull = inv_alpha_cull > 0.0f;
+  float Gv = 0.0f;
+  if (cull) {
+#pragma unroll
+    for (int j = 0; j < ND; ++j)
+      if (j < nd) Gv = fmaxf(Gv, fabsf(fx[j]) + fabsf(fy[j]));
+  }
   float pen = 0.0f;
   for (int i = 0; i < n_moving; ++i) {
     const float4 o = sObs[i];
-    const float4 w = sVel[i];                                  // (Ts vx, Ts vy, ...): the obstacle's step
+    const float4 w = sVel[i];                                  // (Ts vx, Ts vy, 2 |Ts o'|, -): the obstacle's step
     const float ox = fmaf(tf, w.x, o.x), oy = fmaf(tf, w.y, o.y);
+    if (cull) {
+      const float ddx = x - ox, ddy = y - oy, thr = fmaf(w.z + Gv, inv_alpha_cull, o.w);
+      const bool far = fmaf(ddx, ddx, ddy * ddy) >= thr * thr;          // false on NaN
+      if (__all_sync(__activemask(), far)) continue;
+    }
 #pragma unroll
     for (int j = 0; j < ND; ++j) {
       if (j < nd) {
@@ -138,6 +159,11 @@ __device__ __forceinline__ float mpcc_hinge(const DeviceParams& P, const float4*
     for (int j = 0; j < ND; ++j) vv[j] = fmaf(vx[j], vx[j], vy[j] * vy[j]);
     for (int i = n_moving; i < n_obs; ++i) {
       const float4 o = sObs[i];
+      if (cull) {
+        const float ddx = x - o.x, ddy = y - o.y, thr = fmaf(Gv, inv_alpha_cull, o.w);
+        const bool far = fmaf(ddx, ddx, ddy * ddy) >= thr * thr;
+        if (__all_sync(__activemask(), far)) continue;
+      }
 #pragma unroll
       for (int j = 0; j < ND; ++j) {
         if (j < nd) {

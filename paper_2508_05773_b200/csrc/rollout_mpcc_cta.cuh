@@ -92,15 +92,15 @@ template <int ND>
 __device__ __forceinline__ double mpcc_cost_item(const DeviceParams& P, const float4* __restrict__ sObs,
                                                  const float4* __restrict__ sVel, const float4* __restrict__ sPath,
                                                  int n_moving, int n_obs, int M, float dpsi, float inv_dpsi, const float4* row0,
-                                                 const float4* row1, int st, int t, float alpha, bool u_in_row,
-                                                 float2 u, float* track) {
+                                                 const float4* row1, int st, int t, float alpha, float inv_alpha_cull,
+                                                 bool u_in_row, float2 u, float* track) {
   const float4 q0 = row0[0], q1 = row0[st];                                     // (x, y, v, a), (s1, c1, s2, c2)
   const float td = row0[2 * st].x;
   if (u_in_row) { const float4 q3 = row0[3 * st]; u = make_float2(q3.z, q3.w); }
   const float vh = P.dt * q0.z, ah = P.dt * P.dt * q0.w;                         // step units (mpcc_hinge)
   const MpccRates R = mpcc_rates(P, vh, ah, td, q1.x, q1.y, q1.z, q1.w, P.dt * u.y);
   const float pen = mpcc_hinge<ND>(P, sObs, sVel, n_moving, n_obs, ND, (float)t, alpha, q0.x, q0.y, vh, ah, q1.x, q1.y,
-                                   q1.z, q1.w, R);
+                                   q1.z, q1.w, R, inv_alpha_cull);
   // stage cost (13) on (x_{t+1}, u_t, psi_{t+1}): the next row
   const float4 n0 = row1[0], n1 = row1[st], n2 = row1[2 * st], n3 = row1[3 * st];
   float nu;
@@ -179,8 +179,10 @@ rollout_mpcc_cta(const __grid_constant__ DeviceParams P) {
         }
         const int slot = mov ? before_same : n_mov + before_same;
         const float rho = ob[2] + P.disc_radius;
-        sObs[slot] = make_float4(ob[0] - x0, ob[1] - y0, 1.0f / (rho * rho), 0.0f);   // vehicle-centred frame
-        sVel[slot] = make_float4(P.dt * ob[3], P.dt * ob[4], ob[3], ob[4]);
+        // vehicle-centred frame; .w and .z of the two entries: the culling radii of mpcc_hinge, with their margin
+        sObs[slot] = make_float4(ob[0] - x0, ob[1] - y0, 1.0f / (rho * rho), fmaf(1.001f, P.mpcc_lmax + rho, 1e-3f));
+        sVel[slot] = make_float4(P.dt * ob[3], P.dt * ob[4],
+                                 2.0f * P.dt * sqrtf(fmaf(ob[3], ob[3], ob[4] * ob[4])), 0.0f);
       }
       for (int i = tid; i < 4 * M; i += kMpccThreads) {
         float4 c = reinterpret_cast<const float4*>(P.path_coef)[(size_t)scene * 4 * P.max_path_segments + i];
@@ -275,6 +277,8 @@ rollout_mpcc_cta(const __grid_constant__ DeviceParams P) {
       const float alpha = sample_alpha(P, n, (uint32_t)(kk + P.k_offset), key0, key1);
       int n_moving = 0;
       for (int i = 0; i < n_obs; ++i) n_moving += (sVel[i].x != 0.0f || sVel[i].y != 0.0f) ? 1 : 0;
+      // exact culling of far obstacles (mpcc_hinge): off for alpha <= 0 and under BRMPPI_FLAG_NO_CULL
+      const float inv_alpha_cull = (alpha > 0.0f && !(P.flags & BRMPPI_FLAG_NO_CULL)) ? 1.001f / alpha : 0.0f;
       double acc = 0.0;
       for (int c = 0; c < n_chunks; ++c) {
         const uint32_t gg = g + (uint32_t)c;
@@ -287,7 +291,7 @@ rollout_mpcc_cta(const __grid_constant__ DeviceParams P) {
             float track;
             const float4* row0 = sPlanes + slot * slot_quads + r * row_quads + s;
             acc += mpcc_cost_item<ND>(P, sObs, sVel, sPath, n_moving, n_obs, M, dpsi, inv_dpsi, row0, row0 + row_quads, st, t,
-                                      alpha, true, make_float2(0.0f, 0.0f), &track);
+                                      alpha, inv_alpha_cull, true, make_float2(0.0f, 0.0f), &track);
             if (t == T - 1) acc += (double)(P.w_term * track);       // terminal cost: the same four terms at (x_N, psi_N)
           }
         }

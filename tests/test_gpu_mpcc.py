@@ -172,6 +172,30 @@ def test_long_horizon_without_control_planes(B, O):
     check(O, gpu_mpcc(B, sc, sc.params), sc, sc.params)
 
 
+@pytest.mark.parametrize("case", ["recipe", "near", "alpha_from_zero", "fast_far_obstacles"])
+def test_culling_is_bit_exact(B, case):
+    """The phase-split kernel skips obstacles that provably add nothing (mpcc_hinge): S_k, x_T and U must be
+    bit-identical to the same launch with every (obstacle, disc, step) evaluated (BRMPPI_FLAG_NO_CULL)."""
+    if case == "recipe":
+        sc = scenes.scene_mpcc(2, K=3000, T=80, dt=0.05, n_obs=8, M=16)
+        sc = scenes.PathScene(sc.x0, sc.psi0, sc.obstacles, sc.coef, sc.dpsi, sc.params.with_(n_iter=1), sc.name)
+    elif case == "near":
+        sc = path_scene(8, 8, K=3000, T=40)
+    elif case == "alpha_from_zero":
+        sc = path_scene(3, 6, K=3000, T=40, alpha_lo=0.0, alpha_hi=0.05)
+    else:       # far obstacles that close in fast: 2 |Ts o'| / alpha must keep them in
+        sc = path_scene(8, 8, K=3000, T=60)
+        sc.obstacles[:, :2] += np.float32(25.0)
+        sc.obstacles[:, 3:] = np.float32(-9.0)
+    a = gpu_mpcc(B, sc, sc.params)
+    b = gpu_mpcc(B, sc, sc.params, B.FLAG_NO_CULL)
+    assert np.array_equal(a["S"], b["S"]) and np.array_equal(a["XT"], b["XT"]) and np.array_equal(a["U"], b["U"])
+    assert a["diag"]["argmin"] == b["diag"]["argmin"]
+    if case != "recipe":      # the case is not vacuous: some hinge is active somewhere
+        free = scenes.PathScene(sc.x0, sc.psi0, np.zeros((0, 5)), sc.coef, sc.dpsi, sc.params, sc.name)
+        assert (a["S"] > gpu_mpcc(B, free, sc.params)["S"] + 1e-3).any()
+
+
 def test_warm_nominal_moving_obstacles_off_axle_hitch_four_discs(B, O, kern):
     discs = ((0, 0.0), (0, 2.5), (1, -2.0), (1, -4.5))
     sc = path_scene(6, 6, K=800, T=50, Lh=0.75, discs=discs, nu_bar=2.5, hitch_kappa=0.05, alpha_lo=0.0, alpha_hi=1.0)
