@@ -211,7 +211,7 @@ int launch_rollout(brmppi_ctx* c) {
   if (c->plan.cta_kernel) {
     CU(launch_rollout_cta(d, c->plan.cta, precise, c->stream));
   } else if (c->plan.mpcc_cta) {
-    mpcc_cta_kernel_for(precise, d.n_discs)<<<(unsigned)c->plan.mpcc.grid, kMpccThreads, c->smem_rollout, c->stream>>>(d);
+    mpcc_cta_kernel_for(precise, d.n_discs, !(c->p.flags & BRMPPI_FLAG_NO_CULL))<<<(unsigned)c->plan.mpcc.grid, kMpccThreads, c->smem_rollout, c->stream>>>(d);
     CU(cudaGetLastError());
   } else if (c->p.flags & BRMPPI_FLAG_MPCC) {
     dim3 grid((unsigned)c->plan.n_partials, (unsigned)d.n_scenes);
@@ -437,7 +437,8 @@ int brmppi_create(const brmppi_params* p, void* dev_workspace, size_t workspace_
     e = configure_rollout_cta((p->flags & BRMPPI_FLAG_PRECISE_MATH) != 0, p->n_discs, c->smem_rollout);
   } else if (c->plan.mpcc_cta) {
     c->smem_rollout = c->plan.mpcc.smem;
-    e = cudaFuncSetAttribute(mpcc_cta_kernel_for((p->flags & BRMPPI_FLAG_PRECISE_MATH) != 0, p->n_discs),
+    e = cudaFuncSetAttribute(mpcc_cta_kernel_for((p->flags & BRMPPI_FLAG_PRECISE_MATH) != 0, p->n_discs,
+                                                 !(p->flags & BRMPPI_FLAG_NO_CULL)),
                              cudaFuncAttributeMaxDynamicSharedMemorySize, (int)prop.sharedMemPerBlockOptin);
   } else {
     c->smem_rollout = (p->flags & BRMPPI_FLAG_PROJECTED) ? rollout_projected_smem_bytes(d)

@@ -101,7 +101,7 @@ __device__ __forceinline__ MpccRates mpcc_rates(const DeviceParams& P, float v, 
 // if D >= l_max + rho + (G + 2 |Ts o'|) / alpha.  The table carries (l_max + rho) and 2 |Ts o'| with a 0.1 % + 1 mm
 // margin that covers the fp32 rounding of the test and of Q; an obstacle is skipped only when every active lane of
 // the warp agrees (the samples of a warp sit at the same step, close together), so the result is bit-identical.
-template <int ND>
+template <int ND, bool CULL = false>
 __device__ __forceinline__ float mpcc_hinge(const DeviceParams& P, const float4* __restrict__ sObs,
                                             const float4* __restrict__ sVel, int n_moving, int n_obs, int nd, float tf,
                                             float alpha, float x, float y, float vh, float ah, float s1, float c1,
@@ -124,9 +124,9 @@ __device__ __forceinline__ float mpcc_hinge(const DeviceParams& P, const float4*
     fx[j] = fmaf(l1, f1x, fmaf(l2, f2x, f0x));
     fy[j] = fmaf(l1, f1y, fmaf(l2, f2y, f0y));
   }
-  const bool cull = inv_alpha_cull > 0.0f;
+  const bool cull = CULL && inv_alpha_cull > 0.0f;
   float Gv = 0.0f;
-  if (cull) {
+  if (CULL && cull) {
 #pragma unroll
     for (int j = 0; j < ND; ++j)
       if (j < nd) Gv = fmaxf(Gv, fabsf(fx[j]) + fabsf(fy[j]));
@@ -136,7 +136,7 @@ __device__ __forceinline__ float mpcc_hinge(const DeviceParams& P, const float4*
     const float4 o = sObs[i];
     const float4 w = sVel[i];                                  // (Ts vx, Ts vy, 2 |Ts o'|, -): the obstacle's step
     const float ox = fmaf(tf, w.x, o.x), oy = fmaf(tf, w.y, o.y);
-    if (cull) {
+    if (CULL && cull) {
       const float ddx = x - ox, ddy = y - oy, thr = fmaf(w.z + Gv, inv_alpha_cull, o.w);
       const bool far = fmaf(ddx, ddx, ddy * ddy) >= thr * thr;          // false on NaN
       if (__all_sync(__activemask(), far)) continue;
@@ -159,7 +159,7 @@ __device__ __forceinline__ float mpcc_hinge(const DeviceParams& P, const float4*
     for (int j = 0; j < ND; ++j) vv[j] = fmaf(vx[j], vx[j], vy[j] * vy[j]);
     for (int i = n_moving; i < n_obs; ++i) {
       const float4 o = sObs[i];
-      if (cull) {
+      if (CULL && cull) {
         const float ddx = x - o.x, ddy = y - o.y, thr = fmaf(Gv, inv_alpha_cull, o.w);
         const bool far = fmaf(ddx, ddx, ddy * ddy) >= thr * thr;
         if (__all_sync(__activemask(), far)) continue;

@@ -88,7 +88,7 @@ inline MpccCtaPlan make_mpcc_cta_plan(int K, int T, int n_scenes, int max_obstac
 // One (sample, step) item of the cost phase: everything of step t that is not the state recursion.  Returns the
 // stage cost (13) with the barrier term; *track = the four tracking terms at (x_{t+1}, psi_{t+1}).  row0 / row1:
 // quad 0 of rows t and t + 1, already offset by the sample; st = plane stride (in float4).
-template <int ND>
+template <int ND, bool CULL>
 __device__ __forceinline__ double mpcc_cost_item(const DeviceParams& P, const float4* __restrict__ sObs,
                                                  const float4* __restrict__ sVel, const float4* __restrict__ sPath,
                                                  int n_moving, int n_obs, int M, float dpsi, float inv_dpsi, const float4* row0,
@@ -99,7 +99,7 @@ __device__ __forceinline__ double mpcc_cost_item(const DeviceParams& P, const fl
   if (u_in_row) { const float4 q3 = row0[3 * st]; u = make_float2(q3.z, q3.w); }
   const float vh = P.dt * q0.z, ah = P.dt * P.dt * q0.w;                         // step units (mpcc_hinge)
   const MpccRates R = mpcc_rates(P, vh, ah, td, q1.x, q1.y, q1.z, q1.w, P.dt * u.y);
-  const float pen = mpcc_hinge<ND>(P, sObs, sVel, n_moving, n_obs, ND, (float)t, alpha, q0.x, q0.y, vh, ah, q1.x, q1.y,
+  const float pen = mpcc_hinge<ND, CULL>(P, sObs, sVel, n_moving, n_obs, ND, (float)t, alpha, q0.x, q0.y, vh, ah, q1.x, q1.y,
                                    q1.z, q1.w, R, inv_alpha_cull);
   // stage cost (13) on (x_{t+1}, u_t, psi_{t+1}): the next row
   const float4 n0 = row1[0], n1 = row1[st], n2 = row1[2 * st], n3 = row1[3 * st];
@@ -110,7 +110,7 @@ __device__ __forceinline__ double mpcc_cost_item(const DeviceParams& P, const fl
   return (double)stage + (double)P.w_bar * (double)pen;
 }
 
-template <bool PRECISE, int ND>
+template <bool PRECISE, int ND, bool CULL>
 __global__ void __launch_bounds__(kMpccThreads, 1)
 rollout_mpcc_cta(const __grid_constant__ DeviceParams P) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -278,7 +278,7 @@ rollout_mpcc_cta(const __grid_constant__ DeviceParams P) {
       int n_moving = 0;
       for (int i = 0; i < n_obs; ++i) n_moving += (sVel[i].x != 0.0f || sVel[i].y != 0.0f) ? 1 : 0;
       // exact culling of far obstacles (mpcc_hinge): off for alpha <= 0 and under BRMPPI_FLAG_NO_CULL
-      const float inv_alpha_cull = (alpha > 0.0f && !(P.flags & BRMPPI_FLAG_NO_CULL)) ? 1.001f / alpha : 0.0f;
+      const float inv_alpha_cull = (CULL && alpha > 0.0f) ? 1.001f / alpha : 0.0f;
       double acc = 0.0;
       for (int c = 0; c < n_chunks; ++c) {
         const uint32_t gg = g + (uint32_t)c;
@@ -290,7 +290,7 @@ rollout_mpcc_cta(const __grid_constant__ DeviceParams P) {
           if (t < T) {
             float track;
             const float4* row0 = sPlanes + slot * slot_quads + r * row_quads + s;
-            acc += mpcc_cost_item<ND>(P, sObs, sVel, sPath, n_moving, n_obs, M, dpsi, inv_dpsi, row0, row0 + row_quads, st, t,
+            acc += mpcc_cost_item<ND, CULL>(P, sObs, sVel, sPath, n_moving, n_obs, M, dpsi, inv_dpsi, row0, row0 + row_quads, st, t,
                                       alpha, inv_alpha_cull, true, make_float2(0.0f, 0.0f), &track);
             if (t == T - 1) acc += (double)(P.w_term * track);       // terminal cost: the same four terms at (x_N, psi_N)
           }
@@ -398,13 +398,19 @@ rollout_mpcc_cta(const __grid_constant__ DeviceParams P) {
 
 typedef void (*MpccCtaKernel)(const DeviceParams);
 
-inline MpccCtaKernel mpcc_cta_kernel_for(bool precise, int n_discs) {
+template <bool CULL>
+inline MpccCtaKernel mpcc_cta_kernel_pick(bool precise, int n_discs) {
   switch (n_discs) {
-    case 1: return precise ? rollout_mpcc_cta<true, 1> : rollout_mpcc_cta<false, 1>;
-    case 2: return precise ? rollout_mpcc_cta<true, 2> : rollout_mpcc_cta<false, 2>;
-    case 3: return precise ? rollout_mpcc_cta<true, 3> : rollout_mpcc_cta<false, 3>;
-    default: return precise ? rollout_mpcc_cta<true, 4> : rollout_mpcc_cta<false, 4>;
+    case 1: return precise ? rollout_mpcc_cta<true, 1, CULL> : rollout_mpcc_cta<false, 1, CULL>;
+    case 2: return precise ? rollout_mpcc_cta<true, 2, CULL> : rollout_mpcc_cta<false, 2, CULL>;
+    case 3: return precise ? rollout_mpcc_cta<true, 3, CULL> : rollout_mpcc_cta<false, 3, CULL>;
+    default: return precise ? rollout_mpcc_cta<true, 4, CULL> : rollout_mpcc_cta<false, 4, CULL>;
   }
+}
+
+// cull = false (BRMPPI_FLAG_NO_CULL): the instantiation without the culling test
+inline MpccCtaKernel mpcc_cta_kernel_for(bool precise, int n_discs, bool cull) {
+  return cull ? mpcc_cta_kernel_pick<true>(precise, n_discs) : mpcc_cta_kernel_pick<false>(precise, n_discs);
 }
 
 }  // namespace brmppi
