@@ -95,10 +95,12 @@ typedef struct { int body; float offset; } brmppi_disc;
                                           (PAPER.md:221-225), contouring / lag / heading / effort / progress cost
                                           (13)-(15) along a cubic reference path.  Controls are
                                           (j, omega); the state is set with brmppi_set_state7 and the path with
-                                          brmppi_set_reference_path (no goal).  One thread per sample; not with
-                                          PROJECTED, super-ellipses or the hitch filter.                        */
+                                          brmppi_set_reference_path (no goal).  Default kernel: phase-split,
+                                          persistent; with KERNEL_THREAD_PER_SAMPLE the simple one.
+                                          Not with PROJECTED, super-ellipses or the hitch filter.               */
 #define BRMPPI_FLAG_NO_CULL 16u         /* evaluate every (obstacle, disc, step) even where the
-                                          hinge is provably zero; same results  */
+                                          hinge is provably zero (and 9.2 for BRMPPI_FLAG_MPCC);
+                                          bit-identical results                                  */
 
 typedef struct {
   int K;              /* samples per iteration, >= 1                                            */
