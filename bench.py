@@ -323,7 +323,7 @@ def measure(B, torch, name, rank, steps, warmup, dist, dev, local_rank, closed_l
         if name in MPCC:
             solver.set_reference_path(hg, sc.dpsi); solver.set_state7(hx, sc.psi0); solver.set_obstacles(ho)
             return
-        solver.set_state(hx); solver.set_goal(hg); solver.set_obstacles(ho)
+        solver.set_inputs(hx, hg, ho)                        # state, goal, obstacles: one call, one copy
         if hs is not None:
             solver.set_superellipses(hs)
     for _ in range(3):

@@ -190,6 +190,13 @@ int brmppi_set_reference_path(brmppi_ctx* ctx, int scene, int M, float dpsi, con
 int brmppi_set_goal(brmppi_ctx* ctx, int scene, const float g[4]);
 /* Obstacles of one scene at rollout time 0; 0 <= n <= max_obstacles (NULL allowed when n = 0). */
 int brmppi_set_obstacles(brmppi_ctx* ctx, int scene, int n, const brmppi_obstacle* obstacles);
+/* State, goal and obstacles of one scene in ONE call: the same checks, meaning and error codes as brmppi_set_state +
+ * brmppi_set_goal + brmppi_set_obstacles (in that order; nothing is changed if any of them would fail).  In a
+ * single-scene context the three pieces leave through one host-to-device copy from a page-locked staging buffer the
+ * context owns (two buffers used in turn, so the call never waits for the copy of the call before the last one);
+ * with several scenes it is the three copies.  HOST pointers; asynchronous on the stream.  Not with BRMPPI_FLAG_MPCC. */
+int brmppi_set_inputs(brmppi_ctx* ctx, int scene, const float x[4], const float g[4], int n,
+                      const brmppi_obstacle* obstacles);
 /* Super-ellipse obstacles of one scene at rollout time 0; 0 <= n <= max_superellipses (NULL allowed
  * when n = 0).  mx, my > 0; exponent 2 or 4 (else BRMPPI_ERR_INVALID_ARG). */
 int brmppi_set_superellipses(brmppi_ctx* ctx, int scene, int n, const brmppi_superellipse* obstacles);

@@ -34,7 +34,7 @@ EXPORTS = [
     "brmppi_debug_philox_raw", "brmppi_hitch_filter_scratch_bytes", "brmppi_project_scratch_bytes",
     "brmppi_measure_peaks_scratch_bytes", "brmppi_shard_words", "brmppi_shard_export", "brmppi_shard_import",
     "brmppi_set_state7", "brmppi_set_reference_path", "brmppi_get_state7", "brmppi_get_final_states7",
-    "brmppi_hitch_filter_static",
+    "brmppi_hitch_filter_static", "brmppi_set_inputs",
 ]
 
 
@@ -110,6 +110,7 @@ def lib():
         L.brmppi_get_state7.argtypes = [vp, C.c_int, _fp]
         L.brmppi_get_final_states7.argtypes = [vp, C.c_int, _fp]
         L.brmppi_set_obstacles.argtypes = [vp, C.c_int, C.c_int, C.POINTER(Obstacle)]
+        L.brmppi_set_inputs.argtypes = [vp, C.c_int, vp, vp, C.c_int, vp]     # addresses passed as integers
         L.brmppi_set_superellipses.argtypes = [vp, C.c_int, C.c_int, C.POINTER(Superellipse)]
         L.brmppi_get_superellipses.argtypes = [vp, C.c_int, C.POINTER(C.c_int), C.POINTER(Superellipse)]
         L.brmppi_set_nominal.argtypes = [vp, C.c_int, _fp]
@@ -255,6 +256,13 @@ class Solver:
         n = obs.shape[0]
         ptr = obs.ctypes.data_as(C.POINTER(Obstacle)) if n else None
         _check(lib().brmppi_set_obstacles(self._ctx, scene, n, ptr))
+
+    def set_inputs(self, x, g, obstacles, scene=0):
+        """State, goal and obstacles of one scene in one call (one host-to-device copy in a single-scene context)."""
+        x, g, obs = _f32(x, (4,)), _f32(g, (4,)), _f32(obstacles).reshape(-1, 5)
+        n = obs.shape[0]
+        adr = lambda a: a.__array_interface__["data"][0]       # cheaper than building ctypes pointer objects
+        _check(lib().brmppi_set_inputs(self._ctx, scene, adr(x), adr(g), n, adr(obs) if n else None))
 
     def set_superellipses(self, superellipses, scene=0):
         """rows (cx, cy, mx, my, theta, vx, vy, exponent)"""

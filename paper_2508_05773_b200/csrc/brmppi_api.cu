@@ -200,6 +200,9 @@ struct brmppi_ctx {
   cudaGraphExec_t solve_graph, step_graph;
   float* pinned_u0;             // [n_scenes][2] staging for brmppi_step
   float* path_len;              // [n_scenes] M dpsi of the reference path (BRMPPI_FLAG_MPCC), host
+  unsigned char* pinned_in[2];  // single-scene contexts: page-locked images of the workspace's input span
+  cudaEvent_t pinned_in_done[2];//   (state .. obstacles), used in turn by brmppi_set_inputs
+  int pinned_in_next;
   size_t smem_rollout, smem_update;
 };
 
@@ -343,6 +346,9 @@ int brmppi_create(const brmppi_params* p, void* dev_workspace, size_t workspace_
   c->step_graph = nullptr;
   c->pinned_u0 = nullptr;
   c->path_len = (float*)calloc((size_t)p->n_scenes, sizeof(float));
+  c->pinned_in[0] = c->pinned_in[1] = nullptr;
+  c->pinned_in_done[0] = c->pinned_in_done[1] = nullptr;
+  c->pinned_in_next = 0;
 
   DeviceParams& d = c->d;
   memset(&d, 0, sizeof(d));
@@ -466,8 +472,20 @@ int brmppi_create(const brmppi_params* p, void* dev_workspace, size_t workspace_
   if (e == cudaSuccess) e = cudaMemsetAsync(base + L.diag, 0, (size_t)p->n_scenes * sizeof(brmppi_diag), c->stream);
   if (e == cudaSuccess) e = cudaHostAlloc((void**)&c->pinned_u0, sizeof(float) * 2 * (size_t)p->n_scenes, cudaHostAllocMapped);
   if (e == cudaSuccess) e = cudaHostGetDevicePointer((void**)&d.u0_host, c->pinned_u0, 0);
+  if (p->n_scenes == 1 && !(p->flags & BRMPPI_FLAG_MPCC)) {
+    const size_t span = L.obstacles + (size_t)(p->max_obstacles > 0 ? p->max_obstacles : 1) * 20 - L.state;
+    for (int i = 0; i < 2 && e == cudaSuccess; ++i) {
+      e = cudaHostAlloc((void**)&c->pinned_in[i], span, cudaHostAllocDefault);
+      if (e == cudaSuccess) { memset(c->pinned_in[i], 0, span); e = cudaEventCreateWithFlags(&c->pinned_in_done[i], cudaEventDisableTiming); }
+    }
+  }
   if (e != cudaSuccess) {
     free(c->state_set); free(c->goal_set); free(c->path_len);
+    for (int i = 0; i < 2; ++i) {
+      if (c->pinned_in[i]) cudaFreeHost(c->pinned_in[i]);
+      if (c->pinned_in_done[i]) cudaEventDestroy(c->pinned_in_done[i]);
+    }
+    if (c->pinned_u0) cudaFreeHost(c->pinned_u0);
     delete c;
     return cuda_fail(e);
   }
@@ -480,6 +498,10 @@ int brmppi_destroy(brmppi_ctx* c) {
   if (c->solve_graph) cudaGraphExecDestroy(c->solve_graph);
   if (c->step_graph) cudaGraphExecDestroy(c->step_graph);
   if (c->pinned_u0) cudaFreeHost(c->pinned_u0);
+  for (int i = 0; i < 2; ++i) {
+    if (c->pinned_in[i]) cudaFreeHost(c->pinned_in[i]);
+    if (c->pinned_in_done[i]) cudaEventDestroy(c->pinned_in_done[i]);
+  }
   free(c->state_set);
   free(c->goal_set);
   free(c->path_len);
@@ -570,6 +592,47 @@ int brmppi_set_obstacles(brmppi_ctx* c, int scene, int n, const brmppi_obstacle*
     CU(cudaMemcpyAsync(c->d.obstacles + (size_t)scene * c->p.max_obstacles * 5, obs,
                        sizeof(brmppi_obstacle) * (size_t)n, cudaMemcpyHostToDevice, c->stream));
   CU(cudaMemcpyAsync(c->d.n_obs + scene, &n, sizeof(int), cudaMemcpyHostToDevice, c->stream));
+  return BRMPPI_OK;
+}
+
+int brmppi_set_inputs(brmppi_ctx* c, int scene, const float x[4], const float g[4], int n,
+                      const brmppi_obstacle* obs) {
+  int r = check_scene(c, scene);
+  if (r) return r;
+  // every check of the three calls first, so that a failure changes nothing
+  if (!x || !g) return BRMPPI_ERR_NULL;
+  if (c->p.flags & BRMPPI_FLAG_MPCC) return BRMPPI_ERR_INVALID_ARG;
+  if (!finite_all(x, 4) || !finite_all(g, 4)) return BRMPPI_ERR_NONFINITE_INPUT;
+  if (n < 0) return BRMPPI_ERR_INVALID_ARG;
+  if (n > c->p.max_obstacles) return BRMPPI_ERR_TOO_MANY_OBSTACLES;
+  if (n > 0 && !obs) return BRMPPI_ERR_NULL;
+  for (int i = 0; i < n; ++i) {
+    if (!finite_all(&obs[i].cx, 5)) return BRMPPI_ERR_NONFINITE_INPUT;
+    if (!(obs[i].radius > 0.f)) return BRMPPI_ERR_INVALID_ARG;
+  }
+  if (!c->pinned_in[0]) {                    // several scenes: the three copies
+    r = brmppi_set_state(c, scene, x);
+    if (!r) r = brmppi_set_goal(c, scene, g);
+    if (!r) r = brmppi_set_obstacles(c, scene, n, obs);
+    return r;
+  }
+  // one scene: an image of the workspace's input span (state | goal | n_obs | obstacles, each where the layout
+  // puts it) in page-locked memory, one copy.  Obstacle slots beyond n keep what the image held: never read.
+  const Layout& L = c->layout;
+  const int b = c->pinned_in_next;
+  c->pinned_in_next ^= 1;
+  CU(cudaEventSynchronize(c->pinned_in_done[b]));       // the copy that last used this buffer has been made
+  unsigned char* img = c->pinned_in[b];
+  const float v[4] = {x[0], x[1], wrap_pi(x[2]), wrap_pi(x[3])};
+  memcpy(img + (L.state - L.state), v, 16);
+  memcpy(img + (L.goal - L.state), g, 16);
+  memcpy(img + (L.n_obs - L.state), &n, sizeof(int));
+  if (n > 0) memcpy(img + (L.obstacles - L.state), obs, sizeof(brmppi_obstacle) * (size_t)n);
+  const size_t span = L.obstacles + sizeof(brmppi_obstacle) * (size_t)n - L.state;
+  CU(cudaMemcpyAsync((unsigned char*)c->d.state, img, span, cudaMemcpyHostToDevice, c->stream));
+  CU(cudaEventRecord(c->pinned_in_done[b], c->stream));
+  c->state_set[scene] = 1;
+  c->goal_set[scene] = 1;
   return BRMPPI_OK;
 }
 

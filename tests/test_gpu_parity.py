@@ -606,3 +606,38 @@ def test_velocity_dependent_hitch_limit(B, O, kernel):
     check_against_oracle(O, got, sc2, p)
     base = gpu_solve(B, sc2, p.with_(hitch_kappa=0.0), kernel)
     assert (got["S"] >= base["S"] - 1e-3).all() and (got["S"] > base["S"] + 1e-2).any()
+
+
+def test_set_inputs_equals_the_three_calls(B):
+    """brmppi_set_inputs (one call, one copy in a single-scene context) leaves exactly what set_state + set_goal +
+    set_obstacles leave: bit-identical solves, in a single-scene and in a two-scene context, repeated calls (the two
+    staging buffers in turn), fewer obstacles than before, and the same argument errors with nothing changed."""
+    sc = scenes.scene_cfg2(1)
+    p = sc.params.with_(K=1500, T=40, n_iter=2)
+    for n_scenes in (1, 2):
+        a = B.Solver(p, n_scenes, 8, B.FLAG_WRITE_SAMPLES)
+        b = B.Solver(p, n_scenes, 8, B.FLAG_WRITE_SAMPLES)
+        for rep_, n_obs in enumerate((8, 8, 3, 0, 5)):
+            x = sc.x0 + np.float32(0.1 * rep_)
+            for i in range(n_scenes):
+                a.set_state(x, i); a.set_goal(sc.goal, i); a.set_obstacles(sc.obstacles[:n_obs], i)
+                b.set_inputs(x, sc.goal, sc.obstacles[:n_obs], i)
+            a.set_nominal(None); b.set_nominal(None); a.set_counter(rep_); b.set_counter(rep_)
+            a.solve(); b.solve()
+            for i in range(n_scenes):
+                assert np.array_equal(a.get_costs(i), b.get_costs(i)) and np.array_equal(a.get_controls(i), b.get_controls(i))
+                assert np.array_equal(a.get_state(i), b.get_state(i)) and np.array_equal(a.get_obstacles(i), b.get_obstacles(i))
+        before = b.get_state(0).copy()
+        bad = sc.obstacles.copy(); bad[2, 2] = -1.0
+        for args, status in (((sc.x0, sc.goal, bad), B.ERR_INVALID_ARG),
+                             ((np.array([0, np.nan, 0, 0]), sc.goal, sc.obstacles), B.ERR_NONFINITE_INPUT),
+                             ((sc.x0, sc.goal, np.zeros((9, 5)) + 1.0), B.ERR_TOO_MANY_OBSTACLES)):
+            with pytest.raises(B.BrmppiError) as e:
+                b.set_inputs(*args)
+            assert e.value.status == status
+        assert np.array_equal(b.get_state(0), before) and len(b.get_obstacles(0)) == 5
+        a.close(); b.close()
+    fresh = B.Solver(p, 1, 8, 0)
+    fresh.set_inputs(sc.x0, sc.goal, sc.obstacles)      # marks state and goal as set
+    fresh.solve()
+    fresh.close()
