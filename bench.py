@@ -336,7 +336,9 @@ def measure(B, torch, name, rank, steps, warmup, dist, dev, local_rank, closed_l
         solver.get_controls()                                # synchronises; T*2 floats back
     barrier()
     e2e_s_max = max_over_ranks(time.perf_counter() - t0, dist, dev)
-    h2d = 16 + 16 + 20 * n_obs + 4 + (32 * n_se + 4 if n_se else 0)
+    # brmppi_set_inputs copies the padded input span of the workspace in one piece: state, goal and the obstacle
+    # count in 256-byte slots, then n_obs obstacles of 20 bytes (196 payload bytes at 8 obstacles)
+    h2d = 3 * 256 + 20 * n_obs + (32 * n_se + 4 if n_se else 0)
     if name in MPCC:                                         # state and psi, path table with M and dpsi, obstacles
         h2d = 32 + (64 * n_seg + 8) + 20 * n_obs + 4
     d2h = 8 * p.T
