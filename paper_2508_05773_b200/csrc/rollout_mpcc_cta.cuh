@@ -334,28 +334,51 @@ rollout_mpcc_cta(const __grid_constant__ DeviceParams P) {
     }
     __syncthreads();
     if (noise_planes) {
-      // weighted control sums from the kept controls: one warp per output (step, channel), lanes over the samples,
-      // four outputs at a time so that the four shuffle reductions overlap
+      // weighted control sums from the kept controls: a warp takes EIGHT outputs (step, channel) at a time, lanes
+      // over the samples; the eight per-lane sums are reduced together by a transposing butterfly (4 + 2 + 1
+      // exchanges leave each lane with one output's sum over its 4-lane class, two more finish it): 9 shuffles
+      // for 8 outputs instead of 40, and the lane's weights are loaded once
       const int n_warps = kMpccThreads / 32;
-      for (int o = warp; o < 2 * T; o += 4 * n_warps) {
-        float a[4];
+      float wl[kMpccTileMax / 32];
 #pragma unroll
-        for (int q = 0; q < 4; ++q) {
-          const int oq = min(o + q * n_warps, 2 * T - 1);
-          const float* u = sNoise + (size_t)oq * st;
+      for (int i = 0; i < kMpccTileMax / 32; ++i) wl[i] = (lane + 32 * i < st) ? sW[lane + 32 * i] : 0.0f;
+#pragma unroll 1
+      for (int o0 = 8 * warp; o0 < 2 * T; o0 += 8 * n_warps) {
+        float a[8];
+#pragma unroll
+        for (int q = 0; q < 8; ++q) {
+          const float* u = sNoise + (size_t)min(o0 + q, 2 * T - 1) * st + lane;
           float acc = 0.0f;
-          for (int es = lane; es < st; es += 32) acc = fmaf(sW[es], u[es], acc);
+#pragma unroll
+          for (int i = 0; i < kMpccTileMax / 32; ++i)
+            if (32 * i < st) acc = fmaf(wl[i], u[32 * i], acc);
           a[q] = acc;
         }
+        // after the round with mask m a lane keeps the outputs whose bit agrees with its own lane bit
+        float b4[4], b2[2], b1;
 #pragma unroll
-        for (int off = 16; off > 0; off >>= 1) {
-#pragma unroll
-          for (int q = 0; q < 4; ++q) a[q] += __shfl_xor_sync(0xffffffffu, a[q], off);
+        for (int q = 0; q < 4; ++q) {
+          const bool hi = (lane & 16) != 0;
+          const float send = hi ? a[q] : a[q + 4], keep = hi ? a[q + 4] : a[q];
+          b4[q] = keep + __shfl_xor_sync(0xffffffffu, send, 16);
         }
 #pragma unroll
-        for (int q = 0; q < 4; ++q)
-          if (lane == 0 && o + q * n_warps < 2 * T)
-            P.part_A[((size_t)scene * 2 * T + o + q * n_warps) * P.n_partials + part] = a[q];
+        for (int q = 0; q < 2; ++q) {
+          const bool hi = (lane & 8) != 0;
+          const float send = hi ? b4[q] : b4[q + 2], keep = hi ? b4[q + 2] : b4[q];
+          b2[q] = keep + __shfl_xor_sync(0xffffffffu, send, 8);
+        }
+        {
+          const bool hi = (lane & 4) != 0;
+          const float send = hi ? b2[0] : b2[1], keep = hi ? b2[1] : b2[0];
+          b1 = keep + __shfl_xor_sync(0xffffffffu, send, 4);
+        }
+        b1 += __shfl_xor_sync(0xffffffffu, b1, 2);
+        b1 += __shfl_xor_sync(0xffffffffu, b1, 1);
+        // lane bits (16, 8, 4) -> output bits (4, 2, 1)
+        const int q_own = ((lane >> 4) & 1) * 4 + ((lane >> 3) & 1) * 2 + ((lane >> 2) & 1);
+        if ((lane & 3) == 0 && o0 + q_own < 2 * T)
+          P.part_A[((size_t)scene * 2 * T + o0 + q_own) * P.n_partials + part] = b1;
       }
     } else {
       // the sampled controls regenerated from the counter-based generator: thread -> (sample slot es, every n_pg-th
