@@ -43,12 +43,43 @@ __device__ __forceinline__ void thread_kernel_epilogue(const DeviceParams& P, co
   float nf = warp_sum((valid && !finite) ? 1.0f : 0.0f);
   if (lane == 0) { sRedF[warp] = eta; sRedF[4 + warp] = w2; sRedF[8 + warp] = nf; }
 
-  // weighted control sums: regenerate u_k[t] from the counter-based generator
-  for (int t = 0; t < T; ++t) {
-    float2 u = make_float2(0.0f, 0.0f);
-    if (finite) u = sample_control<PRECISE>(P, sU[t], (uint32_t)t, n, (uint32_t)(k + P.k_offset), key0, key1);
-    const float av = warp_sum(wk * u.x), ad = warp_sum(wk * u.y);
-    if (lane == 0) { sA[warp * 2 * T + 2 * t] = av; sA[warp * 2 * T + 2 * t + 1] = ad; }
+  // weighted control sums: regenerate u_k[t] from the counter-based generator, two Philox blocks = four steps =
+  // eight outputs at a time; the eight per-lane products are reduced together by a transposing butterfly (4 + 2 + 1
+  // exchanges leave each lane with one output's sum over its 4-lane class, two more finish it: 9 shuffles for 8
+  // outputs)
+  for (int t0 = 0; t0 < T; t0 += 4) {
+    float a[8];
+#pragma unroll
+    for (int h = 0; h < 2; ++h) {
+      float2 u0 = make_float2(0.0f, 0.0f), u1 = u0;
+      const int t = t0 + 2 * h;
+      if (finite && t < T)
+        sample_control_pair<PRECISE>(P, sU[t], sU[min(t + 1, T - 1)], (uint32_t)(t >> 1), n, (uint32_t)(k + P.k_offset),
+                                     key0, key1, &u0, &u1);
+      a[4 * h + 0] = wk * u0.x; a[4 * h + 1] = wk * u0.y; a[4 * h + 2] = wk * u1.x; a[4 * h + 3] = wk * u1.y;
+    }
+    float b4[4], b2[2], b1;
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+      const bool hi = (lane & 16) != 0;
+      const float send = hi ? a[q] : a[q + 4], keep = hi ? a[q + 4] : a[q];
+      b4[q] = keep + __shfl_xor_sync(0xffffffffu, send, 16);
+    }
+#pragma unroll
+    for (int q = 0; q < 2; ++q) {
+      const bool hi = (lane & 8) != 0;
+      const float send = hi ? b4[q] : b4[q + 2], keep = hi ? b4[q + 2] : b4[q];
+      b2[q] = keep + __shfl_xor_sync(0xffffffffu, send, 8);
+    }
+    {
+      const bool hi = (lane & 4) != 0;
+      const float send = hi ? b2[0] : b2[1], keep = hi ? b2[1] : b2[0];
+      b1 = keep + __shfl_xor_sync(0xffffffffu, send, 4);
+    }
+    b1 += __shfl_xor_sync(0xffffffffu, b1, 2);
+    b1 += __shfl_xor_sync(0xffffffffu, b1, 1);
+    const int o = 2 * t0 + ((lane >> 4) & 1) * 4 + ((lane >> 3) & 1) * 2 + ((lane >> 2) & 1);   // lane bits -> output
+    if ((lane & 3) == 0 && o < 2 * T) sA[warp * 2 * T + o] = b1;
   }
   __syncthreads();
 
