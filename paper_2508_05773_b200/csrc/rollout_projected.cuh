@@ -178,15 +178,15 @@ rollout_projected(const __grid_constant__ DeviceParams P) {
         for (int c = 0; c <= i; ++c) Sm[i][c] = fmaf(a0, g0[c], a1 * g1[c]);
         Sm[i][i] = fmaf(h[i] * ma, h[i], Sm[i][i]);
       }
-      bool drop[NO];
 #pragma unroll
       for (int c = 0; c < NO; ++c) {
         const float d0 = Sm[c][c];
         float dkk = d0;
 #pragma unroll
         for (int m = 0; m < c; ++m) dkk = fmaf(-Sm[c][m], Sm[c][m], dkk);
-        drop[c] = !(dkk > 1e-6f * d0);            // a row that adds nothing new is dropped (multiplier 0)
-        const float inv = drop[c] ? 0.0f : rsqrtf(dkk);
+        // a row that adds nothing new is dropped: 1 / L_cc = 0 makes its column of L zero and its multiplier
+        // zero in both triangular solves (its own entries L_cm are finite and only ever meet that zero)
+        const float inv = (dkk > 1e-6f * d0) ? fast_rsqrt(dkk) : 0.0f;
         Sm[c][c] = inv;
 #pragma unroll
         for (int i = c + 1; i < NO; ++i) {
@@ -195,9 +195,6 @@ rollout_projected(const __grid_constant__ DeviceParams P) {
           for (int m = 0; m < c; ++m) v = fmaf(-Sm[i][m], Sm[c][m], v);
           Sm[i][c] = v * inv;
         }
-        const float keep = drop[c] ? 0.0f : 1.0f;
-#pragma unroll
-        for (int m = 0; m < c; ++m) Sm[c][m] *= keep;
       }
 #pragma unroll
       for (int i = 0; i < NO; ++i) {              // L w = r
