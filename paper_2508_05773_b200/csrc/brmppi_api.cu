@@ -225,7 +225,7 @@ int launch_rollout(brmppi_ctx* c) {
     CU(cudaGetLastError());
   } else if (c->p.flags & BRMPPI_FLAG_PROJECTED) {
     dim3 grid((unsigned)c->plan.n_partials, (unsigned)d.n_scenes);
-    projected_kernel_for(precise, d.max_obstacles)<<<grid, kThreadBlock, c->smem_rollout, c->stream>>>(d);
+    projected_kernel_for(precise, d.max_obstacles, d.n_discs)<<<grid, kThreadBlock, c->smem_rollout, c->stream>>>(d);
     CU(cudaGetLastError());
   } else {
     dim3 grid((unsigned)c->plan.n_partials, (unsigned)d.n_scenes);
@@ -452,7 +452,7 @@ int brmppi_create(const brmppi_params* p, void* dev_workspace, size_t workspace_
                                                          : rollout_thread_smem_bytes(d);
     // per function and device, not per context: always the opt-in maximum, never lowered
     if (p->flags & BRMPPI_FLAG_PROJECTED)
-      e = cudaFuncSetAttribute(projected_kernel_for((p->flags & BRMPPI_FLAG_PRECISE_MATH) != 0, p->max_obstacles),
+      e = cudaFuncSetAttribute(projected_kernel_for((p->flags & BRMPPI_FLAG_PRECISE_MATH) != 0, p->max_obstacles, p->n_discs),
                                cudaFuncAttributeMaxDynamicSharedMemorySize, (int)prop.sharedMemPerBlockOptin);
     if (e == cudaSuccess)
       e = cudaFuncSetAttribute(rollout_mpcc<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)prop.sharedMemPerBlockOptin);

@@ -31,53 +31,55 @@ __device__ __forceinline__ void normals4(uint32_t t, uint32_t n, uint32_t k, uin
 }
 
 // Rows of (9) for all obstacles at state X, step t: h_i on the closest disc (lowest index on ties),
-// L_g h_i (2), L_f h_i.  Obstacle i: sObs = (ox, oy, 1/rho^2, -) in the vehicle frame, sVel = dt vel; the
-// table is padded to NO entries with null obstacles (1/rho^2 = 0), so the loop has no branch: a null row
-// comes out as h = 1, L_g h = 0, L_f h = 0.
-template <bool PRECISE, int NO>
+// L_g h_i (2), L_f h_i.  Obstacle i: sObs = (ox, oy, 1/rho^2, 2 dt/rho^2) in the vehicle frame, sVel = (dt vel, vel);
+// the table is padded to NO entries with null obstacles (1/rho^2 = 0), so the loop has no branch: a null row comes
+// out as h = 1, L_g h = 0, L_f h = 0.  ND = the number of vehicle discs when it is 3 (the vehicle of every
+// recipe), else BRMPPI_MAX_DISCS with the discs beyond P.n_discs masked.
+template <bool PRECISE, int NO, int ND>
 __device__ __forceinline__ void barrier_rows(const DeviceParams& P, const State& X, int n_obs, float tf,
-                                             const float4* __restrict__ sObs, const float2* __restrict__ sVel,
+                                             const float4* __restrict__ sObs, const float4* __restrict__ sVel,
                                              float (&h)[NO], float (&g0)[NO], float (&g1)[NO], float (&lf)[NO]) {
   float s1, c1, s2, c2;
   sincos_t<PRECISE>(X.psi1, &s1, &c1);
   sincos_t<PRECISE>(X.psi2, &s2, &c2);
-  float cx[kMaxDiscs], cy[kMaxDiscs];
-  disc_centres(P, X, s1, c1, s2, c2, cx, cy);
+  float cx[ND], cy[ND];
+  disc_centres_n<ND>(P, X.x, X.y, s1, c1, s2, c2, cx, cy);
   const float sb = s1 * c2 - c1 * s2, cb = fmaf(c1, c2, s1 * s2);   // sin / cos (psi1 - psi2)
+  const float sbL = sb * P.inv_L2, cbL = P.Lh_over_L1 * P.inv_L2 * cb;
 #pragma unroll
   for (int i = 0; i < NO; ++i) {
     const float4 o = sObs[i];
-    const float2 w = sVel[i];
+    const float4 w = sVel[i];
     const float ox = fmaf(tf, w.x, o.x), oy = fmaf(tf, w.y, o.y);                 // o(t)
     // closest disc: h_j, the offset c_j - o, and the disc's lever arms on the two headings
     // (d c_j / d psi1 = (a1_j - Lh)(-sin psi1, cos psi1), d c_j / d psi2 = a2_j (-sin psi2, cos psi2))
     float hb = CUDART_INF_F, ex = 0.0f, ey = 0.0f, l1 = 0.0f, l2 = 0.0f;
 #pragma unroll
-    for (int j = 0; j < kMaxDiscs; ++j) {
+    for (int j = 0; j < ND; ++j) {
       const float dx = cx[j] - ox, dy = cy[j] - oy;
-      const float hj = j < P.n_discs ? fmaf(fmaf(dx, dx, dy * dy), o.z, -1.0f) : CUDART_INF_F;
+      const float hj = (ND < kMaxDiscs || j < P.n_discs) ? fmaf(fmaf(dx, dx, dy * dy), o.z, -1.0f) : CUDART_INF_F;
       const bool take = hj < hb;
       hb = take ? hj : hb; ex = take ? dx : ex; ey = take ? dy : ey;
       l1 = take ? P.disc_a1[j] - P.Lh : l1; l2 = take ? P.disc_a2[j] : l2;
     }
-    const float gx = 2.0f * ex * o.z, gy = 2.0f * ey * o.z;                       // grad_c h
+    const float gx = ex * o.w, gy = ey * o.w;                                     // dt grad_c h
     const float dpsi1 = l1 * fmaf(gy, c1, -gx * s1), dpsi2 = l2 * fmaf(gy, c2, -gx * s2);
     h[i] = i < n_obs ? hb : 1.0f;
-    g0[i] = P.dt * fmaf(gx, c1, fmaf(gy, s1, dpsi2 * sb * P.inv_L2));
-    g1[i] = P.dt * fmaf(dpsi1, P.inv_L1, -(dpsi2 * P.Lh_over_L1 * P.inv_L2) * cb);
-    lf[i] = -fmaf(gx, w.x, gy * w.y);                                             // w = dt vel
+    g0[i] = fmaf(gx, c1, fmaf(gy, s1, dpsi2 * sbL));
+    g1[i] = fmaf(dpsi1, P.inv_L1, -dpsi2 * cbL);
+    lf[i] = -fmaf(gx, w.z, gy * w.w);                                             // dt grad_c h . vel
   }
 }
 
-template <bool PRECISE, int NO>
+template <bool PRECISE, int NO, int ND>
 __global__ void __launch_bounds__(kThreadBlock)
 rollout_projected(const __grid_constant__ DeviceParams P) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   // layout of rollout_thread_per_sample with NO obstacle slots
   const int T = P.T;
   float4* sObs = reinterpret_cast<float4*>(smem_raw);
-  float2* sVel = reinterpret_cast<float2*>(sObs + NO);
-  float2* sU = sVel + NO;
+  float4* sVel = sObs + NO;
+  float2* sU = reinterpret_cast<float2*>(sVel + NO);
   double* sRedM = reinterpret_cast<double*>(sU + T);
   int* sRedI = reinterpret_cast<int*>(sRedM + 4);
   float* sRedF = reinterpret_cast<float*>(sRedI + 4);
@@ -101,11 +103,12 @@ rollout_projected(const __grid_constant__ DeviceParams P) {
     if (i < n_obs) {
       const float* ob = P.obstacles + ((size_t)scene * P.max_obstacles + i) * 5;
       const float rho = ob[2] + P.disc_radius;
-      sObs[i] = make_float4(ob[0] - x0.x, ob[1] - x0.y, 1.0f / (rho * rho), 0.0f);
-      sVel[i] = make_float2(P.dt * ob[3], P.dt * ob[4]);
+      const float ir2 = 1.0f / (rho * rho);
+      sObs[i] = make_float4(ob[0] - x0.x, ob[1] - x0.y, ir2, 2.0f * P.dt * ir2);
+      sVel[i] = make_float4(P.dt * ob[3], P.dt * ob[4], ob[3], ob[4]);
     } else {                                                 // null obstacle: no gradient, no motion
       sObs[i] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
-      sVel[i] = make_float2(0.0f, 0.0f);
+      sVel[i] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
     }
   }
   __syncthreads();
@@ -124,7 +127,7 @@ rollout_projected(const __grid_constant__ DeviceParams P) {
       for (int i = 0; i < NO; ++i) alpha[i] = a0;
     }
     float h[NO], g0[NO], g1[NO], lf[NO];
-    barrier_rows<PRECISE, NO>(P, X, n_obs, 0.0f, sObs, sVel, h, g0, g1, lf);
+    barrier_rows<PRECISE, NO, ND>(P, X, n_obs, 0.0f, sObs, sVel, h, g0, g1, lf);
     double cost = 0.0;
     // The draws of step t + 1 do not depend on the state: they are generated during step t, so that the long
     // Philox / Box-Muller chains fill the issue slots the Cholesky chain leaves empty.
@@ -233,7 +236,7 @@ rollout_projected(const __grid_constant__ DeviceParams P) {
         X = N;
       }
       // rows of (9) at the new state: the alpha cost now, A and b of the next step
-      barrier_rows<PRECISE, NO>(P, X, n_obs, (float)(t + 1), sObs, sVel, h, g0, g1, lf);
+      barrier_rows<PRECISE, NO, ND>(P, X, n_obs, (float)(t + 1), sObs, sVel, h, g0, g1, lf);
       float ca = 0.0f;
 #pragma unroll
       for (int i = 0; i < NO; ++i)
@@ -254,24 +257,31 @@ rollout_projected(const __grid_constant__ DeviceParams P) {
 }
 
 inline size_t rollout_projected_smem_bytes(const DeviceParams& P) {
-  return sizeof(float4) * BRMPPI_PROJECT_MAX_NO + sizeof(float2) * BRMPPI_PROJECT_MAX_NO + sizeof(float2) * P.T +
+  return sizeof(float4) * BRMPPI_PROJECT_MAX_NO + sizeof(float4) * BRMPPI_PROJECT_MAX_NO + sizeof(float2) * P.T +
          sizeof(double) * 4 + sizeof(int) * 4 + sizeof(float) * 12 + sizeof(float) * 4 * 2 * P.T;
 }
 
 using ProjectedKernel = void (*)(const DeviceParams);
 
-inline ProjectedKernel projected_kernel_for(bool precise, int max_obstacles) {
+template <int ND>
+inline ProjectedKernel projected_kernel_pick(bool precise, int max_obstacles) {
   const int cap = max_obstacles <= 1 ? 1 : max_obstacles <= 2 ? 2 : max_obstacles <= 4 ? 4 : 8;
   switch (cap * 2 + (precise ? 1 : 0)) {
-    case 2: return rollout_projected<false, 1>;
-    case 3: return rollout_projected<true, 1>;
-    case 4: return rollout_projected<false, 2>;
-    case 5: return rollout_projected<true, 2>;
-    case 8: return rollout_projected<false, 4>;
-    case 9: return rollout_projected<true, 4>;
-    case 16: return rollout_projected<false, 8>;
-    default: return rollout_projected<true, 8>;
+    case 2: return rollout_projected<false, 1, ND>;
+    case 3: return rollout_projected<true, 1, ND>;
+    case 4: return rollout_projected<false, 2, ND>;
+    case 5: return rollout_projected<true, 2, ND>;
+    case 8: return rollout_projected<false, 4, ND>;
+    case 9: return rollout_projected<true, 4, ND>;
+    case 16: return rollout_projected<false, 8, ND>;
+    default: return rollout_projected<true, 8, ND>;
   }
+}
+
+// three vehicle discs get their own instantiation; any other count runs the masked four-disc one
+inline ProjectedKernel projected_kernel_for(bool precise, int max_obstacles, int n_discs) {
+  return n_discs == 3 ? projected_kernel_pick<3>(precise, max_obstacles)
+                      : projected_kernel_pick<kMaxDiscs>(precise, max_obstacles);
 }
 
 }  // namespace brmppi
