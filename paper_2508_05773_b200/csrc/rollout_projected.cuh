@@ -38,10 +38,12 @@ __device__ __forceinline__ void normals4(uint32_t t, uint32_t n, uint32_t k, uin
 template <bool PRECISE, int NO, int ND>
 __device__ __forceinline__ void barrier_rows(const DeviceParams& P, const State& X, int n_obs, float tf,
                                              const float4* __restrict__ sObs, const float4* __restrict__ sVel,
-                                             float (&h)[NO], float (&g0)[NO], float (&g1)[NO], float (&lf)[NO]) {
+                                             float (&h)[NO], float (&g0)[NO], float (&g1)[NO], float (&lf)[NO],
+                                             float4* trig) {
   float s1, c1, s2, c2;
   sincos_t<PRECISE>(X.psi1, &s1, &c1);
   sincos_t<PRECISE>(X.psi2, &s2, &c2);
+  *trig = make_float4(s1, c1, s2, c2);       // the model step out of this state needs the same four
   float cx[ND], cy[ND];
   disc_centres_n<ND>(P, X.x, X.y, s1, c1, s2, c2, cx, cy);
   const float sb = s1 * c2 - c1 * s2, cb = fmaf(c1, c2, s1 * s2);   // sin / cos (psi1 - psi2)
@@ -127,7 +129,8 @@ rollout_projected(const __grid_constant__ DeviceParams P) {
       for (int i = 0; i < NO; ++i) alpha[i] = a0;
     }
     float h[NO], g0[NO], g1[NO], lf[NO];
-    barrier_rows<PRECISE, NO, ND>(P, X, n_obs, 0.0f, sObs, sVel, h, g0, g1, lf);
+    float4 trig;
+    barrier_rows<PRECISE, NO, ND>(P, X, n_obs, 0.0f, sObs, sVel, h, g0, g1, lf, &trig);
     double cost = 0.0;
     // The draws of step t + 1 do not depend on the state: they are generated during step t, so that the long
     // Philox / Box-Muller chains fill the issue slots the Cholesky chain leaves empty.
@@ -223,9 +226,7 @@ rollout_projected(const __grid_constant__ DeviceParams P) {
         if (i < n_obs) alpha[i] += fmaf(-ma * h[i], r[i], ya[i]);   // alpha_{tau+1} = alpha_tau + u^alpha_proj
       // x_{tau+1} = x_tau + dt G(x_tau) w_proj
       {
-        float s1, c1, s2, c2;
-        sincos_t<PRECISE>(X.psi1, &s1, &c1);
-        sincos_t<PRECISE>(X.psi2, &s2, &c2);
+        const float s1 = trig.x, c1 = trig.y, s2 = trig.z, c2 = trig.w;      // of X, from barrier_rows
         const float sb = s1 * c2 - c1 * s2, cb = fmaf(c1, c2, s1 * s2);
         const float a = P.dt * vp;
         State N;
@@ -236,7 +237,7 @@ rollout_projected(const __grid_constant__ DeviceParams P) {
         X = N;
       }
       // rows of (9) at the new state: the alpha cost now, A and b of the next step
-      barrier_rows<PRECISE, NO, ND>(P, X, n_obs, (float)(t + 1), sObs, sVel, h, g0, g1, lf);
+      barrier_rows<PRECISE, NO, ND>(P, X, n_obs, (float)(t + 1), sObs, sVel, h, g0, g1, lf, &trig);
       float ca = 0.0f;
 #pragma unroll
       for (int i = 0; i < NO; ++i)
