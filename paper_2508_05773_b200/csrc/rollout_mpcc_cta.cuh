@@ -89,11 +89,11 @@ inline MpccCtaPlan make_mpcc_cta_plan(int K, int T, int n_scenes, int max_obstac
 // stage cost (13) with the barrier term; *track = the four tracking terms at (x_{t+1}, psi_{t+1}).  row0 / row1:
 // quad 0 of rows t and t + 1, already offset by the sample; st = plane stride (in float4).
 template <int ND, bool CULL>
-__device__ __forceinline__ double mpcc_cost_item(const DeviceParams& P, const float4* __restrict__ sObs,
+__device__ __forceinline__ float mpcc_cost_item(const DeviceParams& P, const float4* __restrict__ sObs,
                                                  const float4* __restrict__ sVel, const float4* __restrict__ sPath,
                                                  int n_moving, int n_obs, int M, float dpsi, float inv_dpsi, const float4* row0,
                                                  const float4* row1, int st, int t, float alpha, float inv_alpha_cull,
-                                                 bool u_in_row, float2 u, float* track) {
+                                                 bool u_in_row, float2 u, float* track, float* pen_out) {
   const float4 q0 = row0[0], q1 = row0[st];                                     // (x, y, v, a), (s1, c1, s2, c2)
   const float td = row0[2 * st].x;
   if (u_in_row) { const float4 q3 = row0[3 * st]; u = make_float2(q3.z, q3.w); }
@@ -106,8 +106,8 @@ __device__ __forceinline__ double mpcc_cost_item(const DeviceParams& P, const fl
   float nu;
   *track = mpcc_tracking_sc(P, n0.x, n0.y, n2.y, n2.z, n0.z, n1.x, n1.y, path_eval(sPath, M, dpsi, inv_dpsi, n2.w), n3.x,
                             n3.y, &nu);
-  const float stage = *track + mpcc_stage_rest(P, n2.y, n2.z, n0.z, nu, u);
-  return (double)stage + (double)P.w_bar * (double)pen;
+  *pen_out = pen;
+  return *track + mpcc_stage_rest(P, n2.y, n2.z, n0.z, nu, u);
 }
 
 template <bool PRECISE, int ND, bool CULL>
@@ -279,7 +279,10 @@ rollout_mpcc_cta(const __grid_constant__ DeviceParams P) {
       for (int i = 0; i < n_obs; ++i) n_moving += (sVel[i].x != 0.0f || sVel[i].y != 0.0f) ? 1 : 0;
       // exact culling of far obstacles (mpcc_hinge): off for alpha <= 0 and under BRMPPI_FLAG_NO_CULL
       const float inv_alpha_cull = (CULL && alpha > 0.0f) ? 1.001f / alpha : 0.0f;
-      double acc = 0.0;
+      // a thread's T / G items are summed in fp32 (at most a few tens of terms of like size), the stage costs and the
+      // hinge sums apart; fp64 takes over where magnitudes mix: w_bar times the hinge sum, the terminal cost, and
+      // the sum over the G threads of a sample in phase D
+      float acc_stage = 0.0f, acc_pen = 0.0f, term = 0.0f;
       for (int c = 0; c < n_chunks; ++c) {
         const uint32_t gg = g + (uint32_t)c;
         const int slot = (int)(gg & 1u);
@@ -290,14 +293,16 @@ rollout_mpcc_cta(const __grid_constant__ DeviceParams P) {
           if (t < T) {
             float track;
             const float4* row0 = sPlanes + slot * slot_quads + r * row_quads + s;
-            acc += mpcc_cost_item<ND, CULL>(P, sObs, sVel, sPath, n_moving, n_obs, M, dpsi, inv_dpsi, row0, row0 + row_quads, st, t,
-                                      alpha, inv_alpha_cull, true, make_float2(0.0f, 0.0f), &track);
-            if (t == T - 1) acc += (double)(P.w_term * track);       // terminal cost: the same four terms at (x_N, psi_N)
+            float pen;
+            acc_stage += mpcc_cost_item<ND, CULL>(P, sObs, sVel, sPath, n_moving, n_obs, M, dpsi, inv_dpsi, row0, row0 + row_quads, st, t,
+                                      alpha, inv_alpha_cull, true, make_float2(0.0f, 0.0f), &track, &pen);
+            acc_pen += pen;
+            if (t == T - 1) term = P.w_term * track;                 // terminal cost: the same four terms at (x_N, psi_N)
           }
         }
         mbar_arrive(smem_addr(&bars[2 + slot]));
       }
-      sPart[grp * st + s] = acc;
+      sPart[grp * st + s] = ((double)acc_stage + (double)term) + (double)P.w_bar * (double)acc_pen;
     }
     g += (uint32_t)n_chunks;
     __syncthreads();
