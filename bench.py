@@ -69,7 +69,7 @@ def workload(name, rank=0):
 
 PROJECTED = ("cfg2proj", "paperproj")
 MPCC = ("cfg2mpcc", "papermpcc")
-THREAD_PER_SAMPLE = PROJECTED + MPCC          # workloads whose rollout is a one-thread-per-sample kernel (no culling)
+LONG_STEPS = PROJECTED + MPCC                 # workloads whose control step takes 0.1 ms or more: fewer timed steps
 
 
 def solver_flags(B, name, no_cull=False):
@@ -462,7 +462,7 @@ def run_ours(args):
     if world == 1 and not args.no_others:
         for name in ("cfg0", "cfg1", "cfg2", "cfg3", "cfg2se", "cfg2proj", "paperproj", "cfg2mpcc", "papermpcc"):
             if name != args.workload:
-                steps_o = 20 if name in THREAD_PER_SAMPLE else 50
+                steps_o = 20 if name in LONG_STEPS else 50
                 others.append(record(name, measure(B, torch, name, 0, steps_o, 5, None, dev, local_rank, 100, False), 1))
         others.append(batch64_record(B))
     cores = os.cpu_count() or 1
