@@ -18,7 +18,7 @@ constexpr int kUpdateBlock = 256;
 constexpr int kUpdateOutputsPerBlock = 1;   // one CTA per output channel o = 2 t + c
 
 // One CTA per (output channel, scene): every thread takes partials p = tid, tid + 256, ...
-// (coalesced rows, all loads of a thread independent, so the kernel is two L2 round trips deep),
+// (coalesced rows, all loads of a thread independent and the first partial's issued together: one L2 round trip),
 // then a fixed-order block reduction.  Every CTA recomputes the global minimum itself -- P * 12
 // bytes from L2 -- rather than paying a third kernel or a grid-wide sync for it.
 //
@@ -64,10 +64,28 @@ merge_update(const __grid_constant__ DeviceParams P, float* shard, int n_shards)
   auto part_m = [&](int p) { return MODE == kMergeImport ? *reinterpret_cast<const double*>(rec(p)) : pm[p]; };
   auto part_i = [&](int p) { return MODE == kMergeImport ? __float_as_int(rec(p)[2]) : pi[p]; };
 
+  // A thread's first partial (its only one while there are no more partials than threads: one per SM) is
+  // loaded whole before the minimum is known, so that the kernel is ONE L2 round trip deep, not two.
+  const bool diag_cta = (o == 0);
+  const bool have = tid < Pn;
+  double m0 = CUDART_INF;
+  int i0 = 0x7fffffff;
+  float eta0 = 0.0f, acc0 = 0.0f, w20 = 0.0f, nf0 = 0.0f;
+  if (have) {
+    m0 = part_m(tid); i0 = part_i(tid);
+    if (MODE == kMergeImport) {
+      const float* r = rec(tid);
+      eta0 = r[3]; acc0 = r[kShardHeader + o];
+      if (diag_cta) { w20 = r[4]; nf0 = (float)__float_as_int(r[5]); }
+    } else {
+      eta0 = peta[tid]; acc0 = pa[tid];
+      if (diag_cta) { w20 = pw2[tid]; nf0 = (float)pnf[tid]; }
+    }
+  }
   // global minimum and its sample index (lowest index on ties)
-  double m = CUDART_INF;
-  int idx = 0x7fffffff;
-  for (int p = tid; p < Pn; p += kUpdateBlock) {
+  double m = m0;
+  int idx = i0;
+  for (int p = tid + kUpdateBlock; p < Pn; p += kUpdateBlock) {
     const double om = part_m(p);
     const int oi = part_i(p);
     if (om < m || (om == m && oi < idx)) { m = om; idx = oi; }
@@ -81,9 +99,13 @@ merge_update(const __grid_constant__ DeviceParams P, float* shard, int n_shards)
     if (sM[w] < m || (sM[w] == m && sI[w] < idx)) { m = sM[w]; idx = sI[w]; }
   const bool any_finite = m < CUDART_INF;
 
-  const bool diag_cta = (o == 0);
   float eta = 0.0f, acc = 0.0f, w2 = 0.0f, nf = 0.0f;
-  for (int p = tid; p < Pn; p += kUpdateBlock) {
+  if (have) {
+    const float c = (any_finite && m0 < CUDART_INF) ? expf((float)(-(m0 - m) * (double)P.inv_lambda)) : 0.0f;
+    eta = c * eta0; acc = c * acc0;
+    if (diag_cta) { w2 = (c * c) * w20; nf = nf0; }
+  }
+  for (int p = tid + kUpdateBlock; p < Pn; p += kUpdateBlock) {
     const double mp = part_m(p);
     const float c = (any_finite && mp < CUDART_INF) ? expf((float)(-(mp - m) * (double)P.inv_lambda)) : 0.0f;
     if (MODE == kMergeImport) {
