@@ -212,6 +212,11 @@ int brmppi_reset(brmppi_ctx* ctx);
  * Asynchronous on the stream.  A sample with non-finite cost gets weight 0; if all K are
  * non-finite U is left unchanged (diag.nonfinite == K). */
 int brmppi_solve(brmppi_ctx* ctx);
+/* brmppi_solve followed by brmppi_get_controls of every scene, as one call with no copy behind the solve: the
+ * last iteration's update (5) writes the new nominal into page-locked host memory the context owns as well (the
+ * way brmppi_step returns u0), the call waits for the stream and hands it over.  U_out: HOST, [n_scenes][T][2]
+ * floats, owned by the caller.  Synchronous.  Everything else as brmppi_solve (same kernels, same results). */
+int brmppi_solve_get_controls(brmppi_ctx* ctx, float* U_out);
 /* K-sharded solve.  The online-softmax state (m, eta, A[2T]) of
  * eq. (5) is associative, so G contexts (on G GPUs, or on one) can each own K/G of the samples of ONE solve:
  * same seed, state, goal, obstacles and nominal in every context, k_offset = first global sample index.

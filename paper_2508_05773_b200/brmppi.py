@@ -27,7 +27,7 @@ HITCH_STATIC_MAX_N = 16384
 EXPORTS = [
     "brmppi_workspace_bytes", "brmppi_create", "brmppi_destroy", "brmppi_set_state",
     "brmppi_set_goal", "brmppi_set_obstacles", "brmppi_set_superellipses", "brmppi_get_superellipses", "brmppi_set_nominal", "brmppi_set_counter",
-    "brmppi_reset", "brmppi_solve", "brmppi_shift", "brmppi_step", "brmppi_get_controls",
+    "brmppi_reset", "brmppi_solve", "brmppi_solve_get_controls", "brmppi_shift", "brmppi_step", "brmppi_get_controls",
     "brmppi_get_state", "brmppi_get_obstacles", "brmppi_get_costs", "brmppi_get_final_states",
     "brmppi_get_diag", "brmppi_get_phase_times", "brmppi_time_kernels", "brmppi_launch_count", "brmppi_strerror", "brmppi_debug_philox",
     "brmppi_debug_sample_controls", "brmppi_measure_peaks", "brmppi_get_hitch_filter", "brmppi_hitch_filter", "brmppi_project",
@@ -117,6 +117,7 @@ def lib():
         L.brmppi_set_counter.argtypes = [vp, C.c_uint]
         L.brmppi_reset.argtypes = [vp]
         L.brmppi_solve.argtypes = [vp]
+        L.brmppi_solve_get_controls.argtypes = [vp, vp]
         L.brmppi_shift.argtypes = [vp]
         L.brmppi_shard_words.argtypes = [vp]
         L.brmppi_shard_words.restype = C.c_size_t
@@ -312,6 +313,14 @@ class Solver:
     # ---- work ---------------------------------------------------------------------------
     def solve(self):
         _check(lib().brmppi_solve(self._ctx))
+
+    def solve_get_controls(self, out=None):
+        """solve() and the new nominal of every scene, [n_scenes][T][2], in one call (no copy behind the solve)."""
+        if out is None:
+            out = np.empty((self.n_scenes, self.T, 2), dtype=np.float32)
+        assert out.dtype == np.float32 and out.flags.c_contiguous and out.size == self.n_scenes * self.T * 2
+        _check(lib().brmppi_solve_get_controls(self._ctx, C.c_void_p(out.ctypes.data)))
+        return out
 
     def shift(self):
         _check(lib().brmppi_shift(self._ctx))

@@ -197,8 +197,10 @@ struct brmppi_ctx {
   unsigned char* goal_set;
   unsigned long long launches;
   unsigned int n_host;          // host mirror of the device iteration counter
-  cudaGraphExec_t solve_graph, step_graph;
+  cudaGraphExec_t solve_graph, step_graph, solve_host_graph;
   float* pinned_u0;             // [n_scenes][2] staging for brmppi_step
+  float* pinned_U;              // [n_scenes][T][2] page-locked host copy of U that the last merge_update of
+  float* pinned_U_dev;          //   brmppi_solve_get_controls writes (device address of the same memory)
   float* path_len;              // [n_scenes] M dpsi of the reference path (BRMPPI_FLAG_MPCC), host
   unsigned char* pinned_in[2];  // single-scene contexts: page-locked images of the workspace's input span
   cudaEvent_t pinned_in_done[2];//   (state .. obstacles), used in turn by brmppi_set_inputs
@@ -238,8 +240,10 @@ int launch_rollout(brmppi_ctx* c) {
   return BRMPPI_OK;
 }
 
-int launch_update(brmppi_ctx* c) {
-  const DeviceParams& d = c->d;
+// to_host: the update also writes the new nominal into the context's page-locked host copy of U
+int launch_update(brmppi_ctx* c, bool to_host = false) {
+  DeviceParams d = c->d;
+  d.U_host = to_host ? c->pinned_U_dev : nullptr;
   dim3 ugrid((unsigned)((2 * d.T + kUpdateOutputsPerBlock - 1) / kUpdateOutputsPerBlock),
              (unsigned)d.n_scenes);
   merge_update<kMergeLocal><<<ugrid, kUpdateBlock, c->smem_update, c->stream>>>(d, nullptr, 0);
@@ -247,15 +251,16 @@ int launch_update(brmppi_ctx* c) {
   return BRMPPI_OK;
 }
 
-int enqueue_iteration(brmppi_ctx* c) {
+int enqueue_iteration(brmppi_ctx* c, bool to_host = false) {
   int r = launch_rollout(c);
   if (r) return r;
-  return launch_update(c);
+  return launch_update(c, to_host);
 }
 
-int enqueue_solve(brmppi_ctx* c) {
+// to_host: the LAST iteration's update leaves the result in page-locked host memory as well
+int enqueue_solve(brmppi_ctx* c, bool to_host = false) {
   for (int it = 0; it < c->p.n_iter; ++it) {
-    int r = enqueue_iteration(c);
+    int r = enqueue_iteration(c, to_host && it == c->p.n_iter - 1);
     if (r) return r;
   }
   return BRMPPI_OK;
@@ -344,7 +349,10 @@ int brmppi_create(const brmppi_params* p, void* dev_workspace, size_t workspace_
   c->n_host = 0;
   c->solve_graph = nullptr;
   c->step_graph = nullptr;
+  c->solve_host_graph = nullptr;
   c->pinned_u0 = nullptr;
+  c->pinned_U = nullptr;
+  c->pinned_U_dev = nullptr;
   c->path_len = (float*)calloc((size_t)p->n_scenes, sizeof(float));
   c->pinned_in[0] = c->pinned_in[1] = nullptr;
   c->pinned_in_done[0] = c->pinned_in_done[1] = nullptr;
@@ -472,6 +480,9 @@ int brmppi_create(const brmppi_params* p, void* dev_workspace, size_t workspace_
   if (e == cudaSuccess) e = cudaMemsetAsync(base + L.diag, 0, (size_t)p->n_scenes * sizeof(brmppi_diag), c->stream);
   if (e == cudaSuccess) e = cudaHostAlloc((void**)&c->pinned_u0, sizeof(float) * 2 * (size_t)p->n_scenes, cudaHostAllocMapped);
   if (e == cudaSuccess) e = cudaHostGetDevicePointer((void**)&d.u0_host, c->pinned_u0, 0);
+  if (e == cudaSuccess) e = cudaHostAlloc((void**)&c->pinned_U, sizeof(float) * 2 * (size_t)p->T * (size_t)p->n_scenes, cudaHostAllocMapped);
+  if (e == cudaSuccess) e = cudaHostGetDevicePointer((void**)&c->pinned_U_dev, c->pinned_U, 0);
+  d.U_host = nullptr;
   if (p->n_scenes == 1 && !(p->flags & BRMPPI_FLAG_MPCC)) {
     const size_t span = L.obstacles + (size_t)(p->max_obstacles > 0 ? p->max_obstacles : 1) * 20 - L.state;
     for (int i = 0; i < 2 && e == cudaSuccess; ++i) {
@@ -486,6 +497,7 @@ int brmppi_create(const brmppi_params* p, void* dev_workspace, size_t workspace_
       if (c->pinned_in_done[i]) cudaEventDestroy(c->pinned_in_done[i]);
     }
     if (c->pinned_u0) cudaFreeHost(c->pinned_u0);
+    if (c->pinned_U) cudaFreeHost(c->pinned_U);
     delete c;
     return cuda_fail(e);
   }
@@ -497,7 +509,9 @@ int brmppi_destroy(brmppi_ctx* c) {
   if (!c) return BRMPPI_ERR_NULL;
   if (c->solve_graph) cudaGraphExecDestroy(c->solve_graph);
   if (c->step_graph) cudaGraphExecDestroy(c->step_graph);
+  if (c->solve_host_graph) cudaGraphExecDestroy(c->solve_host_graph);
   if (c->pinned_u0) cudaFreeHost(c->pinned_u0);
+    if (c->pinned_U) cudaFreeHost(c->pinned_U);
   for (int i = 0; i < 2; ++i) {
     if (c->pinned_in[i]) cudaFreeHost(c->pinned_in[i]);
     if (c->pinned_in_done[i]) cudaEventDestroy(c->pinned_in_done[i]);
@@ -702,6 +716,29 @@ int brmppi_solve(brmppi_ctx* c) {
   }
   c->launches += 2ull * (unsigned)c->p.n_iter;
   c->n_host += (unsigned)c->p.n_iter;
+  return BRMPPI_OK;
+}
+
+int brmppi_solve_get_controls(brmppi_ctx* c, float* U_out) {
+  if (!c || !U_out) return BRMPPI_ERR_NULL;
+  int r = ready(c);
+  if (r) return r;
+  if (c->stream == nullptr) {           // the legacy default stream cannot be captured
+    r = enqueue_solve(c, true);
+    if (r) return r;
+  } else {
+    if (!c->solve_host_graph) {
+      r = capture(c, &c->solve_host_graph, [&] { return enqueue_solve(c, true); });
+      if (r) return r;
+    }
+    CU(cudaGraphLaunch(c->solve_host_graph, c->stream));
+  }
+  c->launches += 2ull * (unsigned)c->p.n_iter;
+  c->n_host += (unsigned)c->p.n_iter;
+  // the last update wrote U straight into the page-locked host copy (mapped under unified addressing): no copy
+  // node behind the graph, the sync makes it visible
+  CU(cudaStreamSynchronize(c->stream));
+  memcpy(U_out, c->pinned_U, sizeof(float) * 2 * (size_t)c->p.T * (size_t)c->p.n_scenes);
   return BRMPPI_OK;
 }
 

@@ -69,6 +69,7 @@ struct DeviceParams {
   uint32_t* counter;          // global iteration counter n
   float* u0_applied;          // [n_scenes][2]  control applied by the last plant step
   float* u0_host;             // the same, in page-locked HOST memory the device writes directly (brmppi_step's result)
+  float* U_host;              // [n_scenes][T][2]  mirror of U in page-locked host memory, written by every merge_update
   float* state7;              // [n_scenes][8]  (p_x, p_y, v, a, theta1, theta2, delta, psi)  (FLAG_MPCC)
   int* path_M;                // [n_scenes]     cubic segments of the reference path
   float* path_dpsi;           // [n_scenes]     knot spacing

@@ -136,7 +136,15 @@ merge_update(const __grid_constant__ DeviceParams P, float* shard, int n_shards)
       }
       return;
     }
-    if (any_finite && eta > 0.0f) P.U[(size_t)scene * 2 * P.T + o] = acc / eta;
+    {
+      // the new nominal also goes straight to its page-locked host mirror (zero-copy: brmppi_get_controls after a
+      // solve then needs no copy node behind the graph); an update that is skipped mirrors the value that stays
+      float* u = P.U + (size_t)scene * 2 * P.T + o;
+      const bool upd = any_finite && eta > 0.0f;
+      const float u_new = upd ? acc / eta : *u;
+      if (upd) *u = u_new;
+      if (P.U_host != nullptr) P.U_host[(size_t)scene * 2 * P.T + o] = u_new;
+    }
     if (diag_cta) {
       brmppi_diag d;
       d.S_min = any_finite ? (float)m : CUDART_INF_F;

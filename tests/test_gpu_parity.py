@@ -641,3 +641,36 @@ def test_set_inputs_equals_the_three_calls(B):
     fresh.set_inputs(sc.x0, sc.goal, sc.obstacles)      # marks state and goal as set
     fresh.solve()
     fresh.close()
+
+
+def test_solve_get_controls_equals_solve_then_get_controls(B):
+    """brmppi_solve_get_controls (the last update writes U into page-locked host memory too, no copy behind the
+    solve) returns the bits that brmppi_solve + brmppi_get_controls return and leaves the same U on the device: one
+    scene and three, repeated and mixed with plain solves, shifts and a step, and when an iteration leaves U as it
+    was (every cost non-finite)."""
+    sc = scenes.scene_cfg2(2)
+    p = sc.params.with_(K=1200, T=37, n_iter=2)
+    for n_scenes in (1, 3):
+        a = B.Solver(p, n_scenes, 8, 0)
+        b = B.Solver(p, n_scenes, 8, 0)
+        for s in (a, b):
+            for i in range(n_scenes):
+                s.set_state(sc.x0 + np.float32(0.05 * i), i); s.set_goal(sc.goal, i); s.set_obstacles(sc.obstacles, i)
+        for rep_ in range(4):
+            a.solve()
+            Ua = np.stack([a.get_controls(i) for i in range(n_scenes)])
+            Ub = b.solve_get_controls()
+            assert Ub.shape == (n_scenes, p.T, 2) and np.array_equal(Ua, Ub) and np.abs(Ub).max() > 0
+            assert all(np.array_equal(b.get_controls(i), Ub[i]) for i in range(n_scenes))     # the device copy
+            if rep_ == 1:
+                a.shift(); b.shift()
+            if rep_ == 2:
+                assert np.array_equal(a.step(), b.step())
+        a.close(); b.close()
+    bad = sc.params.with_(K=256, T=20, n_iter=1, w_pos=3e38)      # every stage cost overflows fp32
+    s = B.Solver(bad, 1, 8, 0)
+    s.set_scene(sc)
+    U0 = np.tile(np.array([[0.5, 0.1]], dtype=np.float32), (20, 1))
+    s.set_nominal(U0)
+    assert np.array_equal(s.solve_get_controls()[0], U0) and s.get_diag()["argmin"] == -1
+    s.close()
