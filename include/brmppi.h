@@ -217,6 +217,15 @@ int brmppi_solve(brmppi_ctx* ctx);
  * way brmppi_step returns u0), the call waits for the stream and hands it over.  U_out: HOST, [n_scenes][T][2]
  * floats, owned by the caller.  Synchronous.  Everything else as brmppi_solve (same kernels, same results). */
 int brmppi_solve_get_controls(brmppi_ctx* ctx, float* U_out);
+/* One receding-horizon solve from host buffers to host buffers: brmppi_set_inputs(ctx, 0, x, g, n, obstacles)
+ * followed by brmppi_solve_get_controls(ctx, U_out) -- same checks and error codes (nothing is changed or launched
+ * if a check fails), same results.  In a single-scene context with a stream it is ONE graph launch: the copy of the
+ * inputs from the context's page-locked staging buffer, the n_iter iterations, the last update writing U_out's
+ * contents into page-locked host memory; otherwise it is the two calls.  HOST pointers; U_out [T][2] (scene 0; with
+ * several scenes [n_scenes][T][2], the other scenes solved on the inputs they have).  Synchronous.  Not with
+ * BRMPPI_FLAG_MPCC. */
+int brmppi_solve_host(brmppi_ctx* ctx, const float x[4], const float g[4], int n, const brmppi_obstacle* obstacles,
+                      float* U_out);
 /* K-sharded solve.  The online-softmax state (m, eta, A[2T]) of
  * eq. (5) is associative, so G contexts (on G GPUs, or on one) can each own K/G of the samples of ONE solve:
  * same seed, state, goal, obstacles and nominal in every context, k_offset = first global sample index.

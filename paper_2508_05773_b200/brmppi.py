@@ -27,7 +27,7 @@ HITCH_STATIC_MAX_N = 16384
 EXPORTS = [
     "brmppi_workspace_bytes", "brmppi_create", "brmppi_destroy", "brmppi_set_state",
     "brmppi_set_goal", "brmppi_set_obstacles", "brmppi_set_superellipses", "brmppi_get_superellipses", "brmppi_set_nominal", "brmppi_set_counter",
-    "brmppi_reset", "brmppi_solve", "brmppi_solve_get_controls", "brmppi_shift", "brmppi_step", "brmppi_get_controls",
+    "brmppi_reset", "brmppi_solve", "brmppi_solve_get_controls", "brmppi_solve_host", "brmppi_shift", "brmppi_step", "brmppi_get_controls",
     "brmppi_get_state", "brmppi_get_obstacles", "brmppi_get_costs", "brmppi_get_final_states",
     "brmppi_get_diag", "brmppi_get_phase_times", "brmppi_time_kernels", "brmppi_launch_count", "brmppi_strerror", "brmppi_debug_philox",
     "brmppi_debug_sample_controls", "brmppi_measure_peaks", "brmppi_get_hitch_filter", "brmppi_hitch_filter", "brmppi_project",
@@ -118,6 +118,7 @@ def lib():
         L.brmppi_reset.argtypes = [vp]
         L.brmppi_solve.argtypes = [vp]
         L.brmppi_solve_get_controls.argtypes = [vp, vp]
+        L.brmppi_solve_host.argtypes = [vp, vp, vp, C.c_int, vp, vp]
         L.brmppi_shift.argtypes = [vp]
         L.brmppi_shard_words.argtypes = [vp]
         L.brmppi_shard_words.restype = C.c_size_t
@@ -320,6 +321,17 @@ class Solver:
             out = np.empty((self.n_scenes, self.T, 2), dtype=np.float32)
         assert out.dtype == np.float32 and out.flags.c_contiguous and out.size == self.n_scenes * self.T * 2
         _check(lib().brmppi_solve_get_controls(self._ctx, C.c_void_p(out.ctypes.data)))
+        return out
+
+    def solve_host(self, x, g, obstacles, out=None):
+        """set_inputs(x, g, obstacles) + solve_get_controls() as one call (one graph launch in a single-scene context)."""
+        x, g, obs = _f32(x, (4,)), _f32(g, (4,)), _f32(obstacles).reshape(-1, 5)
+        n = obs.shape[0]
+        if out is None:
+            out = np.empty((self.n_scenes, self.T, 2), dtype=np.float32)
+        assert out.dtype == np.float32 and out.flags.c_contiguous and out.size == self.n_scenes * self.T * 2
+        adr = lambda a: a.__array_interface__["data"][0]
+        _check(lib().brmppi_solve_host(self._ctx, adr(x), adr(g), n, adr(obs) if n else None, adr(out)))
         return out
 
     def shift(self):

@@ -197,7 +197,7 @@ struct brmppi_ctx {
   unsigned char* goal_set;
   unsigned long long launches;
   unsigned int n_host;          // host mirror of the device iteration counter
-  cudaGraphExec_t solve_graph, step_graph, solve_host_graph;
+  cudaGraphExec_t solve_graph, step_graph, solve_host_graph, solve_io_graph;
   float* pinned_u0;             // [n_scenes][2] staging for brmppi_step
   float* pinned_U;              // [n_scenes][T][2] page-locked host copy of U that the last merge_update of
   float* pinned_U_dev;          //   brmppi_solve_get_controls writes (device address of the same memory)
@@ -350,6 +350,7 @@ int brmppi_create(const brmppi_params* p, void* dev_workspace, size_t workspace_
   c->solve_graph = nullptr;
   c->step_graph = nullptr;
   c->solve_host_graph = nullptr;
+  c->solve_io_graph = nullptr;
   c->pinned_u0 = nullptr;
   c->pinned_U = nullptr;
   c->pinned_U_dev = nullptr;
@@ -510,6 +511,7 @@ int brmppi_destroy(brmppi_ctx* c) {
   if (c->solve_graph) cudaGraphExecDestroy(c->solve_graph);
   if (c->step_graph) cudaGraphExecDestroy(c->step_graph);
   if (c->solve_host_graph) cudaGraphExecDestroy(c->solve_host_graph);
+  if (c->solve_io_graph) cudaGraphExecDestroy(c->solve_io_graph);
   if (c->pinned_u0) cudaFreeHost(c->pinned_u0);
     if (c->pinned_U) cudaFreeHost(c->pinned_U);
   for (int i = 0; i < 2; ++i) {
@@ -609,11 +611,10 @@ int brmppi_set_obstacles(brmppi_ctx* c, int scene, int n, const brmppi_obstacle*
   return BRMPPI_OK;
 }
 
-int brmppi_set_inputs(brmppi_ctx* c, int scene, const float x[4], const float g[4], int n,
-                      const brmppi_obstacle* obs) {
+// every check of brmppi_set_state + brmppi_set_goal + brmppi_set_obstacles, nothing changed
+static int check_inputs(brmppi_ctx* c, int scene, const float x[4], const float g[4], int n, const brmppi_obstacle* obs) {
   int r = check_scene(c, scene);
   if (r) return r;
-  // every check of the three calls first, so that a failure changes nothing
   if (!x || !g) return BRMPPI_ERR_NULL;
   if (c->p.flags & BRMPPI_FLAG_MPCC) return BRMPPI_ERR_INVALID_ARG;
   if (!finite_all(x, 4) || !finite_all(g, 4)) return BRMPPI_ERR_NONFINITE_INPUT;
@@ -624,24 +625,38 @@ int brmppi_set_inputs(brmppi_ctx* c, int scene, const float x[4], const float g[
     if (!finite_all(&obs[i].cx, 5)) return BRMPPI_ERR_NONFINITE_INPUT;
     if (!(obs[i].radius > 0.f)) return BRMPPI_ERR_INVALID_ARG;
   }
+  return BRMPPI_OK;
+}
+
+// the image of the workspace's input span (state | goal | n_obs | obstacles, each where the layout puts it); obstacle
+// slots beyond n keep what the image held: never read
+static void fill_input_image(const brmppi_ctx* c, unsigned char* img, const float x[4], const float g[4], int n,
+                             const brmppi_obstacle* obs) {
+  const Layout& L = c->layout;
+  const float v[4] = {x[0], x[1], wrap_pi(x[2]), wrap_pi(x[3])};
+  memcpy(img + (L.state - L.state), v, 16);
+  memcpy(img + (L.goal - L.state), g, 16);
+  memcpy(img + (L.n_obs - L.state), &n, sizeof(int));
+  if (n > 0) memcpy(img + (L.obstacles - L.state), obs, sizeof(brmppi_obstacle) * (size_t)n);
+}
+
+int brmppi_set_inputs(brmppi_ctx* c, int scene, const float x[4], const float g[4], int n,
+                      const brmppi_obstacle* obs) {
+  int r = check_inputs(c, scene, x, g, n, obs);       // first, so that a failure changes nothing
+  if (r) return r;
   if (!c->pinned_in[0]) {                    // several scenes: the three copies
     r = brmppi_set_state(c, scene, x);
     if (!r) r = brmppi_set_goal(c, scene, g);
     if (!r) r = brmppi_set_obstacles(c, scene, n, obs);
     return r;
   }
-  // one scene: an image of the workspace's input span (state | goal | n_obs | obstacles, each where the layout
-  // puts it) in page-locked memory, one copy.  Obstacle slots beyond n keep what the image held: never read.
+  // one scene: the image of the input span in page-locked memory, one copy
   const Layout& L = c->layout;
   const int b = c->pinned_in_next;
   c->pinned_in_next ^= 1;
   CU(cudaEventSynchronize(c->pinned_in_done[b]));       // the copy that last used this buffer has been made
   unsigned char* img = c->pinned_in[b];
-  const float v[4] = {x[0], x[1], wrap_pi(x[2]), wrap_pi(x[3])};
-  memcpy(img + (L.state - L.state), v, 16);
-  memcpy(img + (L.goal - L.state), g, 16);
-  memcpy(img + (L.n_obs - L.state), &n, sizeof(int));
-  if (n > 0) memcpy(img + (L.obstacles - L.state), obs, sizeof(brmppi_obstacle) * (size_t)n);
+  fill_input_image(c, img, x, g, n, obs);
   const size_t span = L.obstacles + sizeof(brmppi_obstacle) * (size_t)n - L.state;
   CU(cudaMemcpyAsync((unsigned char*)c->d.state, img, span, cudaMemcpyHostToDevice, c->stream));
   CU(cudaEventRecord(c->pinned_in_done[b], c->stream));
@@ -739,6 +754,38 @@ int brmppi_solve_get_controls(brmppi_ctx* c, float* U_out) {
   // node behind the graph, the sync makes it visible
   CU(cudaStreamSynchronize(c->stream));
   memcpy(U_out, c->pinned_U, sizeof(float) * 2 * (size_t)c->p.T * (size_t)c->p.n_scenes);
+  return BRMPPI_OK;
+}
+
+int brmppi_solve_host(brmppi_ctx* c, const float x[4], const float g[4], int n, const brmppi_obstacle* obs,
+                      float* U_out) {
+  if (!c || !U_out) return BRMPPI_ERR_NULL;
+  int r = check_inputs(c, 0, x, g, n, obs);
+  if (r) return r;
+  if (!c->pinned_in[0] || c->stream == nullptr) {       // several scenes, or no stream to capture on: the two calls
+    r = brmppi_set_inputs(c, 0, x, g, n, obs);
+    return r ? r : brmppi_solve_get_controls(c, U_out);
+  }
+  // ONE graph launch: copy of the input image (page-locked, fixed address: staging buffer 0) into the workspace,
+  // the solve, the last update writing U into page-locked host memory
+  CU(cudaEventSynchronize(c->pinned_in_done[0]));        // a brmppi_set_inputs copy out of this buffer has been made
+  fill_input_image(c, c->pinned_in[0], x, g, n, obs);
+  c->state_set[0] = 1;
+  c->goal_set[0] = 1;
+  if (!c->solve_io_graph) {
+    const Layout& L = c->layout;
+    const size_t span = L.obstacles + sizeof(brmppi_obstacle) * (size_t)(c->p.max_obstacles > 0 ? c->p.max_obstacles : 1) - L.state;
+    r = capture(c, &c->solve_io_graph, [&] {
+      CU(cudaMemcpyAsync((unsigned char*)c->d.state, c->pinned_in[0], span, cudaMemcpyHostToDevice, c->stream));
+      return enqueue_solve(c, true);
+    });
+    if (r) return r;
+  }
+  CU(cudaGraphLaunch(c->solve_io_graph, c->stream));
+  c->launches += 2ull * (unsigned)c->p.n_iter;
+  c->n_host += (unsigned)c->p.n_iter;
+  CU(cudaStreamSynchronize(c->stream));
+  memcpy(U_out, c->pinned_U, sizeof(float) * 2 * (size_t)c->p.T);
   return BRMPPI_OK;
 }
 

@@ -674,3 +674,44 @@ def test_solve_get_controls_equals_solve_then_get_controls(B):
     s.set_nominal(U0)
     assert np.array_equal(s.solve_get_controls()[0], U0) and s.get_diag()["argmin"] == -1
     s.close()
+
+
+def test_solve_host_equals_set_inputs_solve_get_controls(B):
+    """brmppi_solve_host (inputs, solve and result in one call; one graph launch in a single-scene context) returns
+    the bits of brmppi_set_inputs + brmppi_solve + brmppi_get_controls and leaves the same state, obstacles and U on
+    the device: changing inputs and obstacle counts over repeated calls, mixed with set_inputs (the staging buffer it
+    shares), in a two-scene context (the two calls underneath), and the same argument errors with nothing changed."""
+    sc = scenes.scene_cfg2(3)
+    p = sc.params.with_(K=1500, T=40, n_iter=2)
+    for n_scenes in (1, 2):
+        a = B.Solver(p, n_scenes, 8, B.FLAG_WRITE_SAMPLES)
+        b = B.Solver(p, n_scenes, 8, B.FLAG_WRITE_SAMPLES)
+        for s in (a, b):
+            for i in range(n_scenes):
+                s.set_inputs(sc.x0, sc.goal, sc.obstacles, i)
+        for rep_, n_obs in enumerate((8, 8, 3, 0, 5, 8)):
+            x = sc.x0 + np.float32(0.1 * rep_)
+            g = sc.goal + np.float32(0.01 * rep_)
+            a.set_inputs(x, g, sc.obstacles[:n_obs]); a.solve()
+            Ua = np.stack([a.get_controls(i) for i in range(n_scenes)])
+            Ub = b.solve_host(x, g, sc.obstacles[:n_obs])
+            assert np.array_equal(Ua, Ub) and np.abs(Ub).max() > 0
+            for i in range(n_scenes):
+                assert np.array_equal(a.get_costs(i), b.get_costs(i)) and np.array_equal(a.get_controls(i), b.get_controls(i))
+                assert np.array_equal(a.get_state(i), b.get_state(i)) and np.array_equal(a.get_obstacles(i), b.get_obstacles(i))
+            if rep_ == 2:                                   # a plain set_inputs + solve in between
+                a.set_inputs(sc.x0, sc.goal, sc.obstacles); b.set_inputs(sc.x0, sc.goal, sc.obstacles)
+                a.solve(); b.solve()
+        before, U_before = b.get_state(0).copy(), b.get_controls(0).copy()
+        bad = sc.obstacles.copy(); bad[2, 2] = -1.0
+        for args, status in (((sc.x0, sc.goal, bad), B.ERR_INVALID_ARG),
+                             ((np.array([0, np.nan, 0, 0]), sc.goal, sc.obstacles), B.ERR_NONFINITE_INPUT),
+                             ((sc.x0, sc.goal, np.zeros((9, 5)) + 1.0), B.ERR_TOO_MANY_OBSTACLES)):
+            with pytest.raises(B.BrmppiError) as e:
+                b.solve_host(*args)
+            assert e.value.status == status
+        assert np.array_equal(b.get_state(0), before) and np.array_equal(b.get_controls(0), U_before)
+        a.close(); b.close()
+    fresh = B.Solver(p, 1, 8, 0)
+    assert np.abs(fresh.solve_host(sc.x0, sc.goal, sc.obstacles)).max() > 0      # marks state and goal as set
+    fresh.close()
