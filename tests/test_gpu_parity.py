@@ -715,3 +715,57 @@ def test_solve_host_equals_set_inputs_solve_get_controls(B):
     fresh = B.Solver(p, 1, 8, 0)
     assert np.abs(fresh.solve_host(sc.x0, sc.goal, sc.obstacles)).max() > 0      # marks state and goal as set
     fresh.close()
+
+
+def test_random_configurations(B, O):
+    """A seeded sweep over sizes the named cases do not visit: K from 1 to 20 000 (tiles of every width, ragged last
+    tiles), T from 1 to 150 (one chunk to many, odd and even), 0 to 64 obstacles with and without motion (one to eight
+    groups, table padding), one to three scenes, one to four discs, hitch offset, warm and zero nominal, a random
+    iteration counter.  Per configuration: the culled launch equals the un-culled one bit for bit, and both kernels
+    meet the flat tolerances on x_T and S_k against the oracle.  alpha_lo >= 0.05 and lambda >= 10 as in every recipe
+    (DESIGN.md 2 says what happens below that)."""
+    rng = np.random.default_rng(20250811)
+    disc_sets = [((0, 2.0),), ((0, 2.0), (1, -3.0)), ((0, 2.0), (1, -2.0), (1, -6.0)), ((0, 0.0), (0, 2.5), (1, -2.0), (1, -4.5))]
+    n_done = 0
+    while n_done < 200:
+        K = int(rng.choice([1, 7, 31, 33, 100, 333, 1000, 2049, 4097, 9000, 20000]))
+        T = int(rng.choice([1, 2, 3, 5, 6, 7, 11, 12, 13, 24, 25, 40, 81, 150]))
+        n_obs = int(rng.choice([0, 1, 2, 3, 5, 8, 9, 16, 17, 31, 32, 33, 64]))
+        if K * T * max(n_obs, 1) > 2_000_000:
+            continue
+        ns = int(rng.choice([1, 1, 2, 3]))
+        scs = []
+        for _ in range(ns):
+            sc = scenes.scene_static(int(rng.integers(0, 1000)), n_obs, K=K, T=T)
+            if n_obs and rng.random() < 0.6:
+                ob = sc.obstacles.copy()
+                m = rng.random(n_obs) < 0.5
+                ob[m, 3:] = rng.uniform(-2, 2, (int(m.sum()), 2))
+                sc.obstacles = ob.astype(np.float32).astype(np.float64)
+            scs.append(sc)
+        p = scs[0].params.with_(discs=disc_sets[int(rng.integers(0, 4))], Lh=float(rng.choice([0.0, 0.6])),
+                                alpha_lo=float(rng.choice([0.05, 0.1, 0.3])), lam=float(rng.choice([10.0, 100.0])),
+                                seed=int(rng.integers(0, 2**40)))
+        cap = max(n_obs, 1) if rng.random() < 0.5 else 64
+        n0 = int(rng.integers(0, 100))
+        U0 = None if rng.random() < 0.5 else np.tile(np.array([[0.5, 0.05]], dtype=np.float32), (T, 1))
+        outs = {}
+        for name, fl in (("cta", 0), ("nocull", B.FLAG_NO_CULL), ("thread", B.FLAG_KERNEL_THREAD_PER_SAMPLE)):
+            s = B.Solver(p, ns, cap, fl | B.FLAG_WRITE_SAMPLES)
+            for i, sc in enumerate(scs):
+                s.set_scene(sc, i)
+                s.set_nominal(U0, i)
+            s.set_counter(n0)
+            s.solve()
+            outs[name] = [(s.get_costs(i), s.get_final_states(i), s.get_controls(i)) for i in range(ns)]
+            s.close()
+        what = f"K={K} T={T} n_obs={n_obs} scenes={ns} discs={len(p.discs)} cap={cap}"
+        for i in range(ns):
+            a, b, c = outs["cta"][i], outs["nocull"][i], outs["thread"][i]
+            assert all(np.array_equal(x, y) for x, y in zip(a, b)), "culled != un-culled: " + what
+            U = np.zeros((T, 2)) if U0 is None else U0.astype(np.float64)
+            ref = O.solve(p.with_(seed=p.seed + i), n0, scs[i].x0, scs[i].goal, scs[i].obstacles, U, n_threads=8)[-1]
+            for name, g in (("tile", a), ("thread", c)):
+                assert close(g[0], ref["S"], 1.0).all(), f"{name} S_k: " + what
+                assert close(g[1], ref["XT"], 1.0).all(), f"{name} x_T: " + what
+        n_done += 1
