@@ -368,3 +368,30 @@ def test_full_size_against_the_oracle(B, O, kern):
     got = dict(U=s.get_controls(), S=s.get_costs(), XT=s.get_final_states7(), diag=s.get_diag())
     s.close()
     check(O, got, sc, p)
+
+
+def test_random_configurations(B, O):
+    """A seeded sweep over sizes the named cases do not visit (K 1 to 1000: tiles of every width; T 1 to 81: one chunk
+    to several, with and without control planes; 0 to 8 obstacles, some moving; one to four discs; hitch offset; two
+    ranges of alpha; a random iteration counter).  Per configuration: culled == un-culled bit for bit on the CTA
+    kernel, and both kernels against the oracle by the module's rule."""
+    rng = np.random.default_rng(20250812)
+    disc_sets = [((0, 2.0),), ((0, 2.0), (1, -3.0)), ((0, 2.0), (1, -2.0), (1, -6.0)), ((0, 0.0), (0, 2.5), (1, -2.0), (1, -4.5))]
+    for _ in range(150):
+        K = int(rng.choice([1, 7, 31, 33, 100, 333, 1000]))
+        T = int(rng.choice([1, 2, 3, 5, 6, 7, 11, 12, 13, 24, 25, 40, 81]))
+        n_obs = int(rng.integers(0, 9))
+        sc = path_scene(int(rng.integers(0, 50)), n_obs, K=K, T=T, discs=disc_sets[int(rng.integers(0, 4))],
+                        Lh=float(rng.choice([0.0, 0.5])), alpha_lo=float(rng.choice([0.1, 0.3])))
+        sc.params = sc.params.with_(seed=int(rng.integers(0, 2**40)))
+        if n_obs and rng.random() < 0.5:
+            m = rng.random(n_obs) < 0.5
+            sc.obstacles[m, 3:] = rng.uniform(-1.5, 1.5, (int(m.sum()), 2)).astype(np.float32)
+        n0 = int(rng.integers(0, 100))
+        what = f"K={K} T={T} n_obs={n_obs} discs={len(sc.params.discs)}"
+        a = gpu_mpcc(B, sc, sc.params, 0, n0=n0, max_obstacles=8)
+        b = gpu_mpcc(B, sc, sc.params, B.FLAG_NO_CULL, n0=n0, max_obstacles=8)
+        c = gpu_mpcc(B, sc, sc.params, B.FLAG_KERNEL_THREAD_PER_SAMPLE, n0=n0, max_obstacles=8)
+        assert all(np.array_equal(a[q], b[q]) for q in ("U", "S", "XT")), "culled != un-culled: " + what
+        for got in (a, c):
+            check(O, got, sc, sc.params, n0=n0)
