@@ -208,3 +208,35 @@ def test_closed_loop_and_errors(B, O):
     with pytest.raises(B.BrmppiError):
         B.Solver(sc.params.with_(proj_rho=-1.0), 1, 8, B.FLAG_PROJECTED)
     B.Solver(sc.params.with_(proj_qalpha=0.0), 1, 8, 0).close()          # not read without the flag
+
+
+def test_random_configurations(B, O):
+    """A seeded sweep over sizes the named cases do not visit (K 1 to 1000, T 1 to 60, 0 to 8 obstacles -- every
+    obstacle-capacity instantiation, with unused capacity --, some moving, one to four discs, hitch offset, two
+    projection weights rho, warm and zero nominal, a random iteration counter), each against the oracle by the
+    module's rule."""
+    rng = np.random.default_rng(20250813)
+    disc_sets = [((0, 2.0),), ((0, 2.0), (1, -3.0)), ((0, 2.0), (1, -2.0), (1, -6.0)), ((0, 0.0), (0, 2.5), (1, -2.0), (1, -4.5))]
+    n_off = 0
+    for _ in range(200):
+        K = int(rng.choice([1, 7, 31, 33, 100, 129, 333, 1000]))
+        T = int(rng.choice([1, 2, 3, 5, 6, 7, 11, 12, 13, 24, 25, 40, 60]))
+        n_obs = int(rng.integers(0, 9))
+        sc = near_scene(int(rng.integers(0, 40)), n_obs, K=K, T=T, discs=disc_sets[int(rng.integers(0, 4))],
+                        Lh=float(rng.choice([0.0, 0.75])), proj_rho=float(rng.choice([0.1, 1.0])))
+        sc.params = sc.params.with_(seed=int(rng.integers(0, 2**40)))
+        if n_obs and rng.random() < 0.5:
+            m = rng.random(n_obs) < 0.5
+            sc.obstacles[m, 3:] = rng.uniform(-1.5, 1.5, (int(m.sum()), 2)).astype(np.float32)
+        n0 = int(rng.integers(0, 100))
+        U0 = None if rng.random() < 0.5 else np.tile(np.array([[0.8, 0.1]], dtype=np.float32), (T, 1))
+        cap = max(n_obs, 1) if rng.random() < 0.5 else 8
+        s = B.Solver(sc.params, 1, cap, B.FLAG_PROJECTED | B.FLAG_WRITE_SAMPLES)
+        s.set_scene(sc)
+        s.set_nominal(U0)
+        s.set_counter(n0)
+        s.solve()
+        got = dict(U=s.get_controls(), S=s.get_costs(), XT=s.get_final_states(), diag=s.get_diag())
+        s.close()
+        n_off += check(O, got, sc, sc.params, n0=n0, U0=U0)
+    assert n_off <= 200         # pinned-and-off samples stay the exception over the whole sweep
