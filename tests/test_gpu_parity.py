@@ -769,3 +769,35 @@ def test_random_configurations(B, O):
                 assert close(g[0], ref["S"], 1.0).all(), f"{name} S_k: " + what
                 assert close(g[1], ref["XT"], 1.0).all(), f"{name} x_T: " + what
         n_done += 1
+
+
+def test_random_configurations_with_superellipses(B, O):
+    """The seeded sweep with eq. (16)'s obstacles: 1 to 16 super-ellipses (e = 2 and 4, oriented, some moving) beside
+    0 to 16 discs, K 1 to 9000, T 1 to 81, one to four vehicle discs, with and without unused capacity; S_k and x_T
+    at the flat tolerances against the oracle."""
+    rng = np.random.default_rng(20250814)
+    disc_sets = [((0, 2.0),), ((0, 2.0), (1, -3.0)), ((0, 2.0), (1, -2.0), (1, -6.0)), ((0, 0.0), (0, 2.5), (1, -2.0), (1, -4.5))]
+    n_done = 0
+    while n_done < 80:
+        K = int(rng.choice([1, 7, 31, 33, 100, 333, 1000, 2049, 9000]))
+        T = int(rng.choice([1, 2, 3, 5, 6, 7, 11, 12, 13, 24, 25, 40, 81]))
+        n_obs = int(rng.choice([0, 0, 1, 3, 8, 9, 16]))
+        n_se = int(rng.choice([1, 2, 3, 4, 5, 8, 9, 16]))
+        if K * T * (n_obs + 3 * n_se) > 4_000_000:
+            continue
+        sc = scenes.scene_static(int(rng.integers(0, 1000)), n_obs, K=K, T=T)
+        se = np.array([[sc.x0[0] + rng.uniform(-15, 15), sc.x0[1] + rng.uniform(-15, 15), rng.uniform(0.5, 2.5),
+                        rng.uniform(0.4, 1.2), rng.uniform(-3, 3), rng.uniform(-1, 1) * (i % 2), rng.uniform(-1, 1) * (i % 2),
+                        4.0 if i % 3 else 2.0] for i in range(n_se)], dtype=np.float32).astype(np.float64)
+        p = sc.params.with_(discs=disc_sets[int(rng.integers(0, 4))], Lh=float(rng.choice([0.0, 0.6])),
+                            alpha_lo=float(rng.choice([0.05, 0.1, 0.3])), lam=float(rng.choice([10.0, 100.0])),
+                            seed=int(rng.integers(0, 2**40)))
+        n0 = int(rng.integers(0, 100))
+        U0 = None if rng.random() < 0.5 else np.tile(np.array([[0.5, 0.05]], dtype=np.float32), (T, 1))
+        got = gpu_solve_se(B, sc, p, se, n0=n0, U0=U0, max_se=n_se if rng.random() < 0.5 else 16)
+        U = np.zeros((T, 2)) if U0 is None else U0.astype(np.float64)
+        ref = O.solve(p, n0, sc.x0, sc.goal, sc.obstacles, U, n_threads=8, superellipses=se)[-1]
+        what = f"K={K} T={T} n_obs={n_obs} n_se={n_se} discs={len(p.discs)}"
+        assert close(got["S"], ref["S"], 1.0).all(), "S_k: " + what
+        assert close(got["XT"], ref["XT"], 1.0).all(), "x_T: " + what
+        n_done += 1
