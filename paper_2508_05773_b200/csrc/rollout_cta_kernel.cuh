@@ -161,7 +161,9 @@ __device__ __forceinline__ GroupCost hinge_chunk(const DeviceParams& P, const fl
           const f32x2 zn = fma2(gprev[p][j], noma, gn);             // g_{t+1} - (1-alpha) g_t = -z
           float za, zb;
           unpack2(zn, za, zb);
-          pen = fma2(nw[p], pack2(fminf(za, 0.0f), fminf(zb, 0.0f)), pen);   // + max(0, z) / rho^2
+          // + max(0, z) / rho^2: min(0, zn) as (zn - |zn|) / 2 -- exact (0 or 2 zn), one full-rate FADD with the
+          // |.| source modifier instead of a half-rate FMNMX; the table's weight carries the 1/2
+          pen = fma2(nw[p], pack2(za - fabsf(za), zb - fabsf(zb)), pen);
           gprev[p][j] = gn;
         }
       }
@@ -520,7 +522,7 @@ rollout_cta(const __grid_constant__ DeviceParams P) {
           float* ob = reinterpret_cast<float*>(sObs) + (dst >> 1) * 8 + (dst & 1);
           ob[0] = -(ob_in[h][0] - x0_in.x);
           ob[2] = -(ob_in[h][1] - x0_in.y);
-          ob[4] = -2.0f * (0.5f / (rho * rho));
+          ob[4] = -(0.5f / (rho * rho));                 // -1 / (2 rho^2): the hinge is formed as zn - |zn| = 2 min(0, zn)
           ob[6] = -(rho * rho);
           float* vl = reinterpret_cast<float*>(sVel) + (dst >> 1) * 4 + (dst & 1);
           vl[0] = -(P.dt * ob_in[h][3]);
