@@ -62,9 +62,9 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
 //     max(0, (1-alpha) h_t - h_{t+1}) = -(1 / rho^2) min(0, zn),   zn = g_{t+1} - (1-alpha) g_t.
 // Obstacles are taken two at a time on packed f32x2 operands (add/fma.rn.f32x2: each half rounds
 // like the scalar instruction): per (obstacle pair, disc) 2 packed subtractions, 2 packed FMAs for
-// g, 1 for zn, 2 scalar FMNMX, 1 packed accumulate.
+// g, 1 for zn, 2 scalar FADDs zn - |zn| (= 2 min(0, zn) exactly; the weight carries the 1/2), 1 packed accumulate.
 // The table (written by warp 0) interleaves obstacles 2p and 2p+1 field by field, already
-// negated -- (-ox, -ox'), (-oy, -oy'), (-1/rho^2, ..), (-rho^2, ..) -- so every packed operand is
+// negated -- (-ox, -ox'), (-oy, -oy'), (-1/(2 rho^2), ..), (-rho^2, ..) -- so every packed operand is
 // one 64-bit shared-memory load; built from scalars, ptxas re-packs them with two MOVs per use.
 // A null (padding) obstacle is all zeros: its weight is 0, so it adds exactly 0.  MOVING: some
 // obstacle of the group moves, o(t) = o(0) + t dt vel (a static one has vel == 0, so the update is
@@ -90,7 +90,7 @@ __device__ __forceinline__ GroupCost hinge_chunk(const DeviceParams& P, const fl
                                                  const float4 g) {
   double bar = 0.0, track = 0.0;
   constexpr int NA = NACT > 0 ? NACT : 1;
-  // obstacles in pairs (2p, 2p+1): negated centres, -rho^2, -1/rho^2 and g of the previous state
+  // obstacles in pairs (2p, 2p+1): negated centres, -rho^2, -1/(2 rho^2) and g of the previous state
   f32x2 nox[NA], noy[NA], mrho2[NA], nw[NA], gprev[NA][ND];
   const f32x2 noma = pack2(-one_minus_alpha, -one_minus_alpha);
   float s1, c1;
@@ -450,7 +450,7 @@ rollout_cta(const __grid_constant__ DeviceParams P) {
       // to its culling threshold at the start state (the obstacles a chunk has to evaluate are then
       // mostly the first pairs of the table), null padding behind.
       // Obstacles 2p and 2p+1 are interleaved field by field -- (-ox, -ox'), (-oy, -oy'),
-      // (-1/rho^2, ..), (-rho^2, ..); velocities (-dt vx, ..), (-dt vy, ..) -- so that phase C
+      // (-1/(2 rho^2), ..), (-rho^2, ..); velocities (-dt vx, ..), (-dt vy, ..) -- so that phase C
       // loads each pair of fields as one packed f32x2 operand.
       // Lane l holds obstacles l and l + 32 in registers and ranks them by counting over shuffles.
       //
